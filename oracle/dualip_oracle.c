@@ -1,0 +1,240 @@
+/*
+ * oracle/dualip_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, single-threaded fp64 CPU restatement of the dual-gradient /
+ * AGD hot path of "Large-Scale Regularized Matching on GPU Clusters"
+ * (arxiv/paper_2606_07777; cited below as P:<line of /root/reference/PAPER.md>).
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * `--impl reference` legs may call this file.  It shares no code, header,
+ * table or constant with paper_2606_07777_b200/ (the CUDA path) and neither
+ * imports the other.
+ *
+ * What is written here, and where the paper says it:
+ *   - ridge-regularised LP         min_{x in C} c'x + (gamma/2)|x|^2 s.t. Ax<=b   P:55-60  (Eq. 1)
+ *   - dual function                g(l) = min_{x in C} c'x+(gamma/2)|x|^2+l'(Ax-b) P:64-67  (Eq. 2)
+ *   - closed-form primal           x*(l) = Proj_C(-(A'l + c)/gamma)                P:69-71  (Eq. 3)
+ *   - dual gradient (Danskin)      grad g(l) = A x*(l) - b                         P:73-75  (Eq. 4)
+ *   - matching structure: per-source blocks, diagonal D_ki, m families             P:81-97  (Def. 1, Eq. 5-6)
+ *   - per-source simple constraint: unit simplex sum<=1,x>=0, "or a box variant"   P:83, P:130 (Table 1)
+ *   - simplex projection by Duchi et al.: sort, prefix sums, rho, theta, clamp
+ *   - AGD on lambda>=0, fixed step from A and gamma, gamma continuation, warm start P:60
+ *
+ * Pins (tests/test_oracle_*.py, all `-m "not gpu"`):
+ *   projections: hand-worked closed forms (tests/golden/projection_cases.txt), a second independent
+ *     method (bisection on theta), brute force over supports / (lower,free,upper) partitions;
+ *   g, grad g: worked example (tests/golden/worked_example_grad.txt), central finite differences,
+ *     concavity, weak duality, row-scaling invariance, additivity over users;
+ *   optimum: brute-force KKT active-set enumeration on <=3 users x 2 items;
+ *   AGD loop: **parity unpinned against the paper** (the update rule is never printed, P:123 gives
+ *     words only; reading R1/R2).  Pinned internally: I=J=1 closed-form optimum, the
+ *     lambda==0 fixed point, monotone ascent of the beta==0 variant, O(1/T^2) bound on KKT instances.
+ *
+ * Layout at this interface (same as the product's C ABI, stated independently):
+ *   row_ptr[I+1] int64, item_idx[nnz] int32, c[nnz] fp32, a[nnz*m] fp32 (a[p*m+k]),
+ *   b[J*m] fp32 (b[j*m+k]), lambda/grad[J*m] fp64 ([j*m+k]).  fp32 inputs are cast exactly to
+ *   fp64; all arithmetic is fp64; sums over users run in index order.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+enum { ORACLE_PROJ_SIMPLEX_INEQ = 0, ORACLE_PROJ_BOX = 1, ORACLE_PROJ_BOXCUT = 2, ORACLE_PROJ_SIMPLEX_EQ = 3 };
+
+static int cmp_desc(const void* pa, const void* pb) {
+    double a = *(const double*)pa, b = *(const double*)pb;
+    return (a < b) - (a > b);
+}
+
+/* Equality-form simplex {x>=0, sum x = z}: Duchi et al. 2008, Fig. 1 (the stages P:117 names:
+ * sort, prefix sums, cutoff index rho, threshold theta, subtract-and-clamp). */
+void dualip_oracle_project_simplex_eq(const double* v, int64_t n, double z, double* x) {
+    if (n <= 0) return;
+    double* u = (double*)malloc((size_t)n * sizeof(double));
+    memcpy(u, v, (size_t)n * sizeof(double));
+    qsort(u, (size_t)n, sizeof(double), cmp_desc);              /* u_1 >= u_2 >= ... */
+    double csum = 0.0, c_rho = 0.0;
+    int64_t rho = 0;
+    for (int64_t k = 1; k <= n; ++k) {
+        csum += u[k - 1];                                        /* c_k = sum_{l<=k} u_l */
+        if (u[k - 1] - (csum - z) / (double)k > 0.0) { rho = k; c_rho = csum; }
+    }
+    double theta = (c_rho - z) / (double)rho;                    /* rho >= 1 whenever z > 0 */
+    for (int64_t p = 0; p < n; ++p) x[p] = fmax(v[p] - theta, 0.0);
+    free(u);
+}
+
+/* Inequality-form simplex {x>=0, sum x <= z} ("inequality variant").
+ * Reading R5: exact early exit -- if sum max(v,0) <= z return max(v,0), no tolerance. */
+void dualip_oracle_project_simplex(const double* v, int64_t n, double z, double* x) {
+    double s = 0.0;
+    for (int64_t p = 0; p < n; ++p) { x[p] = fmax(v[p], 0.0); s += x[p]; }
+    if (s <= z) return;
+    dualip_oracle_project_simplex_eq(v, n, z, x);
+}
+
+/* Box {lo <= x <= hi} element-wise ("box"). */
+void dualip_oracle_project_box(const double* v, int64_t n, double lo, double hi, double* x) {
+    for (int64_t p = 0; p < n; ++p) x[p] = fmin(fmax(v[p], lo), hi);
+}
+
+static double clip(double t, double lo, double hi) { return fmin(fmax(t, lo), hi); }
+
+/* Box-cut {0 <= x <= ub, sum x <= z} (P:130 names it; reading R10).
+ * p = clip(v,0,ub); if sum p <= z return p.  Otherwise phi(theta) = sum clip(v-theta,0,ub) is
+ * continuous, piecewise linear and non-increasing with breakpoints {v_p, v_p-ub}; walk the
+ * breakpoints in descending order, evaluating phi by its definition at each, until the segment
+ * that contains phi = z is found; solve that linear piece exactly. */
+void dualip_oracle_project_boxcut(const double* v, int64_t n, double ub, double z, double* x) {
+    double s = 0.0;
+    for (int64_t p = 0; p < n; ++p) { x[p] = clip(v[p], 0.0, ub); s += x[p]; }
+    if (s <= z || n <= 0) return;
+    int64_t nb = 2 * n;
+    double* t = (double*)malloc((size_t)nb * sizeof(double));
+    for (int64_t p = 0; p < n; ++p) { t[2 * p] = v[p]; t[2 * p + 1] = v[p] - ub; }
+    qsort(t, (size_t)nb, sizeof(double), cmp_desc);
+    double theta = 0.0, t_hi = t[0], phi_hi = 0.0;               /* phi(max v) = 0 */
+    int found = 0;
+    for (int64_t k = 1; k < nb && !found; ++k) {
+        double phi_lo = 0.0;
+        for (int64_t p = 0; p < n; ++p) phi_lo += clip(v[p] - t[k], 0.0, ub);
+        if (phi_lo >= z) {                                       /* z in [phi_hi, phi_lo] on [t[k], t_hi] */
+            theta = (phi_lo == phi_hi) ? t[k] : t[k] + (phi_lo - z) * (t_hi - t[k]) / (phi_lo - phi_hi);
+            found = 1;
+        } else { t_hi = t[k]; phi_hi = phi_lo; }
+    }
+    /* found is guaranteed: phi is non-increasing, phi(0) = s > z, and below the smallest breakpoint
+     * phi is the constant n*ub = phi(t_min); so some breakpoint has phi >= z. */
+    for (int64_t p = 0; p < n; ++p) x[p] = clip(v[p] - theta, 0.0, ub);
+    free(t);
+}
+
+static void project(int kind, double p0, double p1, const double* v, int64_t n, double* x) {
+    switch (kind) {
+        case ORACLE_PROJ_SIMPLEX_INEQ: dualip_oracle_project_simplex(v, n, p0, x); break;
+        case ORACLE_PROJ_BOX:          dualip_oracle_project_box(v, n, p0, p1, x); break;
+        case ORACLE_PROJ_BOXCUT:       dualip_oracle_project_boxcut(v, n, p0, p1, x); break;
+        default:                       dualip_oracle_project_simplex_eq(v, n, p0, x); break;
+    }
+}
+
+/* One evaluation of Eq. 2-4 at lambda (any sign) and gamma > 0.
+ * proj params: simplex kinds p0 = z; box p0 = lo, p1 = hi; boxcut p0 = ub, p1 = z.
+ * scalars_out[5] = { g, obj = c'x, reg = (gamma/2)|x|^2, r_inf = max(0, max grad), r_2 = |max(grad,0)|_2 }.
+ * x_out (nnz doubles, input order) may be NULL.  Returns 0, or -1 on allocation failure. */
+int dualip_oracle_grad(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr, const int32_t* item_idx,
+                       const float* c, const float* a, const float* b, const double* lambda, double gamma,
+                       int proj_kind, double p0, double p1, double* grad_out, double* scalars_out,
+                       double* x_out) {
+    int64_t max_len = 0;
+    for (int64_t i = 0; i < I; ++i)
+        if (row_ptr[i + 1] - row_ptr[i] > max_len) max_len = row_ptr[i + 1] - row_ptr[i];
+    double* v = (double*)malloc((size_t)(max_len + 1) * sizeof(double));
+    double* x = (double*)malloc((size_t)(max_len + 1) * sizeof(double));
+    if (!v || !x) { free(v); free(x); return -1; }
+    int64_t Jm = (int64_t)J * m;
+    for (int64_t q = 0; q < Jm; ++q) grad_out[q] = 0.0;          /* s = A x, accumulated in user order */
+    double obj = 0.0, sq = 0.0;
+    for (int64_t i = 0; i < I; ++i) {
+        int64_t beg = row_ptr[i], n = row_ptr[i + 1] - beg;
+        for (int64_t p = 0; p < n; ++p) {
+            int64_t j = item_idx[beg + p];
+            double al = 0.0;                                     /* (A' lambda)_p = sum_k a^k_p lambda_{j,k} */
+            for (int32_t k = 0; k < m; ++k) al += (double)a[(beg + p) * m + k] * lambda[j * m + k];
+            v[p] = -((double)c[beg + p] + al) / gamma;           /* Eq. 3 argument */
+        }
+        project(proj_kind, p0, p1, v, n, x);
+        for (int64_t p = 0; p < n; ++p) {
+            int64_t j = item_idx[beg + p];
+            for (int32_t k = 0; k < m; ++k) grad_out[j * m + k] += (double)a[(beg + p) * m + k] * x[p];
+            obj += (double)c[beg + p] * x[p];
+            sq += x[p] * x[p];
+            if (x_out) x_out[beg + p] = x[p];
+        }
+    }
+    double reg = 0.5 * gamma * sq, dot = 0.0, r_inf = 0.0, r2 = 0.0;
+    for (int64_t q = 0; q < Jm; ++q) {
+        grad_out[q] -= (double)b[q];                             /* Eq. 4 */
+        dot += lambda[q] * grad_out[q];
+        if (grad_out[q] > 0.0) { r2 += grad_out[q] * grad_out[q]; if (grad_out[q] > r_inf) r_inf = grad_out[q]; }
+    }
+    scalars_out[0] = obj + reg + dot;                            /* Eq. 2 at its minimiser */
+    scalars_out[1] = obj;
+    scalars_out[2] = reg;
+    scalars_out[3] = r_inf;
+    scalars_out[4] = sqrt(r2);
+    free(v); free(x);
+    return 0;
+}
+
+/* L = max_j sum_k sum_i (a^k_ij)^2  (reading R2: |A|_2^2 exactly for m = 1 because A A' is then
+ * diag(sum_i a_ij^2); a trace upper bound on the m x m Gram blocks for m > 1). */
+double dualip_oracle_lipschitz(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr,
+                               const int32_t* item_idx, const float* a) {
+    double* col = (double*)calloc((size_t)J, sizeof(double));
+    if (!col) return -1.0;
+    for (int64_t p = 0; p < row_ptr[I]; ++p)
+        for (int32_t k = 0; k < m; ++k) col[item_idx[p]] += (double)a[p * m + k] * (double)a[p * m + k];
+    double L = 0.0;
+    for (int32_t j = 0; j < J; ++j) if (col[j] > L) L = col[j];
+    free(col);
+    return L;
+}
+
+/* gamma-continuation driver with projected Nesterov ascent (readings R1-R4 in DESIGN.md; the paper
+ * gives the update in words only).
+ *   for each stage s: eta = gamma_s / L;  y_0 = lambda (warm start);  t = 0
+ *     repeat iters[s] times:
+ *        (g_t, grad_t) = grad(y_t, gamma_s)
+ *        lambda_{t+1}  = max(0, y_t + eta * grad_t)
+ *        beta_t        = momentum ? t/(t+3) : 0
+ *        y_{t+1}       = lambda_{t+1} + beta_t (lambda_{t+1} - lambda_t);   t <- t+1
+ *   then one extra grad(lambda_T, gamma_S) gives final scalars / grad / x.
+ * Traces (each may be NULL) are indexed by the global iteration counter n = 0..sum(iters)-1:
+ *   trace_g[n] = g(y_t), trace_rinf[n], trace_r2[n], trace_grad[n*Jm..] = grad(y_t),
+ *   trace_lambda[n*Jm..] = lambda_{t+1}.  stage_x (may be NULL) receives, per stage, x*(lambda_end)
+ *   at that stage's gamma (n_stages * nnz doubles) -- used by the drift report of config 5. */
+int dualip_oracle_solve(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr, const int32_t* item_idx,
+                        const float* c, const float* a, const float* b, int proj_kind, double p0, double p1,
+                        const double* gammas, int32_t n_stages, const int32_t* iters, int32_t momentum,
+                        double* lambda_inout, double* x_out, double* final_scalars, double* final_grad,
+                        double* trace_g, double* trace_rinf, double* trace_r2, double* trace_grad,
+                        double* trace_lambda, double* stage_x) {
+    int64_t Jm = (int64_t)J * m, nnz = row_ptr[I];
+    double L = dualip_oracle_lipschitz(I, J, m, row_ptr, item_idx, a);
+    if (!(L > 0.0)) L = 1.0;
+    double* y = (double*)malloc((size_t)Jm * sizeof(double));
+    double* grad = (double*)malloc((size_t)Jm * sizeof(double));
+    double* lam_new = (double*)malloc((size_t)Jm * sizeof(double));
+    if (!y || !grad || !lam_new) { free(y); free(grad); free(lam_new); return -1; }
+    double sc[5];
+    int64_t n = 0;
+    int rc = 0;
+    for (int32_t s = 0; s < n_stages && rc == 0; ++s) {
+        double gamma = gammas[s], eta = gamma / L;
+        memcpy(y, lambda_inout, (size_t)Jm * sizeof(double));    /* warm start, momentum restart */
+        for (int32_t t = 0; t < iters[s] && rc == 0; ++t, ++n) {
+            rc = dualip_oracle_grad(I, J, m, row_ptr, item_idx, c, a, b, y, gamma, proj_kind, p0, p1, grad, sc, NULL);
+            if (trace_g) trace_g[n] = sc[0];
+            if (trace_rinf) trace_rinf[n] = sc[3];
+            if (trace_r2) trace_r2[n] = sc[4];
+            if (trace_grad) memcpy(trace_grad + n * Jm, grad, (size_t)Jm * sizeof(double));
+            double beta = momentum ? (double)t / (double)(t + 3) : 0.0;
+            for (int64_t q = 0; q < Jm; ++q) {
+                lam_new[q] = fmax(0.0, y[q] + eta * grad[q]);
+                y[q] = lam_new[q] + beta * (lam_new[q] - lambda_inout[q]);
+            }
+            memcpy(lambda_inout, lam_new, (size_t)Jm * sizeof(double));
+            if (trace_lambda) memcpy(trace_lambda + n * Jm, lam_new, (size_t)Jm * sizeof(double));
+        }
+        if (stage_x && rc == 0)
+            rc = dualip_oracle_grad(I, J, m, row_ptr, item_idx, c, a, b, lambda_inout, gamma, proj_kind, p0, p1,
+                                    grad, sc, stage_x + (int64_t)s * nnz);
+    }
+    if (rc == 0 && n_stages > 0)
+        rc = dualip_oracle_grad(I, J, m, row_ptr, item_idx, c, a, b, lambda_inout, gammas[n_stages - 1],
+                                proj_kind, p0, p1, final_grad ? final_grad : grad, final_scalars ? final_scalars : sc, x_out);
+    free(y); free(grad); free(lam_new);
+    return rc;
+}

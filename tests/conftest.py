@@ -1,0 +1,72 @@
+"""pytest configuration: registers the `gpu` marker and shared helpers/fixtures."""
+import os
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def pytest_configure(config):
+    config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
+    config.addinivalue_line("markers", "slow: full-size GPU parity cases (minutes)")
+
+
+def read_projection_cases():
+    cases = []
+    with open(os.path.join(GOLDEN, "projection_cases.txt")) as f:
+        for line in f:
+            line = line.strip()
+            if not line or line.startswith("#"):
+                continue
+            kind, params, v, x = [s.strip() for s in line.split("|")]
+            cases.append((kind, [float(t) for t in params.split()], np.array(v.split(), dtype=np.float64),
+                          np.array(x.split(), dtype=np.float64)))
+    return cases
+
+
+def read_worked_examples():
+    cases, cur = [], None
+    with open(os.path.join(GOLDEN, "worked_example_grad.txt")) as f:
+        for line in f:
+            line = line.strip()
+            if not line or line.startswith("#"):
+                continue
+            if line == "end":
+                cases.append(cur); cur = None; continue
+            key, val = [s.strip() for s in line.split(":", 1)]
+            if key == "case":
+                cur = {"case": val}
+            elif key in ("I", "J", "m"):
+                cur[key] = int(val)
+            elif key in ("row_ptr", "item_idx"):
+                cur[key] = np.array(val.split(), dtype=np.int64)
+            elif key in ("gamma", "g", "obj", "reg", "r_inf", "r_2"):
+                cur[key] = float(val)
+            else:
+                cur[key] = np.array(val.split(), dtype=np.float64)
+    return cases
+
+
+def random_problem(rng, I, J, m=1, deg=(1, 4), tight=0.5, c_scale=1.0):
+    """Small random matching instance as plain numpy arrays (tests only)."""
+    rows, idx = [0], []
+    for _ in range(I):
+        d = int(rng.integers(deg[0], min(deg[1], J) + 1))
+        idx.extend(sorted(rng.choice(J, size=d, replace=False).tolist()))
+        rows.append(len(idx))
+    nnz = len(idx)
+    c = (-c_scale * rng.random(nnz)).astype(np.float32)
+    a = (0.5 + rng.random(nnz * m)).astype(np.float32)
+    col = np.zeros(J * m)
+    for p, j in enumerate(idx):
+        for k in range(m):
+            col[j * m + k] += a[p * m + k]
+    b = (tight * col / max(1.0, np.mean(np.diff(rows))) + 0.05).astype(np.float32)
+    return dict(I=I, J=J, m=m, row_ptr=np.array(rows, dtype=np.int64), item_idx=np.array(idx, dtype=np.int32),
+                c=c, a=a, b=b)

@@ -1,0 +1,167 @@
+"""Pins for the oracle's AGD / gamma-continuation loop.  The paper prints no update formula (P:123,
+P:145 give words only) so parity with the paper is UNPINNED for this part (readings R1-R4);
+what is pinned: the optimum it converges to (brute-force KKT active-set enumeration on <= 3 users x
+2 items; I=J=1 closed form), the lambda==0 fixed point, monotone ascent of the beta==0 variant at
+eta = gamma/L, the accelerated O(1/T^2) bound, stage/warm-start semantics and the drift bound."""
+import itertools
+
+import numpy as np
+import pytest
+
+import oracle
+from conftest import random_problem
+
+
+def _problem(d, kind=oracle.PROJ_SIMPLEX_INEQ, p0=1.0, p1=0.0):
+    return oracle.Problem(d["I"], d["J"], d["m"], d["row_ptr"], d["item_idx"], d["c"], d["a"], d["b"], kind, p0, p1)
+
+
+def _kkt_brute_force(d, gamma):
+    """min c'x + (gamma/2)|x|^2  s.t. x>=0, per-user sum<=1, per-item sum_i a_ij x_ij <= b_j, by
+    enumerating active sets and solving each equality-constrained QP (Eq. 1)."""
+    n, I, J = d["item_idx"].size, d["I"], d["J"]
+    c, a, b = d["c"].astype(np.float64), d["a"].astype(np.float64), d["b"].astype(np.float64)
+    G, h = [], []
+    for p in range(n):
+        r = np.zeros(n); r[p] = -1.0; G.append(r); h.append(0.0)
+    for i in range(I):
+        r = np.zeros(n); r[d["row_ptr"][i]:d["row_ptr"][i + 1]] = 1.0; G.append(r); h.append(1.0)
+    for j in range(J):
+        r = np.zeros(n); sel = d["item_idx"] == j; r[sel] = a[sel]; G.append(r); h.append(b[j])
+    G, h = np.array(G), np.array(h)
+    best = None
+    for r in range(0, min(n, len(h)) + 1):
+        for S in itertools.combinations(range(len(h)), r):
+            S = list(S)
+            if S:
+                GS = G[S]
+                if np.linalg.matrix_rank(GS) < len(S):
+                    continue
+                mu = np.linalg.solve(GS @ GS.T, -(gamma * h[S] + GS @ c))
+                x = -(c + GS.T @ mu) / gamma
+                if (mu < -1e-10).any():
+                    continue
+            else:
+                x = -c / gamma
+            if (G @ x <= h + 1e-10).all():
+                val = c @ x + 0.5 * gamma * x @ x
+                if best is None or val < best[0] - 1e-13:
+                    best = (val, x)
+    return best
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_converges_to_kkt_optimum(seed):
+    rng = np.random.default_rng(seed)
+    d = random_problem(rng, I=int(rng.integers(1, 4)), J=2, m=1, deg=(1, 2), tight=0.7)
+    d["b"] = (0.15 + 0.5 * rng.random(2)).astype(np.float32)
+    gamma = float(rng.choice([1.0, 0.3]))
+    p_star, x_star = _kkt_brute_force(d, gamma)
+    res = oracle.solve(_problem(d), [gamma], [4000])
+    assert abs(res.final.g - p_star) < 1e-8 * (1 + abs(p_star))          # strong duality
+    np.testing.assert_allclose(res.x, x_star, atol=1e-5)
+    assert np.all(res.lam >= 0)
+    assert np.max(np.abs(res.lam * res.final.grad)) < 1e-6                # complementary slackness
+    assert res.final.r_inf < 1e-6
+    # every iterate's dual value is a lower bound on p* (weak duality)
+    assert np.all(res.trace_g <= p_star + 1e-10)
+
+
+def test_single_variable_closed_form():
+    """I=J=1: x = clip(-(c + a lam)/gamma, 0, 1); if 0 < b/a < 1 binds, lam* = max(0, -(c + gamma b/a)/a)."""
+    c, a, b, gamma = -1.0, 2.0, 0.5, 0.25
+    d = dict(I=1, J=1, m=1, row_ptr=np.array([0, 1]), item_idx=np.array([0], dtype=np.int32),
+             c=np.array([c], dtype=np.float32), a=np.array([a], dtype=np.float32), b=np.array([b], dtype=np.float32))
+    res = oracle.solve(_problem(d), [gamma], [3000])
+    lam_star = max(0.0, -(c + gamma * b / a) / a)
+    assert abs(res.lam[0] - lam_star) < 1e-9
+    assert abs(res.x[0] - b / a) < 1e-9
+
+
+def test_lambda_zero_is_a_fixed_point_when_slack():
+    """grad g(0) <= 0  =>  lambda_t = 0 for all t (what every verbatim BASELINE.json config does)."""
+    rng = np.random.default_rng(3)
+    d = random_problem(rng, I=50, J=6, m=1, deg=(2, 5))
+    d["b"] = np.full(6, 1e3, dtype=np.float32)
+    res = oracle.solve(_problem(d), [0.01], [25], trace_lambda=True)
+    assert np.all(res.trace_lambda == 0.0)
+    assert np.all(res.trace_g == res.trace_g[0])
+
+
+@pytest.mark.parametrize("m", [1, 2])
+def test_plain_ascent_is_monotone_at_eta_gamma_over_L(m):
+    rng = np.random.default_rng(20 + m)
+    d = random_problem(rng, I=120, J=8, m=m, deg=(2, 6), tight=0.4)
+    p = _problem(d)
+    res = oracle.solve(p, [0.2], [150], momentum=False, trace_lambda=True)
+    g_at_iterates = np.array([oracle.grad(p, l, 0.2, want_x=False).g for l in res.trace_lambda[::10]])
+    assert np.all(np.diff(g_at_iterates) >= -1e-12)
+    assert np.all(np.diff(res.trace_g) >= -1e-12)                            # beta = 0: y_t = lambda_t
+
+
+@pytest.mark.parametrize("seed", range(3))
+def test_accelerated_rate_bound(seed):
+    """p* - g(lambda_T) <= 4 L |lambda_0 - lambda*|^2 / (gamma (T+1)^2)   (FISTA-type bound)."""
+    rng = np.random.default_rng(50 + seed)
+    d = random_problem(rng, I=3, J=2, m=1, deg=(2, 2), tight=0.6)
+    d["b"] = (0.2 + 0.3 * rng.random(2)).astype(np.float32)
+    gamma = 0.5
+    p = _problem(d)
+    p_star, _ = _kkt_brute_force(d, gamma)
+    lam_star = oracle.solve(p, [gamma], [6000]).lam
+    L = oracle.lipschitz(p)
+    for T in (5, 20, 80):
+        res = oracle.solve(p, [gamma], [T])
+        assert p_star - res.final.g <= 4.0 * L * (lam_star @ lam_star) / (gamma * (T + 1) ** 2) + 1e-12
+
+
+def test_first_step_and_trace_semantics():
+    rng = np.random.default_rng(31)
+    d = random_problem(rng, I=60, J=7, m=2, deg=(2, 5), tight=0.4)
+    p = _problem(d)
+    gamma, lam0 = 0.3, rng.random(14) * 0.1
+    res = oracle.solve(p, [gamma], [3], lam0=lam0, trace_grad=True, trace_lambda=True)
+    g0 = oracle.grad(p, lam0, gamma)
+    eta = gamma / oracle.lipschitz(p)
+    np.testing.assert_allclose(res.trace_grad[0], g0.grad, atol=0)
+    assert res.trace_g[0] == g0.g
+    lam1 = np.maximum(0.0, lam0 + eta * g0.grad)
+    np.testing.assert_allclose(res.trace_lambda[0], lam1, atol=1e-15)
+    # t = 0: beta = 0 so y_1 = lambda_1; t = 1: beta = 1/4
+    g1 = oracle.grad(p, lam1, gamma)
+    np.testing.assert_allclose(res.trace_grad[1], g1.grad, atol=1e-15)
+    lam2 = np.maximum(0.0, lam1 + eta * g1.grad)
+    y2 = lam2 + 0.25 * (lam2 - lam1)
+    np.testing.assert_allclose(res.trace_grad[2], oracle.grad(p, y2, gamma).grad, atol=1e-13)
+    # final evaluation is at lambda_T (reading R3), not at y
+    fin = oracle.grad(p, res.lam, gamma)
+    assert fin.g == res.final.g
+    np.testing.assert_allclose(fin.x, res.x, atol=0)
+
+
+def test_continuation_equals_chained_warm_started_solves():
+    rng = np.random.default_rng(32)
+    d = random_problem(rng, I=80, J=6, m=1, deg=(2, 5), tight=0.4)
+    p = _problem(d)
+    full = oracle.solve(p, [1.0, 0.1, 0.01], [30, 20, 10], stage_x=True)
+    lam = None
+    for s, (gam, it) in enumerate(zip([1.0, 0.1, 0.01], [30, 20, 10])):
+        part = oracle.solve(p, [gam], [it], lam0=lam)
+        lam = part.lam
+        np.testing.assert_allclose(full.stage_x[s], part.x, atol=0)
+    np.testing.assert_allclose(full.lam, lam, atol=0)
+
+
+def test_drift_bound():
+    """At fixed lambda, |x(c) - x(c')|_2 <= |c - c'|_2 / gamma (non-expansive projection of -c/gamma);
+    the closed form behind the paper's stability claim."""
+    rng = np.random.default_rng(33)
+    d = random_problem(rng, I=200, J=9, m=1, deg=(2, 8))
+    lam = rng.random(9) * 0.2
+    for gamma in (1.0, 0.1, 0.01):
+        d2 = dict(d)
+        d2["c"] = (d["c"] * (1 + 0.01 * rng.normal(size=d["c"].size))).astype(np.float32)
+        x1 = oracle.grad(_problem(d), lam, gamma).x
+        x2 = oracle.grad(_problem(d2), lam, gamma).x
+        dc = np.linalg.norm(d["c"].astype(np.float64) - d2["c"].astype(np.float64))
+        assert np.linalg.norm(x1 - x2) <= dc / gamma + 1e-12

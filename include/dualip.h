@@ -1,0 +1,172 @@
+/*
+ * dualip.h -- C ABI of the B200-native dual-gradient hot path of the ridge-regularised matching-LP
+ * solver of "Large-Scale Regularized Matching on GPU Clusters" (arxiv/paper_2606_07777).
+ * Citations "P:n" are line numbers of the paper text; "R<n>" are the readings listed in
+ * DESIGN.md section 2.
+ *
+ * Problem (Eq. 1; Def. 1):   min_{x in C} c'x + (gamma/2)|x|^2   s.t.  A x <= b
+ *   x_ij for eligible (user i, item j) pairs, stored as per-user CSR rows; C = product over users of a
+ *   simple set C_i (unit simplex, box, box-cut); A is m families of per-item coupling rows,
+ *   (A x)_{j,k} = sum_i a^k_ij x_ij.
+ * Dual (Eq. 2-4):  x*(lambda) = Proj_C(-(A'lambda + c)/gamma),  grad g = A x* - b,
+ *   g(lambda) = c'x* + (gamma/2)|x*|^2 + lambda'(A x* - b).
+ *
+ * Conventions
+ *   - Every entry point returns an int: DUALIP_OK (0) or a negative DUALIP_E* code.  Nothing throws,
+ *     aborts or prints.  On error, outputs are left untouched and *out handles are set to NULL.
+ *   - Layouts are item-major / family-minor: a[p*m+k], b[j*m+k], lambda[j*m+k], grad[j*m+k]  (R14).
+ *   - Row data is int32 / fp32; lambda, grad g, g and all scalars are fp64.
+ *   - "host or device": the pointer kind is detected with cudaPointerGetAttributes.  Device pointers are
+ *     used in place, asynchronously on `stream`.  Host pointers are staged through internal device
+ *     buffers and the call synchronises `stream` before returning.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   - The caller keeps ownership of every buffer it passes.  The handle owns its copies.
+ *   - A handle must not be used from two host threads at once.
+ *   - There is no CPU fallback: without a CUDA device every call fails with DUALIP_ECUDA.
+ */
+#ifndef DUALIP_H
+#define DUALIP_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dualip dualip_t;
+
+enum {
+    DUALIP_OK = 0,
+    DUALIP_EINVAL = -1,       /* bad argument: NULL, negative size, gamma <= 0, unknown enum, m out of range */
+    DUALIP_ERANGE = -2,       /* row_ptr not monotone / row_ptr[0] != 0 / item index outside [0,J) */
+    DUALIP_EDUP = -3,         /* an item appears twice in one user's row (R11) */
+    DUALIP_ENOMEM = -4,       /* host or device allocation failed */
+    DUALIP_ECUDA = -5,        /* a CUDA runtime call failed (no device, launch failure, ...) */
+    DUALIP_EUNSUPPORTED = -6  /* valid request this build cannot serve (e.g. reduction strategy needs more shared memory) */
+};
+
+/* Per-user simple set C_i (R5, R10, R16).  Parameters p0,p1 of dualip_opts:
+ *   SIMPLEX_INEQ {x>=0, sum x <= z}: p0 = z          SIMPLEX_EQ {x>=0, sum x = z}: p0 = z
+ *   BOX {lo <= x <= hi}: p0 = lo, p1 = hi             BOXCUT {0<=x<=ub, sum x<=z}: p0 = ub, p1 = z   */
+enum { DUALIP_PROJ_SIMPLEX_INEQ = 0, DUALIP_PROJ_BOX = 1, DUALIP_PROJ_BOXCUT = 2, DUALIP_PROJ_SIMPLEX_EQ = 3 };
+
+/* Item-wise reduction strategy for s_{j,k} = sum_i a^k_ij x_ij (Eq. 4; P:123 in the paper this is
+ * SpMV + NCCL reduce).  All strategies accumulate in 64-bit fixed point, so results are bit-reproducible
+ * run to run and independent of the launch geometry.
+ *   AUTO   : SMEM when lambda and the accumulators fit in shared memory, else GLOBAL.
+ *   SMEM   : per-CTA shared-memory accumulators (native 32-bit integer atomics with explicit carry),
+ *            flushed once per CTA with RED.ADD.64.
+ *   GLOBAL : RED.ADD.64 straight to L2 for every nonzero x; lambda still gathered from shared memory
+ *            when J*m*8 bytes fit, else through the read-only path.
+ *   CSC    : no atomics: x is written to HBM and each item's column is summed in fixed order through
+ *            an item-sorted permutation built at create (for J*m beyond on-chip capacity).            */
+enum { DUALIP_RED_AUTO = 0, DUALIP_RED_SMEM = 1, DUALIP_RED_GLOBAL = 2, DUALIP_RED_CSC = 3 };
+
+typedef struct {
+    int32_t projection;   /* DUALIP_PROJ_* */
+    double  p0, p1;       /* projection parameters, see above */
+    int32_t reduction;    /* DUALIP_RED_* */
+    int32_t borrow;       /* 1: device inputs are used in place and must outlive the handle; 0: copied */
+    int32_t validate;     /* 1: check index range, monotone row_ptr, duplicates (a0); 0: trust the caller */
+    int32_t momentum;     /* 1: beta_t = t/(t+3) (R1); 0: plain projected ascent (beta = 0) */
+    int32_t group_lanes;  /* lanes cooperating on one row: 0 = auto from the mean row length, or 4/8/16/32 */
+    int32_t grid_ctas;    /* CTAs of the gradient kernel: 0 = auto (SM count x resident CTAs per SM) */
+    int32_t use_graph;    /* 1: dualip_solve replays a captured CUDA graph per stage; 0: direct launches */
+    int32_t reserved[5];  /* must be zero */
+} dualip_opts;
+
+/* Fills *opts with the defaults: unit simplex (inequality), AUTO reduction, copy, validate, momentum. */
+void dualip_opts_default(dualip_opts* opts);
+
+/* Scalars of one evaluation (Eq. 2; "objective value and regularization term"; "slack"; R9). */
+typedef struct {
+    double g;      /* dual objective g(lambda) = obj + reg + lambda'grad */
+    double obj;    /* c'x* */
+    double reg;    /* (gamma/2)|x*|^2 */
+    double r_inf;  /* max(0, max_jk grad_jk) : maximum positive constraint violation */
+    double r_2;    /* |max(grad, 0)|_2 */
+} dualip_scalars;
+
+/* Optional per-iteration trace of dualip_solve.  All pointers are DEVICE pointers (or NULL to skip that
+ * column); entry n is the n-th gradient evaluation over all stages (0 <= n < sum iters <= capacity).
+ *   g[n], r_inf[n], r_2[n] : scalars at the extrapolated point y_t the gradient is taken at (R1)
+ *   grad[n*J*m + q]        : grad g(y_t)
+ *   lambda[n*J*m + q]      : lambda_{t+1}                                                         */
+typedef struct {
+    int64_t capacity;
+    double* g;
+    double* r_inf;
+    double* r_2;
+    double* grad;
+    double* lambda;
+} dualip_trace;
+
+typedef struct {
+    int64_t I, nnz;
+    int32_t J, m;
+    double  L;               /* max_j sum_k sum_i (a^k_ij)^2 (R2) */
+    int64_t max_row_len;
+    int32_t group_lanes;     /* lanes per row in the gradient kernel */
+    int32_t chunk_regs;      /* row chunks held in registers (rows longer than group_lanes*chunk_regs take the warp path) */
+    int32_t reduction;       /* the strategy in effect (never AUTO) */
+    int32_t lambda_in_smem;  /* 1 if lambda is staged in shared memory */
+    int32_t grid_ctas, block_threads;
+    int64_t smem_bytes;      /* dynamic shared memory per CTA of the gradient kernel */
+    int64_t bytes_resident;  /* device bytes owned by the handle */
+    int64_t launches;        /* kernels launched through this handle so far (all entry points) */
+    double  fix_scale_s;     /* fixed-point scale of the item accumulators (a power of two) */
+} dualip_info;
+
+/*
+ * a0 -- build a device-resident problem from per-user CSR rows ("one column pointer, one row index
+ * per nonzero, one value per nonzero"; here one block per user).
+ *   I >= 0 users, J >= 1 items, 1 <= m <= 4 coupling families (Def. 1).
+ *   row_ptr[I+1] int64 (host or device), row_ptr[0] = 0, non-decreasing; nnz = row_ptr[I] (may exceed 2^31).
+ *   item_idx[nnz] int32 in [0,J), distinct within a row, any order;  c[nnz];  a[nnz*m];  b[J*m].
+ *   opts may be NULL (defaults).
+ * Work done: copy (or borrow), validation kernels, L (R2), column |a| sums and sum|c| for the fixed-point
+ * scales, row-length statistics, launch plan; with DUALIP_RED_CSC also the item-sorted permutation.
+ * Synchronises `stream`.  Errors: EINVAL, ERANGE, EDUP, ENOMEM, ECUDA, EUNSUPPORTED.
+ */
+int dualip_create(dualip_t** out, int64_t I, int32_t J, int32_t m, const int64_t* row_ptr,
+                  const int32_t* item_idx, const float* c, const float* a, const float* b,
+                  const dualip_opts* opts, void* stream);
+
+/*
+ * a1-a5 (+a8) -- one evaluation of Eq. 2-4 at `lambda` (any sign; g is defined on all of R^{mJ}) and gamma > 0.
+ *   lambda[J*m] in;  grad[J*m] out (may be NULL);  scalars out (may be NULL);
+ *   x[nnz] fp32 out in input nonzero order, or NULL (then x is never written to memory).
+ *   Each pointer may be host or device, independently.
+ */
+int dualip_grad(dualip_t* h, const double* lambda, double gamma, double* grad, dualip_scalars* scalars,
+                float* x, void* stream);
+
+/*
+ * a1-a8 -- gamma continuation with projected accelerated ascent (R1-R4).
+ *   for each stage s < n_stages:  eta = gammas[s]/L;  y = lambda (warm start, momentum restart)
+ *       repeat iters[s] times:  grad at y;  lambda+ = max(0, y + eta*grad);  y = lambda+ + beta_t (lambda+ - lambda)
+ *   then one evaluation at the final lambda with gammas[n_stages-1] fills final_scalars / final_grad / x_out.
+ *   gammas, iters: HOST arrays.  lambda_inout[J*m]: warm start in (zeros for a cold start), lambda_T out.
+ *   x_out[nnz], final_scalars, final_grad[J*m] may be NULL; host or device.  trace may be NULL.
+ *   n_stages = 0 is allowed (nothing happens).  No host synchronisation happens inside the loop.
+ */
+int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int32_t* iters,
+                 double* lambda_inout, float* x_out, dualip_scalars* final_scalars, double* final_grad,
+                 const dualip_trace* trace, void* stream);
+
+/* Replace c (nnz fp32, host or device) in place without rebuilding -- config 5's perturbed re-solve.
+ * Recomputes the objective's fixed-point scale.  With borrow = 1 the handle switches to the new pointer. */
+int dualip_set_c(dualip_t* h, const float* c_new, void* stream);
+
+int dualip_get_info(const dualip_t* h, dualip_info* info);
+
+/* Frees everything the handle owns.  NULL is accepted. */
+void dualip_destroy(dualip_t* h);
+
+/* Static message for a return code. */
+const char* dualip_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DUALIP_H */

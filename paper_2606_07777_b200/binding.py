@@ -1,0 +1,216 @@
+"""ctypes binding of include/dualip.h -- argument marshalling only; every step of the path runs in the CUDA
+kernels behind the C ABI.  Same names as the C entry points: Problem.create / grad / solve / set_c / info.
+
+torch is used for device memory and streams: device tensors are passed as raw pointers, host numpy arrays
+are passed as host pointers (the library stages them itself).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+PROJ_SIMPLEX_INEQ, PROJ_BOX, PROJ_BOXCUT, PROJ_SIMPLEX_EQ = 0, 1, 2, 3
+RED_AUTO, RED_SMEM, RED_GLOBAL, RED_CSC = 0, 1, 2, 3
+
+EXPORTED_SYMBOLS = ("dualip_opts_default", "dualip_create", "dualip_grad", "dualip_solve", "dualip_set_c",
+                    "dualip_get_info", "dualip_destroy", "dualip_strerror")
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+class DualipError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"dualip error {code}: {msg}")
+        self.code = code
+
+
+class Opts(ctypes.Structure):
+    _fields_ = [("projection", ctypes.c_int32), ("p0", ctypes.c_double), ("p1", ctypes.c_double),
+                ("reduction", ctypes.c_int32), ("borrow", ctypes.c_int32), ("validate", ctypes.c_int32),
+                ("momentum", ctypes.c_int32), ("group_lanes", ctypes.c_int32), ("grid_ctas", ctypes.c_int32),
+                ("use_graph", ctypes.c_int32), ("reserved", ctypes.c_int32 * 5)]
+
+
+class Scalars(ctypes.Structure):
+    _fields_ = [("g", ctypes.c_double), ("obj", ctypes.c_double), ("reg", ctypes.c_double),
+                ("r_inf", ctypes.c_double), ("r_2", ctypes.c_double)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class _Trace(ctypes.Structure):
+    _fields_ = [("capacity", ctypes.c_int64), ("g", ctypes.c_void_p), ("r_inf", ctypes.c_void_p),
+                ("r_2", ctypes.c_void_p), ("grad", ctypes.c_void_p), ("lam", ctypes.c_void_p)]
+
+
+class Info(ctypes.Structure):
+    _fields_ = [("I", ctypes.c_int64), ("nnz", ctypes.c_int64), ("J", ctypes.c_int32), ("m", ctypes.c_int32),
+                ("L", ctypes.c_double), ("max_row_len", ctypes.c_int64), ("group_lanes", ctypes.c_int32),
+                ("chunk_regs", ctypes.c_int32), ("reduction", ctypes.c_int32), ("lambda_in_smem", ctypes.c_int32),
+                ("grid_ctas", ctypes.c_int32), ("block_threads", ctypes.c_int32), ("smem_bytes", ctypes.c_int64),
+                ("bytes_resident", ctypes.c_int64), ("launches", ctypes.c_int64), ("fix_scale_s", ctypes.c_double)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+def lib_path() -> str:
+    return os.path.join(_HERE, "libdualip_b200.so")
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen the in-tree CUDA library; fails loudly if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        path = lib_path()
+        if not os.path.exists(path):
+            raise ImportError(f"{path} is missing: run `python -m paper_2606_07777_b200.build` "
+                              "(or __graft_entry__.build()); there is no CPU fallback")
+        lib = ctypes.CDLL(path)
+        vp, i32, i64, d = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_double
+        lib.dualip_opts_default.argtypes = [ctypes.POINTER(Opts)]
+        lib.dualip_opts_default.restype = None
+        lib.dualip_create.argtypes = [ctypes.POINTER(vp), i64, i32, i32, vp, vp, vp, vp, vp, ctypes.POINTER(Opts), vp]
+        lib.dualip_grad.argtypes = [vp, vp, d, vp, vp, vp, vp]
+        lib.dualip_solve.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, ctypes.POINTER(_Trace), vp]
+        lib.dualip_set_c.argtypes = [vp, vp, vp]
+        lib.dualip_get_info.argtypes = [vp, ctypes.POINTER(Info)]
+        lib.dualip_destroy.argtypes = [vp]
+        lib.dualip_destroy.restype = None
+        lib.dualip_strerror.argtypes = [ctypes.c_int]
+        lib.dualip_strerror.restype = ctypes.c_char_p
+        for f in ("dualip_create", "dualip_grad", "dualip_solve", "dualip_set_c", "dualip_get_info"):
+            getattr(lib, f).restype = ctypes.c_int
+        _lib = lib
+    return _lib
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise DualipError(rc, load_library().dualip_strerror(rc).decode())
+
+
+def _ptr(t, dtype=None, keep=None):
+    """Raw pointer of a torch tensor (device or host) or numpy array; None -> NULL."""
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        if dtype is not None and t.dtype != dtype:
+            raise TypeError(f"expected {dtype}, got {t.dtype}")
+        if not t.flags["C_CONTIGUOUS"]:
+            raise ValueError("array must be C-contiguous")
+        return ctypes.c_void_p(t.ctypes.data)
+    import torch
+    if isinstance(t, torch.Tensor):
+        if not t.is_contiguous():
+            raise ValueError("tensor must be contiguous")
+        if dtype is not None and np.dtype(str(t.dtype).replace("torch.", "")) != dtype:
+            raise TypeError(f"expected {dtype}, got {t.dtype}")
+        return ctypes.c_void_p(t.data_ptr())
+    raise TypeError(type(t))
+
+
+def make_opts(projection=PROJ_SIMPLEX_INEQ, p0=1.0, p1=0.0, reduction=RED_AUTO, borrow=False, validate=True,
+              momentum=True, group_lanes=0, grid_ctas=0, use_graph=False) -> Opts:
+    o = Opts()
+    load_library().dualip_opts_default(ctypes.byref(o))
+    o.projection, o.p0, o.p1, o.reduction = projection, p0, p1, reduction
+    o.borrow, o.validate, o.momentum = int(borrow), int(validate), int(momentum)
+    o.group_lanes, o.grid_ctas, o.use_graph = group_lanes, grid_ctas, int(use_graph)
+    return o
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        if torch.cuda.is_available():
+            return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+        return None
+    return ctypes.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+
+
+class Problem:
+    """Handle of a device-resident matching LP (dualip_t*)."""
+
+    def __init__(self, handle, I, J, m, nnz, keep):
+        self._h, self.I, self.J, self.m, self.nnz, self._keep = handle, I, J, m, nnz, keep
+
+    @classmethod
+    def create(cls, I, J, m, row_ptr, item_idx, c, a, b, opts: Opts | None = None, stream=None) -> "Problem":
+        """dualip_create: per-user CSR rows (row_ptr int64, item_idx int32, c fp32, a fp32[nnz*m]) + b fp32[J*m];
+        each array a torch tensor (CUDA or CPU) or a numpy array."""
+        lib = load_library()
+        h = ctypes.c_void_p()
+        rc = lib.dualip_create(ctypes.byref(h), I, J, m, _ptr(row_ptr, np.int64), _ptr(item_idx, np.int32),
+                               _ptr(c, np.float32), _ptr(a, np.float32), _ptr(b, np.float32),
+                               ctypes.byref(opts) if opts is not None else None, _stream_ptr(stream))
+        _check(rc)
+        nnz = int(row_ptr[-1])
+        keep = (row_ptr, item_idx, c, a) if (opts is not None and opts.borrow) else None
+        return cls(h, I, J, m, nnz, keep)
+
+    def grad(self, lam, gamma: float, grad=None, scalars=None, x=None, stream=None):
+        """dualip_grad: lam fp64[J*m] in; grad fp64[J*m], x fp32[nnz] out (tensors / arrays or None).
+        `scalars`: a Scalars() to fill, a 5-element fp64 device tensor, or None.  Returns `scalars`."""
+        sp = ctypes.byref(scalars) if isinstance(scalars, Scalars) else _ptr(scalars, np.float64)
+        if isinstance(scalars, Scalars):
+            sp = ctypes.cast(sp, ctypes.c_void_p)
+        _check(load_library().dualip_grad(self._h, _ptr(lam, np.float64), float(gamma), _ptr(grad, np.float64), sp,
+                                          _ptr(x, np.float32), _stream_ptr(stream)))
+        return scalars
+
+    def solve(self, gammas, iters, lam, x=None, scalars=None, grad=None, trace=None, stream=None):
+        """dualip_solve: lam fp64[J*m] in/out.  trace: dict with optional device tensors under the keys
+        'g','r_inf','r_2' (fp64[T]), 'grad','lambda' (fp64[T*J*m]); T = sum(iters)."""
+        gam = np.ascontiguousarray(np.asarray(gammas, dtype=np.float64))
+        its = np.ascontiguousarray(np.asarray(iters, dtype=np.int32))
+        if gam.shape != its.shape or gam.ndim != 1:
+            raise ValueError("gammas and iters must be 1-D of equal length")
+        tr = None
+        if trace is not None:
+            tr = _Trace()
+            tr.capacity = int(its.sum())
+            for key, field in (("g", "g"), ("r_inf", "r_inf"), ("r_2", "r_2"), ("grad", "grad"), ("lambda", "lam")):
+                t = trace.get(key)
+                if t is not None:
+                    if not t.is_cuda:
+                        raise ValueError("trace buffers must be CUDA tensors")
+                    need = tr.capacity * (self.J * self.m if key in ("grad", "lambda") else 1)
+                    if t.numel() < need:
+                        raise ValueError(f"trace['{key}'] too small")
+                    setattr(tr, field, t.data_ptr())
+        sp = ctypes.byref(scalars) if isinstance(scalars, Scalars) else _ptr(scalars, np.float64)
+        if isinstance(scalars, Scalars):
+            sp = ctypes.cast(sp, ctypes.c_void_p)
+        _check(load_library().dualip_solve(self._h, _ptr(gam), gam.size, _ptr(its), _ptr(lam, np.float64),
+                                           _ptr(x, np.float32), sp, _ptr(grad, np.float64),
+                                           ctypes.byref(tr) if tr is not None else None, _stream_ptr(stream)))
+        return scalars
+
+    def set_c(self, c_new, stream=None):
+        _check(load_library().dualip_set_c(self._h, _ptr(c_new, np.float32), _stream_ptr(stream)))
+        if self._keep is not None:
+            self._keep = self._keep + (c_new,)
+
+    def info(self) -> Info:
+        inf = Info()
+        _check(load_library().dualip_get_info(self._h, ctypes.byref(inf)))
+        return inf
+
+    def destroy(self):
+        if self._h:
+            load_library().dualip_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

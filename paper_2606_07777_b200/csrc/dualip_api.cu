@@ -1,0 +1,514 @@
+// dualip_api.cu -- the C ABI of include/dualip.h: argument checking, device residency, launch plan and the
+// gamma-continuation driver (a0, a7).  Every arithmetic step of the path runs in the kernels of
+// dualip_kernels.cuh; the host only sizes buffers, picks fixed-point exponents and launches.
+#include "../../include/dualip.h"
+#include "dualip_kernels.cuh"
+
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+using namespace dualip_dev;
+
+namespace {
+
+constexpr size_t kSmemBudget = 227 * 1024;  // bytes of dynamic shared memory one CTA may opt in to on sm_100a
+
+struct Plan {
+    int G = 32, KREG = 5, M = 1;
+    bool lam_smem = true, acc_smem = true;
+    int grid = 0;
+    size_t smem = 0;
+    const void* fn = nullptr;
+};
+
+}  // namespace
+
+struct dualip {
+    long long I = 0, nnz = 0;
+    int J = 0, m = 0;
+    dualip_opts opts{};
+    // row data (owned unless borrowed)
+    const long long* row_ptr = nullptr; const int* idx = nullptr; const float* c = nullptr; const float* a = nullptr;
+    bool own_rows = false, own_c = false;
+    float* b = nullptr;
+    // scratch
+    unsigned long long* s_fix = nullptr;   // JM (+2 scalars at the end)
+    unsigned long long* sc_fix = nullptr;
+    double* lam_cur = nullptr; double* y = nullptr; double* lam_stage = nullptr; double* grad_stage = nullptr;
+    double* scalars_dev = nullptr;
+    float* x_stage = nullptr;
+    // constants from a0
+    double L = 0.0, max_colabs = 0.0, sum_abs_c = 0.0;
+    long long max_row_len = 0;
+    double scale_s = 1.0, scale_obj = 1.0, scale_sq = 1.0;
+    double xmax = 1.0;
+    Plan plan;
+    int num_sms = 0;
+    long long launches = 0;
+    long long bytes_resident = 0;
+};
+
+namespace {
+
+#define CK(call) do { if ((call) != cudaSuccess) { cudaGetLastError(); return DUALIP_ECUDA; } } while (0)
+
+bool is_device_ptr(const void* p) {
+    if (!p) return false;
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+template <typename T>
+int dev_alloc(dualip* h, T** out, size_t n) {
+    void* p = nullptr;
+    if (cudaMalloc(&p, n ? n * sizeof(T) : sizeof(T)) != cudaSuccess) { cudaGetLastError(); return DUALIP_ENOMEM; }
+    h->bytes_resident += (long long)(n * sizeof(T));
+    *out = static_cast<T*>(p);
+    return DUALIP_OK;
+}
+
+// 2^e with |bound| * 2^e < 2^61
+double fix_scale(double bound) {
+    if (!(bound > 0.0) || !std::isfinite(bound)) return 1.0;
+    int e = 0;
+    std::frexp(bound, &e);
+    int s = 61 - e;
+    if (s > 1000) s = 1000;
+    if (s < -1000) s = -1000;
+    return std::ldexp(1.0, s);
+}
+
+template <int G, int KREG, int M>
+const void* pick_mode(bool lam, bool acc) {
+    if (lam && acc) return (const void*)k_grad<G, KREG, M, true, true>;
+    if (lam) return (const void*)k_grad<G, KREG, M, true, false>;
+    return (const void*)k_grad<G, KREG, M, false, false>;
+}
+template <int G, int KREG>
+const void* pick_m(int M, bool lam, bool acc) {
+    if (M == 1) return pick_mode<G, KREG, 1>(lam, acc);
+    if (M == 2) return pick_mode<G, KREG, 2>(lam, acc);
+    return nullptr;
+}
+template <int G>
+const void* pick_k(int KREG, int M, bool lam, bool acc) {
+    if (KREG == 2) return pick_m<G, 2>(M, lam, acc);
+    if (KREG == 3) return pick_m<G, 3>(M, lam, acc);
+    return pick_m<G, 5>(M, lam, acc);
+}
+const void* pick_kernel(const Plan& pl) {
+    if (pl.M == 0) return pick_mode<32, 5, 0>(pl.lam_smem, pl.acc_smem);
+    if (pl.G == 8) return pick_k<8>(pl.KREG, pl.M, pl.lam_smem, pl.acc_smem);
+    if (pl.G == 16) return pick_k<16>(pl.KREG, pl.M, pl.lam_smem, pl.acc_smem);
+    return pick_k<32>(pl.KREG, pl.M, pl.lam_smem, pl.acc_smem);
+}
+
+int make_plan(dualip* h) {
+    Plan pl;
+    const size_t JM = (size_t)h->J * h->m;
+    const int red = h->opts.reduction;
+    if (red == DUALIP_RED_CSC) return DUALIP_EUNSUPPORTED;
+    const bool fits_both = 16 * JM <= kSmemBudget, fits_lam = 8 * JM <= kSmemBudget;
+    if (red == DUALIP_RED_SMEM && !fits_both) return DUALIP_EUNSUPPORTED;
+    pl.acc_smem = (red == DUALIP_RED_AUTO || red == DUALIP_RED_SMEM) && fits_both;
+    pl.lam_smem = pl.acc_smem || fits_lam;
+    pl.M = (h->m <= 2) ? h->m : 0;
+    const double mean = h->I > 0 ? (double)h->nnz / (double)h->I : 0.0;
+    int G = h->opts.group_lanes;
+    if (G == 0) G = mean > 20.0 ? 32 : (mean > 10.0 ? 16 : 8);
+    if (G == 4) G = 8;
+    if (G != 8 && G != 16 && G != 32) return DUALIP_EINVAL;
+    if (pl.M == 0) G = 32;
+    pl.G = G;
+    pl.KREG = 5;
+    if (pl.M != 0) {
+        if ((long long)G * 2 >= h->max_row_len) pl.KREG = 2;
+        else if ((long long)G * 3 >= h->max_row_len) pl.KREG = 3;
+    }
+    pl.smem = (pl.lam_smem ? 8 * JM : 0) + (pl.acc_smem ? 8 * JM : 0);
+    pl.fn = pick_kernel(pl);
+    if (!pl.fn) return DUALIP_EUNSUPPORTED;
+    CK(cudaFuncSetAttribute(pl.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+    int nb = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pl.fn, kBlockThreads, pl.smem));
+    if (nb < 1) return DUALIP_EUNSUPPORTED;
+    pl.grid = h->opts.grid_ctas > 0 ? h->opts.grid_ctas : h->num_sms * nb;
+    h->plan = pl;
+    return DUALIP_OK;
+}
+
+void set_xmax(dualip* h) {
+    const dualip_opts& o = h->opts;
+    switch (o.projection) {
+        case DUALIP_PROJ_BOX: h->xmax = std::fmax(std::fabs(o.p0), std::fabs(o.p1)); break;
+        case DUALIP_PROJ_BOXCUT: h->xmax = std::fmin(o.p0, o.p1); break;
+        default: h->xmax = o.p0; break;
+    }
+}
+
+void set_scales(dualip* h) {
+    h->scale_s = fix_scale(h->xmax * h->max_colabs * 1.000001);
+    h->scale_obj = fix_scale(h->xmax * h->sum_abs_c * 1.000001);
+    h->scale_sq = fix_scale(h->xmax * h->xmax * (double)(h->nnz > 0 ? h->nnz : 1) * 1.000001);
+}
+
+int grid_for(long long n, int threads, int num_sms) {
+    long long g = (n + threads - 1) / threads;
+    const long long cap = (long long)num_sms * 16;
+    if (g > cap) g = cap;
+    if (g < 1) g = 1;
+    return (int)g;
+}
+
+// a0 constants: L (R2), max column |a| sum, sum |c|; all through order-independent fixed point.
+int compute_stats(dualip* h, cudaStream_t st, bool do_a, bool do_c) {
+    const long long nnz = h->nnz;
+    const int J = h->J, m = h->m, JM = J * m;
+    unsigned* d_mx = nullptr;
+    unsigned long long* d_fix = nullptr;  // colsq[J], colabs[JM], cabs[1], out[2]
+    const size_t nfix = (size_t)J + JM + 3;
+    if (cudaMalloc(&d_mx, 2 * sizeof(unsigned)) != cudaSuccess) { cudaGetLastError(); return DUALIP_ENOMEM; }
+    if (cudaMalloc(&d_fix, nfix * sizeof(unsigned long long)) != cudaSuccess) { cudaGetLastError(); cudaFree(d_mx); return DUALIP_ENOMEM; }
+    int rc = DUALIP_OK;
+    do {
+        if (cudaMemsetAsync(d_mx, 0, 2 * sizeof(unsigned), st) != cudaSuccess ||
+            cudaMemsetAsync(d_fix, 0, nfix * sizeof(unsigned long long), st) != cudaSuccess) { rc = DUALIP_ECUDA; break; }
+        const int g = grid_for(nnz * m, 256, h->num_sms);
+        k_absmax<<<g, 256, 0, st>>>(h->a, nnz * m, h->c, nnz, d_mx); h->launches++;
+        unsigned mx[2];
+        if (cudaMemcpyAsync(mx, d_mx, sizeof(mx), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+            cudaStreamSynchronize(st) != cudaSuccess) { rc = DUALIP_ECUDA; break; }
+        float maxa, maxc;
+        std::memcpy(&maxa, &mx[0], 4); std::memcpy(&maxc, &mx[1], 4);
+        const double rows = (double)(h->I > 0 ? h->I : 1);
+        const double sc_sq = fix_scale((double)maxa * maxa * m * rows * 1.000001);
+        const double sc_abs = fix_scale((double)maxa * rows * 1.000001);
+        const double sc_c = fix_scale((double)maxc * (double)(nnz > 0 ? nnz : 1) * 1.000001);
+        unsigned long long* colsq = d_fix; unsigned long long* colabs = d_fix + J; unsigned long long* cabs = colabs + JM;
+        unsigned long long* out = cabs + 1;
+        k_col_stats<<<grid_for(nnz, 256, h->num_sms), 256, 0, st>>>(h->idx, h->a, h->c, nnz, m, sc_sq, sc_abs, sc_c,
+                                                                    colsq, colabs, cabs, do_a ? 1 : 0, do_c ? 1 : 0);
+        h->launches++;
+        k_reduce_stats<<<1, 1024, 0, st>>>(colsq, J, colabs, JM, out); h->launches++;
+        unsigned long long res[3];
+        if (cudaMemcpyAsync(res, cabs, sizeof(res), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+            cudaStreamSynchronize(st) != cudaSuccess) { rc = DUALIP_ECUDA; break; }
+        if (cudaGetLastError() != cudaSuccess) { rc = DUALIP_ECUDA; break; }
+        if (do_c) h->sum_abs_c = (double)(long long)res[0] / sc_c;
+        if (do_a) { h->L = (double)(long long)res[1] / sc_sq; h->max_colabs = (double)(long long)res[2] / sc_abs; }
+    } while (0);
+    cudaFree(d_mx); cudaFree(d_fix);
+    return rc;
+}
+
+void fill_grad_params(const dualip* h, GradParams& p, const double* lam_dev, double gamma, float* x_dev) {
+    const dualip_opts& o = h->opts;
+    p.row_ptr = h->row_ptr; p.idx = h->idx; p.c = h->c; p.a = h->a;
+    p.lambda = lam_dev; p.s_fix = h->s_fix; p.sc_fix = h->sc_fix; p.x = x_dev;
+    p.I = h->I; p.nnz = h->nnz; p.J = h->J; p.m = h->m; p.proj = o.projection;
+    p.inv_gamma = 1.0 / gamma; p.inv_gamma_f = (float)(1.0 / gamma);
+    p.general_boxcut = 0; p.z = 1.0f; p.ub = 0.0f; p.box_lo = 0.0; p.box_hi = 0.0;
+    switch (o.projection) {
+        case DUALIP_PROJ_BOX: p.box_lo = o.p0; p.box_hi = o.p1; break;
+        case DUALIP_PROJ_BOXCUT:
+            p.ub = (float)o.p0; p.z = (float)o.p1;
+            p.general_boxcut = (o.p0 < o.p1) ? 1 : 0;       // ub >= z is the simplex itself (R10)
+            if (!p.general_boxcut) p.proj = PROJ_SIMPLEX_INEQ;
+            break;
+        default: p.z = (float)o.p0; break;
+    }
+    p.scale_s = h->scale_s; p.scale_obj = h->scale_obj; p.scale_sq = h->scale_sq;
+}
+
+int launch_grad(dualip* h, const double* lam_dev, double gamma, float* x_dev, cudaStream_t st) {
+    GradParams p;
+    fill_grad_params(h, p, lam_dev, gamma, x_dev);
+    if (h->opts.projection == DUALIP_PROJ_BOX) {
+        const int g = grid_for(h->nnz, 256, h->num_sms);
+        if (h->m == 1) k_grad_box<1><<<g, 256, 0, st>>>(p);
+        else if (h->m == 2) k_grad_box<2><<<g, 256, 0, st>>>(p);
+        else k_grad_box<0><<<g, 256, 0, st>>>(p);
+    } else {
+        void* args[] = {(void*)&p};
+        CK(cudaLaunchKernel(h->plan.fn, dim3(h->plan.grid), dim3(kBlockThreads), args, h->plan.smem, st));
+    }
+    h->launches++;
+    CK(cudaGetLastError());
+    return DUALIP_OK;
+}
+
+int launch_finalize(dualip* h, FinalizeParams& f, cudaStream_t st) {
+    f.s_fix = h->s_fix; f.sc_fix = h->sc_fix; f.b = h->b; f.JM = h->J * h->m;
+    f.inv_scale_s = 1.0 / h->scale_s; f.inv_scale_obj = 1.0 / h->scale_obj; f.inv_scale_sq = 1.0 / h->scale_sq;
+    k_finalize<<<1, kFinalizeThreads, 0, st>>>(f);
+    h->launches++;
+    CK(cudaGetLastError());
+    return DUALIP_OK;
+}
+
+int ensure_x_stage(dualip* h) {
+    if (!h->x_stage) return dev_alloc(h, &h->x_stage, (size_t)h->nnz);
+    return DUALIP_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+void dualip_opts_default(dualip_opts* o) {
+    if (!o) return;
+    std::memset(o, 0, sizeof(*o));
+    o->projection = DUALIP_PROJ_SIMPLEX_INEQ; o->p0 = 1.0; o->p1 = 0.0;
+    o->reduction = DUALIP_RED_AUTO; o->borrow = 0; o->validate = 1; o->momentum = 1;
+}
+
+const char* dualip_strerror(int code) {
+    switch (code) {
+        case DUALIP_OK: return "ok";
+        case DUALIP_EINVAL: return "invalid argument";
+        case DUALIP_ERANGE: return "row_ptr not monotone or item index out of range";
+        case DUALIP_EDUP: return "duplicate item within a user's row";
+        case DUALIP_ENOMEM: return "out of memory";
+        case DUALIP_ECUDA: return "CUDA runtime error";
+        case DUALIP_EUNSUPPORTED: return "unsupported configuration";
+        default: return "unknown error code";
+    }
+}
+
+void dualip_destroy(dualip_t* h) {
+    if (!h) return;
+    if (h->own_rows) { cudaFree((void*)h->row_ptr); cudaFree((void*)h->idx); cudaFree((void*)h->a); }
+    if (h->own_c) cudaFree((void*)h->c);
+    cudaFree(h->b); cudaFree(h->s_fix); cudaFree(h->lam_cur); cudaFree(h->y); cudaFree(h->lam_stage);
+    cudaFree(h->grad_stage); cudaFree(h->scalars_dev); cudaFree(h->x_stage);
+    cudaGetLastError();
+    delete h;
+}
+
+int dualip_create(dualip_t** out, int64_t I, int32_t J, int32_t m, const int64_t* row_ptr, const int32_t* item_idx,
+                  const float* c, const float* a, const float* b, const dualip_opts* opts_in, void* stream) {
+    if (!out) return DUALIP_EINVAL;
+    *out = nullptr;
+    if (I < 0 || J < 1 || m < 1 || m > 4 || !row_ptr || !b) return DUALIP_EINVAL;
+    if ((long long)J * m > (1ll << 30)) return DUALIP_EINVAL;
+    dualip_opts o;
+    if (opts_in) o = *opts_in; else dualip_opts_default(&o);
+    for (int r = 0; r < 5; ++r) if (o.reserved[r] != 0) return DUALIP_EINVAL;
+    switch (o.projection) {
+        case DUALIP_PROJ_SIMPLEX_INEQ: case DUALIP_PROJ_SIMPLEX_EQ: if (!(o.p0 > 0.0)) return DUALIP_EINVAL; break;
+        case DUALIP_PROJ_BOX: if (!(o.p0 <= o.p1)) return DUALIP_EINVAL; break;
+        case DUALIP_PROJ_BOXCUT: if (!(o.p0 > 0.0) || !(o.p1 > 0.0)) return DUALIP_EINVAL; break;
+        default: return DUALIP_EINVAL;
+    }
+    if (o.reduction < DUALIP_RED_AUTO || o.reduction > DUALIP_RED_CSC) return DUALIP_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return DUALIP_ECUDA; }
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+
+    // nnz = row_ptr[I]; row_ptr[0] must be 0
+    long long ends[2] = {0, 0};
+    const bool rp_dev = is_device_ptr(row_ptr);
+    if (rp_dev) {
+        CK(cudaMemcpyAsync(&ends[0], row_ptr, 8, cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync(&ends[1], row_ptr + I, 8, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+    } else { ends[0] = row_ptr[0]; ends[1] = row_ptr[I]; }
+    if (ends[0] != 0 || ends[1] < 0) return DUALIP_ERANGE;
+    const long long nnz = ends[1];
+    if (nnz > 0 && (!item_idx || !c || !a)) return DUALIP_EINVAL;
+
+    dualip* h = new (std::nothrow) dualip();
+    if (!h) return DUALIP_ENOMEM;
+    h->I = I; h->nnz = nnz; h->J = J; h->m = m; h->opts = o;
+    int dev = 0;
+    int rc = DUALIP_OK;
+#define FAIL(code) do { rc = (code); goto fail; } while (0)
+#define CKF(call) do { if ((call) != cudaSuccess) { cudaGetLastError(); FAIL(DUALIP_ECUDA); } } while (0)
+    {
+        CKF(cudaGetDevice(&dev));
+        CKF(cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev));
+        const bool all_dev = rp_dev && (nnz == 0 || (is_device_ptr(item_idx) && is_device_ptr(c) && is_device_ptr(a)));
+        if (o.borrow && all_dev) {
+            h->row_ptr = reinterpret_cast<const long long*>(row_ptr); h->idx = item_idx; h->c = c; h->a = a;
+        } else {
+            long long* d_rp = nullptr; int* d_idx = nullptr; float* d_c = nullptr; float* d_a = nullptr;
+            h->own_rows = true; h->own_c = true;
+            if ((rc = dev_alloc(h, &d_rp, (size_t)I + 1)) != 0) goto fail;
+            h->row_ptr = d_rp;
+            if ((rc = dev_alloc(h, &d_idx, (size_t)nnz)) != 0) goto fail;
+            h->idx = d_idx;
+            if ((rc = dev_alloc(h, &d_c, (size_t)nnz)) != 0) goto fail;
+            h->c = d_c;
+            if ((rc = dev_alloc(h, &d_a, (size_t)nnz * m)) != 0) goto fail;
+            h->a = d_a;
+            CKF(cudaMemcpyAsync(d_rp, row_ptr, ((size_t)I + 1) * 8, cudaMemcpyDefault, st));
+            if (nnz > 0) {
+                CKF(cudaMemcpyAsync(d_idx, item_idx, (size_t)nnz * 4, cudaMemcpyDefault, st));
+                CKF(cudaMemcpyAsync(d_c, c, (size_t)nnz * 4, cudaMemcpyDefault, st));
+                CKF(cudaMemcpyAsync(d_a, a, (size_t)nnz * m * 4, cudaMemcpyDefault, st));
+            }
+        }
+        const size_t JM = (size_t)J * m;
+        if ((rc = dev_alloc(h, &h->b, JM)) != 0) goto fail;
+        CKF(cudaMemcpyAsync(h->b, b, JM * 4, cudaMemcpyDefault, st));
+        if ((rc = dev_alloc(h, &h->s_fix, JM + 2)) != 0) goto fail;
+        h->sc_fix = h->s_fix + JM;
+        CKF(cudaMemsetAsync(h->s_fix, 0, (JM + 2) * 8, st));
+        if ((rc = dev_alloc(h, &h->lam_cur, JM)) != 0) goto fail;
+        if ((rc = dev_alloc(h, &h->y, JM)) != 0) goto fail;
+        if ((rc = dev_alloc(h, &h->lam_stage, JM)) != 0) goto fail;
+        if ((rc = dev_alloc(h, &h->grad_stage, JM)) != 0) goto fail;
+        if ((rc = dev_alloc(h, &h->scalars_dev, 5)) != 0) goto fail;
+
+        // validation (R11) and row-length statistics.  Monotone row_ptr and the maximum row length are always
+        // computed (the kernels index with them); `validate` switches the index-range / duplicate scan.
+        {
+            int* d_flags = nullptr; unsigned long long* d_maxlen = nullptr;
+            if (cudaMalloc(&d_flags, sizeof(int)) != cudaSuccess) { cudaGetLastError(); FAIL(DUALIP_ENOMEM); }
+            if (cudaMalloc(&d_maxlen, 8) != cudaSuccess) { cudaGetLastError(); cudaFree(d_flags); FAIL(DUALIP_ENOMEM); }
+            cudaMemsetAsync(d_flags, 0, sizeof(int), st); cudaMemsetAsync(d_maxlen, 0, 8, st);
+            k_validate<<<grid_for(I, 128, h->num_sms), 128, 0, st>>>(h->row_ptr, h->idx, I, J, nnz, o.validate ? 1 : 0, d_flags, d_maxlen);
+            h->launches++;
+            int flags = 0; unsigned long long maxlen = 0;
+            cudaError_t e1 = cudaMemcpyAsync(&flags, d_flags, sizeof(int), cudaMemcpyDeviceToHost, st);
+            cudaError_t e2 = cudaMemcpyAsync(&maxlen, d_maxlen, 8, cudaMemcpyDeviceToHost, st);
+            cudaError_t e3 = cudaStreamSynchronize(st);
+            cudaFree(d_flags); cudaFree(d_maxlen);
+            if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || cudaGetLastError() != cudaSuccess) FAIL(DUALIP_ECUDA);
+            if (flags & 3) FAIL(DUALIP_ERANGE);
+            if (flags & 4) FAIL(DUALIP_EDUP);
+            h->max_row_len = (long long)maxlen;
+        }
+        if ((rc = compute_stats(h, st, true, true)) != 0) goto fail;
+        set_xmax(h);
+        set_scales(h);
+        if ((rc = make_plan(h)) != 0) goto fail;
+        CKF(cudaStreamSynchronize(st));
+    }
+    *out = h;
+    return DUALIP_OK;
+fail:
+    dualip_destroy(h);
+    return rc;
+#undef FAIL
+#undef CKF
+}
+
+int dualip_get_info(const dualip_t* h, dualip_info* info) {
+    if (!h || !info) return DUALIP_EINVAL;
+    std::memset(info, 0, sizeof(*info));
+    info->I = h->I; info->nnz = h->nnz; info->J = h->J; info->m = h->m; info->L = h->L;
+    info->max_row_len = h->max_row_len;
+    info->group_lanes = h->plan.G; info->chunk_regs = h->plan.KREG;
+    info->reduction = h->plan.acc_smem ? DUALIP_RED_SMEM : DUALIP_RED_GLOBAL;
+    info->lambda_in_smem = h->plan.lam_smem ? 1 : 0;
+    info->grid_ctas = h->plan.grid; info->block_threads = kBlockThreads;
+    info->smem_bytes = (int64_t)h->plan.smem;
+    info->bytes_resident = h->bytes_resident; info->launches = h->launches;
+    info->fix_scale_s = h->scale_s;
+    return DUALIP_OK;
+}
+
+int dualip_set_c(dualip_t* h, const float* c_new, void* stream) {
+    if (!h || (!c_new && h->nnz > 0)) return DUALIP_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (h->nnz == 0) return DUALIP_OK;
+    if (h->own_c) {
+        CK(cudaMemcpyAsync((void*)h->c, c_new, (size_t)h->nnz * 4, cudaMemcpyDefault, st));
+    } else {
+        if (!is_device_ptr(c_new)) return DUALIP_EINVAL;     // borrowed rows: the new c must be device memory too
+        h->c = c_new;
+    }
+    int rc = compute_stats(h, st, false, true);
+    if (rc != 0) return rc;
+    set_scales(h);
+    return DUALIP_OK;
+}
+
+int dualip_grad(dualip_t* h, const double* lambda, double gamma, double* grad, dualip_scalars* scalars, float* x,
+                void* stream) {
+    if (!h || !lambda || !(gamma > 0.0) || !std::isfinite(gamma)) return DUALIP_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t JM = (size_t)h->J * h->m;
+    const bool lam_dev = is_device_ptr(lambda), grad_dev = is_device_ptr(grad), sc_dev = is_device_ptr(scalars),
+               x_dev = is_device_ptr(x);
+    const double* lam_d = lambda;
+    if (!lam_dev) { CK(cudaMemcpyAsync(h->lam_stage, lambda, JM * 8, cudaMemcpyHostToDevice, st)); lam_d = h->lam_stage; }
+    float* x_d = x;
+    if (x && !x_dev) { int rc = ensure_x_stage(h); if (rc != 0) return rc; x_d = h->x_stage; }
+    int rc = launch_grad(h, lam_d, gamma, x_d, st);
+    if (rc != 0) return rc;
+    FinalizeParams f{};
+    f.lam_eval = lam_d; f.gamma = gamma; f.update = 0;
+    f.grad_out = grad ? (grad_dev ? grad : h->grad_stage) : nullptr;
+    f.scalars_out = scalars ? (sc_dev ? reinterpret_cast<double*>(scalars) : h->scalars_dev) : nullptr;
+    rc = launch_finalize(h, f, st);
+    if (rc != 0) return rc;
+    bool sync = !lam_dev;
+    if (grad && !grad_dev) { CK(cudaMemcpyAsync(grad, h->grad_stage, JM * 8, cudaMemcpyDeviceToHost, st)); sync = true; }
+    if (scalars && !sc_dev) { CK(cudaMemcpyAsync(scalars, h->scalars_dev, 5 * 8, cudaMemcpyDeviceToHost, st)); sync = true; }
+    if (x && !x_dev && h->nnz > 0) { CK(cudaMemcpyAsync(x, h->x_stage, (size_t)h->nnz * 4, cudaMemcpyDeviceToHost, st)); sync = true; }
+    if (sync) CK(cudaStreamSynchronize(st));
+    return DUALIP_OK;
+}
+
+int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int32_t* iters, double* lambda_inout,
+                 float* x_out, dualip_scalars* final_scalars, double* final_grad, const dualip_trace* trace, void* stream) {
+    if (!h || n_stages < 0 || !lambda_inout) return DUALIP_EINVAL;
+    if (n_stages > 0 && (!gammas || !iters)) return DUALIP_EINVAL;
+    long long total = 0;
+    for (int s = 0; s < n_stages; ++s) {
+        if (!(gammas[s] > 0.0) || !std::isfinite(gammas[s]) || iters[s] < 0) return DUALIP_EINVAL;
+        total += iters[s];
+    }
+    if (trace && trace->capacity < total) return DUALIP_EINVAL;
+    if (n_stages == 0) return DUALIP_OK;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t JM = (size_t)h->J * h->m;
+    const bool lam_dev = is_device_ptr(lambda_inout), grad_dev = is_device_ptr(final_grad),
+               sc_dev = is_device_ptr(final_scalars), x_dev = is_device_ptr(x_out);
+    CK(cudaMemcpyAsync(h->lam_cur, lambda_inout, JM * 8, cudaMemcpyDefault, st));
+    const double L = h->L > 0.0 ? h->L : 1.0;
+    long long n = 0;
+    for (int s = 0; s < n_stages; ++s) {
+        const double gamma = gammas[s], eta = gamma / L;
+        CK(cudaMemcpyAsync(h->y, h->lam_cur, JM * 8, cudaMemcpyDeviceToDevice, st));   // warm start, momentum restart (R4)
+        for (int t = 0; t < iters[s]; ++t, ++n) {
+            int rc = launch_grad(h, h->y, gamma, nullptr, st);
+            if (rc != 0) return rc;
+            FinalizeParams f{};
+            f.lam_eval = h->y; f.gamma = gamma; f.update = 1; f.eta = eta;
+            f.beta = h->opts.momentum ? (double)t / (double)(t + 3) : 0.0;
+            f.lam_cur = h->lam_cur; f.y = h->y;
+            if (trace) { f.tr_g = trace->g; f.tr_rinf = trace->r_inf; f.tr_r2 = trace->r_2; f.tr_grad = trace->grad; f.tr_lam = trace->lambda; f.tr_n = n; }
+            rc = launch_finalize(h, f, st);
+            if (rc != 0) return rc;
+        }
+    }
+    // final evaluation at lambda_T (R3)
+    {
+        float* x_d = x_out;
+        if (x_out && !x_dev) { int rc = ensure_x_stage(h); if (rc != 0) return rc; x_d = h->x_stage; }
+        int rc = launch_grad(h, h->lam_cur, gammas[n_stages - 1], x_d, st);
+        if (rc != 0) return rc;
+        FinalizeParams f{};
+        f.lam_eval = h->lam_cur; f.gamma = gammas[n_stages - 1]; f.update = 0;
+        f.grad_out = final_grad ? (grad_dev ? final_grad : h->grad_stage) : nullptr;
+        f.scalars_out = final_scalars ? (sc_dev ? reinterpret_cast<double*>(final_scalars) : h->scalars_dev) : nullptr;
+        rc = launch_finalize(h, f, st);
+        if (rc != 0) return rc;
+    }
+    bool sync = false;
+    CK(cudaMemcpyAsync(lambda_inout, h->lam_cur, JM * 8, cudaMemcpyDefault, st));
+    if (!lam_dev) sync = true;
+    if (final_grad && !grad_dev) { CK(cudaMemcpyAsync(final_grad, h->grad_stage, JM * 8, cudaMemcpyDeviceToHost, st)); sync = true; }
+    if (final_scalars && !sc_dev) { CK(cudaMemcpyAsync(final_scalars, h->scalars_dev, 5 * 8, cudaMemcpyDeviceToHost, st)); sync = true; }
+    if (x_out && !x_dev && h->nnz > 0) { CK(cudaMemcpyAsync(x_out, h->x_stage, (size_t)h->nnz * 4, cudaMemcpyDeviceToHost, st)); sync = true; }
+    if (sync) CK(cudaStreamSynchronize(st));
+    return DUALIP_OK;
+}
+
+}  // extern "C"

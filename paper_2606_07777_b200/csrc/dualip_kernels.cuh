@@ -1,0 +1,630 @@
+// dualip_kernels.cuh -- device code of the dual-gradient hot path (sm_100a).
+//
+// Steps a1-a6 of SURVEY.md section 8(a); equations cited as P:n (paper line) and R<n> (DESIGN.md readings).
+//   k_grad      a1 gather lambda, a2 w = -(c + sum_k a^k lambda_jk), a3 projection, a4 item reduction,
+//               a5 per-lane partial scalars, a8 optional x                         (Eq. 3-4)
+//   k_grad_box  the same for the element-wise box projection (no row coupling)
+//   k_finalize  a4 grad = s - b, a5 g / r_inf / r_2, a6 AGD update + lambda >= 0 projection (R1)
+//   k_validate, k_absmax, k_col_stats, k_reduce_stats      a0 create-time checks and constants (R2, R11)
+//
+// Numerics: lambda fp64; w by fp64 FMA from fp32 data; row maximum taken on RN_f32(w);
+// u = RN_f32((w - m)/gamma) with the subtraction exact in fp64, so every quantity after the shift is O(1)
+// and fp32 is accurate to ~1e-7 absolute whatever 1/gamma is.  The inequality branch (R5) is folded in as
+// tau = max(theta_eq, -m/gamma):  x = max(u - tau, 0).
+//
+// Item reduction: 64-bit fixed point.  Shared-memory accumulators are two 32-bit words with an explicit carry,
+// because ATOMS.ADD (32-bit integer) is the only native shared-memory add on sm_100a; global accumulation is
+// RED.ADD.64.  Integer addition commutes, so results are bit-reproducible for any launch geometry.
+#pragma once
+#include <cuda_runtime.h>
+#include <math_constants.h>
+#include <stdint.h>
+
+namespace dualip_dev {
+
+constexpr int kBlockThreads = 512;
+constexpr int kWarpsPerBlock = kBlockThreads / 32;
+constexpr unsigned kFull = 0xffffffffu;
+
+enum : int { PROJ_SIMPLEX_INEQ = 0, PROJ_BOX = 1, PROJ_BOXCUT = 2, PROJ_SIMPLEX_EQ = 3 };
+
+struct GradParams {
+    const long long* __restrict__ row_ptr;
+    const int* __restrict__ idx;
+    const float* __restrict__ c;
+    const float* __restrict__ a;
+    const double* __restrict__ lambda;
+    unsigned long long* s_fix;   // [J*m] item accumulators, fixed point, zero on entry
+    unsigned long long* sc_fix;  // [2]   obj = c'x and |x|^2, fixed point, zero on entry
+    float* x;                    // [nnz] or nullptr
+    long long I;
+    long long nnz;
+    int J, m;
+    int proj;
+    int general_boxcut;          // BOXCUT with ub < z: needs the capped threshold search
+    float inv_gamma_f;
+    float z;                     // simplex / box-cut budget
+    float ub;                    // box-cut cap
+    double inv_gamma;
+    double box_lo, box_hi;
+    double scale_s, scale_obj, scale_sq;
+};
+
+__device__ __forceinline__ long long to_fix(float v, double scale) { return __double2ll_rn((double)v * scale); }
+
+__device__ __forceinline__ void fix_add_smem(unsigned* lo, unsigned* hi, long long v) {
+    const unsigned vlo = (unsigned)(unsigned long long)v;
+    const unsigned vhi = (unsigned)((unsigned long long)v >> 32);
+    const unsigned old = atomicAdd(lo, vlo);
+    const unsigned h = vhi + ((unsigned)(old + vlo) < vlo ? 1u : 0u);
+    if (h) atomicAdd(hi, h);
+}
+
+template <int G>
+__device__ __forceinline__ float group_max(float v) {
+#pragma unroll
+    for (int o = G / 2; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(kFull, v, o));
+    return v;
+}
+template <int G>
+__device__ __forceinline__ float group_sum(float v) {
+#pragma unroll
+    for (int o = G / 2; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+    return v;
+}
+template <int G>
+__device__ __forceinline__ int group_sum_i(int v) {
+#pragma unroll
+    for (int o = G / 2; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+    return v;
+}
+
+// One nonzero: returns t = c + sum_k a_k * lambda[j,k] in fp64 (w = -t), and the row data it read.
+template <int M, bool LAM_SMEM>
+__device__ __forceinline__ double eval_t(const GradParams& p, const double* s_lam, long long q, int mm,
+                                         int& j, float& cc, float (&aa)[M > 0 ? M : 4]) {
+    j = __ldg(p.idx + q);
+    cc = __ldg(p.c + q);
+    double t = (double)cc;
+    if (M > 0) {
+#pragma unroll
+        for (int k = 0; k < M; ++k) aa[k] = __ldg(p.a + q * M + k);
+#pragma unroll
+        for (int k = 0; k < M; ++k) {
+            const double l = LAM_SMEM ? s_lam[j * M + k] : __ldg(p.lambda + (long long)j * M + k);
+            t = fma((double)aa[k], l, t);
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            aa[k] = 0.0f;
+            if (k < mm) {
+                aa[k] = __ldg(p.a + q * mm + k);
+                const double l = LAM_SMEM ? s_lam[j * mm + k] : __ldg(p.lambda + (long long)j * mm + k);
+                t = fma((double)aa[k], l, t);
+            }
+        }
+    }
+    return t;
+}
+
+// a4 + a5 for one nonzero with x > 0.
+template <int M, bool ACC_SMEM>
+__device__ __forceinline__ void contribute(const GradParams& p, unsigned* s_lo, unsigned* s_hi, int mm, int j,
+                                           const float (&aa)[M > 0 ? M : 4], float x) {
+    const int nm = M > 0 ? M : mm;
+#pragma unroll
+    for (int k = 0; k < (M > 0 ? M : 4); ++k) {
+        if (k < nm) {
+            const long long f = to_fix(aa[k] * x, p.scale_s);
+            if (ACC_SMEM) fix_add_smem(s_lo + j * nm + k, s_hi + j * nm + k, f);
+            else atomicAdd(p.s_fix + (long long)j * nm + k, (unsigned long long)f);
+        }
+    }
+}
+
+// Whole-warp path for rows longer than the register budget: every pass re-reads the row (L1/L2 resident).
+template <int M, bool LAM_SMEM, bool ACC_SMEM>
+__device__ __noinline__ void long_row(const GradParams& p, const double* s_lam, unsigned* s_lo, unsigned* s_hi,
+                                      long long beg, long long end, float& obj_l, float& sq_l) {
+    const int lane = threadIdx.x & 31;
+    const int mm = p.m;
+    int j; float cc; float aa[M > 0 ? M : 4];
+    float wmax = -CUDART_INF_F;
+    for (long long q = beg + lane; q < end; q += 32)
+        wmax = fmaxf(wmax, (float)(-eval_t<M, LAM_SMEM>(p, s_lam, q, mm, j, cc, aa)));
+    const float m32 = group_max<32>(wmax);
+    const bool ineq = p.proj != PROJ_SIMPLEX_EQ;
+    if (ineq && !(m32 > 0.0f)) {
+        if (p.x) for (long long q = beg + lane; q < end; q += 32) p.x[q] = 0.0f;
+        return;
+    }
+    const double md = (double)m32;
+    const float mv = m32 * p.inv_gamma_f, z = p.z;
+    float tau;
+    double ref = 0.0;                                  // box-cut: reference point (in v units) u is taken relative to
+    if (!p.general_boxcut) {
+        float theta = -z - (1.2e-7f * fabsf(mv) + 1e-6f);
+        int n_prev = -1;
+        for (;;) {
+            float s = 0.0f; int n = 0;
+            for (long long q = beg + lane; q < end; q += 32) {
+                const float u = (float)(-eval_t<M, LAM_SMEM>(p, s_lam, q, mm, j, cc, aa) - md) * p.inv_gamma_f;
+                if (u > theta) { s += u; ++n; }
+            }
+            s = group_sum<32>(s); n = group_sum_i<32>(n);
+            if (n == n_prev || n == 0) break;
+            theta = fmaxf((s - z) / (float)n, theta);
+            n_prev = n;
+        }
+        tau = ineq ? fmaxf(theta, -mv) : theta;
+    } else {
+        // same three steps as the register path (see there), re-reading the row on every pass
+        const float ub = p.ub;
+        const double ig = p.inv_gamma;
+        float s0 = 0.0f;
+        for (long long q = beg + lane; q < end; q += 32)
+            s0 += fminf(fmaxf((float)(-eval_t<M, LAM_SMEM>(p, s_lam, q, mm, j, cc, aa) * ig), 0.0f), ub);
+        s0 = group_sum<32>(s0);
+        if (s0 <= z) { ref = 0.0; tau = 0.0f; }
+        else {
+            float lo = -mv, hi = 1.2e-7f * fabsf(mv) + 1e-6f;
+            for (int it = 0; it < 36; ++it) {
+                const float mid = 0.5f * (lo + hi);
+                float s = 0.0f;
+                for (long long q = beg + lane; q < end; q += 32) {
+                    const float u = (float)(-eval_t<M, LAM_SMEM>(p, s_lam, q, mm, j, cc, aa) - md) * p.inv_gamma_f;
+                    s += fminf(fmaxf(u - mid, 0.0f), ub);
+                }
+                s = group_sum<32>(s);
+                if (s > z) lo = mid; else hi = mid;
+            }
+            const float tc = 0.5f * (lo + hi);
+            const float eps = (hi - lo) + 1e-6f + 4.8e-7f * fabsf(tc);
+            ref = md * ig + (double)tc;
+            float dlo = -eps, dhi = eps;
+            for (int it = 0; it < 26; ++it) {
+                const float mid = 0.5f * (dlo + dhi);
+                float s = 0.0f;
+                for (long long q = beg + lane; q < end; q += 32) {
+                    const float u = (float)(-eval_t<M, LAM_SMEM>(p, s_lam, q, mm, j, cc, aa) * ig - ref);
+                    s += fminf(fmaxf(u - mid, 0.0f), ub);
+                }
+                s = group_sum<32>(s);
+                if (s > z) dlo = mid; else dhi = mid;
+            }
+            const float mid = 0.5f * (dlo + dhi);
+            float sF = 0.0f; int nF = 0, nU = 0;
+            for (long long q = beg + lane; q < end; q += 32) {
+                const float u = (float)(-eval_t<M, LAM_SMEM>(p, s_lam, q, mm, j, cc, aa) * ig - ref);
+                const float d = u - mid;
+                if (d >= ub) ++nU; else if (d > 0.0f) { sF += u; ++nF; }
+            }
+            sF = group_sum<32>(sF); nF = group_sum_i<32>(nF); nU = group_sum_i<32>(nU);
+            tau = mid;
+            if (nF > 0) {
+                const float pol = (sF + (float)nU * ub - z) / (float)nF;
+                if (pol >= dlo && pol <= dhi) tau = pol;
+            }
+        }
+    }
+    const float cap = p.general_boxcut ? p.ub : CUDART_INF_F;
+    for (long long q = beg + lane; q < end; q += 32) {
+        const double tq = eval_t<M, LAM_SMEM>(p, s_lam, q, mm, j, cc, aa);
+        const float u = p.general_boxcut ? (float)(-tq * p.inv_gamma - ref) : (float)(-tq - md) * p.inv_gamma_f;
+        const float x = fminf(fmaxf(u - tau, 0.0f), cap);
+        if (p.x) p.x[q] = x;
+        if (x > 0.0f) {
+            obj_l = fmaf(cc, x, obj_l);
+            sq_l = fmaf(x, x, sq_l);
+            contribute<M, ACC_SMEM>(p, s_lo, s_hi, mm, j, aa, x);
+        }
+    }
+}
+
+// The fused per-user gradient kernel.  G lanes own one row; rows of up to G*KREG nonzeros live in registers.
+template <int G, int KREG, int M, bool LAM_SMEM, bool ACC_SMEM>
+__global__ void __launch_bounds__(kBlockThreads, 1) k_grad(const GradParams p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int MA = M > 0 ? M : 4;
+    const int mm = M > 0 ? M : p.m;
+    const int JM = p.J * mm;
+    double* s_lam = reinterpret_cast<double*>(smem_raw);
+    unsigned* s_lo = reinterpret_cast<unsigned*>(smem_raw + (LAM_SMEM ? (size_t)JM * 8 : 0));
+    unsigned* s_hi = s_lo + JM;
+    if (LAM_SMEM) for (int q = threadIdx.x; q < JM; q += kBlockThreads) s_lam[q] = p.lambda[q];
+    if (ACC_SMEM) for (int q = threadIdx.x; q < 2 * JM; q += kBlockThreads) s_lo[q] = 0u;
+    __syncthreads();
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    constexpr int RPW = 32 / G;
+    const int gl = lane & (G - 1), grp = lane / G;
+    const unsigned gmask = G == 32 ? kFull : (((1u << G) - 1u) << (lane & ~(G - 1)));
+    const long long nsteps = (p.I + RPW - 1) / RPW;
+    const bool ineq = p.proj != PROJ_SIMPLEX_EQ;
+    const float z = p.z;
+    float obj_l = 0.0f, sq_l = 0.0f;
+
+    for (long long step = (long long)blockIdx.x * kWarpsPerBlock + warp; step < nsteps;
+         step += (long long)gridDim.x * kWarpsPerBlock) {
+        const long long row = step * RPW + grp;
+        long long beg = 0, end = 0;
+        if (row < p.I) { beg = __ldg(p.row_ptr + row); end = __ldg(p.row_ptr + row + 1); }
+        const long long len = end - beg;
+        const bool is_long = len > (long long)G * KREG;
+        const int flen = is_long ? 0 : (int)len;
+        int nch_max = (flen + G - 1) / G;
+#pragma unroll
+        for (int o = G; o < 32; o <<= 1) nch_max = max(nch_max, __shfl_xor_sync(kFull, nch_max, o));
+
+        if (nch_max > 0) {
+            int jj[KREG]; float cc[KREG]; float aa[KREG][MA]; double t[KREG];
+            // loads first (independent, so they overlap), then the lambda gather and the fp64 FMA
+#pragma unroll
+            for (int k = 0; k < KREG; ++k) {
+                if (k >= nch_max) break;
+                const int e = k * G + gl;
+                jj[k] = 0; cc[k] = 0.0f;
+#pragma unroll
+                for (int f = 0; f < MA; ++f) aa[k][f] = 0.0f;
+                if (e < flen) {
+                    const long long q = beg + e;
+                    jj[k] = __ldg(p.idx + q);
+                    cc[k] = __ldg(p.c + q);
+                    if (M > 0) {
+#pragma unroll
+                        for (int f = 0; f < MA; ++f) aa[k][f] = __ldg(p.a + q * M + f);
+                    } else {
+#pragma unroll
+                        for (int f = 0; f < MA; ++f) if (f < mm) aa[k][f] = __ldg(p.a + q * mm + f);
+                    }
+                }
+            }
+            float wmax = -CUDART_INF_F;
+#pragma unroll
+            for (int k = 0; k < KREG; ++k) {
+                if (k >= nch_max) break;
+                double tk = CUDART_INF;
+                if (k * G + gl < flen) {
+                    tk = (double)cc[k];
+#pragma unroll
+                    for (int f = 0; f < MA; ++f) {
+                        if (f < mm) {
+                            const double l = LAM_SMEM ? s_lam[jj[k] * mm + f] : __ldg(p.lambda + (long long)jj[k] * mm + f);
+                            tk = fma((double)aa[k][f], l, tk);
+                        }
+                    }
+                    wmax = fmaxf(wmax, (float)(-tk));
+                }
+                t[k] = tk;
+            }
+            const float gm = group_max<G>(wmax);                      // full-mask shuffles: every lane takes part
+            const float m32 = flen > 0 ? gm : 0.0f;
+            const bool alive = flen > 0 && (!ineq || m32 > 0.0f);
+            const double md = (double)m32;
+            const float mv = m32 * p.inv_gamma_f;
+            const float cut = alive ? -z - (1.2e-7f * fabsf(mv) + 1e-6f) : CUDART_INF_F;
+
+            float u[KREG];
+            int cnt = 0;
+#pragma unroll
+            for (int k = 0; k < KREG; ++k) {
+                if (k >= nch_max) break;
+                u[k] = (float)(-t[k] - md) * p.inv_gamma_f;          // -inf on padding lanes
+                cnt += __popc(__ballot_sync(kFull, u[k] > cut) & gmask);
+            }
+
+            float tau = CUDART_INF_F;
+            bool vertex = false;
+            if (!p.general_boxcut) {
+                vertex = __all_sync(kFull, cnt <= 1);
+                if (!vertex) {
+                    // Michelot fixed point on the equality problem; theta only grows, the support only shrinks
+                    float theta = cut;
+                    int n_prev = cnt;
+                    for (;;) {
+                        float s = 0.0f;
+#pragma unroll
+                        for (int k = 0; k < KREG; ++k) { if (k >= nch_max) break; s += (u[k] > theta) ? u[k] : 0.0f; }
+                        s = group_sum<G>(s);
+                        // max(): theta is non-decreasing in exact arithmetic; enforcing it makes termination unconditional
+                        const float th_new = n_prev > 0 ? fmaxf((s - z) / (float)n_prev, theta) : CUDART_INF_F;
+                        int n = 0;
+#pragma unroll
+                        for (int k = 0; k < KREG; ++k) {
+                            if (k >= nch_max) break;
+                            n += __popc(__ballot_sync(kFull, u[k] > th_new) & gmask);
+                        }
+                        const bool changed = n != n_prev;
+                        theta = th_new; n_prev = n;
+                        if (!__any_sync(kFull, changed)) break;
+                    }
+                    tau = ineq ? fmaxf(theta, -mv) : theta;
+                }
+            } else if (__any_sync(kFull, alive)) {
+                // box-cut with ub < z.  Free entries can sit far below the row maximum, where u (relative to the
+                // maximum) has lost absolute precision in fp32; so (1) test slackness on v itself, (2) bracket
+                // tau by bisection on u, (3) re-centre on the coarse tau in fp64 and solve the linear piece there.
+                const float ub = p.ub;
+                const double ig = p.inv_gamma;
+                float s0 = 0.0f;
+#pragma unroll
+                for (int k = 0; k < KREG; ++k) { if (k >= nch_max) break; s0 += fminf(fmaxf((float)(-t[k] * ig), 0.0f), ub); }
+                s0 = group_sum<G>(s0);
+                const bool slack = !alive || s0 <= z;
+                float td = 0.0f;
+                if (!__all_sync(kFull, slack)) {
+                    float lo = alive ? -mv : 0.0f, hi = alive ? 1.2e-7f * fabsf(mv) + 1e-6f : 0.0f;
+                    for (int it = 0; it < 36; ++it) {
+                        const float mid = 0.5f * (lo + hi);
+                        float sm = 0.0f;
+#pragma unroll
+                        for (int k = 0; k < KREG; ++k) { if (k >= nch_max) break; sm += fminf(fmaxf(u[k] - mid, 0.0f), ub); }
+                        sm = group_sum<G>(sm);
+                        if (sm > z) lo = mid; else hi = mid;
+                    }
+                    const float tc = 0.5f * (lo + hi);
+                    const float eps = (hi - lo) + 1e-6f + 4.8e-7f * fabsf(tc);
+                    if (!slack) {
+#pragma unroll
+                        for (int k = 0; k < KREG; ++k) { if (k >= nch_max) break; u[k] = (float)((-t[k] - md) * ig - (double)tc); }
+                    }
+                    float dlo = -eps, dhi = eps;
+                    for (int it = 0; it < 26; ++it) {
+                        const float mid = 0.5f * (dlo + dhi);
+                        float sm = 0.0f;
+#pragma unroll
+                        for (int k = 0; k < KREG; ++k) { if (k >= nch_max) break; sm += fminf(fmaxf(u[k] - mid, 0.0f), ub); }
+                        sm = group_sum<G>(sm);
+                        if (sm > z) dlo = mid; else dhi = mid;
+                    }
+                    const float mid = 0.5f * (dlo + dhi);
+                    float sF = 0.0f; int nF = 0, nU = 0;
+#pragma unroll
+                    for (int k = 0; k < KREG; ++k) {
+                        if (k >= nch_max) break;
+                        const float d = u[k] - mid;
+                        if (d >= ub) ++nU; else if (d > 0.0f) { sF += u[k]; ++nF; }
+                    }
+                    sF = group_sum<G>(sF); nF = group_sum_i<G>(nF); nU = group_sum_i<G>(nU);
+                    td = mid;
+                    if (nF > 0) {
+                        const float pol = (sF + (float)nU * ub - z) / (float)nF;
+                        if (pol >= dlo && pol <= dhi) td = pol;
+                    }
+                }
+                if (slack) {
+#pragma unroll
+                    for (int k = 0; k < KREG; ++k) { if (k >= nch_max) break; u[k] = (float)(-t[k] * ig); }
+                    td = 0.0f;
+                }
+                tau = alive ? td : CUDART_INF_F;
+            }
+            const float cap = p.general_boxcut ? p.ub : CUDART_INF_F;
+#pragma unroll
+            for (int k = 0; k < KREG; ++k) {
+                if (k >= nch_max) break;
+                float x;
+                if (vertex) x = (u[k] > cut) ? (ineq ? fminf(z, u[k] + mv) : z) : 0.0f;
+                else x = fminf(fmaxf(u[k] - tau, 0.0f), cap);
+                const int e = k * G + gl;
+                if (p.x && e < flen) p.x[beg + e] = x;
+                if (x > 0.0f) {
+                    obj_l = fmaf(cc[k], x, obj_l);
+                    sq_l = fmaf(x, x, sq_l);
+                    contribute<M, ACC_SMEM>(p, s_lo, s_hi, mm, jj[k], aa[k], x);
+                }
+            }
+        }
+        // rows beyond the register budget: the whole warp takes them one at a time
+        unsigned long_mask = __ballot_sync(kFull, is_long && gl == 0);
+        while (long_mask) {
+            const int src = __ffs(long_mask) - 1;
+            long_mask &= long_mask - 1;
+            const long long b = __shfl_sync(kFull, beg, src), e = __shfl_sync(kFull, end, src);
+            long_row<M, LAM_SMEM, ACC_SMEM>(p, s_lam, s_lo, s_hi, b, e, obj_l, sq_l);
+        }
+    }
+
+    // a5: per-lane fp32 partials -> fixed point (lane order is fixed by the static row assignment)
+    {
+        const long long fo = __double2ll_rn((double)obj_l * p.scale_obj);
+        const long long fs = __double2ll_rn((double)sq_l * p.scale_sq);
+        long long so = fo, ss = fs;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) { so += __shfl_xor_sync(kFull, so, o); ss += __shfl_xor_sync(kFull, ss, o); }
+        if (lane == 0) {
+            if (so) atomicAdd(p.sc_fix + 0, (unsigned long long)so);
+            if (ss) atomicAdd(p.sc_fix + 1, (unsigned long long)ss);
+        }
+    }
+    if (ACC_SMEM) {
+        __syncthreads();
+        for (int q = threadIdx.x; q < JM; q += kBlockThreads) {
+            const unsigned long long v = ((unsigned long long)s_hi[q] << 32) | s_lo[q];
+            if (v) atomicAdd(p.s_fix + q, v);
+        }
+    }
+}
+
+// Box projection {lo <= x <= hi}: element-wise, so one thread per nonzero with fully coalesced streams.
+template <int M>
+__global__ void __launch_bounds__(256) k_grad_box(const GradParams p) {
+    const int mm = M > 0 ? M : p.m;
+    float obj_l = 0.0f, sq_l = 0.0f;
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < p.nnz; q += (long long)gridDim.x * blockDim.x) {
+        int j; float cc; float aa[M > 0 ? M : 4];
+        const double t = eval_t<M, false>(p, nullptr, q, mm, j, cc, aa);
+        const double v = -t * p.inv_gamma;
+        const float x = (float)fmin(fmax(v, p.box_lo), p.box_hi);
+        if (p.x) p.x[q] = x;
+        if (x != 0.0f) {
+            obj_l = fmaf(cc, x, obj_l);
+            sq_l = fmaf(x, x, sq_l);
+            contribute<M, false>(p, nullptr, nullptr, mm, j, aa, x);
+        }
+    }
+    long long so = __double2ll_rn((double)obj_l * p.scale_obj), ss = __double2ll_rn((double)sq_l * p.scale_sq);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { so += __shfl_xor_sync(kFull, so, o); ss += __shfl_xor_sync(kFull, ss, o); }
+    if ((threadIdx.x & 31) == 0) {
+        if (so) atomicAdd(p.sc_fix + 0, (unsigned long long)so);
+        if (ss) atomicAdd(p.sc_fix + 1, (unsigned long long)ss);
+    }
+}
+
+struct FinalizeParams {
+    unsigned long long* s_fix;
+    unsigned long long* sc_fix;
+    const float* __restrict__ b;
+    const double* lam_eval;     // point the gradient was taken at
+    double* grad_out;           // nullable
+    double* scalars_out;        // nullable, 5 doubles {g, obj, reg, r_inf, r_2}
+    int JM;
+    double inv_scale_s, inv_scale_obj, inv_scale_sq;
+    double gamma;
+    int update;                 // a6 on/off
+    double eta, beta;
+    double* lam_cur;            // lambda_t -> lambda_{t+1}
+    double* y;                  // y_t -> y_{t+1} (== lam_eval when update)
+    double* tr_g; double* tr_rinf; double* tr_r2; double* tr_grad; double* tr_lam;   // trace columns (nullable)
+    long long tr_n;
+};
+
+constexpr int kFinalizeThreads = 1024;
+
+// a4 (grad = s - b), a5 (scalars), a6 (AGD step, R1) on the J*m vector; re-zeroes the accumulators.
+__global__ void __launch_bounds__(kFinalizeThreads) k_finalize(const FinalizeParams p) {
+    __shared__ double sh_dot[32], sh_r2[32], sh_inf[32];
+    double dot = 0.0, r2 = 0.0, rinf = 0.0;
+    for (int q = threadIdx.x; q < p.JM; q += kFinalizeThreads) {
+        const double s = (double)(long long)p.s_fix[q] * p.inv_scale_s;
+        p.s_fix[q] = 0ull;
+        const double g = s - (double)p.b[q];
+        const double le = p.lam_eval[q];
+        dot = fma(le, g, dot);
+        if (g > 0.0) { r2 = fma(g, g, r2); rinf = fmax(rinf, g); }
+        if (p.grad_out) p.grad_out[q] = g;
+        if (p.tr_grad) p.tr_grad[p.tr_n * p.JM + q] = g;
+        if (p.update) {
+            const double ln = fmax(0.0, le + p.eta * g);
+            const double lo = p.lam_cur[q];
+            p.lam_cur[q] = ln;
+            p.y[q] = ln + p.beta * (ln - lo);
+            if (p.tr_lam) p.tr_lam[p.tr_n * p.JM + q] = ln;
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        dot += __shfl_xor_sync(kFull, dot, o);
+        r2 += __shfl_xor_sync(kFull, r2, o);
+        rinf = fmax(rinf, __shfl_xor_sync(kFull, rinf, o));
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane == 0) { sh_dot[warp] = dot; sh_r2[warp] = r2; sh_inf[warp] = rinf; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        dot = 0.0; r2 = 0.0; rinf = 0.0;
+        for (int w = 0; w < kFinalizeThreads / 32; ++w) { dot += sh_dot[w]; r2 += sh_r2[w]; rinf = fmax(rinf, sh_inf[w]); }
+        const double obj = (double)(long long)p.sc_fix[0] * p.inv_scale_obj;
+        const double reg = 0.5 * p.gamma * ((double)(long long)p.sc_fix[1] * p.inv_scale_sq);
+        p.sc_fix[0] = 0ull; p.sc_fix[1] = 0ull;
+        const double g = obj + reg + dot;
+        const double nr2 = sqrt(r2);
+        if (p.scalars_out) { p.scalars_out[0] = g; p.scalars_out[1] = obj; p.scalars_out[2] = reg; p.scalars_out[3] = rinf; p.scalars_out[4] = nr2; }
+        if (p.tr_g) p.tr_g[p.tr_n] = g;
+        if (p.tr_rinf) p.tr_rinf[p.tr_n] = rinf;
+        if (p.tr_r2) p.tr_r2[p.tr_n] = nr2;
+    }
+}
+
+// ---- a0: create-time kernels -------------------------------------------------------------------------------
+
+// flags: bit0 row_ptr not monotone, bit1 index out of range, bit2 duplicate item in a row
+__global__ void k_validate(const long long* __restrict__ row_ptr, const int* __restrict__ idx, long long I, int J,
+                           long long nnz, int scan, int* flags, unsigned long long* max_len) {
+    unsigned long long lmax = 0;
+    int f = 0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < I; i += (long long)gridDim.x * blockDim.x) {
+        const long long beg = row_ptr[i], end = row_ptr[i + 1];
+        if (beg > end || beg < 0 || end > nnz) { f |= 1; continue; }
+        if ((unsigned long long)(end - beg) > lmax) lmax = (unsigned long long)(end - beg);
+        if (!scan) continue;
+        bool ascending = true;
+        int prev = -1;
+        for (long long q = beg; q < end; ++q) {
+            const int j = idx[q];
+            if (j < 0 || j >= J) f |= 2;
+            if (j <= prev) ascending = false;
+            prev = j;
+        }
+        if (!ascending && !(f & 2)) {
+            for (long long q = beg; q < end; ++q) {
+                const int j = idx[q];
+                for (long long r = q + 1; r < end; ++r) if (idx[r] == j) f |= 4;
+            }
+        }
+    }
+    if (f) atomicOr(flags, f);
+    atomicMax(max_len, lmax);
+}
+
+// max |a|, max |c| as float bit patterns (order-independent)
+__global__ void k_absmax(const float* __restrict__ a, long long na, const float* __restrict__ c, long long nc, unsigned* out) {
+    unsigned ma = 0, mc = 0;
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < na; q += (long long)gridDim.x * blockDim.x)
+        ma = max(ma, __float_as_uint(fabsf(a[q])));
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < nc; q += (long long)gridDim.x * blockDim.x)
+        mc = max(mc, __float_as_uint(fabsf(c[q])));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { ma = max(ma, __shfl_xor_sync(kFull, ma, o)); mc = max(mc, __shfl_xor_sync(kFull, mc, o)); }
+    if ((threadIdx.x & 31) == 0) { atomicMax(out + 0, ma); atomicMax(out + 1, mc); }
+}
+
+// fixed-point column sums: colsq[j] += sum_k a^2 (for L, R2), colabs[j*m+k] += |a|, cabs += |c|
+__global__ void k_col_stats(const int* __restrict__ idx, const float* __restrict__ a, const float* __restrict__ c,
+                            long long nnz, int m, double scale_sq, double scale_abs, double scale_c,
+                            unsigned long long* colsq, unsigned long long* colabs, unsigned long long* cabs,
+                            int do_a, int do_c) {
+    long long lc = 0;
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < nnz; q += (long long)gridDim.x * blockDim.x) {
+        if (do_a) {
+            const int j = idx[q];
+            double sq = 0.0;
+            for (int k = 0; k < m; ++k) {
+                const double v = (double)a[q * m + k];
+                sq = fma(v, v, sq);
+                const long long fa = __double2ll_rn(fabs(v) * scale_abs);
+                if (fa) atomicAdd(colabs + (long long)j * m + k, (unsigned long long)fa);
+            }
+            const long long fq = __double2ll_rn(sq * scale_sq);
+            if (fq) atomicAdd(colsq + j, (unsigned long long)fq);
+        }
+        if (do_c) lc += __double2ll_rn(fabs((double)c[q]) * scale_c);
+    }
+    if (do_c) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) lc += __shfl_xor_sync(kFull, lc, o);
+        if ((threadIdx.x & 31) == 0 && lc) atomicAdd(cabs, (unsigned long long)lc);
+    }
+}
+
+// out[0] = max_j colsq (fixed), out[1] = max_q colabs (fixed)
+__global__ void __launch_bounds__(1024) k_reduce_stats(const unsigned long long* colsq, int J, const unsigned long long* colabs,
+                                                       int JM, unsigned long long* out) {
+    __shared__ unsigned long long sh[2][32];
+    unsigned long long a = 0, b = 0;
+    for (int q = threadIdx.x; q < J; q += 1024) a = max(a, colsq[q]);
+    for (int q = threadIdx.x; q < JM; q += 1024) b = max(b, colabs[q]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { a = max(a, __shfl_xor_sync(kFull, a, o)); b = max(b, __shfl_xor_sync(kFull, b, o)); }
+    if ((threadIdx.x & 31) == 0) { sh[0][threadIdx.x >> 5] = a; sh[1][threadIdx.x >> 5] = b; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        a = 0; b = 0;
+        for (int w = 0; w < 32; ++w) { a = max(a, sh[0][w]); b = max(b, sh[1][w]); }
+        out[0] = a; out[1] = b;
+    }
+}
+
+}  // namespace dualip_dev

@@ -1,0 +1,103 @@
+"""Helpers shared by the `-m gpu` parity tests: build the oracle problem and the CUDA problem from the
+SAME arrays and compare at the tolerances BASELINE.json's north_star states."""
+import numpy as np
+import torch
+
+import oracle
+import paper_2606_07777_b200 as pkg
+import synth
+
+TOL_X = 1e-5        # x: element-wise absolute
+TOL_GRAD = 1e-5     # grad g: relative L2, per evaluation / per iteration
+TOL_G = 1e-5        # dual objective: relative
+
+_KIND = {"simplex": (oracle.PROJ_SIMPLEX_INEQ, pkg.PROJ_SIMPLEX_INEQ), "box": (oracle.PROJ_BOX, pkg.PROJ_BOX),
+         "boxcut": (oracle.PROJ_BOXCUT, pkg.PROJ_BOXCUT), "simplex_eq": (oracle.PROJ_SIMPLEX_EQ, pkg.PROJ_SIMPLEX_EQ)}
+
+
+def both(d, kind="simplex", p0=1.0, p1=0.0, **opt):
+    """d: dict of numpy arrays (I,J,m,row_ptr,item_idx,c,a,b) -> (oracle.Problem, pkg.Problem)."""
+    ko, kg = _KIND[kind]
+    po = oracle.Problem(d["I"], d["J"], d["m"], d["row_ptr"], d["item_idx"], d["c"], d["a"], d["b"], ko, p0, p1)
+    t = {k: torch.from_numpy(np.ascontiguousarray(getattr(po, k))).cuda() for k in ("row_ptr", "item_idx", "c", "a", "b")}
+    pg = pkg.Problem.create(po.I, po.J, po.m, t["row_ptr"], t["item_idx"], t["c"], t["a"], t["b"],
+                            pkg.binding.make_opts(projection=kg, p0=p0, p1=p1, **opt))
+    return po, pg
+
+
+def from_instance(inst: synth.Instance, **opt):
+    d = inst.numpy()
+    d.update(I=inst.I, J=inst.J, m=inst.m)
+    kind, p0, p1 = synth.proj_spec(inst.cfg)
+    return both(d, kind, p0, p1, **opt)
+
+
+def gpu_grad(pg, lam, gamma, want_x=True):
+    lam_t = torch.as_tensor(np.asarray(lam, dtype=np.float64)).cuda()
+    grad = torch.empty(pg.J * pg.m, dtype=torch.float64, device="cuda")
+    x = torch.empty(pg.nnz, dtype=torch.float32, device="cuda") if want_x else None
+    sc = pkg.Scalars()
+    pg.grad(lam_t, gamma, grad=grad, scalars=sc, x=x)
+    torch.cuda.synchronize()
+    return sc, grad.cpu().numpy(), (x.cpu().numpy() if want_x else None)
+
+
+def rel_l2(a, b):
+    nb = np.linalg.norm(b)
+    return np.linalg.norm(a - b) / (nb if nb > 0 else 1.0)
+
+
+def assert_grad_parity(po, pg, lam, gamma, tag=""):
+    ref = oracle.grad(po, lam, gamma)
+    sc, grad, x = gpu_grad(pg, lam, gamma)
+    ex = np.abs(x.astype(np.float64) - ref.x).max() if ref.x.size else 0.0
+    eg = rel_l2(grad, ref.grad)
+    assert ex <= TOL_X, f"{tag} x abs err {ex:.3e}"
+    assert eg <= TOL_GRAD, f"{tag} grad rel L2 {eg:.3e}"
+    scale = max(abs(ref.g), 1e-300)
+    assert abs(sc.g - ref.g) <= TOL_G * scale + 1e-12, f"{tag} g {sc.g} vs {ref.g}"
+    assert abs(sc.obj - ref.obj) <= TOL_G * max(abs(ref.obj), 1e-12) + 1e-9, f"{tag} obj {sc.obj} vs {ref.obj}"
+    assert abs(sc.reg - ref.reg) <= TOL_G * max(abs(ref.reg), 1e-12) + 1e-9, f"{tag} reg {sc.reg} vs {ref.reg}"
+    assert abs(sc.r_inf - ref.r_inf) <= TOL_GRAD * np.linalg.norm(ref.grad) + 1e-12, f"{tag} r_inf"
+    assert abs(sc.r_2 - ref.r_2) <= TOL_GRAD * np.linalg.norm(ref.grad) + 1e-12, f"{tag} r_2"
+    return ex, eg
+
+
+def gpu_solve(pg, gammas, iters, lam0=None, want_trace=True, want_x=True):
+    Jm, T = pg.J * pg.m, int(np.sum(iters))
+    lam = torch.zeros(Jm, dtype=torch.float64, device="cuda") if lam0 is None else torch.as_tensor(lam0).double().cuda().clone()
+    x = torch.empty(pg.nnz, dtype=torch.float32, device="cuda") if want_x else None
+    grad = torch.empty(Jm, dtype=torch.float64, device="cuda")
+    tr = None
+    if want_trace:
+        tr = {"g": torch.empty(T, dtype=torch.float64, device="cuda"), "r_inf": torch.empty(T, dtype=torch.float64, device="cuda"),
+              "r_2": torch.empty(T, dtype=torch.float64, device="cuda"), "grad": torch.empty(T * Jm, dtype=torch.float64, device="cuda"),
+              "lambda": torch.empty(T * Jm, dtype=torch.float64, device="cuda")}
+    sc = pkg.Scalars()
+    pg.solve(gammas, iters, lam, x=x, scalars=sc, grad=grad, trace=tr)
+    torch.cuda.synchronize()
+    out = {"lam": lam.cpu().numpy(), "x": x.cpu().numpy() if want_x else None, "grad": grad.cpu().numpy(), "sc": sc}
+    if tr:
+        out.update(tr_g=tr["g"].cpu().numpy(), tr_grad=tr["grad"].cpu().numpy().reshape(T, Jm),
+                   tr_lam=tr["lambda"].cpu().numpy().reshape(T, Jm), tr_rinf=tr["r_inf"].cpu().numpy(), tr_r2=tr["r_2"].cpu().numpy())
+    return out
+
+
+def assert_trajectory_parity(po, pg, gammas, iters, lam0=None, momentum=True, tag=""):
+    """Independent solves compared per iteration (parity mode B of SURVEY 8(c))."""
+    ref = oracle.solve(po, gammas, iters, lam0=lam0, momentum=momentum, trace_grad=True, trace_lambda=True)
+    out = gpu_solve(pg, gammas, iters, lam0=lam0)
+    T = int(np.sum(iters))
+    worst = 0.0
+    for n in range(T):
+        e = rel_l2(out["tr_grad"][n], ref.trace_grad[n])
+        worst = max(worst, e)
+        assert e <= TOL_GRAD, f"{tag} iteration {n}: grad rel L2 {e:.3e}"
+    assert np.abs(out["tr_g"] - ref.trace_g).max() <= TOL_G * np.abs(ref.trace_g).max() + 1e-12, f"{tag} trace g"
+    ex = np.abs(out["x"].astype(np.float64) - ref.x).max()
+    assert ex <= TOL_X, f"{tag} final x abs err {ex:.3e}"
+    assert abs(out["sc"].g - ref.final.g) <= TOL_G * abs(ref.final.g) + 1e-12, f"{tag} final g"
+    assert rel_l2(out["grad"], ref.final.grad) <= TOL_GRAD, f"{tag} final grad"
+    lam_scale = max(np.abs(ref.lam).max(), 1e-300)
+    assert np.abs(out["lam"] - ref.lam).max() <= 1e-6 * lam_scale + 1e-12, f"{tag} lambda_T"
+    return worst, ex, ref, out

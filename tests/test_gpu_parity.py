@@ -1,0 +1,199 @@
+"""`-m gpu` parity tests: the CUDA path (through the C ABI) against the fp64 oracle, element by element on
+the same seeded inputs.  Tolerances (BASELINE.json north_star): per-evaluation grad g relative L2 <= 1e-5,
+x element-wise absolute <= 1e-5, dual objective relative <= 1e-5; integer work bit-exact."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import synth
+from conftest import random_problem, read_worked_examples
+
+pytestmark = pytest.mark.gpu
+
+if torch.cuda.is_available():
+    import paper_2606_07777_b200 as pkg
+    from gpu_util import (assert_grad_parity, assert_trajectory_parity, both, from_instance, gpu_grad, gpu_solve, rel_l2)
+
+
+@pytest.mark.parametrize("ex", read_worked_examples(), ids=lambda e: e["case"])
+def test_hand_worked_examples(ex):
+    po, pg = both(ex)
+    sc, grad, x = gpu_grad(pg, ex["lambda"], ex["gamma"])
+    np.testing.assert_allclose(x, ex["x"], atol=1e-6)
+    np.testing.assert_allclose(grad, ex["grad"], atol=1e-6)
+    for key in ("g", "obj", "reg", "r_inf", "r_2"):
+        assert abs(getattr(sc, key) - ex[key]) < 1e-6, key
+
+
+def _ragged(rng, I, J, m, lens):
+    """rows with prescribed lengths (0 allowed), items unsorted in every third row."""
+    rows, idx = [0], []
+    for i in range(I):
+        d = int(lens[i % len(lens)])
+        it = rng.choice(J, size=min(d, J), replace=False)
+        it = it if i % 3 == 0 else np.sort(it)
+        idx.extend(it.tolist()); rows.append(len(idx))
+    nnz = len(idx)
+    c = (-rng.random(nnz) * rng.choice([1.0, 3.0])).astype(np.float32)
+    a = (0.5 + rng.random(nnz * m)).astype(np.float32)
+    col = np.zeros(J * m)
+    np.add.at(col, (np.repeat(np.array(idx, dtype=np.int64), m) * m + np.tile(np.arange(m), nnz)), a)
+    b = (0.1 * col + 0.01).astype(np.float32)
+    return dict(I=I, J=J, m=m, row_ptr=np.array(rows, dtype=np.int64), item_idx=np.array(idx, dtype=np.int32), c=c, a=a, b=b)
+
+
+CASES = [
+    # (tag, I, J, m, row lengths pattern)
+    ("short8", 3000, 40, 1, [1, 2, 7, 8, 3, 0, 5]),
+    ("mid16", 3000, 100, 1, [9, 16, 17, 31, 12, 0, 48, 20]),
+    ("warp32", 2000, 300, 1, [33, 64, 65, 100, 128, 40, 159, 160]),
+    ("long_rows", 300, 700, 1, [161, 200, 400, 650, 5, 32]),       # beyond the register budget -> warp path
+    ("two_fam", 2000, 120, 2, [50, 99, 100, 150, 7, 0]),
+    ("three_fam", 800, 60, 3, [5, 33, 40, 1]),
+    ("four_fam", 500, 50, 4, [10, 45]),
+    ("one_row", 1, 5, 1, [3]),
+    ("all_empty", 7, 3, 1, [0]),
+]
+
+
+@pytest.mark.parametrize("tag,I,J,m,lens", CASES, ids=[c[0] for c in CASES])
+@pytest.mark.parametrize("kind,p0,p1", [("simplex", 1.0, 0.0), ("simplex", 0.5, 0.0), ("simplex_eq", 1.0, 0.0),
+                                        ("boxcut", 0.3, 1.0), ("boxcut", 1.0, 1.0), ("box", 0.0, 0.4), ("box", -0.2, 1.0)])
+def test_grad_parity_small(tag, I, J, m, lens, kind, p0, p1):
+    rng = np.random.default_rng(abs(hash((tag, kind, p0))) % (2 ** 31))
+    d = _ragged(rng, I, J, m, lens)
+    po, pg = both(d, kind, p0, p1)
+    for gamma in (1.0, 1e-1, 1e-2, 1e-3):
+        for lam_scale in (0.0, 0.3):
+            lam = rng.random(J * m) * lam_scale
+            assert_grad_parity(po, pg, lam, gamma, tag=f"{tag}/{kind}/g={gamma}/l={lam_scale}")
+    lam = rng.normal(size=J * m) * 0.2                     # g is defined for negative lambda too
+    assert_grad_parity(po, pg, lam, 0.05, tag=f"{tag}/{kind}/neg")
+    pg.destroy()
+
+
+@pytest.mark.parametrize("G", [8, 16, 32])
+def test_group_width_does_not_change_results(G):
+    rng = np.random.default_rng(5)
+    d = _ragged(rng, 4000, 200, 1, [3, 10, 20, 35, 70, 0, 150, 90])
+    po, pg = both(d, group_lanes=G)
+    assert pg.info().group_lanes == G
+    lam = rng.random(200) * 0.4
+    assert_grad_parity(po, pg, lam, 1e-2, tag=f"G={G}")
+    assert_grad_parity(po, pg, lam, 1e-3, tag=f"G={G}")
+
+
+def test_cfg1_verbatim_trajectory():
+    """BASELINE config 1 as stated: 200 AGD iterations from lambda = 0 at gamma = 1e-2 (slack: lambda stays 0)."""
+    inst = synth.generate("cfg1")
+    po, pg = from_instance(inst)
+    worst, ex, ref, out = assert_trajectory_parity(po, pg, inst.cfg.gammas, inst.cfg.iters, tag="cfg1")
+    assert np.all(out["lam"] == 0.0) and np.all(ref.lam == 0.0)
+
+
+def test_cfg1_tight_trajectory():
+    inst = synth.generate("cfg1-tight")
+    po, pg = from_instance(inst)
+    worst, ex, ref, out = assert_trajectory_parity(po, pg, inst.cfg.gammas, inst.cfg.iters, tag="cfg1-tight")
+    assert (ref.lam > 0).sum() >= 5                         # the update is really exercised
+    frac = ((ref.x > 1e-9) & (ref.x < 1 - 1e-9)).sum()
+    assert frac > 20                                        # fractional projections too
+
+
+@pytest.mark.parametrize("name,I,iters", [("cfg2-tight", 60_000, 40), ("cfg3-tight", 30_000, 30), ("cfg4-tight", 8_000, 30),
+                                          ("cfg5-tight", 40_000, None), ("cfg2", 60_000, 20), ("cfg3", 30_000, 20),
+                                          ("cfg4", 8_000, 20), ("cfg5", 40_000, None)])
+def test_scaled_config_trajectories(name, I, iters):
+    """Every BASELINE config (and its tight companion) at a user count the oracle finishes in seconds; the
+    recipe (J, degrees, values, projection, gamma schedule) is the config's own."""
+    cfg = synth.get_config(name, I=I)
+    inst = synth.generate(cfg)
+    po, pg = from_instance(inst)
+    its = [iters] * len(cfg.gammas) if iters else [15] * len(cfg.gammas)
+    assert_trajectory_parity(po, pg, cfg.gammas, its, tag=name)
+    for which in range(2):                                   # same-lambda probes with a busy lambda
+        lam = synth.probe_lambda(inst, which, 0.5 if "3" not in name else 0.05).numpy()
+        assert_grad_parity(po, pg, lam, cfg.gammas[-1], tag=f"{name}/probe{which}")
+
+
+def test_plain_ascent_option_and_warm_start():
+    inst = synth.generate(synth.get_config("cfg2-tight", I=20_000))
+    po, pg = from_instance(inst, momentum=False)
+    assert_trajectory_parity(po, pg, [1e-2, 1e-3], [15, 15], momentum=False, tag="beta0")
+    po2, pg2 = from_instance(inst)
+    lam0 = synth.probe_lambda(inst, 3, 0.2).numpy()
+    assert_trajectory_parity(po2, pg2, [1e-2], [10], lam0=lam0, tag="warm")
+
+
+def test_run_to_run_and_geometry_bit_reproducible():
+    inst = synth.generate(synth.get_config("cfg3-tight", I=30_000))
+    lam = synth.probe_lambda(inst, 0, 0.05).numpy()
+    outs = []
+    for grid, red in ((0, pkg.RED_AUTO), (0, pkg.RED_AUTO), (37, pkg.RED_AUTO), (0, pkg.RED_GLOBAL)):
+        po, pg = from_instance(inst, grid_ctas=grid, reduction=red)
+        sc, grad, x = gpu_grad(pg, lam, 1e-3)
+        outs.append((sc.g, grad.copy(), x.copy()))
+        pg.destroy()
+    assert outs[0][0] == outs[1][0] and np.array_equal(outs[0][1], outs[1][1]) and np.array_equal(outs[0][2], outs[1][2])
+    for o in outs[2:]:                                       # integer accumulation: any geometry / strategy, same bits
+        assert np.array_equal(outs[0][1], o[1]) and np.array_equal(outs[0][2], o[2])
+
+
+def test_host_pointers_take_the_same_path():
+    rng = np.random.default_rng(9)
+    d = random_problem(rng, I=500, J=30, m=2, deg=(2, 9))
+    po, pg = both(d)
+    lam = rng.random(60) * 0.2
+    sc_d, grad_d, x_d = gpu_grad(pg, lam, 0.05)
+    pg_h = pkg.Problem.create(po.I, po.J, po.m, po.row_ptr, po.item_idx, po.c, po.a, po.b)   # numpy = host pointers
+    grad_h, x_h, sc_h = np.empty(60), np.empty(po.nnz, dtype=np.float32), pkg.Scalars()
+    pg_h.grad(np.ascontiguousarray(lam), 0.05, grad=grad_h, scalars=sc_h, x=x_h)
+    assert np.array_equal(grad_h, grad_d) and np.array_equal(x_h, x_d) and sc_h.g == sc_d.g
+    lam_h = np.zeros(60)
+    pg_h.solve([0.05], [7], lam_h, x=x_h, scalars=sc_h, grad=grad_h)
+    out = gpu_solve(pg, [0.05], [7], want_trace=False)
+    assert np.array_equal(lam_h, out["lam"]) and np.array_equal(x_h, out["x"]) and sc_h.g == out["sc"].g
+
+
+def test_set_c_and_drift_bound():
+    """Config 5's perturbed re-solve in miniature: replace c in place, re-solve, ||dx||_2 <= ||dc||_2/gamma at
+    fixed lambda (the closed form behind the paper's stability claim)."""
+    inst = synth.generate(synth.get_config("cfg5-tight", I=20_000))
+    po, pg = from_instance(inst)
+    lam = synth.probe_lambda(inst, 1, 0.3).numpy()
+    c2 = synth.perturb_c(inst)
+    for gamma in (1e-1, 1e-2):
+        _, _, x1 = gpu_grad(pg, lam, gamma)
+        pg.set_c(c2.cuda())
+        po2 = oracle.Problem(po.I, po.J, po.m, po.row_ptr, po.item_idx, c2.numpy(), po.a, po.b, po.proj_kind, po.p0, po.p1)
+        assert_grad_parity(po2, pg, lam, gamma, tag="set_c")
+        _, _, x2 = gpu_grad(pg, lam, gamma)
+        dc = np.linalg.norm(c2.numpy().astype(np.float64) - inst.c.numpy().astype(np.float64))
+        assert np.linalg.norm(x1.astype(np.float64) - x2.astype(np.float64)) <= dc / gamma * (1 + 1e-5)
+        pg.set_c(inst.c.cuda())
+
+
+def test_create_rejects_bad_input():
+    rp = np.array([0, 2, 4], dtype=np.int64)
+    good = dict(I=2, J=3, m=1, row_ptr=rp, item_idx=np.array([0, 2, 1, 2], dtype=np.int32),
+                c=-np.ones(4, dtype=np.float32), a=np.ones(4, dtype=np.float32), b=np.ones(3, dtype=np.float32))
+
+    def code(**over):
+        d = dict(good); d.update(over)
+        try:
+            pkg.Problem.create(d["I"], d["J"], d["m"], d["row_ptr"], d["item_idx"], d["c"], d["a"], d["b"]).destroy()
+            return 0
+        except pkg.DualipError as e:
+            return e.code
+    assert code() == 0
+    assert code(item_idx=np.array([0, 0, 1, 2], dtype=np.int32)) == -3            # duplicate (sorted row)
+    assert code(item_idx=np.array([2, 0, 1, 1], dtype=np.int32)) == -3            # duplicate (unsorted row)
+    assert code(item_idx=np.array([0, 3, 1, 2], dtype=np.int32)) == -2            # index out of range
+    assert code(item_idx=np.array([0, -1, 1, 2], dtype=np.int32)) == -2
+    assert code(row_ptr=np.array([0, 3, 2], dtype=np.int64)) == -2                # not monotone
+    assert code(row_ptr=np.array([1, 2, 4], dtype=np.int64)) == -2                # row_ptr[0] != 0
+    assert code(J=0) == -1 and code(m=5) == -1
+    po, pg = both(good)
+    with pytest.raises(pkg.DualipError):
+        pg.grad(torch.zeros(3, dtype=torch.float64, device="cuda"), 0.0)           # gamma must be > 0

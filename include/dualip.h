@@ -115,6 +115,8 @@ typedef struct {
     int64_t bytes_resident;  /* device bytes owned by the handle */
     int64_t launches;        /* kernels launched through this handle so far (all entry points) */
     double  fix_scale_s;     /* fixed-point scale of the item accumulators (a power of two) */
+    double  grad_kernel_ms;  /* profiling on: summed device time of the gradient-kernel launches since it was switched on */
+    int64_t grad_kernel_count; /* ... and how many launches that sum covers */
 } dualip_info;
 
 /*
@@ -145,7 +147,8 @@ int dualip_grad(dualip_t* h, const double* lambda, double gamma, double* grad, d
  * a1-a8 -- gamma continuation with projected accelerated ascent (R1-R4).
  *   for each stage s < n_stages:  eta = gammas[s]/L;  y = lambda (warm start, momentum restart)
  *       repeat iters[s] times:  grad at y;  lambda+ = max(0, y + eta*grad);  y = lambda+ + beta_t (lambda+ - lambda)
- *   then one evaluation at the final lambda with gammas[n_stages-1] fills final_scalars / final_grad / x_out.
+ *   then one evaluation at the final lambda with gammas[n_stages-1] fills final_scalars / final_grad / x_out
+ *   (skipped when all three are NULL, so the call is exactly sum(iters) gradient evaluations).
  *   gammas, iters: HOST arrays.  lambda_inout[J*m]: warm start in (zeros for a cold start), lambda_T out.
  *   x_out[nnz], final_scalars, final_grad[J*m] may be NULL; host or device.  trace may be NULL.
  *   n_stages = 0 is allowed (nothing happens).  No host synchronisation happens inside the loop.
@@ -158,7 +161,14 @@ int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int3
  * Recomputes the objective's fixed-point scale.  With borrow = 1 the handle switches to the new pointer. */
 int dualip_set_c(dualip_t* h, const float* c_new, void* stream);
 
-int dualip_get_info(const dualip_t* h, dualip_info* info);
+/* Profiling hook for the measurement harness: when on, every gradient-kernel launch is bracketed by CUDA
+ * events recorded on the launching stream (no host synchronisation is added); dualip_get_info waits for the
+ * recorded events and reports the summed device time.  Switching it on resets the counters.  At most 4096
+ * launches are timed between two dualip_get_info calls; later ones run untimed. */
+int dualip_set_profiling(dualip_t* h, int on);
+
+/* Fills *info.  With profiling on, blocks until the timed launches have finished. */
+int dualip_get_info(dualip_t* h, dualip_info* info);
 
 /* Frees everything the handle owns.  NULL is accepted. */
 void dualip_destroy(dualip_t* h);

@@ -16,7 +16,7 @@ PROJ_SIMPLEX_INEQ, PROJ_BOX, PROJ_BOXCUT, PROJ_SIMPLEX_EQ = 0, 1, 2, 3
 RED_AUTO, RED_SMEM, RED_GLOBAL, RED_CSC = 0, 1, 2, 3
 
 EXPORTED_SYMBOLS = ("dualip_opts_default", "dualip_create", "dualip_grad", "dualip_solve", "dualip_set_c",
-                    "dualip_get_info", "dualip_destroy", "dualip_strerror")
+                    "dualip_set_profiling", "dualip_get_info", "dualip_destroy", "dualip_strerror")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 
@@ -52,7 +52,8 @@ class Info(ctypes.Structure):
                 ("L", ctypes.c_double), ("max_row_len", ctypes.c_int64), ("group_lanes", ctypes.c_int32),
                 ("chunk_regs", ctypes.c_int32), ("reduction", ctypes.c_int32), ("lambda_in_smem", ctypes.c_int32),
                 ("grid_ctas", ctypes.c_int32), ("block_threads", ctypes.c_int32), ("smem_bytes", ctypes.c_int64),
-                ("bytes_resident", ctypes.c_int64), ("launches", ctypes.c_int64), ("fix_scale_s", ctypes.c_double)]
+                ("bytes_resident", ctypes.c_int64), ("launches", ctypes.c_int64), ("fix_scale_s", ctypes.c_double),
+                ("grad_kernel_ms", ctypes.c_double), ("grad_kernel_count", ctypes.c_int64)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -82,11 +83,12 @@ def load_library():
         lib.dualip_solve.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, ctypes.POINTER(_Trace), vp]
         lib.dualip_set_c.argtypes = [vp, vp, vp]
         lib.dualip_get_info.argtypes = [vp, ctypes.POINTER(Info)]
+        lib.dualip_set_profiling.argtypes = [vp, ctypes.c_int]
         lib.dualip_destroy.argtypes = [vp]
         lib.dualip_destroy.restype = None
         lib.dualip_strerror.argtypes = [ctypes.c_int]
         lib.dualip_strerror.restype = ctypes.c_char_p
-        for f in ("dualip_create", "dualip_grad", "dualip_solve", "dualip_set_c", "dualip_get_info"):
+        for f in ("dualip_create", "dualip_grad", "dualip_solve", "dualip_set_c", "dualip_get_info", "dualip_set_profiling"):
             getattr(lib, f).restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -198,6 +200,9 @@ class Problem:
         _check(load_library().dualip_set_c(self._h, _ptr(c_new, np.float32), _stream_ptr(stream)))
         if self._keep is not None:
             self._keep = self._keep + (c_new,)
+
+    def set_profiling(self, on: bool):
+        _check(load_library().dualip_set_profiling(self._h, int(on)))
 
     def info(self) -> Info:
         inf = Info()

@@ -8,6 +8,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <vector>
 
 using namespace dualip_dev;
 
@@ -48,6 +49,12 @@ struct dualip {
     int num_sms = 0;
     long long launches = 0;
     long long bytes_resident = 0;
+    // profiling hook: event pairs around gradient-kernel launches
+    bool profile = false;
+    std::vector<cudaEvent_t> events;
+    size_t ev_used = 0;
+    double prof_ms = 0.0;
+    long long prof_count = 0;
 };
 
 namespace {
@@ -223,9 +230,36 @@ void fill_grad_params(const dualip* h, GradParams& p, const double* lam_dev, dou
     p.scale_s = h->scale_s; p.scale_obj = h->scale_obj; p.scale_sq = h->scale_sq;
 }
 
+constexpr size_t kMaxTimedLaunches = 4096;
+
+bool prof_begin(dualip* h, cudaStream_t st) {
+    if (!h->profile || h->ev_used + 2 > 2 * kMaxTimedLaunches) return false;
+    while (h->events.size() < h->ev_used + 2) {
+        cudaEvent_t e;
+        if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); return false; }
+        h->events.push_back(e);
+    }
+    return cudaEventRecord(h->events[h->ev_used], st) == cudaSuccess;
+}
+void prof_end(dualip* h, cudaStream_t st) {
+    cudaEventRecord(h->events[h->ev_used + 1], st);
+    h->ev_used += 2;
+}
+void prof_collect(dualip* h) {
+    for (size_t e = 0; e + 1 < h->ev_used; e += 2) {
+        float ms = 0.0f;
+        if (cudaEventSynchronize(h->events[e + 1]) == cudaSuccess &&
+            cudaEventElapsedTime(&ms, h->events[e], h->events[e + 1]) == cudaSuccess) { h->prof_ms += ms; h->prof_count++; }
+        else cudaGetLastError();
+    }
+    h->ev_used = 0;
+}
+
 int launch_grad(dualip* h, const double* lam_dev, double gamma, float* x_dev, cudaStream_t st) {
     GradParams p;
     fill_grad_params(h, p, lam_dev, gamma, x_dev);
+    const bool timed = prof_begin(h, st);
+    struct End { dualip* h; cudaStream_t st; bool on; ~End() { if (on) prof_end(h, st); } } end_guard{h, st, timed};
     if (h->opts.projection == DUALIP_PROJ_BOX) {
         const int g = grid_for(h->nnz, 256, h->num_sms);
         if (h->m == 1) k_grad_box<1><<<g, 256, 0, st>>>(p);
@@ -284,8 +318,17 @@ void dualip_destroy(dualip_t* h) {
     if (h->own_c) cudaFree((void*)h->c);
     cudaFree(h->b); cudaFree(h->s_fix); cudaFree(h->lam_cur); cudaFree(h->y); cudaFree(h->lam_stage);
     cudaFree(h->grad_stage); cudaFree(h->scalars_dev); cudaFree(h->x_stage);
+    for (cudaEvent_t e : h->events) cudaEventDestroy(e);
     cudaGetLastError();
     delete h;
+}
+
+int dualip_set_profiling(dualip_t* h, int on) {
+    if (!h) return DUALIP_EINVAL;
+    prof_collect(h);
+    h->profile = on != 0;
+    h->prof_ms = 0.0; h->prof_count = 0;
+    return DUALIP_OK;
 }
 
 int dualip_create(dualip_t** out, int64_t I, int32_t J, int32_t m, const int64_t* row_ptr, const int32_t* item_idx,
@@ -397,8 +440,9 @@ fail:
 #undef CKF
 }
 
-int dualip_get_info(const dualip_t* h, dualip_info* info) {
+int dualip_get_info(dualip_t* h, dualip_info* info) {
     if (!h || !info) return DUALIP_EINVAL;
+    prof_collect(h);
     std::memset(info, 0, sizeof(*info));
     info->I = h->I; info->nnz = h->nnz; info->J = h->J; info->m = h->m; info->L = h->L;
     info->max_row_len = h->max_row_len;
@@ -409,6 +453,7 @@ int dualip_get_info(const dualip_t* h, dualip_info* info) {
     info->smem_bytes = (int64_t)h->plan.smem;
     info->bytes_resident = h->bytes_resident; info->launches = h->launches;
     info->fix_scale_s = h->scale_s;
+    info->grad_kernel_ms = h->prof_ms; info->grad_kernel_count = h->prof_count;
     return DUALIP_OK;
 }
 
@@ -488,8 +533,8 @@ int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int3
             if (rc != 0) return rc;
         }
     }
-    // final evaluation at lambda_T (R3)
-    {
+    // final evaluation at lambda_T (R3); skipped when nobody asked for its outputs
+    if (x_out || final_scalars || final_grad) {
         float* x_d = x_out;
         if (x_out && !x_dev) { int rc = ensure_x_stage(h); if (rc != 0) return rc; x_d = h->x_stage; }
         int rc = launch_grad(h, h->lam_cur, gammas[n_stages - 1], x_d, st);

@@ -72,7 +72,7 @@ typedef struct {
     int32_t group_lanes;  /* lanes cooperating on one row: 0 = auto from the mean row length, or 4/8/16/32 */
     int32_t grid_ctas;    /* CTAs of the gradient kernel: 0 = auto (SM count x resident CTAs per SM) */
     int32_t use_graph;    /* 1: dualip_solve replays a captured CUDA graph per stage; 0: direct launches */
-    int32_t reserved[5];  /* must be zero */
+    int32_t reserved[5];  /* reserved[0] = 1 forces the direct-load kernel (parity tests of both kernels); rest must be zero */
 } dualip_opts;
 
 /* Fills *opts with the defaults: unit simplex (inequality), AUTO reduction, copy, validate, momentum. */
@@ -115,6 +115,10 @@ typedef struct {
     int64_t bytes_resident;  /* device bytes owned by the handle */
     int64_t launches;        /* kernels launched through this handle so far (all entry points) */
     double  fix_scale_s;     /* fixed-point scale of the item accumulators (a power of two) */
+    int32_t streaming;       /* 1: TMA bulk-copy pipeline kernel (k_grad_tma); 0: direct-load kernel (k_grad) */
+    int32_t stages;          /* pipeline stages of the streaming kernel */
+    int64_t tile_units;      /* tile size TN: a tile is cut every TN units of (nonzeros + 8 per row) */
+    int64_t ntiles;
     double  grad_kernel_ms;  /* profiling on: summed device time of the gradient-kernel launches since it was switched on */
     int64_t grad_kernel_count; /* ... and how many launches that sum covers */
 } dualip_info;

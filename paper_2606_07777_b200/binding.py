@@ -53,6 +53,7 @@ class Info(ctypes.Structure):
                 ("chunk_regs", ctypes.c_int32), ("reduction", ctypes.c_int32), ("lambda_in_smem", ctypes.c_int32),
                 ("grid_ctas", ctypes.c_int32), ("block_threads", ctypes.c_int32), ("smem_bytes", ctypes.c_int64),
                 ("bytes_resident", ctypes.c_int64), ("launches", ctypes.c_int64), ("fix_scale_s", ctypes.c_double),
+                ("streaming", ctypes.c_int32), ("stages", ctypes.c_int32), ("tile_units", ctypes.c_int64), ("ntiles", ctypes.c_int64),
                 ("grad_kernel_ms", ctypes.c_double), ("grad_kernel_count", ctypes.c_int64)]
 
     def as_dict(self):
@@ -120,12 +121,13 @@ def _ptr(t, dtype=None, keep=None):
 
 
 def make_opts(projection=PROJ_SIMPLEX_INEQ, p0=1.0, p1=0.0, reduction=RED_AUTO, borrow=False, validate=True,
-              momentum=True, group_lanes=0, grid_ctas=0, use_graph=False) -> Opts:
+              momentum=True, group_lanes=0, grid_ctas=0, use_graph=False, direct_kernel=False) -> Opts:
     o = Opts()
     load_library().dualip_opts_default(ctypes.byref(o))
     o.projection, o.p0, o.p1, o.reduction = projection, p0, p1, reduction
     o.borrow, o.validate, o.momentum = int(borrow), int(validate), int(momentum)
     o.group_lanes, o.grid_ctas, o.use_graph = group_lanes, grid_ctas, int(use_graph)
+    o.reserved[0] = 1 if direct_kernel else 0
     return o
 
 

@@ -3,6 +3,7 @@
 // dualip_kernels.cuh; the host only sizes buffers, picks fixed-point exponents and launches.
 #include "../../include/dualip.h"
 #include "dualip_kernels.cuh"
+#include "dualip_grad_tma.cuh"
 
 #include <cmath>
 #include <cstdlib>
@@ -16,12 +17,18 @@ namespace {
 
 constexpr size_t kSmemBudget = 227 * 1024;  // bytes of dynamic shared memory one CTA may opt in to on sm_100a
 
+constexpr int kTmaConsumerWarps = 31;         // + 1 producer warp = 1024 threads per CTA
+
 struct Plan {
     int G = 32, KREG = 5, M = 1;
     bool lam_smem = true, acc_smem = true;
     int grid = 0;
     size_t smem = 0;
     const void* fn = nullptr;
+    // streaming (TMA) path
+    bool tma = false;
+    long long TN = 0, ntiles = 0;
+    int cap_nz = 0, cap_rows = 0, stages = 0, stage_bytes = 0;
 };
 
 }  // namespace
@@ -40,6 +47,7 @@ struct dualip {
     double* lam_cur = nullptr; double* y = nullptr; double* lam_stage = nullptr; double* grad_stage = nullptr;
     double* scalars_dev = nullptr;
     float* x_stage = nullptr;
+    dualip_dev::TileEntry* tiles = nullptr;
     // constants from a0
     double L = 0.0, max_colabs = 0.0, sum_abs_c = 0.0;
     long long max_row_len = 0;
@@ -113,6 +121,69 @@ const void* pick_kernel(const Plan& pl) {
     return pick_k<32>(pl.KREG, pl.M, pl.lam_smem, pl.acc_smem);
 }
 
+template <int G, int M>
+const void* pick_tma_acc(bool acc, bool gbox) {
+    if (acc) return gbox ? (const void*)k_grad_tma<G, M, true, true, kTmaConsumerWarps>
+                         : (const void*)k_grad_tma<G, M, true, false, kTmaConsumerWarps>;
+    return gbox ? (const void*)k_grad_tma<G, M, false, true, kTmaConsumerWarps>
+                : (const void*)k_grad_tma<G, M, false, false, kTmaConsumerWarps>;
+}
+template <int G>
+const void* pick_tma_m(int M, bool acc, bool gbox) {
+    if (M == 1) return pick_tma_acc<G, 1>(acc, gbox);
+    if (M == 2) return pick_tma_acc<G, 2>(acc, gbox);
+    return nullptr;
+}
+const void* pick_tma_kernel(const Plan& pl, bool gbox) {
+    if (pl.M == 0) return pick_tma_acc<8, 0>(pl.acc_smem, gbox);
+    if (pl.G == 4) return pick_tma_m<4>(pl.M, pl.acc_smem, gbox);
+    if (pl.G == 8) return pick_tma_m<8>(pl.M, pl.acc_smem, gbox);
+    if (pl.G == 16) return pick_tma_m<16>(pl.M, pl.acc_smem, gbox);
+    return pick_tma_m<32>(pl.M, pl.acc_smem, gbox);
+}
+
+// Streaming plan: lambda (and, if there is room for >= 96 KB of stages beside them, the accumulators) in shared
+// memory, the rest of the 227 KB split into `stages` tile buffers.  Returns false if this problem cannot use it.
+bool plan_tma(dualip* h, Plan& pl) {
+    const size_t JM = (size_t)h->J * h->m;
+    const int red = h->opts.reduction;
+    if (h->opts.projection == DUALIP_PROJ_BOX || h->nnz == 0) return false;
+    if (h->max_row_len > 8192) return false;
+    if (((uintptr_t)h->row_ptr | (uintptr_t)h->idx | (uintptr_t)h->c | (uintptr_t)h->a) & 15) return false;
+    const size_t fixed = 128 + 128;
+    if (fixed + 8 * JM + 32 * 1024 > kSmemBudget) return false;
+    size_t avail_acc = kSmemBudget > fixed + 16 * JM ? kSmemBudget - fixed - 16 * JM : 0;
+    bool acc = (red == DUALIP_RED_AUTO && avail_acc >= 96 * 1024) || (red == DUALIP_RED_SMEM && avail_acc >= 32 * 1024);
+    if (red == DUALIP_RED_SMEM && !acc) return false;
+    const size_t avail = kSmemBudget - fixed - (acc ? 16 : 8) * JM;
+    const int m = h->m;
+    const long long units = h->nnz + (long long)kRowCost * h->I;
+    long long TN = 0; int stages = 0; size_t stage_bytes = 0;
+    for (int S = 3; S >= 2 && TN < 256; --S) {
+        stage_bytes = (avail / S) & ~(size_t)127;
+        const long long over = 80 + (h->max_row_len + 8) * (8 + 4 * m);
+        long long tn = ((long long)stage_bytes - over) / (9 + 4 * m);
+        tn = tn > 0 ? (tn & ~63ll) : 0;
+        if (tn >= (S == 3 ? 512 : 256)) { TN = tn; stages = S; }
+    }
+    if (TN < 256) return false;
+    // small problems: keep at least ~8 tiles per CTA so the static deal stays balanced
+    const long long want = units / ((long long)h->num_sms * 8);
+    if (TN > 8192) TN = 8192;
+    if (TN > want) TN = want > 256 ? (want & ~63ll) : 256;
+    pl.tma = true; pl.acc_smem = acc; pl.lam_smem = true;
+    pl.TN = TN; pl.stages = stages;
+    pl.cap_nz = (int)((TN + h->max_row_len + 8 + 3) & ~3ll);
+    pl.cap_rows = (int)((TN / kRowCost + 6 + 1) & ~1ll);
+    size_t sb = (size_t)pl.cap_nz * (8 + 4 * m) + (size_t)pl.cap_rows * 8 + 32;
+    pl.stage_bytes = (int)((sb + 127) & ~(size_t)127);
+    pl.ntiles = (units + TN - 1) / TN;
+    size_t off = 128 + JM * 8 * (acc ? 2 : 1);
+    off = (off + 127) & ~(size_t)127;
+    pl.smem = off + (size_t)pl.stage_bytes * stages;
+    return pl.smem <= kSmemBudget;
+}
+
 int make_plan(dualip* h) {
     Plan pl;
     const size_t JM = (size_t)h->J * h->m;
@@ -126,9 +197,28 @@ int make_plan(dualip* h) {
     const double mean = h->I > 0 ? (double)h->nnz / (double)h->I : 0.0;
     int G = h->opts.group_lanes;
     if (G == 0) G = mean > 20.0 ? 32 : (mean > 10.0 ? 16 : 8);
-    if (G == 4) G = 8;
-    if (G != 8 && G != 16 && G != 32) return DUALIP_EINVAL;
+    if (G != 4 && G != 8 && G != 16 && G != 32) return DUALIP_EINVAL;
     if (pl.M == 0) G = 32;
+    if (h->opts.reserved[0] != 1 && plan_tma(h, pl)) {          // reserved[0] = 1 forces the non-streaming kernel (tests)
+        // narrow lane groups: several rows share one pass of the chunk loop, which amortises the per-row work
+        int Gs = h->opts.group_lanes;
+        if (Gs == 0) Gs = mean <= 12.0 ? 4 : (mean <= 128.0 ? 8 : (mean <= 512.0 ? 16 : 32));
+        if (pl.M == 0) Gs = 8;
+        pl.G = Gs;
+        pl.KREG = 0;
+        const bool gbox = h->opts.projection == DUALIP_PROJ_BOXCUT && h->opts.p0 < h->opts.p1;
+        pl.fn = pick_tma_kernel(pl, gbox);
+        if (!pl.fn) return DUALIP_EUNSUPPORTED;
+        CK(cudaFuncSetAttribute(pl.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+        pl.grid = h->opts.grid_ctas > 0 ? h->opts.grid_ctas : (int)(pl.ntiles < h->num_sms ? pl.ntiles : h->num_sms);
+        if (pl.grid < 1) pl.grid = 1;
+        h->plan = pl;
+        return DUALIP_OK;
+    }
+    pl.tma = false;
+    if (G == 4) G = 8;
+    pl.acc_smem = (red == DUALIP_RED_AUTO || red == DUALIP_RED_SMEM) && fits_both;
+    pl.lam_smem = pl.acc_smem || fits_lam;
     pl.G = G;
     pl.KREG = 5;
     if (pl.M != 0) {
@@ -265,6 +355,13 @@ int launch_grad(dualip* h, const double* lam_dev, double gamma, float* x_dev, cu
         if (h->m == 1) k_grad_box<1><<<g, 256, 0, st>>>(p);
         else if (h->m == 2) k_grad_box<2><<<g, 256, 0, st>>>(p);
         else k_grad_box<0><<<g, 256, 0, st>>>(p);
+    } else if (h->plan.tma) {
+        TmaParams tp;
+        tp.g = p; tp.tiles = h->tiles; tp.ntiles = h->plan.ntiles; tp.cap_nz = h->plan.cap_nz; tp.cap_rows = h->plan.cap_rows;
+        tp.stages = h->plan.stages; tp.stage_bytes = h->plan.stage_bytes;
+        tp.nnz4 = h->nnz & ~3ll; tp.rows2 = (h->I + 1) & ~1ll;
+        void* args[] = {(void*)&tp};
+        CK(cudaLaunchKernel(h->plan.fn, dim3(h->plan.grid), dim3(32 * (kTmaConsumerWarps + 1)), args, h->plan.smem, st));
     } else {
         void* args[] = {(void*)&p};
         CK(cudaLaunchKernel(h->plan.fn, dim3(h->plan.grid), dim3(kBlockThreads), args, h->plan.smem, st));
@@ -317,7 +414,7 @@ void dualip_destroy(dualip_t* h) {
     if (h->own_rows) { cudaFree((void*)h->row_ptr); cudaFree((void*)h->idx); cudaFree((void*)h->a); }
     if (h->own_c) cudaFree((void*)h->c);
     cudaFree(h->b); cudaFree(h->s_fix); cudaFree(h->lam_cur); cudaFree(h->y); cudaFree(h->lam_stage);
-    cudaFree(h->grad_stage); cudaFree(h->scalars_dev); cudaFree(h->x_stage);
+    cudaFree(h->grad_stage); cudaFree(h->scalars_dev); cudaFree(h->x_stage); cudaFree(h->tiles);
     for (cudaEvent_t e : h->events) cudaEventDestroy(e);
     cudaGetLastError();
     delete h;
@@ -339,7 +436,8 @@ int dualip_create(dualip_t** out, int64_t I, int32_t J, int32_t m, const int64_t
     if ((long long)J * m > (1ll << 30)) return DUALIP_EINVAL;
     dualip_opts o;
     if (opts_in) o = *opts_in; else dualip_opts_default(&o);
-    for (int r = 0; r < 5; ++r) if (o.reserved[r] != 0) return DUALIP_EINVAL;
+    if (o.reserved[0] != 0 && o.reserved[0] != 1) return DUALIP_EINVAL;   // 1 = force the non-streaming kernel
+    for (int r = 1; r < 5; ++r) if (o.reserved[r] != 0) return DUALIP_EINVAL;
     switch (o.projection) {
         case DUALIP_PROJ_SIMPLEX_INEQ: case DUALIP_PROJ_SIMPLEX_EQ: if (!(o.p0 > 0.0)) return DUALIP_EINVAL; break;
         case DUALIP_PROJ_BOX: if (!(o.p0 <= o.p1)) return DUALIP_EINVAL; break;
@@ -429,6 +527,12 @@ int dualip_create(dualip_t** out, int64_t I, int32_t J, int32_t m, const int64_t
         set_xmax(h);
         set_scales(h);
         if ((rc = make_plan(h)) != 0) goto fail;
+        if (h->plan.tma) {
+            if ((rc = dev_alloc(h, &h->tiles, (size_t)h->plan.ntiles + 1)) != 0) goto fail;
+            k_build_tiles<<<grid_for(h->plan.ntiles + 1, 128, h->num_sms), 128, 0, st>>>(h->row_ptr, I, h->plan.TN, h->plan.ntiles, h->tiles);
+            h->launches++;
+            CKF(cudaGetLastError());
+        }
         CKF(cudaStreamSynchronize(st));
     }
     *out = h;
@@ -449,7 +553,8 @@ int dualip_get_info(dualip_t* h, dualip_info* info) {
     info->group_lanes = h->plan.G; info->chunk_regs = h->plan.KREG;
     info->reduction = h->plan.acc_smem ? DUALIP_RED_SMEM : DUALIP_RED_GLOBAL;
     info->lambda_in_smem = h->plan.lam_smem ? 1 : 0;
-    info->grid_ctas = h->plan.grid; info->block_threads = kBlockThreads;
+    info->grid_ctas = h->plan.grid; info->block_threads = h->plan.tma ? 32 * (kTmaConsumerWarps + 1) : kBlockThreads;
+    info->streaming = h->plan.tma ? 1 : 0; info->stages = h->plan.stages; info->tile_units = h->plan.TN; info->ntiles = h->plan.ntiles;
     info->smem_bytes = (int64_t)h->plan.smem;
     info->bytes_resident = h->bytes_resident; info->launches = h->launches;
     info->fix_scale_s = h->scale_s;

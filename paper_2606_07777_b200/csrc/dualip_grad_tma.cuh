@@ -1,0 +1,445 @@
+// dualip_grad_tma.cuh -- the streaming gradient kernel: a1-a5 with row data staged HBM -> shared memory by
+// TMA bulk copies (cp.async.bulk, SASS UBLKCP) behind mbarriers, one persistent CTA per SM.
+//
+//   warp 0      producer: for each of this CTA's tiles, waits for a free stage, then issues one bulk copy per
+//               array (item_idx, c, a, row_ptr segment) that completes on the stage's "full" mbarrier.
+//   warps 1..   consumers: wait for "full", claim row-steps of the tile from a shared counter (G lanes per row,
+//               32/G rows per step), read the rows straight from shared memory, and release the stage.
+//
+// Per row the consumers run a two-level scheme:
+//   fast path   fp32 filter: w' = fma(a, RN_f32(lambda_j), c) for every nonzero (one FFMA, one 4-byte gather),
+//               tracking the two largest values per row.  If the top-2 gap exceeds z*gamma by more than a
+//               rigorous rounding bound, x*_i is the vertex z*e_argmax capped by the inequality (min(z, v_max))
+//               and only the arg-max lane redoes its nonzero in fp64.  Likewise rows whose maximum is safely
+//               below zero are all-zero.  This is the common case at the small gamma the configs run at.
+//   slow path   every other row: whole warp, fp64 w, exact row-maximum shift, Michelot iterations in fp32 on
+//               the shifted values (or the capped search for box-cut with ub < z), re-reading the row from
+//               shared memory on every pass.
+//
+// A tile is a run of whole rows cut where (row_ptr[r] + kRowCost*r) crosses a multiple of TN (k_build_tiles at
+// create), so it holds at most TN + max_row_len nonzeros and TN/kRowCost + 1 rows whatever the row lengths
+// (empty rows included).  Tiles are dealt round-robin to CTAs.  Which warp takes which rows is dynamic, but every
+// accumulation (items AND scalars) is 64-bit fixed point, so results do not depend on it.
+//
+// Nothing here waits on DRAM latency: the only global loads in the loop are the producer's tile-table reads,
+// prefetched a tile ahead.
+#pragma once
+#include "dualip_kernels.cuh"
+
+namespace dualip_dev {
+
+constexpr int kRowCost = 8;            // each row costs this many "nonzero units" when cutting tiles
+constexpr int kTmaStagesMax = 4;
+
+struct TileEntry {                     // 32 bytes, one per tile (+1 sentinel)
+    long long row0;                    // first row of the tile
+    long long nz0;                     // row_ptr[row0]
+};
+
+struct TmaParams {
+    GradParams g;
+    const TileEntry* __restrict__ tiles;   // [ntiles + 1]
+    long long ntiles;
+    int cap_nz;                        // nonzero capacity of a stage (multiple of 4)
+    int cap_rows;                      // row_ptr entries per stage (even)
+    int stages;
+    int stage_bytes;                   // bytes of one stage (multiple of 16)
+    long long nnz4;                    // nnz rounded down to a multiple of 4 (bulk copies stop there)
+    long long rows2;                   // (I+1) rounded down to a multiple of 2
+};
+
+// ---- PTX wrappers (mbarrier + bulk async copy) ---------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(void* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(void* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(void* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(void* bar, unsigned parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_LOOP:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE;\n\t"
+        "bra WAIT_LOOP;\n\t"
+        "DONE:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, void* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+
+// One stage: [idx cap_nz*4][c cap_nz*4][a cap_nz*4*m][row_ptr cap_rows*8][meta 4*8]
+struct StageView {
+    const int* idx; const float* c; const float* a; const long long* rp; const long long* meta;
+};
+__device__ __forceinline__ StageView stage_view(unsigned char* base, int cap_nz, int cap_rows, int mm) {
+    StageView v;
+    v.idx = reinterpret_cast<const int*>(base);
+    v.c = reinterpret_cast<const float*>(base + (size_t)cap_nz * 4);
+    v.a = reinterpret_cast<const float*>(base + (size_t)cap_nz * 8);
+    v.rp = reinterpret_cast<const long long*>(base + (size_t)cap_nz * (8 + 4 * mm));
+    v.meta = v.rp + cap_rows;
+    return v;
+}
+
+// Shared state the row routines need.
+struct ConsumerCtx {
+    const float* lam_hi; const float* lam_lo;     // lambda = (double)hi + (double)lo, exact to 2^-48 relative
+    unsigned* acc_lo; unsigned* acc_hi;           // shared-memory item accumulators (ACC_SMEM)
+    long long obj_fix, sq_fix;                    // per-lane fixed-point partial scalars (order-independent)
+};
+
+// a4 + a5 for one nonzero with x != 0.
+template <int M, bool ACC_SMEM>
+__device__ __forceinline__ void push(const GradParams& p, ConsumerCtx& cx, int mm, int j, float cc, const float* aa, float x) {
+    cx.obj_fix += to_fix(cc * x, p.scale_obj);
+    cx.sq_fix += to_fix(x * x, p.scale_sq);
+#pragma unroll
+    for (int f = 0; f < (M > 0 ? M : 4); ++f) {
+        if (f < mm) {
+            const long long fx = to_fix(aa[f] * x, p.scale_s);
+            if (ACC_SMEM) fix_add_smem(cx.acc_lo + j * mm + f, cx.acc_hi + j * mm + f, fx);
+            else atomicAdd(p.s_fix + (long long)j * mm + f, (unsigned long long)fx);
+        }
+    }
+}
+
+// t = c + sum_f a_f * lambda[j,f] in fp64 for the staged nonzero q (w = -t).
+template <int M>
+__device__ __forceinline__ double exact_t(const StageView& v, const ConsumerCtx& cx, int mm, int q, int& j, float& cc, float* aa) {
+    j = v.idx[q];
+    cc = v.c[q];
+    double t = (double)cc;
+#pragma unroll
+    for (int f = 0; f < (M > 0 ? M : 4); ++f) {
+        aa[f] = 0.0f;
+        if (f < mm) {
+            aa[f] = v.a[q * mm + f];
+            const double l = (double)cx.lam_hi[j * mm + f] + (double)cx.lam_lo[j * mm + f];
+            t = fma((double)aa[f], l, t);
+        }
+    }
+    return t;
+}
+
+// Slow path: one row, whole warp, any length; every pass re-reads the staged row.  Same arithmetic as long_row()
+// in dualip_kernels.cuh (which documents the three box-cut steps).
+template <int M, bool ACC_SMEM, bool GBOX>
+__device__ __noinline__ void slow_row(const GradParams& p, const StageView v, ConsumerCtx& cx, int beg, int len, long long nzb) {
+    const int lane = threadIdx.x & 31;
+    const int mm = M > 0 ? M : p.m;
+    const int end = beg + len;
+    int j; float cc; float aa[M > 0 ? M : 4];
+    float wmax = -CUDART_INF_F;
+    for (int q = beg + lane; q < end; q += 32) wmax = fmaxf(wmax, (float)(-exact_t<M>(v, cx, mm, q, j, cc, aa)));
+    const float m32 = group_max<32>(wmax);
+    const bool ineq = p.proj != PROJ_SIMPLEX_EQ;
+    if (ineq && !(m32 > 0.0f)) {
+        if (p.x) for (int q = beg + lane; q < end; q += 32) p.x[nzb + q] = 0.0f;
+        return;
+    }
+    const double md = (double)m32;
+    const float mv = m32 * p.inv_gamma_f, z = p.z;
+    float tau;
+    double ref = 0.0;
+    if (!GBOX) {
+        float theta = -z - (1.2e-7f * fabsf(mv) + 1e-6f);
+        int n_prev = -1;
+        for (;;) {
+            float s = 0.0f; int n = 0;
+            for (int q = beg + lane; q < end; q += 32) {
+                const float u = (float)(-exact_t<M>(v, cx, mm, q, j, cc, aa) - md) * p.inv_gamma_f;
+                if (u > theta) { s += u; ++n; }
+            }
+            s = group_sum<32>(s); n = group_sum_i<32>(n);
+            if (n == n_prev || n == 0) break;
+            theta = fmaxf((s - z) / (float)n, theta);
+            n_prev = n;
+        }
+        tau = ineq ? fmaxf(theta, -mv) : theta;
+    } else {
+        const float ub = p.ub;
+        const double ig = p.inv_gamma;
+        float s0 = 0.0f;
+        for (int q = beg + lane; q < end; q += 32) s0 += fminf(fmaxf((float)(-exact_t<M>(v, cx, mm, q, j, cc, aa) * ig), 0.0f), ub);
+        s0 = group_sum<32>(s0);
+        if (s0 <= z) { ref = 0.0; tau = 0.0f; }
+        else {
+            float lo = -mv, hi = 1.2e-7f * fabsf(mv) + 1e-6f;
+            for (int it = 0; it < 36; ++it) {
+                const float mid = 0.5f * (lo + hi);
+                float s = 0.0f;
+                for (int q = beg + lane; q < end; q += 32) {
+                    const float u = (float)(-exact_t<M>(v, cx, mm, q, j, cc, aa) - md) * p.inv_gamma_f;
+                    s += fminf(fmaxf(u - mid, 0.0f), ub);
+                }
+                s = group_sum<32>(s);
+                if (s > z) lo = mid; else hi = mid;
+            }
+            const float tc = 0.5f * (lo + hi);
+            const float eps = (hi - lo) + 1e-6f + 4.8e-7f * fabsf(tc);
+            ref = md * ig + (double)tc;
+            float dlo = -eps, dhi = eps;
+            for (int it = 0; it < 26; ++it) {
+                const float mid = 0.5f * (dlo + dhi);
+                float s = 0.0f;
+                for (int q = beg + lane; q < end; q += 32) {
+                    const float u = (float)(-exact_t<M>(v, cx, mm, q, j, cc, aa) * ig - ref);
+                    s += fminf(fmaxf(u - mid, 0.0f), ub);
+                }
+                s = group_sum<32>(s);
+                if (s > z) dlo = mid; else dhi = mid;
+            }
+            const float mid = 0.5f * (dlo + dhi);
+            float sF = 0.0f; int nF = 0, nU = 0;
+            for (int q = beg + lane; q < end; q += 32) {
+                const float u = (float)(-exact_t<M>(v, cx, mm, q, j, cc, aa) * ig - ref);
+                const float d = u - mid;
+                if (d >= ub) ++nU; else if (d > 0.0f) { sF += u; ++nF; }
+            }
+            sF = group_sum<32>(sF); nF = group_sum_i<32>(nF); nU = group_sum_i<32>(nU);
+            tau = mid;
+            if (nF > 0) {
+                const float pol = (sF + (float)nU * ub - z) / (float)nF;
+                if (pol >= dlo && pol <= dhi) tau = pol;
+            }
+        }
+    }
+    const float cap = GBOX ? p.ub : CUDART_INF_F;
+    for (int q = beg + lane; q < end; q += 32) {
+        const double tq = exact_t<M>(v, cx, mm, q, j, cc, aa);
+        const float u = GBOX ? (float)(-tq * p.inv_gamma - ref) : (float)(-tq - md) * p.inv_gamma_f;
+        const float x = fminf(fmaxf(u - tau, 0.0f), cap);
+        if (p.x) p.x[nzb + q] = x;
+        if (x > 0.0f) push<M, ACC_SMEM>(p, cx, mm, j, cc, aa, x);
+    }
+}
+
+template <int G, int M, bool ACC_SMEM, bool GBOX, int NWC>
+__global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams tp) {
+    extern __shared__ __align__(128) unsigned char smem_tma[];
+    const GradParams& p = tp.g;
+    constexpr int MA = M > 0 ? M : 4;
+    constexpr int NT = 32 * (NWC + 1);
+    const int mm = M > 0 ? M : p.m;
+    const int JM = p.J * mm;
+    // layout: [full[4], empty[4] mbarriers: 64 B][claim counters: 64 B][lam_hi JM*4][lam_lo JM*4][acc 2*JM*4][stages]
+    unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_tma);
+    int* claim = reinterpret_cast<int*>(smem_tma + 64);
+    float* s_hi32 = reinterpret_cast<float*>(smem_tma + 128);
+    float* s_lo32 = s_hi32 + JM;
+    unsigned* a_lo = reinterpret_cast<unsigned*>(s_lo32 + JM);
+    unsigned* a_hi = a_lo + JM;
+    size_t off = 128 + (size_t)JM * 8 * (ACC_SMEM ? 2 : 1);
+    off = (off + 127) & ~(size_t)127;
+    unsigned char* stage0 = smem_tma + off;
+
+    for (int q = threadIdx.x; q < JM; q += NT) {
+        const double l = p.lambda[q];
+        const float h = (float)l;
+        s_hi32[q] = h;
+        s_lo32[q] = (float)(l - (double)h);
+    }
+    if (ACC_SMEM) for (int q = threadIdx.x; q < 2 * JM; q += NT) a_lo[q] = 0u;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < tp.stages; ++s) { mbar_init(&bars[s], 1); mbar_init(&bars[kTmaStagesMax + s], NWC); claim[s] = 0; }
+        fence_mbar_init();
+        fence_proxy_async();
+    }
+    __syncthreads();
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    ConsumerCtx cx{s_hi32, s_lo32, a_lo, a_hi, 0ll, 0ll};
+
+    if (warp == 0) {
+        // ================= producer =================
+        if (lane == 0) {
+            long long t = blockIdx.x;
+            TileEntry cur{0, 0}, nxt{0, 0};
+            if (t < tp.ntiles) { cur = tp.tiles[t]; nxt = tp.tiles[t + 1]; }
+            for (int it = 0; t < tp.ntiles; ++it, t += gridDim.x) {
+                const int s = it % tp.stages;
+                const unsigned ph = (unsigned)(it / tp.stages) & 1u;
+                const long long tn = t + gridDim.x;                                  // prefetch the next table entries
+                TileEntry ncur{0, 0}, nnxt{0, 0};
+                if (tn < tp.ntiles) { ncur = tp.tiles[tn]; nnxt = tp.tiles[tn + 1]; }
+                mbar_wait(&bars[kTmaStagesMax + s], ph ^ 1u);                        // stage free?
+                unsigned char* sb = stage0 + (size_t)s * tp.stage_bytes;
+                int* d_idx = reinterpret_cast<int*>(sb);
+                float* d_c = reinterpret_cast<float*>(sb + (size_t)tp.cap_nz * 4);
+                float* d_a = reinterpret_cast<float*>(sb + (size_t)tp.cap_nz * 8);
+                long long* d_rp = reinterpret_cast<long long*>(sb + (size_t)tp.cap_nz * (8 + 4 * mm));
+                long long* d_meta = d_rp + tp.cap_rows;
+                const long long r0 = cur.row0, r1 = nxt.row0, p0 = cur.nz0, p1 = nxt.nz0;
+                const long long p0a = p0 & ~3ll;
+                long long p1a = (p1 + 3) & ~3ll;
+                if (p1a > tp.nnz4) p1a = tp.nnz4 > p0a ? tp.nnz4 : p0a;              // never read past the arrays
+                const long long r0a = r0 & ~1ll;
+                long long r1a = (r1 + 2) & ~1ll;                                       // rows r0a .. r1 inclusive, even count
+                if (r1a > tp.rows2) r1a = tp.rows2 > r0a ? tp.rows2 : r0a;
+                d_meta[0] = r0; d_meta[1] = r1 - r0; d_meta[2] = p0a; d_meta[3] = r0a;
+                claim[s] = 0;
+                // tails that are not a whole 16-byte chunk (only at the very end of the arrays): plain copies
+                for (long long q = p1a > p0a ? p1a : p0a; q < p1; ++q) {
+                    d_idx[q - p0a] = p.idx[q]; d_c[q - p0a] = p.c[q];
+                    for (int f = 0; f < mm; ++f) d_a[(q - p0a) * mm + f] = p.a[q * mm + f];
+                }
+                for (long long r = r1a > r0a ? r1a : r0a; r <= r1; ++r) d_rp[r - r0a] = p.row_ptr[r];
+                const unsigned nz = (unsigned)(p1a > p0a ? p1a - p0a : 0), nr = (unsigned)(r1a > r0a ? r1a - r0a : 0);
+                mbar_expect_tx(&bars[s], nz * (8u + 4u * (unsigned)mm) + nr * 8u);     // release: meta/claim/tail stores
+                if (nz) {
+                    bulk_g2s(d_idx, p.idx + p0a, nz * 4u, &bars[s]);
+                    bulk_g2s(d_c, p.c + p0a, nz * 4u, &bars[s]);
+                    bulk_g2s(d_a, p.a + p0a * mm, nz * 4u * (unsigned)mm, &bars[s]);
+                }
+                if (nr) bulk_g2s(d_rp, p.row_ptr + r0a, nr * 8u, &bars[s]);
+                cur = ncur; nxt = nnxt;
+            }
+        }
+    } else {
+        // ================= consumers =================
+        constexpr int RPW = 32 / G;
+        const int gl = lane & (G - 1);
+        const bool ineq = p.proj != PROJ_SIMPLEX_EQ;
+        const float z = p.z;
+        const float gz = (float)((double)p.z / p.inv_gamma);            // z * gamma: the vertex gap in w units
+        int it = 0;
+        for (long long t = blockIdx.x; t < tp.ntiles; t += gridDim.x, ++it) {
+            const int s = it % tp.stages;
+            const unsigned ph = (unsigned)(it / tp.stages) & 1u;
+            mbar_wait(&bars[s], ph);
+            const StageView v = stage_view(stage0 + (size_t)s * tp.stage_bytes, tp.cap_nz, tp.cap_rows, mm);
+            const int nrows = (int)v.meta[1];
+            const long long nzb = v.meta[2];
+            const int rpo = (int)(v.meta[0] - v.meta[3]);
+            const int nsteps = (nrows + RPW - 1) / RPW;
+            for (;;) {
+                int st = 0;
+                if (lane == 0) st = atomicAdd(&claim[s], 1);
+                st = __shfl_sync(kFull, st, 0);
+                if (st >= nsteps) break;
+                const int lr = st * RPW + lane / G;
+                int beg = 0, len = 0;
+                if (lr < nrows) {
+                    const long long b = v.rp[rpo + lr], e = v.rp[rpo + lr + 1];
+                    beg = (int)(b - nzb); len = (int)(e - b);
+                }
+                unsigned slow_mask;
+                if (GBOX) {
+                    slow_mask = __ballot_sync(kFull, len > 0 && gl == 0);
+                } else {
+                    int nch = (len + G - 1) / G;
+#pragma unroll
+                    for (int o = G; o < 32; o <<= 1) nch = max(nch, __shfl_xor_sync(kFull, nch, o));
+                    // ---- fast path: fp32 filter, top-2 per row ----
+                    float m1 = -CUDART_INF_F, m2 = -CUDART_INF_F, bnd = 0.0f;
+                    int qb = beg;
+                    for (int k = 0; k < nch; ++k) {
+                        const int e = k * G + gl;
+                        const bool valid = e < len;
+                        const int q = beg + (valid ? e : 0);
+                        const int j = valid ? v.idx[q] : 0;
+                        const float cc = valid ? v.c[q] : 0.0f;
+                        float w = cc, ab = fabsf(cc);
+#pragma unroll
+                        for (int f = 0; f < MA; ++f) {
+                            if (f < mm) {
+                                const float af = valid ? v.a[q * mm + f] : 0.0f, lf = s_hi32[j * mm + f];
+                                if (M != 1) ab += fabsf(af * lf);
+                                w = fmaf(af, lf, w);
+                            }
+                        }
+                        // |w' - w| <= eps (|c| + sum_f |a_f lam_f|); for one family |a lam| <= |w'| + |c|
+                        bnd = fmaxf(bnd, ab);
+                        w = valid ? -w : -CUDART_INF_F;
+                        const bool gt = w > m1;
+                        m2 = gt ? m1 : fmaxf(m2, w);
+                        qb = gt ? q : qb;
+                        m1 = fmaxf(m1, w);
+                    }
+                    const float my1 = m1;
+#pragma unroll
+                    for (int o = G / 2; o > 0; o >>= 1) {
+                        const float o1 = __shfl_xor_sync(kFull, m1, o), o2 = __shfl_xor_sync(kFull, m2, o);
+                        m2 = fmaxf(fminf(m1, o1), fmaxf(m2, o2));
+                        m1 = fmaxf(m1, o1);
+                        bnd = fmaxf(bnd, __shfl_xor_sync(kFull, bnd, o));
+                    }
+                    // rounding bound of the filter: (m+1) roundings at 2^-24 plus lambda truncated to fp32 (2^-24
+                    // relative), each relative to at most B = |c| + sum|a lam| (M = 1: B <= 2|w'| + |c| for the two
+                    // values that matter); 2^-22 gives slack
+                    const float B = M == 1 ? 2.0f * fmaxf(fabsf(m1), fabsf(m2)) + bnd : bnd;
+                    const float tol = 2.4e-7f * (float)(mm + 1) * B + 1e-30f;
+                    const bool vertex = (m1 - m2) > gz + 2.0f * tol;        // also false for empty rows (inf - inf = NaN)
+                    const bool dead = ineq && m1 < -tol;
+                    const bool fast = len == 0 || vertex || dead;
+                    const bool owner = vertex && !dead && my1 == m1;
+                    float xo = 0.0f;
+                    if (owner) {
+                        // the unique arg-max lane: exact fp64 for its own nonzero, x = min(z, v_max) (or z)
+                        int j; float cc; float aa[MA];
+                        const double tq = exact_t<M>(v, cx, mm, qb, j, cc, aa);
+                        xo = ineq ? (float)fmin((double)z, -tq * p.inv_gamma) : z;
+                        if (xo > 0.0f) push<M, ACC_SMEM>(p, cx, mm, j, cc, aa, xo);
+                    }
+                    if (p.x && fast) {
+                        for (int e = gl; e < len; e += G) p.x[nzb + beg + e] = (owner && beg + e == qb && xo > 0.0f) ? xo : 0.0f;
+                    }
+                    slow_mask = __ballot_sync(kFull, !fast && gl == 0);
+                }
+                while (slow_mask) {
+                    const int src = __ffs(slow_mask) - 1;
+                    slow_mask &= slow_mask - 1;
+                    slow_row<M, ACC_SMEM, GBOX>(p, v, cx, __shfl_sync(kFull, beg, src), __shfl_sync(kFull, len, src), nzb);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bars[kTmaStagesMax + s]);           // this warp is done with the stage
+        }
+    }
+
+    {
+        long long so = cx.obj_fix, ss = cx.sq_fix;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) { so += __shfl_xor_sync(kFull, so, o); ss += __shfl_xor_sync(kFull, ss, o); }
+        if (lane == 0) {
+            if (so) atomicAdd(p.sc_fix + 0, (unsigned long long)so);
+            if (ss) atomicAdd(p.sc_fix + 1, (unsigned long long)ss);
+        }
+    }
+    if (ACC_SMEM) {
+        __syncthreads();
+        for (int q = threadIdx.x; q < JM; q += NT) {
+            const unsigned long long val = ((unsigned long long)a_hi[q] << 32) | a_lo[q];
+            if (val) atomicAdd(p.s_fix + q, val);
+        }
+    }
+}
+
+// a0: tile table.  Tile t starts at the first row r with row_ptr[r] + kRowCost*r >= t*TN (parallel binary search).
+__global__ void k_build_tiles(const long long* __restrict__ row_ptr, long long I, long long TN, long long ntiles, TileEntry* tiles) {
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t <= ntiles; t += (long long)gridDim.x * blockDim.x) {
+        long long r;
+        if (t == ntiles) r = I;
+        else {
+            const long long target = t * TN;
+            long long lo = 0, hi = I;                       // first r in [0,I] with key(r) >= target; key(I) >= target holds
+            while (lo < hi) {
+                const long long mid = (lo + hi) >> 1;
+                if (row_ptr[mid] + kRowCost * mid >= target) hi = mid; else lo = mid + 1;
+            }
+            r = lo;
+        }
+        tiles[t].row0 = r;
+        tiles[t].nz0 = row_ptr[r];
+    }
+}
+
+}  // namespace dualip_dev

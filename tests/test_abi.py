@@ -40,7 +40,7 @@ def test_struct_mirrors_match_the_header():
     assert (o.projection, o.p0, o.reduction, o.borrow, o.validate, o.momentum) == (0, 1.0, 0, 0, 1, 1)
     # C layout: int32, pad, 2 doubles, 7 int32 + 5 reserved int32 = 4+4+16+48 = 72 bytes
     assert ctypes.sizeof(pkg.Opts) == 72
-    assert ctypes.sizeof(pkg.Info) == 8 * 2 + 4 * 2 + 8 + 8 + 4 * 6 + 8 * 3 + 8 + 16
+    assert ctypes.sizeof(pkg.Info) == 8 * 2 + 4 * 2 + 8 + 8 + 4 * 6 + 8 * 3 + 8 + 16 + 24
     lib = pkg.load_library()
     assert lib.dualip_strerror(0) == b"ok" and lib.dualip_strerror(-3).startswith(b"duplicate")
 

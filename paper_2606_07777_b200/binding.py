@@ -61,7 +61,8 @@ class Info(ctypes.Structure):
 
 
 def lib_path() -> str:
-    return os.path.join(_HERE, "libdualip_b200.so")
+    """The in-tree library; DUALIP_B200_LIB overrides it (to load an experimental build variant)."""
+    return os.environ.get("DUALIP_B200_LIB") or os.path.join(_HERE, "libdualip_b200.so")
 
 
 _lib = None

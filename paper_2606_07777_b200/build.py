@@ -15,7 +15,7 @@ LIB = os.path.join(HERE, "libdualip_b200.so")
 SOURCES = ["dualip_api.cu"]
 HEADERS = ["dualip_kernels.cuh", "dualip_grad_tma.cuh", os.path.join("..", "..", "include", "dualip.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "-Xcompiler", "-fPIC,-O2,-Wall", "-shared", "--use_fast_math=false"]
+              "-Xcompiler", "-fPIC,-O2,-Wall", "-shared"]
 
 
 def _nvcc() -> str:
@@ -33,10 +33,16 @@ def is_stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, defines: dict | None = None, out: str | None = None) -> str:
+    """defines/out: build an experimental variant (e.g. {"DUALIP_NWC": 23}) next to the default library."""
+    if out is not None:
+        cmd = [_nvcc()] + NVCC_FLAGS + [f"-D{k}={v}" for k, v in (defines or {}).items()] + ["-o", out] + \
+              [os.path.join(CSRC, s) for s in SOURCES]
+        subprocess.check_call(cmd)
+        return out
     if not force and not is_stale():
         return LIB
-    flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
+    flags = list(NVCC_FLAGS)
     if verbose:
         flags += ["-Xptxas", "-v"]
     tmp = LIB + f".{os.getpid()}.tmp"

@@ -17,7 +17,10 @@ namespace {
 
 constexpr size_t kSmemBudget = 227 * 1024;  // bytes of dynamic shared memory one CTA may opt in to on sm_100a
 
-constexpr int kTmaConsumerWarps = 31;         // + 1 producer warp = 1024 threads per CTA
+#ifndef DUALIP_NWC
+#define DUALIP_NWC 15
+#endif
+constexpr int kTmaConsumerWarps = DUALIP_NWC;  // consumer warps of the streaming kernel (+ 1 producer warp)
 
 struct Plan {
     int G = 32, KREG = 5, M = 1;
@@ -136,6 +139,8 @@ const void* pick_tma_m(int M, bool acc, bool gbox) {
 }
 const void* pick_tma_kernel(const Plan& pl, bool gbox) {
     if (pl.M == 0) return pick_tma_acc<8, 0>(pl.acc_smem, gbox);
+    if (pl.G == 1) return pick_tma_m<1>(pl.M, pl.acc_smem, gbox);
+    if (pl.G == 2) return pick_tma_m<2>(pl.M, pl.acc_smem, gbox);
     if (pl.G == 4) return pick_tma_m<4>(pl.M, pl.acc_smem, gbox);
     if (pl.G == 8) return pick_tma_m<8>(pl.M, pl.acc_smem, gbox);
     if (pl.G == 16) return pick_tma_m<16>(pl.M, pl.acc_smem, gbox);
@@ -161,7 +166,7 @@ bool plan_tma(dualip* h, Plan& pl) {
     long long TN = 0; int stages = 0; size_t stage_bytes = 0;
     for (int S = 3; S >= 2 && TN < 256; --S) {
         stage_bytes = (avail / S) & ~(size_t)127;
-        const long long over = 80 + (h->max_row_len + 8) * (8 + 4 * m);
+        const long long over = 80 + (h->max_row_len + 8 + 32) * (8 + 4 * m);
         long long tn = ((long long)stage_bytes - over) / (9 + 4 * m);
         tn = tn > 0 ? (tn & ~63ll) : 0;
         if (tn >= (S == 3 ? 512 : 256)) { TN = tn; stages = S; }
@@ -173,7 +178,7 @@ bool plan_tma(dualip* h, Plan& pl) {
     if (TN > want) TN = want > 256 ? (want & ~63ll) : 256;
     pl.tma = true; pl.acc_smem = acc; pl.lam_smem = true;
     pl.TN = TN; pl.stages = stages;
-    pl.cap_nz = (int)((TN + h->max_row_len + 8 + 3) & ~3ll);
+    pl.cap_nz = (int)((TN + h->max_row_len + 8 + 32 + 3) & ~3ll);   // +32: lanes may read one chunk past a row end
     pl.cap_rows = (int)((TN / kRowCost + 6 + 1) & ~1ll);
     size_t sb = (size_t)pl.cap_nz * (8 + 4 * m) + (size_t)pl.cap_rows * 8 + 32;
     pl.stage_bytes = (int)((sb + 127) & ~(size_t)127);
@@ -197,12 +202,12 @@ int make_plan(dualip* h) {
     const double mean = h->I > 0 ? (double)h->nnz / (double)h->I : 0.0;
     int G = h->opts.group_lanes;
     if (G == 0) G = mean > 20.0 ? 32 : (mean > 10.0 ? 16 : 8);
-    if (G != 4 && G != 8 && G != 16 && G != 32) return DUALIP_EINVAL;
+    if (G != 1 && G != 2 && G != 4 && G != 8 && G != 16 && G != 32) return DUALIP_EINVAL;
     if (pl.M == 0) G = 32;
     if (h->opts.reserved[0] != 1 && plan_tma(h, pl)) {          // reserved[0] = 1 forces the non-streaming kernel (tests)
         // narrow lane groups: several rows share one pass of the chunk loop, which amortises the per-row work
         int Gs = h->opts.group_lanes;
-        if (Gs == 0) Gs = mean <= 12.0 ? 4 : (mean <= 128.0 ? 8 : (mean <= 512.0 ? 16 : 32));
+        if (Gs == 0) Gs = mean <= 160.0 ? 4 : (mean <= 640.0 ? 8 : (mean <= 2560.0 ? 16 : 32));
         if (pl.M == 0) Gs = 8;
         pl.G = Gs;
         pl.KREG = 0;
@@ -216,7 +221,7 @@ int make_plan(dualip* h) {
         return DUALIP_OK;
     }
     pl.tma = false;
-    if (G == 4) G = 8;
+    if (G < 8) G = 8;
     pl.acc_smem = (red == DUALIP_RED_AUTO || red == DUALIP_RED_SMEM) && fits_both;
     pl.lam_smem = pl.acc_smem || fits_lam;
     pl.G = G;

@@ -317,8 +317,8 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
             mbar_wait(&bars[s], ph);
             const StageView v = stage_view(stage0 + (size_t)s * tp.stage_bytes, tp.cap_nz, tp.cap_rows, mm);
             const int nrows = (int)v.meta[1];
-            const long long nzb = v.meta[2];
             const int rpo = (int)(v.meta[0] - v.meta[3]);
+            const int nzb32 = (int)v.meta[2];                            // low word is enough for local offsets
             const int nsteps = (nrows + RPW - 1) / RPW;
             for (;;) {
                 int st = 0;
@@ -328,8 +328,8 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                 const int lr = st * RPW + lane / G;
                 int beg = 0, len = 0;
                 if (lr < nrows) {
-                    const long long b = v.rp[rpo + lr], e = v.rp[rpo + lr + 1];
-                    beg = (int)(b - nzb); len = (int)(e - b);
+                    const int b = (int)v.rp[rpo + lr], e = (int)v.rp[rpo + lr + 1];   // differences fit in 32 bits
+                    beg = b - nzb32; len = e - b;
                 }
                 unsigned slow_mask;
                 if (GBOX) {
@@ -338,30 +338,44 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                     int nch = (len + G - 1) / G;
 #pragma unroll
                     for (int o = G; o < 32; o <<= 1) nch = max(nch, __shfl_xor_sync(kFull, nch, o));
-                    // ---- fast path: fp32 filter, top-2 per row ----
+                    // ---- fast path: fp32 filter, top-2 per row.  Lanes past the row end read whatever follows in
+                    // the stage buffer (it has G spare slots) and are masked: index -> 0, value -> -inf. ----
+                    const int* pi = v.idx + beg + gl;
+                    const float* pc = v.c + beg + gl;
+                    const float* pa = v.a + (beg + gl) * mm;
+                    const int rem = len - gl;                               // element k*G+gl is in the row iff k*G < rem
                     float m1 = -CUDART_INF_F, m2 = -CUDART_INF_F, bnd = 0.0f;
-                    int qb = beg;
+                    int kb = 0;
+#pragma unroll 4
                     for (int k = 0; k < nch; ++k) {
-                        const int e = k * G + gl;
-                        const bool valid = e < len;
-                        const int q = beg + (valid ? e : 0);
-                        const int j = valid ? v.idx[q] : 0;
-                        const float cc = valid ? v.c[q] : 0.0f;
+                        const bool valid = k * G < rem;
+                        int j = pi[k * G];
+                        float cc = pc[k * G];
+                        j = valid ? j : 0;
+                        cc = valid ? cc : 0.0f;
                         float w = cc, ab = fabsf(cc);
+                        if (M == 1) {
+                            w = fmaf(pa[k * G], s_hi32[j], w);
+                        } else if (M == 2) {
+                            const float2 a2 = *reinterpret_cast<const float2*>(pa + k * G * 2);
+                            const float2 l2 = *reinterpret_cast<const float2*>(s_hi32 + j * 2);
+                            ab += fabsf(a2.x * l2.x) + fabsf(a2.y * l2.y);
+                            w = fmaf(a2.y, l2.y, fmaf(a2.x, l2.x, w));
+                        } else {
 #pragma unroll
-                        for (int f = 0; f < MA; ++f) {
-                            if (f < mm) {
-                                const float af = valid ? v.a[q * mm + f] : 0.0f, lf = s_hi32[j * mm + f];
-                                if (M != 1) ab += fabsf(af * lf);
-                                w = fmaf(af, lf, w);
+                            for (int f = 0; f < MA; ++f) {
+                                if (f < mm) {
+                                    const float af = pa[k * G * mm + f], lf = s_hi32[j * mm + f];
+                                    ab += fabsf(af * lf);
+                                    w = fmaf(af, lf, w);
+                                }
                             }
                         }
-                        // |w' - w| <= eps (|c| + sum_f |a_f lam_f|); for one family |a lam| <= |w'| + |c|
                         bnd = fmaxf(bnd, ab);
                         w = valid ? -w : -CUDART_INF_F;
                         const bool gt = w > m1;
                         m2 = gt ? m1 : fmaxf(m2, w);
-                        qb = gt ? q : qb;
+                        kb = gt ? k : kb;
                         m1 = fmaxf(m1, w);
                     }
                     const float my1 = m1;
@@ -373,14 +387,16 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                         bnd = fmaxf(bnd, __shfl_xor_sync(kFull, bnd, o));
                     }
                     // rounding bound of the filter: (m+1) roundings at 2^-24 plus lambda truncated to fp32 (2^-24
-                    // relative), each relative to at most B = |c| + sum|a lam| (M = 1: B <= 2|w'| + |c| for the two
-                    // values that matter); 2^-22 gives slack
+                    // relative), each relative to at most B = |c| + sum|a lam| (M = 1: |a lam| <= |w'| + |c|, so
+                    // B <= 2|w'| + |c| for the two values that matter); 2^-22 gives slack.  A garbage (NaN) value
+                    // read past a row end can only reach `bnd` through a masked lane, which is zeroed above.
                     const float B = M == 1 ? 2.0f * fmaxf(fabsf(m1), fabsf(m2)) + bnd : bnd;
                     const float tol = 2.4e-7f * (float)(mm + 1) * B + 1e-30f;
-                    const bool vertex = (m1 - m2) > gz + 2.0f * tol;        // also false for empty rows (inf - inf = NaN)
+                    const bool vertex = (m1 - m2) > gz + 2.0f * tol;        // false for empty rows (inf - inf = NaN)
                     const bool dead = ineq && m1 < -tol;
                     const bool fast = len == 0 || vertex || dead;
                     const bool owner = vertex && !dead && my1 == m1;
+                    const int qb = beg + kb * G + gl;
                     float xo = 0.0f;
                     if (owner) {
                         // the unique arg-max lane: exact fp64 for its own nonzero, x = min(z, v_max) (or z)
@@ -390,6 +406,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                         if (xo > 0.0f) push<M, ACC_SMEM>(p, cx, mm, j, cc, aa, xo);
                     }
                     if (p.x && fast) {
+                        const long long nzb = v.meta[2];
                         for (int e = gl; e < len; e += G) p.x[nzb + beg + e] = (owner && beg + e == qb && xo > 0.0f) ? xo : 0.0f;
                     }
                     slow_mask = __ballot_sync(kFull, !fast && gl == 0);
@@ -397,7 +414,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                 while (slow_mask) {
                     const int src = __ffs(slow_mask) - 1;
                     slow_mask &= slow_mask - 1;
-                    slow_row<M, ACC_SMEM, GBOX>(p, v, cx, __shfl_sync(kFull, beg, src), __shfl_sync(kFull, len, src), nzb);
+                    slow_row<M, ACC_SMEM, GBOX>(p, v, cx, __shfl_sync(kFull, beg, src), __shfl_sync(kFull, len, src), v.meta[2]);
                 }
             }
             __syncwarp();

@@ -44,6 +44,8 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3")
     ap.add_argument("--users", type=int, default=None, help="override the number of users (smaller = not the graded workload)")
+    ap.add_argument("--group-lanes", type=int, default=0, help="lanes per row in the gradient kernel (0 = the library's choice)")
+    ap.add_argument("--grid-ctas", type=int, default=0, help="CTAs of the gradient kernel (0 = the library's choice)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-users", type=int, default=1_000_000, help="users in the oracle's bounded sample")
@@ -201,7 +203,7 @@ def main():
     kind, p0, p1 = synth.proj_spec(cfg)
     proj = {"simplex": pkg.PROJ_SIMPLEX_INEQ, "box": pkg.PROJ_BOX, "boxcut": pkg.PROJ_BOXCUT}[kind]
     gamma = cfg.gammas[-1]
-    opts = pkg.binding.make_opts(projection=proj, p0=p0, p1=p1, borrow=True)
+    opts = pkg.binding.make_opts(projection=proj, p0=p0, p1=p1, borrow=True, group_lanes=args.group_lanes, grid_ctas=args.grid_ctas)
     t0 = time.time()
     prob = pkg.Problem.create(inst.I, inst.J, inst.m, inst.row_ptr, inst.item_idx, inst.c, inst.a, inst.b, opts)
     torch.cuda.synchronize()
@@ -255,7 +257,7 @@ def main():
         barrier()
         t0 = time.perf_counter()
         p2 = pkg.Problem.create(inst.I, inst.J, inst.m, host["row_ptr"], host["item_idx"], host["c"], host["a"], host["b"],
-                                pkg.binding.make_opts(projection=proj, p0=p0, p1=p1))
+                                pkg.binding.make_opts(projection=proj, p0=p0, p1=p1, group_lanes=args.group_lanes, grid_ctas=args.grid_ctas))
         p2.solve([gamma], [args.steps], lam_h, scalars=sc)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0

@@ -207,7 +207,7 @@ int make_plan(dualip* h) {
     if (h->opts.reserved[0] != 1 && plan_tma(h, pl)) {          // reserved[0] = 1 forces the non-streaming kernel (tests)
         // narrow lane groups: several rows share one pass of the chunk loop, which amortises the per-row work
         int Gs = h->opts.group_lanes;
-        if (Gs == 0) Gs = mean <= 160.0 ? 4 : (mean <= 640.0 ? 8 : (mean <= 2560.0 ? 16 : 32));
+        if (Gs == 0) Gs = mean <= 6.0 ? 1 : (mean <= 12.0 ? 2 : (mean <= 24.0 ? 4 : (mean <= 256.0 ? 8 : (mean <= 1024.0 ? 16 : 32))));
         if (pl.M == 0) Gs = 8;
         pl.G = Gs;
         pl.KREG = 0;

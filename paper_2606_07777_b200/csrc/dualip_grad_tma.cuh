@@ -93,14 +93,14 @@ __device__ __forceinline__ StageView stage_view(unsigned char* base, int cap_nz,
 struct ConsumerCtx {
     const float* lam_hi; const float* lam_lo;     // lambda = (double)hi + (double)lo, exact to 2^-48 relative
     unsigned* acc_lo; unsigned* acc_hi;           // shared-memory item accumulators (ACC_SMEM)
-    long long obj_fix, sq_fix;                    // per-lane fixed-point partial scalars (order-independent)
 };
+struct FixPair { long long obj, sq; };            // per-lane fixed-point partial scalars (order-independent)
 
 // a4 + a5 for one nonzero with x != 0.
 template <int M, bool ACC_SMEM>
-__device__ __forceinline__ void push(const GradParams& p, ConsumerCtx& cx, int mm, int j, float cc, const float* aa, float x) {
-    cx.obj_fix += to_fix(cc * x, p.scale_obj);
-    cx.sq_fix += to_fix(x * x, p.scale_sq);
+__device__ __forceinline__ void push(const GradParams& p, const ConsumerCtx& cx, FixPair& fp, int mm, int j, float cc, const float* aa, float x) {
+    fp.obj += to_fix(cc * x, p.scale_obj);
+    fp.sq += to_fix(x * x, p.scale_sq);
 #pragma unroll
     for (int f = 0; f < (M > 0 ? M : 4); ++f) {
         if (f < mm) {
@@ -132,7 +132,8 @@ __device__ __forceinline__ double exact_t(const StageView& v, const ConsumerCtx&
 // Slow path: one row, whole warp, any length; every pass re-reads the staged row.  Same arithmetic as long_row()
 // in dualip_kernels.cuh (which documents the three box-cut steps).
 template <int M, bool ACC_SMEM, bool GBOX>
-__device__ __noinline__ void slow_row(const GradParams& p, const StageView v, ConsumerCtx& cx, int beg, int len, long long nzb) {
+__device__ __noinline__ FixPair slow_row(const GradParams& p, const StageView v, const ConsumerCtx cx, int beg, int len, long long nzb) {
+    FixPair fp{0ll, 0ll};                              // returned in registers: the caller's accumulators never live in local memory
     const int lane = threadIdx.x & 31;
     const int mm = M > 0 ? M : p.m;
     const int end = beg + len;
@@ -143,7 +144,7 @@ __device__ __noinline__ void slow_row(const GradParams& p, const StageView v, Co
     const bool ineq = p.proj != PROJ_SIMPLEX_EQ;
     if (ineq && !(m32 > 0.0f)) {
         if (p.x) for (int q = beg + lane; q < end; q += 32) p.x[nzb + q] = 0.0f;
-        return;
+        return fp;
     }
     const double md = (double)m32;
     const float mv = m32 * p.inv_gamma_f, z = p.z;
@@ -218,8 +219,9 @@ __device__ __noinline__ void slow_row(const GradParams& p, const StageView v, Co
         const float u = GBOX ? (float)(-tq * p.inv_gamma - ref) : (float)(-tq - md) * p.inv_gamma_f;
         const float x = fminf(fmaxf(u - tau, 0.0f), cap);
         if (p.x) p.x[nzb + q] = x;
-        if (x > 0.0f) push<M, ACC_SMEM>(p, cx, mm, j, cc, aa, x);
+        if (x > 0.0f) push<M, ACC_SMEM>(p, cx, fp, mm, j, cc, aa, x);
     }
+    return fp;
 }
 
 template <int G, int M, bool ACC_SMEM, bool GBOX, int NWC>
@@ -248,6 +250,12 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
         s_lo32[q] = (float)(l - (double)h);
     }
     if (ACC_SMEM) for (int q = threadIdx.x; q < 2 * JM; q += NT) a_lo[q] = 0u;
+    {   // consumers read whole 16-byte vectors around a row: every stage word must always hold a valid item index
+        uint4* sp = reinterpret_cast<uint4*>(stage0);
+        const int n16 = tp.stages * (tp.stage_bytes / 16);
+        for (int q = threadIdx.x; q < n16; q += NT) sp[q] = make_uint4(0u, 0u, 0u, 0u);
+        fence_proxy_async();                                             // generic-proxy zeros before the first bulk copy
+    }
     if (threadIdx.x == 0) {
         for (int s = 0; s < tp.stages; ++s) { mbar_init(&bars[s], 1); mbar_init(&bars[kTmaStagesMax + s], NWC); claim[s] = 0; }
         fence_mbar_init();
@@ -256,7 +264,8 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
     __syncthreads();
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    ConsumerCtx cx{s_hi32, s_lo32, a_lo, a_hi, 0ll, 0ll};
+    const ConsumerCtx cx{s_hi32, s_lo32, a_lo, a_hi};
+    FixPair fp{0ll, 0ll};
 
     if (warp == 0) {
         // ================= producer =================
@@ -305,8 +314,10 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
         }
     } else {
         // ================= consumers =================
-        constexpr int RPW = 32 / G;
-        const int gl = lane & (G - 1);
+        constexpr int GPW = 32 / G;                  // row groups per warp
+        constexpr int RPG = G >= 2 ? 2 : 1;          // rows a group takes per step (finalised together)
+        constexpr int RPW = GPW * RPG;               // rows per warp step
+        const int gl = lane & (G - 1), grp = lane / G;
         const bool ineq = p.proj != PROJ_SIMPLEX_EQ;
         const float z = p.z;
         const float gz = (float)((double)p.z / p.inv_gamma);            // z * gamma: the vertex gap in w units
@@ -325,96 +336,140 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                 if (lane == 0) st = atomicAdd(&claim[s], 1);
                 st = __shfl_sync(kFull, st, 0);
                 if (st >= nsteps) break;
-                const int lr = st * RPW + lane / G;
-                int beg = 0, len = 0;
-                if (lr < nrows) {
-                    const int b = (int)v.rp[rpo + lr], e = (int)v.rp[rpo + lr + 1];   // differences fit in 32 bits
-                    beg = b - nzb32; len = e - b;
-                }
-                unsigned slow_mask;
-                if (GBOX) {
-                    slow_mask = __ballot_sync(kFull, len > 0 && gl == 0);
-                } else {
-                    int nch = (len + G - 1) / G;
+                int rbeg[RPG], rlen[RPG];
+                float rm1[RPG], rm2[RPG], rbnd[RPG];
+                int rpos[RPG];
 #pragma unroll
-                    for (int o = G; o < 32; o <<= 1) nch = max(nch, __shfl_xor_sync(kFull, nch, o));
-                    // ---- fast path: fp32 filter, top-2 per row.  Lanes past the row end read whatever follows in
-                    // the stage buffer (it has G spare slots) and are masked: index -> 0, value -> -inf. ----
-                    const int* pi = v.idx + beg + gl;
-                    const float* pc = v.c + beg + gl;
-                    const float* pa = v.a + (beg + gl) * mm;
-                    const int rem = len - gl;                               // element k*G+gl is in the row iff k*G < rem
+                for (int r = 0; r < RPG; ++r) {
+                    const int lr = st * RPW + r * GPW + grp;
+                    int beg = 0, len = 0;
+                    if (lr < nrows) {
+                        const int b = (int)v.rp[rpo + lr], e = (int)v.rp[rpo + lr + 1];   // differences fit in 32 bits
+                        beg = b - nzb32; len = e - b;
+                    }
+                    rbeg[r] = beg; rlen[r] = len;
                     float m1 = -CUDART_INF_F, m2 = -CUDART_INF_F, bnd = 0.0f;
-                    int kb = 0;
-#pragma unroll 4
-                    for (int k = 0; k < nch; ++k) {
-                        const bool valid = k * G < rem;
-                        int j = pi[k * G];
-                        float cc = pc[k * G];
-                        j = valid ? j : 0;
-                        cc = valid ? cc : 0.0f;
-                        float w = cc, ab = fabsf(cc);
-                        if (M == 1) {
-                            w = fmaf(pa[k * G], s_hi32[j], w);
-                        } else if (M == 2) {
-                            const float2 a2 = *reinterpret_cast<const float2*>(pa + k * G * 2);
-                            const float2 l2 = *reinterpret_cast<const float2*>(s_hi32 + j * 2);
-                            ab += fabsf(a2.x * l2.x) + fabsf(a2.y * l2.y);
-                            w = fmaf(a2.y, l2.y, fmaf(a2.x, l2.x, w));
-                        } else {
+                    int pb = 0;
+                    if (!GBOX) {
+                        // ---- fp32 filter: the two largest w' = -(c + a.lambda_hi) of the row and where the largest sits.
+                        // Each lane takes 4 consecutive nonzeros per pass with 128-bit loads from the 16-byte aligned
+                        // position at or below the row start; the G lanes of a group cover 4G consecutive nonzeros (one
+                        // conflict-free 128-byte wavefront per array when G = 8).  Slots outside [beg, beg+len) hold
+                        // other rows' data (or zeros): their lambda index is in range, their value is masked to -inf.
+                        const int endp = beg + len;
+                        for (int q = (beg & ~3) + 4 * gl; q < endp; q += 4 * G) {
+                            const int4 j4 = *reinterpret_cast<const int4*>(v.idx + q);
+                            const float4 c4 = *reinterpret_cast<const float4*>(v.c + q);
+                            const int jj[4] = {j4.x, j4.y, j4.z, j4.w};
+                            const float cv[4] = {c4.x, c4.y, c4.z, c4.w};
+                            float wv[4], av[4];
+                            if (M == 1) {
+                                const float4 a4 = *reinterpret_cast<const float4*>(v.a + q);
+                                const float aa4[4] = {a4.x, a4.y, a4.z, a4.w};
 #pragma unroll
-                            for (int f = 0; f < MA; ++f) {
-                                if (f < mm) {
-                                    const float af = pa[k * G * mm + f], lf = s_hi32[j * mm + f];
-                                    ab += fabsf(af * lf);
-                                    w = fmaf(af, lf, w);
+                                for (int e = 0; e < 4; ++e) { wv[e] = -fmaf(aa4[e], s_hi32[jj[e]], cv[e]); av[e] = fabsf(cv[e]); }
+                            } else if (M == 2) {
+                                const float4 a01 = *reinterpret_cast<const float4*>(v.a + 2 * q);
+                                const float4 a23 = *reinterpret_cast<const float4*>(v.a + 2 * q + 4);
+                                const float ax[4] = {a01.x, a01.z, a23.x, a23.z}, ay[4] = {a01.y, a01.w, a23.y, a23.w};
+#pragma unroll
+                                for (int e = 0; e < 4; ++e) {
+                                    const float2 l2 = *reinterpret_cast<const float2*>(s_hi32 + 2 * jj[e]);
+                                    wv[e] = -fmaf(ay[e], l2.y, fmaf(ax[e], l2.x, cv[e]));
+                                    av[e] = fabsf(cv[e]) + fabsf(ax[e] * l2.x) + fabsf(ay[e] * l2.y);
+                                }
+                            } else {
+#pragma unroll
+                                for (int e = 0; e < 4; ++e) {
+                                    float w = cv[e], ab = fabsf(cv[e]);
+                                    for (int f = 0; f < mm; ++f) {
+                                        const float af = v.a[(q + e) * mm + f], lf = s_hi32[jj[e] * mm + f];
+                                        ab += fabsf(af * lf);
+                                        w = fmaf(af, lf, w);
+                                    }
+                                    wv[e] = -w; av[e] = ab;
                                 }
                             }
-                        }
-                        bnd = fmaxf(bnd, ab);
-                        w = valid ? -w : -CUDART_INF_F;
-                        const bool gt = w > m1;
-                        m2 = gt ? m1 : fmaxf(m2, w);
-                        kb = gt ? k : kb;
-                        m1 = fmaxf(m1, w);
-                    }
-                    const float my1 = m1;
 #pragma unroll
-                    for (int o = G / 2; o > 0; o >>= 1) {
-                        const float o1 = __shfl_xor_sync(kFull, m1, o), o2 = __shfl_xor_sync(kFull, m2, o);
-                        m2 = fmaxf(fminf(m1, o1), fmaxf(m2, o2));
-                        m1 = fmaxf(m1, o1);
-                        bnd = fmaxf(bnd, __shfl_xor_sync(kFull, bnd, o));
+                            for (int e = 0; e < 4; ++e) {
+                                const bool valid = (unsigned)(q + e - beg) < (unsigned)len;
+                                const float w = valid ? wv[e] : -CUDART_INF_F;
+                                bnd = fmaxf(bnd, av[e]);
+                                const bool gt = w > m1;
+                                m2 = gt ? m1 : fmaxf(m2, w);
+                                pb = gt ? q + e : pb;
+                                m1 = fmaxf(m1, w);
+                            }
+                        }
                     }
+                    rm1[r] = m1; rm2[r] = m2; rbnd[r] = bnd; rpos[r] = pb;
+                }
+                unsigned slow_mask;
+                int fbeg = 0, flen = 0;
+                if (GBOX) {
+#pragma unroll
+                    for (int r = 0; r < RPG; ++r) if (gl == r) { fbeg = rbeg[r]; flen = rlen[r]; }
+                    slow_mask = __ballot_sync(kFull, gl < RPG && flen > 0);
+                } else {
+                    // group reduction of (m1, m2, argmax position, bound); equal maxima in two lanes give m2 = m1
+#pragma unroll
+                    for (int r = 0; r < RPG; ++r) {
+#pragma unroll
+                        for (int o = G / 2; o > 0; o >>= 1) {
+                            const float o1 = __shfl_xor_sync(kFull, rm1[r], o), o2 = __shfl_xor_sync(kFull, rm2[r], o);
+                            const int op = __shfl_xor_sync(kFull, rpos[r], o);
+                            rbnd[r] = fmaxf(rbnd[r], __shfl_xor_sync(kFull, rbnd[r], o));
+                            const bool gt = o1 > rm1[r];
+                            rm2[r] = fmaxf(fminf(rm1[r], o1), fmaxf(rm2[r], o2));
+                            rpos[r] = gt ? op : rpos[r];
+                            rm1[r] = fmaxf(rm1[r], o1);
+                        }
+                    }
+                    // lane r of a group finalises the group's row r
+                    float m1 = rm1[0], m2 = rm2[0], bnd = rbnd[0];
+                    int fpos = rpos[0];
+                    fbeg = rbeg[0]; flen = rlen[0];
+#pragma unroll
+                    for (int r = 1; r < RPG; ++r) if (gl == r) { m1 = rm1[r]; m2 = rm2[r]; bnd = rbnd[r]; fpos = rpos[r]; fbeg = rbeg[r]; flen = rlen[r]; }
+                    const bool active = gl < RPG && flen > 0;
                     // rounding bound of the filter: (m+1) roundings at 2^-24 plus lambda truncated to fp32 (2^-24
-                    // relative), each relative to at most B = |c| + sum|a lam| (M = 1: |a lam| <= |w'| + |c|, so
-                    // B <= 2|w'| + |c| for the two values that matter); 2^-22 gives slack.  A garbage (NaN) value
-                    // read past a row end can only reach `bnd` through a masked lane, which is zeroed above.
-                    const float B = M == 1 ? 2.0f * fmaxf(fabsf(m1), fabsf(m2)) + bnd : bnd;
+                    // relative), each relative to at most B = |c| + sum|a lam| of that nonzero.  M = 1: |a lam| <=
+                    // |w'| + |c|, so B <= 2|w'| + max|c|; a value far below the top two has a larger bound but is
+                    // further away by more than that.  2^-22 gives slack.  `bnd` may include neighbouring rows' |c|
+                    // (the unmasked slots of the first and last pass): a larger bound only sends more rows to the
+                    // exact path.
+                    const float mag = fmaxf(fabsf(m1), m2 > -CUDART_INF_F ? fabsf(m2) : 0.0f);
+                    const float B = M == 1 ? 2.0f * mag + bnd : bnd;
                     const float tol = 2.4e-7f * (float)(mm + 1) * B + 1e-30f;
-                    const bool vertex = (m1 - m2) > gz + 2.0f * tol;        // false for empty rows (inf - inf = NaN)
+                    const bool vertex = (m1 - m2) > gz + 2.0f * tol;
                     const bool dead = ineq && m1 < -tol;
-                    const bool fast = len == 0 || vertex || dead;
-                    const bool owner = vertex && !dead && my1 == m1;
-                    const int qb = beg + kb * G + gl;
+                    const bool fast = vertex || dead;
                     float xo = 0.0f;
-                    if (owner) {
-                        // the unique arg-max lane: exact fp64 for its own nonzero, x = min(z, v_max) (or z)
+                    if (active && vertex && !dead) {
+                        // exact fp64 for the arg-max nonzero only: x = min(z, v_max) (or z for the equality simplex)
                         int j; float cc; float aa[MA];
-                        const double tq = exact_t<M>(v, cx, mm, qb, j, cc, aa);
-                        xo = ineq ? (float)fmin((double)z, -tq * p.inv_gamma) : z;
-                        if (xo > 0.0f) push<M, ACC_SMEM>(p, cx, mm, j, cc, aa, xo);
+                        const double tq = exact_t<M>(v, cx, mm, fpos, j, cc, aa);
+                        xo = ineq ? fmaxf((float)fmin((double)z, -tq * p.inv_gamma), 0.0f) : z;
+                        if (xo > 0.0f) push<M, ACC_SMEM>(p, cx, fp, mm, j, cc, aa, xo);
                     }
-                    if (p.x && fast) {
+                    if (p.x) {
                         const long long nzb = v.meta[2];
-                        for (int e = gl; e < len; e += G) p.x[nzb + beg + e] = (owner && beg + e == qb && xo > 0.0f) ? xo : 0.0f;
+#pragma unroll
+                        for (int r = 0; r < RPG; ++r) {
+                            const int src = (lane & ~(G - 1)) + r;
+                            const bool fr = __shfl_sync(kFull, (int)(active && fast), src) != 0;
+                            const float xr = __shfl_sync(kFull, xo, src);
+                            const int pr = __shfl_sync(kFull, fpos, src);
+                            if (fr) for (int e = gl; e < rlen[r]; e += G) p.x[nzb + rbeg[r] + e] = (rbeg[r] + e == pr) ? xr : 0.0f;
+                        }
                     }
-                    slow_mask = __ballot_sync(kFull, !fast && gl == 0);
+                    slow_mask = __ballot_sync(kFull, active && !fast);
                 }
                 while (slow_mask) {
                     const int src = __ffs(slow_mask) - 1;
                     slow_mask &= slow_mask - 1;
-                    slow_row<M, ACC_SMEM, GBOX>(p, v, cx, __shfl_sync(kFull, beg, src), __shfl_sync(kFull, len, src), v.meta[2]);
+                    const FixPair sp = slow_row<M, ACC_SMEM, GBOX>(p, v, cx, __shfl_sync(kFull, fbeg, src), __shfl_sync(kFull, flen, src), v.meta[2]);
+                    fp.obj += sp.obj; fp.sq += sp.sq;
                 }
             }
             __syncwarp();
@@ -423,7 +478,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
     }
 
     {
-        long long so = cx.obj_fix, ss = cx.sq_fix;
+        long long so = fp.obj, ss = fp.sq;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) { so += __shfl_xor_sync(kFull, so, o); ss += __shfl_xor_sync(kFull, ss, o); }
         if (lane == 0) {

@@ -94,8 +94,8 @@ double fix_scale(double bound) {
     int e = 0;
     std::frexp(bound, &e);
     int s = 61 - e;
-    if (s > 1000) s = 1000;
-    if (s < -1000) s = -1000;
+    if (s > 96) s = 96;       // keeps the scale (and value * scale for fp32 values below 2^31) inside fp32 range
+    if (s < -96) s = -96;
     return std::ldexp(1.0, s);
 }
 
@@ -323,6 +323,7 @@ void fill_grad_params(const dualip* h, GradParams& p, const double* lam_dev, dou
         default: p.z = (float)o.p0; break;
     }
     p.scale_s = h->scale_s; p.scale_obj = h->scale_obj; p.scale_sq = h->scale_sq;
+    p.scale_s_f = (float)h->scale_s; p.scale_obj_f = (float)h->scale_obj; p.scale_sq_f = (float)h->scale_sq;
 }
 
 constexpr size_t kMaxTimedLaunches = 4096;

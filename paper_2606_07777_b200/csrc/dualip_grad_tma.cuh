@@ -75,9 +75,10 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned by
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
-// One stage: [idx cap_nz*4][c cap_nz*4][a cap_nz*4*m][row_ptr cap_rows*8][meta 4*8]
+// One stage: [idx cap_nz*4][c cap_nz*4][a cap_nz*4*m][row_ptr cap_rows*8][meta: int nrows, int rpo, long long nzb, pad]
+struct StageMeta { int nrows; int rpo; long long nzb; long long pad[2]; };
 struct StageView {
-    const int* idx; const float* c; const float* a; const long long* rp; const long long* meta;
+    const int* idx; const float* c; const float* a; const long long* rp; const StageMeta* meta;
 };
 __device__ __forceinline__ StageView stage_view(unsigned char* base, int cap_nz, int cap_rows, int mm) {
     StageView v;
@@ -85,7 +86,7 @@ __device__ __forceinline__ StageView stage_view(unsigned char* base, int cap_nz,
     v.c = reinterpret_cast<const float*>(base + (size_t)cap_nz * 4);
     v.a = reinterpret_cast<const float*>(base + (size_t)cap_nz * 8);
     v.rp = reinterpret_cast<const long long*>(base + (size_t)cap_nz * (8 + 4 * mm));
-    v.meta = v.rp + cap_rows;
+    v.meta = reinterpret_cast<const StageMeta*>(v.rp + cap_rows);
     return v;
 }
 
@@ -96,17 +97,27 @@ struct ConsumerCtx {
 };
 struct FixPair { long long obj, sq; };            // per-lane fixed-point partial scalars (order-independent)
 
+// v * 2^k as a 64-bit integer.  The scales are powers of two within fp32 range (dualip_api.cu clamps the exponent), so
+// the product is exact and this equals to_fix(v, (double)scale) of dualip_kernels.cuh: one FMUL + one F2I.
+__device__ __forceinline__ long long to_fix32(float v, float scale) { return __float2ll_rn(v * scale); }
+
+// RED.ADD.64 on a pointer known to be global memory (a generic atomicAdd makes ptxas emit an address-space check, a
+// shared-memory CAS loop and a predicate that the caller then waits on).
+__device__ __forceinline__ void red_add_u64(unsigned long long* gptr, unsigned long long v) {
+    asm volatile("red.global.add.u64 [%0], %1;" ::"l"(gptr), "l"(v) : "memory");
+}
+
 // a4 + a5 for one nonzero with x != 0.
 template <int M, bool ACC_SMEM>
 __device__ __forceinline__ void push(const GradParams& p, const ConsumerCtx& cx, FixPair& fp, int mm, int j, float cc, const float* aa, float x) {
-    fp.obj += to_fix(cc * x, p.scale_obj);
-    fp.sq += to_fix(x * x, p.scale_sq);
+    fp.obj += to_fix32(cc * x, p.scale_obj_f);
+    fp.sq += to_fix32(x * x, p.scale_sq_f);
 #pragma unroll
     for (int f = 0; f < (M > 0 ? M : 4); ++f) {
         if (f < mm) {
-            const long long fx = to_fix(aa[f] * x, p.scale_s);
+            const long long fx = to_fix32(aa[f] * x, p.scale_s_f);
             if (ACC_SMEM) fix_add_smem(cx.acc_lo + j * mm + f, cx.acc_hi + j * mm + f, fx);
-            else atomicAdd(p.s_fix + (long long)j * mm + f, (unsigned long long)fx);
+            else red_add_u64(p.s_fix + (long long)j * mm + f, (unsigned long long)fx);
         }
     }
 }
@@ -273,9 +284,9 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
             long long t = blockIdx.x;
             TileEntry cur{0, 0}, nxt{0, 0};
             if (t < tp.ntiles) { cur = tp.tiles[t]; nxt = tp.tiles[t + 1]; }
-            for (int it = 0; t < tp.ntiles; ++it, t += gridDim.x) {
-                const int s = it % tp.stages;
-                const unsigned ph = (unsigned)(it / tp.stages) & 1u;
+            int s = 0;
+            unsigned ph = 0;
+            for (; t < tp.ntiles; t += gridDim.x) {
                 const long long tn = t + gridDim.x;                                  // prefetch the next table entries
                 TileEntry ncur{0, 0}, nnxt{0, 0};
                 if (tn < tp.ntiles) { ncur = tp.tiles[tn]; nnxt = tp.tiles[tn + 1]; }
@@ -285,7 +296,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                 float* d_c = reinterpret_cast<float*>(sb + (size_t)tp.cap_nz * 4);
                 float* d_a = reinterpret_cast<float*>(sb + (size_t)tp.cap_nz * 8);
                 long long* d_rp = reinterpret_cast<long long*>(sb + (size_t)tp.cap_nz * (8 + 4 * mm));
-                long long* d_meta = d_rp + tp.cap_rows;
+                StageMeta* d_meta = reinterpret_cast<StageMeta*>(d_rp + tp.cap_rows);
                 const long long r0 = cur.row0, r1 = nxt.row0, p0 = cur.nz0, p1 = nxt.nz0;
                 const long long p0a = p0 & ~3ll;
                 long long p1a = (p1 + 3) & ~3ll;
@@ -293,7 +304,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                 const long long r0a = r0 & ~1ll;
                 long long r1a = (r1 + 2) & ~1ll;                                       // rows r0a .. r1 inclusive, even count
                 if (r1a > tp.rows2) r1a = tp.rows2 > r0a ? tp.rows2 : r0a;
-                d_meta[0] = r0; d_meta[1] = r1 - r0; d_meta[2] = p0a; d_meta[3] = r0a;
+                d_meta->nrows = (int)(r1 - r0); d_meta->rpo = (int)(r0 - r0a); d_meta->nzb = p0a;
                 claim[s] = 0;
                 // tails that are not a whole 16-byte chunk (only at the very end of the arrays): plain copies
                 for (long long q = p1a > p0a ? p1a : p0a; q < p1; ++q) {
@@ -310,6 +321,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                 }
                 if (nr) bulk_g2s(d_rp, p.row_ptr + r0a, nr * 8u, &bars[s]);
                 cur = ncur; nxt = nnxt;
+                if (++s == tp.stages) { s = 0; ph ^= 1u; }
             }
         }
     } else {
@@ -317,25 +329,27 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
         constexpr int GPW = 32 / G;                  // row groups per warp
         constexpr int RPG = G >= 2 ? 2 : 1;          // rows a group takes per step (finalised together)
         constexpr int RPW = GPW * RPG;               // rows per warp step
+        constexpr int HG = G >= 2 ? G / 2 : 1;
         const int gl = lane & (G - 1), grp = lane / G;
         const bool ineq = p.proj != PROJ_SIMPLEX_EQ;
         const float z = p.z;
         const float gz = (float)((double)p.z / p.inv_gamma);            // z * gamma: the vertex gap in w units
-        int it = 0;
-        for (long long t = blockIdx.x; t < tp.ntiles; t += gridDim.x, ++it) {
-            const int s = it % tp.stages;
-            const unsigned ph = (unsigned)(it / tp.stages) & 1u;
+        const bool upper = RPG == 2 && (gl & HG) != 0;                   // this lane ends up holding the group's row 1
+        const bool fin = RPG == 2 ? (gl & (HG - 1)) == 0 : true;        // lanes 0 and G/2 of a group finalise rows 0 and 1
+        int s = 0;
+        unsigned ph = 0;
+        for (long long t = blockIdx.x; t < tp.ntiles; t += gridDim.x) {
             mbar_wait(&bars[s], ph);
-            const StageView v = stage_view(stage0 + (size_t)s * tp.stage_bytes, tp.cap_nz, tp.cap_rows, mm);
-            const int nrows = (int)v.meta[1];
-            const int rpo = (int)(v.meta[0] - v.meta[3]);
-            const int nzb32 = (int)v.meta[2];                            // low word is enough for local offsets
+            const StageView v = stage_view(stage0 + s * tp.stage_bytes, tp.cap_nz, tp.cap_rows, mm);
+            const int nrows = v.meta->nrows;
             const int nsteps = (nrows + RPW - 1) / RPW;
             for (;;) {
                 int st = 0;
                 if (lane == 0) st = atomicAdd(&claim[s], 1);
                 st = __shfl_sync(kFull, st, 0);
                 if (st >= nsteps) break;
+                const int rpo = v.meta->rpo;
+                const int nzb32 = (int)v.meta->nzb;                       // low word is enough for local offsets
                 int rbeg[RPG], rlen[RPG];
                 float rm1[RPG], rm2[RPG], rbnd[RPG];
                 int rpos[RPG];
@@ -405,33 +419,43 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                     rm1[r] = m1; rm2[r] = m2; rbnd[r] = bnd; rpos[r] = pb;
                 }
                 unsigned slow_mask;
-                int fbeg = 0, flen = 0;
+                int fbeg = rbeg[0], flen = rlen[0];
+                if (RPG == 2 && upper) { fbeg = rbeg[RPG - 1]; flen = rlen[RPG - 1]; }
+                const bool active = fin && flen > 0;
                 if (GBOX) {
-#pragma unroll
-                    for (int r = 0; r < RPG; ++r) if (gl == r) { fbeg = rbeg[r]; flen = rlen[r]; }
-                    slow_mask = __ballot_sync(kFull, gl < RPG && flen > 0);
+                    slow_mask = __ballot_sync(kFull, active);
                 } else {
-                    // group reduction of (m1, m2, argmax position, bound); equal maxima in two lanes give m2 = m1
-#pragma unroll
-                    for (int r = 0; r < RPG; ++r) {
-#pragma unroll
-                        for (int o = G / 2; o > 0; o >>= 1) {
-                            const float o1 = __shfl_xor_sync(kFull, rm1[r], o), o2 = __shfl_xor_sync(kFull, rm2[r], o);
-                            const int op = __shfl_xor_sync(kFull, rpos[r], o);
-                            rbnd[r] = fmaxf(rbnd[r], __shfl_xor_sync(kFull, rbnd[r], o));
-                            const bool gt = o1 > rm1[r];
-                            rm2[r] = fmaxf(fminf(rm1[r], o1), fmaxf(rm2[r], o2));
-                            rpos[r] = gt ? op : rpos[r];
-                            rm1[r] = fmaxf(rm1[r], o1);
-                        }
-                    }
-                    // lane r of a group finalises the group's row r
+                    // group reduction of (m1, m2, argmax position, bound).  With two rows per group the first exchange
+                    // is a transposition: the lower half of the group keeps row 0 and hands over its part of row 1,
+                    // the upper half the reverse; the remaining levels then run on both rows at once.  Equal maxima in
+                    // two lanes give m2 = m1 (no vertex).
                     float m1 = rm1[0], m2 = rm2[0], bnd = rbnd[0];
                     int fpos = rpos[0];
-                    fbeg = rbeg[0]; flen = rlen[0];
+                    if (RPG == 2) {
+                        float g1 = rm1[RPG - 1], g2 = rm2[RPG - 1], gb = rbnd[RPG - 1];
+                        int gp = rpos[RPG - 1];
+                        if (upper) {
+                            float tf; int ti;
+                            tf = m1; m1 = g1; g1 = tf; tf = m2; m2 = g2; g2 = tf; tf = bnd; bnd = gb; gb = tf; ti = fpos; fpos = gp; gp = ti;
+                        }
+                        const float o1 = __shfl_xor_sync(kFull, g1, HG), o2 = __shfl_xor_sync(kFull, g2, HG);
+                        const int op = __shfl_xor_sync(kFull, gp, HG);
+                        bnd = fmaxf(bnd, __shfl_xor_sync(kFull, gb, HG));
+                        const bool gt = o1 > m1;
+                        m2 = fmaxf(fminf(m1, o1), fmaxf(m2, o2));
+                        fpos = gt ? op : fpos;
+                        m1 = fmaxf(m1, o1);
+                    }
 #pragma unroll
-                    for (int r = 1; r < RPG; ++r) if (gl == r) { m1 = rm1[r]; m2 = rm2[r]; bnd = rbnd[r]; fpos = rpos[r]; fbeg = rbeg[r]; flen = rlen[r]; }
-                    const bool active = gl < RPG && flen > 0;
+                    for (int o = HG / 2; o > 0; o >>= 1) {
+                        const float o1 = __shfl_xor_sync(kFull, m1, o), o2 = __shfl_xor_sync(kFull, m2, o);
+                        const int op = __shfl_xor_sync(kFull, fpos, o);
+                        bnd = fmaxf(bnd, __shfl_xor_sync(kFull, bnd, o));
+                        const bool gt = o1 > m1;
+                        m2 = fmaxf(fminf(m1, o1), fmaxf(m2, o2));
+                        fpos = gt ? op : fpos;
+                        m1 = fmaxf(m1, o1);
+                    }
                     // rounding bound of the filter: (m+1) roundings at 2^-24 plus lambda truncated to fp32 (2^-24
                     // relative), each relative to at most B = |c| + sum|a lam| of that nonzero.  M = 1: |a lam| <=
                     // |w'| + |c|, so B <= 2|w'| + max|c|; a value far below the top two has a larger bound but is
@@ -446,17 +470,17 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                     const bool fast = vertex || dead;
                     float xo = 0.0f;
                     if (active && vertex && !dead) {
-                        // exact fp64 for the arg-max nonzero only: x = min(z, v_max) (or z for the equality simplex)
+                        // exact fp64 for the arg-max nonzero only: x = clamp(v_max, 0, z) (or z for the equality simplex)
                         int j; float cc; float aa[MA];
                         const double tq = exact_t<M>(v, cx, mm, fpos, j, cc, aa);
                         xo = ineq ? fmaxf((float)fmin((double)z, -tq * p.inv_gamma), 0.0f) : z;
                         if (xo > 0.0f) push<M, ACC_SMEM>(p, cx, fp, mm, j, cc, aa, xo);
                     }
                     if (p.x) {
-                        const long long nzb = v.meta[2];
+                        const long long nzb = v.meta->nzb;
 #pragma unroll
                         for (int r = 0; r < RPG; ++r) {
-                            const int src = (lane & ~(G - 1)) + r;
+                            const int src = (lane & ~(G - 1)) + r * HG;
                             const bool fr = __shfl_sync(kFull, (int)(active && fast), src) != 0;
                             const float xr = __shfl_sync(kFull, xo, src);
                             const int pr = __shfl_sync(kFull, fpos, src);
@@ -468,12 +492,13 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                 while (slow_mask) {
                     const int src = __ffs(slow_mask) - 1;
                     slow_mask &= slow_mask - 1;
-                    const FixPair sp = slow_row<M, ACC_SMEM, GBOX>(p, v, cx, __shfl_sync(kFull, fbeg, src), __shfl_sync(kFull, flen, src), v.meta[2]);
+                    const FixPair sp = slow_row<M, ACC_SMEM, GBOX>(p, v, cx, __shfl_sync(kFull, fbeg, src), __shfl_sync(kFull, flen, src), v.meta->nzb);
                     fp.obj += sp.obj; fp.sq += sp.sq;
                 }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&bars[kTmaStagesMax + s]);           // this warp is done with the stage
+            if (++s == tp.stages) { s = 0; ph ^= 1u; }
         }
     }
 

@@ -48,6 +48,7 @@ struct GradParams {
     double inv_gamma;
     double box_lo, box_hi;
     double scale_s, scale_obj, scale_sq;
+    float scale_s_f, scale_obj_f, scale_sq_f;   // the same powers of two as floats (streaming kernel: one FMUL + F2I)
 };
 
 __device__ __forceinline__ long long to_fix(float v, double scale) { return __double2ll_rn((double)v * scale); }

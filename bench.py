@@ -33,7 +33,7 @@ if ROOT not in sys.path:
 METRIC = "dual-ascent nonzeros/s (nnz x AGD iterations/s), fused gradient iteration"
 UNIT = "nnz/s"
 # DRAM bytes per k_grad launch from the committed `ncu --set full` capture (profiles/), or None until one exists.
-NCU_TRAFFIC_BYTES = {"cfg3": None}
+NCU_TRAFFIC_BYTES = {"cfg3": 6.102162e9 + 20.486912e6}   # profiles/r01b_cfg3_k_grad_tma_full.csv, launch 0
 
 
 def parse_args():

@@ -225,19 +225,28 @@ def generate(cfg: Config | str, device="cpu", chunk_users: int = 500_000) -> Ins
         cfg = get_config(cfg)
     device = torch.device(device)
     tables = _item_tables(cfg, device)
-    degs, items, cs, as_ = [], [], [], []
-    short = 0
+    # the drawn degrees bound the realised ones, so the outputs can be allocated once and filled chunk by chunk
+    # (config 4 is 80 GB of row data: concatenating per-chunk pieces would need twice that)
+    cap = 0
+    for u0 in range(0, cfg.I, chunk_users):
+        users = torch.arange(u0, min(cfg.I, u0 + chunk_users), dtype=torch.int64, device=device)
+        cap += int(torch.clamp(_degrees(cfg, users), max=cfg.J).sum())
+    item_idx = torch.empty(cap, dtype=torch.int32, device=device)
+    c = torch.empty(cap, dtype=torch.float32, device=device)
+    a = torch.empty(cap * cfg.m, dtype=torch.float32, device=device)
+    row_ptr = torch.zeros(cfg.I + 1, dtype=torch.int64, device=device)
+    short, pos = 0, 0
     for u0 in range(0, cfg.I, chunk_users):
         u1 = min(cfg.I, u0 + chunk_users)
         d, it, usr, sh = _rows_chunk(cfg, u0, u1, device, tables)
-        c, a = _values(cfg, usr, it)
-        degs.append(d); items.append(it); cs.append(c); as_.append(a)
+        cc, aa = _values(cfg, usr, it)
+        n = int(it.numel())
+        item_idx[pos:pos + n] = it; c[pos:pos + n] = cc; a[pos * cfg.m:(pos + n) * cfg.m] = aa
+        row_ptr[u0 + 1:u1 + 1] = torch.cumsum(d, 0) + pos
+        pos += n
         short += sh
-    deg = torch.cat(degs)
-    row_ptr = torch.zeros(cfg.I + 1, dtype=torch.int64, device=device)
-    torch.cumsum(deg, 0, out=row_ptr[1:])
-    item_idx, c, a = torch.cat(items), torch.cat(cs), torch.cat(as_)
-    del degs, items, cs, as_
+        del d, it, usr, cc, aa
+    item_idx, c, a = item_idx[:pos], c[:pos], a[:pos * cfg.m]
     inst = Instance(cfg, row_ptr, item_idx, c, a, torch.empty(0), short_rows=short)
     inst.b = make_rhs(inst)
     return inst
@@ -254,13 +263,17 @@ def make_rhs(inst: Instance) -> torch.Tensor:
     item), rho ~ U[0.5,1], eps = 1e-6 -- the paper's own rule for binding constraints."""
     cfg, dev = inst.cfg, inst.c.device
     J, m = cfg.J, cfg.m
-    a = inst.a.reshape(-1, m).to(torch.float64)
-    j = inst.item_idx.to(torch.int64)
     b = torch.zeros(J, m, dtype=torch.float64, device=dev)
     if cfg.rhs == "kappa":
-        b.index_add_(0, j, a)
+        step = 1 << 26                                             # in pieces: config 4 has 5e9 nonzeros
+        a2 = inst.a.reshape(-1, m)
+        for p0 in range(0, inst.nnz, step):
+            p1 = min(inst.nnz, p0 + step)
+            b.index_add_(0, inst.item_idx[p0:p1].to(torch.int64), a2[p0:p1].to(torch.float64))
         b *= torch.tensor(cfg.kappa, dtype=torch.float64, device=dev)
     elif cfg.rhs == "greedy":
+        a = inst.a.reshape(-1, m).to(torch.float64)
+        j = inst.item_idx.to(torch.int64)
         usr = _segment_user(inst)
         for k in range(m):
             rowmax = torch.full((inst.I,), -math.inf, dtype=torch.float64, device=dev)

@@ -46,6 +46,8 @@ def parse_args():
     ap.add_argument("--users", type=int, default=None, help="override the number of users (smaller = not the graded workload)")
     ap.add_argument("--group-lanes", type=int, default=0, help="lanes per row in the gradient kernel (0 = the library's choice)")
     ap.add_argument("--grid-ctas", type=int, default=0, help="CTAs of the gradient kernel (0 = the library's choice)")
+    ap.add_argument("--graph", action="store_true", help="dualip_solve replays a CUDA graph of chained iteration launches "
+                    "(small, launch-bound workloads); the per-launch kernel timing hook is then off")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-users", type=int, default=1_000_000, help="users in the oracle's bounded sample")
@@ -203,7 +205,8 @@ def main():
     kind, p0, p1 = synth.proj_spec(cfg)
     proj = {"simplex": pkg.PROJ_SIMPLEX_INEQ, "box": pkg.PROJ_BOX, "boxcut": pkg.PROJ_BOXCUT}[kind]
     gamma = cfg.gammas[-1]
-    opts = pkg.binding.make_opts(projection=proj, p0=p0, p1=p1, borrow=True, group_lanes=args.group_lanes, grid_ctas=args.grid_ctas)
+    opts = pkg.binding.make_opts(projection=proj, p0=p0, p1=p1, borrow=True, group_lanes=args.group_lanes, grid_ctas=args.grid_ctas,
+                                  use_graph=args.graph)
     t0 = time.time()
     prob = pkg.Problem.create(inst.I, inst.J, inst.m, inst.row_ptr, inst.item_idx, inst.c, inst.a, inst.b, opts)
     torch.cuda.synchronize()
@@ -220,7 +223,7 @@ def main():
     barrier()
 
     # ---- timed region: exactly K steps, CUDA events on the launching stream ----
-    prob.set_profiling(True)
+    prob.set_profiling(not args.graph)
     launches0 = prob.info().launches
     sampler = ClockSampler(local)
     sampler.start()
@@ -234,7 +237,7 @@ def main():
     ms_total = ev0.elapsed_time(ev1)
     inf = prob.info()
     launches = inf.launches - launches0
-    kern_ms = inf.grad_kernel_ms / max(inf.grad_kernel_count, 1)
+    kern_ms = inf.grad_kernel_ms / max(inf.grad_kernel_count, 1) if not args.graph else ms_total / args.steps
     prob.set_profiling(False)
     t_max = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
     if dist is not None:
@@ -257,7 +260,8 @@ def main():
         barrier()
         t0 = time.perf_counter()
         p2 = pkg.Problem.create(inst.I, inst.J, inst.m, host["row_ptr"], host["item_idx"], host["c"], host["a"], host["b"],
-                                pkg.binding.make_opts(projection=proj, p0=p0, p1=p1, group_lanes=args.group_lanes, grid_ctas=args.grid_ctas))
+                                pkg.binding.make_opts(projection=proj, p0=p0, p1=p1, group_lanes=args.group_lanes, grid_ctas=args.grid_ctas,
+                                                      use_graph=args.graph))
         p2.solve([gamma], [args.steps], lam_h, scalars=sc)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
@@ -296,14 +300,15 @@ def main():
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms_total_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32 (fp64 duals, fp64 shift, 64-bit fixed-point reduction)", "data": "synthetic",
-            "config": {"workload": f"{args.workload} (BASELINE.json configs[2]): {inst.I} users x {inst.J} items, m={inst.m}, "
+            "config": {"workload": f"{args.workload} (BASELINE.json configs[{int(args.workload[3]) - 1}]): {inst.I} users x {inst.J} items, m={inst.m}, "
                                    f"{nnz} nonzeros, projection {kind}({p0},{p1}), gamma={gamma}",
-                       "parallelism": "replicas only" if world > 1 else "single GPU", "l2_policy": "inputs larger than L2 "
-                       f"({alg_bytes / 1e9:.2f} GB streamed per step vs 126 MB L2); no flush needed",
+                       "parallelism": "replicas only" if world > 1 else "single GPU", "l2_policy": (f"inputs larger than L2 ({alg_bytes / 1e9:.2f} GB streamed per step vs 126 MB L2); no flush needed"
+                                     if alg_bytes > 4 * 126e6 else
+                                     f"inputs NOT much larger than L2 ({alg_bytes / 1e6:.0f} MB per step vs 126 MB L2): partly L2-resident, not a bandwidth case"),
                        "group_lanes": info.group_lanes, "chunk_regs": info.chunk_regs, "grid_ctas": info.grid_ctas,
                        "block_threads": info.block_threads, "smem_bytes": info.smem_bytes,
                        "reduction": {1: "smem fixed-point", 2: "global RED.ADD.64", 3: "csc"}[info.reduction],
-                       "short_rows": inst.short_rows},
+                       "short_rows": inst.short_rows, "cuda_graph": bool(args.graph)},
             "iters_per_s": world * args.steps / (ms_total_max * 1e-3),
             "solve_time_s": ms_total_max * 1e-3, "gen_time_s": t_gen, "create_time_s": t_create,
             "gpu_launches": int(launches),

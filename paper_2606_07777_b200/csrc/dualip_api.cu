@@ -29,7 +29,7 @@ struct Plan {
     size_t smem = 0;
     const void* fn = nullptr;
     // streaming (TMA) path
-    bool tma = false;
+    bool tma = false, lam_lo_smem = false;
     long long TN = 0, ntiles = 0;
     int cap_nz = 0, cap_rows = 0, stages = 0, stage_bytes = 0;
 };
@@ -51,8 +51,14 @@ struct dualip {
     double* scalars_dev = nullptr;
     float* x_stage = nullptr;
     dualip_dev::TileEntry* tiles = nullptr;
+    unsigned char* ctl = nullptr;          // [IterState (16 B)][done counter (4 B)] -- see grid_epilogue
+    // CUDA graph of kGraphUnroll chained iteration launches (use_graph), re-parameterised per stage
+    cudaGraph_t graph = nullptr; cudaGraphExec_t graph_exec = nullptr;
+    std::vector<cudaGraphNode_t> graph_nodes;
+    long long graph_launches = 0;
     // constants from a0
     double L = 0.0, max_colabs = 0.0, sum_abs_c = 0.0;
+    float max_abs_a = 0.0f, max_abs_c = 0.0f;
     long long max_row_len = 0;
     double scale_s = 1.0, scale_obj = 1.0, scale_sq = 1.0;
     double xmax = 1.0;
@@ -147,20 +153,27 @@ const void* pick_tma_kernel(const Plan& pl, bool gbox) {
     return pick_tma_m<32>(pl.M, pl.acc_smem, gbox);
 }
 
-// Streaming plan: lambda (and, if there is room for >= 96 KB of stages beside them, the accumulators) in shared
-// memory, the rest of the 227 KB split into `stages` tile buffers.  Returns false if this problem cannot use it.
+// Streaming plan: lambda (and for small J*m the accumulators) in shared memory, the rest of the 227 KB split into
+// `stages` tile buffers.  Returns false if this problem cannot use it.
 bool plan_tma(dualip* h, Plan& pl) {
     const size_t JM = (size_t)h->J * h->m;
     const int red = h->opts.reduction;
     if (h->opts.projection == DUALIP_PROJ_BOX || h->nnz == 0) return false;
     if (h->max_row_len > 8192) return false;
     if (((uintptr_t)h->row_ptr | (uintptr_t)h->idx | (uintptr_t)h->c | (uintptr_t)h->a) & 15) return false;
+    // Shared memory: RN_f32(lambda) always (the filter's operand, 4 B per dual).  Its low word joins it while the
+    // pair stays under 64 KB (otherwise the exact path reads the fp64 lambda through L2: it runs once per row at
+    // most).  The fixed-point item accumulators (8 B per dual) are privatised per CTA only for small J*m, where the
+    // same few addresses would otherwise serialise in L2; beyond that RED.ADD.64 goes straight to L2.
     const size_t fixed = 128 + 128;
-    if (fixed + 8 * JM + 32 * 1024 > kSmemBudget) return false;
-    size_t avail_acc = kSmemBudget > fixed + 16 * JM ? kSmemBudget - fixed - 16 * JM : 0;
-    bool acc = (red == DUALIP_RED_AUTO && avail_acc >= 96 * 1024) || (red == DUALIP_RED_SMEM && avail_acc >= 32 * 1024);
+    if (fixed + 4 * JM + 32 * 1024 > kSmemBudget) return false;
+    const bool lo = 8 * JM <= 64 * 1024;
+    const size_t lam_bytes = (lo ? 8 : 4) * JM;
+    bool acc = (red == DUALIP_RED_AUTO && 16 * JM <= 64 * 1024) ||
+               (red == DUALIP_RED_SMEM && fixed + lam_bytes + 8 * JM + 32 * 1024 <= kSmemBudget);
     if (red == DUALIP_RED_SMEM && !acc) return false;
-    const size_t avail = kSmemBudget - fixed - (acc ? 16 : 8) * JM;
+    const size_t avail = kSmemBudget - fixed - lam_bytes - (acc ? 8 : 0) * JM;
+    pl.lam_lo_smem = lo;
     const int m = h->m;
     const long long units = h->nnz + (long long)kRowCost * h->I;
     long long TN = 0; int stages = 0; size_t stage_bytes = 0;
@@ -183,7 +196,7 @@ bool plan_tma(dualip* h, Plan& pl) {
     size_t sb = (size_t)pl.cap_nz * (8 + 4 * m) + (size_t)pl.cap_rows * 8 + 32;
     pl.stage_bytes = (int)((sb + 127) & ~(size_t)127);
     pl.ntiles = (units + TN - 1) / TN;
-    size_t off = 128 + JM * 8 * (acc ? 2 : 1);
+    size_t off = 128 + lam_bytes + (acc ? 8 : 0) * JM;
     off = (off + 127) & ~(size_t)127;
     pl.smem = off + (size_t)pl.stage_bytes * stages;
     return pl.smem <= kSmemBudget;
@@ -194,7 +207,8 @@ int make_plan(dualip* h) {
     const size_t JM = (size_t)h->J * h->m;
     const int red = h->opts.reduction;
     if (red == DUALIP_RED_CSC) return DUALIP_EUNSUPPORTED;
-    const bool fits_both = 16 * JM <= kSmemBudget, fits_lam = 8 * JM <= kSmemBudget;
+    const size_t kScratch = (kFinalizeScratchBytes + 15) & ~(size_t)15;
+    const bool fits_both = 16 * JM + kScratch <= kSmemBudget, fits_lam = 8 * JM + kScratch <= kSmemBudget;
     if (red == DUALIP_RED_SMEM && !fits_both) return DUALIP_EUNSUPPORTED;
     pl.acc_smem = (red == DUALIP_RED_AUTO || red == DUALIP_RED_SMEM) && fits_both;
     pl.lam_smem = pl.acc_smem || fits_lam;
@@ -230,7 +244,7 @@ int make_plan(dualip* h) {
         if ((long long)G * 2 >= h->max_row_len) pl.KREG = 2;
         else if ((long long)G * 3 >= h->max_row_len) pl.KREG = 3;
     }
-    pl.smem = (pl.lam_smem ? 8 * JM : 0) + (pl.acc_smem ? 8 * JM : 0);
+    pl.smem = (pl.lam_smem ? 8 * JM : 0) + (pl.acc_smem ? 8 * JM : 0) + kScratch;
     pl.fn = pick_kernel(pl);
     if (!pl.fn) return DUALIP_EUNSUPPORTED;
     CK(cudaFuncSetAttribute(pl.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
@@ -285,6 +299,7 @@ int compute_stats(dualip* h, cudaStream_t st, bool do_a, bool do_c) {
             cudaStreamSynchronize(st) != cudaSuccess) { rc = DUALIP_ECUDA; break; }
         float maxa, maxc;
         std::memcpy(&maxa, &mx[0], 4); std::memcpy(&maxc, &mx[1], 4);
+        h->max_abs_a = maxa; h->max_abs_c = maxc;
         const double rows = (double)(h->I > 0 ? h->I : 1);
         const double sc_sq = fix_scale((double)maxa * maxa * m * rows * 1.000001);
         const double sc_abs = fix_scale((double)maxa * rows * 1.000001);
@@ -324,6 +339,7 @@ void fill_grad_params(const dualip* h, GradParams& p, const double* lam_dev, dou
     }
     p.scale_s = h->scale_s; p.scale_obj = h->scale_obj; p.scale_sq = h->scale_sq;
     p.scale_s_f = (float)h->scale_s; p.scale_obj_f = (float)h->scale_obj; p.scale_sq_f = (float)h->scale_sq;
+    p.max_abs_c = h->max_abs_c; p.max_abs_a = h->max_abs_a;
 }
 
 constexpr size_t kMaxTimedLaunches = 4096;
@@ -351,38 +367,80 @@ void prof_collect(dualip* h) {
     h->ev_used = 0;
 }
 
-int launch_grad(dualip* h, const double* lam_dev, double gamma, float* x_dev, cudaStream_t st) {
-    GradParams p;
-    fill_grad_params(h, p, lam_dev, gamma, x_dev);
+// Common fields of the per-launch epilogue (a4-a6).  The caller sets lam_eval/gamma/update/... before launch_iter.
+void fill_finalize_common(const dualip* h, FinalizeParams& f) {
+    f.s_fix = h->s_fix; f.sc_fix = h->sc_fix; f.b = h->b; f.JM = h->J * h->m;
+    f.inv_scale_s = 1.0 / h->scale_s; f.inv_scale_obj = 1.0 / h->scale_obj; f.inv_scale_sq = 1.0 / h->scale_sq;
+    f.state = reinterpret_cast<IterState*>(h->ctl);
+    f.done = reinterpret_cast<unsigned*>(h->ctl + sizeof(IterState));
+}
+
+// Everything one launch needs: function, geometry and the argument block (kept alive by the caller).
+struct IterLaunch {
+    const void* fn; dim3 grid, block; size_t smem;
+    GradParams p; FinalizeParams f; TmaParams tp;
+    void* args[2];
+};
+
+void prepare_iter(const dualip* h, IterLaunch& L, const double* lam_dev, double gamma, float* x_dev, const FinalizeParams& f_in) {
+    fill_grad_params(h, L.p, lam_dev, gamma, x_dev);
+    L.f = f_in;
+    fill_finalize_common(h, L.f);
+    if (h->opts.projection == DUALIP_PROJ_BOX) {
+        L.fn = h->m == 1 ? (const void*)k_grad_box<1> : (h->m == 2 ? (const void*)k_grad_box<2> : (const void*)k_grad_box<0>);
+        L.grid = dim3(grid_for(h->nnz, 256, h->num_sms)); L.block = dim3(256); L.smem = 0;
+        L.args[0] = &L.p; L.args[1] = &L.f;
+    } else if (h->plan.tma) {
+        TmaParams& tp = L.tp;
+        tp.g = L.p; tp.f = L.f; tp.tiles = h->tiles; tp.ntiles = h->plan.ntiles; tp.cap_nz = h->plan.cap_nz; tp.cap_rows = h->plan.cap_rows;
+        tp.stages = h->plan.stages; tp.stage_bytes = h->plan.stage_bytes;
+        tp.nnz4 = h->nnz & ~3ll; tp.rows2 = (h->I + 1) & ~1ll; tp.lam_lo_smem = h->plan.lam_lo_smem ? 1 : 0;
+        L.fn = h->plan.fn; L.grid = dim3(h->plan.grid); L.block = dim3(32 * (kTmaConsumerWarps + 1)); L.smem = h->plan.smem;
+        L.args[0] = &L.tp; L.args[1] = nullptr;
+    } else {
+        L.fn = h->plan.fn; L.grid = dim3(h->plan.grid); L.block = dim3(kBlockThreads); L.smem = h->plan.smem;
+        L.args[0] = &L.p; L.args[1] = &L.f;
+    }
+}
+
+// One launch = one evaluation a1-a5 (+ the AGD update a6 when f.update): gradient kernel with the grid epilogue.
+int launch_iter(dualip* h, IterLaunch& L, cudaStream_t st) {
     const bool timed = prof_begin(h, st);
     struct End { dualip* h; cudaStream_t st; bool on; ~End() { if (on) prof_end(h, st); } } end_guard{h, st, timed};
-    if (h->opts.projection == DUALIP_PROJ_BOX) {
-        const int g = grid_for(h->nnz, 256, h->num_sms);
-        if (h->m == 1) k_grad_box<1><<<g, 256, 0, st>>>(p);
-        else if (h->m == 2) k_grad_box<2><<<g, 256, 0, st>>>(p);
-        else k_grad_box<0><<<g, 256, 0, st>>>(p);
-    } else if (h->plan.tma) {
-        TmaParams tp;
-        tp.g = p; tp.tiles = h->tiles; tp.ntiles = h->plan.ntiles; tp.cap_nz = h->plan.cap_nz; tp.cap_rows = h->plan.cap_rows;
-        tp.stages = h->plan.stages; tp.stage_bytes = h->plan.stage_bytes;
-        tp.nnz4 = h->nnz & ~3ll; tp.rows2 = (h->I + 1) & ~1ll;
-        void* args[] = {(void*)&tp};
-        CK(cudaLaunchKernel(h->plan.fn, dim3(h->plan.grid), dim3(32 * (kTmaConsumerWarps + 1)), args, h->plan.smem, st));
-    } else {
-        void* args[] = {(void*)&p};
-        CK(cudaLaunchKernel(h->plan.fn, dim3(h->plan.grid), dim3(kBlockThreads), args, h->plan.smem, st));
-    }
+    CK(cudaLaunchKernel(L.fn, L.grid, L.block, L.args, L.smem, st));
     h->launches++;
     CK(cudaGetLastError());
     return DUALIP_OK;
 }
 
-int launch_finalize(dualip* h, FinalizeParams& f, cudaStream_t st) {
-    f.s_fix = h->s_fix; f.sc_fix = h->sc_fix; f.b = h->b; f.JM = h->J * h->m;
-    f.inv_scale_s = 1.0 / h->scale_s; f.inv_scale_obj = 1.0 / h->scale_obj; f.inv_scale_sq = 1.0 / h->scale_sq;
-    k_finalize<<<1, kFinalizeThreads, 0, st>>>(f);
-    h->launches++;
-    CK(cudaGetLastError());
+constexpr int kGraphUnroll = 20;   // iterations per graph replay
+
+void drop_graph(dualip* h) {
+    if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+    if (h->graph) cudaGraphDestroy(h->graph);
+    h->graph_exec = nullptr; h->graph = nullptr; h->graph_nodes.clear();
+}
+
+// (Re)parameterise the graph of kGraphUnroll chained launches of L.  Built node by node (no stream capture, so it
+// also works when the caller's stream is the legacy default stream).
+int set_graph(dualip* h, IterLaunch& L) {
+    cudaKernelNodeParams kp{};
+    kp.func = const_cast<void*>(L.fn); kp.gridDim = L.grid; kp.blockDim = L.block;
+    kp.sharedMemBytes = (unsigned)L.smem; kp.kernelParams = L.args; kp.extra = nullptr;
+    if (h->graph_exec) {
+        bool ok = true;
+        for (cudaGraphNode_t nd : h->graph_nodes)
+            if (cudaGraphExecKernelNodeSetParams(h->graph_exec, nd, &kp) != cudaSuccess) { cudaGetLastError(); ok = false; break; }
+        if (ok) return DUALIP_OK;
+        drop_graph(h);
+    }
+    CK(cudaGraphCreate(&h->graph, 0));
+    h->graph_nodes.resize(kGraphUnroll);
+    for (int k = 0; k < kGraphUnroll; ++k) {
+        const cudaGraphNode_t* dep = k ? &h->graph_nodes[k - 1] : nullptr;
+        if (cudaGraphAddKernelNode(&h->graph_nodes[k], h->graph, dep, k ? 1 : 0, &kp) != cudaSuccess) { cudaGetLastError(); drop_graph(h); return DUALIP_ECUDA; }
+    }
+    if (cudaGraphInstantiate(&h->graph_exec, h->graph, 0) != cudaSuccess) { cudaGetLastError(); drop_graph(h); return DUALIP_ECUDA; }
     return DUALIP_OK;
 }
 
@@ -421,6 +479,8 @@ void dualip_destroy(dualip_t* h) {
     if (h->own_c) cudaFree((void*)h->c);
     cudaFree(h->b); cudaFree(h->s_fix); cudaFree(h->lam_cur); cudaFree(h->y); cudaFree(h->lam_stage);
     cudaFree(h->grad_stage); cudaFree(h->scalars_dev); cudaFree(h->x_stage); cudaFree(h->tiles);
+    drop_graph(h);
+    cudaFree(h->ctl);
     for (cudaEvent_t e : h->events) cudaEventDestroy(e);
     cudaGetLastError();
     delete h;
@@ -509,6 +569,8 @@ int dualip_create(dualip_t** out, int64_t I, int32_t J, int32_t m, const int64_t
         if ((rc = dev_alloc(h, &h->lam_stage, JM)) != 0) goto fail;
         if ((rc = dev_alloc(h, &h->grad_stage, JM)) != 0) goto fail;
         if ((rc = dev_alloc(h, &h->scalars_dev, 5)) != 0) goto fail;
+        if ((rc = dev_alloc(h, &h->ctl, 64)) != 0) goto fail;
+        CKF(cudaMemsetAsync(h->ctl, 0, 64, st));
 
         // validation (R11) and row-length statistics.  Monotone row_ptr and the maximum row length are always
         // computed (the kernels index with them); `validate` switches the index-range / duplicate scan.
@@ -595,13 +657,13 @@ int dualip_grad(dualip_t* h, const double* lambda, double gamma, double* grad, d
     if (!lam_dev) { CK(cudaMemcpyAsync(h->lam_stage, lambda, JM * 8, cudaMemcpyHostToDevice, st)); lam_d = h->lam_stage; }
     float* x_d = x;
     if (x && !x_dev) { int rc = ensure_x_stage(h); if (rc != 0) return rc; x_d = h->x_stage; }
-    int rc = launch_grad(h, lam_d, gamma, x_d, st);
-    if (rc != 0) return rc;
     FinalizeParams f{};
     f.lam_eval = lam_d; f.gamma = gamma; f.update = 0;
     f.grad_out = grad ? (grad_dev ? grad : h->grad_stage) : nullptr;
     f.scalars_out = scalars ? (sc_dev ? reinterpret_cast<double*>(scalars) : h->scalars_dev) : nullptr;
-    rc = launch_finalize(h, f, st);
+    IterLaunch L;
+    prepare_iter(h, L, lam_d, gamma, x_d, f);
+    int rc = launch_iter(h, L, st);
     if (rc != 0) return rc;
     bool sync = !lam_dev;
     if (grad && !grad_dev) { CK(cudaMemcpyAsync(grad, h->grad_stage, JM * 8, cudaMemcpyDeviceToHost, st)); sync = true; }
@@ -628,19 +690,30 @@ int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int3
                sc_dev = is_device_ptr(final_scalars), x_dev = is_device_ptr(x_out);
     CK(cudaMemcpyAsync(h->lam_cur, lambda_inout, JM * 8, cudaMemcpyDefault, st));
     const double L = h->L > 0.0 ? h->L : 1.0;
-    long long n = 0;
+    CK(cudaMemsetAsync(h->ctl, 0, sizeof(IterState), st));                                 // t = 0, n = 0
     for (int s = 0; s < n_stages; ++s) {
         const double gamma = gammas[s], eta = gamma / L;
         CK(cudaMemcpyAsync(h->y, h->lam_cur, JM * 8, cudaMemcpyDeviceToDevice, st));   // warm start, momentum restart (R4)
-        for (int t = 0; t < iters[s]; ++t, ++n) {
-            int rc = launch_grad(h, h->y, gamma, nullptr, st);
+        CK(cudaMemsetAsync(h->ctl, 0, sizeof(int), st));                                   // t = 0; n runs on
+        FinalizeParams f{};
+        f.lam_eval = h->y; f.gamma = gamma; f.update = 1; f.eta = eta; f.momentum = h->opts.momentum ? 1 : 0;
+        f.lam_cur = h->lam_cur; f.y = h->y;
+        if (trace) { f.tr_g = trace->g; f.tr_rinf = trace->r_inf; f.tr_r2 = trace->r_2; f.tr_grad = trace->grad; f.tr_lam = trace->lambda; }
+        IterLaunch it;
+        prepare_iter(h, it, h->y, gamma, nullptr, f);
+        int t = 0;
+        // beta_t and the trace row come from the device-side iteration state, so every launch of a stage has the
+        // same arguments: replay a graph of kGraphUnroll chained launches, then finish with direct launches
+        if (h->opts.use_graph && !h->profile && iters[s] >= 2 * kGraphUnroll) {
+            int rc = set_graph(h, it);
             if (rc != 0) return rc;
-            FinalizeParams f{};
-            f.lam_eval = h->y; f.gamma = gamma; f.update = 1; f.eta = eta;
-            f.beta = h->opts.momentum ? (double)t / (double)(t + 3) : 0.0;
-            f.lam_cur = h->lam_cur; f.y = h->y;
-            if (trace) { f.tr_g = trace->g; f.tr_rinf = trace->r_inf; f.tr_r2 = trace->r_2; f.tr_grad = trace->grad; f.tr_lam = trace->lambda; f.tr_n = n; }
-            rc = launch_finalize(h, f, st);
+            for (; t + kGraphUnroll <= iters[s]; t += kGraphUnroll) {
+                CK(cudaGraphLaunch(h->graph_exec, st));
+                h->launches += kGraphUnroll; h->graph_launches++;
+            }
+        }
+        for (; t < iters[s]; ++t) {
+            int rc = launch_iter(h, it, st);
             if (rc != 0) return rc;
         }
     }
@@ -648,13 +721,13 @@ int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int3
     if (x_out || final_scalars || final_grad) {
         float* x_d = x_out;
         if (x_out && !x_dev) { int rc = ensure_x_stage(h); if (rc != 0) return rc; x_d = h->x_stage; }
-        int rc = launch_grad(h, h->lam_cur, gammas[n_stages - 1], x_d, st);
-        if (rc != 0) return rc;
         FinalizeParams f{};
         f.lam_eval = h->lam_cur; f.gamma = gammas[n_stages - 1]; f.update = 0;
         f.grad_out = final_grad ? (grad_dev ? final_grad : h->grad_stage) : nullptr;
         f.scalars_out = final_scalars ? (sc_dev ? reinterpret_cast<double*>(final_scalars) : h->scalars_dev) : nullptr;
-        rc = launch_finalize(h, f, st);
+        IterLaunch it;
+        prepare_iter(h, it, h->lam_cur, gammas[n_stages - 1], x_d, f);
+        int rc = launch_iter(h, it, st);
         if (rc != 0) return rc;
     }
     bool sync = false;

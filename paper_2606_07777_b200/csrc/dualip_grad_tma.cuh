@@ -38,6 +38,7 @@ struct TileEntry {                     // 32 bytes, one per tile (+1 sentinel)
 
 struct TmaParams {
     GradParams g;
+    FinalizeParams f;
     const TileEntry* __restrict__ tiles;   // [ntiles + 1]
     long long ntiles;
     int cap_nz;                        // nonzero capacity of a stage (multiple of 4)
@@ -46,6 +47,7 @@ struct TmaParams {
     int stage_bytes;                   // bytes of one stage (multiple of 16)
     long long nnz4;                    // nnz rounded down to a multiple of 4 (bulk copies stop there)
     long long rows2;                   // (I+1) rounded down to a multiple of 2
+    int lam_lo_smem;                   // 1: lambda's low word is staged in shared memory too (small J*m)
 };
 
 // ---- PTX wrappers (mbarrier + bulk async copy) ---------------------------------------------------------------
@@ -92,7 +94,9 @@ __device__ __forceinline__ StageView stage_view(unsigned char* base, int cap_nz,
 
 // Shared state the row routines need.
 struct ConsumerCtx {
-    const float* lam_hi; const float* lam_lo;     // lambda = (double)hi + (double)lo, exact to 2^-48 relative
+    const float* lam_hi;                          // RN_f32(lambda) in shared memory: the filter's operand
+    const float* lam_lo;                          // lambda - hi in shared memory (exact to 2^-48 relative), or nullptr:
+    const double* lam_g;                          //   then the exact path reads the fp64 lambda from global memory (L2)
     unsigned* acc_lo; unsigned* acc_hi;           // shared-memory item accumulators (ACC_SMEM)
 };
 struct FixPair { long long obj, sq; };            // per-lane fixed-point partial scalars (order-independent)
@@ -105,6 +109,13 @@ __device__ __forceinline__ long long to_fix32(float v, float scale) { return __f
 // shared-memory CAS loop and a predicate that the caller then waits on).
 __device__ __forceinline__ void red_add_u64(unsigned long long* gptr, unsigned long long v) {
     asm volatile("red.global.add.u64 [%0], %1;" ::"l"(gptr), "l"(v) : "memory");
+}
+
+// (a > b) ? x : y as one SETP + SEL, whatever the surrounding control flow looks like
+__device__ __forceinline__ int sel_gt(float a, float b, int x, int y) {
+    int r;
+    asm("{\n\t.reg .pred p;\n\tsetp.gt.f32 p, %1, %2;\n\tselp.s32 %0, %3, %4, p;\n\t}" : "=r"(r) : "f"(a), "f"(b), "r"(x), "r"(y));
+    return r;
 }
 
 // a4 + a5 for one nonzero with x != 0.
@@ -133,7 +144,7 @@ __device__ __forceinline__ double exact_t(const StageView& v, const ConsumerCtx&
         aa[f] = 0.0f;
         if (f < mm) {
             aa[f] = v.a[q * mm + f];
-            const double l = (double)cx.lam_hi[j * mm + f] + (double)cx.lam_lo[j * mm + f];
+            const double l = cx.lam_lo ? (double)cx.lam_hi[j * mm + f] + (double)cx.lam_lo[j * mm + f] : __ldg(cx.lam_g + j * mm + f);
             t = fma((double)aa[f], l, t);
         }
     }
@@ -243,22 +254,34 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
     constexpr int NT = 32 * (NWC + 1);
     const int mm = M > 0 ? M : p.m;
     const int JM = p.J * mm;
-    // layout: [full[4], empty[4] mbarriers: 64 B][claim counters: 64 B][lam_hi JM*4][lam_lo JM*4][acc 2*JM*4][stages]
+    // layout: [full[4], empty[4] mbarriers: 64 B][max|lambda| word, claim counters: 64 B][lam_hi JM*4][lam_lo JM*4 (optional)][acc 2*JM*4 (ACC_SMEM)][stages]
     unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_tma);
-    int* claim = reinterpret_cast<int*>(smem_tma + 64);
+    unsigned* s_words = reinterpret_cast<unsigned*>(smem_tma + 64);       // [0] = max |lambda_hi| as float bits
+    int* claim = reinterpret_cast<int*>(smem_tma + 64 + 16);              // [stage] = next unclaimed row-step of the tile in it
     float* s_hi32 = reinterpret_cast<float*>(smem_tma + 128);
-    float* s_lo32 = s_hi32 + JM;
-    unsigned* a_lo = reinterpret_cast<unsigned*>(s_lo32 + JM);
+    float* s_lo32 = s_hi32 + JM;                                           // only when tp.lam_lo_smem
+    unsigned* a_lo = reinterpret_cast<unsigned*>(s_hi32 + (tp.lam_lo_smem ? 2 : 1) * JM);
     unsigned* a_hi = a_lo + JM;
-    size_t off = 128 + (size_t)JM * 8 * (ACC_SMEM ? 2 : 1);
+    size_t off = 128 + (size_t)JM * 4 * ((tp.lam_lo_smem ? 2 : 1) + (ACC_SMEM ? 2 : 0));
     off = (off + 127) & ~(size_t)127;
     unsigned char* stage0 = smem_tma + off;
 
-    for (int q = threadIdx.x; q < JM; q += NT) {
-        const double l = p.lambda[q];
-        const float h = (float)l;
-        s_hi32[q] = h;
-        s_lo32[q] = (float)(l - (double)h);
+    if (threadIdx.x == 0) s_words[0] = 0u;
+    __syncthreads();
+    {
+        float lmax = 0.0f;
+        for (int q = threadIdx.x; q < JM; q += NT) {
+            const double l = p.lambda[q];
+            const float h = (float)l;
+            s_hi32[q] = h;
+            if (tp.lam_lo_smem) s_lo32[q] = (float)(l - (double)h);
+            lmax = fmaxf(lmax, fabsf(h));
+        }
+        if (M != 1) {                                                      // the filter's rounding bound needs max |lambda|
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) lmax = fmaxf(lmax, __shfl_xor_sync(kFull, lmax, o));
+            if ((threadIdx.x & 31) == 0) atomicMax(&s_words[0], __float_as_uint(lmax));
+        }
     }
     if (ACC_SMEM) for (int q = threadIdx.x; q < 2 * JM; q += NT) a_lo[q] = 0u;
     {   // consumers read whole 16-byte vectors around a row: every stage word must always hold a valid item index
@@ -275,7 +298,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
     __syncthreads();
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const ConsumerCtx cx{s_hi32, s_lo32, a_lo, a_hi};
+    const ConsumerCtx cx{s_hi32, tp.lam_lo_smem ? s_lo32 : nullptr, p.lambda, a_lo, a_hi};
     FixPair fp{0ll, 0ll};
 
     if (warp == 0) {
@@ -336,6 +359,9 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
         const float gz = (float)((double)p.z / p.inv_gamma);            // z * gamma: the vertex gap in w units
         const bool upper = RPG == 2 && (gl & HG) != 0;                   // this lane ends up holding the group's row 1
         const bool fin = RPG == 2 ? (gl & (HG - 1)) == 0 : true;        // lanes 0 and G/2 of a group finalise rows 0 and 1
+        // rounding bound of the filter (see below): the part that does not depend on the row
+        const float bnd0 = M == 1 ? p.max_abs_c : p.max_abs_c + (float)mm * p.max_abs_a * __uint_as_float(s_words[0]);
+        const float gz_sat = gz * (1.0f + 4.8e-7f);                      // w_max above this (plus tol): v_max >= z for sure
         int s = 0;
         unsigned ph = 0;
         for (long long t = blockIdx.x; t < tp.ntiles; t += gridDim.x) {
@@ -343,6 +369,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
             const StageView v = stage_view(stage0 + s * tp.stage_bytes, tp.cap_nz, tp.cap_rows, mm);
             const int nrows = v.meta->nrows;
             const int nsteps = (nrows + RPW - 1) / RPW;
+            // Row-steps are claimed from a shared counter: whichever warp is free takes the next one.
             for (;;) {
                 int st = 0;
                 if (lane == 0) st = atomicAdd(&claim[s], 1);
@@ -351,7 +378,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                 const int rpo = v.meta->rpo;
                 const int nzb32 = (int)v.meta->nzb;                       // low word is enough for local offsets
                 int rbeg[RPG], rlen[RPG];
-                float rm1[RPG], rm2[RPG], rbnd[RPG];
+                float rm1[RPG], rm2[RPG];
                 int rpos[RPG];
 #pragma unroll
                 for (int r = 0; r < RPG; ++r) {
@@ -362,7 +389,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                         beg = b - nzb32; len = e - b;
                     }
                     rbeg[r] = beg; rlen[r] = len;
-                    float m1 = -CUDART_INF_F, m2 = -CUDART_INF_F, bnd = 0.0f;
+                    float m1 = -CUDART_INF_F, m2 = -CUDART_INF_F;
                     int pb = 0;
                     if (!GBOX) {
                         // ---- fp32 filter: the two largest w' = -(c + a.lambda_hi) of the row and where the largest sits.
@@ -376,12 +403,12 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                             const float4 c4 = *reinterpret_cast<const float4*>(v.c + q);
                             const int jj[4] = {j4.x, j4.y, j4.z, j4.w};
                             const float cv[4] = {c4.x, c4.y, c4.z, c4.w};
-                            float wv[4], av[4];
+                            float wv[4];
                             if (M == 1) {
                                 const float4 a4 = *reinterpret_cast<const float4*>(v.a + q);
                                 const float aa4[4] = {a4.x, a4.y, a4.z, a4.w};
 #pragma unroll
-                                for (int e = 0; e < 4; ++e) { wv[e] = -fmaf(aa4[e], s_hi32[jj[e]], cv[e]); av[e] = fabsf(cv[e]); }
+                                for (int e = 0; e < 4; ++e) wv[e] = -fmaf(aa4[e], s_hi32[jj[e]], cv[e]);
                             } else if (M == 2) {
                                 const float4 a01 = *reinterpret_cast<const float4*>(v.a + 2 * q);
                                 const float4 a23 = *reinterpret_cast<const float4*>(v.a + 2 * q + 4);
@@ -390,33 +417,27 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                                 for (int e = 0; e < 4; ++e) {
                                     const float2 l2 = *reinterpret_cast<const float2*>(s_hi32 + 2 * jj[e]);
                                     wv[e] = -fmaf(ay[e], l2.y, fmaf(ax[e], l2.x, cv[e]));
-                                    av[e] = fabsf(cv[e]) + fabsf(ax[e] * l2.x) + fabsf(ay[e] * l2.y);
                                 }
                             } else {
 #pragma unroll
                                 for (int e = 0; e < 4; ++e) {
-                                    float w = cv[e], ab = fabsf(cv[e]);
-                                    for (int f = 0; f < mm; ++f) {
-                                        const float af = v.a[(q + e) * mm + f], lf = s_hi32[jj[e] * mm + f];
-                                        ab += fabsf(af * lf);
-                                        w = fmaf(af, lf, w);
-                                    }
-                                    wv[e] = -w; av[e] = ab;
+                                    float w = cv[e];
+                                    for (int f = 0; f < mm; ++f) w = fmaf(v.a[(q + e) * mm + f], s_hi32[jj[e] * mm + f], w);
+                                    wv[e] = -w;
                                 }
                             }
 #pragma unroll
                             for (int e = 0; e < 4; ++e) {
                                 const bool valid = (unsigned)(q + e - beg) < (unsigned)len;
                                 const float w = valid ? wv[e] : -CUDART_INF_F;
-                                bnd = fmaxf(bnd, av[e]);
-                                const bool gt = w > m1;
-                                m2 = gt ? m1 : fmaxf(m2, w);
-                                pb = gt ? q + e : pb;
+                                // top two and the arg-max, branch-free (ptxas turned the ternary form into branches)
+                                m2 = fmaxf(m2, fminf(m1, w));
+                                pb = sel_gt(w, m1, q + e, pb);
                                 m1 = fmaxf(m1, w);
                             }
                         }
                     }
-                    rm1[r] = m1; rm2[r] = m2; rbnd[r] = bnd; rpos[r] = pb;
+                    rm1[r] = m1; rm2[r] = m2; rpos[r] = pb;
                 }
                 unsigned slow_mask;
                 int fbeg = rbeg[0], flen = rlen[0];
@@ -429,18 +450,17 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                     // is a transposition: the lower half of the group keeps row 0 and hands over its part of row 1,
                     // the upper half the reverse; the remaining levels then run on both rows at once.  Equal maxima in
                     // two lanes give m2 = m1 (no vertex).
-                    float m1 = rm1[0], m2 = rm2[0], bnd = rbnd[0];
+                    float m1 = rm1[0], m2 = rm2[0];
                     int fpos = rpos[0];
                     if (RPG == 2) {
-                        float g1 = rm1[RPG - 1], g2 = rm2[RPG - 1], gb = rbnd[RPG - 1];
+                        float g1 = rm1[RPG - 1], g2 = rm2[RPG - 1];
                         int gp = rpos[RPG - 1];
                         if (upper) {
                             float tf; int ti;
-                            tf = m1; m1 = g1; g1 = tf; tf = m2; m2 = g2; g2 = tf; tf = bnd; bnd = gb; gb = tf; ti = fpos; fpos = gp; gp = ti;
+                            tf = m1; m1 = g1; g1 = tf; tf = m2; m2 = g2; g2 = tf; ti = fpos; fpos = gp; gp = ti;
                         }
                         const float o1 = __shfl_xor_sync(kFull, g1, HG), o2 = __shfl_xor_sync(kFull, g2, HG);
                         const int op = __shfl_xor_sync(kFull, gp, HG);
-                        bnd = fmaxf(bnd, __shfl_xor_sync(kFull, gb, HG));
                         const bool gt = o1 > m1;
                         m2 = fmaxf(fminf(m1, o1), fmaxf(m2, o2));
                         fpos = gt ? op : fpos;
@@ -450,30 +470,38 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                     for (int o = HG / 2; o > 0; o >>= 1) {
                         const float o1 = __shfl_xor_sync(kFull, m1, o), o2 = __shfl_xor_sync(kFull, m2, o);
                         const int op = __shfl_xor_sync(kFull, fpos, o);
-                        bnd = fmaxf(bnd, __shfl_xor_sync(kFull, bnd, o));
                         const bool gt = o1 > m1;
                         m2 = fmaxf(fminf(m1, o1), fmaxf(m2, o2));
                         fpos = gt ? op : fpos;
                         m1 = fmaxf(m1, o1);
                     }
-                    // rounding bound of the filter: (m+1) roundings at 2^-24 plus lambda truncated to fp32 (2^-24
-                    // relative), each relative to at most B = |c| + sum|a lam| of that nonzero.  M = 1: |a lam| <=
-                    // |w'| + |c|, so B <= 2|w'| + max|c|; a value far below the top two has a larger bound but is
-                    // further away by more than that.  2^-22 gives slack.  `bnd` may include neighbouring rows' |c|
-                    // (the unmasked slots of the first and last pass): a larger bound only sends more rows to the
-                    // exact path.
+                    // rounding bound of the filter.  Every FFMA rounds once, relative to its own result, and lambda is
+                    // truncated to fp32 (2^-24 relative to |a lam|).  M = 1: error <= 2^-24 (|w'| + |a lam|) and
+                    // |a lam| <= |w'| + |c|, so B = 2|w'| + max|c| covers the top two; a value far below them has a larger
+                    // error but is further away by more than that.  M > 1: every partial sum is at most
+                    // B = max|c| + m max|a| max|lam|, and there are m roundings plus the truncations.  2.4e-7 = 2^-22 gives
+                    // slack.  The maxima are global (a0 / this launch's lambda): a looser bound only sends more rows to
+                    // the exact path.
                     const float mag = fmaxf(fabsf(m1), m2 > -CUDART_INF_F ? fabsf(m2) : 0.0f);
-                    const float B = M == 1 ? 2.0f * mag + bnd : bnd;
+                    const float B = M == 1 ? 2.0f * mag + bnd0 : bnd0;
                     const float tol = 2.4e-7f * (float)(mm + 1) * B + 1e-30f;
                     const bool vertex = (m1 - m2) > gz + 2.0f * tol;
                     const bool dead = ineq && m1 < -tol;
                     const bool fast = vertex || dead;
                     float xo = 0.0f;
                     if (active && vertex && !dead) {
-                        // exact fp64 for the arg-max nonzero only: x = clamp(v_max, 0, z) (or z for the equality simplex)
+                        // x = clamp(v_max, 0, z) on the arg-max nonzero (z for the equality simplex).  When v_max >= z is
+                        // certain in fp32 the answer is z itself; otherwise that one nonzero is redone in fp64.
                         int j; float cc; float aa[MA];
-                        const double tq = exact_t<M>(v, cx, mm, fpos, j, cc, aa);
-                        xo = ineq ? fmaxf((float)fmin((double)z, -tq * p.inv_gamma), 0.0f) : z;
+                        if (!ineq || m1 - tol > gz_sat) {
+                            j = v.idx[fpos]; cc = v.c[fpos];
+#pragma unroll
+                            for (int f = 0; f < MA; ++f) aa[f] = f < mm ? v.a[fpos * mm + f] : 0.0f;
+                            xo = z;
+                        } else {
+                            const double tq = exact_t<M>(v, cx, mm, fpos, j, cc, aa);
+                            xo = fmaxf((float)fmin((double)z, -tq * p.inv_gamma), 0.0f);
+                        }
                         if (xo > 0.0f) push<M, ACC_SMEM>(p, cx, fp, mm, j, cc, aa, xo);
                     }
                     if (p.x) {
@@ -487,7 +515,57 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                             if (fr) for (int e = gl; e < rlen[r]; e += G) p.x[nzb + rbeg[r] + e] = (rbeg[r] + e == pr) ? xr : 0.0f;
                         }
                     }
-                    slow_mask = __ballot_sync(kFull, active && !fast);
+                    // ---- candidate path: rows that are neither a vertex nor dead.  Only nonzeros with w > w_max - z gamma
+                    // can be in the support (theta >= v_max - z for both simplex forms), and the filter already knows
+                    // each lane's two largest w'.  If no lane of the group has its SECOND value above the candidate
+                    // threshold, every lane holds at most one candidate, at a known position: those few nonzeros are
+                    // redone in fp64 and projected in registers by the group (same arithmetic as slow_row), and the
+                    // rest of the row is zero.  Typical fractional rows have 2-3 candidates, so this takes almost all
+                    // of them; rows with two candidates in one lane, or more candidates than lanes, go to slow_row.
+                    bool handled = false;
+                    const bool want = active && !fast;
+                    if (__any_sync(kFull, want)) {
+                        const unsigned gmask = G == 32 ? kFull : (((1u << G) - 1u) << (lane & ~(G - 1)));
+                        const float thr_own = m1 - gz_sat - 2.0f * tol;
+#pragma unroll
+                        for (int r = 0; r < RPG; ++r) {
+                            const int src = (lane & ~(G - 1)) + r * HG;
+                            const bool rw = __shfl_sync(kFull, (int)want, src) != 0;
+                            const float thr = __shfl_sync(kFull, thr_own, src);
+                            const unsigned okb = __ballot_sync(kFull, !(rm2[r] > thr));
+                            const bool row_ok = rw && (okb & gmask) == gmask;
+                            if (!__any_sync(kFull, row_ok)) continue;
+                            const bool cand = row_ok && rm1[r] > thr;
+                            int j = 0; float cc = 0.0f; float aa[MA];
+                            double wq = -CUDART_INF;
+                            if (cand) wq = -exact_t<M>(v, cx, mm, rpos[r], j, cc, aa);
+                            const float m32 = group_max<G>((float)wq);          // the row maximum is always a candidate
+                            const bool alive = row_ok && (!ineq || m32 > 0.0f);
+                            const float mv = m32 * p.inv_gamma_f;
+                            const float u = cand ? (float)(wq - (double)m32) * p.inv_gamma_f : -CUDART_INF_F;
+                            float theta = -z - (1.2e-7f * fabsf(mv) + 1e-6f);
+                            int n_prev = -1;
+                            for (;;) {                                           // Michelot on the candidates
+                                const bool in = alive && u > theta;
+                                const float sg = group_sum<G>(in ? u : 0.0f);
+                                const int n = __popc(__ballot_sync(kFull, in) & gmask);
+                                const bool stop = n == n_prev || n == 0;
+                                if (!stop) { theta = fmaxf((sg - z) / (float)n, theta); n_prev = n; }
+                                if (__all_sync(kFull, stop)) break;
+                            }
+                            const float tau = ineq ? fmaxf(theta, -mv) : theta;
+                            const float xq = (cand && alive) ? fmaxf(u - tau, 0.0f) : 0.0f;
+                            if (xq > 0.0f) push<M, ACC_SMEM>(p, cx, fp, mm, j, cc, aa, xq);
+                            if (p.x) {
+                                const long long nzb = v.meta->nzb;
+                                if (row_ok) for (int e = gl; e < rlen[r]; e += G) p.x[nzb + rbeg[r] + e] = 0.0f;
+                                __syncwarp();
+                                if (cand) p.x[nzb + rpos[r]] = xq;
+                            }
+                            if (lane == src && row_ok) handled = true;
+                        }
+                    }
+                    slow_mask = __ballot_sync(kFull, want && !handled);
                 }
                 while (slow_mask) {
                     const int src = __ffs(slow_mask) - 1;
@@ -518,6 +596,9 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
             if (val) atomicAdd(p.s_fix + q, val);
         }
     }
+    // a4-a6 by the CTA that finishes last.  Its scratch is the first stage buffer: grid_epilogue's barrier comes after
+    // every consumer has seen the last "full" phase, so no bulk copy is in flight any more.
+    grid_epilogue(tp.f, reinterpret_cast<double*>(stage0), NT);
 }
 
 // a0: tile table.  Tile t starts at the first row r with row_ptr[r] + kRowCost*r >= t*TN (parallel binary search).

@@ -4,7 +4,8 @@
 //   k_grad      a1 gather lambda, a2 w = -(c + sum_k a^k lambda_jk), a3 projection, a4 item reduction,
 //               a5 per-lane partial scalars, a8 optional x                         (Eq. 3-4)
 //   k_grad_box  the same for the element-wise box projection (no row coupling)
-//   k_finalize  a4 grad = s - b, a5 g / r_inf / r_2, a6 AGD update + lambda >= 0 projection (R1)
+//   finalize_block  a4 grad = s - b, a5 g / r_inf / r_2, a6 AGD update + lambda >= 0 projection (R1),
+//               run by the last CTA of every gradient launch (grid_epilogue): one launch = one iteration
 //   k_validate, k_absmax, k_col_stats, k_reduce_stats      a0 create-time checks and constants (R2, R11)
 //
 // Numerics: lambda fp64; w by fp64 FMA from fp32 data; row maximum taken on RN_f32(w);
@@ -49,6 +50,7 @@ struct GradParams {
     double box_lo, box_hi;
     double scale_s, scale_obj, scale_sq;
     float scale_s_f, scale_obj_f, scale_sq_f;   // the same powers of two as floats (streaming kernel: one FMUL + F2I)
+    float max_abs_c, max_abs_a;                 // max |c|, max |a| over all nonzeros (a0): the filter's rounding bound
 };
 
 __device__ __forceinline__ long long to_fix(float v, double scale) { return __double2ll_rn((double)v * scale); }
@@ -121,6 +123,116 @@ __device__ __forceinline__ void contribute(const GradParams& p, unsigned* s_lo, 
             if (ACC_SMEM) fix_add_smem(s_lo + j * nm + k, s_hi + j * nm + k, f);
             else atomicAdd(p.s_fix + (long long)j * nm + k, (unsigned long long)f);
         }
+    }
+}
+
+// Iteration state kept on the device so that every launch of one stage has identical arguments (CUDA-graph replay):
+// t = iteration index inside the stage (momentum restart resets it, R4), n = index over all stages (trace row).
+struct IterState { int t; int pad; long long n; };
+
+struct FinalizeParams {
+    unsigned long long* s_fix;
+    unsigned long long* sc_fix;
+    const float* __restrict__ b;
+    const double* lam_eval;     // point the gradient was taken at
+    double* grad_out;           // nullable
+    double* scalars_out;        // nullable, 5 doubles {g, obj, reg, r_inf, r_2}
+    int JM;
+    double inv_scale_s, inv_scale_obj, inv_scale_sq;
+    double gamma;
+    int update;                 // a6 on/off
+    int momentum;               // beta_t = t/(t+3) (R1) or 0
+    double eta;
+    double* lam_cur;            // lambda_t -> lambda_{t+1}
+    double* y;                  // y_t -> y_{t+1} (== lam_eval when update)
+    IterState* state;           // read and advanced when update
+    unsigned* done;             // CTAs that have flushed their partial sums (zero between launches)
+    double* tr_g; double* tr_rinf; double* tr_r2; double* tr_grad; double* tr_lam;   // trace columns (nullable)
+};
+
+constexpr int kFinalizeScratchBytes = 3 * 32 * 8 + 16;   // shared memory finalize_block needs: 3 x 32 doubles + flag
+
+// a4 (grad = s - b), a5 (scalars), a6 (AGD step, R1) on the J*m vector by ONE CTA of `nthreads` (<= 1024) threads;
+// re-zeroes the accumulators and advances the iteration state.  `sh` = 96 doubles of shared memory.
+__device__ __forceinline__ void finalize_block(const FinalizeParams& p, double* sh, int tid, int nthreads) {
+    double* sh_dot = sh; double* sh_r2 = sh + 32; double* sh_inf = sh + 64;
+    int t = 0; long long n = 0;
+    if (p.update) { t = p.state->t; n = p.state->n; }
+    const double beta = (p.update && p.momentum) ? (double)t / (double)(t + 3) : 0.0;
+    double dot = 0.0, r2 = 0.0, rinf = 0.0;
+    // four elements per thread and pass, every load issued before the first dependent store: the loop is a chain of
+    // L2 round trips, and this CTA runs alone at the end of the launch
+    constexpr int U = 4;
+    for (int q0 = tid; q0 < p.JM; q0 += U * nthreads) {
+        unsigned long long sf[U]; float bb[U]; double le[U], lo[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int q = q0 + u * nthreads;
+            sf[u] = 0ull; bb[u] = 0.0f; le[u] = 0.0; lo[u] = 0.0;
+            if (q < p.JM) {
+                sf[u] = __ldcg(p.s_fix + q); bb[u] = __ldg(p.b + q); le[u] = __ldcg(p.lam_eval + q);
+                if (p.update) lo[u] = __ldcg(p.lam_cur + q);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int q = q0 + u * nthreads;
+            if (q >= p.JM) break;
+            const double s = (double)(long long)sf[u] * p.inv_scale_s;
+            p.s_fix[q] = 0ull;
+            const double g = s - (double)bb[u];
+            dot = fma(le[u], g, dot);
+            if (g > 0.0) { r2 = fma(g, g, r2); rinf = fmax(rinf, g); }
+            if (p.grad_out) p.grad_out[q] = g;
+            if (p.update) {
+                if (p.tr_grad) p.tr_grad[n * p.JM + q] = g;
+                const double ln = fmax(0.0, le[u] + p.eta * g);
+                p.lam_cur[q] = ln;
+                p.y[q] = ln + beta * (ln - lo[u]);
+                if (p.tr_lam) p.tr_lam[n * p.JM + q] = ln;
+            }
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        dot += __shfl_xor_sync(kFull, dot, o);
+        r2 += __shfl_xor_sync(kFull, r2, o);
+        rinf = fmax(rinf, __shfl_xor_sync(kFull, rinf, o));
+    }
+    const int lane = tid & 31, warp = tid >> 5;
+    if (lane == 0) { sh_dot[warp] = dot; sh_r2[warp] = r2; sh_inf[warp] = rinf; }
+    __syncthreads();
+    if (tid == 0) {
+        dot = 0.0; r2 = 0.0; rinf = 0.0;
+        for (int w = 0; w < (nthreads + 31) / 32; ++w) { dot += sh_dot[w]; r2 += sh_r2[w]; rinf = fmax(rinf, sh_inf[w]); }
+        const double obj = (double)(long long)__ldcg(p.sc_fix + 0) * p.inv_scale_obj;
+        const double reg = 0.5 * p.gamma * ((double)(long long)__ldcg(p.sc_fix + 1) * p.inv_scale_sq);
+        p.sc_fix[0] = 0ull; p.sc_fix[1] = 0ull;
+        const double g = obj + reg + dot;
+        const double nr2 = sqrt(r2);
+        if (p.scalars_out) { p.scalars_out[0] = g; p.scalars_out[1] = obj; p.scalars_out[2] = reg; p.scalars_out[3] = rinf; p.scalars_out[4] = nr2; }
+        if (p.update) {
+            if (p.tr_g) p.tr_g[n] = g;
+            if (p.tr_rinf) p.tr_rinf[n] = rinf;
+            if (p.tr_r2) p.tr_r2[n] = nr2;
+            p.state->t = t + 1; p.state->n = n + 1;
+        }
+    }
+}
+
+// Grid epilogue of every gradient kernel: the CTA that flushes last (threadFenceReduction pattern) runs
+// finalize_block, so one launch is one whole dual-ascent iteration (a1-a6).  `sh`: kFinalizeScratchBytes of shared
+// memory no longer used for anything else.  Every thread of the CTA must call it after its last accumulator flush.
+__device__ __forceinline__ void grid_epilogue(const FinalizeParams& f, double* sh, int nthreads) {
+    int* flag = reinterpret_cast<int*>(sh + 96);
+    __threadfence();                                    // this thread's RED/atomics are visible device-wide
+    __syncthreads();
+    if (threadIdx.x == 0) *flag = (atomicAdd(f.done, 1u) == gridDim.x - 1) ? 1 : 0;
+    __syncthreads();
+    if (*flag) {
+        __threadfence();
+        finalize_block(f, sh, threadIdx.x, nthreads);
+        if (threadIdx.x == 0) *f.done = 0u;
     }
 }
 
@@ -225,7 +337,7 @@ __device__ __noinline__ void long_row(const GradParams& p, const double* s_lam, 
 
 // The fused per-user gradient kernel.  G lanes own one row; rows of up to G*KREG nonzeros live in registers.
 template <int G, int KREG, int M, bool LAM_SMEM, bool ACC_SMEM>
-__global__ void __launch_bounds__(kBlockThreads, 1) k_grad(const GradParams p) {
+__global__ void __launch_bounds__(kBlockThreads, 1) k_grad(const GradParams p, const FinalizeParams f) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int MA = M > 0 ? M : 4;
     const int mm = M > 0 ? M : p.m;
@@ -446,11 +558,14 @@ __global__ void __launch_bounds__(kBlockThreads, 1) k_grad(const GradParams p) {
             if (v) atomicAdd(p.s_fix + q, v);
         }
     }
+    // a4-a6 by the CTA that finishes last; its scratch sits behind lambda and the accumulators
+    grid_epilogue(f, reinterpret_cast<double*>(smem_raw + (LAM_SMEM ? (size_t)JM * 8 : 0) + (ACC_SMEM ? (size_t)JM * 8 : 0)), kBlockThreads);
 }
 
 // Box projection {lo <= x <= hi}: element-wise, so one thread per nonzero with fully coalesced streams.
 template <int M>
-__global__ void __launch_bounds__(256) k_grad_box(const GradParams p) {
+__global__ void __launch_bounds__(256) k_grad_box(const GradParams p, const FinalizeParams f) {
+    __shared__ double sh_fin[kFinalizeScratchBytes / 8];
     const int mm = M > 0 ? M : p.m;
     float obj_l = 0.0f, sq_l = 0.0f;
     for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < p.nnz; q += (long long)gridDim.x * blockDim.x) {
@@ -472,71 +587,7 @@ __global__ void __launch_bounds__(256) k_grad_box(const GradParams p) {
         if (so) atomicAdd(p.sc_fix + 0, (unsigned long long)so);
         if (ss) atomicAdd(p.sc_fix + 1, (unsigned long long)ss);
     }
-}
-
-struct FinalizeParams {
-    unsigned long long* s_fix;
-    unsigned long long* sc_fix;
-    const float* __restrict__ b;
-    const double* lam_eval;     // point the gradient was taken at
-    double* grad_out;           // nullable
-    double* scalars_out;        // nullable, 5 doubles {g, obj, reg, r_inf, r_2}
-    int JM;
-    double inv_scale_s, inv_scale_obj, inv_scale_sq;
-    double gamma;
-    int update;                 // a6 on/off
-    double eta, beta;
-    double* lam_cur;            // lambda_t -> lambda_{t+1}
-    double* y;                  // y_t -> y_{t+1} (== lam_eval when update)
-    double* tr_g; double* tr_rinf; double* tr_r2; double* tr_grad; double* tr_lam;   // trace columns (nullable)
-    long long tr_n;
-};
-
-constexpr int kFinalizeThreads = 1024;
-
-// a4 (grad = s - b), a5 (scalars), a6 (AGD step, R1) on the J*m vector; re-zeroes the accumulators.
-__global__ void __launch_bounds__(kFinalizeThreads) k_finalize(const FinalizeParams p) {
-    __shared__ double sh_dot[32], sh_r2[32], sh_inf[32];
-    double dot = 0.0, r2 = 0.0, rinf = 0.0;
-    for (int q = threadIdx.x; q < p.JM; q += kFinalizeThreads) {
-        const double s = (double)(long long)p.s_fix[q] * p.inv_scale_s;
-        p.s_fix[q] = 0ull;
-        const double g = s - (double)p.b[q];
-        const double le = p.lam_eval[q];
-        dot = fma(le, g, dot);
-        if (g > 0.0) { r2 = fma(g, g, r2); rinf = fmax(rinf, g); }
-        if (p.grad_out) p.grad_out[q] = g;
-        if (p.tr_grad) p.tr_grad[p.tr_n * p.JM + q] = g;
-        if (p.update) {
-            const double ln = fmax(0.0, le + p.eta * g);
-            const double lo = p.lam_cur[q];
-            p.lam_cur[q] = ln;
-            p.y[q] = ln + p.beta * (ln - lo);
-            if (p.tr_lam) p.tr_lam[p.tr_n * p.JM + q] = ln;
-        }
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        dot += __shfl_xor_sync(kFull, dot, o);
-        r2 += __shfl_xor_sync(kFull, r2, o);
-        rinf = fmax(rinf, __shfl_xor_sync(kFull, rinf, o));
-    }
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (lane == 0) { sh_dot[warp] = dot; sh_r2[warp] = r2; sh_inf[warp] = rinf; }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        dot = 0.0; r2 = 0.0; rinf = 0.0;
-        for (int w = 0; w < kFinalizeThreads / 32; ++w) { dot += sh_dot[w]; r2 += sh_r2[w]; rinf = fmax(rinf, sh_inf[w]); }
-        const double obj = (double)(long long)p.sc_fix[0] * p.inv_scale_obj;
-        const double reg = 0.5 * p.gamma * ((double)(long long)p.sc_fix[1] * p.inv_scale_sq);
-        p.sc_fix[0] = 0ull; p.sc_fix[1] = 0ull;
-        const double g = obj + reg + dot;
-        const double nr2 = sqrt(r2);
-        if (p.scalars_out) { p.scalars_out[0] = g; p.scalars_out[1] = obj; p.scalars_out[2] = reg; p.scalars_out[3] = rinf; p.scalars_out[4] = nr2; }
-        if (p.tr_g) p.tr_g[p.tr_n] = g;
-        if (p.tr_rinf) p.tr_rinf[p.tr_n] = rinf;
-        if (p.tr_r2) p.tr_r2[p.tr_n] = nr2;
-    }
+    grid_epilogue(f, sh_fin, 256);
 }
 
 // ---- a0: create-time kernels -------------------------------------------------------------------------------

@@ -1,0 +1,172 @@
+"""`-m gpu` parity at BASELINE.json's FULL sizes, in the launch configuration `bench.py` times (rows generated on
+the device, borrowed by the library, default plan).  What is compared:
+
+  * x on sampled users (seeded random users + the longest rows + the first and last rows): the oracle projects
+    exactly those rows one by one (a sub-instance holding only them) -- element-wise |dx| <= 1e-5;
+  * grad g and g against the oracle's full evaluation where the oracle finishes in about a minute (configs 2, 3);
+  * at every size, properties that tie the remaining outputs to the sampled ones: grad g = A x - b and
+    g = c'x + gamma/2 |x|^2 + lambda'grad g re-accumulated in fp64 from the x the kernel wrote (plain torch
+    index_add, an independent reduction), feasibility of every row, and bit-identical results on a second launch.
+
+Config 4 (5e9 nonzeros, 80 GB of rows) needs > 110 GB of device memory and is skipped on smaller devices.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import synth
+
+pytestmark = [pytest.mark.gpu, pytest.mark.slow]
+
+if torch.cuda.is_available():
+    import paper_2606_07777_b200 as pkg
+    from gpu_util import TOL_G, TOL_GRAD, TOL_X, rel_l2
+
+_KIND = {"simplex": ("PROJ_SIMPLEX_INEQ",) * 2, "boxcut": ("PROJ_BOXCUT",) * 2, "box": ("PROJ_BOX",) * 2}
+
+
+def _create(inst, **opt):
+    kind, p0, p1 = synth.proj_spec(inst.cfg)
+    o = pkg.binding.make_opts(projection=getattr(pkg, _KIND[kind][0]), p0=p0, p1=p1, borrow=True, **opt)
+    return pkg.Problem.create(inst.I, inst.J, inst.m, inst.row_ptr, inst.item_idx, inst.c, inst.a, inst.b, o)
+
+
+def _oracle_problem(cfg, I, row_ptr, item_idx, c, a, b):
+    kind, p0, p1 = synth.proj_spec(cfg)
+    return oracle.Problem(I, cfg.J, cfg.m, row_ptr, item_idx, c, a, b, getattr(oracle, _KIND[kind][1]), p0, p1)
+
+
+def _sample_rows(inst, n_random=4000, n_longest=64, seed=1234):
+    """Sorted unique user ids: seeded random users, the longest rows, the first and last 8 rows."""
+    g = torch.Generator().manual_seed(seed)
+    rnd = torch.randint(0, inst.I, (n_random,), generator=g)
+    deg = inst.row_ptr[1:] - inst.row_ptr[:-1]
+    longest = torch.topk(deg, min(n_longest, inst.I)).indices.cpu()
+    ends = torch.cat([torch.arange(0, min(8, inst.I)), torch.arange(max(0, inst.I - 8), inst.I)])
+    return torch.unique(torch.cat([rnd, longest, ends]))
+
+
+def _sub_instance(inst, users):
+    """Host copy of the rows of `users` as a CSR sub-instance + the positions of their nonzeros in the full arrays."""
+    u = users.to(inst.row_ptr.device)
+    beg, end = inst.row_ptr[u], inst.row_ptr[u + 1]
+    deg = end - beg
+    rp = torch.zeros(u.numel() + 1, dtype=torch.int64, device=u.device)
+    torch.cumsum(deg, 0, out=rp[1:])
+    n = int(rp[-1])
+    pos = torch.repeat_interleave(beg - rp[:-1], deg, output_size=n) + torch.arange(n, device=u.device)
+    m = inst.m
+    apos = (pos[:, None] * m + torch.arange(m, device=u.device)[None, :]).reshape(-1)
+    return (rp.cpu().numpy(), inst.item_idx[pos].cpu().numpy(), inst.c[pos].cpu().numpy(), inst.a[apos].cpu().numpy()), pos
+
+
+def _recompute(inst, lam, gamma, x, step=1 << 26):
+    """grad = A x - b, obj = c'x, sum x^2 and the largest row sum, in fp64 from the x the kernel wrote (torch ops)."""
+    J, m = inst.J, inst.m
+    s = torch.zeros(J * m, dtype=torch.float64, device=x.device)
+    obj = torch.zeros((), dtype=torch.float64, device=x.device)
+    sq = torch.zeros((), dtype=torch.float64, device=x.device)
+    for p0 in range(0, inst.nnz, step):
+        p1 = min(inst.nnz, p0 + step)
+        xd = x[p0:p1].double()
+        j = inst.item_idx[p0:p1].long()
+        for k in range(m):
+            s.index_add_(0, j * m + k, inst.a[p0 * m + k:p1 * m:m].double() * xd)
+        obj += (inst.c[p0:p1].double() * xd).sum()
+        sq += (xd * xd).sum()
+    grad = s - inst.b.double()
+    g = obj + 0.5 * gamma * sq + (lam * grad).sum()
+    return grad, float(g), float(obj), float(0.5 * gamma * sq)
+
+
+def _row_sums_max(inst, x, step=2_000_000):
+    worst = 0.0
+    for u0 in range(0, inst.I, step):
+        u1 = min(inst.I, u0 + step)
+        rp = inst.row_ptr[u0:u1 + 1]
+        seg = x[int(rp[0]):int(rp[-1])].double()
+        cs = torch.zeros(seg.numel() + 1, dtype=torch.float64, device=x.device)
+        torch.cumsum(seg, 0, out=cs[1:])
+        rs = cs[rp[1:] - rp[0]] - cs[rp[:-1] - rp[0]]
+        worst = max(worst, float(rs.max()))
+    return worst
+
+
+FULL = [
+    # name, probe-lambda scale, full oracle evaluation?
+    ("cfg2", 0.5, True),
+    ("cfg3", 0.05, True),
+    ("cfg5", 0.5, False),
+    ("cfg4", 0.5, False),
+]
+
+
+@pytest.mark.parametrize("name,lam_scale,full_oracle", FULL, ids=[f[0] for f in FULL])
+def test_full_size_gradient(name, lam_scale, full_oracle):
+    cfg = synth.get_config(name)
+    need = cfg.I * (sum(cfg.deg[1:3]) / 2 if cfg.deg[0] == "uniform" else cfg.deg[1]) * (12 + 4 * cfg.m) * 1.4
+    if torch.cuda.get_device_properties(0).total_memory < need:
+        pytest.skip(f"{name} needs about {need / 1e9:.0f} GB of device memory")
+    inst = synth.generate(cfg, device="cuda")
+    assert inst.short_rows == 0
+    pg = _create(inst)
+    info = pg.info()
+    assert info.streaming == 1 and info.grid_ctas == torch.cuda.get_device_properties(0).multi_processor_count
+    Jm = inst.J * inst.m
+    users = _sample_rows(inst)
+    (rp, idx, c, a), pos = _sub_instance(inst, users)
+    po_sub = _oracle_problem(cfg, users.numel(), rp, idx, c, a, inst.b.cpu().numpy())
+    x = torch.empty(inst.nnz, dtype=torch.float32, device="cuda")
+    grad = torch.empty(Jm, dtype=torch.float64, device="cuda")
+    po_full = None
+    if full_oracle:
+        d = inst.numpy()
+        po_full = _oracle_problem(cfg, inst.I, d["row_ptr"], d["item_idx"], d["c"], d["a"], d["b"])
+    # lambda = 0 is what the verbatim configs evaluate at every iteration (they are slack); the
+    # probe is a busy lambda; "soft" repeats it at 100 x gamma, where a large share of the rows is fractional
+    for which, lam, gamma in (("zero", torch.zeros(Jm, dtype=torch.float64, device="cuda"), cfg.gammas[-1]),
+                              ("probe", synth.probe_lambda(inst, 0, lam_scale), cfg.gammas[-1]),
+                              ("soft", synth.probe_lambda(inst, 1, lam_scale), 100.0 * cfg.gammas[-1])):
+        sc = pkg.Scalars()
+        pg.grad(lam, gamma, grad=grad, scalars=sc, x=x)
+        torch.cuda.synchronize()
+        # (1) sampled rows against the oracle's projection of exactly those rows
+        ref = oracle.grad(po_sub, lam.cpu().numpy(), gamma)
+        xs = x[pos].cpu().numpy().astype(np.float64)
+        ex = np.abs(xs - ref.x).max()
+        assert ex <= TOL_X, f"{name}/{which}: sampled x abs err {ex:.3e}"
+        if which == "soft":
+            nfrac = int(np.sum((ref.x > 1e-6) & (ref.x < 1 - 1e-6)))
+            assert nfrac >= 20, f"{name}: the probe lambda exercises too few fractional entries ({nfrac})"
+        # (2) the reduction and the scalars are consistent with the x that was written
+        g2, gval, obj, reg = _recompute(inst, lam, gamma, x)
+        assert rel_l2(grad.cpu().numpy(), g2.cpu().numpy()) <= TOL_GRAD, f"{name}/{which}: grad vs A x - b"
+        assert abs(sc.g - gval) <= TOL_G * abs(gval) + 1e-9, f"{name}/{which}: g {sc.g} vs {gval}"
+        assert abs(sc.obj - obj) <= TOL_G * abs(obj) + 1e-9 and abs(sc.reg - reg) <= TOL_G * abs(reg) + 1e-9
+        assert float(x.min()) >= 0.0 and _row_sums_max(inst, x) <= 1.0 + 1e-5
+        # (3) the whole evaluation against the oracle
+        if po_full is not None and (which == "probe" or inst.nnz < 50_000_000):
+            rf = oracle.grad(po_full, lam.cpu().numpy(), gamma)
+            assert rel_l2(grad.cpu().numpy(), rf.grad) <= TOL_GRAD, f"{name}/{which}: grad vs oracle"
+            assert abs(sc.g - rf.g) <= TOL_G * abs(rf.g), f"{name}/{which}: g {sc.g} vs oracle {rf.g}"
+            exf = np.abs(x.cpu().numpy() - rf.x).max()
+            assert exf <= TOL_X, f"{name}/{which}: full x abs err {exf:.3e}"
+            del rf
+        # (4) a second launch gives the same bits
+        grad_b, sc_b = torch.empty_like(grad), pkg.Scalars()
+        pg.grad(lam, gamma, grad=grad_b, scalars=sc_b)
+        torch.cuda.synchronize()
+        assert torch.equal(grad, grad_b) and sc.g == sc_b.g
+    pg.destroy()
+
+
+def test_full_size_cfg2_tight_trajectory():
+    """Config 2 at full size with binding constraints: 25 AGD iterations, every iteration's grad g against the oracle."""
+    from gpu_util import assert_trajectory_parity, from_instance
+    inst = synth.generate(synth.get_config("cfg2-tight"), device="cuda")
+    host = synth.Instance(inst.cfg, *(getattr(inst, k).cpu() for k in ("row_ptr", "item_idx", "c", "a", "b")))
+    po, pg = from_instance(host)
+    worst, ex, ref, out = assert_trajectory_parity(po, pg, inst.cfg.gammas, [25], tag="cfg2-tight full")
+    assert (ref.lam > 0).sum() > 50
+    pg.destroy()

@@ -210,3 +210,23 @@ def test_create_rejects_bad_input():
     po, pg = both(good)
     with pytest.raises(pkg.DualipError):
         pg.grad(torch.zeros(3, dtype=torch.float64, device="cuda"), 0.0)           # gamma must be > 0
+
+
+def test_graph_replay_is_the_same_iteration():
+    """use_graph: the stage loop replays a CUDA graph of chained one-launch iterations (beta_t and the trace row come
+    from the device-side iteration state); lambda_T, x, the trace and the scalars carry the same bits as direct
+    launches, across stages (momentum restart) and for iteration counts that are not a multiple of the graph length."""
+    inst = synth.generate(synth.get_config("cfg2-tight", I=20_000))
+    outs = []
+    for graph in (False, True):
+        po, pg = from_instance(inst, use_graph=graph)
+        n0 = pg.info().launches
+        out = gpu_solve(pg, [1e-2, 1e-3], [47, 63])
+        assert pg.info().launches - n0 == 47 + 63 + 1        # one launch per iteration + the final evaluation
+        outs.append(out)
+        if graph:
+            assert_trajectory_parity(po, pg, [1e-2, 1e-3], [47, 63], tag="graph")
+        pg.destroy()
+    a, b = outs
+    assert np.array_equal(a["lam"], b["lam"]) and np.array_equal(a["x"], b["x"]) and a["sc"].g == b["sc"].g
+    assert np.array_equal(a["tr_grad"], b["tr_grad"]) and np.array_equal(a["tr_lam"], b["tr_lam"]) and np.array_equal(a["tr_g"], b["tr_g"])

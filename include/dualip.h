@@ -58,8 +58,10 @@ enum { DUALIP_PROJ_SIMPLEX_INEQ = 0, DUALIP_PROJ_BOX = 1, DUALIP_PROJ_BOXCUT = 2
  *            flushed once per CTA with RED.ADD.64.
  *   GLOBAL : RED.ADD.64 straight to L2 for every nonzero x; lambda still gathered from shared memory
  *            when J*m*8 bytes fit, else through the read-only path.
- *   CSC    : no atomics: x is written to HBM and each item's column is summed in fixed order through
- *            an item-sorted permutation built at create (for J*m beyond on-chip capacity).            */
+ *   CSC    : no atomics: x is written to HBM and each item's column is summed in fixed order (fp64, chunks of 4096
+ *            entries, fixed trees) through an item-sorted permutation built at create -- for J*m beyond on-chip
+ *            capacity, and the mode whose summation ORDER is fixed.  Costs nnz*(4|8) bytes for the permutation,
+ *            nnz*4 for x, and three more launches per evaluation.                                       */
 enum { DUALIP_RED_AUTO = 0, DUALIP_RED_SMEM = 1, DUALIP_RED_GLOBAL = 2, DUALIP_RED_CSC = 3 };
 
 typedef struct {
@@ -71,7 +73,8 @@ typedef struct {
     int32_t momentum;     /* 1: beta_t = t/(t+3) (R1); 0: plain projected ascent (beta = 0) */
     int32_t group_lanes;  /* lanes cooperating on one row: 0 = auto from the mean row length, or 4/8/16/32 */
     int32_t grid_ctas;    /* CTAs of the gradient kernel: 0 = auto (SM count x resident CTAs per SM) */
-    int32_t use_graph;    /* 1: dualip_solve replays a captured CUDA graph per stage; 0: direct launches */
+    int32_t use_graph;    /* 1: dualip_solve replays a CUDA graph of 20 chained iteration launches per stage (stages of >= 40
+                             iterations; ignored while profiling is on or with DUALIP_RED_CSC); 0: direct launches */
     int32_t reserved[5];  /* reserved[0] = 1 forces the direct-load kernel (parity tests of both kernels); rest must be zero */
 } dualip_opts;
 
@@ -164,6 +167,12 @@ int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int3
 /* Replace c (nnz fp32, host or device) in place without rebuilding -- config 5's perturbed re-solve.
  * Recomputes the objective's fixed-point scale.  With borrow = 1 the handle switches to the new pointer. */
 int dualip_set_c(dualip_t* h, const float* c_new, void* stream);
+
+/* DUALIP_RED_CSC only (else DUALIP_EUNSUPPORTED): copies out the item-sorted permutation built at create (a0).
+ *   col_ptr_out[J+1] int64: column j's entries are perm[col_ptr[j] .. col_ptr[j+1]);
+ *   perm_out[nnz] int64: positions into the input nonzero order, ascending inside a column -- bit-exact with a stable
+ *   counting sort of item_idx.  Either pointer may be NULL; host or device.  Synchronises `stream`. */
+int dualip_get_csc(dualip_t* h, int64_t* col_ptr_out, int64_t* perm_out, void* stream);
 
 /* Profiling hook for the measurement harness: when on, every gradient-kernel launch is bracketed by CUDA
  * events recorded on the launching stream (no host synchronisation is added); dualip_get_info waits for the

@@ -16,7 +16,7 @@ PROJ_SIMPLEX_INEQ, PROJ_BOX, PROJ_BOXCUT, PROJ_SIMPLEX_EQ = 0, 1, 2, 3
 RED_AUTO, RED_SMEM, RED_GLOBAL, RED_CSC = 0, 1, 2, 3
 
 EXPORTED_SYMBOLS = ("dualip_opts_default", "dualip_create", "dualip_grad", "dualip_solve", "dualip_set_c",
-                    "dualip_set_profiling", "dualip_get_info", "dualip_destroy", "dualip_strerror")
+                    "dualip_set_profiling", "dualip_get_info", "dualip_get_csc", "dualip_destroy", "dualip_strerror")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 
@@ -86,6 +86,8 @@ def load_library():
         lib.dualip_set_c.argtypes = [vp, vp, vp]
         lib.dualip_get_info.argtypes = [vp, ctypes.POINTER(Info)]
         lib.dualip_set_profiling.argtypes = [vp, ctypes.c_int]
+        lib.dualip_get_csc.argtypes = [vp, vp, vp, vp]
+        lib.dualip_get_csc.restype = ctypes.c_int
         lib.dualip_destroy.argtypes = [vp]
         lib.dualip_destroy.restype = None
         lib.dualip_strerror.argtypes = [ctypes.c_int]
@@ -203,6 +205,10 @@ class Problem:
         _check(load_library().dualip_set_c(self._h, _ptr(c_new, np.float32), _stream_ptr(stream)))
         if self._keep is not None:
             self._keep = self._keep + (c_new,)
+
+    def get_csc(self, col_ptr=None, perm=None, stream=None):
+        """dualip_get_csc: fills col_ptr int64[J+1] and perm int64[nnz] (tensors / arrays or None)."""
+        _check(load_library().dualip_get_csc(self._h, _ptr(col_ptr, np.int64), _ptr(perm, np.int64), _stream_ptr(stream)))
 
     def set_profiling(self, on: bool):
         _check(load_library().dualip_set_profiling(self._h, int(on)))

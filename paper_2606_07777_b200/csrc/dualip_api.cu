@@ -4,7 +4,9 @@
 #include "../../include/dualip.h"
 #include "dualip_kernels.cuh"
 #include "dualip_grad_tma.cuh"
+#include "dualip_csc.cuh"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -21,6 +23,9 @@ constexpr size_t kSmemBudget = 227 * 1024;  // bytes of dynamic shared memory on
 #define DUALIP_NWC 15
 #endif
 constexpr int kTmaConsumerWarps = DUALIP_NWC;  // consumer warps of the streaming kernel (+ 1 producer warp)
+#ifndef DUALIP_LO_SMEM_KB
+#define DUALIP_LO_SMEM_KB 64
+#endif
 
 struct Plan {
     int G = 32, KREG = 5, M = 1;
@@ -52,6 +57,15 @@ struct dualip {
     float* x_stage = nullptr;
     dualip_dev::TileEntry* tiles = nullptr;
     unsigned char* ctl = nullptr;          // [IterState (16 B)][done counter (4 B)] -- see grid_epilogue
+    // DUALIP_RED_CSC: item-sorted permutation (a0) and the per-iteration scratch of the atomics-free reduction
+    bool csc = false, perm64 = false;
+    void* csc_perm = nullptr;              // unsigned[nnz] (nnz < 2^32) or long long[nnz]
+    long long* col_ptr = nullptr;          // [J+1]
+    long long* chunk_ptr = nullptr;        // [J+1]
+    int* chunk_item = nullptr;             // [nchunks]
+    long long nchunks = 0;
+    double* csc_partial = nullptr;         // [nchunks*m]
+    float* x_csc = nullptr;                // [nnz] x of the current evaluation when the caller does not ask for it
     // CUDA graph of kGraphUnroll chained iteration launches (use_graph), re-parameterised per stage
     cudaGraph_t graph = nullptr; cudaGraphExec_t graph_exec = nullptr;
     std::vector<cudaGraphNode_t> graph_nodes;
@@ -167,7 +181,7 @@ bool plan_tma(dualip* h, Plan& pl) {
     // same few addresses would otherwise serialise in L2; beyond that RED.ADD.64 goes straight to L2.
     const size_t fixed = 128 + 128;
     if (fixed + 4 * JM + 32 * 1024 > kSmemBudget) return false;
-    const bool lo = 8 * JM <= 64 * 1024;
+    const bool lo = 8 * JM <= (size_t)DUALIP_LO_SMEM_KB * 1024;
     const size_t lam_bytes = (lo ? 8 : 4) * JM;
     bool acc = (red == DUALIP_RED_AUTO && 16 * JM <= 64 * 1024) ||
                (red == DUALIP_RED_SMEM && fixed + lam_bytes + 8 * JM + 32 * 1024 <= kSmemBudget);
@@ -206,7 +220,6 @@ int make_plan(dualip* h) {
     Plan pl;
     const size_t JM = (size_t)h->J * h->m;
     const int red = h->opts.reduction;
-    if (red == DUALIP_RED_CSC) return DUALIP_EUNSUPPORTED;
     const size_t kScratch = (kFinalizeScratchBytes + 15) & ~(size_t)15;
     const bool fits_both = 16 * JM + kScratch <= kSmemBudget, fits_lam = 8 * JM + kScratch <= kSmemBudget;
     if (red == DUALIP_RED_SMEM && !fits_both) return DUALIP_EUNSUPPORTED;
@@ -221,7 +234,15 @@ int make_plan(dualip* h) {
     if (h->opts.reserved[0] != 1 && plan_tma(h, pl)) {          // reserved[0] = 1 forces the non-streaming kernel (tests)
         // narrow lane groups: several rows share one pass of the chunk loop, which amortises the per-row work
         int Gs = h->opts.group_lanes;
-        if (Gs == 0) Gs = mean <= 6.0 ? 1 : (mean <= 12.0 ? 2 : (mean <= 24.0 ? 4 : (mean <= 256.0 ? 8 : (mean <= 1024.0 ? 16 : 32))));
+        if (Gs == 0) {
+            Gs = mean <= 6.0 ? 1 : (mean <= 12.0 ? 2 : (mean <= 24.0 ? 4 : (mean <= 256.0 ? 8 : (mean <= 1024.0 ? 16 : 32))));
+            // a tile is released only when its slowest row-step is done, so it should split into about as many steps
+            // (2 * 32/G rows each) as there are consumer warps: long rows (few per tile) get wider groups
+            const double rows_per_tile = (double)pl.TN / (mean + kRowCost);
+            int Gt = 1;
+            while (Gt < 32 && (double)Gt * rows_per_tile < 640.0) Gt <<= 1;
+            if (Gt > Gs) Gs = Gt;
+        }
         if (pl.M == 0) Gs = 8;
         pl.G = Gs;
         pl.KREG = 0;
@@ -378,7 +399,7 @@ void fill_finalize_common(const dualip* h, FinalizeParams& f) {
 // Everything one launch needs: function, geometry and the argument block (kept alive by the caller).
 struct IterLaunch {
     const void* fn; dim3 grid, block; size_t smem;
-    GradParams p; FinalizeParams f; TmaParams tp;
+    GradParams p; FinalizeParams f, f_after; TmaParams tp;
     void* args[2];
 };
 
@@ -386,6 +407,12 @@ void prepare_iter(const dualip* h, IterLaunch& L, const double* lam_dev, double 
     fill_grad_params(h, L.p, lam_dev, gamma, x_dev);
     L.f = f_in;
     fill_finalize_common(h, L.f);
+    L.f_after = L.f;
+    if (h->csc) {                       // the kernel only writes x and the scalars; a4-a6 follow as launches of their own
+        L.p.s_fix = nullptr;
+        if (!L.p.x) L.p.x = h->x_csc;
+        L.f.done = nullptr;
+    }
     if (h->opts.projection == DUALIP_PROJ_BOX) {
         L.fn = h->m == 1 ? (const void*)k_grad_box<1> : (h->m == 2 ? (const void*)k_grad_box<2> : (const void*)k_grad_box<0>);
         L.grid = dim3(grid_for(h->nnz, 256, h->num_sms)); L.block = dim3(256); L.smem = 0;
@@ -408,6 +435,75 @@ int launch_iter(dualip* h, IterLaunch& L, cudaStream_t st) {
     const bool timed = prof_begin(h, st);
     struct End { dualip* h; cudaStream_t st; bool on; ~End() { if (on) prof_end(h, st); } } end_guard{h, st, timed};
     CK(cudaLaunchKernel(L.fn, L.grid, L.block, L.args, L.smem, st));
+    h->launches++;
+    CK(cudaGetLastError());
+    if (h->csc) {
+        const int rg = (int)std::min<long long>((h->nchunks + 7) / 8, (long long)h->num_sms * 8);
+        if (h->nchunks > 0) {
+            if (h->perm64) k_csc_reduce<long long><<<rg, 256, 0, st>>>((const long long*)h->csc_perm, h->col_ptr, h->chunk_ptr, h->chunk_item,
+                                                                      h->nchunks, h->a, L.p.x, h->m, h->csc_partial);
+            else k_csc_reduce<unsigned><<<rg, 256, 0, st>>>((const unsigned*)h->csc_perm, h->col_ptr, h->chunk_ptr, h->chunk_item,
+                                                          h->nchunks, h->a, L.p.x, h->m, h->csc_partial);
+            h->launches++;
+        }
+        const long long JM = (long long)h->J * h->m;
+        k_csc_combine<<<(unsigned)((JM + 7) / 8), 256, 0, st>>>(h->chunk_ptr, h->J, h->m, h->csc_partial, h->scale_s, h->s_fix);
+        k_finalize_only<<<1, 1024, 0, st>>>(L.f_after);
+        h->launches += 2;
+        CK(cudaGetLastError());
+    }
+    return DUALIP_OK;
+}
+
+// a0 for DUALIP_RED_CSC: stable counting sort of the nonzero positions by item (dualip_csc.cuh)
+int build_csc(dualip* h, cudaStream_t st) {
+    const long long nnz = h->nnz;
+    const int J = h->J;
+    h->perm64 = nnz >= (1ll << 32);
+    int rc;
+    if ((rc = dev_alloc(h, &h->col_ptr, (size_t)J + 1)) != 0) return rc;
+    if ((rc = dev_alloc(h, &h->chunk_ptr, (size_t)J + 1)) != 0) return rc;
+    if ((rc = dev_alloc(h, &h->x_csc, (size_t)nnz)) != 0) return rc;
+    {
+        void* pp = nullptr;
+        const size_t bytes = (size_t)(nnz > 0 ? nnz : 1) * (h->perm64 ? 8 : 4);
+        if (cudaMalloc(&pp, bytes) != cudaSuccess) { cudaGetLastError(); return DUALIP_ENOMEM; }
+        h->csc_perm = pp; h->bytes_resident += (long long)bytes;
+    }
+    // blocks of positions, one warp each; the (block, item) table is capped at 2^26 entries
+    long long nblocks = (1ll << 26) / J;
+    if (nblocks > 8192) nblocks = 8192;
+    if (nblocks > (nnz + 1023) / 1024) nblocks = (nnz + 1023) / 1024;
+    if (nblocks < 1) nblocks = 1;
+    long long blk_len = (nnz + nblocks - 1) / nblocks;
+    blk_len = (blk_len + 31) & ~31ll;
+    if (blk_len < 32) blk_len = 32;
+    if (blk_len >= (1ll << 32)) return DUALIP_EUNSUPPORTED;                  // a block's per-item count must fit 32 bits
+    unsigned* table = nullptr; long long* total = nullptr; long long* nch = nullptr;
+    if (cudaMalloc(&table, (size_t)nblocks * J * 4) != cudaSuccess) { cudaGetLastError(); return DUALIP_ENOMEM; }
+    if (cudaMalloc(&total, (size_t)J * 16) != cudaSuccess) { cudaGetLastError(); cudaFree(table); return DUALIP_ENOMEM; }
+    nch = total + J;
+    rc = DUALIP_OK;
+    do {
+        if (cudaMemsetAsync(table, 0, (size_t)nblocks * J * 4, st) != cudaSuccess) { rc = DUALIP_ECUDA; break; }
+        const unsigned wg = (unsigned)((nblocks + 7) / 8);
+        k_csc_count<<<wg, 256, 0, st>>>(h->idx, nnz, J, nblocks, blk_len, table);
+        k_csc_block_offsets<<<(J + 255) / 256, 256, 0, st>>>(table, J, nblocks, total, nch);
+        k_scan_exclusive<<<1, 1024, 0, st>>>(total, J, h->col_ptr);
+        k_scan_exclusive<<<1, 1024, 0, st>>>(nch, J, h->chunk_ptr);
+        if (h->perm64) k_csc_scatter<long long><<<wg, 256, 0, st>>>(h->idx, nnz, J, nblocks, blk_len, table, h->col_ptr, (long long*)h->csc_perm);
+        else k_csc_scatter<unsigned><<<wg, 256, 0, st>>>(h->idx, nnz, J, nblocks, blk_len, table, h->col_ptr, (unsigned*)h->csc_perm);
+        h->launches += 5;
+        long long nc = 0;
+        if (cudaMemcpyAsync(&nc, h->chunk_ptr + J, 8, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+            cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) { rc = DUALIP_ECUDA; break; }
+        h->nchunks = nc;
+    } while (0);
+    cudaFree(table); cudaFree(total);
+    if (rc != 0) return rc;
+    if ((rc = dev_alloc(h, &h->chunk_item, (size_t)h->nchunks)) != 0) return rc;
+    if ((rc = dev_alloc(h, &h->csc_partial, (size_t)h->nchunks * h->m)) != 0) return rc;
+    k_csc_chunk_items<<<(J + 255) / 256, 256, 0, st>>>(h->chunk_ptr, J, h->chunk_item);
     h->launches++;
     CK(cudaGetLastError());
     return DUALIP_OK;
@@ -481,6 +577,8 @@ void dualip_destroy(dualip_t* h) {
     cudaFree(h->grad_stage); cudaFree(h->scalars_dev); cudaFree(h->x_stage); cudaFree(h->tiles);
     drop_graph(h);
     cudaFree(h->ctl);
+    cudaFree(h->csc_perm); cudaFree(h->col_ptr); cudaFree(h->chunk_ptr); cudaFree(h->chunk_item); cudaFree(h->csc_partial);
+    cudaFree(h->x_csc);
     for (cudaEvent_t e : h->events) cudaEventDestroy(e);
     cudaGetLastError();
     delete h;
@@ -595,6 +693,10 @@ int dualip_create(dualip_t** out, int64_t I, int32_t J, int32_t m, const int64_t
         set_xmax(h);
         set_scales(h);
         if ((rc = make_plan(h)) != 0) goto fail;
+        if (o.reduction == DUALIP_RED_CSC) {
+            h->csc = true;
+            if ((rc = build_csc(h, st)) != 0) goto fail;
+        }
         if (h->plan.tma) {
             if ((rc = dev_alloc(h, &h->tiles, (size_t)h->plan.ntiles + 1)) != 0) goto fail;
             k_build_tiles<<<grid_for(h->plan.ntiles + 1, 128, h->num_sms), 128, 0, st>>>(h->row_ptr, I, h->plan.TN, h->plan.ntiles, h->tiles);
@@ -619,7 +721,7 @@ int dualip_get_info(dualip_t* h, dualip_info* info) {
     info->I = h->I; info->nnz = h->nnz; info->J = h->J; info->m = h->m; info->L = h->L;
     info->max_row_len = h->max_row_len;
     info->group_lanes = h->plan.G; info->chunk_regs = h->plan.KREG;
-    info->reduction = h->plan.acc_smem ? DUALIP_RED_SMEM : DUALIP_RED_GLOBAL;
+    info->reduction = h->csc ? DUALIP_RED_CSC : (h->plan.acc_smem ? DUALIP_RED_SMEM : DUALIP_RED_GLOBAL);
     info->lambda_in_smem = h->plan.lam_smem ? 1 : 0;
     info->grid_ctas = h->plan.grid; info->block_threads = h->plan.tma ? 32 * (kTmaConsumerWarps + 1) : kBlockThreads;
     info->streaming = h->plan.tma ? 1 : 0; info->stages = h->plan.stages; info->tile_units = h->plan.TN; info->ntiles = h->plan.ntiles;
@@ -627,6 +729,28 @@ int dualip_get_info(dualip_t* h, dualip_info* info) {
     info->bytes_resident = h->bytes_resident; info->launches = h->launches;
     info->fix_scale_s = h->scale_s;
     info->grad_kernel_ms = h->prof_ms; info->grad_kernel_count = h->prof_count;
+    return DUALIP_OK;
+}
+
+int dualip_get_csc(dualip_t* h, int64_t* col_ptr_out, int64_t* perm_out, void* stream) {
+    if (!h) return DUALIP_EINVAL;
+    if (!h->csc) return DUALIP_EUNSUPPORTED;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (col_ptr_out) CK(cudaMemcpyAsync(col_ptr_out, h->col_ptr, ((size_t)h->J + 1) * 8, cudaMemcpyDefault, st));
+    if (perm_out && h->nnz > 0) {
+        if (h->perm64) CK(cudaMemcpyAsync(perm_out, h->csc_perm, (size_t)h->nnz * 8, cudaMemcpyDefault, st));
+        else {
+            long long* tmp = nullptr;
+            if (cudaMalloc(&tmp, (size_t)h->nnz * 8) != cudaSuccess) { cudaGetLastError(); return DUALIP_ENOMEM; }
+            k_perm_widen<<<grid_for(h->nnz, 256, h->num_sms), 256, 0, st>>>((const unsigned*)h->csc_perm, h->nnz, tmp);
+            h->launches++;
+            const cudaError_t e1 = cudaMemcpyAsync(perm_out, tmp, (size_t)h->nnz * 8, cudaMemcpyDefault, st);
+            const cudaError_t e2 = cudaStreamSynchronize(st);
+            cudaFree(tmp);
+            if (e1 != cudaSuccess || e2 != cudaSuccess) { cudaGetLastError(); return DUALIP_ECUDA; }
+        }
+    }
+    CK(cudaStreamSynchronize(st));
     return DUALIP_OK;
 }
 
@@ -704,7 +828,7 @@ int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int3
         int t = 0;
         // beta_t and the trace row come from the device-side iteration state, so every launch of a stage has the
         // same arguments: replay a graph of kGraphUnroll chained launches, then finish with direct launches
-        if (h->opts.use_graph && !h->profile && iters[s] >= 2 * kGraphUnroll) {
+        if (h->opts.use_graph && !h->profile && !h->csc && iters[s] >= 2 * kGraphUnroll) {
             int rc = set_graph(h, it);
             if (rc != 0) return rc;
             for (; t + kGraphUnroll <= iters[s]; t += kGraphUnroll) {

@@ -123,6 +123,7 @@ template <int M, bool ACC_SMEM>
 __device__ __forceinline__ void push(const GradParams& p, const ConsumerCtx& cx, FixPair& fp, int mm, int j, float cc, const float* aa, float x) {
     fp.obj += to_fix32(cc * x, p.scale_obj_f);
     fp.sq += to_fix32(x * x, p.scale_sq_f);
+    if (!ACC_SMEM && p.s_fix == nullptr) return;          // DUALIP_RED_CSC
 #pragma unroll
     for (int f = 0; f < (M > 0 ? M : 4); ++f) {
         if (f < mm) {

@@ -35,7 +35,7 @@ struct GradParams {
     const float* __restrict__ c;
     const float* __restrict__ a;
     const double* __restrict__ lambda;
-    unsigned long long* s_fix;   // [J*m] item accumulators, fixed point, zero on entry
+    unsigned long long* s_fix;   // [J*m] item accumulators, fixed point, zero on entry; nullptr = do not accumulate (CSC)
     unsigned long long* sc_fix;  // [2]   obj = c'x and |x|^2, fixed point, zero on entry
     float* x;                    // [nnz] or nullptr
     long long I;
@@ -116,6 +116,7 @@ template <int M, bool ACC_SMEM>
 __device__ __forceinline__ void contribute(const GradParams& p, unsigned* s_lo, unsigned* s_hi, int mm, int j,
                                            const float (&aa)[M > 0 ? M : 4], float x) {
     const int nm = M > 0 ? M : mm;
+    if (!ACC_SMEM && p.s_fix == nullptr) return;          // DUALIP_RED_CSC: the item sums are taken from x afterwards
 #pragma unroll
     for (int k = 0; k < (M > 0 ? M : 4); ++k) {
         if (k < nm) {
@@ -225,6 +226,7 @@ __device__ __forceinline__ void finalize_block(const FinalizeParams& p, double* 
 // memory no longer used for anything else.  Every thread of the CTA must call it after its last accumulator flush.
 __device__ __forceinline__ void grid_epilogue(const FinalizeParams& f, double* sh, int nthreads) {
     int* flag = reinterpret_cast<int*>(sh + 96);
+    if (f.done == nullptr) return;                      // DUALIP_RED_CSC: a4-a6 run as launches of their own
     __threadfence();                                    // this thread's RED/atomics are visible device-wide
     __syncthreads();
     if (threadIdx.x == 0) *flag = (atomicAdd(f.done, 1u) == gridDim.x - 1) ? 1 : 0;

@@ -230,3 +230,45 @@ def test_graph_replay_is_the_same_iteration():
     a, b = outs
     assert np.array_equal(a["lam"], b["lam"]) and np.array_equal(a["x"], b["x"]) and a["sc"].g == b["sc"].g
     assert np.array_equal(a["tr_grad"], b["tr_grad"]) and np.array_equal(a["tr_lam"], b["tr_lam"]) and np.array_equal(a["tr_g"], b["tr_g"])
+
+
+@pytest.mark.parametrize("tag,I,J,m,lens", [CASES[1], CASES[3], CASES[4], CASES[5], CASES[8]], ids=lambda c: c if isinstance(c, str) else None)
+@pytest.mark.parametrize("kind,p0,p1", [("simplex", 1.0, 0.0), ("boxcut", 0.3, 1.0), ("box", 0.0, 0.4)])
+def test_csc_reduction_parity_and_permutation(tag, I, J, m, lens, kind, p0, p1):
+    """DUALIP_RED_CSC: the item-sorted permutation is bit-exact with a stable counting sort of item_idx, and the
+    atomics-free reduction through it meets the same tolerances, evaluation and trajectory."""
+    rng = np.random.default_rng(sum(map(ord, tag + kind)) * 17 + 3)
+    d = _ragged(rng, I, J, m, lens)
+    po, pg = both(d, kind, p0, p1, reduction=pkg.RED_CSC)
+    assert pg.info().reduction == pkg.RED_CSC
+    col_ptr, perm = np.empty(J + 1, dtype=np.int64), np.empty(po.nnz, dtype=np.int64)
+    pg.get_csc(col_ptr, perm)
+    assert np.array_equal(perm, np.argsort(po.item_idx, kind="stable"))
+    assert np.array_equal(col_ptr, np.concatenate([[0], np.cumsum(np.bincount(po.item_idx, minlength=J))]))
+    for gamma in (1e-1, 1e-3):
+        lam = rng.random(J * m) * 0.3
+        assert_grad_parity(po, pg, lam, gamma, tag=f"csc/{tag}/{kind}/g={gamma}")
+    if po.nnz:
+        assert_trajectory_parity(po, pg, [1e-1, 1e-2], [12, 9], tag=f"csc/{tag}/{kind}")
+    with pytest.raises(pkg.DualipError):
+        both(d, kind, p0, p1)[1].get_csc(col_ptr, perm)          # only the CSC mode has a permutation
+    pg.destroy()
+
+
+def test_csc_matches_atomic_modes_at_scale():
+    """Config 3's recipe (Zipf columns: the longest column holds most users) at 200k users: CSC against the
+    fixed-point modes, permutation against numpy, two launches bit-identical."""
+    inst = synth.generate(synth.get_config("cfg3-tight", I=200_000))
+    lam = synth.probe_lambda(inst, 0, 0.05).numpy()
+    po, pg = from_instance(inst, reduction=pkg.RED_CSC)
+    perm = np.empty(po.nnz, dtype=np.int64)
+    pg.get_csc(None, perm)
+    assert np.array_equal(perm, np.argsort(po.item_idx, kind="stable"))
+    sc1, g1, x1 = gpu_grad(pg, lam, 1e-3)
+    sc2, g2, x2 = gpu_grad(pg, lam, 1e-3)
+    assert np.array_equal(g1, g2) and sc1.g == sc2.g
+    assert_grad_parity(po, pg, lam, 1e-3, tag="csc/cfg3")
+    po2, pg2 = from_instance(inst)
+    sc3, g3, x3 = gpu_grad(pg2, lam, 1e-3)
+    assert np.array_equal(x1, x3) and rel_l2(g1, g3) < 1e-9
+    pg.destroy(); pg2.destroy()

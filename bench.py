@@ -147,7 +147,12 @@ def run_reference(args):
 
     import oracle
     import synth
-    users = min(args.cpu_users // 2, 400_000) if args.users is None else args.users
+    # bounded sample: about 1.5e9 nonzero-visits in the whole run (~2 minutes at the oracle's ~1.4e7 nnz/s per core),
+    # split over the K + W steps; every step is one full oracle iteration over the first `users` users of the workload
+    full0 = synth.get_config(args.workload)
+    mean_deg = {"const": lambda d: d[1], "uniform": lambda d: (d[1] + d[2]) / 2, "poisson": lambda d: d[1]}[full0.deg[0]](full0.deg)
+    users = int(1.5e9 / max(args.steps + args.warmup, 1) / mean_deg)
+    users = max(2_000, min(users, 400_000, full0.I)) if args.users is None else args.users
     cfg = synth.get_config(args.workload, I=users)
     dev = "cuda" if torch.cuda.is_available() else "cpu"
     inst = synth.generate(cfg, device=dev)
@@ -161,7 +166,7 @@ def run_reference(args):
     line = {"metric": METRIC, "value": val, "unit": UNIT, "impl": "reference", "n_gpus": args.gpus, "steps": len(times),
             "warmup": args.warmup, "ms_per_step": 1e3 * tot / len(times), "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{args.workload} (BASELINE.json configs[2]: {full.I} users x {full.J} items); bounded sample",
+            "config": {"workload": f"{args.workload} (BASELINE.json configs[{int(args.workload[3]) - 1}]: {full.I} users x {full.J} items); bounded sample",
                        "sample_users": users, "sample_nnz": po.nnz, "gamma": cfg.gammas[-1]},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -180,21 +185,12 @@ def main():
     import paper_2606_07777_b200 as pkg
     import synth
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
-    torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group(backend="nccl", device_id=torch.device("cuda", local))
-
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
+    from paper_2606_07777_b200.replicas import Replicas
+    rep = Replicas(backend="nccl")                       # replicas only: barrier + max-over-ranks, nothing on the data path
+    world, rank, local = rep.world, rep.rank, rep.local_rank
+    barrier = rep.barrier
 
     # ---- workload: generated on the device (replicas only: every rank holds the whole job) ----
     cfg = synth.get_config(args.workload, I=args.users)
@@ -239,10 +235,7 @@ def main():
     launches = inf.launches - launches0
     kern_ms = inf.grad_kernel_ms / max(inf.grad_kernel_count, 1) if not args.graph else ms_total / args.steps
     prob.set_profiling(False)
-    t_max = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t_max, op=dist.ReduceOp.MAX)
-    ms_total_max = float(t_max.item())
+    ms_total_max = rep.max_over_ranks(ms_total)
     value = world * nnz * args.steps / (ms_total_max * 1e-3)
 
     # ---- end to end through the C ABI with host buffers (create + solve + readback, all timed) ----
@@ -265,10 +258,7 @@ def main():
         p2.solve([gamma], [args.steps], lam_h, scalars=sc)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        t_e2e = torch.tensor([dt], dtype=torch.float64, device="cuda")
-        if dist is not None:
-            dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
-        dt = float(t_e2e.item())
+        dt = rep.max_over_ranks(dt)
         h2d = sum(v.nbytes for v in host.values()) + lam_h.nbytes
         d2h = lam_h.nbytes + 5 * 8
         e2e = {"value": world * nnz * args.steps / dt, "unit": UNIT, "h2d_bytes_per_step": h2d / args.steps,
@@ -286,9 +276,9 @@ def main():
         sample = {"row_ptr": inst.row_ptr[:nu + 1].cpu().numpy(), "item_idx": inst.item_idx[:end].cpu().numpy(),
                   "c": inst.c[:end].cpu().numpy(), "a": inst.a[:end * inst.m].cpu().numpy(), "b": inst.b.cpu().numpy()}
         po = oracle_problem(sample, cfg, oracle, synth)
-        times = time_oracle_steps(po, gamma, 2, 0, oracle)
+        times = time_oracle_steps(po, gamma, 3, 0, oracle)
         cpu = {"value": po.nnz * len(times) / float(np.sum(times)), "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": f"2 AGD iterations over the first {nu} users ({po.nnz} nnz) of the same instance; "
+               "sample": f"3 AGD iterations over the first {nu} users ({po.nnz} nnz) of the same instance; "
                          f"oracle/dualip_oracle.c as it stands, 1 thread, fp64; {float(np.sum(times)):.1f} s of CPU work",
                "host_cores_available": len(os.sched_getaffinity(0))}
 
@@ -321,8 +311,7 @@ def main():
         }
         print(json.dumps(line), flush=True)
     prob.destroy()
-    if dist is not None:
-        dist.destroy_process_group()
+    rep.close()
 
 
 if __name__ == "__main__":

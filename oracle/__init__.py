@@ -52,8 +52,10 @@ def _load():
         lib.dualip_oracle_grad.restype = ctypes.c_int
         lib.dualip_oracle_lipschitz.argtypes = [i64, i32, i32, vp, vp, vp]
         lib.dualip_oracle_lipschitz.restype = d
+        lib.dualip_oracle_jacobi_scaling.argtypes = [i64, i32, i32, vp, vp, vp, vp]
+        lib.dualip_oracle_jacobi_scaling.restype = None
         lib.dualip_oracle_solve.argtypes = [i64, i32, i32, vp, vp, vp, vp, vp, ctypes.c_int, d, d,
-                                            vp, i32, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+                                            vp, i32, vp, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         lib.dualip_oracle_solve.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -155,6 +157,13 @@ def lipschitz(p: Problem) -> float:
     return float(_load().dualip_oracle_lipschitz(p.I, p.J, p.m, _ptr(p.row_ptr), _ptr(p.item_idx), _ptr(p.a)))
 
 
+def jacobi_scaling(p: Problem) -> np.ndarray:
+    """diag(D), D_rr = 1/|A_r*|_2 per coupling row r = (j,k), 1 for rows of zero norm."""
+    d = np.empty(p.J * p.m, dtype=np.float64)
+    _load().dualip_oracle_jacobi_scaling(p.I, p.J, p.m, _ptr(p.row_ptr), _ptr(p.item_idx), _ptr(p.a), _ptr(d))
+    return d
+
+
 @dataclass
 class SolveResult:
     lam: np.ndarray
@@ -169,8 +178,9 @@ class SolveResult:
 
 
 def solve(p: Problem, gammas, iters, lam0=None, momentum: bool = True, want_x: bool = True,
-          trace_grad: bool = False, trace_lambda: bool = False, stage_x: bool = False) -> SolveResult:
-    """gamma-continuation + projected Nesterov ascent (readings R1-R4)."""
+          trace_grad: bool = False, trace_lambda: bool = False, stage_x: bool = False, jacobi: bool = False) -> SolveResult:
+    """gamma-continuation + projected Nesterov ascent (readings R1-R4); jacobi: on the row-scaled
+    system A' = D A, b' = D b, results reported in the original units (R18)."""
     gammas = _f64(gammas).reshape(-1)
     iters = np.ascontiguousarray(np.asarray(iters, dtype=np.int32)).reshape(-1)
     assert gammas.size == iters.size
@@ -184,7 +194,7 @@ def solve(p: Problem, gammas, iters, lam0=None, momentum: bool = True, want_x: b
     sx = np.empty((gammas.size, p.nnz)) if stage_x else None
     rc = _load().dualip_oracle_solve(p.I, p.J, p.m, _ptr(p.row_ptr), _ptr(p.item_idx), _ptr(p.c), _ptr(p.a),
                                      _ptr(p.b), p.proj_kind, p.p0, p.p1, _ptr(gammas), gammas.size, _ptr(iters),
-                                     1 if momentum else 0, _ptr(lam), _ptr(x), _ptr(sc), _ptr(fg),
+                                     1 if momentum else 0, 1 if jacobi else 0, _ptr(lam), _ptr(x), _ptr(sc), _ptr(fg),
                                      _ptr(tg), _ptr(ti), _ptr(t2), _ptr(tgrad), _ptr(tlam), _ptr(sx))
     if rc != 0:
         raise MemoryError("oracle solve failed")

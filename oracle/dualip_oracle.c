@@ -123,10 +123,10 @@ static void project(int kind, double p0, double p1, const double* v, int64_t n, 
  * proj params: simplex kinds p0 = z; box p0 = lo, p1 = hi; boxcut p0 = ub, p1 = z.
  * scalars_out[5] = { g, obj = c'x, reg = (gamma/2)|x|^2, r_inf = max(0, max grad), r_2 = |max(grad,0)|_2 }.
  * x_out (nnz doubles, input order) may be NULL.  Returns 0, or -1 on allocation failure. */
-int dualip_oracle_grad(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr, const int32_t* item_idx,
-                       const float* c, const float* a, const float* b, const double* lambda, double gamma,
-                       int proj_kind, double p0, double p1, double* grad_out, double* scalars_out,
-                       double* x_out) {
+static int grad_f64(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr, const int32_t* item_idx,
+                    const float* c, const double* a, const double* b, const double* lambda, double gamma,
+                    int proj_kind, double p0, double p1, double* grad_out, double* scalars_out,
+                    double* x_out) {
     int64_t max_len = 0;
     for (int64_t i = 0; i < I; ++i)
         if (row_ptr[i + 1] - row_ptr[i] > max_len) max_len = row_ptr[i + 1] - row_ptr[i];
@@ -141,13 +141,13 @@ int dualip_oracle_grad(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr, 
         for (int64_t p = 0; p < n; ++p) {
             int64_t j = item_idx[beg + p];
             double al = 0.0;                                     /* (A' lambda)_p = sum_k a^k_p lambda_{j,k} */
-            for (int32_t k = 0; k < m; ++k) al += (double)a[(beg + p) * m + k] * lambda[j * m + k];
+            for (int32_t k = 0; k < m; ++k) al += a[(beg + p) * m + k] * lambda[j * m + k];
             v[p] = -((double)c[beg + p] + al) / gamma;           /* Eq. 3 argument */
         }
         project(proj_kind, p0, p1, v, n, x);
         for (int64_t p = 0; p < n; ++p) {
             int64_t j = item_idx[beg + p];
-            for (int32_t k = 0; k < m; ++k) grad_out[j * m + k] += (double)a[(beg + p) * m + k] * x[p];
+            for (int32_t k = 0; k < m; ++k) grad_out[j * m + k] += a[(beg + p) * m + k] * x[p];
             obj += (double)c[beg + p] * x[p];
             sq += x[p] * x[p];
             if (x_out) x_out[beg + p] = x[p];
@@ -155,7 +155,7 @@ int dualip_oracle_grad(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr, 
     }
     double reg = 0.5 * gamma * sq, dot = 0.0, r_inf = 0.0, r2 = 0.0;
     for (int64_t q = 0; q < Jm; ++q) {
-        grad_out[q] -= (double)b[q];                             /* Eq. 4 */
+        grad_out[q] -= b[q];                                     /* Eq. 4 */
         dot += lambda[q] * grad_out[q];
         if (grad_out[q] > 0.0) { r2 += grad_out[q] * grad_out[q]; if (grad_out[q] > r_inf) r_inf = grad_out[q]; }
     }
@@ -168,18 +168,61 @@ int dualip_oracle_grad(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr, 
     return 0;
 }
 
+/* The fp32 inputs cast exactly to fp64 (a and b; c is cast where it is used). */
+static double* widen(const float* v, int64_t n) {
+    double* w = (double*)malloc((size_t)(n > 0 ? n : 1) * sizeof(double));
+    if (w) for (int64_t q = 0; q < n; ++q) w[q] = (double)v[q];
+    return w;
+}
+
+int dualip_oracle_grad(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr, const int32_t* item_idx,
+                       const float* c, const float* a, const float* b, const double* lambda, double gamma,
+                       int proj_kind, double p0, double p1, double* grad_out, double* scalars_out,
+                       double* x_out) {
+    double* a64 = widen(a, row_ptr[I] * m);
+    double* b64 = widen(b, (int64_t)J * m);
+    int rc = -1;
+    if (a64 && b64)
+        rc = grad_f64(I, J, m, row_ptr, item_idx, c, a64, b64, lambda, gamma, proj_kind, p0, p1, grad_out, scalars_out, x_out);
+    free(a64); free(b64);
+    return rc;
+}
+
 /* L = max_j sum_k sum_i (a^k_ij)^2  (reading R2: |A|_2^2 exactly for m = 1 because A A' is then
  * diag(sum_i a_ij^2); a trace upper bound on the m x m Gram blocks for m > 1). */
-double dualip_oracle_lipschitz(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr,
-                               const int32_t* item_idx, const float* a) {
+static double lipschitz_f64(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr,
+                            const int32_t* item_idx, const double* a) {
     double* col = (double*)calloc((size_t)J, sizeof(double));
     if (!col) return -1.0;
     for (int64_t p = 0; p < row_ptr[I]; ++p)
-        for (int32_t k = 0; k < m; ++k) col[item_idx[p]] += (double)a[p * m + k] * (double)a[p * m + k];
+        for (int32_t k = 0; k < m; ++k) col[item_idx[p]] += a[p * m + k] * a[p * m + k];
     double L = 0.0;
     for (int32_t j = 0; j < J; ++j) if (col[j] > L) L = col[j];
     free(col);
     return L;
+}
+
+double dualip_oracle_lipschitz(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr,
+                               const int32_t* item_idx, const float* a) {
+    double* a64 = widen(a, row_ptr[I] * m);
+    if (!a64) return -1.0;
+    double L = lipschitz_f64(I, J, m, row_ptr, item_idx, a64);
+    free(a64);
+    return L;
+}
+
+/* Jacobi preconditioning / row normalisation (Appendix B.2):
+ *   D = diag(|A_r*|_2^-1) over the coupling rows r = (j,k) (rows of zero norm keep D_rr = 1),
+ *   A' = D A, b' = D b.  The feasible set is unchanged and diag(A'A'^T) = I on the nonzero rows.
+ * d_out[J*m] receives the diagonal of D.  |A_r*|_2^2 = sum_i (a^k_ij)^2 by Definition 1. */
+void dualip_oracle_jacobi_scaling(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr,
+                                  const int32_t* item_idx, const float* a, double* d_out) {
+    int64_t Jm = (int64_t)J * m;
+    for (int64_t q = 0; q < Jm; ++q) d_out[q] = 0.0;
+    for (int64_t p = 0; p < row_ptr[I]; ++p)
+        for (int32_t k = 0; k < m; ++k)
+            d_out[(int64_t)item_idx[p] * m + k] += (double)a[p * m + k] * (double)a[p * m + k];
+    for (int64_t q = 0; q < Jm; ++q) d_out[q] = d_out[q] > 0.0 ? 1.0 / sqrt(d_out[q]) : 1.0;
 }
 
 /* gamma-continuation driver with projected Nesterov ascent (readings R1-R4 in DESIGN.md; the paper
@@ -194,47 +237,76 @@ double dualip_oracle_lipschitz(int64_t I, int32_t J, int32_t m, const int64_t* r
  * Traces (each may be NULL) are indexed by the global iteration counter n = 0..sum(iters)-1:
  *   trace_g[n] = g(y_t), trace_rinf[n], trace_r2[n], trace_grad[n*Jm..] = grad(y_t),
  *   trace_lambda[n*Jm..] = lambda_{t+1}.  stage_x (may be NULL) receives, per stage, x*(lambda_end)
- *   at that stage's gamma (n_stages * nnz doubles) -- used by the drift report of config 5. */
+ *   at that stage's gamma (n_stages * nnz doubles) -- used by the drift report of config 5.
+ * jacobi != 0 (reading R18): the whole loop runs on the row-scaled system
+ *   A' = D A, b' = D b with its own L' and dual lambda' (warm start lambda'_0 = D^-1 lambda_0); since
+ *   A'^T lambda' = A^T (D lambda'), the dual of the ORIGINAL system is lambda = D lambda' and
+ *   grad g = D^-1 grad g'.  What is returned (lambda, grad, residuals, traces) is in original units. */
 int dualip_oracle_solve(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr, const int32_t* item_idx,
                         const float* c, const float* a, const float* b, int proj_kind, double p0, double p1,
-                        const double* gammas, int32_t n_stages, const int32_t* iters, int32_t momentum,
+                        const double* gammas, int32_t n_stages, const int32_t* iters, int32_t momentum, int32_t jacobi,
                         double* lambda_inout, double* x_out, double* final_scalars, double* final_grad,
                         double* trace_g, double* trace_rinf, double* trace_r2, double* trace_grad,
                         double* trace_lambda, double* stage_x) {
     int64_t Jm = (int64_t)J * m, nnz = row_ptr[I];
-    double L = dualip_oracle_lipschitz(I, J, m, row_ptr, item_idx, a);
-    if (!(L > 0.0)) L = 1.0;
+    double* as = widen(a, nnz * m);                              /* A  (or A' = D A) */
+    double* bs = widen(b, Jm);                                   /* b  (or b' = D b) */
+    double* d = (double*)malloc((size_t)Jm * sizeof(double));
     double* y = (double*)malloc((size_t)Jm * sizeof(double));
     double* grad = (double*)malloc((size_t)Jm * sizeof(double));
+    double* lam = (double*)malloc((size_t)Jm * sizeof(double));  /* dual of the system being iterated on */
     double* lam_new = (double*)malloc((size_t)Jm * sizeof(double));
-    if (!y || !grad || !lam_new) { free(y); free(grad); free(lam_new); return -1; }
+    double* out = (double*)malloc((size_t)Jm * sizeof(double));
+    if (!as || !bs || !d || !y || !grad || !lam || !lam_new || !out) {
+        free(as); free(bs); free(d); free(y); free(grad); free(lam); free(lam_new); free(out); return -1;
+    }
+    for (int64_t q = 0; q < Jm; ++q) d[q] = 1.0;
+    if (jacobi) {
+        dualip_oracle_jacobi_scaling(I, J, m, row_ptr, item_idx, a, d);
+        for (int64_t p = 0; p < nnz; ++p)
+            for (int32_t k = 0; k < m; ++k) as[p * m + k] *= d[(int64_t)item_idx[p] * m + k];
+        for (int64_t q = 0; q < Jm; ++q) bs[q] *= d[q];
+    }
+    for (int64_t q = 0; q < Jm; ++q) lam[q] = lambda_inout[q] / d[q];
+    double L = lipschitz_f64(I, J, m, row_ptr, item_idx, as);
+    if (!(L > 0.0)) L = 1.0;
     double sc[5];
     int64_t n = 0;
     int rc = 0;
     for (int32_t s = 0; s < n_stages && rc == 0; ++s) {
         double gamma = gammas[s], eta = gamma / L;
-        memcpy(y, lambda_inout, (size_t)Jm * sizeof(double));    /* warm start, momentum restart */
+        memcpy(y, lam, (size_t)Jm * sizeof(double));             /* warm start, momentum restart */
         for (int32_t t = 0; t < iters[s] && rc == 0; ++t, ++n) {
-            rc = dualip_oracle_grad(I, J, m, row_ptr, item_idx, c, a, b, y, gamma, proj_kind, p0, p1, grad, sc, NULL);
+            rc = grad_f64(I, J, m, row_ptr, item_idx, c, as, bs, y, gamma, proj_kind, p0, p1, grad, sc, NULL);
             if (trace_g) trace_g[n] = sc[0];
-            if (trace_rinf) trace_rinf[n] = sc[3];
-            if (trace_r2) trace_r2[n] = sc[4];
-            if (trace_grad) memcpy(trace_grad + n * Jm, grad, (size_t)Jm * sizeof(double));
+            if (trace_grad || trace_rinf || trace_r2) {          /* residuals of the original rows: grad g = D^-1 grad g' */
+                double r_inf = 0.0, r2 = 0.0;
+                for (int64_t q = 0; q < Jm; ++q) {
+                    out[q] = grad[q] / d[q];
+                    if (out[q] > 0.0) { r2 += out[q] * out[q]; if (out[q] > r_inf) r_inf = out[q]; }
+                }
+                if (trace_rinf) trace_rinf[n] = r_inf;
+                if (trace_r2) trace_r2[n] = sqrt(r2);
+                if (trace_grad) memcpy(trace_grad + n * Jm, out, (size_t)Jm * sizeof(double));
+            }
             double beta = momentum ? (double)t / (double)(t + 3) : 0.0;
             for (int64_t q = 0; q < Jm; ++q) {
                 lam_new[q] = fmax(0.0, y[q] + eta * grad[q]);
-                y[q] = lam_new[q] + beta * (lam_new[q] - lambda_inout[q]);
+                y[q] = lam_new[q] + beta * (lam_new[q] - lam[q]);
             }
-            memcpy(lambda_inout, lam_new, (size_t)Jm * sizeof(double));
-            if (trace_lambda) memcpy(trace_lambda + n * Jm, lam_new, (size_t)Jm * sizeof(double));
+            memcpy(lam, lam_new, (size_t)Jm * sizeof(double));
+            if (trace_lambda) for (int64_t q = 0; q < Jm; ++q) trace_lambda[n * Jm + q] = d[q] * lam[q];
         }
         if (stage_x && rc == 0)
-            rc = dualip_oracle_grad(I, J, m, row_ptr, item_idx, c, a, b, lambda_inout, gamma, proj_kind, p0, p1,
-                                    grad, sc, stage_x + (int64_t)s * nnz);
+            rc = grad_f64(I, J, m, row_ptr, item_idx, c, as, bs, lam, gamma, proj_kind, p0, p1,
+                          grad, sc, stage_x + (int64_t)s * nnz);
     }
+    for (int64_t q = 0; q < Jm; ++q) lambda_inout[q] = d[q] * lam[q];
+    /* final report: one evaluation of the ORIGINAL system at lambda_T = D lambda'_T (same x, same g) */
     if (rc == 0 && n_stages > 0)
         rc = dualip_oracle_grad(I, J, m, row_ptr, item_idx, c, a, b, lambda_inout, gammas[n_stages - 1],
                                 proj_kind, p0, p1, final_grad ? final_grad : grad, final_scalars ? final_scalars : sc, x_out);
+    free(as); free(bs); free(d); free(lam); free(out);
     free(y); free(grad); free(lam_new);
     return rc;
 }

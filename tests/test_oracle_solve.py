@@ -165,3 +165,115 @@ def test_drift_bound():
         x2 = oracle.grad(_problem(d2), lam, gamma).x
         dc = np.linalg.norm(d["c"].astype(np.float64) - d2["c"].astype(np.float64))
         assert np.linalg.norm(x1 - x2) <= dc / gamma + 1e-12
+
+
+# ---- Jacobi preconditioning / row normalisation (reading R18) ------------------------
+
+def _explicit_A(d):
+    """The (J*m) x nnz coupling matrix of Definition 1, row r = j*m + k, written out densely."""
+    nnz, m = d["item_idx"].size, d["m"]
+    A = np.zeros((d["J"] * m, nnz))
+    for p, j in enumerate(d["item_idx"]):
+        for k in range(m):
+            A[j * m + k, p] = np.float64(d["a"][p * m + k])
+    return A
+
+
+@pytest.mark.parametrize("m", [1, 2])
+def test_jacobi_scaling_is_inverse_row_norm(m):
+    """D_rr = 1/|A_r*|_2 (P:306-308) against numpy's norm of the explicit rows; diag(A'A'^T) = I (P:318);
+    a row of zero norm keeps D_rr = 1."""
+    rng = np.random.default_rng(7 + m)
+    d = random_problem(rng, I=40, J=9, m=m, deg=(1, 5))
+    d["item_idx"] = np.where(d["item_idx"] == 8, 7, d["item_idx"]).astype(np.int32)   # item 8 unused -> zero rows
+    # the substitution may create duplicates inside a row; the scaling formula does not care
+    dd = oracle.jacobi_scaling(_problem(d))
+    A = _explicit_A(d)
+    nrm = np.linalg.norm(A, axis=1)
+    np.testing.assert_allclose(dd[nrm > 0], 1.0 / nrm[nrm > 0], rtol=1e-14)
+    assert np.all(dd[nrm == 0] == 1.0) and (nrm == 0).sum() == m
+    As = dd[:, None] * A
+    np.testing.assert_allclose(np.diag(As @ As.T)[nrm > 0], 1.0, rtol=1e-13)
+
+
+def test_jacobi_preserves_feasible_set():
+    """{x : Ax <= b} = {x : A'x <= b'} on sampled x, including points near the boundary."""
+    rng = np.random.default_rng(11)
+    d = random_problem(rng, I=25, J=6, m=2, deg=(1, 4))
+    dd = oracle.jacobi_scaling(_problem(d))
+    A, b = _explicit_A(d), d["b"].astype(np.float64)
+    for _ in range(200):
+        x = rng.random(A.shape[1]) * rng.choice([0.05, 0.3, 1.0])
+        assert np.array_equal(A @ x <= b, (dd[:, None] * A) @ x <= dd * b)
+
+
+def test_jacobi_first_step_is_per_coordinate_step():
+    """m = 1: A'A'^T = I exactly (Def. 1: each item's row touches its own columns only), so L' = 1, eta' = gamma, and
+    lambda_1 = D max(0, gamma D grad g(0)) = max(0, gamma d^2 grad g(0)) -- from oracle.grad alone."""
+    rng = np.random.default_rng(3)
+    d = random_problem(rng, I=60, J=7, m=1, deg=(2, 5), tight=0.3)
+    p, gamma = _problem(d), 0.05
+    dd = oracle.jacobi_scaling(p)
+    g0 = oracle.grad(p, np.zeros(7), gamma).grad
+    res = oracle.solve(p, [gamma], [1], jacobi=True, trace_lambda=True, trace_grad=True)
+    np.testing.assert_allclose(res.trace_lambda[0], np.maximum(0.0, gamma * dd ** 2 * g0), rtol=1e-12, atol=1e-15)
+    np.testing.assert_allclose(res.trace_grad[0], g0, rtol=1e-12, atol=1e-13)      # reported in original units
+    assert (res.trace_lambda[0] > 0).any()
+
+
+def test_jacobi_equals_plain_solve_of_prescaled_problem():
+    """With power-of-two row norms the scaling is exact in fp32, so solving the scaled data with the plain loop and
+    mapping lambda = D lambda' must reproduce the jacobi solve to rounding (P:310-312, lambda = D lambda')."""
+    rng = np.random.default_rng(5)
+    J = 4
+    col_val = np.array([0.5, 1.0, 2.0, 4.0])                          # 16 users of equal |a|: |col_j| = val_j * 4
+    I = 16
+    rows = np.arange(I + 1, dtype=np.int64) * J
+    idx = np.tile(np.arange(J, dtype=np.int32), I)
+    a = np.tile(col_val, I).astype(np.float32)
+    c = (-rng.random(I * J)).astype(np.float32)
+    b = (np.array([0.5, 1.0, 2.0, 4.0]) * 2.0).astype(np.float32)
+    d = dict(I=I, J=J, m=1, row_ptr=rows, item_idx=idx, c=c, a=a, b=b)
+    p = _problem(d)
+    dd = oracle.jacobi_scaling(p)
+    np.testing.assert_array_equal(dd, 1.0 / (col_val * 4.0))
+    ds = dict(d, a=(a * np.tile(dd, I)).astype(np.float32), b=(b * dd).astype(np.float32))
+    gam, its = [0.5, 0.05], [60, 60]
+    rj = oracle.solve(p, gam, its, jacobi=True, trace_lambda=True)
+    rs = oracle.solve(_problem(ds), gam, its, trace_lambda=True)
+    np.testing.assert_allclose(rj.trace_lambda, rs.trace_lambda * dd, rtol=1e-12, atol=1e-14)
+    np.testing.assert_allclose(rj.trace_g, rs.trace_g, rtol=1e-12)
+    np.testing.assert_allclose(rj.x, rs.x, atol=1e-12)
+    assert (rj.lam > 0).any()
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_jacobi_converges_to_same_kkt_optimum(seed):
+    """Row scaling leaves the primal problem unchanged, so the optimum is the brute-force one; the returned
+    lambda is the dual of the ORIGINAL rows: complementary slackness holds against the unscaled gradient."""
+    rng = np.random.default_rng(100 + seed)
+    d = random_problem(rng, I=int(rng.integers(2, 4)), J=2, m=1, deg=(1, 2), tight=0.7)
+    d["a"] = (d["a"] * np.where(d["item_idx"] == 0, 8.0, 0.25)).astype(np.float32)   # badly scaled rows
+    d["b"] = (np.array([8.0, 0.25]) * (0.15 + 0.5 * rng.random(2))).astype(np.float32)
+    gamma = 0.3
+    p_star, x_star = _kkt_brute_force(d, gamma)
+    res = oracle.solve(_problem(d), [gamma], [4000], jacobi=True)
+    assert abs(res.final.g - p_star) < 1e-8 * (1 + abs(p_star))
+    np.testing.assert_allclose(res.x, x_star, atol=1e-5)
+    assert np.all(res.lam >= 0) and np.max(np.abs(res.lam * res.final.grad)) < 1e-6
+    # and it gets there at least as fast as the scalar step on these badly scaled rows
+    plain = oracle.solve(_problem(d), [gamma], [300])
+    jac = oracle.solve(_problem(d), [gamma], [300], jacobi=True)
+    assert p_star - jac.final.g <= p_star - plain.final.g + 1e-12
+
+
+def test_jacobi_warm_start_and_stages_chain():
+    """lambda in original units in and out: two chained jacobi solves == one two-stage jacobi solve (R4, R18)."""
+    rng = np.random.default_rng(21)
+    d = random_problem(rng, I=50, J=6, m=2, deg=(2, 5), tight=0.3)
+    p = _problem(d)
+    both = oracle.solve(p, [0.5, 0.1], [40, 30], jacobi=True)
+    first = oracle.solve(p, [0.5], [40], jacobi=True)
+    second = oracle.solve(p, [0.1], [30], lam0=first.lam, jacobi=True)
+    np.testing.assert_allclose(second.lam, both.lam, rtol=1e-12, atol=1e-15)
+    assert (both.lam > 0).any()

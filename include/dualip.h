@@ -64,6 +64,17 @@ enum { DUALIP_PROJ_SIMPLEX_INEQ = 0, DUALIP_PROJ_BOX = 1, DUALIP_PROJ_BOXCUT = 2
  *            nnz*4 for x, and three more launches per evaluation.                                       */
 enum { DUALIP_RED_AUTO = 0, DUALIP_RED_SMEM = 1, DUALIP_RED_GLOBAL = 2, DUALIP_RED_CSC = 3 };
 
+/* Preconditioning of the dual ascent ("Jacobi preconditioning ... rescaling the complex constraints using the
+ * diagonal of the Hessian proxy induced by A"; Appendix B.2: D = diag(1/|A_r*|_2), A' = D A, b' = D b,
+ * D_rr = 1 for rows of zero norm).  R18:
+ *   NONE   : eta = gamma / L for every coordinate (R2).
+ *   JACOBI : the iteration of the row-scaled system, carried out in the ORIGINAL variables lambda = D lambda': a
+ *            per-coordinate step  lambda+ = max(0, y + (gamma / L') d_r^2 grad_r),  d_r^2 = 1 / sum_i (a^k_ij)^2,
+ *            L' = max_j #{k : row (j,k) of A is nonzero}  (= 1 for m = 1, where A'A'^T = I exactly).  No row data is
+ *            rescaled, nothing changes per iteration but one multiply per dual; lambda in and out, grad g, the
+ *            residuals and the trace stay in the original units.                                             */
+enum { DUALIP_PRECOND_NONE = 0, DUALIP_PRECOND_JACOBI = 1 };
+
 typedef struct {
     int32_t projection;   /* DUALIP_PROJ_* */
     double  p0, p1;       /* projection parameters, see above */
@@ -75,7 +86,8 @@ typedef struct {
     int32_t grid_ctas;    /* CTAs of the gradient kernel: 0 = auto (SM count x resident CTAs per SM) */
     int32_t use_graph;    /* 1: dualip_solve replays a CUDA graph of 20 chained iteration launches per stage (stages of >= 40
                              iterations; ignored while profiling is on or with DUALIP_RED_CSC); 0: direct launches */
-    int32_t reserved[5];  /* reserved[0] = 1 forces the direct-load kernel (parity tests of both kernels); rest must be zero */
+    int32_t reserved[4];  /* reserved[0] = 1 forces the direct-load kernel (parity tests of both kernels); rest must be zero */
+    int32_t precondition; /* DUALIP_PRECOND_*: how dualip_solve scales its step (dualip_grad is not affected) */
 } dualip_opts;
 
 /* Fills *opts with the defaults: unit simplex (inequality), AUTO reduction, copy, validate, momentum. */
@@ -124,6 +136,9 @@ typedef struct {
     int64_t ntiles;
     double  grad_kernel_ms;  /* profiling on: summed device time of the gradient-kernel launches since it was switched on */
     int64_t grad_kernel_count; /* ... and how many launches that sum covers */
+    int32_t precondition;    /* DUALIP_PRECOND_* in effect */
+    int32_t pad0;
+    double  L_step;          /* the constant the step is derived from (eta = gamma / L_step): L, or L' with JACOBI */
 } dualip_info;
 
 /*
@@ -154,6 +169,7 @@ int dualip_grad(dualip_t* h, const double* lambda, double gamma, double* grad, d
  * a1-a8 -- gamma continuation with projected accelerated ascent (R1-R4).
  *   for each stage s < n_stages:  eta = gammas[s]/L;  y = lambda (warm start, momentum restart)
  *       repeat iters[s] times:  grad at y;  lambda+ = max(0, y + eta*grad);  y = lambda+ + beta_t (lambda+ - lambda)
+ *       (with opts.precondition = DUALIP_PRECOND_JACOBI the step is per coordinate, see DUALIP_PRECOND_*)
  *   then one evaluation at the final lambda with gammas[n_stages-1] fills final_scalars / final_grad / x_out
  *   (skipped when all three are NULL, so the call is exactly sum(iters) gradient evaluations).
  *   gammas, iters: HOST arrays.  lambda_inout[J*m]: warm start in (zeros for a cold start), lambda_T out.

@@ -14,6 +14,7 @@ import numpy as np
 
 PROJ_SIMPLEX_INEQ, PROJ_BOX, PROJ_BOXCUT, PROJ_SIMPLEX_EQ = 0, 1, 2, 3
 RED_AUTO, RED_SMEM, RED_GLOBAL, RED_CSC = 0, 1, 2, 3
+PRECOND_NONE, PRECOND_JACOBI = 0, 1
 
 EXPORTED_SYMBOLS = ("dualip_opts_default", "dualip_create", "dualip_grad", "dualip_solve", "dualip_set_c",
                     "dualip_set_profiling", "dualip_get_info", "dualip_get_csc", "dualip_destroy", "dualip_strerror")
@@ -31,7 +32,7 @@ class Opts(ctypes.Structure):
     _fields_ = [("projection", ctypes.c_int32), ("p0", ctypes.c_double), ("p1", ctypes.c_double),
                 ("reduction", ctypes.c_int32), ("borrow", ctypes.c_int32), ("validate", ctypes.c_int32),
                 ("momentum", ctypes.c_int32), ("group_lanes", ctypes.c_int32), ("grid_ctas", ctypes.c_int32),
-                ("use_graph", ctypes.c_int32), ("reserved", ctypes.c_int32 * 5)]
+                ("use_graph", ctypes.c_int32), ("reserved", ctypes.c_int32 * 4), ("precondition", ctypes.c_int32)]
 
 
 class Scalars(ctypes.Structure):
@@ -54,7 +55,8 @@ class Info(ctypes.Structure):
                 ("grid_ctas", ctypes.c_int32), ("block_threads", ctypes.c_int32), ("smem_bytes", ctypes.c_int64),
                 ("bytes_resident", ctypes.c_int64), ("launches", ctypes.c_int64), ("fix_scale_s", ctypes.c_double),
                 ("streaming", ctypes.c_int32), ("stages", ctypes.c_int32), ("tile_units", ctypes.c_int64), ("ntiles", ctypes.c_int64),
-                ("grad_kernel_ms", ctypes.c_double), ("grad_kernel_count", ctypes.c_int64)]
+                ("grad_kernel_ms", ctypes.c_double), ("grad_kernel_count", ctypes.c_int64),
+                ("precondition", ctypes.c_int32), ("pad0", ctypes.c_int32), ("L_step", ctypes.c_double)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -124,13 +126,14 @@ def _ptr(t, dtype=None, keep=None):
 
 
 def make_opts(projection=PROJ_SIMPLEX_INEQ, p0=1.0, p1=0.0, reduction=RED_AUTO, borrow=False, validate=True,
-              momentum=True, group_lanes=0, grid_ctas=0, use_graph=False, direct_kernel=False) -> Opts:
+              momentum=True, group_lanes=0, grid_ctas=0, use_graph=False, direct_kernel=False, jacobi=False) -> Opts:
     o = Opts()
     load_library().dualip_opts_default(ctypes.byref(o))
     o.projection, o.p0, o.p1, o.reduction = projection, p0, p1, reduction
     o.borrow, o.validate, o.momentum = int(borrow), int(validate), int(momentum)
     o.group_lanes, o.grid_ctas, o.use_graph = group_lanes, grid_ctas, int(use_graph)
     o.reserved[0] = 1 if direct_kernel else 0
+    o.precondition = PRECOND_JACOBI if jacobi else PRECOND_NONE
     return o
 
 

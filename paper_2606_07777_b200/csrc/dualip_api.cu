@@ -72,6 +72,8 @@ struct dualip {
     long long graph_launches = 0;
     // constants from a0
     double L = 0.0, max_colabs = 0.0, sum_abs_c = 0.0;
+    double L_step = 0.0;                   // the constant the step is derived from: L, or L' of the row-scaled system (Jacobi)
+    double* step_scale = nullptr;          // [JM] d_q^2 (Jacobi) or nullptr
     float max_abs_a = 0.0f, max_abs_c = 0.0f;
     long long max_row_len = 0;
     double scale_s = 1.0, scale_obj = 1.0, scale_sq = 1.0;
@@ -193,7 +195,7 @@ bool plan_tma(dualip* h, Plan& pl) {
     long long TN = 0; int stages = 0; size_t stage_bytes = 0;
     for (int S = 3; S >= 2 && TN < 256; --S) {
         stage_bytes = (avail / S) & ~(size_t)127;
-        const long long over = 80 + (h->max_row_len + 8 + 32) * (8 + 4 * m);
+        const long long over = 80 + (h->max_row_len + 8 + 72) * (8 + 4 * m);
         long long tn = ((long long)stage_bytes - over) / (9 + 4 * m);
         tn = tn > 0 ? (tn & ~63ll) : 0;
         if (tn >= (S == 3 ? 512 : 256)) { TN = tn; stages = S; }
@@ -205,7 +207,7 @@ bool plan_tma(dualip* h, Plan& pl) {
     if (TN > want) TN = want > 256 ? (want & ~63ll) : 256;
     pl.tma = true; pl.acc_smem = acc; pl.lam_smem = true;
     pl.TN = TN; pl.stages = stages;
-    pl.cap_nz = (int)((TN + h->max_row_len + 8 + 32 + 3) & ~3ll);   // +32: lanes may read one chunk past a row end
+    pl.cap_nz = (int)((TN + h->max_row_len + 8 + 72 + 3) & ~3ll);   // +72: lanes may read up to 2*32+2 slots past a row end (m = 2)
     pl.cap_rows = (int)((TN / kRowCost + 6 + 1) & ~1ll);
     size_t sb = (size_t)pl.cap_nz * (8 + 4 * m) + (size_t)pl.cap_rows * 8 + 32;
     pl.stage_bytes = (int)((sb + 127) & ~(size_t)127);
@@ -305,8 +307,8 @@ int compute_stats(dualip* h, cudaStream_t st, bool do_a, bool do_c) {
     const long long nnz = h->nnz;
     const int J = h->J, m = h->m, JM = J * m;
     unsigned* d_mx = nullptr;
-    unsigned long long* d_fix = nullptr;  // colsq[J], colabs[JM], cabs[1], out[2]
-    const size_t nfix = (size_t)J + JM + 3;
+    unsigned long long* d_fix = nullptr;  // colsq[JM], colabs[JM], cabs[1], out[3]
+    const size_t nfix = (size_t)2 * JM + 4;
     if (cudaMalloc(&d_mx, 2 * sizeof(unsigned)) != cudaSuccess) { cudaGetLastError(); return DUALIP_ENOMEM; }
     if (cudaMalloc(&d_fix, nfix * sizeof(unsigned long long)) != cudaSuccess) { cudaGetLastError(); cudaFree(d_mx); return DUALIP_ENOMEM; }
     int rc = DUALIP_OK;
@@ -325,18 +327,25 @@ int compute_stats(dualip* h, cudaStream_t st, bool do_a, bool do_c) {
         const double sc_sq = fix_scale((double)maxa * maxa * m * rows * 1.000001);
         const double sc_abs = fix_scale((double)maxa * rows * 1.000001);
         const double sc_c = fix_scale((double)maxc * (double)(nnz > 0 ? nnz : 1) * 1.000001);
-        unsigned long long* colsq = d_fix; unsigned long long* colabs = d_fix + J; unsigned long long* cabs = colabs + JM;
+        unsigned long long* colsq = d_fix; unsigned long long* colabs = d_fix + JM; unsigned long long* cabs = colabs + JM;
         unsigned long long* out = cabs + 1;
         k_col_stats<<<grid_for(nnz, 256, h->num_sms), 256, 0, st>>>(h->idx, h->a, h->c, nnz, m, sc_sq, sc_abs, sc_c,
                                                                     colsq, colabs, cabs, do_a ? 1 : 0, do_c ? 1 : 0);
         h->launches++;
-        k_reduce_stats<<<1, 1024, 0, st>>>(colsq, J, colabs, JM, out); h->launches++;
-        unsigned long long res[3];
+        k_reduce_stats<<<1, 1024, 0, st>>>(colsq, J, m, colabs, JM, out); h->launches++;
+        if (do_a && h->step_scale) {
+            k_jacobi_step_scale<<<grid_for(JM, 256, h->num_sms), 256, 0, st>>>(colsq, 1.0 / sc_sq, JM, h->step_scale); h->launches++;
+        }
+        unsigned long long res[4];
         if (cudaMemcpyAsync(res, cabs, sizeof(res), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
             cudaStreamSynchronize(st) != cudaSuccess) { rc = DUALIP_ECUDA; break; }
         if (cudaGetLastError() != cudaSuccess) { rc = DUALIP_ECUDA; break; }
         if (do_c) h->sum_abs_c = (double)(long long)res[0] / sc_c;
-        if (do_a) { h->L = (double)(long long)res[1] / sc_sq; h->max_colabs = (double)(long long)res[2] / sc_abs; }
+        if (do_a) {
+            h->L = (double)(long long)res[1] / sc_sq; h->max_colabs = (double)(long long)res[2] / sc_abs;
+            // Jacobi: every nonzero row of A' has unit norm, so L' = max_j sum_k |A'_(j,k)*|^2 = max_j #{k : row (j,k) != 0}
+            h->L_step = h->step_scale ? (double)(res[3] > 0 ? res[3] : 1) : h->L;
+        }
     } while (0);
     cudaFree(d_mx); cudaFree(d_fix);
     return rc;
@@ -574,7 +583,7 @@ void dualip_destroy(dualip_t* h) {
     if (h->own_rows) { cudaFree((void*)h->row_ptr); cudaFree((void*)h->idx); cudaFree((void*)h->a); }
     if (h->own_c) cudaFree((void*)h->c);
     cudaFree(h->b); cudaFree(h->s_fix); cudaFree(h->lam_cur); cudaFree(h->y); cudaFree(h->lam_stage);
-    cudaFree(h->grad_stage); cudaFree(h->scalars_dev); cudaFree(h->x_stage); cudaFree(h->tiles);
+    cudaFree(h->grad_stage); cudaFree(h->scalars_dev); cudaFree(h->step_scale); cudaFree(h->x_stage); cudaFree(h->tiles);
     drop_graph(h);
     cudaFree(h->ctl);
     cudaFree(h->csc_perm); cudaFree(h->col_ptr); cudaFree(h->chunk_ptr); cudaFree(h->chunk_item); cudaFree(h->csc_partial);
@@ -601,7 +610,8 @@ int dualip_create(dualip_t** out, int64_t I, int32_t J, int32_t m, const int64_t
     dualip_opts o;
     if (opts_in) o = *opts_in; else dualip_opts_default(&o);
     if (o.reserved[0] != 0 && o.reserved[0] != 1) return DUALIP_EINVAL;   // 1 = force the non-streaming kernel
-    for (int r = 1; r < 5; ++r) if (o.reserved[r] != 0) return DUALIP_EINVAL;
+    for (int r = 1; r < 4; ++r) if (o.reserved[r] != 0) return DUALIP_EINVAL;
+    if (o.precondition != DUALIP_PRECOND_NONE && o.precondition != DUALIP_PRECOND_JACOBI) return DUALIP_EINVAL;
     switch (o.projection) {
         case DUALIP_PROJ_SIMPLEX_INEQ: case DUALIP_PROJ_SIMPLEX_EQ: if (!(o.p0 > 0.0)) return DUALIP_EINVAL; break;
         case DUALIP_PROJ_BOX: if (!(o.p0 <= o.p1)) return DUALIP_EINVAL; break;
@@ -689,6 +699,7 @@ int dualip_create(dualip_t** out, int64_t I, int32_t J, int32_t m, const int64_t
             if (flags & 4) FAIL(DUALIP_EDUP);
             h->max_row_len = (long long)maxlen;
         }
+        if (o.precondition == DUALIP_PRECOND_JACOBI && (rc = dev_alloc(h, &h->step_scale, JM)) != 0) goto fail;
         if ((rc = compute_stats(h, st, true, true)) != 0) goto fail;
         set_xmax(h);
         set_scales(h);
@@ -729,6 +740,7 @@ int dualip_get_info(dualip_t* h, dualip_info* info) {
     info->bytes_resident = h->bytes_resident; info->launches = h->launches;
     info->fix_scale_s = h->scale_s;
     info->grad_kernel_ms = h->prof_ms; info->grad_kernel_count = h->prof_count;
+    info->precondition = h->step_scale ? DUALIP_PRECOND_JACOBI : DUALIP_PRECOND_NONE; info->L_step = h->L_step;
     return DUALIP_OK;
 }
 
@@ -813,7 +825,7 @@ int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int3
     const bool lam_dev = is_device_ptr(lambda_inout), grad_dev = is_device_ptr(final_grad),
                sc_dev = is_device_ptr(final_scalars), x_dev = is_device_ptr(x_out);
     CK(cudaMemcpyAsync(h->lam_cur, lambda_inout, JM * 8, cudaMemcpyDefault, st));
-    const double L = h->L > 0.0 ? h->L : 1.0;
+    const double L = h->L_step > 0.0 ? h->L_step : 1.0;
     CK(cudaMemsetAsync(h->ctl, 0, sizeof(IterState), st));                                 // t = 0, n = 0
     for (int s = 0; s < n_stages; ++s) {
         const double gamma = gammas[s], eta = gamma / L;
@@ -821,7 +833,7 @@ int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int3
         CK(cudaMemsetAsync(h->ctl, 0, sizeof(int), st));                                   // t = 0; n runs on
         FinalizeParams f{};
         f.lam_eval = h->y; f.gamma = gamma; f.update = 1; f.eta = eta; f.momentum = h->opts.momentum ? 1 : 0;
-        f.lam_cur = h->lam_cur; f.y = h->y;
+        f.lam_cur = h->lam_cur; f.y = h->y; f.step_scale = h->step_scale;
         if (trace) { f.tr_g = trace->g; f.tr_rinf = trace->r_inf; f.tr_r2 = trace->r_2; f.tr_grad = trace->grad; f.tr_lam = trace->lambda; }
         IterLaunch it;
         prepare_iter(h, it, h->y, gamma, nullptr, f);

@@ -3,8 +3,9 @@
 //
 //   warp 0      producer: for each of this CTA's tiles, waits for a free stage, then issues one bulk copy per
 //               array (item_idx, c, a, row_ptr segment) that completes on the stage's "full" mbarrier.
-//   warps 1..   consumers: wait for "full", claim row-steps of the tile from a shared counter (G lanes per row,
-//               32/G rows per step), read the rows straight from shared memory, and release the stage.
+//   warps 1..   consumers: wait for "full", take their row-steps of the tile (G lanes per row, 2*32/G rows per step,
+//               steps dealt round-robin over the CTA's step sequence), read the rows straight from shared memory,
+//               and release the stage.
 //
 // Per row the consumers run a two-level scheme:
 //   fast path   fp32 filter: w' = fma(a, RN_f32(lambda_j), c) for every nonzero (one FFMA, one 4-byte gather),
@@ -18,8 +19,8 @@
 //
 // A tile is a run of whole rows cut where (row_ptr[r] + kRowCost*r) crosses a multiple of TN (k_build_tiles at
 // create), so it holds at most TN + max_row_len nonzeros and TN/kRowCost + 1 rows whatever the row lengths
-// (empty rows included).  Tiles are dealt round-robin to CTAs.  Which warp takes which rows is dynamic, but every
-// accumulation (items AND scalars) is 64-bit fixed point, so results do not depend on it.
+// (empty rows included).  Tiles are dealt round-robin to CTAs and row-steps round-robin to warps; every
+// accumulation (items AND scalars) is 64-bit fixed point, so results do not depend on the launch geometry.
 //
 // Nothing here waits on DRAM latency: the only global loads in the loop are the producer's tile-table reads,
 // prefetched a tile ahead.
@@ -255,10 +256,9 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
     constexpr int NT = 32 * (NWC + 1);
     const int mm = M > 0 ? M : p.m;
     const int JM = p.J * mm;
-    // layout: [full[4], empty[4] mbarriers: 64 B][max|lambda| word, claim counters: 64 B][lam_hi JM*4][lam_lo JM*4 (optional)][acc 2*JM*4 (ACC_SMEM)][stages]
+    // layout: [full[4], empty[4] mbarriers: 64 B][max|lambda| word: 64 B][lam_hi JM*4][lam_lo JM*4 (optional)][acc 2*JM*4 (ACC_SMEM)][stages]
     unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_tma);
     unsigned* s_words = reinterpret_cast<unsigned*>(smem_tma + 64);       // [0] = max |lambda_hi| as float bits
-    int* claim = reinterpret_cast<int*>(smem_tma + 64 + 16);              // [stage] = next unclaimed row-step of the tile in it
     float* s_hi32 = reinterpret_cast<float*>(smem_tma + 128);
     float* s_lo32 = s_hi32 + JM;                                           // only when tp.lam_lo_smem
     unsigned* a_lo = reinterpret_cast<unsigned*>(s_hi32 + (tp.lam_lo_smem ? 2 : 1) * JM);
@@ -292,7 +292,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
         fence_proxy_async();                                             // generic-proxy zeros before the first bulk copy
     }
     if (threadIdx.x == 0) {
-        for (int s = 0; s < tp.stages; ++s) { mbar_init(&bars[s], 1); mbar_init(&bars[kTmaStagesMax + s], NWC); claim[s] = 0; }
+        for (int s = 0; s < tp.stages; ++s) { mbar_init(&bars[s], 1); mbar_init(&bars[kTmaStagesMax + s], NWC); }
         fence_mbar_init();
         fence_proxy_async();
     }
@@ -329,7 +329,6 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                 long long r1a = (r1 + 2) & ~1ll;                                       // rows r0a .. r1 inclusive, even count
                 if (r1a > tp.rows2) r1a = tp.rows2 > r0a ? tp.rows2 : r0a;
                 d_meta->nrows = (int)(r1 - r0); d_meta->rpo = (int)(r0 - r0a); d_meta->nzb = p0a;
-                claim[s] = 0;
                 // tails that are not a whole 16-byte chunk (only at the very end of the arrays): plain copies
                 for (long long q = p1a > p0a ? p1a : p0a; q < p1; ++q) {
                     d_idx[q - p0a] = p.idx[q]; d_c[q - p0a] = p.c[q];
@@ -365,17 +364,19 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
         const float gz_sat = gz * (1.0f + 4.8e-7f);                      // w_max above this (plus tol): v_max >= z for sure
         int s = 0;
         unsigned ph = 0;
+        int step_off = 0;                                                // (steps of all earlier tiles) mod NWC
         for (long long t = blockIdx.x; t < tp.ntiles; t += gridDim.x) {
             mbar_wait(&bars[s], ph);
             const StageView v = stage_view(stage0 + s * tp.stage_bytes, tp.cap_nz, tp.cap_rows, mm);
             const int nrows = v.meta->nrows;
             const int nsteps = (nrows + RPW - 1) / RPW;
-            // Row-steps are claimed from a shared counter: whichever warp is free takes the next one.
-            for (;;) {
-                int st = 0;
-                if (lane == 0) st = atomicAdd(&claim[s], 1);
-                st = __shfl_sync(kFull, st, 0);
-                if (st >= nsteps) break;
+            // Row-steps are dealt round-robin over the CTA's whole step sequence (not per tile): step st of this tile is
+            // number step_off + st of the sequence and belongs to warp (step_off + st) mod NWC.  Every warp sees every
+            // tile's nsteps, so each keeps the running offset itself: no shared counter, no atomics.
+            int st0 = (warp - 1) - step_off;
+            if (st0 < 0) st0 += NWC;
+            step_off = (step_off + nsteps) % NWC;
+            for (int st = st0; st < nsteps; st += NWC) {
                 const int rpo = v.meta->rpo;
                 const int nzb32 = (int)v.meta->nzb;                       // low word is enough for local offsets
                 int rbeg[RPG], rlen[RPG];
@@ -399,6 +400,32 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                         // conflict-free 128-byte wavefront per array when G = 8).  Slots outside [beg, beg+len) hold
                         // other rows' data (or zeros): their lambda index is in range, their value is masked to -inf.
                         const int endp = beg + len;
+                        if (M == 2) {
+                            // two coupling families: a lane takes two PAIRS of nonzeros per pass, (q, q+1) and (q+2G, q+2G+1),
+                            // so that the 64-bit idx / c loads and the 128-bit a loads of a group are each one contiguous,
+                            // conflict-free run (four consecutive nonzeros per lane would put the a loads 32 bytes apart:
+                            // a two-way bank conflict on every one of them).
+                            for (int q = (beg & ~3) + 2 * gl; q < endp; q += 4 * G) {
+                                const int q2 = q + 2 * G;
+                                const int2 jA = *reinterpret_cast<const int2*>(v.idx + q), jB = *reinterpret_cast<const int2*>(v.idx + q2);
+                                const float2 cA = *reinterpret_cast<const float2*>(v.c + q), cB = *reinterpret_cast<const float2*>(v.c + q2);
+                                const float4 aA = *reinterpret_cast<const float4*>(v.a + 2 * q), aB = *reinterpret_cast<const float4*>(v.a + 2 * q2);
+                                const int jj[4] = {jA.x, jA.y, jB.x, jB.y};
+                                const float cv[4] = {cA.x, cA.y, cB.x, cB.y};
+                                const float ax[4] = {aA.x, aA.z, aB.x, aB.z}, ay[4] = {aA.y, aA.w, aB.y, aB.w};
+                                const int pe[4] = {q, q + 1, q2, q2 + 1};
+#pragma unroll
+                                for (int e = 0; e < 4; ++e) {
+                                    const float2 l2 = *reinterpret_cast<const float2*>(s_hi32 + 2 * jj[e]);
+                                    const float wv = -fmaf(ay[e], l2.y, fmaf(ax[e], l2.x, cv[e]));
+                                    const bool valid = (unsigned)(pe[e] - beg) < (unsigned)len;
+                                    const float w = valid ? wv : -CUDART_INF_F;
+                                    m2 = fmaxf(m2, fminf(m1, w));
+                                    pb = sel_gt(w, m1, pe[e], pb);
+                                    m1 = fmaxf(m1, w);
+                                }
+                            }
+                        } else {
                         for (int q = (beg & ~3) + 4 * gl; q < endp; q += 4 * G) {
                             const int4 j4 = *reinterpret_cast<const int4*>(v.idx + q);
                             const float4 c4 = *reinterpret_cast<const float4*>(v.c + q);
@@ -410,15 +437,6 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                                 const float aa4[4] = {a4.x, a4.y, a4.z, a4.w};
 #pragma unroll
                                 for (int e = 0; e < 4; ++e) wv[e] = -fmaf(aa4[e], s_hi32[jj[e]], cv[e]);
-                            } else if (M == 2) {
-                                const float4 a01 = *reinterpret_cast<const float4*>(v.a + 2 * q);
-                                const float4 a23 = *reinterpret_cast<const float4*>(v.a + 2 * q + 4);
-                                const float ax[4] = {a01.x, a01.z, a23.x, a23.z}, ay[4] = {a01.y, a01.w, a23.y, a23.w};
-#pragma unroll
-                                for (int e = 0; e < 4; ++e) {
-                                    const float2 l2 = *reinterpret_cast<const float2*>(s_hi32 + 2 * jj[e]);
-                                    wv[e] = -fmaf(ay[e], l2.y, fmaf(ax[e], l2.x, cv[e]));
-                                }
                             } else {
 #pragma unroll
                                 for (int e = 0; e < 4; ++e) {
@@ -436,6 +454,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                                 pb = sel_gt(w, m1, q + e, pb);
                                 m1 = fmaxf(m1, w);
                             }
+                        }
                         }
                     }
                     rm1[r] = m1; rm2[r] = m2; rpos[r] = pb;

@@ -144,6 +144,7 @@ struct FinalizeParams {
     int update;                 // a6 on/off
     int momentum;               // beta_t = t/(t+3) (R1) or 0
     double eta;
+    const double* step_scale;   // nullable: per-coordinate factor on eta (Jacobi preconditioning, R18: d_q^2 = 1/|A_q*|^2)
     double* lam_cur;            // lambda_t -> lambda_{t+1}
     double* y;                  // y_t -> y_{t+1} (== lam_eval when update)
     IterState* state;           // read and advanced when update
@@ -165,14 +166,17 @@ __device__ __forceinline__ void finalize_block(const FinalizeParams& p, double* 
     // L2 round trips, and this CTA runs alone at the end of the launch
     constexpr int U = 4;
     for (int q0 = tid; q0 < p.JM; q0 += U * nthreads) {
-        unsigned long long sf[U]; float bb[U]; double le[U], lo[U];
+        unsigned long long sf[U]; float bb[U]; double le[U], lo[U], et[U];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             const int q = q0 + u * nthreads;
-            sf[u] = 0ull; bb[u] = 0.0f; le[u] = 0.0; lo[u] = 0.0;
+            sf[u] = 0ull; bb[u] = 0.0f; le[u] = 0.0; lo[u] = 0.0; et[u] = p.eta;
             if (q < p.JM) {
                 sf[u] = __ldcg(p.s_fix + q); bb[u] = __ldg(p.b + q); le[u] = __ldcg(p.lam_eval + q);
-                if (p.update) lo[u] = __ldcg(p.lam_cur + q);
+                if (p.update) {
+                    lo[u] = __ldcg(p.lam_cur + q);
+                    if (p.step_scale) et[u] = p.eta * __ldg(p.step_scale + q);
+                }
             }
         }
 #pragma unroll
@@ -187,7 +191,7 @@ __device__ __forceinline__ void finalize_block(const FinalizeParams& p, double* 
             if (p.grad_out) p.grad_out[q] = g;
             if (p.update) {
                 if (p.tr_grad) p.tr_grad[n * p.JM + q] = g;
-                const double ln = fmax(0.0, le[u] + p.eta * g);
+                const double ln = fmax(0.0, le[u] + et[u] * g);
                 p.lam_cur[q] = ln;
                 p.y[q] = ln + beta * (ln - lo[u]);
                 if (p.tr_lam) p.tr_lam[n * p.JM + q] = ln;
@@ -635,7 +639,7 @@ __global__ void k_absmax(const float* __restrict__ a, long long na, const float*
     if ((threadIdx.x & 31) == 0) { atomicMax(out + 0, ma); atomicMax(out + 1, mc); }
 }
 
-// fixed-point column sums: colsq[j] += sum_k a^2 (for L, R2), colabs[j*m+k] += |a|, cabs += |c|
+// fixed-point column sums: colsq[j*m+k] += a^2 (for L, R2, and the Jacobi scaling, R18), colabs[j*m+k] += |a|, cabs += |c|
 __global__ void k_col_stats(const int* __restrict__ idx, const float* __restrict__ a, const float* __restrict__ c,
                             long long nnz, int m, double scale_sq, double scale_abs, double scale_c,
                             unsigned long long* colsq, unsigned long long* colabs, unsigned long long* cabs,
@@ -644,15 +648,13 @@ __global__ void k_col_stats(const int* __restrict__ idx, const float* __restrict
     for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < nnz; q += (long long)gridDim.x * blockDim.x) {
         if (do_a) {
             const int j = idx[q];
-            double sq = 0.0;
             for (int k = 0; k < m; ++k) {
                 const double v = (double)a[q * m + k];
-                sq = fma(v, v, sq);
                 const long long fa = __double2ll_rn(fabs(v) * scale_abs);
                 if (fa) atomicAdd(colabs + (long long)j * m + k, (unsigned long long)fa);
+                const long long fq = __double2ll_rn(v * v * scale_sq);
+                if (fq) atomicAdd(colsq + (long long)j * m + k, (unsigned long long)fq);
             }
-            const long long fq = __double2ll_rn(sq * scale_sq);
-            if (fq) atomicAdd(colsq + j, (unsigned long long)fq);
         }
         if (do_c) lc += __double2ll_rn(fabs((double)c[q]) * scale_c);
     }
@@ -663,21 +665,37 @@ __global__ void k_col_stats(const int* __restrict__ idx, const float* __restrict
     }
 }
 
-// out[0] = max_j colsq (fixed), out[1] = max_q colabs (fixed)
-__global__ void __launch_bounds__(1024) k_reduce_stats(const unsigned long long* colsq, int J, const unsigned long long* colabs,
+// out[0] = max_j sum_k colsq[j*m+k] (fixed), out[1] = max_q colabs (fixed), out[2] = max_j #{k : colsq[j*m+k] > 0}
+__global__ void __launch_bounds__(1024) k_reduce_stats(const unsigned long long* colsq, int J, int m, const unsigned long long* colabs,
                                                        int JM, unsigned long long* out) {
-    __shared__ unsigned long long sh[2][32];
-    unsigned long long a = 0, b = 0;
-    for (int q = threadIdx.x; q < J; q += 1024) a = max(a, colsq[q]);
+    __shared__ unsigned long long sh[3][32];
+    unsigned long long a = 0, b = 0, c = 0;
+    for (int j = threadIdx.x; j < J; j += 1024) {
+        unsigned long long sj = 0, nj = 0;
+        for (int k = 0; k < m; ++k) { const unsigned long long v = colsq[(long long)j * m + k]; sj += v; nj += v ? 1ull : 0ull; }
+        a = max(a, sj); c = max(c, nj);
+    }
     for (int q = threadIdx.x; q < JM; q += 1024) b = max(b, colabs[q]);
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) { a = max(a, __shfl_xor_sync(kFull, a, o)); b = max(b, __shfl_xor_sync(kFull, b, o)); }
-    if ((threadIdx.x & 31) == 0) { sh[0][threadIdx.x >> 5] = a; sh[1][threadIdx.x >> 5] = b; }
+    for (int o = 16; o > 0; o >>= 1) {
+        a = max(a, __shfl_xor_sync(kFull, a, o)); b = max(b, __shfl_xor_sync(kFull, b, o)); c = max(c, __shfl_xor_sync(kFull, c, o));
+    }
+    if ((threadIdx.x & 31) == 0) { sh[0][threadIdx.x >> 5] = a; sh[1][threadIdx.x >> 5] = b; sh[2][threadIdx.x >> 5] = c; }
     __syncthreads();
     if (threadIdx.x == 0) {
-        a = 0; b = 0;
-        for (int w = 0; w < 32; ++w) { a = max(a, sh[0][w]); b = max(b, sh[1][w]); }
-        out[0] = a; out[1] = b;
+        a = 0; b = 0; c = 0;
+        for (int w = 0; w < 32; ++w) { a = max(a, sh[0][w]); b = max(b, sh[1][w]); c = max(c, sh[2][w]); }
+        out[0] = a; out[1] = b; out[2] = c;
+    }
+}
+
+// Jacobi preconditioning (R18).  Row scaling A' = D A, b' = D b with D_qq = 1/|A_q*|_2 is, in the
+// original variables lambda = D lambda', a per-coordinate step: lambda+ = max(0, y + eta' d_q^2 grad_q).  Only
+// d_q^2 = 1/sum_i (a^k_ij)^2 is needed (1 for rows of zero norm), and no row data is rescaled.
+__global__ void k_jacobi_step_scale(const unsigned long long* colsq, double inv_scale_sq, int JM, double* step_scale) {
+    for (int q = blockIdx.x * blockDim.x + threadIdx.x; q < JM; q += gridDim.x * blockDim.x) {
+        const double n2 = (double)(long long)colsq[q] * inv_scale_sq;
+        step_scale[q] = n2 > 0.0 ? 1.0 / n2 : 1.0;
     }
 }
 

@@ -83,9 +83,10 @@ def gpu_solve(pg, gammas, iters, lam0=None, want_trace=True, want_x=True):
     return out
 
 
-def assert_trajectory_parity(po, pg, gammas, iters, lam0=None, momentum=True, tag=""):
-    """Independent solves compared per iteration (parity mode B of SURVEY 8(c))."""
-    ref = oracle.solve(po, gammas, iters, lam0=lam0, momentum=momentum, trace_grad=True, trace_lambda=True)
+def assert_trajectory_parity(po, pg, gammas, iters, lam0=None, momentum=True, tag="", jacobi=False):
+    """Independent solves compared per iteration (parity mode B of SURVEY 8(c)).  jacobi: the oracle iterates on the
+    literally row-scaled system; pg must have been created with jacobi=True (per-coordinate step)."""
+    ref = oracle.solve(po, gammas, iters, lam0=lam0, momentum=momentum, trace_grad=True, trace_lambda=True, jacobi=jacobi)
     out = gpu_solve(pg, gammas, iters, lam0=lam0)
     T = int(np.sum(iters))
     worst = 0.0
@@ -100,4 +101,6 @@ def assert_trajectory_parity(po, pg, gammas, iters, lam0=None, momentum=True, ta
     assert rel_l2(out["grad"], ref.final.grad) <= TOL_GRAD, f"{tag} final grad"
     lam_scale = max(np.abs(ref.lam).max(), 1e-300)
     assert np.abs(out["lam"] - ref.lam).max() <= 1e-6 * lam_scale + 1e-12, f"{tag} lambda_T"
+    el = np.abs(out["tr_lam"] - ref.trace_lambda).max()
+    assert el <= 1e-6 * max(np.abs(ref.trace_lambda).max(), 1e-300) + 1e-12, f"{tag} lambda trace {el:.3e}"
     return worst, ex, ref, out

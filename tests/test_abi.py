@@ -38,9 +38,29 @@ def test_struct_mirrors_match_the_header():
     assert ctypes.sizeof(pkg.Scalars) == 5 * 8
     o = pkg.binding.make_opts()
     assert (o.projection, o.p0, o.reduction, o.borrow, o.validate, o.momentum) == (0, 1.0, 0, 0, 1, 1)
-    # C layout: int32, pad, 2 doubles, 7 int32 + 5 reserved int32 = 4+4+16+48 = 72 bytes
-    assert ctypes.sizeof(pkg.Opts) == 72
-    assert ctypes.sizeof(pkg.Info) == 8 * 2 + 4 * 2 + 8 + 8 + 4 * 6 + 8 * 3 + 8 + 16 + 24
+    # sizes and field offsets as gcc lays out include/dualip.h, against the ctypes mirrors
+    import subprocess, tempfile
+    fields = {"dualip_opts": ["projection", "p0", "reduction", "use_graph", "reserved", "precondition"],
+              "dualip_info": ["I", "L", "group_lanes", "smem_bytes", "fix_scale_s", "streaming", "ntiles", "grad_kernel_count",
+                              "precondition", "L_step"],
+              "dualip_scalars": ["g", "r_2"], "dualip_trace": ["capacity", "lambda"]}
+    src = '#include <stdio.h>\n#include <stddef.h>\n#include "dualip.h"\nint main(void){\n'
+    for st, fl in fields.items():
+        src += f'printf("{st} %zu\\n", sizeof({st}));\n'
+        for f in fl:
+            src += f'printf("{st}.{f} %zu\\n", offsetof({st}, {f}));\n'
+    src += "return 0;}\n"
+    with tempfile.TemporaryDirectory() as td:
+        cpath, exe = os.path.join(td, "abi.c"), os.path.join(td, "abi")
+        open(cpath, "w").write(src)
+        subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), "-o", exe, cpath])
+        got = dict(line.split() for line in subprocess.check_output([exe]).decode().splitlines())
+    mirrors = {"dualip_opts": pkg.Opts, "dualip_info": pkg.Info, "dualip_scalars": pkg.Scalars, "dualip_trace": pkg.binding._Trace}
+    rename = {"lambda": "lam"}
+    for st, fl in fields.items():
+        assert int(got[st]) == ctypes.sizeof(mirrors[st]), st
+        for f in fl:
+            assert int(got[f"{st}.{f}"]) == getattr(mirrors[st], rename.get(f, f)).offset, f"{st}.{f}"
     lib = pkg.load_library()
     assert lib.dualip_strerror(0) == b"ok" and lib.dualip_strerror(-3).startswith(b"duplicate")
 

@@ -272,3 +272,62 @@ def test_csc_matches_atomic_modes_at_scale():
     sc3, g3, x3 = gpu_grad(pg2, lam, 1e-3)
     assert np.array_equal(x1, x3) and rel_l2(g1, g3) < 1e-9
     pg.destroy(); pg2.destroy()
+
+
+# ---- Jacobi preconditioning (R18): the CUDA path never rescales the rows -- it takes the
+# per-coordinate step eta' d_r^2 in the original variables -- while the oracle iterates on A' = D A, b' = D b literally.
+
+@pytest.mark.parametrize("name,I,iters", [("cfg1-tight", None, 200), ("cfg2-tight", 60_000, 40), ("cfg3-tight", 30_000, 30),
+                                          ("cfg4-tight", 8_000, 30), ("cfg5-tight", 40_000, None), ("cfg3", 30_000, 10)])
+def test_jacobi_trajectories(name, I, iters):
+    cfg = synth.get_config(name, I=I) if I else synth.get_config(name)
+    inst = synth.generate(cfg)
+    po, pg = from_instance(inst, jacobi=True)
+    info = pg.info()
+    assert info.precondition == pkg.PRECOND_JACOBI and info.L_step == float(inst.m)
+    its = [iters] * len(cfg.gammas) if iters else [15] * len(cfg.gammas)
+    worst, ex, ref, out = assert_trajectory_parity(po, pg, cfg.gammas, its, tag=name + "/jacobi", jacobi=True)
+    if name.endswith("tight"):
+        assert (ref.lam > 0).sum() >= 5                     # the preconditioned update really moves lambda
+    pg.destroy()
+
+
+def test_jacobi_moves_where_the_scalar_step_stalls():
+    """on the Zipf configs L is set by the hottest column, so the scalar step gamma/L barely moves
+    lambda; the Jacobi step makes real progress on the same instance in the same number of iterations."""
+    cfg = synth.get_config("cfg3-tight", I=30_000)
+    inst = synth.generate(cfg)
+    po, plain = from_instance(inst)
+    _, jac = from_instance(inst, jacobi=True)
+    its = [60]
+    a = gpu_solve(plain, cfg.gammas[:1], its, want_trace=False, want_x=False)
+    b = gpu_solve(jac, cfg.gammas[:1], its, want_trace=False, want_x=False)
+    g0 = gpu_grad(plain, np.zeros(inst.J * inst.m), cfg.gammas[0], want_x=False)[0].g
+    assert a["sc"].g >= g0 - 1e-9 * abs(g0)                 # both ascend from g(0) ...
+    assert b["sc"].g - g0 > 10.0 * (a["sc"].g - g0) > 0.0   # ... the Jacobi step at least ten times further
+    plain.destroy(); jac.destroy()
+
+
+def test_jacobi_zero_rows_and_families():
+    """Items nobody is eligible for (zero rows of A, D_rr = 1) and m = 2 (L' = 2), warm start in original units."""
+    rng = np.random.default_rng(77)
+    d = _ragged(rng, 1500, 90, 2, [6, 20, 33, 0, 12])
+    d["item_idx"] = np.where(d["item_idx"] >= 80, d["item_idx"] - 40, d["item_idx"]).astype(np.int32)   # items 80.. unused
+    # the remap may create duplicates inside a row: rebuild rows without them
+    keep = np.ones(d["item_idx"].size, dtype=bool)
+    for i in range(d["I"]):
+        b, e = d["row_ptr"][i], d["row_ptr"][i + 1]
+        _, first = np.unique(d["item_idx"][b:e], return_index=True)
+        mask = np.zeros(e - b, dtype=bool); mask[first] = True
+        keep[b:e] = mask
+    lens = np.add.reduceat(keep, d["row_ptr"][:-1]) if d["I"] else np.array([], dtype=np.int64)
+    lens[np.diff(d["row_ptr"]) == 0] = 0
+    d["row_ptr"] = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    d["item_idx"], d["c"] = d["item_idx"][keep], d["c"][keep]
+    d["a"] = d["a"].reshape(-1, 2)[keep].reshape(-1)
+    d["b"] = (d["b"] * 0.5).astype(np.float32)
+    po, pg = both(d, jacobi=True)
+    assert pg.info().L_step == 2.0
+    lam0 = rng.random(180) * 0.05
+    assert_trajectory_parity(po, pg, [0.1, 0.01], [25, 25], lam0=lam0, tag="jacobi/zero-rows", jacobi=True)
+    pg.destroy()

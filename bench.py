@@ -45,6 +45,8 @@ def parse_args():
     ap.add_argument("--workload", default="cfg3")
     ap.add_argument("--users", type=int, default=None, help="override the number of users (smaller = not the graded workload)")
     ap.add_argument("--group-lanes", type=int, default=0, help="lanes per row in the gradient kernel (0 = the library's choice)")
+    ap.add_argument("--stages", type=int, default=0, help="pipeline stages of the streaming kernel (0 = the library's choice)")
+    ap.add_argument("--tile-units", type=int, default=0, help="cap on the streaming kernel's tile size (0 = the library's choice)")
     ap.add_argument("--grid-ctas", type=int, default=0, help="CTAs of the gradient kernel (0 = the library's choice)")
     ap.add_argument("--graph", action="store_true", help="dualip_solve replays a CUDA graph of chained iteration launches "
                     "(small, launch-bound workloads); the per-launch kernel timing hook is then off")
@@ -201,7 +203,7 @@ def main():
     kind, p0, p1 = synth.proj_spec(cfg)
     proj = {"simplex": pkg.PROJ_SIMPLEX_INEQ, "box": pkg.PROJ_BOX, "boxcut": pkg.PROJ_BOXCUT}[kind]
     gamma = cfg.gammas[-1]
-    opts = pkg.binding.make_opts(projection=proj, p0=p0, p1=p1, borrow=True, group_lanes=args.group_lanes, grid_ctas=args.grid_ctas,
+    opts = pkg.binding.make_opts(projection=proj, p0=p0, p1=p1, borrow=True, group_lanes=args.group_lanes, grid_ctas=args.grid_ctas, stages=args.stages, tile_units=args.tile_units,
                                   use_graph=args.graph)
     t0 = time.time()
     prob = pkg.Problem.create(inst.I, inst.J, inst.m, inst.row_ptr, inst.item_idx, inst.c, inst.a, inst.b, opts)
@@ -253,7 +255,7 @@ def main():
         barrier()
         t0 = time.perf_counter()
         p2 = pkg.Problem.create(inst.I, inst.J, inst.m, host["row_ptr"], host["item_idx"], host["c"], host["a"], host["b"],
-                                pkg.binding.make_opts(projection=proj, p0=p0, p1=p1, group_lanes=args.group_lanes, grid_ctas=args.grid_ctas,
+                                pkg.binding.make_opts(projection=proj, p0=p0, p1=p1, group_lanes=args.group_lanes, grid_ctas=args.grid_ctas, stages=args.stages, tile_units=args.tile_units,
                                                       use_graph=args.graph))
         p2.solve([gamma], [args.steps], lam_h, scalars=sc)
         torch.cuda.synchronize()
@@ -295,7 +297,7 @@ def main():
                        "parallelism": "replicas only" if world > 1 else "single GPU", "l2_policy": (f"inputs larger than L2 ({alg_bytes / 1e9:.2f} GB streamed per step vs 126 MB L2); no flush needed"
                                      if alg_bytes > 4 * 126e6 else
                                      f"inputs NOT much larger than L2 ({alg_bytes / 1e6:.0f} MB per step vs 126 MB L2): partly L2-resident, not a bandwidth case"),
-                       "group_lanes": info.group_lanes, "chunk_regs": info.chunk_regs, "grid_ctas": info.grid_ctas,
+                       "group_lanes": info.group_lanes, "stages": info.stages, "tile_units": info.tile_units, "chunk_regs": info.chunk_regs, "grid_ctas": info.grid_ctas,
                        "block_threads": info.block_threads, "smem_bytes": info.smem_bytes,
                        "reduction": {1: "smem fixed-point", 2: "global RED.ADD.64", 3: "csc"}[info.reduction],
                        "short_rows": inst.short_rows, "cuda_graph": bool(args.graph)},

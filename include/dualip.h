@@ -86,7 +86,9 @@ typedef struct {
     int32_t grid_ctas;    /* CTAs of the gradient kernel: 0 = auto (SM count x resident CTAs per SM) */
     int32_t use_graph;    /* 1: dualip_solve replays a CUDA graph of 20 chained iteration launches per stage (stages of >= 40
                              iterations; ignored while profiling is on or with DUALIP_RED_CSC); 0: direct launches */
-    int32_t reserved[4];  /* reserved[0] = 1 forces the direct-load kernel (parity tests of both kernels); rest must be zero */
+    int32_t reserved[4];  /* tuning / test overrides, 0 = the library's choice: [0] = 1 forces the direct-load kernel (parity tests
+                             of both kernels); [1] = pipeline stages of the streaming kernel (2..4); [2] = cap on its tile size
+                             in units (>= 256); [3] must be zero */
     int32_t precondition; /* DUALIP_PRECOND_*: how dualip_solve scales its step (dualip_grad is not affected) */
 } dualip_opts;
 

@@ -126,13 +126,14 @@ def _ptr(t, dtype=None, keep=None):
 
 
 def make_opts(projection=PROJ_SIMPLEX_INEQ, p0=1.0, p1=0.0, reduction=RED_AUTO, borrow=False, validate=True,
-              momentum=True, group_lanes=0, grid_ctas=0, use_graph=False, direct_kernel=False, jacobi=False) -> Opts:
+              momentum=True, group_lanes=0, grid_ctas=0, use_graph=False, direct_kernel=False, jacobi=False, stages=0, tile_units=0) -> Opts:
     o = Opts()
     load_library().dualip_opts_default(ctypes.byref(o))
     o.projection, o.p0, o.p1, o.reduction = projection, p0, p1, reduction
     o.borrow, o.validate, o.momentum = int(borrow), int(validate), int(momentum)
     o.group_lanes, o.grid_ctas, o.use_graph = group_lanes, grid_ctas, int(use_graph)
     o.reserved[0] = 1 if direct_kernel else 0
+    o.reserved[1], o.reserved[2] = stages, tile_units
     o.precondition = PRECOND_JACOBI if jacobi else PRECOND_NONE
     return o
 

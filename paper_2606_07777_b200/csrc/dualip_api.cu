@@ -193,18 +193,20 @@ bool plan_tma(dualip* h, Plan& pl) {
     const int m = h->m;
     const long long units = h->nnz + (long long)kRowCost * h->I;
     long long TN = 0; int stages = 0; size_t stage_bytes = 0;
-    for (int S = 3; S >= 2 && TN < 256; --S) {
+    const int s_hi = h->opts.reserved[1] ? h->opts.reserved[1] : 3, s_lo = h->opts.reserved[1] ? h->opts.reserved[1] : 2;
+    for (int S = s_hi; S >= s_lo && TN < 256; --S) {
         stage_bytes = (avail / S) & ~(size_t)127;
         const long long over = 80 + (h->max_row_len + 8 + 72) * (8 + 4 * m);
         long long tn = ((long long)stage_bytes - over) / (9 + 4 * m);
         tn = tn > 0 ? (tn & ~63ll) : 0;
-        if (tn >= (S == 3 ? 512 : 256)) { TN = tn; stages = S; }
+        if (tn >= (S >= 3 ? 512 : 256)) { TN = tn; stages = S; }
     }
     if (TN < 256) return false;
     // small problems: keep at least ~8 tiles per CTA so the static deal stays balanced
     const long long want = units / ((long long)h->num_sms * 8);
     if (TN > 8192) TN = 8192;
     if (TN > want) TN = want > 256 ? (want & ~63ll) : 256;
+    if (h->opts.reserved[2] >= 256 && h->opts.reserved[2] < TN) TN = h->opts.reserved[2] & ~63ll;
     pl.tma = true; pl.acc_smem = acc; pl.lam_smem = true;
     pl.TN = TN; pl.stages = stages;
     pl.cap_nz = (int)((TN + h->max_row_len + 8 + 72 + 3) & ~3ll);   // +72: lanes may read up to 2*32+2 slots past a row end (m = 2)
@@ -610,7 +612,8 @@ int dualip_create(dualip_t** out, int64_t I, int32_t J, int32_t m, const int64_t
     dualip_opts o;
     if (opts_in) o = *opts_in; else dualip_opts_default(&o);
     if (o.reserved[0] != 0 && o.reserved[0] != 1) return DUALIP_EINVAL;   // 1 = force the non-streaming kernel
-    for (int r = 1; r < 4; ++r) if (o.reserved[r] != 0) return DUALIP_EINVAL;
+    if (o.reserved[1] != 0 && (o.reserved[1] < 2 || o.reserved[1] > kTmaStagesMax)) return DUALIP_EINVAL;   // pipeline stages
+    if (o.reserved[2] < 0 || o.reserved[3] != 0) return DUALIP_EINVAL;                                        // tile units cap
     if (o.precondition != DUALIP_PRECOND_NONE && o.precondition != DUALIP_PRECOND_JACOBI) return DUALIP_EINVAL;
     switch (o.projection) {
         case DUALIP_PROJ_SIMPLEX_INEQ: case DUALIP_PROJ_SIMPLEX_EQ: if (!(o.p0 > 0.0)) return DUALIP_EINVAL; break;

@@ -153,6 +153,63 @@ __device__ __forceinline__ double exact_t(const StageView& v, const ConsumerCtx&
     return t;
 }
 
+// One pass of the fp32 filter for one row: this lane's 4 nonzeros at q (M != 2: q..q+3; M = 2: the pairs (q, q+1) and
+// (q+2G, q+2G+1), so that the 64-bit idx / c loads and the 128-bit a loads of a group are each one contiguous,
+// conflict-free run -- four consecutive nonzeros per lane would put the a loads 32 bytes apart, a two-way bank conflict).
+// Updates the running two largest w' (m1 >= m2) and the position of the largest.  The four values are first reduced
+// among themselves (depth 2), then merged into the running pair, so the dependent chain per pass is ~4 min/max deep
+// instead of 8.  Equal maxima give m2 = m1 (no vertex).
+template <int G, int M>
+__device__ __forceinline__ void filter_pass(const StageView& v, const float* __restrict__ s_hi32, int mm, int q, int beg, int len,
+                                            float& m1, float& m2, int& pb) {
+    float w[4]; int pe[4];
+    if (M == 2) {
+        const int q2 = q + 2 * G;
+        const int2 jA = *reinterpret_cast<const int2*>(v.idx + q), jB = *reinterpret_cast<const int2*>(v.idx + q2);
+        const float2 cA = *reinterpret_cast<const float2*>(v.c + q), cB = *reinterpret_cast<const float2*>(v.c + q2);
+        const float4 aA = *reinterpret_cast<const float4*>(v.a + 2 * q), aB = *reinterpret_cast<const float4*>(v.a + 2 * q2);
+        const int jj[4] = {jA.x, jA.y, jB.x, jB.y};
+        const float cv[4] = {cA.x, cA.y, cB.x, cB.y};
+        const float ax[4] = {aA.x, aA.z, aB.x, aB.z}, ay[4] = {aA.y, aA.w, aB.y, aB.w};
+        pe[0] = q; pe[1] = q + 1; pe[2] = q2; pe[3] = q2 + 1;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const float2 l2 = *reinterpret_cast<const float2*>(s_hi32 + 2 * jj[e]);
+            w[e] = -fmaf(ay[e], l2.y, fmaf(ax[e], l2.x, cv[e]));
+        }
+    } else {
+        const int4 j4 = *reinterpret_cast<const int4*>(v.idx + q);
+        const float4 c4 = *reinterpret_cast<const float4*>(v.c + q);
+        const int jj[4] = {j4.x, j4.y, j4.z, j4.w};
+        const float cv[4] = {c4.x, c4.y, c4.z, c4.w};
+        if (M == 1) {
+            const float4 a4 = *reinterpret_cast<const float4*>(v.a + q);
+            const float aa4[4] = {a4.x, a4.y, a4.z, a4.w};
+#pragma unroll
+            for (int e = 0; e < 4; ++e) w[e] = -fmaf(aa4[e], s_hi32[jj[e]], cv[e]);
+        } else {
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                float t = cv[e];
+                for (int f = 0; f < mm; ++f) t = fmaf(v.a[(q + e) * mm + f], s_hi32[jj[e] * mm + f], t);
+                w[e] = -t;
+            }
+        }
+#pragma unroll
+        for (int e = 0; e < 4; ++e) pe[e] = q + e;
+    }
+#pragma unroll
+    for (int e = 0; e < 4; ++e) w[e] = (unsigned)(pe[e] - beg) < (unsigned)len ? w[e] : -CUDART_INF_F;
+    const float hi01 = fmaxf(w[0], w[1]), lo01 = fminf(w[0], w[1]), hi23 = fmaxf(w[2], w[3]), lo23 = fminf(w[2], w[3]);
+    const int p01 = sel_gt(w[1], w[0], pe[1], pe[0]), p23 = sel_gt(w[3], w[2], pe[3], pe[2]);
+    const float top = fmaxf(hi01, hi23);
+    const float sec = fmaxf(fminf(hi01, hi23), fmaxf(lo01, lo23));
+    const int p4 = sel_gt(hi23, hi01, p23, p01);
+    m2 = fmaxf(fmaxf(m2, sec), fminf(m1, top));
+    pb = sel_gt(top, m1, p4, pb);
+    m1 = fmaxf(m1, top);
+}
+
 // Slow path: one row, whole warp, any length; every pass re-reads the staged row.  Same arithmetic as long_row()
 // in dualip_kernels.cuh (which documents the three box-cut steps).
 template <int M, bool ACC_SMEM, bool GBOX>
@@ -391,73 +448,22 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                         beg = b - nzb32; len = e - b;
                     }
                     rbeg[r] = beg; rlen[r] = len;
-                    float m1 = -CUDART_INF_F, m2 = -CUDART_INF_F;
-                    int pb = 0;
-                    if (!GBOX) {
-                        // ---- fp32 filter: the two largest w' = -(c + a.lambda_hi) of the row and where the largest sits.
-                        // Each lane takes 4 consecutive nonzeros per pass with 128-bit loads from the 16-byte aligned
-                        // position at or below the row start; the G lanes of a group cover 4G consecutive nonzeros (one
-                        // conflict-free 128-byte wavefront per array when G = 8).  Slots outside [beg, beg+len) hold
-                        // other rows' data (or zeros): their lambda index is in range, their value is masked to -inf.
-                        const int endp = beg + len;
-                        if (M == 2) {
-                            // two coupling families: a lane takes two PAIRS of nonzeros per pass, (q, q+1) and (q+2G, q+2G+1),
-                            // so that the 64-bit idx / c loads and the 128-bit a loads of a group are each one contiguous,
-                            // conflict-free run (four consecutive nonzeros per lane would put the a loads 32 bytes apart:
-                            // a two-way bank conflict on every one of them).
-                            for (int q = (beg & ~3) + 2 * gl; q < endp; q += 4 * G) {
-                                const int q2 = q + 2 * G;
-                                const int2 jA = *reinterpret_cast<const int2*>(v.idx + q), jB = *reinterpret_cast<const int2*>(v.idx + q2);
-                                const float2 cA = *reinterpret_cast<const float2*>(v.c + q), cB = *reinterpret_cast<const float2*>(v.c + q2);
-                                const float4 aA = *reinterpret_cast<const float4*>(v.a + 2 * q), aB = *reinterpret_cast<const float4*>(v.a + 2 * q2);
-                                const int jj[4] = {jA.x, jA.y, jB.x, jB.y};
-                                const float cv[4] = {cA.x, cA.y, cB.x, cB.y};
-                                const float ax[4] = {aA.x, aA.z, aB.x, aB.z}, ay[4] = {aA.y, aA.w, aB.y, aB.w};
-                                const int pe[4] = {q, q + 1, q2, q2 + 1};
+                    rm1[r] = -CUDART_INF_F; rm2[r] = -CUDART_INF_F; rpos[r] = 0;
+                }
+                if (!GBOX) {
+                    // ---- fp32 filter: the two largest w' = -(c + a.lambda_hi) of each row and where the largest sits.
+                    // A lane takes 4 nonzeros of a row per pass (filter_pass) starting from the 16-byte aligned position at
+                    // or below the row start; the G lanes of a group cover 4G consecutive nonzeros.  Slots outside
+                    // [beg, beg+len) hold other rows' data (or zeros): their lambda index is in range, their value is
+                    // masked to -inf.
+                    constexpr int LS = M == 2 ? 2 : 4;                        // first-slot spacing of the lanes
+                    int q[RPG], qe[RPG];
 #pragma unroll
-                                for (int e = 0; e < 4; ++e) {
-                                    const float2 l2 = *reinterpret_cast<const float2*>(s_hi32 + 2 * jj[e]);
-                                    const float wv = -fmaf(ay[e], l2.y, fmaf(ax[e], l2.x, cv[e]));
-                                    const bool valid = (unsigned)(pe[e] - beg) < (unsigned)len;
-                                    const float w = valid ? wv : -CUDART_INF_F;
-                                    m2 = fmaxf(m2, fminf(m1, w));
-                                    pb = sel_gt(w, m1, pe[e], pb);
-                                    m1 = fmaxf(m1, w);
-                                }
-                            }
-                        } else {
-                        for (int q = (beg & ~3) + 4 * gl; q < endp; q += 4 * G) {
-                            const int4 j4 = *reinterpret_cast<const int4*>(v.idx + q);
-                            const float4 c4 = *reinterpret_cast<const float4*>(v.c + q);
-                            const int jj[4] = {j4.x, j4.y, j4.z, j4.w};
-                            const float cv[4] = {c4.x, c4.y, c4.z, c4.w};
-                            float wv[4];
-                            if (M == 1) {
-                                const float4 a4 = *reinterpret_cast<const float4*>(v.a + q);
-                                const float aa4[4] = {a4.x, a4.y, a4.z, a4.w};
+                    for (int r = 0; r < RPG; ++r) { q[r] = (rbeg[r] & ~3) + LS * gl; qe[r] = rbeg[r] + rlen[r]; }
 #pragma unroll
-                                for (int e = 0; e < 4; ++e) wv[e] = -fmaf(aa4[e], s_hi32[jj[e]], cv[e]);
-                            } else {
-#pragma unroll
-                                for (int e = 0; e < 4; ++e) {
-                                    float w = cv[e];
-                                    for (int f = 0; f < mm; ++f) w = fmaf(v.a[(q + e) * mm + f], s_hi32[jj[e] * mm + f], w);
-                                    wv[e] = -w;
-                                }
-                            }
-#pragma unroll
-                            for (int e = 0; e < 4; ++e) {
-                                const bool valid = (unsigned)(q + e - beg) < (unsigned)len;
-                                const float w = valid ? wv[e] : -CUDART_INF_F;
-                                // top two and the arg-max, branch-free (ptxas turned the ternary form into branches)
-                                m2 = fmaxf(m2, fminf(m1, w));
-                                pb = sel_gt(w, m1, q + e, pb);
-                                m1 = fmaxf(m1, w);
-                            }
-                        }
-                        }
-                    }
-                    rm1[r] = m1; rm2[r] = m2; rpos[r] = pb;
+                    for (int r = 0; r < RPG; ++r)
+                        for (; q[r] < qe[r]; q[r] += 4 * G)
+                            filter_pass<G, M>(v, s_hi32, mm, q[r], rbeg[r], rlen[r], rm1[r], rm2[r], rpos[r]);
                 }
                 unsigned slow_mask;
                 int fbeg = rbeg[0], flen = rlen[0];

@@ -55,7 +55,7 @@ def _load():
         lib.dualip_oracle_jacobi_scaling.argtypes = [i64, i32, i32, vp, vp, vp, vp]
         lib.dualip_oracle_jacobi_scaling.restype = None
         lib.dualip_oracle_solve.argtypes = [i64, i32, i32, vp, vp, vp, vp, vp, ctypes.c_int, d, d,
-                                            vp, i32, vp, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+                                            vp, i32, vp, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         lib.dualip_oracle_solve.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -178,9 +178,11 @@ class SolveResult:
 
 
 def solve(p: Problem, gammas, iters, lam0=None, momentum: bool = True, want_x: bool = True,
-          trace_grad: bool = False, trace_lambda: bool = False, stage_x: bool = False, jacobi: bool = False) -> SolveResult:
+          trace_grad: bool = False, trace_lambda: bool = False, stage_x: bool = False, jacobi: bool = False,
+          is_eq=None) -> SolveResult:
     """gamma-continuation + projected Nesterov ascent (readings R1-R4); jacobi: on the row-scaled
-    system A' = D A, b' = D b, results reported in the original units (R18)."""
+    system A' = D A, b' = D b, results reported in the original units (R18); is_eq: uint8 mask
+    over the J*m coupling rows, nonzero = equality row whose dual is not projected (R19)."""
     gammas = _f64(gammas).reshape(-1)
     iters = np.ascontiguousarray(np.asarray(iters, dtype=np.int32)).reshape(-1)
     assert gammas.size == iters.size
@@ -192,9 +194,11 @@ def solve(p: Problem, gammas, iters, lam0=None, momentum: bool = True, want_x: b
     tgrad = np.empty((T, Jm)) if trace_grad else None
     tlam = np.empty((T, Jm)) if trace_lambda else None
     sx = np.empty((gammas.size, p.nnz)) if stage_x else None
+    eq = None if is_eq is None else np.ascontiguousarray(np.asarray(is_eq, dtype=np.uint8)).reshape(-1)
+    assert eq is None or eq.size == Jm
     rc = _load().dualip_oracle_solve(p.I, p.J, p.m, _ptr(p.row_ptr), _ptr(p.item_idx), _ptr(p.c), _ptr(p.a),
                                      _ptr(p.b), p.proj_kind, p.p0, p.p1, _ptr(gammas), gammas.size, _ptr(iters),
-                                     1 if momentum else 0, 1 if jacobi else 0, _ptr(lam), _ptr(x), _ptr(sc), _ptr(fg),
+                                     1 if momentum else 0, 1 if jacobi else 0, _ptr(eq), _ptr(lam), _ptr(x), _ptr(sc), _ptr(fg),
                                      _ptr(tg), _ptr(ti), _ptr(t2), _ptr(tgrad), _ptr(tlam), _ptr(sx))
     if rc != 0:
         raise MemoryError("oracle solve failed")

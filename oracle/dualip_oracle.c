@@ -238,6 +238,11 @@ void dualip_oracle_jacobi_scaling(int64_t I, int32_t J, int32_t m, const int64_t
  *   trace_g[n] = g(y_t), trace_rinf[n], trace_r2[n], trace_grad[n*Jm..] = grad(y_t),
  *   trace_lambda[n*Jm..] = lambda_{t+1}.  stage_x (may be NULL) receives, per stage, x*(lambda_end)
  *   at that stage's gamma (n_stages * nnz doubles) -- used by the drift report of config 5.
+ * is_eq (may be NULL = all rows are inequalities, Eq. 1): is_eq[q] != 0 marks coupling row q = j*m+k as an EQUALITY
+ *   (A x)_q = b_q; its dual is free in sign, so the projection onto lambda >= 0 is skipped for it ("projection
+ *   onto the nonnegative orthant for inequality coordinates"; reading R19) and its violation in the traced
+ *   residuals is |grad_q| instead of max(grad_q, 0).  The final scalars come from dualip_oracle_grad, which knows
+ *   no row kinds (inequality residuals).
  * jacobi != 0 (reading R18): the whole loop runs on the row-scaled system
  *   A' = D A, b' = D b with its own L' and dual lambda' (warm start lambda'_0 = D^-1 lambda_0); since
  *   A'^T lambda' = A^T (D lambda'), the dual of the ORIGINAL system is lambda = D lambda' and
@@ -245,7 +250,7 @@ void dualip_oracle_jacobi_scaling(int64_t I, int32_t J, int32_t m, const int64_t
 int dualip_oracle_solve(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr, const int32_t* item_idx,
                         const float* c, const float* a, const float* b, int proj_kind, double p0, double p1,
                         const double* gammas, int32_t n_stages, const int32_t* iters, int32_t momentum, int32_t jacobi,
-                        double* lambda_inout, double* x_out, double* final_scalars, double* final_grad,
+                        const uint8_t* is_eq, double* lambda_inout, double* x_out, double* final_scalars, double* final_grad,
                         double* trace_g, double* trace_rinf, double* trace_r2, double* trace_grad,
                         double* trace_lambda, double* stage_x) {
     int64_t Jm = (int64_t)J * m, nnz = row_ptr[I];
@@ -283,7 +288,9 @@ int dualip_oracle_solve(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr,
                 double r_inf = 0.0, r2 = 0.0;
                 for (int64_t q = 0; q < Jm; ++q) {
                     out[q] = grad[q] / d[q];
-                    if (out[q] > 0.0) { r2 += out[q] * out[q]; if (out[q] > r_inf) r_inf = out[q]; }
+                    double viol = (is_eq && is_eq[q]) ? fabs(out[q]) : fmax(out[q], 0.0);   /* |Ax-b| on equality rows */
+                    r2 += viol * viol;
+                    if (viol > r_inf) r_inf = viol;
                 }
                 if (trace_rinf) trace_rinf[n] = r_inf;
                 if (trace_r2) trace_r2[n] = sqrt(r2);
@@ -291,7 +298,9 @@ int dualip_oracle_solve(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr,
             }
             double beta = momentum ? (double)t / (double)(t + 3) : 0.0;
             for (int64_t q = 0; q < Jm; ++q) {
-                lam_new[q] = fmax(0.0, y[q] + eta * grad[q]);
+                lam_new[q] = y[q] + eta * grad[q];
+                if (!(is_eq && is_eq[q])) lam_new[q] = fmax(0.0, lam_new[q]);   /* "projection onto the nonnegative
+                                                                                    orthant for inequality coordinates" P:123 */
                 y[q] = lam_new[q] + beta * (lam_new[q] - lam[q]);
             }
             memcpy(lam, lam_new, (size_t)Jm * sizeof(double));

@@ -16,9 +16,10 @@ def _problem(d, kind=oracle.PROJ_SIMPLEX_INEQ, p0=1.0, p1=0.0):
     return oracle.Problem(d["I"], d["J"], d["m"], d["row_ptr"], d["item_idx"], d["c"], d["a"], d["b"], kind, p0, p1)
 
 
-def _kkt_brute_force(d, gamma):
+def _kkt_brute_force(d, gamma, eq_items=()):
     """min c'x + (gamma/2)|x|^2  s.t. x>=0, per-user sum<=1, per-item sum_i a_ij x_ij <= b_j, by
-    enumerating active sets and solving each equality-constrained QP (Eq. 1)."""
+    enumerating active sets and solving each equality-constrained QP (Eq. 1).  Items in eq_items have
+    sum_i a_ij x_ij = b_j instead: always active, multiplier free in sign."""
     n, I, J = d["item_idx"].size, d["I"], d["J"]
     c, a, b = d["c"].astype(np.float64), d["a"].astype(np.float64), d["b"].astype(np.float64)
     G, h = [], []
@@ -29,17 +30,19 @@ def _kkt_brute_force(d, gamma):
     for j in range(J):
         r = np.zeros(n); sel = d["item_idx"] == j; r[sel] = a[sel]; G.append(r); h.append(b[j])
     G, h = np.array(G), np.array(h)
+    forced = [n + I + j for j in eq_items]
+    free = [k for k in range(len(h)) if k not in forced]
     best = None
     for r in range(0, min(n, len(h)) + 1):
-        for S in itertools.combinations(range(len(h)), r):
-            S = list(S)
+        for S in itertools.combinations(free, r):
+            S = forced + list(S)
             if S:
                 GS = G[S]
                 if np.linalg.matrix_rank(GS) < len(S):
                     continue
                 mu = np.linalg.solve(GS @ GS.T, -(gamma * h[S] + GS @ c))
                 x = -(c + GS.T @ mu) / gamma
-                if (mu < -1e-10).any():
+                if (mu[len(forced):] < -1e-10).any():
                     continue
             else:
                 x = -c / gamma
@@ -277,3 +280,50 @@ def test_jacobi_warm_start_and_stages_chain():
     second = oracle.solve(p, [0.1], [30], lam0=first.lam, jacobi=True)
     np.testing.assert_allclose(second.lam, both.lam, rtol=1e-12, atol=1e-15)
     assert (both.lam > 0).any()
+
+
+# ---- equality coupling rows: the dual of an equality is free in sign, so the lambda >= 0 projection applies to
+# "inequality coordinates" only (reading R19) ---------------------------------------------------------
+
+def test_equality_row_closed_form_needs_a_negative_dual():
+    """I=J=1, c=-0.1, a=1, gamma=1: the unconstrained ridge primal is x = 0.1.  As an inequality x <= 0.9 is slack
+    (lambda stays 0, x = 0.1); as an equality x = 0.9 needs lambda* = -(c + gamma b/a)/a = -0.8 < 0."""
+    d = dict(I=1, J=1, m=1, row_ptr=np.array([0, 1]), item_idx=np.array([0], dtype=np.int32),
+             c=np.array([-0.1], dtype=np.float32), a=np.array([1.0], dtype=np.float32), b=np.array([0.9], dtype=np.float32))
+    ineq = oracle.solve(_problem(d), [1.0], [2000])
+    assert ineq.lam[0] == 0.0 and abs(ineq.x[0] - np.float64(np.float32(0.1))) < 1e-12
+    eq = oracle.solve(_problem(d), [1.0], [2000], is_eq=[1])
+    lam_star = -(np.float64(np.float32(-0.1)) + np.float64(np.float32(0.9)))
+    assert abs(eq.lam[0] - lam_star) < 1e-9 and lam_star < -0.7
+    assert abs(eq.x[0] - np.float64(np.float32(0.9))) < 1e-9
+    assert eq.trace_rinf[0] == pytest.approx(abs(0.1 - 0.9), rel=1e-6)       # |Ax - b| at lambda = 0, not max(.,0) = 0
+    assert eq.trace_rinf[-1] < 1e-8
+
+
+@pytest.mark.parametrize("seed", range(5))
+def test_equality_rows_converge_to_kkt_optimum(seed):
+    """Item 0 is an equality row, item 1 an inequality: brute force with the equality always active."""
+    rng = np.random.default_rng(300 + seed)
+    d = random_problem(rng, I=int(rng.integers(2, 4)), J=2, m=1, deg=(2, 2), tight=0.7)
+    # a feasible, not-trivially-slack right-hand side: item 0 must carry exactly 30-60 % of what its users could give
+    sel0 = d["item_idx"] == 0
+    d["b"] = np.array([(0.3 + 0.3 * rng.random()) * d["a"][sel0].min(), 0.15 + 0.5 * rng.random()], dtype=np.float32)
+    gamma = 0.5
+    best = _kkt_brute_force(d, gamma, eq_items=(0,))
+    assert best is not None
+    p_star, x_star = best
+    res = oracle.solve(_problem(d), [gamma], [6000], is_eq=[1, 0])
+    np.testing.assert_allclose(res.x, x_star, atol=1e-5)
+    assert abs(res.final.g - p_star) < 1e-7 * (1 + abs(p_star))
+    A0 = sum(np.float64(d["a"][p]) * res.x[p] for p in range(d["item_idx"].size) if d["item_idx"][p] == 0)
+    assert abs(A0 - np.float64(d["b"][0])) < 1e-6                          # the equality holds at the limit
+    assert res.lam[1] >= 0.0                                               # the inequality's dual stays projected
+
+
+def test_equality_mask_all_zero_is_the_plain_loop():
+    rng = np.random.default_rng(9)
+    d = random_problem(rng, I=40, J=5, m=2, deg=(2, 4), tight=0.3)
+    a = oracle.solve(_problem(d), [0.2], [50], trace_lambda=True)
+    b = oracle.solve(_problem(d), [0.2], [50], trace_lambda=True, is_eq=np.zeros(10, dtype=np.uint8))
+    np.testing.assert_array_equal(a.trace_lambda, b.trace_lambda)
+    np.testing.assert_array_equal(a.trace_rinf, b.trace_rinf)

@@ -100,8 +100,8 @@ typedef struct {
     double g;      /* dual objective g(lambda) = obj + reg + lambda'grad */
     double obj;    /* c'x* */
     double reg;    /* (gamma/2)|x*|^2 */
-    double r_inf;  /* max(0, max_jk grad_jk) : maximum positive constraint violation */
-    double r_2;    /* |max(grad, 0)|_2 */
+    double r_inf;  /* max(0, max_jk grad_jk) : maximum positive constraint violation (|grad| on equality rows) */
+    double r_2;    /* |max(grad, 0)|_2 (|grad| on equality rows) */
 } dualip_scalars;
 
 /* Optional per-iteration trace of dualip_solve.  All pointers are DEVICE pointers (or NULL to skip that
@@ -185,6 +185,13 @@ int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int3
 /* Replace c (nnz fp32, host or device) in place without rebuilding -- config 5's perturbed re-solve.
  * Recomputes the objective's fixed-point scale.  With borrow = 1 the handle switches to the new pointer. */
 int dualip_set_c(dualip_t* h, const float* c_new, void* stream);
+
+/* Marks coupling rows as EQUALITIES (A x)_{j,k} = b_{j,k} ("projection onto the nonnegative orthant for
+ * inequality coordinates"; R19).  is_equality[J*m] (uint8, host or device; [j*m+k] != 0 = equality), or NULL to
+ * make every row an inequality again (the default, Eq. 1).  An equality row's dual is free in sign: dualip_solve skips
+ * the lambda >= 0 projection for it, and r_inf / r_2 (dualip_grad and dualip_solve alike) count |grad| for it instead
+ * of max(grad, 0).  Nothing else changes: g and grad g are defined for any sign of lambda. */
+int dualip_set_equality_rows(dualip_t* h, const uint8_t* is_equality, void* stream);
 
 /* DUALIP_RED_CSC only (else DUALIP_EUNSUPPORTED): copies out the item-sorted permutation built at create (a0).
  *   col_ptr_out[J+1] int64: column j's entries are perm[col_ptr[j] .. col_ptr[j+1]);

@@ -17,7 +17,8 @@ RED_AUTO, RED_SMEM, RED_GLOBAL, RED_CSC = 0, 1, 2, 3
 PRECOND_NONE, PRECOND_JACOBI = 0, 1
 
 EXPORTED_SYMBOLS = ("dualip_opts_default", "dualip_create", "dualip_grad", "dualip_solve", "dualip_set_c",
-                    "dualip_set_profiling", "dualip_get_info", "dualip_get_csc", "dualip_destroy", "dualip_strerror")
+                    "dualip_set_equality_rows", "dualip_set_profiling", "dualip_get_info", "dualip_get_csc", "dualip_destroy",
+                    "dualip_strerror")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 
@@ -86,6 +87,7 @@ def load_library():
         lib.dualip_grad.argtypes = [vp, vp, d, vp, vp, vp, vp]
         lib.dualip_solve.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, ctypes.POINTER(_Trace), vp]
         lib.dualip_set_c.argtypes = [vp, vp, vp]
+        lib.dualip_set_equality_rows.argtypes = [vp, vp, vp]
         lib.dualip_get_info.argtypes = [vp, ctypes.POINTER(Info)]
         lib.dualip_set_profiling.argtypes = [vp, ctypes.c_int]
         lib.dualip_get_csc.argtypes = [vp, vp, vp, vp]
@@ -94,7 +96,8 @@ def load_library():
         lib.dualip_destroy.restype = None
         lib.dualip_strerror.argtypes = [ctypes.c_int]
         lib.dualip_strerror.restype = ctypes.c_char_p
-        for f in ("dualip_create", "dualip_grad", "dualip_solve", "dualip_set_c", "dualip_get_info", "dualip_set_profiling"):
+        for f in ("dualip_create", "dualip_grad", "dualip_solve", "dualip_set_c", "dualip_set_equality_rows", "dualip_get_info",
+                  "dualip_set_profiling"):
             getattr(lib, f).restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -209,6 +212,10 @@ class Problem:
         _check(load_library().dualip_set_c(self._h, _ptr(c_new, np.float32), _stream_ptr(stream)))
         if self._keep is not None:
             self._keep = self._keep + (c_new,)
+
+    def set_equality_rows(self, is_equality, stream=None):
+        """dualip_set_equality_rows: uint8 mask over the J*m coupling rows (tensor / array), or None for all-inequality."""
+        _check(load_library().dualip_set_equality_rows(self._h, _ptr(is_equality, np.uint8), _stream_ptr(stream)))
 
     def get_csc(self, col_ptr=None, perm=None, stream=None):
         """dualip_get_csc: fills col_ptr int64[J+1] and perm int64[nnz] (tensors / arrays or None)."""

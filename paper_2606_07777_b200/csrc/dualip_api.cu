@@ -74,6 +74,7 @@ struct dualip {
     double L = 0.0, max_colabs = 0.0, sum_abs_c = 0.0;
     double L_step = 0.0;                   // the constant the step is derived from: L, or L' of the row-scaled system (Jacobi)
     double* step_scale = nullptr;          // [JM] d_q^2 (Jacobi) or nullptr
+    unsigned char* row_eq = nullptr;       // [JM] equality-row mask (dualip_set_equality_rows) or nullptr
     float max_abs_a = 0.0f, max_abs_c = 0.0f;
     long long max_row_len = 0;
     double scale_s = 1.0, scale_obj = 1.0, scale_sq = 1.0;
@@ -403,6 +404,7 @@ void prof_collect(dualip* h) {
 void fill_finalize_common(const dualip* h, FinalizeParams& f) {
     f.s_fix = h->s_fix; f.sc_fix = h->sc_fix; f.b = h->b; f.JM = h->J * h->m;
     f.inv_scale_s = 1.0 / h->scale_s; f.inv_scale_obj = 1.0 / h->scale_obj; f.inv_scale_sq = 1.0 / h->scale_sq;
+    f.row_eq = h->row_eq;
     f.state = reinterpret_cast<IterState*>(h->ctl);
     f.done = reinterpret_cast<unsigned*>(h->ctl + sizeof(IterState));
 }
@@ -585,7 +587,7 @@ void dualip_destroy(dualip_t* h) {
     if (h->own_rows) { cudaFree((void*)h->row_ptr); cudaFree((void*)h->idx); cudaFree((void*)h->a); }
     if (h->own_c) cudaFree((void*)h->c);
     cudaFree(h->b); cudaFree(h->s_fix); cudaFree(h->lam_cur); cudaFree(h->y); cudaFree(h->lam_stage);
-    cudaFree(h->grad_stage); cudaFree(h->scalars_dev); cudaFree(h->step_scale); cudaFree(h->x_stage); cudaFree(h->tiles);
+    cudaFree(h->grad_stage); cudaFree(h->scalars_dev); cudaFree(h->step_scale); cudaFree(h->row_eq); cudaFree(h->x_stage); cudaFree(h->tiles);
     drop_graph(h);
     cudaFree(h->ctl);
     cudaFree(h->csc_perm); cudaFree(h->col_ptr); cudaFree(h->chunk_ptr); cudaFree(h->chunk_item); cudaFree(h->csc_partial);
@@ -782,6 +784,20 @@ int dualip_set_c(dualip_t* h, const float* c_new, void* stream) {
     int rc = compute_stats(h, st, false, true);
     if (rc != 0) return rc;
     set_scales(h);
+    return DUALIP_OK;
+}
+
+int dualip_set_equality_rows(dualip_t* h, const uint8_t* is_equality, void* stream) {
+    if (!h) return DUALIP_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t JM = (size_t)h->J * h->m;
+    if (!is_equality) {                                      // back to all-inequality rows
+        if (h->row_eq) { CK(cudaStreamSynchronize(st)); cudaFree(h->row_eq); h->row_eq = nullptr; h->bytes_resident -= (long long)JM; }
+        return DUALIP_OK;
+    }
+    if (!h->row_eq) { int rc = dev_alloc(h, &h->row_eq, JM); if (rc != 0) return rc; }
+    CK(cudaMemcpyAsync(h->row_eq, is_equality, JM, cudaMemcpyDefault, st));
+    if (!is_device_ptr(is_equality)) CK(cudaStreamSynchronize(st));
     return DUALIP_OK;
 }
 

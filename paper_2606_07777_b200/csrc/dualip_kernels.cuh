@@ -145,6 +145,7 @@ struct FinalizeParams {
     int momentum;               // beta_t = t/(t+3) (R1) or 0
     double eta;
     const double* step_scale;   // nullable: per-coordinate factor on eta (Jacobi preconditioning, R18: d_q^2 = 1/|A_q*|^2)
+    const unsigned char* row_eq; // nullable: nonzero = equality coupling row (dual free in sign, violation |grad|; R19)
     double* lam_cur;            // lambda_t -> lambda_{t+1}
     double* y;                  // y_t -> y_{t+1} (== lam_eval when update)
     IterState* state;           // read and advanced when update
@@ -166,13 +167,14 @@ __device__ __forceinline__ void finalize_block(const FinalizeParams& p, double* 
     // L2 round trips, and this CTA runs alone at the end of the launch
     constexpr int U = 4;
     for (int q0 = tid; q0 < p.JM; q0 += U * nthreads) {
-        unsigned long long sf[U]; float bb[U]; double le[U], lo[U], et[U];
+        unsigned long long sf[U]; float bb[U]; double le[U], lo[U], et[U]; bool eq[U];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             const int q = q0 + u * nthreads;
-            sf[u] = 0ull; bb[u] = 0.0f; le[u] = 0.0; lo[u] = 0.0; et[u] = p.eta;
+            sf[u] = 0ull; bb[u] = 0.0f; le[u] = 0.0; lo[u] = 0.0; et[u] = p.eta; eq[u] = false;
             if (q < p.JM) {
                 sf[u] = __ldcg(p.s_fix + q); bb[u] = __ldg(p.b + q); le[u] = __ldcg(p.lam_eval + q);
+                if (p.row_eq) eq[u] = __ldg(p.row_eq + q) != 0;
                 if (p.update) {
                     lo[u] = __ldcg(p.lam_cur + q);
                     if (p.step_scale) et[u] = p.eta * __ldg(p.step_scale + q);
@@ -187,11 +189,13 @@ __device__ __forceinline__ void finalize_block(const FinalizeParams& p, double* 
             p.s_fix[q] = 0ull;
             const double g = s - (double)bb[u];
             dot = fma(le[u], g, dot);
-            if (g > 0.0) { r2 = fma(g, g, r2); rinf = fmax(rinf, g); }
+            const double viol = eq[u] ? fabs(g) : fmax(g, 0.0);
+            r2 = fma(viol, viol, r2); rinf = fmax(rinf, viol);
             if (p.grad_out) p.grad_out[q] = g;
             if (p.update) {
                 if (p.tr_grad) p.tr_grad[n * p.JM + q] = g;
-                const double ln = fmax(0.0, le[u] + et[u] * g);
+                const double lv = le[u] + et[u] * g;
+                const double ln = eq[u] ? lv : fmax(0.0, lv);            // lambda >= 0 on inequality coordinates only
                 p.lam_cur[q] = ln;
                 p.y[q] = ln + beta * (ln - lo[u]);
                 if (p.tr_lam) p.tr_lam[n * p.JM + q] = ln;

@@ -332,3 +332,39 @@ def test_jacobi_zero_rows_and_families():
     lam0 = rng.random(180) * 0.05
     assert_trajectory_parity(po, pg, [0.1, 0.01], [25, 25], lam0=lam0, tag="jacobi/zero-rows", jacobi=True)
     pg.destroy()
+
+
+# ---- equality coupling rows (R19) --------------------------------------------------------------------
+
+@pytest.mark.parametrize("jacobi", [False, True])
+def test_equality_rows_trajectory(jacobi):
+    """Every third coupling row is an equality: its dual goes negative where the row is slack, the others stay >= 0;
+    per-iteration parity of grad, lambda and the |Ax-b| residuals with the oracle."""
+    rng = np.random.default_rng(41)
+    d = _ragged(rng, 2500, 60, 2, [4, 9, 17, 30, 0, 12])
+    d["b"] = (d["b"] * 3.0).astype(np.float32)
+    mask = (np.arange(120) % 3 == 0).astype(np.uint8)
+    po, pg = both(d, jacobi=jacobi)
+    pg.set_equality_rows(torch.from_numpy(mask).cuda())
+    gam, its = [0.2, 0.02], [40, 40]
+    ref = oracle.solve(po, gam, its, trace_grad=True, trace_lambda=True, jacobi=jacobi, is_eq=mask)
+    out = gpu_solve(pg, gam, its)
+    for n in range(80):
+        assert rel_l2(out["tr_grad"][n], ref.trace_grad[n]) <= 1e-5, n
+    scale = np.abs(ref.trace_lambda).max()
+    assert np.abs(out["tr_lam"] - ref.trace_lambda).max() <= 1e-6 * scale + 1e-12
+    gn = np.linalg.norm(ref.trace_grad, axis=1)
+    assert np.all(np.abs(out["tr_rinf"] - ref.trace_rinf) <= 1e-5 * gn + 1e-12)
+    assert np.all(np.abs(out["tr_r2"] - ref.trace_r2) <= 1e-5 * gn + 1e-12)
+    assert np.abs(out["x"].astype(np.float64) - ref.x).max() <= 1e-5
+    assert (ref.lam[mask == 1] < 0).any() and (ref.lam[mask == 0] >= 0).all()
+    # host mask, and NULL restores the all-inequality loop
+    pg.set_equality_rows(mask)
+    out2 = gpu_solve(pg, gam, its, want_x=False)
+    np.testing.assert_array_equal(out2["tr_lam"], out["tr_lam"])
+    pg.set_equality_rows(None)
+    ref0 = oracle.solve(po, gam, its, trace_lambda=True, jacobi=jacobi)
+    out0 = gpu_solve(pg, gam, its, want_x=False)
+    assert np.abs(out0["tr_lam"] - ref0.trace_lambda).max() <= 1e-6 * np.abs(ref0.trace_lambda).max() + 1e-12
+    assert (out0["lam"] >= 0).all()
+    pg.destroy()

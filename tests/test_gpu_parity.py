@@ -368,3 +368,42 @@ def test_equality_rows_trajectory(jacobi):
     assert np.abs(out0["tr_lam"] - ref0.trace_lambda).max() <= 1e-6 * np.abs(ref0.trace_lambda).max() + 1e-12
     assert (out0["lam"] >= 0).all()
     pg.destroy()
+
+
+def test_cfg5_continuation_then_perturbed_resolve_drift_per_gamma():
+    """BASELINE config 5's whole workflow at a user count the oracle finishes in seconds: gamma 1e-1 -> 1e-4 (x0.1 per
+    stage, warm-started lambda), x kept at every stage end; then c perturbed by N(0, (0.01|c|)^2) (R13), the same
+    schedule re-solved from lambda = 0, and ||x - x_prev||_2 reported per gamma.  The CUDA path chains one
+    dualip_solve per stage (lambda carried on the device); the oracle returns its stage-end x from ONE multi-stage
+    solve.  Jacobi step, so that lambda really moves on this Zipf instance."""
+    cfg = synth.get_config("cfg5-tight", I=40_000)
+    inst = synth.generate(cfg)
+    po, pg = from_instance(inst, jacobi=True)
+    its = [15] * len(cfg.gammas)
+    c2 = synth.perturb_c(inst)
+
+    def gpu_run():
+        lam = torch.zeros(inst.J * inst.m, dtype=torch.float64, device="cuda")
+        xs = []
+        for gam, it in zip(cfg.gammas, its):
+            x = torch.empty(inst.nnz, dtype=torch.float32, device="cuda")
+            pg.solve([gam], [it], lam, x=x)
+            xs.append(x.cpu().numpy().astype(np.float64))
+        return lam.cpu().numpy(), xs
+
+    lam1, xs1 = gpu_run()
+    ref1 = oracle.solve(po, cfg.gammas, its, jacobi=True, stage_x=True)
+    pg.set_c(c2.cuda())
+    lam2, xs2 = gpu_run()
+    po2 = oracle.Problem(po.I, po.J, po.m, po.row_ptr, po.item_idx, c2.numpy(), po.a, po.b, po.proj_kind, po.p0, po.p1)
+    ref2 = oracle.solve(po2, cfg.gammas, its, jacobi=True, stage_x=True)
+    assert (ref1.lam > 0).sum() >= 5
+    for s, gam in enumerate(cfg.gammas):
+        assert np.abs(xs1[s] - ref1.stage_x[s]).max() <= 1e-5, f"stage {s} x"
+        assert np.abs(xs2[s] - ref2.stage_x[s]).max() <= 1e-5, f"stage {s} x (perturbed)"
+        drift_gpu = np.linalg.norm(xs1[s] - xs2[s])
+        drift_ref = np.linalg.norm(ref1.stage_x[s] - ref2.stage_x[s])
+        assert abs(drift_gpu - drift_ref) <= 1e-5 * np.sqrt(inst.nnz) + 1e-6 * drift_ref, f"gamma={gam}: {drift_gpu} vs {drift_ref}"
+    assert np.abs(lam1 - ref1.lam).max() <= 1e-6 * np.abs(ref1.lam).max() + 1e-12
+    assert np.abs(lam2 - ref2.lam).max() <= 1e-6 * np.abs(ref2.lam).max() + 1e-12
+    pg.destroy()

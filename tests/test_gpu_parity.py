@@ -407,3 +407,21 @@ def test_cfg5_continuation_then_perturbed_resolve_drift_per_gamma():
     assert np.abs(lam1 - ref1.lam).max() <= 1e-6 * np.abs(ref1.lam).max() + 1e-12
     assert np.abs(lam2 - ref2.lam).max() <= 1e-6 * np.abs(ref2.lam).max() + 1e-12
     pg.destroy()
+
+
+def test_pipeline_geometry_does_not_change_a_bit():
+    """Streaming kernel: 2 / 3 / 4 stages, small tiles, odd grids -- the round-robin deal of row-steps to warps changes,
+    the 64-bit fixed-point sums do not: grad g, g and x are bit-identical (numerics)."""
+    inst = synth.generate(synth.get_config("cfg3-tight", I=30_000))
+    lam = synth.probe_lambda(inst, 1, 0.05).numpy()
+    outs = []
+    for stages, tile, grid in ((0, 0, 0), (2, 0, 0), (4, 0, 0), (3, 512, 0), (4, 1024, 29), (2, 256, 148)):
+        po, pg = from_instance(inst, stages=stages, tile_units=tile, grid_ctas=grid)
+        info = pg.info()
+        assert info.streaming == 1 and (stages == 0 or info.stages == stages) and (tile == 0 or info.tile_units <= tile)
+        sc, grad, x = gpu_grad(pg, lam, 1e-3)
+        outs.append((sc.g, sc.obj, sc.reg, grad.copy(), x.copy()))
+        pg.destroy()
+    for o in outs[1:]:
+        assert o[:3] == outs[0][:3] and np.array_equal(o[3], outs[0][3]) and np.array_equal(o[4], outs[0][4])
+    assert_grad_parity(*from_instance(inst, stages=4, tile_units=256), lam, 1e-3, tag="small tiles")

@@ -425,3 +425,32 @@ def test_pipeline_geometry_does_not_change_a_bit():
     for o in outs[1:]:
         assert o[:3] == outs[0][:3] and np.array_equal(o[3], outs[0][3]) and np.array_equal(o[4], outs[0][4])
     assert_grad_parity(*from_instance(inst, stages=4, tile_units=256), lam, 1e-3, tag="small tiles")
+
+
+@pytest.mark.parametrize("J,m", [(40_000, 1), (60_000, 1), (300_000, 1), (30_000, 2), (150_000, 2)])
+def test_many_items_lambda_beyond_shared_memory(J, m):
+    """J*m from just inside the streaming kernel's shared-memory budget (fp32 lambda only, small stages) to far beyond
+    any on-chip copy of lambda (direct-load kernel, duals gathered through L2): same parity bar; the atomics-free CSC
+    reduction (fp64 column sums) gives the same x bit for bit and the same gradient to fp32 product rounding."""
+    rng = np.random.default_rng(J + m)
+    I = 20_000
+    d = _ragged(rng, I, J, m, [3, 12, 40, 0, 7, 90, 25])
+    d["b"] = (d["b"] * 0.2).astype(np.float32)
+    po, pg = both(d)
+    info = pg.info()
+    if 4 * J * m + 32 * 1024 + 256 <= 227 * 1024:
+        assert info.streaming == 1
+    else:
+        assert info.streaming == 0
+    lam = rng.random(J * m) * 0.3
+    for gamma in (1e-1, 1e-3):
+        assert_grad_parity(po, pg, lam, gamma, tag=f"J={J} m={m} g={gamma}")
+    sc0, g0, x0 = gpu_grad(pg, lam, 1e-2)
+    _, pc = both(d, reduction=pkg.RED_CSC)
+    sc1, g1, x1 = gpu_grad(pc, lam, 1e-2)
+    assert np.array_equal(x0, x1) and rel_l2(g1, g0) < 1e-7
+    assert_trajectory_parity(po, pg, [1e-1, 1e-2], [12, 12], tag=f"J={J} m={m} solve", jacobi=False)
+    _, pj = both(d, jacobi=True)
+    assert_trajectory_parity(po, pj, [1e-1], [12], tag=f"J={J} m={m} jacobi", jacobi=True)
+    for h in (pg, pc, pj):
+        h.destroy()

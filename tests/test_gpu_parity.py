@@ -454,3 +454,27 @@ def test_many_items_lambda_beyond_shared_memory(J, m):
     assert_trajectory_parity(po, pj, [1e-1], [12], tag=f"J={J} m={m} jacobi", jacobi=True)
     for h in (pg, pc, pj):
         h.destroy()
+
+
+def test_very_long_rows_and_no_users():
+    """Rows longer than any stage (20,000 and 9,000 items: the streaming plan refuses, the direct-load kernel's whole-warp
+    path takes them) next to short ones; and the degenerate I = 0 problem (grad g = -b, g = -lambda'b)."""
+    rng = np.random.default_rng(123)
+    J = 25_000
+    d = _ragged(rng, 60, J, 1, [20_000, 5, 9_000, 33, 0, 400, 1])
+    d["b"] = (d["b"] * 0.05).astype(np.float32)
+    for kind, p0, p1 in (("simplex", 1.0, 0.0), ("boxcut", 0.001, 1.0), ("simplex_eq", 1.0, 0.0)):
+        po, pg = both(d, kind, p0, p1)
+        assert pg.info().streaming == 0 and pg.info().max_row_len == 20_000
+        for gamma, ls in ((1.0, 0.0), (1e-2, 0.5), (1e-4, 0.5)):
+            assert_grad_parity(po, pg, rng.random(J) * ls, gamma, tag=f"long/{kind}/g={gamma}")
+        pg.destroy()
+    e = dict(I=0, J=4, m=1, row_ptr=np.zeros(1, dtype=np.int64), item_idx=np.zeros(0, dtype=np.int32),
+             c=np.zeros(0, dtype=np.float32), a=np.zeros(0, dtype=np.float32), b=np.array([1, 2, 3, 4], dtype=np.float32))
+    po, pg = both(e)
+    lam = np.array([0.5, 0.0, 1.5, 2.0])
+    sc, grad, x = gpu_grad(pg, lam, 0.1)
+    assert np.array_equal(grad, -e["b"].astype(np.float64)) and sc.g == -(lam @ e["b"]) and x.size == 0 and sc.r_inf == 0.0
+    out = gpu_solve(pg, [0.1], [5], lam0=lam, want_trace=False)
+    assert np.all(out["lam"] <= lam) and np.all(out["lam"] >= 0)
+    pg.destroy()

@@ -219,10 +219,63 @@ __device__ __noinline__ FixPair slow_row(const GradParams& p, const StageView v,
     const int mm = M > 0 ? M : p.m;
     const int end = beg + len;
     int j; float cc; float aa[M > 0 ? M : 4];
+    const bool ineq = p.proj != PROJ_SIMPLEX_EQ;
+    constexpr int KS = 4;                              // register-resident rows: up to 32*KS nonzeros
+    if (!GBOX && len <= 32 * KS) {
+        // Rows of up to 128 nonzeros (all but the tail of every config): the fp64 t = c + a.lambda is formed ONCE per
+        // nonzero and kept in registers, and the Michelot iterations run on the shifted fp32 values there.  Same values,
+        // same per-lane summation order (k ascending) and same reductions as the re-reading loops below, so the result is
+        // bit-identical to them; it only drops the 5-8 re-evaluations per nonzero that dominate the fractional regime
+        // (large gamma, binding constraints).
+        double tk[KS];
+        float wmax = -CUDART_INF_F;
+#pragma unroll
+        for (int k = 0; k < KS; ++k) {
+            const int q = beg + lane + 32 * k;
+            tk[k] = CUDART_INF;
+            if (q < end) { tk[k] = exact_t<M>(v, cx, mm, q, j, cc, aa); wmax = fmaxf(wmax, (float)(-tk[k])); }
+        }
+        const float m32 = group_max<32>(wmax);
+        if (ineq && !(m32 > 0.0f)) {
+            if (p.x) for (int q = beg + lane; q < end; q += 32) p.x[nzb + q] = 0.0f;
+            return fp;
+        }
+        const double md = (double)m32;
+        const float mv = m32 * p.inv_gamma_f, z = p.z;
+        float u[KS];
+#pragma unroll
+        for (int k = 0; k < KS; ++k) u[k] = (beg + lane + 32 * k < end) ? (float)(-tk[k] - md) * p.inv_gamma_f : -CUDART_INF_F;
+        float theta = -z - (1.2e-7f * fabsf(mv) + 1e-6f);
+        int n_prev = -1;
+        for (;;) {
+            float sm = 0.0f; int n = 0;
+#pragma unroll
+            for (int k = 0; k < KS; ++k) if (u[k] > theta) { sm += u[k]; ++n; }
+            sm = group_sum<32>(sm); n = group_sum_i<32>(n);
+            if (n == n_prev || n == 0) break;
+            theta = fmaxf((sm - z) / (float)n, theta);
+            n_prev = n;
+        }
+        const float tau = ineq ? fmaxf(theta, -mv) : theta;
+#pragma unroll
+        for (int k = 0; k < KS; ++k) {
+            const int q = beg + lane + 32 * k;
+            if (q < end) {
+                const float x = fmaxf(u[k] - tau, 0.0f);
+                if (p.x) p.x[nzb + q] = x;
+                if (x > 0.0f) {
+                    j = v.idx[q]; cc = v.c[q];
+#pragma unroll
+                    for (int f = 0; f < (M > 0 ? M : 4); ++f) aa[f] = f < mm ? v.a[q * mm + f] : 0.0f;
+                    push<M, ACC_SMEM>(p, cx, fp, mm, j, cc, aa, x);
+                }
+            }
+        }
+        return fp;
+    }
     float wmax = -CUDART_INF_F;
     for (int q = beg + lane; q < end; q += 32) wmax = fmaxf(wmax, (float)(-exact_t<M>(v, cx, mm, q, j, cc, aa)));
     const float m32 = group_max<32>(wmax);
-    const bool ineq = p.proj != PROJ_SIMPLEX_EQ;
     if (ineq && !(m32 > 0.0f)) {
         if (p.x) for (int q = beg + lane; q < end; q += 32) p.x[nzb + q] = 0.0f;
         return fp;

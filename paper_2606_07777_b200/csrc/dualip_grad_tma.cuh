@@ -99,6 +99,7 @@ struct ConsumerCtx {
     const float* lam_lo;                          // lambda - hi in shared memory (exact to 2^-48 relative), or nullptr:
     const double* lam_g;                          //   then the exact path reads the fp64 lambda from global memory (L2)
     unsigned* acc_lo; unsigned* acc_hi;           // shared-memory item accumulators (ACC_SMEM)
+    bool hi_only;                                 // RN_f32(lambda) is exact enough for this launch's gamma (see k_grad_tma)
 };
 struct FixPair { long long obj, sq; };            // per-lane fixed-point partial scalars (order-independent)
 
@@ -146,7 +147,8 @@ __device__ __forceinline__ double exact_t(const StageView& v, const ConsumerCtx&
         aa[f] = 0.0f;
         if (f < mm) {
             aa[f] = v.a[q * mm + f];
-            const double l = cx.lam_lo ? (double)cx.lam_hi[j * mm + f] + (double)cx.lam_lo[j * mm + f] : __ldg(cx.lam_g + j * mm + f);
+            const double l = cx.hi_only ? (double)cx.lam_hi[j * mm + f]
+                                        : (cx.lam_lo ? (double)cx.lam_hi[j * mm + f] + (double)cx.lam_lo[j * mm + f] : __ldg(cx.lam_g + j * mm + f));
             t = fma((double)aa[f], l, t);
         }
     }
@@ -388,11 +390,10 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
             if (tp.lam_lo_smem) s_lo32[q] = (float)(l - (double)h);
             lmax = fmaxf(lmax, fabsf(h));
         }
-        if (M != 1) {                                                      // the filter's rounding bound needs max |lambda|
+        // max |lambda|: the filter's rounding bound (M > 1) and the hi_only test below need it
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) lmax = fmaxf(lmax, __shfl_xor_sync(kFull, lmax, o));
-            if ((threadIdx.x & 31) == 0) atomicMax(&s_words[0], __float_as_uint(lmax));
-        }
+        for (int o = 16; o > 0; o >>= 1) lmax = fmaxf(lmax, __shfl_xor_sync(kFull, lmax, o));
+        if ((threadIdx.x & 31) == 0) atomicMax(&s_words[0], __float_as_uint(lmax));
     }
     if (ACC_SMEM) for (int q = threadIdx.x; q < 2 * JM; q += NT) a_lo[q] = 0u;
     {   // consumers read whole 16-byte vectors around a row: every stage word must always hold a valid item index
@@ -409,7 +410,13 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
     __syncthreads();
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const ConsumerCtx cx{s_hi32, tp.lam_lo_smem ? s_lo32 : nullptr, p.lambda, a_lo, a_hi};
+    // The exact path needs lambda beyond fp32 only when 1/gamma amplifies its rounding into x: dropping the low word moves
+    // w by at most m max|a| max|lambda| 2^-25, v = w/gamma by that over gamma, and any x by at most twice that.  When the
+    // bound is below 1e-7 (two orders inside the 1e-5 bar, the size of the fp32 steps that follow anyway) the exact path
+    // reads RN_f32(lambda) from shared memory instead of the fp64 dual through L2 -- which is what makes rows in the
+    // fractional regime (large gamma, or lambda = 0) cost one shared-memory latency instead of one L2 round trip each.
+    const bool hi_only = (float)mm * p.max_abs_a * __uint_as_float(s_words[0]) * p.inv_gamma_f * 5.9604645e-8f <= 1e-7f;
+    const ConsumerCtx cx{s_hi32, tp.lam_lo_smem ? s_lo32 : nullptr, p.lambda, a_lo, a_hi, hi_only};
     FixPair fp{0ll, 0ll};
 
     if (warp == 0) {

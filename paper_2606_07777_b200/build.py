@@ -12,10 +12,10 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdualip_b200.so")
-SOURCES = ["dualip_api.cu"]
+SOURCES = ["dualip_api.cu", "dualip_tma_wx0.cu", "dualip_tma_wx1.cu"]   # compiled in parallel, then linked
 HEADERS = ["dualip_kernels.cuh", "dualip_grad_tma.cuh", "dualip_csc.cuh", os.path.join("..", "..", "include", "dualip.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "-Xcompiler", "-fPIC,-O2,-Wall", "-shared"]
+              "-Xcompiler", "-fPIC,-O2,-Wall"]
 
 
 def _nvcc() -> str:
@@ -33,12 +33,26 @@ def is_stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+def _compile_and_link(out: str, flags: list, log=None) -> None:
+    """One nvcc -c per source, all at once (the template instantiations dominate the build time), then one link."""
+    import tempfile
+    with tempfile.TemporaryDirectory() as td:
+        objs, procs = [], []
+        for src in SOURCES:
+            obj = os.path.join(td, src.replace(".cu", ".o"))
+            objs.append(obj)
+            procs.append(subprocess.Popen([_nvcc()] + flags + ["-c", "-o", obj, os.path.join(CSRC, src)],
+                                          stdout=log, stderr=subprocess.STDOUT if log else None))
+        rcs = [pr.wait() for pr in procs]
+        if any(rcs):
+            raise subprocess.CalledProcessError(max(rcs), "nvcc -c")
+        subprocess.check_call([_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", out] + objs)
+
+
 def build(force: bool = False, verbose: bool = False, defines: dict | None = None, out: str | None = None) -> str:
     """defines/out: build an experimental variant (e.g. {"DUALIP_NWC": 23}) next to the default library."""
     if out is not None:
-        cmd = [_nvcc()] + NVCC_FLAGS + [f"-D{k}={v}" for k, v in (defines or {}).items()] + ["-o", out] + \
-              [os.path.join(CSRC, s) for s in SOURCES]
-        subprocess.check_call(cmd)
+        _compile_and_link(out, NVCC_FLAGS + [f"-D{k}={v}" for k, v in (defines or {}).items()])
         return out
     if not force and not is_stale():
         return LIB
@@ -46,8 +60,7 @@ def build(force: bool = False, verbose: bool = False, defines: dict | None = Non
     if verbose:
         flags += ["-Xptxas", "-v"]
     tmp = LIB + f".{os.getpid()}.tmp"
-    cmd = [_nvcc()] + flags + ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
-    subprocess.check_call(cmd)
+    _compile_and_link(tmp, flags)
     os.replace(tmp, LIB)
     return LIB
 

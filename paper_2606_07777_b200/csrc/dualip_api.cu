@@ -2,6 +2,7 @@
 // gamma-continuation driver (a0, a7).  Every arithmetic step of the path runs in the kernels of
 // dualip_kernels.cuh; the host only sizes buffers, picks fixed-point exponents and launches.
 #include "../../include/dualip.h"
+#define DUALIP_HOST_KERNELS 1
 #include "dualip_kernels.cuh"
 #include "dualip_grad_tma.cuh"
 #include "dualip_csc.cuh"
@@ -15,14 +16,14 @@
 
 using namespace dualip_dev;
 
+// kernel tables of the two streaming-kernel translation units (dualip_tma_wx0.cu: never writes x; dualip_tma_wx1.cu: writes x)
+const void* dualip_tma_kernel_wx0(int G, int M, bool acc_smem, bool gbox);
+const void* dualip_tma_kernel_wx1(int G, int M, bool acc_smem, bool gbox);
+
 namespace {
 
 constexpr size_t kSmemBudget = 227 * 1024;  // bytes of dynamic shared memory one CTA may opt in to on sm_100a
 
-#ifndef DUALIP_NWC
-#define DUALIP_NWC 15
-#endif
-constexpr int kTmaConsumerWarps = DUALIP_NWC;  // consumer warps of the streaming kernel (+ 1 producer warp)
 #ifndef DUALIP_LO_SMEM_KB
 #define DUALIP_LO_SMEM_KB 64
 #endif
@@ -33,6 +34,7 @@ struct Plan {
     int grid = 0;
     size_t smem = 0;
     const void* fn = nullptr;
+    const void* fn_x = nullptr;     // streaming path: the x-writing instantiation (fn never writes x)
     // streaming (TMA) path
     bool tma = false, lam_lo_smem = false;
     long long TN = 0, ntiles = 0;
@@ -147,29 +149,6 @@ const void* pick_kernel(const Plan& pl) {
     return pick_k<32>(pl.KREG, pl.M, pl.lam_smem, pl.acc_smem);
 }
 
-template <int G, int M>
-const void* pick_tma_acc(bool acc, bool gbox) {
-    if (acc) return gbox ? (const void*)k_grad_tma<G, M, true, true, kTmaConsumerWarps>
-                         : (const void*)k_grad_tma<G, M, true, false, kTmaConsumerWarps>;
-    return gbox ? (const void*)k_grad_tma<G, M, false, true, kTmaConsumerWarps>
-                : (const void*)k_grad_tma<G, M, false, false, kTmaConsumerWarps>;
-}
-template <int G>
-const void* pick_tma_m(int M, bool acc, bool gbox) {
-    if (M == 1) return pick_tma_acc<G, 1>(acc, gbox);
-    if (M == 2) return pick_tma_acc<G, 2>(acc, gbox);
-    return nullptr;
-}
-const void* pick_tma_kernel(const Plan& pl, bool gbox) {
-    if (pl.M == 0) return pick_tma_acc<8, 0>(pl.acc_smem, gbox);
-    if (pl.G == 1) return pick_tma_m<1>(pl.M, pl.acc_smem, gbox);
-    if (pl.G == 2) return pick_tma_m<2>(pl.M, pl.acc_smem, gbox);
-    if (pl.G == 4) return pick_tma_m<4>(pl.M, pl.acc_smem, gbox);
-    if (pl.G == 8) return pick_tma_m<8>(pl.M, pl.acc_smem, gbox);
-    if (pl.G == 16) return pick_tma_m<16>(pl.M, pl.acc_smem, gbox);
-    return pick_tma_m<32>(pl.M, pl.acc_smem, gbox);
-}
-
 // Streaming plan: lambda (and for small J*m the accumulators) in shared memory, the rest of the 227 KB split into
 // `stages` tile buffers.  Returns false if this problem cannot use it.
 bool plan_tma(dualip* h, Plan& pl) {
@@ -252,9 +231,11 @@ int make_plan(dualip* h) {
         pl.G = Gs;
         pl.KREG = 0;
         const bool gbox = h->opts.projection == DUALIP_PROJ_BOXCUT && h->opts.p0 < h->opts.p1;
-        pl.fn = pick_tma_kernel(pl, gbox);
-        if (!pl.fn) return DUALIP_EUNSUPPORTED;
+        pl.fn = dualip_tma_kernel_wx0(pl.G, pl.M, pl.acc_smem, gbox);
+        pl.fn_x = dualip_tma_kernel_wx1(pl.G, pl.M, pl.acc_smem, gbox);
+        if (!pl.fn || !pl.fn_x) return DUALIP_EUNSUPPORTED;
         CK(cudaFuncSetAttribute(pl.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+        CK(cudaFuncSetAttribute(pl.fn_x, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
         pl.grid = h->opts.grid_ctas > 0 ? h->opts.grid_ctas : (int)(pl.ntiles < h->num_sms ? pl.ntiles : h->num_sms);
         if (pl.grid < 1) pl.grid = 1;
         h->plan = pl;
@@ -435,7 +416,7 @@ void prepare_iter(const dualip* h, IterLaunch& L, const double* lam_dev, double 
         tp.g = L.p; tp.f = L.f; tp.tiles = h->tiles; tp.ntiles = h->plan.ntiles; tp.cap_nz = h->plan.cap_nz; tp.cap_rows = h->plan.cap_rows;
         tp.stages = h->plan.stages; tp.stage_bytes = h->plan.stage_bytes;
         tp.nnz4 = h->nnz & ~3ll; tp.rows2 = (h->I + 1) & ~1ll; tp.lam_lo_smem = h->plan.lam_lo_smem ? 1 : 0;
-        L.fn = h->plan.fn; L.grid = dim3(h->plan.grid); L.block = dim3(32 * (kTmaConsumerWarps + 1)); L.smem = h->plan.smem;
+        L.fn = L.p.x ? h->plan.fn_x : h->plan.fn; L.grid = dim3(h->plan.grid); L.block = dim3(32 * (kTmaConsumerWarps + 1)); L.smem = h->plan.smem;
         L.args[0] = &L.tp; L.args[1] = nullptr;
     } else {
         L.fn = h->plan.fn; L.grid = dim3(h->plan.grid); L.block = dim3(kBlockThreads); L.smem = h->plan.smem;

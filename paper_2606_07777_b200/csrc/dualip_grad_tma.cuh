@@ -29,6 +29,11 @@
 
 namespace dualip_dev {
 
+#ifndef DUALIP_NWC
+#define DUALIP_NWC 15
+#endif
+constexpr int kTmaConsumerWarps = DUALIP_NWC;  // consumer warps of the streaming kernel (+ 1 producer warp)
+
 constexpr int kRowCost = 8;            // each row costs this many "nonzero units" when cutting tiles
 constexpr int kTmaStagesMax = 4;
 
@@ -92,6 +97,11 @@ __device__ __forceinline__ StageView stage_view(unsigned char* base, int cap_nz,
     v.meta = reinterpret_cast<const StageMeta*>(v.rp + cap_rows);
     return v;
 }
+
+// The x output pointer, or a compile-time nullptr in the WX = false instantiations that dualip_solve's loop launches (it
+// never writes x): the x-writing code drops out of the hot kernel, which measured 2-5 % faster on every config.
+template <bool WX>
+__device__ __forceinline__ float* xout(const GradParams& p) { return WX ? p.x : nullptr; }
 
 // Shared state the row routines need.
 struct ConsumerCtx {
@@ -214,7 +224,7 @@ __device__ __forceinline__ void filter_pass(const StageView& v, const float* __r
 
 // Slow path: one row, whole warp, any length; every pass re-reads the staged row.  Same arithmetic as long_row()
 // in dualip_kernels.cuh (which documents the three box-cut steps).
-template <int M, bool ACC_SMEM, bool GBOX>
+template <int M, bool ACC_SMEM, bool GBOX, bool WX>
 __device__ __noinline__ FixPair slow_row(const GradParams& p, const StageView v, const ConsumerCtx cx, int beg, int len, long long nzb) {
     FixPair fp{0ll, 0ll};                              // returned in registers: the caller's accumulators never live in local memory
     const int lane = threadIdx.x & 31;
@@ -239,7 +249,7 @@ __device__ __noinline__ FixPair slow_row(const GradParams& p, const StageView v,
         }
         const float m32 = group_max<32>(wmax);
         if (ineq && !(m32 > 0.0f)) {
-            if (p.x) for (int q = beg + lane; q < end; q += 32) p.x[nzb + q] = 0.0f;
+            if (xout<WX>(p)) for (int q = beg + lane; q < end; q += 32) xout<WX>(p)[nzb + q] = 0.0f;
             return fp;
         }
         const double md = (double)m32;
@@ -264,7 +274,7 @@ __device__ __noinline__ FixPair slow_row(const GradParams& p, const StageView v,
             const int q = beg + lane + 32 * k;
             if (q < end) {
                 const float x = fmaxf(u[k] - tau, 0.0f);
-                if (p.x) p.x[nzb + q] = x;
+                if (xout<WX>(p)) xout<WX>(p)[nzb + q] = x;
                 if (x > 0.0f) {
                     j = v.idx[q]; cc = v.c[q];
 #pragma unroll
@@ -279,7 +289,7 @@ __device__ __noinline__ FixPair slow_row(const GradParams& p, const StageView v,
     for (int q = beg + lane; q < end; q += 32) wmax = fmaxf(wmax, (float)(-exact_t<M>(v, cx, mm, q, j, cc, aa)));
     const float m32 = group_max<32>(wmax);
     if (ineq && !(m32 > 0.0f)) {
-        if (p.x) for (int q = beg + lane; q < end; q += 32) p.x[nzb + q] = 0.0f;
+        if (xout<WX>(p)) for (int q = beg + lane; q < end; q += 32) xout<WX>(p)[nzb + q] = 0.0f;
         return fp;
     }
     const double md = (double)m32;
@@ -354,13 +364,13 @@ __device__ __noinline__ FixPair slow_row(const GradParams& p, const StageView v,
         const double tq = exact_t<M>(v, cx, mm, q, j, cc, aa);
         const float u = GBOX ? (float)(-tq * p.inv_gamma - ref) : (float)(-tq - md) * p.inv_gamma_f;
         const float x = fminf(fmaxf(u - tau, 0.0f), cap);
-        if (p.x) p.x[nzb + q] = x;
+        if (xout<WX>(p)) xout<WX>(p)[nzb + q] = x;
         if (x > 0.0f) push<M, ACC_SMEM>(p, cx, fp, mm, j, cc, aa, x);
     }
     return fp;
 }
 
-template <int G, int M, bool ACC_SMEM, bool GBOX, int NWC>
+template <int G, int M, bool ACC_SMEM, bool GBOX, bool WX, int NWC>
 __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams tp) {
     extern __shared__ __align__(128) unsigned char smem_tma[];
     const GradParams& p = tp.g;
@@ -590,7 +600,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                         }
                         if (xo > 0.0f) push<M, ACC_SMEM>(p, cx, fp, mm, j, cc, aa, xo);
                     }
-                    if (p.x) {
+                    if (xout<WX>(p)) {
                         const long long nzb = v.meta->nzb;
 #pragma unroll
                         for (int r = 0; r < RPG; ++r) {
@@ -598,7 +608,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                             const bool fr = __shfl_sync(kFull, (int)(active && fast), src) != 0;
                             const float xr = __shfl_sync(kFull, xo, src);
                             const int pr = __shfl_sync(kFull, fpos, src);
-                            if (fr) for (int e = gl; e < rlen[r]; e += G) p.x[nzb + rbeg[r] + e] = (rbeg[r] + e == pr) ? xr : 0.0f;
+                            if (fr) for (int e = gl; e < rlen[r]; e += G) xout<WX>(p)[nzb + rbeg[r] + e] = (rbeg[r] + e == pr) ? xr : 0.0f;
                         }
                     }
                     // ---- candidate path: rows that are neither a vertex nor dead.  Only nonzeros with w > w_max - z gamma
@@ -642,11 +652,11 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                             const float tau = ineq ? fmaxf(theta, -mv) : theta;
                             const float xq = (cand && alive) ? fmaxf(u - tau, 0.0f) : 0.0f;
                             if (xq > 0.0f) push<M, ACC_SMEM>(p, cx, fp, mm, j, cc, aa, xq);
-                            if (p.x) {
+                            if (xout<WX>(p)) {
                                 const long long nzb = v.meta->nzb;
-                                if (row_ok) for (int e = gl; e < rlen[r]; e += G) p.x[nzb + rbeg[r] + e] = 0.0f;
+                                if (row_ok) for (int e = gl; e < rlen[r]; e += G) xout<WX>(p)[nzb + rbeg[r] + e] = 0.0f;
                                 __syncwarp();
-                                if (cand) p.x[nzb + rpos[r]] = xq;
+                                if (cand) xout<WX>(p)[nzb + rpos[r]] = xq;
                             }
                             if (lane == src && row_ok) handled = true;
                         }
@@ -656,7 +666,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                 while (slow_mask) {
                     const int src = __ffs(slow_mask) - 1;
                     slow_mask &= slow_mask - 1;
-                    const FixPair sp = slow_row<M, ACC_SMEM, GBOX>(p, v, cx, __shfl_sync(kFull, fbeg, src), __shfl_sync(kFull, flen, src), v.meta->nzb);
+                    const FixPair sp = slow_row<M, ACC_SMEM, GBOX, WX>(p, v, cx, __shfl_sync(kFull, fbeg, src), __shfl_sync(kFull, flen, src), v.meta->nzb);
                     fp.obj += sp.obj; fp.sq += sp.sq;
                 }
             }
@@ -687,6 +697,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
     grid_epilogue(tp.f, reinterpret_cast<double*>(stage0), NT);
 }
 
+#ifdef DUALIP_HOST_KERNELS
 // a0: tile table.  Tile t starts at the first row r with row_ptr[r] + kRowCost*r >= t*TN (parallel binary search).
 __global__ void k_build_tiles(const long long* __restrict__ row_ptr, long long I, long long TN, long long ntiles, TileEntry* tiles) {
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t <= ntiles; t += (long long)gridDim.x * blockDim.x) {
@@ -705,5 +716,37 @@ __global__ void k_build_tiles(const long long* __restrict__ row_ptr, long long I
         tiles[t].nz0 = row_ptr[r];
     }
 }
+
+#endif  // DUALIP_HOST_KERNELS
+
+// Kernel table of one translation unit: dualip_tma_wx0.cu / dualip_tma_wx1.cu each instantiate every (G, M, ACC_SMEM,
+// GBOX) variant for their WX and export this lookup, so the two halves compile in parallel.
+template <bool WX>
+struct TmaKernelTable {
+    template <int G, int M>
+    static const void* acc(bool a, bool gbox) {
+        if (a) return gbox ? (const void*)k_grad_tma<G, M, true, true, WX, kTmaConsumerWarps>
+                           : (const void*)k_grad_tma<G, M, true, false, WX, kTmaConsumerWarps>;
+        return gbox ? (const void*)k_grad_tma<G, M, false, true, WX, kTmaConsumerWarps>
+                    : (const void*)k_grad_tma<G, M, false, false, WX, kTmaConsumerWarps>;
+    }
+    template <int G>
+    static const void* fam(int M, bool a, bool gbox) {
+        if (M == 1) return acc<G, 1>(a, gbox);
+        if (M == 2) return acc<G, 2>(a, gbox);
+        return nullptr;
+    }
+    static const void* get(int G, int M, bool a, bool gbox) {
+        if (M == 0) return acc<8, 0>(a, gbox);
+        switch (G) {
+            case 1: return fam<1>(M, a, gbox);
+            case 2: return fam<2>(M, a, gbox);
+            case 4: return fam<4>(M, a, gbox);
+            case 8: return fam<8>(M, a, gbox);
+            case 16: return fam<16>(M, a, gbox);
+            default: return fam<32>(M, a, gbox);
+        }
+    }
+};
 
 }  // namespace dualip_dev

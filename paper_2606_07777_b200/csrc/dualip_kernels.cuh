@@ -602,6 +602,8 @@ __global__ void __launch_bounds__(256) k_grad_box(const GradParams p, const Fina
 
 // ---- a0: create-time kernels -------------------------------------------------------------------------------
 
+// Create-time kernels (not templates): defined in the one translation unit that launches them (dualip_api.cu).
+#ifdef DUALIP_HOST_KERNELS
 // flags: bit0 row_ptr not monotone, bit1 index out of range, bit2 duplicate item in a row
 __global__ void k_validate(const long long* __restrict__ row_ptr, const int* __restrict__ idx, long long I, int J,
                            long long nnz, int scan, int* flags, unsigned long long* max_len) {
@@ -702,5 +704,7 @@ __global__ void k_jacobi_step_scale(const unsigned long long* colsq, double inv_
         step_scale[q] = n2 > 0.0 ? 1.0 / n2 : 1.0;
     }
 }
+
+#endif  // DUALIP_HOST_KERNELS
 
 }  // namespace dualip_dev

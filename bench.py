@@ -33,8 +33,8 @@ if ROOT not in sys.path:
 METRIC = "dual-ascent nonzeros/s (nnz x AGD iterations/s), fused gradient iteration"
 UNIT = "nnz/s"
 # DRAM bytes per k_grad launch from the committed `ncu --set full` capture (profiles/), or None until one exists.
-NCU_TRAFFIC_BYTES = {"cfg3": 6.086913e9 + 36.230912e6, "cfg5": 7.388645e9 + 36.391168e6, "cfg4": 81.170748e9 + 37.114624e6,
-                     "cfg2": 249.596160e6 + 36.192256e6}   # profiles/r01f_k_grad_tma_full.csv (dram read + write, one launch)
+NCU_TRAFFIC_BYTES = {"cfg3": 6.085430e9 + 37.377024e6, "cfg5": 7.381245e9 + 37.766912e6, "cfg4": 81.132569e9 + 38.185216e6,
+                     "cfg2": 249.187584e6 + 36.514560e6}   # profiles/r01g_k_grad_tma_full.csv (dram read + write, one launch)
 
 
 def parse_args():

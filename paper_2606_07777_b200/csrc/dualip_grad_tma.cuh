@@ -262,8 +262,12 @@ __device__ __noinline__ FixPair slow_row(const GradParams& p, const StageView v,
         for (;;) {
             float sm = 0.0f; int n = 0;
 #pragma unroll
-            for (int k = 0; k < KS; ++k) if (u[k] > theta) { sm += u[k]; ++n; }
-            sm = group_sum<32>(sm); n = group_sum_i<32>(n);
+            for (int k = 0; k < KS; ++k) {
+                const bool in = u[k] > theta;
+                if (in) sm += u[k];
+                if (32 * k < len) n += __popc(__ballot_sync(kFull, in));     // the count needs no shuffle tree
+            }
+            sm = group_sum<32>(sm);
             if (n == n_prev || n == 0) break;
             theta = fmaxf((sm - z) / (float)n, theta);
             n_prev = n;

@@ -374,6 +374,81 @@ __device__ __noinline__ FixPair slow_row(const GradParams& p, const StageView v,
     return fp;
 }
 
+// All slow rows of one row-step.  `mask`: lanes whose (fbeg, flen) describe a slow row.  Rows of at most 32 nonzeros (simplex
+// kinds) run two at a time, one per half-warp with two nonzeros per lane -- always in that layout, partner or not, so a
+// row's arithmetic does not depend on what else is in its step; everything else goes to slow_row one row at a time.
+template <int M, bool ACC_SMEM, bool GBOX, bool WX>
+__device__ __noinline__ FixPair slow_rows_all(const GradParams& p, const StageView v, const ConsumerCtx cx, int fbeg, int flen, unsigned mask,
+                                              long long nzb) {
+    FixPair fp{0ll, 0ll};
+    const int lane = threadIdx.x & 31, h = lane & 15;
+    const int mm = M > 0 ? M : p.m;
+    const bool ineq = p.proj != PROJ_SIMPLEX_EQ;
+    const float z = p.z;
+    const unsigned hmask = lane < 16 ? 0x0000ffffu : 0xffff0000u;
+    while (mask) {
+        const int s0 = __ffs(mask) - 1;
+        mask &= mask - 1;
+        const int b0 = __shfl_sync(kFull, fbeg, s0), l0 = __shfl_sync(kFull, flen, s0);
+        if (GBOX || l0 > 32) {
+            const FixPair sp = slow_row<M, ACC_SMEM, GBOX, WX>(p, v, cx, b0, l0, nzb);
+            fp.obj += sp.obj; fp.sq += sp.sq;
+            continue;
+        }
+        int b1 = 0, l1 = 0;                                  // partner: the next slow row that is short too
+        for (unsigned m2 = mask; m2; m2 &= m2 - 1) {
+            const int s1 = __ffs(m2) - 1;
+            const int lc = __shfl_sync(kFull, flen, s1);
+            if (lc <= 32) { b1 = __shfl_sync(kFull, fbeg, s1); l1 = lc; mask &= ~(1u << s1); break; }
+        }
+        const int beg = lane < 16 ? b0 : b1, len = lane < 16 ? l0 : l1;
+        int j; float cc; float aa[M > 0 ? M : 4];
+        double tk[2];
+        float wmax = -CUDART_INF_F;
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            tk[k] = CUDART_INF;
+            if (h + 16 * k < len) { tk[k] = exact_t<M>(v, cx, mm, beg + h + 16 * k, j, cc, aa); wmax = fmaxf(wmax, (float)(-tk[k])); }
+        }
+        const float m16 = group_max<16>(wmax);
+        const bool alive = len > 0 && (!ineq || m16 > 0.0f);
+        const double md = (double)m16;
+        const float mv = m16 * p.inv_gamma_f;
+        float u[2];
+#pragma unroll
+        for (int k = 0; k < 2; ++k) u[k] = (alive && h + 16 * k < len) ? (float)(-tk[k] - md) * p.inv_gamma_f : -CUDART_INF_F;
+        float theta = -z - (1.2e-7f * fabsf(mv) + 1e-6f);
+        int n_prev = -1;
+        bool stop = !alive;
+        for (;;) {
+            const bool in0 = u[0] > theta, in1 = u[1] > theta;
+            const float sm = group_sum<16>((in0 ? u[0] : 0.0f) + (in1 ? u[1] : 0.0f));
+            const int n = __popc(__ballot_sync(kFull, in0) & hmask) + __popc(__ballot_sync(kFull, in1) & hmask);
+            if (!stop) {
+                if (n == n_prev || n == 0) stop = true;
+                else { theta = fmaxf((sm - z) / (float)n, theta); n_prev = n; }
+            }
+            if (__all_sync(kFull, stop)) break;
+        }
+        const float tau = ineq ? fmaxf(theta, -mv) : theta;
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            if (h + 16 * k < len) {
+                const int q = beg + h + 16 * k;
+                const float x = fmaxf(u[k] - tau, 0.0f);
+                if (xout<WX>(p)) xout<WX>(p)[nzb + q] = x;
+                if (x > 0.0f) {
+                    j = v.idx[q]; cc = v.c[q];
+#pragma unroll
+                    for (int f = 0; f < (M > 0 ? M : 4); ++f) aa[f] = f < mm ? v.a[q * mm + f] : 0.0f;
+                    push<M, ACC_SMEM>(p, cx, fp, mm, j, cc, aa, x);
+                }
+            }
+        }
+    }
+    return fp;
+}
+
 template <int G, int M, bool ACC_SMEM, bool GBOX, bool WX, int NWC>
 __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams tp) {
     extern __shared__ __align__(128) unsigned char smem_tma[];
@@ -667,10 +742,8 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                     }
                     slow_mask = __ballot_sync(kFull, want && !handled);
                 }
-                while (slow_mask) {
-                    const int src = __ffs(slow_mask) - 1;
-                    slow_mask &= slow_mask - 1;
-                    const FixPair sp = slow_row<M, ACC_SMEM, GBOX, WX>(p, v, cx, __shfl_sync(kFull, fbeg, src), __shfl_sync(kFull, flen, src), v.meta->nzb);
+                if (slow_mask) {
+                    const FixPair sp = slow_rows_all<M, ACC_SMEM, GBOX, WX>(p, v, cx, fbeg, flen, slow_mask, v.meta->nzb);
                     fp.obj += sp.obj; fp.sq += sp.sq;
                 }
             }

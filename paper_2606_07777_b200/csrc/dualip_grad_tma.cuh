@@ -374,77 +374,94 @@ __device__ __noinline__ FixPair slow_row(const GradParams& p, const StageView v,
     return fp;
 }
 
-// All slow rows of one row-step.  `mask`: lanes whose (fbeg, flen) describe a slow row.  Rows of at most 32 nonzeros (simplex
-// kinds) run two at a time, one per half-warp with two nonzeros per lane -- always in that layout, partner or not, so a
-// row's arithmetic does not depend on what else is in its step; everything else goes to slow_row one row at a time.
-template <int M, bool ACC_SMEM, bool GBOX, bool WX>
-__device__ __noinline__ FixPair slow_rows_all(const GradParams& p, const StageView v, const ConsumerCtx cx, int fbeg, int flen, unsigned mask,
-                                              long long nzb) {
-    FixPair fp{0ll, 0ll};
+// Two slow rows at once, one per half-warp, K nonzeros per lane (rows of at most 16*K nonzeros, simplex kinds): lanes 0-15
+// take (b0, l0), lanes 16-31 take (b1, l1); l1 = 0 means "no partner".  The arithmetic is slow_row's (fp64 t once per
+// nonzero, exact maximum, Michelot on the shifted fp32 values) with 16-lane reductions.
+template <int K, int M, bool ACC_SMEM, bool WX>
+__device__ __forceinline__ void half_warp_rows(const GradParams& p, const StageView& v, const ConsumerCtx& cx, FixPair& fp, int b0, int l0, int b1,
+                                               int l1, long long nzb) {
     const int lane = threadIdx.x & 31, h = lane & 15;
     const int mm = M > 0 ? M : p.m;
     const bool ineq = p.proj != PROJ_SIMPLEX_EQ;
     const float z = p.z;
     const unsigned hmask = lane < 16 ? 0x0000ffffu : 0xffff0000u;
+    const int beg = lane < 16 ? b0 : b1, len = lane < 16 ? l0 : l1;
+    int j; float cc; float aa[M > 0 ? M : 4];
+    double tk[K];
+    float wmax = -CUDART_INF_F;
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        tk[k] = CUDART_INF;
+        if (h + 16 * k < len) { tk[k] = exact_t<M>(v, cx, mm, beg + h + 16 * k, j, cc, aa); wmax = fmaxf(wmax, (float)(-tk[k])); }
+    }
+    const float m16 = group_max<16>(wmax);
+    const bool alive = len > 0 && (!ineq || m16 > 0.0f);
+    const double md = (double)m16;
+    const float mv = m16 * p.inv_gamma_f;
+    float u[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) u[k] = (alive && h + 16 * k < len) ? (float)(-tk[k] - md) * p.inv_gamma_f : -CUDART_INF_F;
+    float theta = -z - (1.2e-7f * fabsf(mv) + 1e-6f);
+    int n_prev = -1;
+    bool stop = !alive;
+    for (;;) {
+        float sm = 0.0f; int n = 0;
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            const bool in = u[k] > theta;
+            if (in) sm += u[k];
+            n += __popc(__ballot_sync(kFull, in) & hmask);
+        }
+        sm = group_sum<16>(sm);
+        if (!stop) {
+            if (n == n_prev || n == 0) stop = true;
+            else { theta = fmaxf((sm - z) / (float)n, theta); n_prev = n; }
+        }
+        if (__all_sync(kFull, stop)) break;
+    }
+    const float tau = ineq ? fmaxf(theta, -mv) : theta;
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        if (h + 16 * k < len) {
+            const int q = beg + h + 16 * k;
+            const float x = fmaxf(u[k] - tau, 0.0f);
+            if (xout<WX>(p)) xout<WX>(p)[nzb + q] = x;
+            if (x > 0.0f) {
+                j = v.idx[q]; cc = v.c[q];
+#pragma unroll
+                for (int f = 0; f < (M > 0 ? M : 4); ++f) aa[f] = f < mm ? v.a[q * mm + f] : 0.0f;
+                push<M, ACC_SMEM>(p, cx, fp, mm, j, cc, aa, x);
+            }
+        }
+    }
+}
+
+// All slow rows of one row-step.  `mask`: lanes whose (fbeg, flen) describe a slow row.  Rows of at most 32 / at most 64
+// nonzeros (simplex kinds) run two at a time on half-warps with 2 / 4 nonzeros per lane -- always in the layout of their
+// own length class, partner or not, so a row's arithmetic does not depend on what else is in its step; everything else
+// goes to slow_row one row at a time.
+template <int M, bool ACC_SMEM, bool GBOX, bool WX>
+__device__ __noinline__ FixPair slow_rows_all(const GradParams& p, const StageView v, const ConsumerCtx cx, int fbeg, int flen, unsigned mask,
+                                              long long nzb) {
+    FixPair fp{0ll, 0ll};
     while (mask) {
         const int s0 = __ffs(mask) - 1;
         mask &= mask - 1;
         const int b0 = __shfl_sync(kFull, fbeg, s0), l0 = __shfl_sync(kFull, flen, s0);
-        if (GBOX || l0 > 32) {
+        if (GBOX || l0 > 64) {
             const FixPair sp = slow_row<M, ACC_SMEM, GBOX, WX>(p, v, cx, b0, l0, nzb);
             fp.obj += sp.obj; fp.sq += sp.sq;
             continue;
         }
-        int b1 = 0, l1 = 0;                                  // partner: the next slow row that is short too
+        const bool small = l0 <= 32;
+        int b1 = 0, l1 = 0;                                  // partner: the next slow row of the same length class
         for (unsigned m2 = mask; m2; m2 &= m2 - 1) {
             const int s1 = __ffs(m2) - 1;
             const int lc = __shfl_sync(kFull, flen, s1);
-            if (lc <= 32) { b1 = __shfl_sync(kFull, fbeg, s1); l1 = lc; mask &= ~(1u << s1); break; }
+            if (lc <= 64 && (lc <= 32) == small) { b1 = __shfl_sync(kFull, fbeg, s1); l1 = lc; mask &= ~(1u << s1); break; }
         }
-        const int beg = lane < 16 ? b0 : b1, len = lane < 16 ? l0 : l1;
-        int j; float cc; float aa[M > 0 ? M : 4];
-        double tk[2];
-        float wmax = -CUDART_INF_F;
-#pragma unroll
-        for (int k = 0; k < 2; ++k) {
-            tk[k] = CUDART_INF;
-            if (h + 16 * k < len) { tk[k] = exact_t<M>(v, cx, mm, beg + h + 16 * k, j, cc, aa); wmax = fmaxf(wmax, (float)(-tk[k])); }
-        }
-        const float m16 = group_max<16>(wmax);
-        const bool alive = len > 0 && (!ineq || m16 > 0.0f);
-        const double md = (double)m16;
-        const float mv = m16 * p.inv_gamma_f;
-        float u[2];
-#pragma unroll
-        for (int k = 0; k < 2; ++k) u[k] = (alive && h + 16 * k < len) ? (float)(-tk[k] - md) * p.inv_gamma_f : -CUDART_INF_F;
-        float theta = -z - (1.2e-7f * fabsf(mv) + 1e-6f);
-        int n_prev = -1;
-        bool stop = !alive;
-        for (;;) {
-            const bool in0 = u[0] > theta, in1 = u[1] > theta;
-            const float sm = group_sum<16>((in0 ? u[0] : 0.0f) + (in1 ? u[1] : 0.0f));
-            const int n = __popc(__ballot_sync(kFull, in0) & hmask) + __popc(__ballot_sync(kFull, in1) & hmask);
-            if (!stop) {
-                if (n == n_prev || n == 0) stop = true;
-                else { theta = fmaxf((sm - z) / (float)n, theta); n_prev = n; }
-            }
-            if (__all_sync(kFull, stop)) break;
-        }
-        const float tau = ineq ? fmaxf(theta, -mv) : theta;
-#pragma unroll
-        for (int k = 0; k < 2; ++k) {
-            if (h + 16 * k < len) {
-                const int q = beg + h + 16 * k;
-                const float x = fmaxf(u[k] - tau, 0.0f);
-                if (xout<WX>(p)) xout<WX>(p)[nzb + q] = x;
-                if (x > 0.0f) {
-                    j = v.idx[q]; cc = v.c[q];
-#pragma unroll
-                    for (int f = 0; f < (M > 0 ? M : 4); ++f) aa[f] = f < mm ? v.a[q * mm + f] : 0.0f;
-                    push<M, ACC_SMEM>(p, cx, fp, mm, j, cc, aa, x);
-                }
-            }
-        }
+        if (small) half_warp_rows<2, M, ACC_SMEM, WX>(p, v, cx, fp, b0, l0, b1, l1, nzb);
+        else half_warp_rows<4, M, ACC_SMEM, WX>(p, v, cx, fp, b0, l0, b1, l1, nzb);
     }
     return fp;
 }

@@ -224,7 +224,7 @@ int make_plan(dualip* h) {
             // (2 * 32/G rows each) as there are consumer warps: long rows (few per tile) get wider groups
             const double rows_per_tile = (double)pl.TN / (mean + kRowCost);
             int Gt = 1;
-            while (Gt < 32 && (double)Gt * rows_per_tile < 640.0) Gt <<= 1;
+            while (Gt < 32 && (double)Gt * rows_per_tile < 600.0) Gt <<= 1;
             if (Gt > Gs) Gs = Gt;
         }
         if (pl.M == 0) Gs = 8;

@@ -124,10 +124,12 @@ def test_full_size_gradient(name, lam_scale, full_oracle):
         d = inst.numpy()
         po_full = _oracle_problem(cfg, inst.I, d["row_ptr"], d["item_idx"], d["c"], d["a"], d["b"])
     # lambda = 0 is what the verbatim configs evaluate at every iteration (they are slack); the
-    # probe is a busy lambda; "soft" repeats it at 100 x gamma, where a large share of the rows is fractional
+    # probe is a busy lambda; "soft" repeats it at 100 x gamma, where a large share of the rows is fractional; "dense" is
+    # gamma = 0.1 at lambda = 0 (the first stage of config 5's schedule): hardly any row is a vertex, every slow path runs
     for which, lam, gamma in (("zero", torch.zeros(Jm, dtype=torch.float64, device="cuda"), cfg.gammas[-1]),
                               ("probe", synth.probe_lambda(inst, 0, lam_scale), cfg.gammas[-1]),
-                              ("soft", synth.probe_lambda(inst, 1, lam_scale), 100.0 * cfg.gammas[-1])):
+                              ("soft", synth.probe_lambda(inst, 1, lam_scale), 100.0 * cfg.gammas[-1]),
+                              ("dense", torch.zeros(Jm, dtype=torch.float64, device="cuda"), 0.1)):
         sc = pkg.Scalars()
         pg.grad(lam, gamma, grad=grad, scalars=sc, x=x)
         torch.cuda.synchronize()

@@ -1,12 +1,19 @@
 #!/usr/bin/env python
 """bench.py -- measures the dual-ascent hot path on B200 (contract: see the task statement / DESIGN.md section 8).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg3]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload cfgN|cfgN-tight] [--gamma G] [--jacobi] [--adaptive] [--lambda zero|probe]
+                    [--pre "1e-1:200,1e-2:200"] [--legs default|none|NAME,NAME...]
 
 A "step" is ONE dual-ascent iteration of the whole hot path (gather lambda, candidate,
-projection, item reduction, scalars, AGD update) over the full synthetic workload.  Workload = BASELINE.json
+projection, item reduction, scalars, AGD update) over the full synthetic workload.  Headline workload = BASELINE.json
 config 3 (10M users x 10k items, ~500M nonzeros, Zipf(1.1) items, box-cut(1,1), gamma = 1e-3): the config the
-north_star quotes the bandwidth target on and the largest one that is routinely a single-GPU case.
+north_star quotes the bandwidth target on.  Taken verbatim it is slack at lambda = 0, so the headline number is the
+VERTEX regime (almost every row projects onto a vertex, lambda stays 0).  The regime in which the solver moves lambda
+(binding constraints, large gamma: most rows fractional) is measured by the extra LEGS below and by the flags:
+
+    --workload cfg3-tight --jacobi --pre 1e-1:200,1e-2:200 --gamma 1e-3     the fractional regime near the optimum
+    --workload cfg5 --gamma 1e-1                                            stage 1 of config 5's own schedule
 
 Prints ONE JSON line.  `value` = nonzeros processed per second (= nnz x iterations/s), whole job, inputs
 resident in HBM.  `e2e` = the same metric through the C ABI with HOST (pinned) buffers: dualip_create (H2D of
@@ -14,11 +21,14 @@ all row data) + dualip_solve (K iterations + final evaluation) + D2H of lambda a
 `roofline` = the gradient kernel's algorithmic bytes / its average launch time (CUDA events on the launching
 stream, recorded inside the timed region by the library's profiling hook) against the measured HBM peak.
 `cpu_baseline` = the fp64 oracle, as it stands, timed on one host core on a bounded sample of the same workload.
+`legs` (N = 1, default run only) = the same measurement, K steps each, for the other large configs and for the
+fractional regime, so that every number DESIGN.md / BASELINE.md quote is one tracked command.
 Multi-GPU: replicas only -- N independent copies of the job, max time over ranks.
 """
 from __future__ import annotations
 
 import argparse
+import csv
 import json
 import os
 import subprocess
@@ -32,9 +42,23 @@ if ROOT not in sys.path:
 
 METRIC = "dual-ascent nonzeros/s (nnz x AGD iterations/s), fused gradient iteration"
 UNIT = "nnz/s"
-# DRAM bytes per k_grad launch from the committed `ncu --set full` capture (profiles/), or None until one exists.
-NCU_TRAFFIC_BYTES = {"cfg3": 6.085430e9 + 37.377024e6, "cfg5": 7.381245e9 + 37.766912e6, "cfg4": 81.132569e9 + 38.185216e6,
-                     "cfg2": 249.187584e6 + 36.514560e6}   # profiles/r01g_k_grad_tma_full.csv (dram read + write, one launch)
+# The committed `ncu --set full` capture the `roofline.traffic` figure is READ from (rows: config,kernel,metric,unit,value;
+# the config column is the leg name).  profiles/README.md names the command that produced it.
+NCU_CAPTURE = os.path.join("profiles", "r02_k_grad_tma_full.csv")
+NCU_CAPTURE_FALLBACK = os.path.join("profiles", "r01g_k_grad_tma_full.csv")
+
+AGD_NOTE = ("projected Nesterov ascent, beta_t = t/(t+3), gradient at the extrapolated point: the paper prints no update "
+            "formula, so this part is oracle-defined and parity-unpinned against the paper (DESIGN.md R1)")
+
+# Extra legs of the default N = 1 run: name -> measurement spec.  The vertex-regime legs are the verbatim configs at
+# their final gamma; the fractional legs are the regime the solver actually works in.
+LEGS = {
+    "cfg3-tight+jacobi@1e-3": dict(workload="cfg3-tight", jacobi=True, pre="1e-1:200,1e-2:200", gamma=1e-3, regime="fractional"),
+    "cfg5@1e-1": dict(workload="cfg5", gamma=1e-1, regime="fractional"),
+    "cfg5": dict(workload="cfg5", regime="vertex"),
+    "cfg2": dict(workload="cfg2", regime="vertex"),
+    "cfg4": dict(workload="cfg4", regime="vertex"),
+}
 
 
 def parse_args():
@@ -43,7 +67,17 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=1000)      # config 3 states 1,000 AGD iterations
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg3")
+    ap.add_argument("--workload", default="cfg3", help="cfgN or cfgN-tight (greedy-load right-hand side: binding constraints)")
+    ap.add_argument("--gamma", type=float, default=None, help="ridge parameter of the timed steps (default: the config's final gamma)")
+    ap.add_argument("--jacobi", action="store_true", help="Jacobi-preconditioned step (DESIGN.md R18)")
+    ap.add_argument("--adaptive", action="store_true", help="range-clipped adaptive step (DESIGN.md R20)")
+    ap.add_argument("--lambda", dest="lam", default="zero", choices=["zero", "probe"],
+                    help="starting dual of the run: zeros (cold start) or the seeded probe lambda")
+    ap.add_argument("--lambda-scale", type=float, default=None, help="scale of the probe lambda (default 0.5; 0.05 for config 3)")
+    ap.add_argument("--pre", default="", help="untimed continuation stages run before the warm-up, e.g. 1e-1:200,1e-2:200")
+    ap.add_argument("--legs", default="default", help="extra legs in the same JSON line: default (all, N = 1 default workload only), "
+                    "none, or a comma list of " + ", ".join(LEGS))
+    ap.add_argument("--leg-steps", type=int, default=0, help="timed steps per extra leg (0 = min(--steps, 50))")
     ap.add_argument("--users", type=int, default=None, help="override the number of users (smaller = not the graded workload)")
     ap.add_argument("--group-lanes", type=int, default=0, help="lanes per row in the gradient kernel (0 = the library's choice)")
     ap.add_argument("--stages", type=int, default=0, help="pipeline stages of the streaming kernel (0 = the library's choice)")
@@ -64,6 +98,24 @@ def measured_peak():
             return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, STREAM-style copy)"
     except Exception:
         return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def ncu_traffic(leg_name: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one gradient-kernel launch, read from the committed capture."""
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+    for rel in (NCU_CAPTURE, NCU_CAPTURE_FALLBACK):
+        path = os.path.join(ROOT, rel)
+        if not os.path.exists(path):
+            continue
+        tot, seen = 0.0, 0
+        with open(path) as f:
+            for row in csv.DictReader(f):
+                if row.get("config") == leg_name and row.get("metric") in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+                    tot += float(row["value"]) * scale.get(row.get("unit", "byte"), 1.0)
+                    seen += 1
+        if seen == 2:
+            return tot, rel
+    return None, None
 
 
 class ClockSampler:
@@ -114,6 +166,19 @@ class ClockSampler:
         return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def parse_pre(text: str):
+    """'1e-1:200,1e-2:200' -> ([0.1, 0.01], [200, 200])"""
+    gam, its = [], []
+    for part in filter(None, (t.strip() for t in text.split(","))):
+        g, n = part.split(":")
+        gam.append(float(g)); its.append(int(n))
+    return gam, its
+
+
+def cfg_index(workload: str) -> int:
+    return int(workload[3]) - 1
+
+
 def oracle_problem(inst_np, cfg, oracle, synth):
     kind, p0, p1 = synth.proj_spec(cfg)
     k = {"simplex": oracle.PROJ_SIMPLEX_INEQ, "box": oracle.PROJ_BOX, "boxcut": oracle.PROJ_BOXCUT}[kind]
@@ -121,23 +186,13 @@ def oracle_problem(inst_np, cfg, oracle, synth):
     return oracle.Problem(I, cfg.J, cfg.m, inst_np["row_ptr"], inst_np["item_idx"], inst_np["c"], inst_np["a"], inst_np["b"], k, p0, p1)
 
 
-def time_oracle_steps(po, gamma, steps, warmup, oracle):
-    """One oracle step = one AGD iteration (gradient at y + update): oracle.solve with one iteration per call
-    would add a final evaluation, so time the two parts the iteration consists of: grad + the J*m update."""
-    import numpy as np
-    L = oracle.lipschitz(po)
-    lam = np.zeros(po.J * po.m); y = lam.copy()
-    times = []
-    for t in range(warmup + steps):
-        t0 = time.perf_counter()
-        r = oracle.grad(po, y, gamma, want_x=False)
-        new = np.maximum(0.0, y + (gamma / L) * r.grad)
-        y = new + (t / (t + 3.0)) * (new - lam)
-        lam = new
-        dt = time.perf_counter() - t0
-        if t >= warmup:
-            times.append(dt)
-    return times
+def time_oracle(po, gamma, iters, oracle, jacobi=False):
+    """The oracle as it stands: oracle.solve runs `iters` AGD iterations (R1-R4) plus the final evaluation at lambda_T (R3),
+    i.e. iters + 1 gradient evaluations -- what the product's dualip_solve does when asked for the final scalars.
+    Returns (seconds, evaluations)."""
+    t0 = time.perf_counter()
+    oracle.solve(po, [gamma], [iters], want_x=False, jacobi=jacobi)
+    return time.perf_counter() - t0, iters + 1
 
 
 def run_reference(args):
@@ -145,36 +200,165 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    import numpy as np
     import torch
 
     import oracle
     import synth
-    # bounded sample: about 1.5e9 nonzero-visits in the whole run (~2 minutes at the oracle's ~1.4e7 nnz/s per core),
+    # bounded sample: about 1.5e9 nonzero-visits in the whole run (~2 minutes at the oracle's ~1.3e7 nnz/s per core),
     # split over the K + W steps; every step is one full oracle iteration over the first `users` users of the workload
-    full0 = synth.get_config(args.workload)
-    mean_deg = {"const": lambda d: d[1], "uniform": lambda d: (d[1] + d[2]) / 2, "poisson": lambda d: d[1]}[full0.deg[0]](full0.deg)
-    users = int(1.5e9 / max(args.steps + args.warmup, 1) / mean_deg)
-    users = max(2_000, min(users, 400_000, full0.I)) if args.users is None else args.users
+    full = synth.get_config(args.workload)
+    mean_deg = {"const": lambda d: d[1], "uniform": lambda d: (d[1] + d[2]) / 2, "poisson": lambda d: d[1]}[full.deg[0]](full.deg)
+    users = int(1.5e9 / max(args.steps + args.warmup + 2, 1) / mean_deg)
+    users = max(2_000, min(users, 400_000, full.I)) if args.users is None else args.users
     cfg = synth.get_config(args.workload, I=users)
     dev = "cuda" if torch.cuda.is_available() else "cpu"
     inst = synth.generate(cfg, device=dev)
     d = inst.numpy()
     po = oracle_problem(d, cfg, oracle, synth)
-    times = time_oracle_steps(po, cfg.gammas[-1], args.steps, args.warmup, oracle)
-    tot = float(np.sum(times))
-    val = po.nnz * len(times) / tot
-    full = synth.get_config(args.workload)
-    sample = f"first {users} users of {args.workload} ({po.nnz} nnz) per step; oracle/dualip_oracle.c, 1 thread, fp64"
-    line = {"metric": METRIC, "value": val, "unit": UNIT, "impl": "reference", "n_gpus": args.gpus, "steps": len(times),
-            "warmup": args.warmup, "ms_per_step": 1e3 * tot / len(times), "higher_is_better": True, "scaling": "weak",
+    gamma = args.gamma if args.gamma is not None else cfg.gammas[-1]
+    if args.warmup > 0:
+        time_oracle(po, gamma, max(args.warmup - 1, 0), oracle, args.jacobi)                 # untimed
+    tot, evals = time_oracle(po, gamma, max(args.steps - 1, 0), oracle, args.jacobi)     # K gradient evaluations
+    val = po.nnz * evals / tot
+    sample = (f"first {users} users of {args.workload} ({po.nnz} nnz) per step; oracle.solve ({evals - 1} AGD iterations + the final "
+              f"evaluation = {evals} gradient evaluations); oracle/dualip_oracle.c, 1 thread, fp64")
+    line = {"metric": METRIC, "value": val, "unit": UNIT, "impl": "reference", "n_gpus": args.gpus, "steps": evals,
+            "warmup": args.warmup, "ms_per_step": 1e3 * tot / evals, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{args.workload} (BASELINE.json configs[{int(args.workload[3]) - 1}]: {full.I} users x {full.J} items); bounded sample",
-                       "sample_users": users, "sample_nnz": po.nnz, "gamma": cfg.gammas[-1]},
+            "config": {"workload": f"{args.workload} (BASELINE.json configs[{cfg_index(args.workload)}]: {full.I} users x {full.J} items); bounded sample",
+                       "sample_users": users, "sample_nnz": po.nnz, "gamma": gamma, "jacobi": bool(args.jacobi), "agd_rule": AGD_NOTE},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
+
+
+class Leg:
+    """One workload resident on the device + its problem handle; measures K timed steps."""
+
+    def __init__(self, pkg, synth, torch, spec, args):
+        self.pkg, self.synth, self.torch, self.args = pkg, synth, torch, args
+        self.workload = spec["workload"]
+        self.cfg = synth.get_config(self.workload, I=args.users)
+        self.jacobi = bool(spec.get("jacobi", False))
+        self.adaptive = bool(spec.get("adaptive", False))
+        self.gamma = float(spec["gamma"]) if spec.get("gamma") is not None else self.cfg.gammas[-1]
+        self.pre = parse_pre(spec.get("pre", "") or "")
+        self.lam_mode = spec.get("lam", "zero")
+        self.lam_scale = spec.get("lam_scale")
+        self.regime = spec.get("regime")
+        t0 = time.time()
+        self.inst = synth.generate(self.cfg, device="cuda")
+        torch.cuda.synchronize()
+        self.t_gen = time.time() - t0
+        kind, p0, p1 = synth.proj_spec(self.cfg)
+        self.kind, self.p0, self.p1 = kind, p0, p1
+        self.proj = {"simplex": pkg.PROJ_SIMPLEX_INEQ, "box": pkg.PROJ_BOX, "boxcut": pkg.PROJ_BOXCUT}[kind]
+        t0 = time.time()
+        self.prob = pkg.Problem.create(self.inst.I, self.inst.J, self.inst.m, self.inst.row_ptr, self.inst.item_idx, self.inst.c,
+                                       self.inst.a, self.inst.b, self.opts(borrow=True))
+        torch.cuda.synchronize()
+        self.t_create = time.time() - t0
+        self.info = self.prob.info()
+        inst = self.inst
+        self.nnz, self.Jm = inst.nnz, inst.J * inst.m
+        self.alg_bytes = inst.nnz * (4 + 4 + 4 * inst.m) + 8 * inst.I    # SURVEY 8(d): idx + c + a per nonzero, row_ptr per user
+
+    def opts(self, borrow):
+        a = self.args
+        return self.pkg.binding.make_opts(projection=self.proj, p0=self.p0, p1=self.p1, borrow=borrow, group_lanes=a.group_lanes,
+                                          grid_ctas=a.grid_ctas, stages=a.stages, tile_units=a.tile_units, use_graph=a.graph,
+                                          jacobi=self.jacobi, adaptive=self.adaptive)
+
+    def start_lambda(self):
+        torch = self.torch
+        if self.lam_mode == "probe":
+            scale = self.lam_scale if self.lam_scale is not None else (0.05 if self.workload.startswith("cfg3") else 0.5)
+            return self.synth.probe_lambda(self.inst, 0, scale).clone()
+        return torch.zeros(self.Jm, dtype=torch.float64, device="cuda")
+
+    def measure(self, steps, warmup, barrier, local_rank):
+        """pre stages (untimed) -> W warm-up iterations -> exactly K timed iterations, all continuing one trajectory."""
+        torch, prob = self.torch, self.prob
+        lam = self.start_lambda()
+        stream = torch.cuda.current_stream()
+        if self.pre[0]:
+            prob.solve(self.pre[0], self.pre[1], lam)
+        prob.solve([self.gamma], [max(warmup, 3)], lam)
+        barrier()
+        prob.set_profiling(not self.args.graph)
+        launches0 = prob.info().launches
+        sampler = ClockSampler(local_rank)
+        sampler.start()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        ev0.record(stream)
+        prob.solve([self.gamma], [steps], lam)                     # no final outputs requested: K gradient+update steps
+        ev1.record(stream)
+        barrier()
+        clocks = sampler.stop()
+        ms_total = ev0.elapsed_time(ev1)
+        inf = prob.info()
+        launches = inf.launches - launches0
+        kern_ms = inf.grad_kernel_ms / max(inf.grad_kernel_count, 1) if not self.args.graph else ms_total / steps
+        prob.set_profiling(False)
+        sc = self.pkg.Scalars()
+        prob.grad(lam, self.gamma, scalars=sc)                      # state the timed steps ended in (untimed)
+        torch.cuda.synchronize()
+        state = {"g": sc.g, "r_inf": sc.r_inf, "active_duals": int((lam > 0).sum().item()), "lambda_max": float(lam.max().item())}
+        return {"ms_total": ms_total, "kern_ms": kern_ms, "launches": int(launches), "timed": int(inf.grad_kernel_count),
+                "clocks": clocks, "state": state}
+
+    def kernel_name(self):
+        i = self.info
+        if self.kind == "box":
+            return "k_grad_box"
+        return f"k_grad_tma<G={i.group_lanes}, M={self.inst.m}>" if i.streaming else f"k_grad<G={i.group_lanes}, KREG={i.chunk_regs}, M={self.inst.m}>"
+
+    def config(self, world):
+        i, inst = self.info, self.inst
+        base = self.workload.split("-")[0]
+        return {"workload": f"{self.workload} (BASELINE.json configs[{cfg_index(self.workload)}]" +
+                            (", right-hand side by the paper's greedy-load rule P:264-268: binding constraints" if self.workload.endswith("-tight") else "") +
+                            f"): {inst.I} users x {inst.J} items, m={inst.m}, {self.nnz} nonzeros, projection {self.kind}({self.p0},{self.p1}), gamma={self.gamma}",
+                "regime": self.regime or ("vertex (the verbatim config is slack at lambda = 0: lambda stays 0, almost every row projects onto a vertex)"
+                                          if self.workload == base and self.lam_mode == "zero" and not self.pre[0] and self.gamma <= self.cfg.gammas[-1] else "see gamma / lambda / pre"),
+                "jacobi": self.jacobi, "adaptive_step": self.adaptive, "lambda_start": self.lam_mode,
+                "pre_stages": [f"{g}:{n}" for g, n in zip(*self.pre)],
+                "agd_rule": AGD_NOTE,
+                "parallelism": "replicas only" if world > 1 else "single GPU",
+                "l2_policy": (f"inputs larger than L2 ({self.alg_bytes / 1e9:.2f} GB streamed per step vs 126 MB L2); no flush needed"
+                              if self.alg_bytes > 4 * 126e6 else
+                              f"inputs NOT much larger than L2 ({self.alg_bytes / 1e6:.0f} MB per step vs 126 MB L2): partly L2-resident, not a bandwidth case"),
+                "group_lanes": i.group_lanes, "stages": i.stages, "tile_units": i.tile_units, "chunk_regs": i.chunk_regs, "grid_ctas": i.grid_ctas,
+                "block_threads": i.block_threads, "smem_bytes": i.smem_bytes,
+                "reduction": {1: "smem fixed-point", 2: "global RED.ADD.64", 3: "csc"}[i.reduction],
+                "short_rows": inst.short_rows, "cuda_graph": bool(self.args.graph)}
+
+    def roofline(self, m, steps, leg_name):
+        peak, peak_src = measured_peak()
+        achieved = self.alg_bytes / (m["kern_ms"] * 1e-3) / 1e9 if m["kern_ms"] > 0 else None
+        traffic, src = ncu_traffic(leg_name) if self.args.users is None else (None, None)
+        return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": (achieved / peak) if achieved else None,
+                "traffic": traffic, "traffic_source": src, "peak_source": peak_src, "kernel": self.kernel_name(), "kernel_ms": m["kern_ms"],
+                "kernel_launches_timed": m["timed"], "algorithmic_bytes_per_launch": self.alg_bytes,
+                "kernel_share_of_step": m["kern_ms"] * steps / m["ms_total"] if m["ms_total"] > 0 else None}
+
+    def close(self):
+        self.prob.destroy()
+        del self.inst
+        self.torch.cuda.empty_cache()
+
+
+def leg_name_of(args):
+    n = args.workload
+    if args.jacobi:
+        n += "+jacobi"
+    if args.adaptive:
+        n += "+adaptive"
+    if args.gamma is not None:
+        n += f"@{args.gamma:g}"
+    return n
 
 
 def main():
@@ -195,50 +379,13 @@ def main():
     world, rank, local = rep.world, rep.rank, rep.local_rank
     barrier = rep.barrier
 
-    # ---- workload: generated on the device (replicas only: every rank holds the whole job) ----
-    cfg = synth.get_config(args.workload, I=args.users)
-    t0 = time.time()
-    inst = synth.generate(cfg, device="cuda")
-    torch.cuda.synchronize()
-    t_gen = time.time() - t0
-    kind, p0, p1 = synth.proj_spec(cfg)
-    proj = {"simplex": pkg.PROJ_SIMPLEX_INEQ, "box": pkg.PROJ_BOX, "boxcut": pkg.PROJ_BOXCUT}[kind]
-    gamma = cfg.gammas[-1]
-    opts = pkg.binding.make_opts(projection=proj, p0=p0, p1=p1, borrow=True, group_lanes=args.group_lanes, grid_ctas=args.grid_ctas, stages=args.stages, tile_units=args.tile_units,
-                                  use_graph=args.graph)
-    t0 = time.time()
-    prob = pkg.Problem.create(inst.I, inst.J, inst.m, inst.row_ptr, inst.item_idx, inst.c, inst.a, inst.b, opts)
-    torch.cuda.synchronize()
-    t_create = time.time() - t0
-    info = prob.info()
-    nnz, Jm = inst.nnz, inst.J * inst.m
-    alg_bytes = nnz * (4 + 4 + 4 * inst.m) + 8 * inst.I          # idx + c + a per nonzero, row_ptr per user
-
-    lam = torch.zeros(Jm, dtype=torch.float64, device="cuda")
-    stream = torch.cuda.current_stream()
-    # ---- warm-up (untimed) ----
-    prob.solve([gamma], [max(args.warmup, 3)], lam)
-    lam.zero_()
-    barrier()
-
-    # ---- timed region: exactly K steps, CUDA events on the launching stream ----
-    prob.set_profiling(not args.graph)
-    launches0 = prob.info().launches
-    sampler = ClockSampler(local)
-    sampler.start()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    ev0.record(stream)
-    prob.solve([gamma], [args.steps], lam)                       # no final outputs requested: K gradient+update steps
-    ev1.record(stream)
-    barrier()
-    clocks = sampler.stop()
-    ms_total = ev0.elapsed_time(ev1)
-    inf = prob.info()
-    launches = inf.launches - launches0
-    kern_ms = inf.grad_kernel_ms / max(inf.grad_kernel_count, 1) if not args.graph else ms_total / args.steps
-    prob.set_profiling(False)
-    ms_total_max = rep.max_over_ranks(ms_total)
+    # ---- headline workload: generated on the device (replicas only: every rank holds the whole job) ----
+    spec = dict(workload=args.workload, gamma=args.gamma, jacobi=args.jacobi, adaptive=args.adaptive, lam=args.lam,
+                lam_scale=args.lambda_scale, pre=args.pre)
+    leg = Leg(pkg, synth, torch, spec, args)
+    inst, nnz, Jm = leg.inst, leg.nnz, leg.Jm
+    m = leg.measure(args.steps, args.warmup, barrier, local)
+    ms_total_max = rep.max_over_ranks(m["ms_total"])
     value = world * nnz * args.steps / (ms_total_max * 1e-3)
 
     # ---- end to end through the C ABI with host buffers (create + solve + readback, all timed) ----
@@ -251,22 +398,22 @@ def main():
             hbuf.copy_(t)
             host[k] = hbuf.numpy()
         torch.cuda.synchronize()
-        lam_h = np.zeros(Jm)
+        lam_h = leg.start_lambda().cpu().numpy()
         sc = pkg.Scalars()
+        gam_all, its_all = leg.pre[0] + [leg.gamma], leg.pre[1] + [args.steps]
         barrier()
         t0 = time.perf_counter()
-        p2 = pkg.Problem.create(inst.I, inst.J, inst.m, host["row_ptr"], host["item_idx"], host["c"], host["a"], host["b"],
-                                pkg.binding.make_opts(projection=proj, p0=p0, p1=p1, group_lanes=args.group_lanes, grid_ctas=args.grid_ctas, stages=args.stages, tile_units=args.tile_units,
-                                                      use_graph=args.graph))
-        p2.solve([gamma], [args.steps], lam_h, scalars=sc)
+        p2 = pkg.Problem.create(inst.I, inst.J, inst.m, host["row_ptr"], host["item_idx"], host["c"], host["a"], host["b"], leg.opts(borrow=False))
+        p2.solve(gam_all, its_all, lam_h, scalars=sc)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
         dt = rep.max_over_ranks(dt)
         h2d = sum(v.nbytes for v in host.values()) + lam_h.nbytes
         d2h = lam_h.nbytes + 5 * 8
-        e2e = {"value": world * nnz * args.steps / dt, "unit": UNIT, "h2d_bytes_per_step": h2d / args.steps,
-               "d2h_bytes_per_step": d2h / args.steps, "seconds": dt, "final_g": sc.g,
-               "what": "dualip_create(host pinned rows) + dualip_solve(K its, host lambda, host scalars) incl. final evaluation"}
+        n_e2e = int(sum(its_all))
+        e2e = {"value": world * nnz * n_e2e / dt, "unit": UNIT, "h2d_bytes_per_step": h2d / n_e2e,
+               "d2h_bytes_per_step": d2h / n_e2e, "seconds": dt, "iterations": n_e2e, "final_g": sc.g,
+               "what": "dualip_create(host pinned rows) + dualip_solve(pre stages + K its, host lambda, host scalars) incl. final evaluation"}
         p2.destroy()
         del host
 
@@ -278,42 +425,61 @@ def main():
         end = int(inst.row_ptr[nu].item())
         sample = {"row_ptr": inst.row_ptr[:nu + 1].cpu().numpy(), "item_idx": inst.item_idx[:end].cpu().numpy(),
                   "c": inst.c[:end].cpu().numpy(), "a": inst.a[:end * inst.m].cpu().numpy(), "b": inst.b.cpu().numpy()}
-        po = oracle_problem(sample, cfg, oracle, synth)
-        times = time_oracle_steps(po, gamma, 3, 0, oracle)
-        cpu = {"value": po.nnz * len(times) / float(np.sum(times)), "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": f"3 AGD iterations over the first {nu} users ({po.nnz} nnz) of the same instance; "
-                         f"oracle/dualip_oracle.c as it stands, 1 thread, fp64; {float(np.sum(times)):.1f} s of CPU work",
+        po = oracle_problem(sample, leg.cfg, oracle, synth)
+        secs, evals = time_oracle(po, leg.gamma, 2, oracle, leg.jacobi)
+        cpu = {"value": po.nnz * evals / secs, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"oracle.solve: 2 AGD iterations + the final evaluation = {evals} gradient evaluations over the first {nu} users "
+                         f"({po.nnz} nnz) of the same instance; oracle/dualip_oracle.c as it stands, 1 thread, fp64; {secs:.1f} s of CPU work",
                "host_cores_available": len(os.sched_getaffinity(0))}
+        del po, sample
 
-    peak, peak_src = measured_peak()
-    achieved = alg_bytes / (kern_ms * 1e-3) / 1e9 if kern_ms > 0 else None
-    traffic = NCU_TRAFFIC_BYTES.get(args.workload) if args.users is None else None
+    name = leg_name_of(args)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_total_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32 (fp64 duals, fp64 shift, 64-bit fixed-point reduction)", "data": "synthetic",
+        "config": leg.config(world),
+        "iters_per_s": world * args.steps / (ms_total_max * 1e-3),
+        "solve_time_s": ms_total_max * 1e-3, "gen_time_s": leg.t_gen, "create_time_s": leg.t_create,
+        "gpu_launches": m["launches"],
+        "roofline": leg.roofline(m, args.steps, name),
+        "end_state": m["state"],
+        "e2e": e2e, "cpu_baseline": cpu, "clocks": m["clocks"],
+    }
+    leg.close()
+
+    # ---- extra legs (N = 1): the other large configs and the fractional regime, K steps each ----
+    want = []
+    if args.legs == "default":
+        if world == 1 and args.workload == "cfg3" and args.users is None and args.gamma is None and not args.jacobi and not args.pre \
+                and not args.adaptive and args.lam == "zero":
+            want = list(LEGS)
+    elif args.legs != "none":
+        want = [t.strip() for t in args.legs.split(",") if t.strip()]
+    legs = {}
+    total_mem = torch.cuda.get_device_properties(local).total_memory
+    for nm in want:
+        spec = LEGS[nm]
+        cfg = synth.get_config(spec["workload"], I=args.users)
+        mean_deg = {"const": lambda d: d[1], "uniform": lambda d: (d[1] + d[2]) / 2, "poisson": lambda d: d[1]}[cfg.deg[0]](cfg.deg)
+        need = cfg.I * mean_deg * (8 + 4 * cfg.m) * 1.35
+        if need > total_mem:
+            legs[nm] = {"skipped": f"needs about {need / 1e9:.0f} GB of device memory"}
+            continue
+        k = args.leg_steps if args.leg_steps > 0 else min(args.steps, 50)
+        try:
+            lg = Leg(pkg, synth, torch, spec, args)
+            mm = lg.measure(k, args.warmup, barrier, local)
+            legs[nm] = {"value": lg.nnz * k / (mm["ms_total"] * 1e-3), "unit": UNIT, "steps": k, "ms_per_step": mm["ms_total"] / k,
+                        "config": lg.config(world), "roofline": lg.roofline(mm, k, nm), "end_state": mm["state"], "clocks": mm["clocks"],
+                        "gpu_launches": mm["launches"]}
+            lg.close()
+        except Exception as e:                                       # a leg must never take the headline line down with it
+            legs[nm] = {"error": f"{type(e).__name__}: {e}"}
+    if legs:
+        line["legs"] = legs
     if rank == 0:
-        line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-            "ms_per_step": ms_total_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32 (fp64 duals, fp64 shift, 64-bit fixed-point reduction)", "data": "synthetic",
-            "config": {"workload": f"{args.workload} (BASELINE.json configs[{int(args.workload[3]) - 1}]): {inst.I} users x {inst.J} items, m={inst.m}, "
-                                   f"{nnz} nonzeros, projection {kind}({p0},{p1}), gamma={gamma}",
-                       "parallelism": "replicas only" if world > 1 else "single GPU", "l2_policy": (f"inputs larger than L2 ({alg_bytes / 1e9:.2f} GB streamed per step vs 126 MB L2); no flush needed"
-                                     if alg_bytes > 4 * 126e6 else
-                                     f"inputs NOT much larger than L2 ({alg_bytes / 1e6:.0f} MB per step vs 126 MB L2): partly L2-resident, not a bandwidth case"),
-                       "group_lanes": info.group_lanes, "stages": info.stages, "tile_units": info.tile_units, "chunk_regs": info.chunk_regs, "grid_ctas": info.grid_ctas,
-                       "block_threads": info.block_threads, "smem_bytes": info.smem_bytes,
-                       "reduction": {1: "smem fixed-point", 2: "global RED.ADD.64", 3: "csc"}[info.reduction],
-                       "short_rows": inst.short_rows, "cuda_graph": bool(args.graph)},
-            "iters_per_s": world * args.steps / (ms_total_max * 1e-3),
-            "solve_time_s": ms_total_max * 1e-3, "gen_time_s": t_gen, "create_time_s": t_create,
-            "gpu_launches": int(launches),
-            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": (achieved / peak) if achieved else None, "traffic": traffic, "peak_source": peak_src,
-                         "kernel": "k_grad", "kernel_ms": kern_ms, "kernel_launches_timed": int(inf.grad_kernel_count),
-                         "algorithmic_bytes_per_launch": alg_bytes,
-                         "kernel_share_of_step": kern_ms * args.steps / ms_total if ms_total > 0 else None},
-            "e2e": e2e, "cpu_baseline": cpu, "clocks": clocks,
-        }
         print(json.dumps(line), flush=True)
-    prob.destroy()
     rep.close()
 
 

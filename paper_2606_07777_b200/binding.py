@@ -129,7 +129,10 @@ def _ptr(t, dtype=None, keep=None):
 
 
 def make_opts(projection=PROJ_SIMPLEX_INEQ, p0=1.0, p1=0.0, reduction=RED_AUTO, borrow=False, validate=True,
-              momentum=True, group_lanes=0, grid_ctas=0, use_graph=False, direct_kernel=False, jacobi=False, stages=0, tile_units=0) -> Opts:
+              momentum=True, group_lanes=0, grid_ctas=0, use_graph=False, direct_kernel=False, jacobi=False, stages=0, tile_units=0,
+              adaptive=False) -> Opts:
+    if adaptive:
+        raise ValueError('adaptive step: not in this build yet')
     o = Opts()
     load_library().dualip_opts_default(ctypes.byref(o))
     o.projection, o.p0, o.p1, o.reduction = projection, p0, p1, reduction

@@ -161,7 +161,7 @@ bool plan_tma(dualip* h, Plan& pl) {
     // pair stays under 64 KB (otherwise the exact path reads the fp64 lambda through L2: it runs once per row at
     // most).  The fixed-point item accumulators (8 B per dual) are privatised per CTA only for small J*m, where the
     // same few addresses would otherwise serialise in L2; beyond that RED.ADD.64 goes straight to L2.
-    const size_t fixed = 128 + 128;
+    const size_t fixed = kTmaHeaderBytes + 128;
     if (fixed + 4 * JM + 32 * 1024 > kSmemBudget) return false;
     const bool lo = 8 * JM <= (size_t)DUALIP_LO_SMEM_KB * 1024;
     const size_t lam_bytes = (lo ? 8 : 4) * JM;
@@ -194,7 +194,7 @@ bool plan_tma(dualip* h, Plan& pl) {
     size_t sb = (size_t)pl.cap_nz * (8 + 4 * m) + (size_t)pl.cap_rows * 8 + 32;
     pl.stage_bytes = (int)((sb + 127) & ~(size_t)127);
     pl.ntiles = (units + TN - 1) / TN;
-    size_t off = 128 + lam_bytes + (acc ? 8 : 0) * JM;
+    size_t off = kTmaHeaderBytes + lam_bytes + (acc ? 8 : 0) * JM;
     off = (off + 127) & ~(size_t)127;
     pl.smem = off + (size_t)pl.stage_bytes * stages;
     return pl.smem <= kSmemBudget;

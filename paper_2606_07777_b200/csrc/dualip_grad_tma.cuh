@@ -36,6 +36,7 @@ constexpr int kTmaConsumerWarps = DUALIP_NWC;  // consumer warps of the streamin
 
 constexpr int kRowCost = 8;            // each row costs this many "nonzero units" when cutting tiles
 constexpr int kTmaStagesMax = 4;
+constexpr int kTmaHeaderBytes = 128 + 256 * kTmaConsumerWarps;   // mbarriers + words + per-warp candidate lists (multiple of 128)
 
 struct TileEntry {                     // 32 bytes, one per tile (+1 sentinel)
     long long row0;                    // first row of the tile
@@ -165,16 +166,14 @@ __device__ __forceinline__ double exact_t(const StageView& v, const ConsumerCtx&
     return t;
 }
 
-// One pass of the fp32 filter for one row: this lane's 4 nonzeros at q (M != 2: q..q+3; M = 2: the pairs (q, q+1) and
+// The filter's view of 4 nonzeros of one row: this lane's slots at q (M != 2: q..q+3; M = 2: the pairs (q, q+1) and
 // (q+2G, q+2G+1), so that the 64-bit idx / c loads and the 128-bit a loads of a group are each one contiguous,
 // conflict-free run -- four consecutive nonzeros per lane would put the a loads 32 bytes apart, a two-way bank conflict).
-// Updates the running two largest w' (m1 >= m2) and the position of the largest.  The four values are first reduced
-// among themselves (depth 2), then merged into the running pair, so the dependent chain per pass is ~4 min/max deep
-// instead of 8.  Equal maxima give m2 = m1 (no vertex).
+// w[e] = -(c + a . RN_f32(lambda)) in fp32 (one FFMA per family), -inf for slots outside [beg, beg+len); pe[e] = the
+// slot's position in the stage.
 template <int G, int M>
-__device__ __forceinline__ void filter_pass(const StageView& v, const float* __restrict__ s_hi32, int mm, int q, int beg, int len,
-                                            float& m1, float& m2, int& pb) {
-    float w[4]; int pe[4];
+__device__ __forceinline__ void filter_load(const StageView& v, const float* __restrict__ s_hi32, int mm, int q, int beg, int len,
+                                            float (&w)[4], int (&pe)[4]) {
     if (M == 2) {
         const int q2 = q + 2 * G;
         const int2 jA = *reinterpret_cast<const int2*>(v.idx + q), jB = *reinterpret_cast<const int2*>(v.idx + q2);
@@ -212,6 +211,16 @@ __device__ __forceinline__ void filter_pass(const StageView& v, const float* __r
     }
 #pragma unroll
     for (int e = 0; e < 4; ++e) w[e] = (unsigned)(pe[e] - beg) < (unsigned)len ? w[e] : -CUDART_INF_F;
+}
+
+// One pass of the fp32 filter for one row: updates the running two largest w' (m1 >= m2) and the position of the largest.
+// The four values are first reduced among themselves (depth 2), then merged into the running pair, so the dependent
+// chain per pass is ~4 min/max deep instead of 8.  Equal maxima give m2 = m1 (no vertex).
+template <int G, int M>
+__device__ __forceinline__ void filter_pass(const StageView& v, const float* __restrict__ s_hi32, int mm, int q, int beg, int len,
+                                            float& m1, float& m2, int& pb) {
+    float w[4]; int pe[4];
+    filter_load<G, M>(v, s_hi32, mm, q, beg, len, w, pe);
     const float hi01 = fmaxf(w[0], w[1]), lo01 = fminf(w[0], w[1]), hi23 = fmaxf(w[2], w[3]), lo23 = fminf(w[2], w[3]);
     const int p01 = sel_gt(w[1], w[0], pe[1], pe[0]), p23 = sel_gt(w[3], w[2], pe[3], pe[2]);
     const float top = fmaxf(hi01, hi23);
@@ -474,14 +483,16 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
     constexpr int NT = 32 * (NWC + 1);
     const int mm = M > 0 ? M : p.m;
     const int JM = p.J * mm;
-    // layout: [full[4], empty[4] mbarriers: 64 B][max|lambda| word: 64 B][lam_hi JM*4][lam_lo JM*4 (optional)][acc 2*JM*4 (ACC_SMEM)][stages]
+    // layout: [full[4], empty[4] mbarriers: 64 B][max|lambda| word: 64 B][candidate lists: 256 B per consumer warp][lam_hi JM*4]
+    //         [lam_lo JM*4 (optional)][acc 2*JM*4 (ACC_SMEM)][stages]
     unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_tma);
     unsigned* s_words = reinterpret_cast<unsigned*>(smem_tma + 64);       // [0] = max |lambda_hi| as float bits
-    float* s_hi32 = reinterpret_cast<float*>(smem_tma + 128);
+    int* cand_list = reinterpret_cast<int*>(smem_tma + 128);              // 64 positions per consumer warp (candidate path B)
+    float* s_hi32 = reinterpret_cast<float*>(smem_tma + kTmaHeaderBytes);
     float* s_lo32 = s_hi32 + JM;                                           // only when tp.lam_lo_smem
     unsigned* a_lo = reinterpret_cast<unsigned*>(s_hi32 + (tp.lam_lo_smem ? 2 : 1) * JM);
     unsigned* a_hi = a_lo + JM;
-    size_t off = 128 + (size_t)JM * 4 * ((tp.lam_lo_smem ? 2 : 1) + (ACC_SMEM ? 2 : 0));
+    size_t off = kTmaHeaderBytes + (size_t)JM * 4 * ((tp.lam_lo_smem ? 2 : 1) + (ACC_SMEM ? 2 : 0));
     off = (off + 127) & ~(size_t)127;
     unsigned char* stage0 = smem_tma + off;
 
@@ -708,51 +719,102 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                         }
                     }
                     // ---- candidate path: rows that are neither a vertex nor dead.  Only nonzeros with w > w_max - z gamma
-                    // can be in the support (theta >= v_max - z for both simplex forms), and the filter already knows
-                    // each lane's two largest w'.  If no lane of the group has its SECOND value above the candidate
-                    // threshold, every lane holds at most one candidate, at a known position: those few nonzeros are
-                    // redone in fp64 and projected in registers by the group (same arithmetic as slow_row), and the
-                    // rest of the row is zero.  Typical fractional rows have 2-3 candidates, so this takes almost all
-                    // of them; rows with two candidates in one lane, or more candidates than lanes, go to slow_row.
+                    // can be in the support (theta >= v_max - z for both simplex forms): the CANDIDATES, typically 2-4 of
+                    // a row.  They are brought to one per lane (two per lane when a row has more candidates than its group
+                    // has lanes), redone in fp64 and projected in registers by the group; the rest of the row is zero.
+                    //   (A) the filter already knows each lane's two largest w': if no lane's SECOND value passes the
+                    //       candidate threshold, every lane holds at most one candidate, at a known position;
+                    //   (B) otherwise the group scans the staged row once more and compacts the candidates' positions
+                    //       through a per-warp list in shared memory (ballot + prefix popc), up to 2G of them;
+                    //   rows with more than 2G candidates (gamma of the order of the spread of w) go to slow_rows_all.
                     bool handled = false;
                     const bool want = active && !fast;
                     if (__any_sync(kFull, want)) {
                         const unsigned gmask = G == 32 ? kFull : (((1u << G) - 1u) << (lane & ~(G - 1)));
+                        const unsigned lt_mask = (1u << lane) - 1u;
                         const float thr_own = m1 - gz_sat - 2.0f * tol;
+                        int* const clist = cand_list + (warp - 1) * 64 + grp * (2 * G);
 #pragma unroll
                         for (int r = 0; r < RPG; ++r) {
                             const int src = (lane & ~(G - 1)) + r * HG;
                             const bool rw = __shfl_sync(kFull, (int)want, src) != 0;
                             const float thr = __shfl_sync(kFull, thr_own, src);
                             const unsigned okb = __ballot_sync(kFull, !(rm2[r] > thr));
-                            const bool row_ok = rw && (okb & gmask) == gmask;
+                            const bool rowA = rw && (okb & gmask) == gmask;
+                            const bool needB = rw && !rowA;
+                            bool row_ok = rowA;
+                            int cp0 = (rowA && rm1[r] > thr) ? rpos[r] : -1, cp1 = -1;
+                            if (__any_sync(kFull, needB)) {
+                                constexpr int LS = M == 2 ? 2 : 4;
+                                int qq = (rbeg[r] & ~3) + LS * gl;
+                                const int qe = rbeg[r] + rlen[r];
+                                int ncand = 0;                                   // candidates of this group's row so far
+                                while (__any_sync(kFull, needB && qq < qe)) {
+                                    float w[4]; int pe[4];
+                                    if (needB && qq < qe) filter_load<G, M>(v, s_hi32, mm, qq, rbeg[r], rlen[r], w, pe);
+                                    else {
+#pragma unroll
+                                        for (int e = 0; e < 4; ++e) { w[e] = -CUDART_INF_F; pe[e] = 0; }
+                                    }
+#pragma unroll
+                                    for (int e = 0; e < 4; ++e) {
+                                        const bool isc = w[e] > thr;
+                                        const unsigned bal = __ballot_sync(kFull, isc) & gmask;
+                                        const int k = ncand + __popc(bal & lt_mask);
+                                        if (isc && k < 2 * G) clist[k] = pe[e];
+                                        ncand += __popc(bal);
+                                    }
+                                    qq += 4 * G;
+                                }
+                                __syncwarp();
+                                const bool rowB = needB && ncand <= 2 * G;
+                                if (rowB) { cp0 = gl < ncand ? clist[gl] : -1; cp1 = gl + G < ncand ? clist[gl + G] : -1; }
+                                row_ok = rowA || rowB;
+                                __syncwarp();                                    // the list is reused by the group's next row
+                            }
                             if (!__any_sync(kFull, row_ok)) continue;
-                            const bool cand = row_ok && rm1[r] > thr;
+                            const bool two = __any_sync(kFull, cp1 >= 0);        // warp-uniform: a second candidate per lane is rare
                             int j = 0; float cc = 0.0f; float aa[MA];
-                            double wq = -CUDART_INF;
-                            if (cand) wq = -exact_t<M>(v, cx, mm, rpos[r], j, cc, aa);
-                            const float m32 = group_max<G>((float)wq);          // the row maximum is always a candidate
+                            double wq0 = -CUDART_INF, wq1 = -CUDART_INF;
+                            if (cp0 >= 0) wq0 = -exact_t<M>(v, cx, mm, cp0, j, cc, aa);
+                            if (two && cp1 >= 0) wq1 = -exact_t<M>(v, cx, mm, cp1, j, cc, aa);
+                            const float m32 = group_max<G>(fmaxf((float)wq0, (float)wq1));   // the row maximum is always a candidate
                             const bool alive = row_ok && (!ineq || m32 > 0.0f);
                             const float mv = m32 * p.inv_gamma_f;
-                            const float u = cand ? (float)(wq - (double)m32) * p.inv_gamma_f : -CUDART_INF_F;
+                            const float u0 = cp0 >= 0 ? (float)(wq0 - (double)m32) * p.inv_gamma_f : -CUDART_INF_F;
+                            const float u1 = (two && cp1 >= 0) ? (float)(wq1 - (double)m32) * p.inv_gamma_f : -CUDART_INF_F;
                             float theta = -z - (1.2e-7f * fabsf(mv) + 1e-6f);
                             int n_prev = -1;
                             for (;;) {                                           // Michelot on the candidates
-                                const bool in = alive && u > theta;
-                                const float sg = group_sum<G>(in ? u : 0.0f);
-                                const int n = __popc(__ballot_sync(kFull, in) & gmask);
+                                const bool in0 = alive && u0 > theta, in1 = alive && u1 > theta;
+                                const float sg = group_sum<G>((in0 ? u0 : 0.0f) + (in1 ? u1 : 0.0f));
+                                int n = __popc(__ballot_sync(kFull, in0) & gmask);
+                                if (two) n += __popc(__ballot_sync(kFull, in1) & gmask);
                                 const bool stop = n == n_prev || n == 0;
                                 if (!stop) { theta = fmaxf((sg - z) / (float)n, theta); n_prev = n; }
                                 if (__all_sync(kFull, stop)) break;
                             }
                             const float tau = ineq ? fmaxf(theta, -mv) : theta;
-                            const float xq = (cand && alive) ? fmaxf(u - tau, 0.0f) : 0.0f;
-                            if (xq > 0.0f) push<M, ACC_SMEM>(p, cx, fp, mm, j, cc, aa, xq);
+                            const float xq0 = alive ? fmaxf(u0 - tau, 0.0f) : 0.0f;
+                            const float xq1 = alive ? fmaxf(u1 - tau, 0.0f) : 0.0f;
+                            if (xq0 > 0.0f) {
+                                j = v.idx[cp0]; cc = v.c[cp0];
+#pragma unroll
+                                for (int f = 0; f < MA; ++f) aa[f] = f < mm ? v.a[cp0 * mm + f] : 0.0f;
+                                push<M, ACC_SMEM>(p, cx, fp, mm, j, cc, aa, xq0);
+                            }
+                            if (two && xq1 > 0.0f) {
+                                j = v.idx[cp1]; cc = v.c[cp1];
+#pragma unroll
+                                for (int f = 0; f < MA; ++f) aa[f] = f < mm ? v.a[cp1 * mm + f] : 0.0f;
+                                push<M, ACC_SMEM>(p, cx, fp, mm, j, cc, aa, xq1);
+                            }
                             if (xout<WX>(p)) {
                                 const long long nzb = v.meta->nzb;
                                 if (row_ok) for (int e = gl; e < rlen[r]; e += G) xout<WX>(p)[nzb + rbeg[r] + e] = 0.0f;
                                 __syncwarp();
-                                if (cand) xout<WX>(p)[nzb + rpos[r]] = xq;
+                                if (cp0 >= 0) xout<WX>(p)[nzb + cp0] = xq0;
+                                if (cp1 >= 0) xout<WX>(p)[nzb + cp1] = xq1;
                             }
                             if (lane == src && row_ok) handled = true;
                         }

@@ -90,6 +90,36 @@ def test_group_width_does_not_change_results(G):
     assert_grad_parity(po, pg, lam, 1e-3, tag=f"G={G}")
 
 
+@pytest.mark.parametrize("G", [1, 2, 4, 8, 16, 32])
+@pytest.mark.parametrize("m", [1, 2])
+def test_clustered_near_ties_take_the_compacted_candidate_path(G, m):
+    """Rows whose k largest values are near-tied AND adjacent in the row (so several candidates sit in one lane's four
+    slots), k = 1..40: fewer candidates than lanes (one per lane after compaction), up to 2G (two per lane) and beyond
+    (the row falls through to the slow path).  Every row is fractional at gamma = 1e-2; at 1e-4 most are vertices."""
+    rng = np.random.default_rng(100 * G + m)
+    I, J = 1500, 400
+    rows, idx, cs = [0], [], []
+    for i in range(I):
+        d = int(rng.integers(1, 120))
+        it = np.sort(rng.choice(J, size=d, replace=False))
+        c = -0.5 * rng.random(d)
+        k = min(d, int(rng.integers(1, 41)))
+        off = int(rng.integers(0, d - k + 1))
+        c[off:off + k] = -1.0 - 2e-3 * rng.random(k)          # the cluster: within 2e-3 of each other, well above the rest
+        idx.extend(it.tolist()); cs.extend(c.tolist()); rows.append(len(idx))
+    nnz = len(idx)
+    d_ = dict(I=I, J=J, m=m, row_ptr=np.array(rows, dtype=np.int64), item_idx=np.array(idx, dtype=np.int32),
+              c=np.array(cs, dtype=np.float32), a=(0.5 + rng.random(nnz * m)).astype(np.float32),
+              b=np.full(J * m, 0.5, dtype=np.float32))
+    for kind, p0, p1 in (("simplex", 1.0, 0.0), ("simplex_eq", 1.0, 0.0), ("boxcut", 1.0, 1.0)):
+        po, pg = both(d_, kind, p0, p1, group_lanes=G)
+        assert pg.info().streaming == 1 and pg.info().group_lanes == G
+        for gamma in (1e-2, 1e-3, 1e-4):
+            assert_grad_parity(po, pg, np.zeros(J * m), gamma, tag=f"ties G={G} m={m} {kind} gamma={gamma}")
+            assert_grad_parity(po, pg, 1e-4 * rng.random(J * m), gamma, tag=f"ties G={G} m={m} {kind} gamma={gamma} lam")
+        pg.destroy()
+
+
 def test_cfg1_verbatim_trajectory():
     """BASELINE config 1 as stated: 200 AGD iterations from lambda = 0 at gamma = 1e-2 (slack: lambda stays 0)."""
     inst = synth.generate("cfg1")

@@ -48,14 +48,15 @@ def _load():
         for f in (lib.dualip_oracle_project_simplex, lib.dualip_oracle_project_simplex_eq,
                   lib.dualip_oracle_project_box, lib.dualip_oracle_project_boxcut):
             f.restype = None
-        lib.dualip_oracle_grad.argtypes = [i64, i32, i32, vp, vp, vp, vp, vp, vp, d, ctypes.c_int, d, d, vp, vp, vp]
+        lib.dualip_oracle_grad.argtypes = [i64, i32, i32, vp, vp, vp, vp, vp, vp, d, ctypes.c_int, d, d, vp, i32, d, vp, vp, vp]
         lib.dualip_oracle_grad.restype = ctypes.c_int
-        lib.dualip_oracle_lipschitz.argtypes = [i64, i32, i32, vp, vp, vp]
+        lib.dualip_oracle_lipschitz.argtypes = [i64, i32, i32, vp, vp, vp, i32]
         lib.dualip_oracle_lipschitz.restype = d
         lib.dualip_oracle_jacobi_scaling.argtypes = [i64, i32, i32, vp, vp, vp, vp]
         lib.dualip_oracle_jacobi_scaling.restype = None
         lib.dualip_oracle_solve.argtypes = [i64, i32, i32, vp, vp, vp, vp, vp, ctypes.c_int, d, d,
-                                            vp, i32, vp, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+                                            vp, i32, vp, i32, i32, vp, i32, d, d, i32, d,
+                                            vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         lib.dualip_oracle_solve.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -110,6 +111,12 @@ class Problem:
     proj_kind: int = PROJ_SIMPLEX_INEQ
     p0: float = 1.0
     p1: float = 0.0
+    count_M: float | None = None      # global-count row  sum_{(i,j)} x_ij <= count_M  (reading R21); None = absent
+
+    @property
+    def rows(self) -> int:
+        """coupling rows = duals: J*m, plus one for the global-count row"""
+        return self.J * self.m + (1 if self.count_M is not None else 0)
 
     def __post_init__(self):
         self.row_ptr = np.ascontiguousarray(self.row_ptr, dtype=np.int64)
@@ -136,25 +143,39 @@ class GradResult:
     r_2: float
     grad: np.ndarray
     x: np.ndarray | None
+    gap: float = 0.0
 
 
-def grad(p: Problem, lam, gamma: float, want_x: bool = True) -> GradResult:
-    """(g, grad g, x*) at lambda -- Eq. 2-4."""
+def _eq_mask(p: Problem, is_eq):
+    if is_eq is None:
+        return None
+    eq = np.ascontiguousarray(np.asarray(is_eq, dtype=np.uint8)).reshape(-1)
+    assert eq.size == p.rows
+    return eq
+
+
+def grad(p: Problem, lam, gamma: float, want_x: bool = True, is_eq=None) -> GradResult:
+    """(g, grad g, x*) at lambda -- Eq. 2-4.  lambda / grad have p.rows entries (the last one belongs to the
+    global-count row when the problem has one); is_eq: uint8 mask of equality rows (residuals count |grad| there, R19)."""
     lam = _f64(lam).reshape(-1)
-    assert lam.size == p.J * p.m
-    g = np.empty(p.J * p.m, dtype=np.float64)
-    sc = np.empty(5, dtype=np.float64)
+    assert lam.size == p.rows
+    g = np.empty(p.rows, dtype=np.float64)
+    sc = np.empty(6, dtype=np.float64)
     x = np.empty(p.nnz, dtype=np.float64) if want_x else None
+    eq = _eq_mask(p, is_eq)
     rc = _load().dualip_oracle_grad(p.I, p.J, p.m, _ptr(p.row_ptr), _ptr(p.item_idx), _ptr(p.c), _ptr(p.a),
-                                    _ptr(p.b), _ptr(lam), gamma, p.proj_kind, p.p0, p.p1, _ptr(g), _ptr(sc), _ptr(x))
+                                    _ptr(p.b), _ptr(lam), gamma, p.proj_kind, p.p0, p.p1, _ptr(eq),
+                                    0 if p.count_M is None else 1, 0.0 if p.count_M is None else float(p.count_M),
+                                    _ptr(g), _ptr(sc), _ptr(x))
     if rc != 0:
         raise MemoryError("oracle grad failed")
-    return GradResult(sc[0], sc[1], sc[2], sc[3], sc[4], g, x)
+    return GradResult(sc[0], sc[1], sc[2], sc[3], sc[4], g, x, sc[5])
 
 
 def lipschitz(p: Problem) -> float:
-    """L = max_j sum_k sum_i (a^k_ij)^2 (reading R2)."""
-    return float(_load().dualip_oracle_lipschitz(p.I, p.J, p.m, _ptr(p.row_ptr), _ptr(p.item_idx), _ptr(p.a)))
+    """L = max_j sum_k sum_i (a^k_ij)^2 (reading R2), + nnz with the global-count row (R21)."""
+    return float(_load().dualip_oracle_lipschitz(p.I, p.J, p.m, _ptr(p.row_ptr), _ptr(p.item_idx), _ptr(p.a),
+                                                 0 if p.count_M is None else 1))
 
 
 def jacobi_scaling(p: Problem) -> np.ndarray:
@@ -175,32 +196,36 @@ class SolveResult:
     trace_grad: np.ndarray | None
     trace_lambda: np.ndarray | None
     stage_x: np.ndarray | None
+    trace_eta: np.ndarray | None = None
 
 
 def solve(p: Problem, gammas, iters, lam0=None, momentum: bool = True, want_x: bool = True,
           trace_grad: bool = False, trace_lambda: bool = False, stage_x: bool = False, jacobi: bool = False,
-          is_eq=None) -> SolveResult:
+          is_eq=None, adaptive: bool = False, eta_min: float = 1e-5, eta_max: float = 1e-1) -> SolveResult:
     """gamma-continuation + projected Nesterov ascent (readings R1-R4); jacobi: on the row-scaled
     system A' = D A, b' = D b, results reported in the original units (R18); is_eq: uint8 mask
-    over the J*m coupling rows, nonzero = equality row whose dual is not projected (R19)."""
+    over the coupling rows, nonzero = equality row whose dual is not projected (R19); adaptive: the range-clipped
+    secant step (R20) with the range [eta_min, eta_max * gamma_s / gamma_1]."""
     gammas = _f64(gammas).reshape(-1)
     iters = np.ascontiguousarray(np.asarray(iters, dtype=np.int32)).reshape(-1)
     assert gammas.size == iters.size
-    Jm, T = p.J * p.m, int(iters.sum())
-    lam = np.zeros(Jm) if lam0 is None else _f64(lam0).reshape(-1).copy()
+    R, T = p.rows, int(iters.sum())
+    lam = np.zeros(R) if lam0 is None else _f64(lam0).reshape(-1).copy()
+    assert lam.size == R
     x = np.empty(p.nnz) if want_x else None
-    sc, fg = np.empty(5), np.empty(Jm)
-    tg, ti, t2 = np.empty(T), np.empty(T), np.empty(T)
-    tgrad = np.empty((T, Jm)) if trace_grad else None
-    tlam = np.empty((T, Jm)) if trace_lambda else None
+    sc, fg = np.empty(6), np.empty(R)
+    tg, ti, t2, te = np.empty(T), np.empty(T), np.empty(T), np.empty(T)
+    tgrad = np.empty((T, R)) if trace_grad else None
+    tlam = np.empty((T, R)) if trace_lambda else None
     sx = np.empty((gammas.size, p.nnz)) if stage_x else None
-    eq = None if is_eq is None else np.ascontiguousarray(np.asarray(is_eq, dtype=np.uint8)).reshape(-1)
-    assert eq is None or eq.size == Jm
+    eq = _eq_mask(p, is_eq)
     rc = _load().dualip_oracle_solve(p.I, p.J, p.m, _ptr(p.row_ptr), _ptr(p.item_idx), _ptr(p.c), _ptr(p.a),
                                      _ptr(p.b), p.proj_kind, p.p0, p.p1, _ptr(gammas), gammas.size, _ptr(iters),
-                                     1 if momentum else 0, 1 if jacobi else 0, _ptr(eq), _ptr(lam), _ptr(x), _ptr(sc), _ptr(fg),
-                                     _ptr(tg), _ptr(ti), _ptr(t2), _ptr(tgrad), _ptr(tlam), _ptr(sx))
+                                     1 if momentum else 0, 1 if jacobi else 0, _ptr(eq), 1 if adaptive else 0, float(eta_min),
+                                     float(eta_max), 0 if p.count_M is None else 1, 0.0 if p.count_M is None else float(p.count_M),
+                                     _ptr(lam), _ptr(x), _ptr(sc), _ptr(fg),
+                                     _ptr(tg), _ptr(ti), _ptr(t2), _ptr(tgrad), _ptr(tlam), _ptr(te), _ptr(sx))
     if rc != 0:
         raise MemoryError("oracle solve failed")
-    final = GradResult(sc[0], sc[1], sc[2], sc[3], sc[4], fg, x)
-    return SolveResult(lam, x, final, tg, ti, t2, tgrad, tlam, sx)
+    final = GradResult(sc[0], sc[1], sc[2], sc[3], sc[4], fg, x, sc[5])
+    return SolveResult(lam, x, final, tg, ti, t2, tgrad, tlam, sx, te)

@@ -19,6 +19,7 @@
  *   - per-source simple constraint: unit simplex sum<=1,x>=0, "or a box variant"   P:83, P:130 (Table 1)
  *   - simplex projection by Duchi et al.: sort, prefix sums, rho, theta, clamp
  *   - AGD on lambda>=0, fixed step from A and gamma, gamma continuation, warm start P:60
+ *   - range-clipped adaptive step, equality rows, global-count row: oracle-defined readings
  *
  * Pins (tests/test_oracle_*.py, all `-m "not gpu"`):
  *   projections: hand-worked closed forms (tests/golden/projection_cases.txt), a second independent
@@ -29,6 +30,11 @@
  *   AGD loop: **parity unpinned against the paper** (the update rule is never printed, P:123 gives
  *     words only; reading R1/R2).  Pinned internally: I=J=1 closed-form optimum, the
  *     lambda==0 fixed point, monotone ascent of the beta==0 variant, O(1/T^2) bound on KKT instances.
+ *   adaptive step (R20): **parity unpinned against the paper** (no formula printed).  Pinned internally: a clip range that
+ *     is one point reproduces the fixed step bit for bit; on I=J=1 (grad g linear) the secant step IS gamma/L; every eta_t lies
+ *     in the range, whose maximum scales with gamma_s/gamma_1; the KKT optimum of the tiny instances is reached.
+ *   global-count row (R21): an I=1 closed form, brute-force KKT with the extra row, and J=1 instances, where the count row
+ *     is literally a second coupling family with a = 1 (same gradients, same L, same trajectory) -- tests/test_oracle_extensions.py.
  *
  * Layout at this interface (same as the product's C ABI, stated independently):
  *   row_ptr[I+1] int64, item_idx[nnz] int32, c[nnz] fp32, a[nnz*m] fp32 (a[p*m+k]),
@@ -121,12 +127,19 @@ static void project(int kind, double p0, double p1, const double* v, int64_t n, 
 
 /* One evaluation of Eq. 2-4 at lambda (any sign) and gamma > 0.
  * proj params: simplex kinds p0 = z; box p0 = lo, p1 = hi; boxcut p0 = ub, p1 = z.
- * scalars_out[5] = { g, obj = c'x, reg = (gamma/2)|x|^2, r_inf = max(0, max grad), r_2 = |max(grad,0)|_2 }.
+ * is_eq (may be NULL = every coupling row is an inequality, Eq. 1): is_eq[q] != 0 marks row q as an EQUALITY
+ *   (A x)_q = b_q, whose violation is |grad_q| instead of max(grad_q, 0) (reading R19).
+ * count_coef != 0 adds the GLOBAL-COUNT row  count_coef * sum_{(i,j) in E} x_ij <= count_rhs  as coupling row number
+ *   Jm ("adding a global-count constraint sum x_ij <= M only augments A and lambda"; reading R21):
+ *   lambda, grad_out (and is_eq) then have Jm + 1 entries, the last one being that row's dual / gradient.  The row has
+ *   the coefficient count_coef on EVERY eligible pair (1 for the plain constraint; 1/sqrt(nnz) once row-normalised).
+ * scalars_out[6] = { g, obj = c'x, reg = (gamma/2)|x|^2, r_inf = max violation, r_2 = |violations|_2,
+ *                    gap = (obj + reg) - g = -lambda'grad  (Table 4's primal-dual gap before the absolute value) }.
  * x_out (nnz doubles, input order) may be NULL.  Returns 0, or -1 on allocation failure. */
 static int grad_f64(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr, const int32_t* item_idx,
                     const float* c, const double* a, const double* b, const double* lambda, double gamma,
-                    int proj_kind, double p0, double p1, double* grad_out, double* scalars_out,
-                    double* x_out) {
+                    int proj_kind, double p0, double p1, const uint8_t* is_eq, double count_coef, double count_rhs,
+                    double* grad_out, double* scalars_out, double* x_out) {
     int64_t max_len = 0;
     for (int64_t i = 0; i < I; ++i)
         if (row_ptr[i + 1] - row_ptr[i] > max_len) max_len = row_ptr[i + 1] - row_ptr[i];
@@ -134,14 +147,17 @@ static int grad_f64(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr, con
     double* x = (double*)malloc((size_t)(max_len + 1) * sizeof(double));
     if (!v || !x) { free(v); free(x); return -1; }
     int64_t Jm = (int64_t)J * m;
-    for (int64_t q = 0; q < Jm; ++q) grad_out[q] = 0.0;          /* s = A x, accumulated in user order */
-    double obj = 0.0, sq = 0.0;
+    int64_t nrow = Jm + (count_coef != 0.0 ? 1 : 0);            /* coupling rows = duals */
+    double mu = count_coef != 0.0 ? lambda[Jm] : 0.0;            /* dual of the global-count row */
+    for (int64_t q = 0; q < nrow; ++q) grad_out[q] = 0.0;        /* s = A x, accumulated in user order */
+    double obj = 0.0, sq = 0.0, sumx = 0.0;
     for (int64_t i = 0; i < I; ++i) {
         int64_t beg = row_ptr[i], n = row_ptr[i + 1] - beg;
         for (int64_t p = 0; p < n; ++p) {
             int64_t j = item_idx[beg + p];
-            double al = 0.0;                                     /* (A' lambda)_p = sum_k a^k_p lambda_{j,k} */
+            double al = 0.0;                                     /* (A' lambda)_p = sum_k a^k_p lambda_{j,k} (+ count row) */
             for (int32_t k = 0; k < m; ++k) al += a[(beg + p) * m + k] * lambda[j * m + k];
+            al += count_coef * mu;
             v[p] = -((double)c[beg + p] + al) / gamma;           /* Eq. 3 argument */
         }
         project(proj_kind, p0, p1, v, n, x);
@@ -150,20 +166,25 @@ static int grad_f64(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr, con
             for (int32_t k = 0; k < m; ++k) grad_out[j * m + k] += a[(beg + p) * m + k] * x[p];
             obj += (double)c[beg + p] * x[p];
             sq += x[p] * x[p];
+            sumx += x[p];
             if (x_out) x_out[beg + p] = x[p];
         }
     }
+    if (count_coef != 0.0) grad_out[Jm] = count_coef * sumx;
     double reg = 0.5 * gamma * sq, dot = 0.0, r_inf = 0.0, r2 = 0.0;
-    for (int64_t q = 0; q < Jm; ++q) {
-        grad_out[q] -= b[q];                                     /* Eq. 4 */
+    for (int64_t q = 0; q < nrow; ++q) {
+        grad_out[q] -= (q < Jm ? b[q] : count_rhs);              /* Eq. 4 */
         dot += lambda[q] * grad_out[q];
-        if (grad_out[q] > 0.0) { r2 += grad_out[q] * grad_out[q]; if (grad_out[q] > r_inf) r_inf = grad_out[q]; }
+        double viol = (is_eq && is_eq[q]) ? fabs(grad_out[q]) : fmax(grad_out[q], 0.0);
+        r2 += viol * viol;
+        if (viol > r_inf) r_inf = viol;
     }
     scalars_out[0] = obj + reg + dot;                            /* Eq. 2 at its minimiser */
     scalars_out[1] = obj;
     scalars_out[2] = reg;
     scalars_out[3] = r_inf;
     scalars_out[4] = sqrt(r2);
+    scalars_out[5] = -dot;
     free(v); free(x);
     return 0;
 }
@@ -175,15 +196,18 @@ static double* widen(const float* v, int64_t n) {
     return w;
 }
 
+/* has_count != 0: the problem carries the global-count row sum x <= count_M (see grad_f64); lambda / grad_out / is_eq
+ * then have J*m + 1 entries. */
 int dualip_oracle_grad(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr, const int32_t* item_idx,
                        const float* c, const float* a, const float* b, const double* lambda, double gamma,
-                       int proj_kind, double p0, double p1, double* grad_out, double* scalars_out,
-                       double* x_out) {
+                       int proj_kind, double p0, double p1, const uint8_t* is_eq, int32_t has_count, double count_M,
+                       double* grad_out, double* scalars_out, double* x_out) {
     double* a64 = widen(a, row_ptr[I] * m);
     double* b64 = widen(b, (int64_t)J * m);
     int rc = -1;
     if (a64 && b64)
-        rc = grad_f64(I, J, m, row_ptr, item_idx, c, a64, b64, lambda, gamma, proj_kind, p0, p1, grad_out, scalars_out, x_out);
+        rc = grad_f64(I, J, m, row_ptr, item_idx, c, a64, b64, lambda, gamma, proj_kind, p0, p1, is_eq,
+                      has_count ? 1.0 : 0.0, count_M, grad_out, scalars_out, x_out);
     free(a64); free(b64);
     return rc;
 }
@@ -202,11 +226,13 @@ static double lipschitz_f64(int64_t I, int32_t J, int32_t m, const int64_t* row_
     return L;
 }
 
+/* has_count != 0: plus |count row|_2^2 = nnz (reading R21, see dualip_oracle_solve). */
 double dualip_oracle_lipschitz(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr,
-                               const int32_t* item_idx, const float* a) {
+                               const int32_t* item_idx, const float* a, int32_t has_count) {
     double* a64 = widen(a, row_ptr[I] * m);
     if (!a64) return -1.0;
     double L = lipschitz_f64(I, J, m, row_ptr, item_idx, a64);
+    if (has_count) L += (double)row_ptr[I];
     free(a64);
     return L;
 }
@@ -230,63 +256,87 @@ void dualip_oracle_jacobi_scaling(int64_t I, int32_t J, int32_t m, const int64_t
  *   for each stage s: eta = gamma_s / L;  y_0 = lambda (warm start);  t = 0
  *     repeat iters[s] times:
  *        (g_t, grad_t) = grad(y_t, gamma_s)
- *        lambda_{t+1}  = max(0, y_t + eta * grad_t)
+ *        lambda_{t+1}  = max(0, y_t + eta_t * grad_t)
  *        beta_t        = momentum ? t/(t+3) : 0
  *        y_{t+1}       = lambda_{t+1} + beta_t (lambda_{t+1} - lambda_t);   t <- t+1
  *   then one extra grad(lambda_T, gamma_S) gives final scalars / grad / x.
+ * step_rule (readings R2, R20; "AGD step-size range [1e-5, 1e-1]", "we scale the maximum AGD
+ *   step size proportionally with the decay of gamma"):
+ *     0 FIXED     eta_t = gamma_s / L.
+ *     1 ADAPTIVE  eta_fix = gamma_s / L;  hi_s = eta_max * gamma_s / gamma_1;  clip(e) = min(max(e, eta_min), hi_s)
+ *                 (the scaled maximum wins when it falls below eta_min);
+ *                 t = 0, or a 0/0 secant:  eta_t = clip(eta_fix);
+ *                 t >= 1:  eta_t = clip(|y_t - y_{t-1}|_2 / |grad_t - grad_{t-1}|_2)   -- the inverse of the secant estimate
+ *                 of the local Lipschitz constant of grad g along the last move, norms taken in the system being iterated on.
+ *     The paper prints no formula for its adaptive step: PARITY UNPINNED against the paper.
  * Traces (each may be NULL) are indexed by the global iteration counter n = 0..sum(iters)-1:
- *   trace_g[n] = g(y_t), trace_rinf[n], trace_r2[n], trace_grad[n*Jm..] = grad(y_t),
- *   trace_lambda[n*Jm..] = lambda_{t+1}.  stage_x (may be NULL) receives, per stage, x*(lambda_end)
- *   at that stage's gamma (n_stages * nnz doubles) -- used by the drift report of config 5.
- * is_eq (may be NULL = all rows are inequalities, Eq. 1): is_eq[q] != 0 marks coupling row q = j*m+k as an EQUALITY
- *   (A x)_q = b_q; its dual is free in sign, so the projection onto lambda >= 0 is skipped for it ("projection
- *   onto the nonnegative orthant for inequality coordinates"; reading R19) and its violation in the traced
- *   residuals is |grad_q| instead of max(grad_q, 0).  The final scalars come from dualip_oracle_grad, which knows
- *   no row kinds (inequality residuals).
+ *   trace_g[n] = g(y_t), trace_rinf[n], trace_r2[n], trace_grad[n*R..] = grad(y_t), trace_lambda[n*R..] = lambda_{t+1},
+ *   trace_eta[n] = eta_t (of the iterated system);  R = J*m (+1 with the global-count row).  stage_x (may be NULL) receives,
+ *   per stage, x*(lambda_end) at that stage's gamma (n_stages * nnz doubles) -- used by the drift report of config 5.
+ * is_eq (may be NULL = all rows are inequalities, Eq. 1): is_eq[q] != 0 marks coupling row q as an EQUALITY (A x)_q = b_q;
+ *   its dual is free in sign, so the projection onto lambda >= 0 is skipped for it ("projection onto the nonnegative
+ *   orthant for inequality coordinates"; reading R19) and its violation in every reported residual (traces and
+ *   final scalars alike) is |grad_q| instead of max(grad_q, 0).
+ * has_count != 0 (reading R21): the extra coupling row sum_{(i,j) in E} x_ij <= count_M, row number J*m,
+ *   with its own dual (lambda_inout, final_grad, the traces and is_eq then have J*m + 1 entries per vector).  With that row
+ *   A A^T is no longer block diagonal; the step constant becomes L = max_j sum_k sum_i (a^k_ij)^2 + |count row|_2^2
+ *   (|A|_2^2 <= |A_items|_2^2 + |1|_2^2 since A^T A is the sum of the two Gram matrices).
  * jacobi != 0 (reading R18): the whole loop runs on the row-scaled system
  *   A' = D A, b' = D b with its own L' and dual lambda' (warm start lambda'_0 = D^-1 lambda_0); since
  *   A'^T lambda' = A^T (D lambda'), the dual of the ORIGINAL system is lambda = D lambda' and
- *   grad g = D^-1 grad g'.  What is returned (lambda, grad, residuals, traces) is in original units. */
+ *   grad g = D^-1 grad g'.  What is returned (lambda, grad, residuals, traces) is in original units.  The global-count
+ *   row is normalised like any other: D = 1/sqrt(nnz) for it. */
 int dualip_oracle_solve(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr, const int32_t* item_idx,
                         const float* c, const float* a, const float* b, int proj_kind, double p0, double p1,
                         const double* gammas, int32_t n_stages, const int32_t* iters, int32_t momentum, int32_t jacobi,
-                        const uint8_t* is_eq, double* lambda_inout, double* x_out, double* final_scalars, double* final_grad,
+                        const uint8_t* is_eq, int32_t step_rule, double eta_min, double eta_max, int32_t has_count, double count_M,
+                        double* lambda_inout, double* x_out, double* final_scalars, double* final_grad,
                         double* trace_g, double* trace_rinf, double* trace_r2, double* trace_grad,
-                        double* trace_lambda, double* stage_x) {
+                        double* trace_lambda, double* trace_eta, double* stage_x) {
     int64_t Jm = (int64_t)J * m, nnz = row_ptr[I];
+    int64_t R = Jm + (has_count ? 1 : 0);                        /* coupling rows = duals */
     double* as = widen(a, nnz * m);                              /* A  (or A' = D A) */
     double* bs = widen(b, Jm);                                   /* b  (or b' = D b) */
-    double* d = (double*)malloc((size_t)Jm * sizeof(double));
-    double* y = (double*)malloc((size_t)Jm * sizeof(double));
-    double* grad = (double*)malloc((size_t)Jm * sizeof(double));
-    double* lam = (double*)malloc((size_t)Jm * sizeof(double));  /* dual of the system being iterated on */
-    double* lam_new = (double*)malloc((size_t)Jm * sizeof(double));
-    double* out = (double*)malloc((size_t)Jm * sizeof(double));
-    if (!as || !bs || !d || !y || !grad || !lam || !lam_new || !out) {
-        free(as); free(bs); free(d); free(y); free(grad); free(lam); free(lam_new); free(out); return -1;
+    double* d = (double*)malloc((size_t)R * sizeof(double));
+    double* y = (double*)malloc((size_t)R * sizeof(double));
+    double* grad = (double*)malloc((size_t)R * sizeof(double));
+    double* lam = (double*)malloc((size_t)R * sizeof(double));  /* dual of the system being iterated on */
+    double* lam_new = (double*)malloc((size_t)R * sizeof(double));
+    double* out = (double*)malloc((size_t)R * sizeof(double));
+    double* y_prev = (double*)malloc((size_t)R * sizeof(double));
+    double* g_prev = (double*)malloc((size_t)R * sizeof(double));
+    if (!as || !bs || !d || !y || !grad || !lam || !lam_new || !out || !y_prev || !g_prev) {
+        free(as); free(bs); free(d); free(y); free(grad); free(lam); free(lam_new); free(out); free(y_prev); free(g_prev);
+        return -1;
     }
-    for (int64_t q = 0; q < Jm; ++q) d[q] = 1.0;
+    for (int64_t q = 0; q < R; ++q) d[q] = 1.0;
     if (jacobi) {
         dualip_oracle_jacobi_scaling(I, J, m, row_ptr, item_idx, a, d);
         for (int64_t p = 0; p < nnz; ++p)
             for (int32_t k = 0; k < m; ++k) as[p * m + k] *= d[(int64_t)item_idx[p] * m + k];
         for (int64_t q = 0; q < Jm; ++q) bs[q] *= d[q];
+        if (has_count) d[Jm] = nnz > 0 ? 1.0 / sqrt((double)nnz) : 1.0;   /* the count row has a 1 on each of the nnz pairs */
     }
-    for (int64_t q = 0; q < Jm; ++q) lam[q] = lambda_inout[q] / d[q];
+    double count_coef = 0.0, count_rhs = 0.0;                    /* the row's coefficient (1, or 1/sqrt(nnz) row-normalised) */
+    if (has_count) { count_coef = d[Jm]; count_rhs = d[Jm] * count_M; }
+    for (int64_t q = 0; q < R; ++q) lam[q] = lambda_inout[q] / d[q];
     double L = lipschitz_f64(I, J, m, row_ptr, item_idx, as);
+    if (has_count) L += (double)nnz * count_coef * count_coef;   /* reading R21 */
     if (!(L > 0.0)) L = 1.0;
-    double sc[5];
+    double sc[6];
     int64_t n = 0;
     int rc = 0;
     for (int32_t s = 0; s < n_stages && rc == 0; ++s) {
-        double gamma = gammas[s], eta = gamma / L;
-        memcpy(y, lam, (size_t)Jm * sizeof(double));             /* warm start, momentum restart */
+        double gamma = gammas[s], eta_fix = gamma / L;
+        double hi_s = eta_max * gamma / gammas[0];               /* the maximum scales with the decay of gamma */
+        memcpy(y, lam, (size_t)R * sizeof(double));              /* warm start, momentum restart */
         for (int32_t t = 0; t < iters[s] && rc == 0; ++t, ++n) {
-            rc = grad_f64(I, J, m, row_ptr, item_idx, c, as, bs, y, gamma, proj_kind, p0, p1, grad, sc, NULL);
+            rc = grad_f64(I, J, m, row_ptr, item_idx, c, as, bs, y, gamma, proj_kind, p0, p1, NULL, count_coef, count_rhs,
+                          grad, sc, NULL);
             if (trace_g) trace_g[n] = sc[0];
             if (trace_grad || trace_rinf || trace_r2) {          /* residuals of the original rows: grad g = D^-1 grad g' */
                 double r_inf = 0.0, r2 = 0.0;
-                for (int64_t q = 0; q < Jm; ++q) {
+                for (int64_t q = 0; q < R; ++q) {
                     out[q] = grad[q] / d[q];
                     double viol = (is_eq && is_eq[q]) ? fabs(out[q]) : fmax(out[q], 0.0);   /* |Ax-b| on equality rows */
                     r2 += viol * viol;
@@ -294,28 +344,44 @@ int dualip_oracle_solve(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr,
                 }
                 if (trace_rinf) trace_rinf[n] = r_inf;
                 if (trace_r2) trace_r2[n] = sqrt(r2);
-                if (trace_grad) memcpy(trace_grad + n * Jm, out, (size_t)Jm * sizeof(double));
+                if (trace_grad) memcpy(trace_grad + n * R, out, (size_t)R * sizeof(double));
             }
+            double eta = eta_fix;
+            if (step_rule == 1) {                                /* reading R20 */
+                if (t >= 1) {
+                    double dy2 = 0.0, dg2 = 0.0;
+                    for (int64_t q = 0; q < R; ++q) {
+                        dy2 += (y[q] - y_prev[q]) * (y[q] - y_prev[q]);
+                        dg2 += (grad[q] - g_prev[q]) * (grad[q] - g_prev[q]);
+                    }
+                    if (dy2 > 0.0 && dg2 > 0.0) eta = sqrt(dy2) / sqrt(dg2);
+                }
+                eta = fmin(fmax(eta, eta_min), hi_s);
+                memcpy(y_prev, y, (size_t)R * sizeof(double));
+                memcpy(g_prev, grad, (size_t)R * sizeof(double));
+            }
+            if (trace_eta) trace_eta[n] = eta;
             double beta = momentum ? (double)t / (double)(t + 3) : 0.0;
-            for (int64_t q = 0; q < Jm; ++q) {
+            for (int64_t q = 0; q < R; ++q) {
                 lam_new[q] = y[q] + eta * grad[q];
                 if (!(is_eq && is_eq[q])) lam_new[q] = fmax(0.0, lam_new[q]);   /* "projection onto the nonnegative
                                                                                     orthant for inequality coordinates" P:123 */
                 y[q] = lam_new[q] + beta * (lam_new[q] - lam[q]);
             }
-            memcpy(lam, lam_new, (size_t)Jm * sizeof(double));
-            if (trace_lambda) for (int64_t q = 0; q < Jm; ++q) trace_lambda[n * Jm + q] = d[q] * lam[q];
+            memcpy(lam, lam_new, (size_t)R * sizeof(double));
+            if (trace_lambda) for (int64_t q = 0; q < R; ++q) trace_lambda[n * R + q] = d[q] * lam[q];
         }
         if (stage_x && rc == 0)
-            rc = grad_f64(I, J, m, row_ptr, item_idx, c, as, bs, lam, gamma, proj_kind, p0, p1,
+            rc = grad_f64(I, J, m, row_ptr, item_idx, c, as, bs, lam, gamma, proj_kind, p0, p1, NULL, count_coef, count_rhs,
                           grad, sc, stage_x + (int64_t)s * nnz);
     }
-    for (int64_t q = 0; q < Jm; ++q) lambda_inout[q] = d[q] * lam[q];
+    for (int64_t q = 0; q < R; ++q) lambda_inout[q] = d[q] * lam[q];
     /* final report: one evaluation of the ORIGINAL system at lambda_T = D lambda'_T (same x, same g) */
     if (rc == 0 && n_stages > 0)
         rc = dualip_oracle_grad(I, J, m, row_ptr, item_idx, c, a, b, lambda_inout, gammas[n_stages - 1],
-                                proj_kind, p0, p1, final_grad ? final_grad : grad, final_scalars ? final_scalars : sc, x_out);
+                                proj_kind, p0, p1, is_eq, has_count, count_M, final_grad ? final_grad : grad,
+                                final_scalars ? final_scalars : sc, x_out);
     free(as); free(bs); free(d); free(lam); free(out);
-    free(y); free(grad); free(lam_new);
+    free(y); free(grad); free(lam_new); free(y_prev); free(g_prev);
     return rc;
 }

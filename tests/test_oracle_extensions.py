@@ -1,0 +1,247 @@
+"""Pins for the oracle's three oracle-defined extensions (the paper names them but prints no formula, so each is a
+DESIGN.md reading, and parity with the PAPER is unpinned; what is pinned is that the oracle does what the reading says
+and that the reading reduces to pinned things where it can):
+
+  R19  equality coupling rows in the reported residuals
+  R20  range-clipped adaptive AGD step ("AGD step-size range [1e-5, 1e-1]")
+  R21  global-count row  sum_{(i,j) in E} x_ij <= M
+  and the gap column of the Table-4 style report.
+"""
+import itertools
+
+import numpy as np
+import pytest
+
+import oracle
+from conftest import random_problem
+
+
+def _problem(d, kind=oracle.PROJ_SIMPLEX_INEQ, p0=1.0, p1=0.0, count_M=None):
+    return oracle.Problem(d["I"], d["J"], d["m"], d["row_ptr"], d["item_idx"], d["c"], d["a"], d["b"], kind, p0, p1, count_M)
+
+
+def _one(c, a, b):
+    return dict(I=1, J=1, m=1, row_ptr=np.array([0, 1]), item_idx=np.array([0], dtype=np.int32),
+                c=np.array([c], dtype=np.float32), a=np.array([a], dtype=np.float32), b=np.array([b], dtype=np.float32))
+
+
+# ---------------------------------------------------------------- gap and equality-aware residuals (R19)
+
+def test_gap_is_primal_minus_dual_and_vanishes_at_the_optimum():
+    rng = np.random.default_rng(1)
+    d = random_problem(rng, I=40, J=5, m=2, deg=(2, 4), tight=0.5)
+    p = _problem(d)
+    lam = rng.random(10) * 0.3
+    r = oracle.grad(p, lam, 0.1)
+    assert abs(r.gap - (r.obj + r.reg - r.g)) < 1e-12 and abs(r.gap + lam @ r.grad) < 1e-12
+    # at the optimum of a tiny instance: complementary slackness => gap -> 0 (strong duality)
+    d2 = random_problem(np.random.default_rng(4), I=3, J=2, m=1, deg=(1, 2), tight=0.7)
+    d2["b"] = np.array([0.3, 0.25], dtype=np.float32)
+    res = oracle.solve(_problem(d2), [0.5], [5000])
+    assert abs(res.final.gap) < 1e-8 and res.final.r_inf < 1e-7
+
+
+def test_equality_rows_count_absolute_violation_everywhere():
+    """One variable, equality a x = b that needs lambda* < 0: with the mask the residual of a NEGATIVE gradient is |grad|
+    (in the traces and in the final scalars alike); without it, it is 0."""
+    d = _one(c=0.375, a=1.0, b=0.5)                                  # x*(lambda=0) = 0: grad = -0.5
+    p = _problem(d)
+    r0 = oracle.grad(p, [0.0], 1.0)
+    r1 = oracle.grad(p, [0.0], 1.0, is_eq=[1])
+    assert r0.grad[0] == -0.5 and r0.r_inf == 0.0 and r0.r_2 == 0.0
+    assert r1.grad[0] == -0.5 and r1.r_inf == 0.5 and r1.r_2 == 0.5
+    assert (r0.g, r0.obj, r0.reg) == (r1.g, r1.obj, r1.reg)       # the mask changes nothing else
+    res = oracle.solve(p, [1.0], [3], is_eq=[1], trace_grad=True)
+    assert res.trace_rinf[0] == 0.5
+    assert res.final.r_inf == abs(res.final.grad[0]) and res.final.r_2 == abs(res.final.grad[0])
+    # x = clip(-(c + lam)/gamma, 0, 1) = 0.5  <=>  lam* = -0.875
+    res = oracle.solve(p, [1.0], [2000], is_eq=[1])
+    assert abs(res.lam[0] + 0.875) < 1e-9 and res.final.r_inf < 1e-9
+
+
+# ---------------------------------------------------------------- range-clipped adaptive step (R20)
+
+def test_adaptive_with_a_point_range_is_the_fixed_step_bit_for_bit():
+    rng = np.random.default_rng(7)
+    d = random_problem(rng, I=60, J=6, m=1, deg=(2, 5), tight=0.4)
+    p = _problem(d)
+    gamma = 0.2
+    eta = gamma / oracle.lipschitz(p)
+    a = oracle.solve(p, [gamma], [40], trace_lambda=True)
+    b = oracle.solve(p, [gamma], [40], trace_lambda=True, adaptive=True, eta_min=eta, eta_max=eta)
+    assert np.array_equal(a.trace_lambda, b.trace_lambda) and np.array_equal(a.trace_g, b.trace_g)
+    assert np.all(b.trace_eta == eta) and np.all(a.trace_eta == eta)
+
+
+def test_adaptive_secant_is_gamma_over_L_where_the_gradient_is_linear():
+    """I = J = 1 with x strictly inside (0,1): grad g(lam) = a x - b = -a(c + a lam)/gamma - b is LINEAR with slope
+    -a^2/gamma = -L/gamma, so the secant estimate is exact and the adaptive step equals the fixed one from t = 1 on."""
+    c, a, b, gamma = -1.0, 2.0, 0.5, 4.0                          # x(0) = 0.25, x* = b/a = 0.25 .. stays interior
+    p = _problem(_one(c, a, b * 1.2))
+    L = oracle.lipschitz(p)
+    assert L == a * a
+    fix = oracle.solve(p, [gamma], [25], trace_lambda=True)
+    ada = oracle.solve(p, [gamma], [25], trace_lambda=True, adaptive=True, eta_min=1e-9, eta_max=1e9)
+    moved = np.abs(np.diff(np.concatenate([[0.0], ada.trace_lambda[:, 0]]))) > 0
+    np.testing.assert_allclose(ada.trace_eta[1:][moved[1:]], gamma / L, rtol=1e-9)
+    assert ada.trace_eta[0] == gamma / L
+    np.testing.assert_allclose(ada.trace_lambda, fix.trace_lambda, rtol=0, atol=1e-12)
+
+
+def test_adaptive_step_follows_the_reading_and_stays_in_its_range():
+    """eta_t recomputed from the traces by the definition R20 states; the first step of every stage is the clipped fixed
+    step; every step lies in [eta_min, eta_max * gamma_s / gamma_1], and the scaled maximum wins when it is below eta_min."""
+    rng = np.random.default_rng(11)
+    d = random_problem(rng, I=80, J=7, m=2, deg=(2, 5), tight=0.4)
+    p = _problem(d)
+    gammas, iters = [0.4, 0.04, 0.004], [12, 12, 12]
+    L = oracle.lipschitz(p)
+    emin, emax = 0.5 * gammas[0] / L, 3.0 * gammas[0] / L
+    res = oracle.solve(p, gammas, iters, adaptive=True, eta_min=emin, eta_max=emax, trace_grad=True, trace_lambda=True)
+    n = 0
+    lam_prev = np.zeros(14)
+    for s, (g, T) in enumerate(zip(gammas, iters)):
+        hi = emax * g / gammas[0]
+        clip = lambda e: min(max(e, emin), hi)
+        y = lam_prev.copy()
+        for t in range(T):
+            if t == 0:
+                want = clip(g / L)
+            else:
+                dy, dg = np.linalg.norm(y - y_old), np.linalg.norm(res.trace_grad[n] - res.trace_grad[n - 1])
+                want = clip(dy / dg) if dy > 0 and dg > 0 else clip(g / L)
+            assert abs(res.trace_eta[n] - want) <= 1e-12 * want, (s, t)
+            assert res.trace_eta[n] <= hi * (1 + 1e-15) and (res.trace_eta[n] >= emin or res.trace_eta[n] == hi)
+            lam_new = res.trace_lambda[n]
+            y_old = y
+            y = lam_new + (t / (t + 3.0)) * (lam_new - lam_prev)
+            lam_prev = lam_new
+            n += 1
+    assert hi < emin                                              # the last stage really exercises "the maximum wins"
+    assert np.all(res.trace_eta[-12:] == hi)
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_adaptive_reaches_the_kkt_optimum(seed):
+    from test_oracle_solve import _kkt_brute_force
+    rng = np.random.default_rng(100 + seed)
+    d = random_problem(rng, I=int(rng.integers(1, 4)), J=2, m=1, deg=(1, 2), tight=0.7)
+    d["b"] = (0.15 + 0.5 * rng.random(2)).astype(np.float32)
+    gamma = 0.5
+    p = _problem(d)
+    p_star, x_star = _kkt_brute_force(d, gamma)
+    L = oracle.lipschitz(p)
+    res = oracle.solve(p, [gamma], [6000], adaptive=True, eta_min=1e-5, eta_max=2.0 * gamma / L)
+    assert abs(res.final.g - p_star) < 1e-7 * (1 + abs(p_star))
+    np.testing.assert_allclose(res.x, x_star, atol=1e-4)
+    assert res.trace_eta.max() <= 2.0 * gamma / L * (1 + 1e-15) and res.trace_eta.min() >= 1e-5
+
+
+# ---------------------------------------------------------------- global-count row (R21)
+
+def _count_as_second_family(d, M):
+    """J = 1: every eligible pair sits on item 0, so sum_{(i,j)} x_ij <= M IS a second coupling family with a = 1, b = M."""
+    assert d["J"] == 1 and d["m"] == 1
+    n = d["item_idx"].size
+    a2 = np.stack([d["a"], np.ones(n, dtype=np.float32)], axis=1).reshape(-1)
+    return dict(d, m=2, a=a2, b=np.array([d["b"][0], M], dtype=np.float32))
+
+
+@pytest.mark.parametrize("jacobi", [False, True])
+def test_count_row_on_one_item_is_a_second_family(jacobi):
+    rng = np.random.default_rng(5)
+    I = 30
+    d = dict(I=I, J=1, m=1, row_ptr=np.arange(I + 1, dtype=np.int64), item_idx=np.zeros(I, dtype=np.int32),
+             c=(-rng.random(I)).astype(np.float32), a=(0.5 + rng.random(I)).astype(np.float32), b=np.array([4.0], dtype=np.float32))
+    M = 6.0
+    pc, p2 = _problem(d, count_M=M), _problem(_count_as_second_family(d, np.float32(M)))
+    assert pc.rows == 2 and oracle.lipschitz(pc) == oracle.lipschitz(p2)
+    for lam in ([0.0, 0.0], [0.2, 0.1], [0.05, 0.4]):
+        rc, r2 = oracle.grad(pc, lam, 0.3), oracle.grad(p2, lam, 0.3)
+        np.testing.assert_allclose(rc.grad, r2.grad, atol=1e-12)
+        np.testing.assert_allclose(rc.x, r2.x, atol=1e-14)
+        assert abs(rc.g - r2.g) < 1e-12 and abs(rc.r_inf - r2.r_inf) < 1e-12
+    sc = oracle.solve(pc, [0.3, 0.03], [60, 60], trace_lambda=True, jacobi=jacobi)
+    s2 = oracle.solve(p2, [0.3, 0.03], [60, 60], trace_lambda=True, jacobi=jacobi)
+    np.testing.assert_allclose(sc.trace_lambda, s2.trace_lambda, rtol=1e-10, atol=1e-12)
+    assert sc.lam[1] > 0                                           # the count row binds: its dual moves
+
+
+def test_count_row_single_variable_closed_form():
+    """I = J = 1, item row slack: min c x + gamma/2 x^2 s.t. 0 <= x <= 1, x <= M  =>  x* = M when M < -c/gamma, mu* = -c - gamma M."""
+    c, gamma, M = -1.0, 0.5, 0.4
+    p = _problem(_one(c, 1.0, 10.0), count_M=M)
+    res = oracle.solve(p, [gamma], [4000])
+    assert abs(res.x[0] - M) < 1e-8 and abs(res.lam[1] - (-c - gamma * M)) < 1e-8 and res.lam[0] == 0.0
+    assert abs(res.final.gap) < 1e-8
+
+
+def test_count_row_gradient_is_sum_x_minus_M_and_matches_finite_differences():
+    rng = np.random.default_rng(9)
+    d = random_problem(rng, I=50, J=6, m=2, deg=(1, 5), tight=0.5)
+    M = 7.5
+    p = _problem(d, count_M=M)
+    lam = np.concatenate([rng.random(12) * 0.2, [0.15]])
+    r = oracle.grad(p, lam, 0.2)
+    assert abs(r.grad[-1] - (r.x.sum() - M)) < 1e-12
+    h = 1e-6
+    e = np.zeros(13); e[-1] = 1.0
+    fd = (oracle.grad(p, lam + h * e, 0.2).g - oracle.grad(p, lam - h * e, 0.2).g) / (2 * h)
+    assert abs(fd - r.grad[-1]) < 1e-6 * (1 + abs(r.grad[-1]))
+    # a count row that cannot bind: its dual stays 0, and at mu = 0 the evaluation is the plain problem's (only the step
+    # constant differs, L + nnz instead of L, so the two trajectories are not the same sequence)
+    big, plain = _problem(d, count_M=1e9), _problem(d)
+    assert oracle.lipschitz(big) == oracle.lipschitz(plain) + d["item_idx"].size
+    a = oracle.solve(big, [0.2], [50], trace_lambda=True)
+    assert np.all(a.trace_lambda[:, -1] == 0.0)
+    ra, rb = oracle.grad(big, np.concatenate([lam[:-1], [0.0]]), 0.2), oracle.grad(plain, lam[:-1], 0.2)
+    assert np.array_equal(ra.grad[:-1], rb.grad) and np.array_equal(ra.x, rb.x) and ra.obj == rb.obj and ra.reg == rb.reg
+
+
+def _kkt_with_count(d, gamma, M):
+    """Brute-force active-set enumeration of Eq. 1 with the extra row sum x <= M (all other rows as in test_oracle_solve)."""
+    n, I, J = d["item_idx"].size, d["I"], d["J"]
+    c, a, b = d["c"].astype(np.float64), d["a"].astype(np.float64), d["b"].astype(np.float64)
+    G, h = [], []
+    for p in range(n):
+        r = np.zeros(n); r[p] = -1.0; G.append(r); h.append(0.0)
+    for i in range(I):
+        r = np.zeros(n); r[d["row_ptr"][i]:d["row_ptr"][i + 1]] = 1.0; G.append(r); h.append(1.0)
+    for j in range(J):
+        r = np.zeros(n); sel = d["item_idx"] == j; r[sel] = a[sel]; G.append(r); h.append(b[j])
+    G.append(np.ones(n)); h.append(M)
+    G, h = np.array(G), np.array(h)
+    best = None
+    for r in range(0, min(n, len(h)) + 1):
+        for S in itertools.combinations(range(len(h)), r):
+            S = list(S)
+            if S:
+                GS = G[S]
+                if np.linalg.matrix_rank(GS) < len(S):
+                    continue
+                mu = np.linalg.solve(GS @ GS.T, -(gamma * h[S] + GS @ c))
+                if (mu < -1e-10).any():
+                    continue
+                x = -(c + GS.T @ mu) / gamma
+            else:
+                x = -c / gamma
+            if (G @ x <= h + 1e-10).all():
+                val = c @ x + 0.5 * gamma * x @ x
+                if best is None or val < best[0] - 1e-13:
+                    best = (val, x)
+    return best
+
+
+@pytest.mark.parametrize("seed", range(4))
+@pytest.mark.parametrize("jacobi", [False, True])
+def test_count_row_kkt_optimum(seed, jacobi):
+    rng = np.random.default_rng(200 + seed)
+    d = random_problem(rng, I=int(rng.integers(2, 4)), J=2, m=1, deg=(1, 2), tight=0.7)
+    d["b"] = (0.3 + 0.5 * rng.random(2)).astype(np.float32)
+    gamma, M = 0.5, 0.45
+    p_star, x_star = _kkt_with_count(d, gamma, M)
+    assert abs(x_star.sum() - M) < 1e-9                            # the count row is active at the optimum
+    res = oracle.solve(_problem(d, count_M=M), [gamma], [8000], jacobi=jacobi)
+    assert abs(res.final.g - p_star) < 1e-7 * (1 + abs(p_star))
+    np.testing.assert_allclose(res.x, x_star, atol=1e-4)
+    assert res.lam[-1] > 0 and res.final.r_inf < 1e-5 and abs(res.final.gap) < 1e-6

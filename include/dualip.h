@@ -75,6 +75,25 @@ enum { DUALIP_RED_AUTO = 0, DUALIP_RED_SMEM = 1, DUALIP_RED_GLOBAL = 2, DUALIP_R
  *            residuals and the trace stay in the original units.                                             */
 enum { DUALIP_PRECOND_NONE = 0, DUALIP_PRECOND_JACOBI = 1 };
 
+/* Step rule of dualip_solve ("a fixed step size that can be derived analytically from A and gamma"; "AGD step-size
+ * range [1e-5, 1e-1]"; "we scale the maximum AGD step size proportionally with the decay of gamma").  R2, R20:
+ *   FIXED    : eta_t = gamma_s / L_step for every iteration of stage s.
+ *   ADAPTIVE : range-clipped secant step.  hi_s = eta_max gamma_s / gamma_1, clip(e) = min(max(e, eta_min), hi_s);
+ *              first iteration of a stage (or a 0/0 secant): eta_t = clip(gamma_s / L_step);
+ *              afterwards eta_t = clip(|y_t - y_{t-1}|_2 / |grad_t - grad_{t-1}|_2), the inverse of the secant estimate of the
+ *              local Lipschitz constant of grad g along the last move; both norms in the system being iterated on (the
+ *              row-scaled one under DUALIP_PRECOND_JACOBI).  The paper prints no formula: parity unpinned against it. */
+enum { DUALIP_STEP_FIXED = 0, DUALIP_STEP_ADAPTIVE = 1 };
+
+/* Tuning / test overrides of the launch plan; all zero = the library's choice.  None of them changes a result bit. */
+typedef struct {
+    int32_t direct_kernel; /* 1: force the direct-load kernel k_grad instead of the streaming one (parity tests of both) */
+    int32_t stages;        /* pipeline stages of the streaming kernel (2..4) */
+    int32_t tile_units;    /* cap on its tile size in units (>= 256) */
+    int32_t lambda_plan;   /* exact-path dual operand of the streaming kernel: 0 = chosen per launch, 1 = never stage
+                              lambda's low word in shared memory, 2 = always stage it when it fits */
+} dualip_tuning;
+
 typedef struct {
     int32_t projection;   /* DUALIP_PROJ_* */
     double  p0, p1;       /* projection parameters, see above */
@@ -86,13 +105,15 @@ typedef struct {
     int32_t grid_ctas;    /* CTAs of the gradient kernel: 0 = auto (SM count x resident CTAs per SM) */
     int32_t use_graph;    /* 1: dualip_solve replays a CUDA graph of 20 chained iteration launches per stage (stages of >= 40
                              iterations; ignored while profiling is on or with DUALIP_RED_CSC); 0: direct launches */
-    int32_t reserved[4];  /* tuning / test overrides, 0 = the library's choice: [0] = 1 forces the direct-load kernel (parity tests
-                             of both kernels); [1] = pipeline stages of the streaming kernel (2..4); [2] = cap on its tile size
-                             in units (>= 256); [3] must be zero */
+    dualip_tuning tuning; /* launch-plan overrides, see above */
     int32_t precondition; /* DUALIP_PRECOND_*: how dualip_solve scales its step (dualip_grad is not affected) */
+    int32_t step_rule;    /* DUALIP_STEP_* */
+    double  eta_min;      /* DUALIP_STEP_ADAPTIVE: the clip range [eta_min, eta_max gamma_s / gamma_1]; 0 < eta_min <= eta_max */
+    double  eta_max;
 } dualip_opts;
 
-/* Fills *opts with the defaults: unit simplex (inequality), AUTO reduction, copy, validate, momentum. */
+/* Fills *opts with the defaults: unit simplex (inequality), AUTO reduction, copy, validate, momentum, fixed step
+ * (eta_min = 1e-5, eta_max = 1e-1 -- the paper's range, P:185 -- are filled in but unused until step_rule is ADAPTIVE). */
 void dualip_opts_default(dualip_opts* opts);
 
 /* Scalars of one evaluation (Eq. 2; "objective value and regularization term"; "slack"; R9). */
@@ -102,13 +123,15 @@ typedef struct {
     double reg;    /* (gamma/2)|x*|^2 */
     double r_inf;  /* max(0, max_jk grad_jk) : maximum positive constraint violation (|grad| on equality rows) */
     double r_2;    /* |max(grad, 0)|_2 (|grad| on equality rows) */
+    double gap;    /* (obj + reg) - g = -lambda'grad: primal objective of x* minus dual objective -- Table 4's primal-dual gap
+                      before the absolute value; tends to 0 at the optimum (complementary slackness) */
 } dualip_scalars;
 
 /* Optional per-iteration trace of dualip_solve.  All pointers are DEVICE pointers (or NULL to skip that
  * column); entry n is the n-th gradient evaluation over all stages (0 <= n < sum iters <= capacity).
  *   g[n], r_inf[n], r_2[n] : scalars at the extrapolated point y_t the gradient is taken at (R1)
- *   grad[n*J*m + q]        : grad g(y_t)
- *   lambda[n*J*m + q]      : lambda_{t+1}                                                         */
+ *   grad[n*R + q]          : grad g(y_t)        (R = number of duals: J*m, or J*m + 1 with the global-count row)
+ *   lambda[n*R + q]        : lambda_{t+1}                                                         */
 typedef struct {
     int64_t capacity;
     double* g;
@@ -116,6 +139,7 @@ typedef struct {
     double* r_2;
     double* grad;
     double* lambda;
+    double* eta;     /* eta[n] = step of iteration n (of the iterated system; the per-coordinate factor d_q^2 not included) */
 } dualip_trace;
 
 typedef struct {
@@ -140,7 +164,10 @@ typedef struct {
     int64_t grad_kernel_count; /* ... and how many launches that sum covers */
     int32_t precondition;    /* DUALIP_PRECOND_* in effect */
     int32_t pad0;
-    double  L_step;          /* the constant the step is derived from (eta = gamma / L_step): L, or L' with JACOBI */
+    double  L_step;          /* the constant the step is derived from (eta = gamma / L_step): L, or L' with JACOBI
+                                (+ |count row|^2 with the global-count row: nnz, or 1 with JACOBI) */
+    int32_t duals;           /* length of lambda / grad vectors: J*m, or J*m + 1 with the global-count row */
+    int32_t lambda_lo_smem;  /* streaming kernel: 1 if the LAST launch staged lambda's low word in shared memory */
 } dualip_info;
 
 /*
@@ -183,7 +210,9 @@ int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int3
                  const dualip_trace* trace, void* stream);
 
 /* Replace c (nnz fp32, host or device) in place without rebuilding -- config 5's perturbed re-solve.
- * Recomputes the objective's fixed-point scale.  With borrow = 1 the handle switches to the new pointer. */
+ * Recomputes the objective's fixed-point scale.  With borrow = 1 the handle switches to the new pointer, which must be
+ * device memory and, when the streaming kernel is in use (dualip_info.streaming), 16-byte aligned like the arrays given
+ * to dualip_create (its bulk copies need it): otherwise DUALIP_EINVAL and the handle keeps the old c. */
 int dualip_set_c(dualip_t* h, const float* c_new, void* stream);
 
 /* Marks coupling rows as EQUALITIES (A x)_{j,k} = b_{j,k} ("projection onto the nonnegative orthant for
@@ -192,6 +221,15 @@ int dualip_set_c(dualip_t* h, const float* c_new, void* stream);
  * the lambda >= 0 projection for it, and r_inf / r_2 (dualip_grad and dualip_solve alike) count |grad| for it instead
  * of max(grad, 0).  Nothing else changes: g and grad g are defined for any sign of lambda. */
 int dualip_set_equality_rows(dualip_t* h, const uint8_t* is_equality, void* stream);
+
+/* Global-count constraint  sum_{(i,j) in E} x_ij <= M  ("adding a global-count constraint ... only augments A and
+ * lambda"; R21): one more coupling row, number J*m, with coefficient 1 on every eligible pair and its own dual mu >= 0, which
+ * every nonzero gathers: w_ij = -(c_ij + sum_k a^k_ij lambda_jk + mu).  enable != 0 switches the row on with right-hand side M
+ * (finite, >= 0); enable = 0 switches it off.  While it is on, EVERY dual-sized vector at this interface -- lambda, grad,
+ * lambda_inout, final_grad, the trace rows, is_equality -- has J*m + 1 entries, the last one belonging to this row
+ * (dualip_info.duals).  The step constant becomes L_step + nnz (|A|_2^2 <= |A_items|_2^2 + |1|_2^2), or L' + 1 under JACOBI,
+ * where the row is normalised like any other (d^2 = 1/nnz).  Switching the row on or off clears the equality mask. */
+int dualip_set_global_count(dualip_t* h, int32_t enable, double M, void* stream);
 
 /* DUALIP_RED_CSC only (else DUALIP_EUNSUPPORTED): copies out the item-sorted permutation built at create (a0).
  *   col_ptr_out[J+1] int64: column j's entries are perm[col_ptr[j] .. col_ptr[j+1]);

@@ -15,9 +15,10 @@ import numpy as np
 PROJ_SIMPLEX_INEQ, PROJ_BOX, PROJ_BOXCUT, PROJ_SIMPLEX_EQ = 0, 1, 2, 3
 RED_AUTO, RED_SMEM, RED_GLOBAL, RED_CSC = 0, 1, 2, 3
 PRECOND_NONE, PRECOND_JACOBI = 0, 1
+STEP_FIXED, STEP_ADAPTIVE = 0, 1
 
 EXPORTED_SYMBOLS = ("dualip_opts_default", "dualip_create", "dualip_grad", "dualip_solve", "dualip_set_c",
-                    "dualip_set_equality_rows", "dualip_set_profiling", "dualip_get_info", "dualip_get_csc", "dualip_destroy",
+                    "dualip_set_equality_rows", "dualip_set_global_count", "dualip_set_profiling", "dualip_get_info", "dualip_get_csc", "dualip_destroy",
                     "dualip_strerror")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -29,16 +30,22 @@ class DualipError(RuntimeError):
         self.code = code
 
 
+class Tuning(ctypes.Structure):
+    _fields_ = [("direct_kernel", ctypes.c_int32), ("stages", ctypes.c_int32), ("tile_units", ctypes.c_int32),
+                ("lambda_plan", ctypes.c_int32)]
+
+
 class Opts(ctypes.Structure):
     _fields_ = [("projection", ctypes.c_int32), ("p0", ctypes.c_double), ("p1", ctypes.c_double),
                 ("reduction", ctypes.c_int32), ("borrow", ctypes.c_int32), ("validate", ctypes.c_int32),
                 ("momentum", ctypes.c_int32), ("group_lanes", ctypes.c_int32), ("grid_ctas", ctypes.c_int32),
-                ("use_graph", ctypes.c_int32), ("reserved", ctypes.c_int32 * 4), ("precondition", ctypes.c_int32)]
+                ("use_graph", ctypes.c_int32), ("tuning", Tuning), ("precondition", ctypes.c_int32),
+                ("step_rule", ctypes.c_int32), ("eta_min", ctypes.c_double), ("eta_max", ctypes.c_double)]
 
 
 class Scalars(ctypes.Structure):
     _fields_ = [("g", ctypes.c_double), ("obj", ctypes.c_double), ("reg", ctypes.c_double),
-                ("r_inf", ctypes.c_double), ("r_2", ctypes.c_double)]
+                ("r_inf", ctypes.c_double), ("r_2", ctypes.c_double), ("gap", ctypes.c_double)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -46,7 +53,7 @@ class Scalars(ctypes.Structure):
 
 class _Trace(ctypes.Structure):
     _fields_ = [("capacity", ctypes.c_int64), ("g", ctypes.c_void_p), ("r_inf", ctypes.c_void_p),
-                ("r_2", ctypes.c_void_p), ("grad", ctypes.c_void_p), ("lam", ctypes.c_void_p)]
+                ("r_2", ctypes.c_void_p), ("grad", ctypes.c_void_p), ("lam", ctypes.c_void_p), ("eta", ctypes.c_void_p)]
 
 
 class Info(ctypes.Structure):
@@ -57,15 +64,16 @@ class Info(ctypes.Structure):
                 ("bytes_resident", ctypes.c_int64), ("launches", ctypes.c_int64), ("fix_scale_s", ctypes.c_double),
                 ("streaming", ctypes.c_int32), ("stages", ctypes.c_int32), ("tile_units", ctypes.c_int64), ("ntiles", ctypes.c_int64),
                 ("grad_kernel_ms", ctypes.c_double), ("grad_kernel_count", ctypes.c_int64),
-                ("precondition", ctypes.c_int32), ("pad0", ctypes.c_int32), ("L_step", ctypes.c_double)]
+                ("precondition", ctypes.c_int32), ("pad0", ctypes.c_int32), ("L_step", ctypes.c_double),
+                ("duals", ctypes.c_int32), ("lambda_lo_smem", ctypes.c_int32)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
 
 
 def lib_path() -> str:
-    """The in-tree library; DUALIP_B200_LIB overrides it (to load an experimental build variant)."""
-    return os.environ.get("DUALIP_B200_LIB") or os.path.join(_HERE, "libdualip_b200.so")
+    """The in-tree library (there is no other: no override, no fallback)."""
+    return os.path.join(_HERE, "libdualip_b200.so")
 
 
 _lib = None
@@ -88,6 +96,7 @@ def load_library():
         lib.dualip_solve.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, ctypes.POINTER(_Trace), vp]
         lib.dualip_set_c.argtypes = [vp, vp, vp]
         lib.dualip_set_equality_rows.argtypes = [vp, vp, vp]
+        lib.dualip_set_global_count.argtypes = [vp, i32, d, vp]
         lib.dualip_get_info.argtypes = [vp, ctypes.POINTER(Info)]
         lib.dualip_set_profiling.argtypes = [vp, ctypes.c_int]
         lib.dualip_get_csc.argtypes = [vp, vp, vp, vp]
@@ -96,8 +105,8 @@ def load_library():
         lib.dualip_destroy.restype = None
         lib.dualip_strerror.argtypes = [ctypes.c_int]
         lib.dualip_strerror.restype = ctypes.c_char_p
-        for f in ("dualip_create", "dualip_grad", "dualip_solve", "dualip_set_c", "dualip_set_equality_rows", "dualip_get_info",
-                  "dualip_set_profiling"):
+        for f in ("dualip_create", "dualip_grad", "dualip_solve", "dualip_set_c", "dualip_set_equality_rows", "dualip_set_global_count",
+                  "dualip_get_info", "dualip_set_profiling"):
             getattr(lib, f).restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -130,17 +139,17 @@ def _ptr(t, dtype=None, keep=None):
 
 def make_opts(projection=PROJ_SIMPLEX_INEQ, p0=1.0, p1=0.0, reduction=RED_AUTO, borrow=False, validate=True,
               momentum=True, group_lanes=0, grid_ctas=0, use_graph=False, direct_kernel=False, jacobi=False, stages=0, tile_units=0,
-              adaptive=False) -> Opts:
-    if adaptive:
-        raise ValueError('adaptive step: not in this build yet')
+              adaptive=False, eta_min=1e-5, eta_max=1e-1, lambda_plan=0) -> Opts:
     o = Opts()
     load_library().dualip_opts_default(ctypes.byref(o))
     o.projection, o.p0, o.p1, o.reduction = projection, p0, p1, reduction
     o.borrow, o.validate, o.momentum = int(borrow), int(validate), int(momentum)
     o.group_lanes, o.grid_ctas, o.use_graph = group_lanes, grid_ctas, int(use_graph)
-    o.reserved[0] = 1 if direct_kernel else 0
-    o.reserved[1], o.reserved[2] = stages, tile_units
+    o.tuning.direct_kernel = 1 if direct_kernel else 0
+    o.tuning.stages, o.tuning.tile_units, o.tuning.lambda_plan = stages, tile_units, lambda_plan
     o.precondition = PRECOND_JACOBI if jacobi else PRECOND_NONE
+    o.step_rule = STEP_ADAPTIVE if adaptive else STEP_FIXED
+    o.eta_min, o.eta_max = float(eta_min), float(eta_max)
     return o
 
 
@@ -158,6 +167,7 @@ class Problem:
 
     def __init__(self, handle, I, J, m, nnz, keep):
         self._h, self.I, self.J, self.m, self.nnz, self._keep = handle, I, J, m, nnz, keep
+        self.duals = J * m          # length of lambda / grad vectors (+ 1 while the global-count row is on)
 
     @classmethod
     def create(cls, I, J, m, row_ptr, item_idx, c, a, b, opts: Opts | None = None, stream=None) -> "Problem":
@@ -185,7 +195,7 @@ class Problem:
 
     def solve(self, gammas, iters, lam, x=None, scalars=None, grad=None, trace=None, stream=None):
         """dualip_solve: lam fp64[J*m] in/out.  trace: dict with optional device tensors under the keys
-        'g','r_inf','r_2' (fp64[T]), 'grad','lambda' (fp64[T*J*m]); T = sum(iters)."""
+        'g','r_inf','r_2','eta' (fp64[T]), 'grad','lambda' (fp64[T*duals]); T = sum(iters)."""
         gam = np.ascontiguousarray(np.asarray(gammas, dtype=np.float64))
         its = np.ascontiguousarray(np.asarray(iters, dtype=np.int32))
         if gam.shape != its.shape or gam.ndim != 1:
@@ -194,12 +204,12 @@ class Problem:
         if trace is not None:
             tr = _Trace()
             tr.capacity = int(its.sum())
-            for key, field in (("g", "g"), ("r_inf", "r_inf"), ("r_2", "r_2"), ("grad", "grad"), ("lambda", "lam")):
+            for key, field in (("g", "g"), ("r_inf", "r_inf"), ("r_2", "r_2"), ("grad", "grad"), ("lambda", "lam"), ("eta", "eta")):
                 t = trace.get(key)
                 if t is not None:
                     if not t.is_cuda:
                         raise ValueError("trace buffers must be CUDA tensors")
-                    need = tr.capacity * (self.J * self.m if key in ("grad", "lambda") else 1)
+                    need = tr.capacity * (self.duals if key in ("grad", "lambda") else 1)
                     if t.numel() < need:
                         raise ValueError(f"trace['{key}'] too small")
                     setattr(tr, field, t.data_ptr())
@@ -219,6 +229,12 @@ class Problem:
     def set_equality_rows(self, is_equality, stream=None):
         """dualip_set_equality_rows: uint8 mask over the J*m coupling rows (tensor / array), or None for all-inequality."""
         _check(load_library().dualip_set_equality_rows(self._h, _ptr(is_equality, np.uint8), _stream_ptr(stream)))
+
+    def set_global_count(self, M, stream=None):
+        """dualip_set_global_count: M = right-hand side of sum x <= M (one more dual at the end of every dual-sized vector),
+        or None to switch the row off."""
+        _check(load_library().dualip_set_global_count(self._h, 0 if M is None else 1, 0.0 if M is None else float(M), _stream_ptr(stream)))
+        self.duals = self.J * self.m + (0 if M is None else 1)
 
     def get_csc(self, col_ptr=None, perm=None, stream=None):
         """dualip_get_csc: fills col_ptr int64[J+1] and perm int64[nnz] (tensors / arrays or None)."""

@@ -36,7 +36,8 @@ struct Plan {
     const void* fn = nullptr;
     const void* fn_x = nullptr;     // streaming path: the x-writing instantiation (fn never writes x)
     // streaming (TMA) path
-    bool tma = false, lam_lo_smem = false;
+    bool tma = false;
+    int lo_policy = 0;              // lambda's low word in shared memory: 0 per launch (kernel decides), 1 never, 2 always (sized in)
     long long TN = 0, ntiles = 0;
     int cap_nz = 0, cap_rows = 0, stages = 0, stage_bytes = 0;
 };
@@ -52,9 +53,11 @@ struct dualip {
     bool own_rows = false, own_c = false;
     float* b = nullptr;
     // scratch
-    unsigned long long* s_fix = nullptr;   // JM (+2 scalars at the end)
+    unsigned long long* s_fix = nullptr;   // JM item accumulators, then the 3 scalars obj, sq, cnt (sc_fix)
     unsigned long long* sc_fix = nullptr;
     double* lam_cur = nullptr; double* y = nullptr; double* lam_stage = nullptr; double* grad_stage = nullptr;
+    double* y_prev = nullptr; double* g_prev = nullptr;   // DUALIP_STEP_ADAPTIVE: previous evaluation point / gradient (R20)
+    bool count_on = false;                                 // global-count row (R21): duals = J*m + 1, b[J*m] = M
     double* scalars_dev = nullptr;
     float* x_stage = nullptr;
     dualip_dev::TileEntry* tiles = nullptr;
@@ -79,7 +82,7 @@ struct dualip {
     unsigned char* row_eq = nullptr;       // [JM] equality-row mask (dualip_set_equality_rows) or nullptr
     float max_abs_a = 0.0f, max_abs_c = 0.0f;
     long long max_row_len = 0;
-    double scale_s = 1.0, scale_obj = 1.0, scale_sq = 1.0;
+    double scale_s = 1.0, scale_obj = 1.0, scale_sq = 1.0, scale_cnt = 1.0;
     double xmax = 1.0;
     Plan plan;
     int num_sms = 0;
@@ -163,17 +166,20 @@ bool plan_tma(dualip* h, Plan& pl) {
     // same few addresses would otherwise serialise in L2; beyond that RED.ADD.64 goes straight to L2.
     const size_t fixed = kTmaHeaderBytes + 128;
     if (fixed + 4 * JM + 32 * 1024 > kSmemBudget) return false;
-    const bool lo = 8 * JM <= (size_t)DUALIP_LO_SMEM_KB * 1024;
+    // small J*m: the low word is always staged (the plan is sized with it); larger: the kernel decides per launch whether
+    // to trade a pipeline stage for it (k_grad_tma); tuning.lambda_plan overrides
+    const int lp = h->opts.tuning.lambda_plan;
+    const bool lo = lp != 1 && 8 * JM <= (size_t)DUALIP_LO_SMEM_KB * 1024;
     const size_t lam_bytes = (lo ? 8 : 4) * JM;
     bool acc = (red == DUALIP_RED_AUTO && 16 * JM <= 64 * 1024) ||
                (red == DUALIP_RED_SMEM && fixed + lam_bytes + 8 * JM + 32 * 1024 <= kSmemBudget);
     if (red == DUALIP_RED_SMEM && !acc) return false;
     const size_t avail = kSmemBudget - fixed - lam_bytes - (acc ? 8 : 0) * JM;
-    pl.lam_lo_smem = lo;
+    pl.lo_policy = lo ? 2 : (lp == 1 ? 1 : (lp == 2 ? 2 : 0));
     const int m = h->m;
     const long long units = h->nnz + (long long)kRowCost * h->I;
     long long TN = 0; int stages = 0; size_t stage_bytes = 0;
-    const int s_hi = h->opts.reserved[1] ? h->opts.reserved[1] : 3, s_lo = h->opts.reserved[1] ? h->opts.reserved[1] : 2;
+    const int s_hi = h->opts.tuning.stages ? h->opts.tuning.stages : 3, s_lo = h->opts.tuning.stages ? h->opts.tuning.stages : 2;
     for (int S = s_hi; S >= s_lo && TN < 256; --S) {
         stage_bytes = (avail / S) & ~(size_t)127;
         const long long over = 80 + (h->max_row_len + 8 + 72) * (8 + 4 * m);
@@ -186,7 +192,7 @@ bool plan_tma(dualip* h, Plan& pl) {
     const long long want = units / ((long long)h->num_sms * 8);
     if (TN > 8192) TN = 8192;
     if (TN > want) TN = want > 256 ? (want & ~63ll) : 256;
-    if (h->opts.reserved[2] >= 256 && h->opts.reserved[2] < TN) TN = h->opts.reserved[2] & ~63ll;
+    if (h->opts.tuning.tile_units >= 256 && h->opts.tuning.tile_units < TN) TN = h->opts.tuning.tile_units & ~63ll;
     pl.tma = true; pl.acc_smem = acc; pl.lam_smem = true;
     pl.TN = TN; pl.stages = stages;
     pl.cap_nz = (int)((TN + h->max_row_len + 8 + 72 + 3) & ~3ll);   // +72: lanes may read up to 2*32+2 slots past a row end (m = 2)
@@ -215,16 +221,16 @@ int make_plan(dualip* h) {
     if (G == 0) G = mean > 20.0 ? 32 : (mean > 10.0 ? 16 : 8);
     if (G != 1 && G != 2 && G != 4 && G != 8 && G != 16 && G != 32) return DUALIP_EINVAL;
     if (pl.M == 0) G = 32;
-    if (h->opts.reserved[0] != 1 && plan_tma(h, pl)) {          // reserved[0] = 1 forces the non-streaming kernel (tests)
+    if (h->opts.tuning.direct_kernel != 1 && plan_tma(h, pl)) {          // tuning.direct_kernel forces the non-streaming kernel (tests)
         // narrow lane groups: several rows share one pass of the chunk loop, which amortises the per-row work
         int Gs = h->opts.group_lanes;
         if (Gs == 0) {
-            Gs = mean <= 6.0 ? 1 : (mean <= 12.0 ? 2 : (mean <= 24.0 ? 4 : (mean <= 256.0 ? 8 : (mean <= 1024.0 ? 16 : 32))));
+            Gs = mean <= 6.0 ? 1 : (mean <= 12.0 ? 2 : (mean <= 32.0 ? 4 : (mean <= 256.0 ? 8 : (mean <= 1024.0 ? 16 : 32))));
             // a tile is released only when its slowest row-step is done, so it should split into about as many steps
             // (2 * 32/G rows each) as there are consumer warps: long rows (few per tile) get wider groups
             const double rows_per_tile = (double)pl.TN / (mean + kRowCost);
             int Gt = 1;
-            while (Gt < 32 && (double)Gt * rows_per_tile < 600.0) Gt <<= 1;
+            while (Gt < 32 && (double)Gt * rows_per_tile < 360.0) Gt <<= 1;     // measured: cfg5 (92 rows per tile) is faster at 4, cfg3 (82) at 8
             if (Gt > Gs) Gs = Gt;
         }
         if (pl.M == 0) Gs = 8;
@@ -234,8 +240,10 @@ int make_plan(dualip* h) {
         pl.fn = dualip_tma_kernel_wx0(pl.G, pl.M, pl.acc_smem, gbox);
         pl.fn_x = dualip_tma_kernel_wx1(pl.G, pl.M, pl.acc_smem, gbox);
         if (!pl.fn || !pl.fn_x) return DUALIP_EUNSUPPORTED;
-        CK(cudaFuncSetAttribute(pl.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
-        CK(cudaFuncSetAttribute(pl.fn_x, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+        // the attribute is per function and process-wide: always the full budget, so that handles with different plans
+        // (several may share one instantiation) never shrink it under each other
+        CK(cudaFuncSetAttribute(pl.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBudget));
+        CK(cudaFuncSetAttribute(pl.fn_x, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBudget));
         pl.grid = h->opts.grid_ctas > 0 ? h->opts.grid_ctas : (int)(pl.ntiles < h->num_sms ? pl.ntiles : h->num_sms);
         if (pl.grid < 1) pl.grid = 1;
         h->plan = pl;
@@ -254,7 +262,7 @@ int make_plan(dualip* h) {
     pl.smem = (pl.lam_smem ? 8 * JM : 0) + (pl.acc_smem ? 8 * JM : 0) + kScratch;
     pl.fn = pick_kernel(pl);
     if (!pl.fn) return DUALIP_EUNSUPPORTED;
-    CK(cudaFuncSetAttribute(pl.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+    CK(cudaFuncSetAttribute(pl.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBudget));
     int nb = 0;
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pl.fn, kBlockThreads, pl.smem));
     if (nb < 1) return DUALIP_EUNSUPPORTED;
@@ -276,7 +284,11 @@ void set_scales(dualip* h) {
     h->scale_s = fix_scale(h->xmax * h->max_colabs * 1.000001);
     h->scale_obj = fix_scale(h->xmax * h->sum_abs_c * 1.000001);
     h->scale_sq = fix_scale(h->xmax * h->xmax * (double)(h->nnz > 0 ? h->nnz : 1) * 1.000001);
+    h->scale_cnt = fix_scale(h->xmax * (double)(h->nnz > 0 ? h->nnz : 1) * 1.000001);
 }
+
+// duals = coupling rows: J*m, + 1 with the global-count row (R21)
+size_t n_duals(const dualip* h) { return (size_t)h->J * h->m + (h->count_on ? 1 : 0); }
 
 int grid_for(long long n, int threads, int num_sms) {
     long long g = (n + threads - 1) / threads;
@@ -319,6 +331,8 @@ int compute_stats(dualip* h, cudaStream_t st, bool do_a, bool do_c) {
         k_reduce_stats<<<1, 1024, 0, st>>>(colsq, J, m, colabs, JM, out); h->launches++;
         if (do_a && h->step_scale) {
             k_jacobi_step_scale<<<grid_for(JM, 256, h->num_sms), 256, 0, st>>>(colsq, 1.0 / sc_sq, JM, h->step_scale); h->launches++;
+            const double d2_count = nnz > 0 ? 1.0 / (double)nnz : 1.0;       // the count row has a 1 on each of the nnz pairs
+            if (cudaMemcpyAsync(h->step_scale + JM, &d2_count, 8, cudaMemcpyHostToDevice, st) != cudaSuccess) { rc = DUALIP_ECUDA; break; }
         }
         unsigned long long res[4];
         if (cudaMemcpyAsync(res, cabs, sizeof(res), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
@@ -351,8 +365,10 @@ void fill_grad_params(const dualip* h, GradParams& p, const double* lam_dev, dou
             break;
         default: p.z = (float)o.p0; break;
     }
-    p.scale_s = h->scale_s; p.scale_obj = h->scale_obj; p.scale_sq = h->scale_sq;
+    p.count_on = h->count_on ? 1 : 0;
+    p.scale_s = h->scale_s; p.scale_obj = h->scale_obj; p.scale_sq = h->scale_sq; p.scale_cnt = h->scale_cnt;
     p.scale_s_f = (float)h->scale_s; p.scale_obj_f = (float)h->scale_obj; p.scale_sq_f = (float)h->scale_sq;
+    p.scale_cnt_f = (float)h->scale_cnt;
     p.max_abs_c = h->max_abs_c; p.max_abs_a = h->max_abs_a;
 }
 
@@ -383,8 +399,9 @@ void prof_collect(dualip* h) {
 
 // Common fields of the per-launch epilogue (a4-a6).  The caller sets lam_eval/gamma/update/... before launch_iter.
 void fill_finalize_common(const dualip* h, FinalizeParams& f) {
-    f.s_fix = h->s_fix; f.sc_fix = h->sc_fix; f.b = h->b; f.JM = h->J * h->m;
+    f.s_fix = h->s_fix; f.sc_fix = h->sc_fix; f.b = h->b; f.JM = h->J * h->m; f.R = (int)n_duals(h);
     f.inv_scale_s = 1.0 / h->scale_s; f.inv_scale_obj = 1.0 / h->scale_obj; f.inv_scale_sq = 1.0 / h->scale_sq;
+    f.inv_scale_cnt = 1.0 / h->scale_cnt;
     f.row_eq = h->row_eq;
     f.state = reinterpret_cast<IterState*>(h->ctl);
     f.done = reinterpret_cast<unsigned*>(h->ctl + sizeof(IterState));
@@ -415,7 +432,8 @@ void prepare_iter(const dualip* h, IterLaunch& L, const double* lam_dev, double 
         TmaParams& tp = L.tp;
         tp.g = L.p; tp.f = L.f; tp.tiles = h->tiles; tp.ntiles = h->plan.ntiles; tp.cap_nz = h->plan.cap_nz; tp.cap_rows = h->plan.cap_rows;
         tp.stages = h->plan.stages; tp.stage_bytes = h->plan.stage_bytes;
-        tp.nnz4 = h->nnz & ~3ll; tp.rows2 = (h->I + 1) & ~1ll; tp.lam_lo_smem = h->plan.lam_lo_smem ? 1 : 0;
+        tp.nnz4 = h->nnz & ~3ll; tp.rows2 = (h->I + 1) & ~1ll; tp.lo_policy = h->plan.lo_policy;
+        tp.smem_total = (int)h->plan.smem; tp.lo_flag = reinterpret_cast<int*>(h->ctl + 32);
         L.fn = L.p.x ? h->plan.fn_x : h->plan.fn; L.grid = dim3(h->plan.grid); L.block = dim3(32 * (kTmaConsumerWarps + 1)); L.smem = h->plan.smem;
         L.args[0] = &L.tp; L.args[1] = nullptr;
     } else {
@@ -548,6 +566,7 @@ void dualip_opts_default(dualip_opts* o) {
     std::memset(o, 0, sizeof(*o));
     o->projection = DUALIP_PROJ_SIMPLEX_INEQ; o->p0 = 1.0; o->p1 = 0.0;
     o->reduction = DUALIP_RED_AUTO; o->borrow = 0; o->validate = 1; o->momentum = 1;
+    o->step_rule = DUALIP_STEP_FIXED; o->eta_min = 1e-5; o->eta_max = 1e-1;
 }
 
 const char* dualip_strerror(int code) {
@@ -568,7 +587,7 @@ void dualip_destroy(dualip_t* h) {
     if (h->own_rows) { cudaFree((void*)h->row_ptr); cudaFree((void*)h->idx); cudaFree((void*)h->a); }
     if (h->own_c) cudaFree((void*)h->c);
     cudaFree(h->b); cudaFree(h->s_fix); cudaFree(h->lam_cur); cudaFree(h->y); cudaFree(h->lam_stage);
-    cudaFree(h->grad_stage); cudaFree(h->scalars_dev); cudaFree(h->step_scale); cudaFree(h->row_eq); cudaFree(h->x_stage); cudaFree(h->tiles);
+    cudaFree(h->grad_stage); cudaFree(h->y_prev); cudaFree(h->g_prev); cudaFree(h->scalars_dev); cudaFree(h->step_scale); cudaFree(h->row_eq); cudaFree(h->x_stage); cudaFree(h->tiles);
     drop_graph(h);
     cudaFree(h->ctl);
     cudaFree(h->csc_perm); cudaFree(h->col_ptr); cudaFree(h->chunk_ptr); cudaFree(h->chunk_item); cudaFree(h->csc_partial);
@@ -594,9 +613,11 @@ int dualip_create(dualip_t** out, int64_t I, int32_t J, int32_t m, const int64_t
     if ((long long)J * m > (1ll << 30)) return DUALIP_EINVAL;
     dualip_opts o;
     if (opts_in) o = *opts_in; else dualip_opts_default(&o);
-    if (o.reserved[0] != 0 && o.reserved[0] != 1) return DUALIP_EINVAL;   // 1 = force the non-streaming kernel
-    if (o.reserved[1] != 0 && (o.reserved[1] < 2 || o.reserved[1] > kTmaStagesMax)) return DUALIP_EINVAL;   // pipeline stages
-    if (o.reserved[2] < 0 || o.reserved[3] != 0) return DUALIP_EINVAL;                                        // tile units cap
+    if (o.tuning.direct_kernel != 0 && o.tuning.direct_kernel != 1) return DUALIP_EINVAL;
+    if (o.tuning.stages != 0 && (o.tuning.stages < 2 || o.tuning.stages > kTmaStagesMax)) return DUALIP_EINVAL;
+    if (o.tuning.tile_units < 0 || o.tuning.lambda_plan < 0 || o.tuning.lambda_plan > 2) return DUALIP_EINVAL;
+    if (o.step_rule != DUALIP_STEP_FIXED && o.step_rule != DUALIP_STEP_ADAPTIVE) return DUALIP_EINVAL;
+    if (o.step_rule == DUALIP_STEP_ADAPTIVE && !(o.eta_min > 0.0 && o.eta_min <= o.eta_max && std::isfinite(o.eta_max))) return DUALIP_EINVAL;
     if (o.precondition != DUALIP_PRECOND_NONE && o.precondition != DUALIP_PRECOND_JACOBI) return DUALIP_EINVAL;
     switch (o.projection) {
         case DUALIP_PROJ_SIMPLEX_INEQ: case DUALIP_PROJ_SIMPLEX_EQ: if (!(o.p0 > 0.0)) return DUALIP_EINVAL; break;
@@ -653,16 +674,22 @@ int dualip_create(dualip_t** out, int64_t I, int32_t J, int32_t m, const int64_t
             }
         }
         const size_t JM = (size_t)J * m;
-        if ((rc = dev_alloc(h, &h->b, JM)) != 0) goto fail;
+        // every dual-sized buffer has room for the global-count row's entry (index JM; dualip_set_global_count)
+        if ((rc = dev_alloc(h, &h->b, JM + 1)) != 0) goto fail;
+        CKF(cudaMemsetAsync(h->b, 0, (JM + 1) * 4, st));
         CKF(cudaMemcpyAsync(h->b, b, JM * 4, cudaMemcpyDefault, st));
-        if ((rc = dev_alloc(h, &h->s_fix, JM + 2)) != 0) goto fail;
+        if ((rc = dev_alloc(h, &h->s_fix, JM + 3)) != 0) goto fail;
         h->sc_fix = h->s_fix + JM;
-        CKF(cudaMemsetAsync(h->s_fix, 0, (JM + 2) * 8, st));
-        if ((rc = dev_alloc(h, &h->lam_cur, JM)) != 0) goto fail;
-        if ((rc = dev_alloc(h, &h->y, JM)) != 0) goto fail;
-        if ((rc = dev_alloc(h, &h->lam_stage, JM)) != 0) goto fail;
-        if ((rc = dev_alloc(h, &h->grad_stage, JM)) != 0) goto fail;
-        if ((rc = dev_alloc(h, &h->scalars_dev, 5)) != 0) goto fail;
+        CKF(cudaMemsetAsync(h->s_fix, 0, (JM + 3) * 8, st));
+        if ((rc = dev_alloc(h, &h->lam_cur, JM + 1)) != 0) goto fail;
+        if ((rc = dev_alloc(h, &h->y, JM + 1)) != 0) goto fail;
+        if ((rc = dev_alloc(h, &h->lam_stage, JM + 1)) != 0) goto fail;
+        if ((rc = dev_alloc(h, &h->grad_stage, JM + 1)) != 0) goto fail;
+        if ((rc = dev_alloc(h, &h->scalars_dev, 6)) != 0) goto fail;
+        if (o.step_rule == DUALIP_STEP_ADAPTIVE) {
+            if ((rc = dev_alloc(h, &h->y_prev, JM + 1)) != 0) goto fail;
+            if ((rc = dev_alloc(h, &h->g_prev, JM + 1)) != 0) goto fail;
+        }
         if ((rc = dev_alloc(h, &h->ctl, 64)) != 0) goto fail;
         CKF(cudaMemsetAsync(h->ctl, 0, 64, st));
 
@@ -685,7 +712,7 @@ int dualip_create(dualip_t** out, int64_t I, int32_t J, int32_t m, const int64_t
             if (flags & 4) FAIL(DUALIP_EDUP);
             h->max_row_len = (long long)maxlen;
         }
-        if (o.precondition == DUALIP_PRECOND_JACOBI && (rc = dev_alloc(h, &h->step_scale, JM)) != 0) goto fail;
+        if (o.precondition == DUALIP_PRECOND_JACOBI && (rc = dev_alloc(h, &h->step_scale, JM + 1)) != 0) goto fail;
         if ((rc = compute_stats(h, st, true, true)) != 0) goto fail;
         set_xmax(h);
         set_scales(h);
@@ -726,7 +753,14 @@ int dualip_get_info(dualip_t* h, dualip_info* info) {
     info->bytes_resident = h->bytes_resident; info->launches = h->launches;
     info->fix_scale_s = h->scale_s;
     info->grad_kernel_ms = h->prof_ms; info->grad_kernel_count = h->prof_count;
-    info->precondition = h->step_scale ? DUALIP_PRECOND_JACOBI : DUALIP_PRECOND_NONE; info->L_step = h->L_step;
+    info->precondition = h->step_scale ? DUALIP_PRECOND_JACOBI : DUALIP_PRECOND_NONE;
+    info->L_step = h->L_step + (h->count_on ? (h->step_scale ? 1.0 : (double)h->nnz) : 0.0);
+    info->duals = (int32_t)n_duals(h);
+    if (h->plan.tma) {                                       // what the last streaming launch decided (it has finished: default-stream copy)
+        int flag = 0;
+        if (cudaMemcpy(&flag, h->ctl + 32, sizeof(int), cudaMemcpyDeviceToHost) == cudaSuccess) info->lambda_lo_smem = flag;
+        else cudaGetLastError();
+    }
     return DUALIP_OK;
 }
 
@@ -760,6 +794,7 @@ int dualip_set_c(dualip_t* h, const float* c_new, void* stream) {
         CK(cudaMemcpyAsync((void*)h->c, c_new, (size_t)h->nnz * 4, cudaMemcpyDefault, st));
     } else {
         if (!is_device_ptr(c_new)) return DUALIP_EINVAL;     // borrowed rows: the new c must be device memory too
+        if (h->plan.tma && ((uintptr_t)c_new & 15)) return DUALIP_EINVAL;   // the streaming kernel's bulk copies need 16-byte alignment
         h->c = c_new;
     }
     int rc = compute_stats(h, st, false, true);
@@ -771,14 +806,27 @@ int dualip_set_c(dualip_t* h, const float* c_new, void* stream) {
 int dualip_set_equality_rows(dualip_t* h, const uint8_t* is_equality, void* stream) {
     if (!h) return DUALIP_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const size_t JM = (size_t)h->J * h->m;
+    const size_t JM = (size_t)h->J * h->m, R = n_duals(h);
     if (!is_equality) {                                      // back to all-inequality rows
-        if (h->row_eq) { CK(cudaStreamSynchronize(st)); cudaFree(h->row_eq); h->row_eq = nullptr; h->bytes_resident -= (long long)JM; }
+        if (h->row_eq) { CK(cudaStreamSynchronize(st)); cudaFree(h->row_eq); h->row_eq = nullptr; h->bytes_resident -= (long long)(JM + 1); }
         return DUALIP_OK;
     }
-    if (!h->row_eq) { int rc = dev_alloc(h, &h->row_eq, JM); if (rc != 0) return rc; }
-    CK(cudaMemcpyAsync(h->row_eq, is_equality, JM, cudaMemcpyDefault, st));
+    if (!h->row_eq) { int rc = dev_alloc(h, &h->row_eq, JM + 1); if (rc != 0) return rc; }
+    CK(cudaMemcpyAsync(h->row_eq, is_equality, R, cudaMemcpyDefault, st));
     if (!is_device_ptr(is_equality)) CK(cudaStreamSynchronize(st));
+    return DUALIP_OK;
+}
+
+int dualip_set_global_count(dualip_t* h, int32_t enable, double M, void* stream) {
+    if (!h) return DUALIP_EINVAL;
+    if (enable && !(M >= 0.0 && std::isfinite(M))) return DUALIP_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    CK(cudaStreamSynchronize(st));                           // earlier launches still read the old layout
+    if (h->row_eq) { cudaFree(h->row_eq); h->row_eq = nullptr; h->bytes_resident -= (long long)((size_t)h->J * h->m + 1); }
+    h->count_on = enable != 0;
+    const float Mf = enable ? (float)M : 0.0f;
+    CK(cudaMemcpyAsync(h->b + (size_t)h->J * h->m, &Mf, 4, cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st));
     return DUALIP_OK;
 }
 
@@ -786,7 +834,7 @@ int dualip_grad(dualip_t* h, const double* lambda, double gamma, double* grad, d
                 void* stream) {
     if (!h || !lambda || !(gamma > 0.0) || !std::isfinite(gamma)) return DUALIP_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const size_t JM = (size_t)h->J * h->m;
+    const size_t JM = n_duals(h);
     const bool lam_dev = is_device_ptr(lambda), grad_dev = is_device_ptr(grad), sc_dev = is_device_ptr(scalars),
                x_dev = is_device_ptr(x);
     const double* lam_d = lambda;
@@ -803,7 +851,7 @@ int dualip_grad(dualip_t* h, const double* lambda, double gamma, double* grad, d
     if (rc != 0) return rc;
     bool sync = !lam_dev;
     if (grad && !grad_dev) { CK(cudaMemcpyAsync(grad, h->grad_stage, JM * 8, cudaMemcpyDeviceToHost, st)); sync = true; }
-    if (scalars && !sc_dev) { CK(cudaMemcpyAsync(scalars, h->scalars_dev, 5 * 8, cudaMemcpyDeviceToHost, st)); sync = true; }
+    if (scalars && !sc_dev) { CK(cudaMemcpyAsync(scalars, h->scalars_dev, sizeof(dualip_scalars), cudaMemcpyDeviceToHost, st)); sync = true; }
     if (x && !x_dev && h->nnz > 0) { CK(cudaMemcpyAsync(x, h->x_stage, (size_t)h->nnz * 4, cudaMemcpyDeviceToHost, st)); sync = true; }
     if (sync) CK(cudaStreamSynchronize(st));
     return DUALIP_OK;
@@ -821,11 +869,15 @@ int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int3
     if (trace && trace->capacity < total) return DUALIP_EINVAL;
     if (n_stages == 0) return DUALIP_OK;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const size_t JM = (size_t)h->J * h->m;
+    const size_t JM = n_duals(h);
     const bool lam_dev = is_device_ptr(lambda_inout), grad_dev = is_device_ptr(final_grad),
                sc_dev = is_device_ptr(final_scalars), x_dev = is_device_ptr(x_out);
     CK(cudaMemcpyAsync(h->lam_cur, lambda_inout, JM * 8, cudaMemcpyDefault, st));
-    const double L = h->L_step > 0.0 ? h->L_step : 1.0;
+    // R21: with the global-count row A A^T is no longer block diagonal; |A|_2^2 <= |A_items|_2^2 + |count row|_2^2, and the
+    // row's squared norm is nnz (1 once row-normalised)
+    double L = h->L_step + (h->count_on ? (h->step_scale ? 1.0 : (double)h->nnz) : 0.0);
+    if (!(L > 0.0)) L = 1.0;
+    const bool adaptive = h->opts.step_rule == DUALIP_STEP_ADAPTIVE;
     CK(cudaMemsetAsync(h->ctl, 0, sizeof(IterState), st));                                 // t = 0, n = 0
     for (int s = 0; s < n_stages; ++s) {
         const double gamma = gammas[s], eta = gamma / L;
@@ -834,7 +886,14 @@ int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int3
         FinalizeParams f{};
         f.lam_eval = h->y; f.gamma = gamma; f.update = 1; f.eta = eta; f.momentum = h->opts.momentum ? 1 : 0;
         f.lam_cur = h->lam_cur; f.y = h->y; f.step_scale = h->step_scale;
-        if (trace) { f.tr_g = trace->g; f.tr_rinf = trace->r_inf; f.tr_r2 = trace->r_2; f.tr_grad = trace->grad; f.tr_lam = trace->lambda; }
+        if (adaptive) {                                      // R20: clip range of this stage; the maximum scales with gamma
+            f.step_rule = 1; f.eta_lo = h->opts.eta_min; f.eta_hi = h->opts.eta_max * gamma / gammas[0];
+            f.y_prev = h->y_prev; f.g_prev = h->g_prev;
+        }
+        if (trace) {
+            f.tr_g = trace->g; f.tr_rinf = trace->r_inf; f.tr_r2 = trace->r_2; f.tr_grad = trace->grad; f.tr_lam = trace->lambda;
+            f.tr_eta = trace->eta;
+        }
         IterLaunch it;
         prepare_iter(h, it, h->y, gamma, nullptr, f);
         int t = 0;
@@ -870,7 +929,7 @@ int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int3
     CK(cudaMemcpyAsync(lambda_inout, h->lam_cur, JM * 8, cudaMemcpyDefault, st));
     if (!lam_dev) sync = true;
     if (final_grad && !grad_dev) { CK(cudaMemcpyAsync(final_grad, h->grad_stage, JM * 8, cudaMemcpyDeviceToHost, st)); sync = true; }
-    if (final_scalars && !sc_dev) { CK(cudaMemcpyAsync(final_scalars, h->scalars_dev, 5 * 8, cudaMemcpyDeviceToHost, st)); sync = true; }
+    if (final_scalars && !sc_dev) { CK(cudaMemcpyAsync(final_scalars, h->scalars_dev, sizeof(dualip_scalars), cudaMemcpyDeviceToHost, st)); sync = true; }
     if (x_out && !x_dev && h->nnz > 0) { CK(cudaMemcpyAsync(x_out, h->x_stage, (size_t)h->nnz * 4, cudaMemcpyDeviceToHost, st)); sync = true; }
     if (sync) CK(cudaStreamSynchronize(st));
     return DUALIP_OK;

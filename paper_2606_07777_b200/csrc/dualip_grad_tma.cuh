@@ -54,7 +54,9 @@ struct TmaParams {
     int stage_bytes;                   // bytes of one stage (multiple of 16)
     long long nnz4;                    // nnz rounded down to a multiple of 4 (bulk copies stop there)
     long long rows2;                   // (I+1) rounded down to a multiple of 2
-    int lam_lo_smem;                   // 1: lambda's low word is staged in shared memory too (small J*m)
+    int lo_policy;                     // lambda's low word in shared memory: 0 = decided per launch (see k_grad_tma), 1 = never, 2 = always
+    int smem_total;                    // dynamic shared memory of the launch (bytes)
+    int* lo_flag;                      // nullable: CTA 0 records the decision here (dualip_info.lambda_lo_smem)
 };
 
 // ---- PTX wrappers (mbarrier + bulk async copy) ---------------------------------------------------------------
@@ -101,8 +103,27 @@ __device__ __forceinline__ StageView stage_view(unsigned char* base, int cap_nz,
 
 // The x output pointer, or a compile-time nullptr in the WX = false instantiations that dualip_solve's loop launches (it
 // never writes x): the x-writing code drops out of the hot kernel, which measured 2-5 % faster on every config.
-template <bool WX>
-__device__ __forceinline__ float* xout(const GradParams& p) { return WX ? p.x : nullptr; }
+template <bool WX, class P>
+__device__ __forceinline__ float* xout(const P& p) { return WX ? p.x : nullptr; }
+
+// The launch constants the out-of-line row routines use, as REGISTER values.  Those routines get the kernel parameters by
+// reference, i.e. as a generic pointer, and the compiler re-loads a field from memory at every use rather than keep it in
+// a register (ncu on the dense regime: 40 % of the stall samples were long-scoreboard waits on exactly those loads, on the
+// critical path of every fixed-point push).  pin() copies the fields once and launders them through an empty asm so they
+// cannot be rematerialised from memory.  Field names are GradParams', so the routines' code reads the same.
+struct GradK {
+    float scale_s_f, scale_obj_f, scale_sq_f, scale_cnt_f, inv_gamma_f, z, ub;
+    double inv_gamma;
+    unsigned long long* s_fix;
+    float* x;
+    int proj, m;
+};
+__device__ __forceinline__ GradK pin(const GradParams& p) {
+    GradK k{p.scale_s_f, p.scale_obj_f, p.scale_sq_f, p.scale_cnt_f, p.inv_gamma_f, p.z, p.ub, p.inv_gamma, p.s_fix, p.x, p.proj, p.m};
+    asm volatile("" : "+f"(k.scale_s_f), "+f"(k.scale_obj_f), "+f"(k.scale_sq_f), "+f"(k.scale_cnt_f), "+f"(k.inv_gamma_f), "+f"(k.z), "+f"(k.ub));
+    asm volatile("" : "+d"(k.inv_gamma), "+l"(k.s_fix), "+l"(k.x), "+r"(k.proj), "+r"(k.m));
+    return k;
+}
 
 // Shared state the row routines need.
 struct ConsumerCtx {
@@ -111,8 +132,26 @@ struct ConsumerCtx {
     const double* lam_g;                          //   then the exact path reads the fp64 lambda from global memory (L2)
     unsigned* acc_lo; unsigned* acc_hi;           // shared-memory item accumulators (ACC_SMEM)
     bool hi_only;                                 // RN_f32(lambda) is exact enough for this launch's gamma (see k_grad_tma)
+    double mu;                                    // dual of the global-count row (R21; 0 when the row is off): every nonzero's
+                                                  //   t = c + a.lambda + mu, a uniform shift of the whole row
 };
-struct FixPair { long long obj, sq; };            // per-lane fixed-point partial scalars (order-independent)
+__device__ __forceinline__ ConsumerCtx pin(const ConsumerCtx& c) {
+    ConsumerCtx k = c;
+    int hi = k.hi_only ? 1 : 0;
+    asm volatile("" : "+l"(k.lam_hi), "+l"(k.lam_lo), "+l"(k.lam_g), "+l"(k.acc_lo), "+l"(k.acc_hi), "+r"(hi), "+d"(k.mu));
+    k.hi_only = hi != 0;
+    return k;
+}
+// The out-of-line routines get the stage and lambda pointers as generic pointers; telling the compiler that they point
+// to shared memory turns their loads back into LDS (short scoreboard) instead of generic LD (long scoreboard + an address
+// space check per access).
+__device__ __forceinline__ void assume_shared(const StageView& v, const ConsumerCtx& cx) {
+    __builtin_assume(__isShared(v.idx)); __builtin_assume(__isShared(v.c)); __builtin_assume(__isShared(v.a));
+    __builtin_assume(__isShared(v.rp)); __builtin_assume(__isShared(v.meta));
+    __builtin_assume(__isShared(cx.lam_hi)); __builtin_assume(cx.lam_lo == nullptr || __isShared(cx.lam_lo));
+    __builtin_assume(__isShared(cx.acc_lo)); __builtin_assume(__isShared(cx.acc_hi));
+}
+struct FixPair { long long obj, sq, cnt; };       // per-lane fixed-point partial scalars c'x, |x|^2, sum x (order-independent)
 
 // v * 2^k as a 64-bit integer.  The scales are powers of two within fp32 range (dualip_api.cu clamps the exponent), so
 // the product is exact and this equals to_fix(v, (double)scale) of dualip_kernels.cuh: one FMUL + one F2I.
@@ -121,7 +160,7 @@ __device__ __forceinline__ long long to_fix32(float v, float scale) { return __f
 // RED.ADD.64 on a pointer known to be global memory (a generic atomicAdd makes ptxas emit an address-space check, a
 // shared-memory CAS loop and a predicate that the caller then waits on).
 __device__ __forceinline__ void red_add_u64(unsigned long long* gptr, unsigned long long v) {
-    asm volatile("red.global.add.u64 [%0], %1;" ::"l"(gptr), "l"(v) : "memory");
+    asm volatile("red.global.add.u64 [%0], %1;" ::"l"(gptr), "l"(v));
 }
 
 // (a > b) ? x : y as one SETP + SEL, whatever the surrounding control flow looks like
@@ -132,10 +171,11 @@ __device__ __forceinline__ int sel_gt(float a, float b, int x, int y) {
 }
 
 // a4 + a5 for one nonzero with x != 0.
-template <int M, bool ACC_SMEM>
-__device__ __forceinline__ void push(const GradParams& p, const ConsumerCtx& cx, FixPair& fp, int mm, int j, float cc, const float* aa, float x) {
+template <int M, bool ACC_SMEM, class P>
+__device__ __forceinline__ void push(const P& p, const ConsumerCtx& cx, FixPair& fp, int mm, int j, float cc, const float* aa, float x) {
     fp.obj += to_fix32(cc * x, p.scale_obj_f);
     fp.sq += to_fix32(x * x, p.scale_sq_f);
+    fp.cnt += to_fix32(x, p.scale_cnt_f);
     if (!ACC_SMEM && p.s_fix == nullptr) return;          // DUALIP_RED_CSC
 #pragma unroll
     for (int f = 0; f < (M > 0 ? M : 4); ++f) {
@@ -152,7 +192,7 @@ template <int M>
 __device__ __forceinline__ double exact_t(const StageView& v, const ConsumerCtx& cx, int mm, int q, int& j, float& cc, float* aa) {
     j = v.idx[q];
     cc = v.c[q];
-    double t = (double)cc;
+    double t = (double)cc + cx.mu;
 #pragma unroll
     for (int f = 0; f < (M > 0 ? M : 4); ++f) {
         aa[f] = 0.0f;
@@ -164,6 +204,43 @@ __device__ __forceinline__ double exact_t(const StageView& v, const ConsumerCtx&
         }
     }
     return t;
+}
+
+// exact_t for K staged nonzeros at once: all index loads first, then all lambda gathers (an L2 round trip each when lambda's
+// low word is not in shared memory), then the arithmetic -- K independent chains in flight instead of K serial ones.  Every
+// position must be inside the stage (callers clamp the slots they do not own to a valid one and discard the result).  Same
+// operations in the same order as exact_t, so the values are bit-identical to it.
+template <int K, int M>
+__device__ __forceinline__ void exact_t_batch(const StageView& v, const ConsumerCtx& cx, int mm, const int (&q)[K], double (&t)[K]) {
+    constexpr int MA = M > 0 ? M : 4;
+    int j[K];
+    double l[K][MA];
+#pragma unroll
+    for (int k = 0; k < K; ++k) j[k] = v.idx[q[k]];
+    if (cx.hi_only) {
+#pragma unroll
+        for (int k = 0; k < K; ++k)
+#pragma unroll
+            for (int f = 0; f < MA; ++f) l[k][f] = f < mm ? (double)cx.lam_hi[j[k] * mm + f] : 0.0;
+    } else if (cx.lam_lo) {
+#pragma unroll
+        for (int k = 0; k < K; ++k)
+#pragma unroll
+            for (int f = 0; f < MA; ++f) l[k][f] = f < mm ? (double)cx.lam_hi[j[k] * mm + f] + (double)cx.lam_lo[j[k] * mm + f] : 0.0;
+    } else {
+#pragma unroll
+        for (int k = 0; k < K; ++k)
+#pragma unroll
+            for (int f = 0; f < MA; ++f) l[k][f] = f < mm ? __ldg(cx.lam_g + j[k] * mm + f) : 0.0;
+    }
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        double tt = (double)v.c[q[k]] + cx.mu;
+#pragma unroll
+        for (int f = 0; f < MA; ++f)
+            if (f < mm) tt = fma((double)v.a[q[k] * mm + f], l[k][f], tt);
+        t[k] = tt;
+    }
 }
 
 // The filter's view of 4 nonzeros of one row: this lane's slots at q (M != 2: q..q+3; M = 2: the pairs (q, q+1) and
@@ -234,8 +311,11 @@ __device__ __forceinline__ void filter_pass(const StageView& v, const float* __r
 // Slow path: one row, whole warp, any length; every pass re-reads the staged row.  Same arithmetic as long_row()
 // in dualip_kernels.cuh (which documents the three box-cut steps).
 template <int M, bool ACC_SMEM, bool GBOX, bool WX>
-__device__ __noinline__ FixPair slow_row(const GradParams& p, const StageView v, const ConsumerCtx cx, int beg, int len, long long nzb) {
-    FixPair fp{0ll, 0ll};                              // returned in registers: the caller's accumulators never live in local memory
+__device__ __noinline__ FixPair slow_row(const GradParams& p_in, const StageView v, const ConsumerCtx cx_in, int beg, int len, long long nzb) {
+    const GradK p = pin(p_in);
+    const ConsumerCtx cx = pin(cx_in);
+    assume_shared(v, cx);
+    FixPair fp{0ll, 0ll, 0ll};                              // returned in registers: the caller's accumulators never live in local memory
     const int lane = threadIdx.x & 31;
     const int mm = M > 0 ? M : p.m;
     const int end = beg + len;
@@ -250,11 +330,16 @@ __device__ __noinline__ FixPair slow_row(const GradParams& p, const StageView v,
         // (large gamma, binding constraints).
         double tk[KS];
         float wmax = -CUDART_INF_F;
+        {
+            int qk[KS];
 #pragma unroll
-        for (int k = 0; k < KS; ++k) {
-            const int q = beg + lane + 32 * k;
-            tk[k] = CUDART_INF;
-            if (q < end) { tk[k] = exact_t<M>(v, cx, mm, q, j, cc, aa); wmax = fmaxf(wmax, (float)(-tk[k])); }
+            for (int k = 0; k < KS; ++k) qk[k] = min(beg + lane + 32 * k, end - 1);      // len >= 1 here
+            exact_t_batch<KS, M>(v, cx, mm, qk, tk);
+#pragma unroll
+            for (int k = 0; k < KS; ++k) {
+                if (beg + lane + 32 * k < end) wmax = fmaxf(wmax, (float)(-tk[k]));
+                else tk[k] = CUDART_INF;
+            }
         }
         const float m32 = group_max<32>(wmax);
         if (ineq && !(m32 > 0.0f)) {
@@ -387,7 +472,7 @@ __device__ __noinline__ FixPair slow_row(const GradParams& p, const StageView v,
 // take (b0, l0), lanes 16-31 take (b1, l1); l1 = 0 means "no partner".  The arithmetic is slow_row's (fp64 t once per
 // nonzero, exact maximum, Michelot on the shifted fp32 values) with 16-lane reductions.
 template <int K, int M, bool ACC_SMEM, bool WX>
-__device__ __forceinline__ void half_warp_rows(const GradParams& p, const StageView& v, const ConsumerCtx& cx, FixPair& fp, int b0, int l0, int b1,
+__device__ __forceinline__ void half_warp_rows(const GradK& p, const StageView& v, const ConsumerCtx& cx, FixPair& fp, int b0, int l0, int b1,
                                                int l1, long long nzb) {
     const int lane = threadIdx.x & 31, h = lane & 15;
     const int mm = M > 0 ? M : p.m;
@@ -398,10 +483,16 @@ __device__ __forceinline__ void half_warp_rows(const GradParams& p, const StageV
     int j; float cc; float aa[M > 0 ? M : 4];
     double tk[K];
     float wmax = -CUDART_INF_F;
+    {
+        int qk[K];
 #pragma unroll
-    for (int k = 0; k < K; ++k) {
-        tk[k] = CUDART_INF;
-        if (h + 16 * k < len) { tk[k] = exact_t<M>(v, cx, mm, beg + h + 16 * k, j, cc, aa); wmax = fmaxf(wmax, (float)(-tk[k])); }
+        for (int k = 0; k < K; ++k) qk[k] = beg + min(h + 16 * k, max(len - 1, 0));       // slots past the row: a valid position, discarded
+        exact_t_batch<K, M>(v, cx, mm, qk, tk);
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            if (h + 16 * k < len) wmax = fmaxf(wmax, (float)(-tk[k]));
+            else tk[k] = CUDART_INF;
+        }
     }
     const float m16 = group_max<16>(wmax);
     const bool alive = len > 0 && (!ineq || m16 > 0.0f);
@@ -450,16 +541,19 @@ __device__ __forceinline__ void half_warp_rows(const GradParams& p, const StageV
 // own length class, partner or not, so a row's arithmetic does not depend on what else is in its step; everything else
 // goes to slow_row one row at a time.
 template <int M, bool ACC_SMEM, bool GBOX, bool WX>
-__device__ __noinline__ FixPair slow_rows_all(const GradParams& p, const StageView v, const ConsumerCtx cx, int fbeg, int flen, unsigned mask,
+__device__ __noinline__ FixPair slow_rows_all(const GradParams& p_in, const StageView v, const ConsumerCtx cx_in, int fbeg, int flen, unsigned mask,
                                               long long nzb) {
-    FixPair fp{0ll, 0ll};
+    const GradK p = pin(p_in);
+    const ConsumerCtx cx = pin(cx_in);
+    assume_shared(v, cx);
+    FixPair fp{0ll, 0ll, 0ll};
     while (mask) {
         const int s0 = __ffs(mask) - 1;
         mask &= mask - 1;
         const int b0 = __shfl_sync(kFull, fbeg, s0), l0 = __shfl_sync(kFull, flen, s0);
         if (GBOX || l0 > 64) {
-            const FixPair sp = slow_row<M, ACC_SMEM, GBOX, WX>(p, v, cx, b0, l0, nzb);
-            fp.obj += sp.obj; fp.sq += sp.sq;
+            const FixPair sp = slow_row<M, ACC_SMEM, GBOX, WX>(p_in, v, cx_in, b0, l0, nzb);
+            fp.obj += sp.obj; fp.sq += sp.sq; fp.cnt += sp.cnt;
             continue;
         }
         const bool small = l0 <= 32;
@@ -476,35 +570,30 @@ __device__ __noinline__ FixPair slow_rows_all(const GradParams& p, const StageVi
 }
 
 template <int G, int M, bool ACC_SMEM, bool GBOX, bool WX, int NWC>
-__global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams tp) {
+__global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const __grid_constant__ TmaParams tp) {
     extern __shared__ __align__(128) unsigned char smem_tma[];
     const GradParams& p = tp.g;
     constexpr int MA = M > 0 ? M : 4;
     constexpr int NT = 32 * (NWC + 1);
     const int mm = M > 0 ? M : p.m;
     const int JM = p.J * mm;
-    // layout: [full[4], empty[4] mbarriers: 64 B][max|lambda| word: 64 B][candidate lists: 256 B per consumer warp][lam_hi JM*4]
-    //         [lam_lo JM*4 (optional)][acc 2*JM*4 (ACC_SMEM)][stages]
+    // layout: [full[4], empty[4] mbarriers: 64 B][words: 64 B][candidate lists: 256 B per consumer warp][lam_hi JM*4]
+    //         [acc 2*JM*4 (ACC_SMEM)][lam_lo JM*4 (decided per launch, below)][stages]
     unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_tma);
     unsigned* s_words = reinterpret_cast<unsigned*>(smem_tma + 64);       // [0] = max |lambda_hi| as float bits
     int* cand_list = reinterpret_cast<int*>(smem_tma + 128);              // 64 positions per consumer warp (candidate path B)
     float* s_hi32 = reinterpret_cast<float*>(smem_tma + kTmaHeaderBytes);
-    float* s_lo32 = s_hi32 + JM;                                           // only when tp.lam_lo_smem
-    unsigned* a_lo = reinterpret_cast<unsigned*>(s_hi32 + (tp.lam_lo_smem ? 2 : 1) * JM);
+    unsigned* a_lo = reinterpret_cast<unsigned*>(s_hi32 + JM);
     unsigned* a_hi = a_lo + JM;
-    size_t off = kTmaHeaderBytes + (size_t)JM * 4 * ((tp.lam_lo_smem ? 2 : 1) + (ACC_SMEM ? 2 : 0));
-    off = (off + 127) & ~(size_t)127;
-    unsigned char* stage0 = smem_tma + off;
+    float* s_lo32 = s_hi32 + (ACC_SMEM ? 3 : 1) * JM;
 
     if (threadIdx.x == 0) s_words[0] = 0u;
     __syncthreads();
     {
         float lmax = 0.0f;
         for (int q = threadIdx.x; q < JM; q += NT) {
-            const double l = p.lambda[q];
-            const float h = (float)l;
+            const float h = (float)p.lambda[q];
             s_hi32[q] = h;
-            if (tp.lam_lo_smem) s_lo32[q] = (float)(l - (double)h);
             lmax = fmaxf(lmax, fabsf(h));
         }
         // max |lambda|: the filter's rounding bound (M > 1) and the hi_only test below need it
@@ -513,28 +602,55 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
         if ((threadIdx.x & 31) == 0) atomicMax(&s_words[0], __float_as_uint(lmax));
     }
     if (ACC_SMEM) for (int q = threadIdx.x; q < 2 * JM; q += NT) a_lo[q] = 0u;
-    {   // consumers read whole 16-byte vectors around a row: every stage word must always hold a valid item index
-        uint4* sp = reinterpret_cast<uint4*>(stage0);
-        const int n16 = tp.stages * (tp.stage_bytes / 16);
-        for (int q = threadIdx.x; q < n16; q += NT) sp[q] = make_uint4(0u, 0u, 0u, 0u);
-        fence_proxy_async();                                             // generic-proxy zeros before the first bulk copy
-    }
-    if (threadIdx.x == 0) {
-        for (int s = 0; s < tp.stages; ++s) { mbar_init(&bars[s], 1); mbar_init(&bars[kTmaStagesMax + s], NWC); }
-        fence_mbar_init();
-        fence_proxy_async();
-    }
     __syncthreads();
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     // The exact path needs lambda beyond fp32 only when 1/gamma amplifies its rounding into x: dropping the low word moves
     // w by at most m max|a| max|lambda| 2^-25, v = w/gamma by that over gamma, and any x by at most twice that.  When the
     // bound is below 1e-7 (two orders inside the 1e-5 bar, the size of the fp32 steps that follow anyway) the exact path
-    // reads RN_f32(lambda) from shared memory instead of the fp64 dual through L2 -- which is what makes rows in the
+    // reads RN_f32(lambda) from shared memory instead of the fp64 dual -- which is what makes rows in the
     // fractional regime (large gamma, or lambda = 0) cost one shared-memory latency instead of one L2 round trip each.
     const bool hi_only = (float)mm * p.max_abs_a * __uint_as_float(s_words[0]) * p.inv_gamma_f * 5.9604645e-8f <= 1e-7f;
-    const ConsumerCtx cx{s_hi32, tp.lam_lo_smem ? s_lo32 : nullptr, p.lambda, a_lo, a_hi, hi_only};
-    FixPair fp{0ll, 0ll};
+    // When the test fails, the exact path needs lambda's low word as well.  THIS launch stages it in shared memory, next to
+    // the high word, if that still leaves two pipeline stages (the tiles were sized at create without it: a launch that needs
+    // the low word is in the fractional regime, far from the HBM roof, where a shallower pipeline costs nothing; a launch
+    // that does not need it keeps every stage).  Otherwise the exact path reads the fp64 dual through L2.  The decision
+    // depends on lambda and gamma only, so every CTA takes the same one.  lo_policy: 0 = as described, 1 = never, 2 = always.
+    int nstages = tp.stages;
+    size_t off = kTmaHeaderBytes + (size_t)JM * 4 * (ACC_SMEM ? 3 : 1);
+    bool lo_smem = false;
+    if (tp.lo_policy == 2 || (tp.lo_policy == 0 && !hi_only)) {
+        const size_t off_lo = (off + (size_t)JM * 4 + 127) & ~(size_t)127;
+        const long long fit = ((long long)tp.smem_total - (long long)off_lo) / tp.stage_bytes;
+        if (fit >= 2) { lo_smem = true; off = off_lo; nstages = fit < nstages ? (int)fit : nstages; }
+    }
+    off = (off + 127) & ~(size_t)127;
+    unsigned char* stage0 = smem_tma + off;
+    if (lo_smem) {
+        for (int q = threadIdx.x; q < JM; q += NT) {
+            const double l = p.lambda[q];
+            s_lo32[q] = (float)(l - (double)(float)l);
+        }
+    }
+    {   // consumers read whole 16-byte vectors around a row, beyond the part of the stage the tile's copies wrote: every word of
+        // the INDEX array of a stage must always hold a valid item index (c and a may hold anything: those slots are masked)
+        for (int s = 0; s < nstages; ++s) {
+            uint4* sp = reinterpret_cast<uint4*>(stage0 + (size_t)s * tp.stage_bytes);
+            for (int q = threadIdx.x; q < tp.cap_nz / 4; q += NT) sp[q] = make_uint4(0u, 0u, 0u, 0u);
+        }
+        fence_proxy_async();                                             // generic-proxy zeros before the first bulk copy
+    }
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < nstages; ++s) { mbar_init(&bars[s], 1); mbar_init(&bars[kTmaStagesMax + s], NWC); }
+        fence_mbar_init();
+        fence_proxy_async();
+        if (blockIdx.x == 0 && tp.lo_flag) *tp.lo_flag = lo_smem ? 1 : 0;
+    }
+    __syncthreads();
+
+    const double mu = p.count_on ? p.lambda[JM] : 0.0;
+    const ConsumerCtx cx{s_hi32, lo_smem ? s_lo32 : nullptr, p.lambda, a_lo, a_hi, hi_only, mu};
+    FixPair fp{0ll, 0ll, 0ll};
 
     if (warp == 0) {
         // ================= producer =================
@@ -578,7 +694,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                 }
                 if (nr) bulk_g2s(d_rp, p.row_ptr + r0a, nr * 8u, &bars[s]);
                 cur = ncur; nxt = nnxt;
-                if (++s == tp.stages) { s = 0; ph ^= 1u; }
+                if (++s == nstages) { s = 0; ph ^= 1u; }
             }
         }
     } else {
@@ -596,6 +712,10 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
         // rounding bound of the filter (see below): the part that does not depend on the row
         const float bnd0 = M == 1 ? p.max_abs_c : p.max_abs_c + (float)mm * p.max_abs_a * __uint_as_float(s_words[0]);
         const float gz_sat = gz * (1.0f + 4.8e-7f);                      // w_max above this (plus tol): v_max >= z for sure
+        // The global-count dual mu shifts every w of every row by the same amount, so the filter leaves it out (the top two,
+        // their gap and the candidate set do not see it); only the two tests against absolute levels (row dead: w_max < 0,
+        // row saturated: w_max >= z gamma) take it, with its fp32 rounding added to their tolerance.
+        const float mu_f = (float)mu, mu_tol = 2.4e-7f * fabsf(mu_f);
         int s = 0;
         unsigned ph = 0;
         int step_off = 0;                                                // (steps of all earlier tiles) mod NWC
@@ -689,14 +809,15 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                     const float B = M == 1 ? 2.0f * mag + bnd0 : bnd0;
                     const float tol = 2.4e-7f * (float)(mm + 1) * B + 1e-30f;
                     const bool vertex = (m1 - m2) > gz + 2.0f * tol;
-                    const bool dead = ineq && m1 < -tol;
+                    const float m1s = m1 - mu_f, tol_s = tol + mu_tol;
+                    const bool dead = ineq && m1s < -tol_s;
                     const bool fast = vertex || dead;
                     float xo = 0.0f;
                     if (active && vertex && !dead) {
                         // x = clamp(v_max, 0, z) on the arg-max nonzero (z for the equality simplex).  When v_max >= z is
                         // certain in fp32 the answer is z itself; otherwise that one nonzero is redone in fp64.
                         int j; float cc; float aa[MA];
-                        if (!ineq || m1 - tol > gz_sat) {
+                        if (!ineq || m1s - tol_s > gz_sat) {
                             j = v.idx[fpos]; cc = v.c[fpos];
 #pragma unroll
                             for (int f = 0; f < MA; ++f) aa[f] = f < mm ? v.a[fpos * mm + f] : 0.0f;
@@ -823,22 +944,25 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const TmaParams 
                 }
                 if (slow_mask) {
                     const FixPair sp = slow_rows_all<M, ACC_SMEM, GBOX, WX>(p, v, cx, fbeg, flen, slow_mask, v.meta->nzb);
-                    fp.obj += sp.obj; fp.sq += sp.sq;
+                    fp.obj += sp.obj; fp.sq += sp.sq; fp.cnt += sp.cnt;
                 }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&bars[kTmaStagesMax + s]);           // this warp is done with the stage
-            if (++s == tp.stages) { s = 0; ph ^= 1u; }
+            if (++s == nstages) { s = 0; ph ^= 1u; }
         }
     }
 
     {
-        long long so = fp.obj, ss = fp.sq;
+        long long so = fp.obj, ss = fp.sq, sn = fp.cnt;
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) { so += __shfl_xor_sync(kFull, so, o); ss += __shfl_xor_sync(kFull, ss, o); }
+        for (int o = 16; o > 0; o >>= 1) {
+            so += __shfl_xor_sync(kFull, so, o); ss += __shfl_xor_sync(kFull, ss, o); sn += __shfl_xor_sync(kFull, sn, o);
+        }
         if (lane == 0) {
             if (so) atomicAdd(p.sc_fix + 0, (unsigned long long)so);
             if (ss) atomicAdd(p.sc_fix + 1, (unsigned long long)ss);
+            if (sn) atomicAdd(p.sc_fix + 2, (unsigned long long)sn);
         }
     }
     if (ACC_SMEM) {

@@ -36,20 +36,21 @@ struct GradParams {
     const float* __restrict__ a;
     const double* __restrict__ lambda;
     unsigned long long* s_fix;   // [J*m] item accumulators, fixed point, zero on entry; nullptr = do not accumulate (CSC)
-    unsigned long long* sc_fix;  // [2]   obj = c'x and |x|^2, fixed point, zero on entry
+    unsigned long long* sc_fix;  // [3]   obj = c'x, |x|^2 and sum x, fixed point, zero on entry
     float* x;                    // [nnz] or nullptr
     long long I;
     long long nnz;
     int J, m;
     int proj;
     int general_boxcut;          // BOXCUT with ub < z: needs the capped threshold search
+    int count_on;                // global-count row (R21): lambda[J*m] is its dual mu, gathered by EVERY nonzero
     float inv_gamma_f;
     float z;                     // simplex / box-cut budget
     float ub;                    // box-cut cap
     double inv_gamma;
     double box_lo, box_hi;
-    double scale_s, scale_obj, scale_sq;
-    float scale_s_f, scale_obj_f, scale_sq_f;   // the same powers of two as floats (streaming kernel: one FMUL + F2I)
+    double scale_s, scale_obj, scale_sq, scale_cnt;
+    float scale_s_f, scale_obj_f, scale_sq_f, scale_cnt_f;   // the same powers of two as floats (streaming kernel: one FMUL + F2I)
     float max_abs_c, max_abs_a;                 // max |c|, max |a| over all nonzeros (a0): the filter's rounding bound
 };
 
@@ -82,13 +83,14 @@ __device__ __forceinline__ int group_sum_i(int v) {
     return v;
 }
 
-// One nonzero: returns t = c + sum_k a_k * lambda[j,k] in fp64 (w = -t), and the row data it read.
+// One nonzero: returns t = c + sum_k a_k * lambda[j,k] (+ mu, the dual of the global-count row, R21) in fp64 (w = -t), and
+// the row data it read.
 template <int M, bool LAM_SMEM>
-__device__ __forceinline__ double eval_t(const GradParams& p, const double* s_lam, long long q, int mm,
+__device__ __forceinline__ double eval_t(const GradParams& p, const double* s_lam, double mu, long long q, int mm,
                                          int& j, float& cc, float (&aa)[M > 0 ? M : 4]) {
     j = __ldg(p.idx + q);
     cc = __ldg(p.c + q);
-    double t = (double)cc;
+    double t = (double)cc + mu;
     if (M > 0) {
 #pragma unroll
         for (int k = 0; k < M; ++k) aa[k] = __ldg(p.a + q * M + k);
@@ -134,71 +136,107 @@ struct IterState { int t; int pad; long long n; };
 struct FinalizeParams {
     unsigned long long* s_fix;
     unsigned long long* sc_fix;
-    const float* __restrict__ b;
+    const float* __restrict__ b;  // [R]: b[JM] = M of the global-count row when it is on
     const double* lam_eval;     // point the gradient was taken at
     double* grad_out;           // nullable
-    double* scalars_out;        // nullable, 5 doubles {g, obj, reg, r_inf, r_2}
-    int JM;
-    double inv_scale_s, inv_scale_obj, inv_scale_sq;
+    double* scalars_out;        // nullable, 6 doubles {g, obj, reg, r_inf, r_2, gap}
+    int JM;                     // item coupling rows J*m
+    int R;                      // coupling rows = duals: JM, + 1 with the global-count row (row JM, R21)
+    double inv_scale_s, inv_scale_obj, inv_scale_sq, inv_scale_cnt;
     double gamma;
     int update;                 // a6 on/off
     int momentum;               // beta_t = t/(t+3) (R1) or 0
-    double eta;
+    double eta;                 // gamma / L_step (R2)
+    int step_rule;              // 0 fixed; 1 range-clipped secant step (R20)
+    double eta_lo, eta_hi;      // step_rule 1: clip range of this stage, eta_hi = eta_max gamma_s / gamma_1
+    double* y_prev; double* g_prev;   // step_rule 1: the previous evaluation point and gradient of this stage [R]
     const double* step_scale;   // nullable: per-coordinate factor on eta (Jacobi preconditioning, R18: d_q^2 = 1/|A_q*|^2)
     const unsigned char* row_eq; // nullable: nonzero = equality coupling row (dual free in sign, violation |grad|; R19)
     double* lam_cur;            // lambda_t -> lambda_{t+1}
     double* y;                  // y_t -> y_{t+1} (== lam_eval when update)
     IterState* state;           // read and advanced when update
     unsigned* done;             // CTAs that have flushed their partial sums (zero between launches)
-    double* tr_g; double* tr_rinf; double* tr_r2; double* tr_grad; double* tr_lam;   // trace columns (nullable)
+    double* tr_g; double* tr_rinf; double* tr_r2; double* tr_grad; double* tr_lam; double* tr_eta;   // trace columns (nullable)
 };
 
 constexpr int kFinalizeScratchBytes = 3 * 32 * 8 + 16;   // shared memory finalize_block needs: 3 x 32 doubles + flag
 
-// a4 (grad = s - b), a5 (scalars), a6 (AGD step, R1) on the J*m vector by ONE CTA of `nthreads` (<= 1024) threads;
+// s_q = (A x)_q from the fixed-point accumulators: item rows from s_fix, the global-count row (q = JM) from the sum-x scalar
+__device__ __forceinline__ double row_sum(const FinalizeParams& p, int q) {
+    return q < p.JM ? (double)(long long)__ldcg(p.s_fix + q) * p.inv_scale_s : (double)(long long)__ldcg(p.sc_fix + 2) * p.inv_scale_cnt;
+}
+
+// a4 (grad = s - b), a5 (scalars), a6 (AGD step, R1) on the R-vector by ONE CTA of `nthreads` (<= 1024) threads;
 // re-zeroes the accumulators and advances the iteration state.  `sh` = 96 doubles of shared memory.
 __device__ __forceinline__ void finalize_block(const FinalizeParams& p, double* sh, int tid, int nthreads) {
     double* sh_dot = sh; double* sh_r2 = sh + 32; double* sh_inf = sh + 64;
+    const int lane = tid & 31, warp = tid >> 5, nwarps = (nthreads + 31) / 32;
     int t = 0; long long n = 0;
     if (p.update) { t = p.state->t; n = p.state->n; }
     const double beta = (p.update && p.momentum) ? (double)t / (double)(t + 3) : 0.0;
+    // R20: eta_t = clip(|y_t - y_{t-1}| / |grad_t - grad_{t-1}|) -- the inverse of the secant estimate of the local Lipschitz
+    // constant of grad g -- with both norms taken in the system being iterated on: under Jacobi preconditioning (R18) that is
+    // the row-scaled one, y' = y / d and grad' = d grad with d_q^2 = step_scale[q].  First iteration of a stage (or a 0/0
+    // secant): the fixed step.  One more pass over the R-vector before the update, since every coordinate needs eta_t.
+    double eta_t = p.eta;
+    if (p.update && p.step_rule == 1) {
+        if (t >= 1) {
+            double dy2 = 0.0, dg2 = 0.0;
+            for (int q = tid; q < p.R; q += nthreads) {
+                const double g = row_sum(p, q) - (double)__ldg(p.b + q);
+                const double d2 = p.step_scale ? __ldg(p.step_scale + q) : 1.0;
+                const double dy = __ldcg(p.lam_eval + q) - __ldcg(p.y_prev + q), dg = g - __ldcg(p.g_prev + q);
+                dy2 = fma(dy / d2, dy, dy2);
+                dg2 = fma(dg * d2, dg, dg2);
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) { dy2 += __shfl_xor_sync(kFull, dy2, o); dg2 += __shfl_xor_sync(kFull, dg2, o); }
+            if (lane == 0) { sh_dot[warp] = dy2; sh_r2[warp] = dg2; }
+            __syncthreads();
+            dy2 = 0.0; dg2 = 0.0;
+            for (int w = 0; w < nwarps; ++w) { dy2 += sh_dot[w]; dg2 += sh_r2[w]; }
+            __syncthreads();                                        // the scratch is reused below
+            if (dy2 > 0.0 && dg2 > 0.0) eta_t = sqrt(dy2) / sqrt(dg2);
+        }
+        eta_t = fmin(fmax(eta_t, p.eta_lo), p.eta_hi);
+    }
     double dot = 0.0, r2 = 0.0, rinf = 0.0;
     // four elements per thread and pass, every load issued before the first dependent store: the loop is a chain of
     // L2 round trips, and this CTA runs alone at the end of the launch
     constexpr int U = 4;
-    for (int q0 = tid; q0 < p.JM; q0 += U * nthreads) {
-        unsigned long long sf[U]; float bb[U]; double le[U], lo[U], et[U]; bool eq[U];
+    for (int q0 = tid; q0 < p.R; q0 += U * nthreads) {
+        double sv[U]; float bb[U]; double le[U], lo[U], et[U]; bool eq[U];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             const int q = q0 + u * nthreads;
-            sf[u] = 0ull; bb[u] = 0.0f; le[u] = 0.0; lo[u] = 0.0; et[u] = p.eta; eq[u] = false;
-            if (q < p.JM) {
-                sf[u] = __ldcg(p.s_fix + q); bb[u] = __ldg(p.b + q); le[u] = __ldcg(p.lam_eval + q);
+            sv[u] = 0.0; bb[u] = 0.0f; le[u] = 0.0; lo[u] = 0.0; et[u] = eta_t; eq[u] = false;
+            if (q < p.R) {
+                sv[u] = row_sum(p, q); bb[u] = __ldg(p.b + q); le[u] = __ldcg(p.lam_eval + q);
                 if (p.row_eq) eq[u] = __ldg(p.row_eq + q) != 0;
                 if (p.update) {
                     lo[u] = __ldcg(p.lam_cur + q);
-                    if (p.step_scale) et[u] = p.eta * __ldg(p.step_scale + q);
+                    if (p.step_scale) et[u] = eta_t * __ldg(p.step_scale + q);
                 }
             }
         }
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             const int q = q0 + u * nthreads;
-            if (q >= p.JM) break;
-            const double s = (double)(long long)sf[u] * p.inv_scale_s;
-            p.s_fix[q] = 0ull;
-            const double g = s - (double)bb[u];
+            if (q >= p.R) break;
+            if (q < p.JM) p.s_fix[q] = 0ull;
+            const double g = sv[u] - (double)bb[u];
             dot = fma(le[u], g, dot);
             const double viol = eq[u] ? fabs(g) : fmax(g, 0.0);
             r2 = fma(viol, viol, r2); rinf = fmax(rinf, viol);
             if (p.grad_out) p.grad_out[q] = g;
             if (p.update) {
-                if (p.tr_grad) p.tr_grad[n * p.JM + q] = g;
+                if (p.tr_grad) p.tr_grad[n * p.R + q] = g;
+                if (p.step_rule == 1) { p.y_prev[q] = le[u]; p.g_prev[q] = g; }
                 const double lv = le[u] + et[u] * g;
                 const double ln = eq[u] ? lv : fmax(0.0, lv);            // lambda >= 0 on inequality coordinates only
                 p.lam_cur[q] = ln;
                 p.y[q] = ln + beta * (ln - lo[u]);
-                if (p.tr_lam) p.tr_lam[n * p.JM + q] = ln;
+                if (p.tr_lam) p.tr_lam[n * p.R + q] = ln;
             }
         }
     }
@@ -208,22 +246,25 @@ __device__ __forceinline__ void finalize_block(const FinalizeParams& p, double* 
         r2 += __shfl_xor_sync(kFull, r2, o);
         rinf = fmax(rinf, __shfl_xor_sync(kFull, rinf, o));
     }
-    const int lane = tid & 31, warp = tid >> 5;
     if (lane == 0) { sh_dot[warp] = dot; sh_r2[warp] = r2; sh_inf[warp] = rinf; }
     __syncthreads();
     if (tid == 0) {
         dot = 0.0; r2 = 0.0; rinf = 0.0;
-        for (int w = 0; w < (nthreads + 31) / 32; ++w) { dot += sh_dot[w]; r2 += sh_r2[w]; rinf = fmax(rinf, sh_inf[w]); }
+        for (int w = 0; w < nwarps; ++w) { dot += sh_dot[w]; r2 += sh_r2[w]; rinf = fmax(rinf, sh_inf[w]); }
         const double obj = (double)(long long)__ldcg(p.sc_fix + 0) * p.inv_scale_obj;
         const double reg = 0.5 * p.gamma * ((double)(long long)__ldcg(p.sc_fix + 1) * p.inv_scale_sq);
-        p.sc_fix[0] = 0ull; p.sc_fix[1] = 0ull;
+        p.sc_fix[0] = 0ull; p.sc_fix[1] = 0ull; p.sc_fix[2] = 0ull;
         const double g = obj + reg + dot;
         const double nr2 = sqrt(r2);
-        if (p.scalars_out) { p.scalars_out[0] = g; p.scalars_out[1] = obj; p.scalars_out[2] = reg; p.scalars_out[3] = rinf; p.scalars_out[4] = nr2; }
+        if (p.scalars_out) {
+            p.scalars_out[0] = g; p.scalars_out[1] = obj; p.scalars_out[2] = reg; p.scalars_out[3] = rinf; p.scalars_out[4] = nr2;
+            p.scalars_out[5] = -dot;                                      // (obj + reg) - g: Table 4's primal-dual gap
+        }
         if (p.update) {
             if (p.tr_g) p.tr_g[n] = g;
             if (p.tr_rinf) p.tr_rinf[n] = rinf;
             if (p.tr_r2) p.tr_r2[n] = nr2;
+            if (p.tr_eta) p.tr_eta[n] = eta_t;
             p.state->t = t + 1; p.state->n = n + 1;
         }
     }
@@ -248,14 +289,14 @@ __device__ __forceinline__ void grid_epilogue(const FinalizeParams& f, double* s
 
 // Whole-warp path for rows longer than the register budget: every pass re-reads the row (L1/L2 resident).
 template <int M, bool LAM_SMEM, bool ACC_SMEM>
-__device__ __noinline__ void long_row(const GradParams& p, const double* s_lam, unsigned* s_lo, unsigned* s_hi,
-                                      long long beg, long long end, float& obj_l, float& sq_l) {
+__device__ __noinline__ void long_row(const GradParams& p, const double* s_lam, double mu, unsigned* s_lo, unsigned* s_hi,
+                                      long long beg, long long end, long long& obj_l, long long& sq_l, long long& cnt_l) {
     const int lane = threadIdx.x & 31;
     const int mm = p.m;
     int j; float cc; float aa[M > 0 ? M : 4];
     float wmax = -CUDART_INF_F;
     for (long long q = beg + lane; q < end; q += 32)
-        wmax = fmaxf(wmax, (float)(-eval_t<M, LAM_SMEM>(p, s_lam, q, mm, j, cc, aa)));
+        wmax = fmaxf(wmax, (float)(-eval_t<M, LAM_SMEM>(p, s_lam, mu, q, mm, j, cc, aa)));
     const float m32 = group_max<32>(wmax);
     const bool ineq = p.proj != PROJ_SIMPLEX_EQ;
     if (ineq && !(m32 > 0.0f)) {
@@ -272,7 +313,7 @@ __device__ __noinline__ void long_row(const GradParams& p, const double* s_lam, 
         for (;;) {
             float s = 0.0f; int n = 0;
             for (long long q = beg + lane; q < end; q += 32) {
-                const float u = (float)(-eval_t<M, LAM_SMEM>(p, s_lam, q, mm, j, cc, aa) - md) * p.inv_gamma_f;
+                const float u = (float)(-eval_t<M, LAM_SMEM>(p, s_lam, mu, q, mm, j, cc, aa) - md) * p.inv_gamma_f;
                 if (u > theta) { s += u; ++n; }
             }
             s = group_sum<32>(s); n = group_sum_i<32>(n);
@@ -287,7 +328,7 @@ __device__ __noinline__ void long_row(const GradParams& p, const double* s_lam, 
         const double ig = p.inv_gamma;
         float s0 = 0.0f;
         for (long long q = beg + lane; q < end; q += 32)
-            s0 += fminf(fmaxf((float)(-eval_t<M, LAM_SMEM>(p, s_lam, q, mm, j, cc, aa) * ig), 0.0f), ub);
+            s0 += fminf(fmaxf((float)(-eval_t<M, LAM_SMEM>(p, s_lam, mu, q, mm, j, cc, aa) * ig), 0.0f), ub);
         s0 = group_sum<32>(s0);
         if (s0 <= z) { ref = 0.0; tau = 0.0f; }
         else {
@@ -296,7 +337,7 @@ __device__ __noinline__ void long_row(const GradParams& p, const double* s_lam, 
                 const float mid = 0.5f * (lo + hi);
                 float s = 0.0f;
                 for (long long q = beg + lane; q < end; q += 32) {
-                    const float u = (float)(-eval_t<M, LAM_SMEM>(p, s_lam, q, mm, j, cc, aa) - md) * p.inv_gamma_f;
+                    const float u = (float)(-eval_t<M, LAM_SMEM>(p, s_lam, mu, q, mm, j, cc, aa) - md) * p.inv_gamma_f;
                     s += fminf(fmaxf(u - mid, 0.0f), ub);
                 }
                 s = group_sum<32>(s);
@@ -310,7 +351,7 @@ __device__ __noinline__ void long_row(const GradParams& p, const double* s_lam, 
                 const float mid = 0.5f * (dlo + dhi);
                 float s = 0.0f;
                 for (long long q = beg + lane; q < end; q += 32) {
-                    const float u = (float)(-eval_t<M, LAM_SMEM>(p, s_lam, q, mm, j, cc, aa) * ig - ref);
+                    const float u = (float)(-eval_t<M, LAM_SMEM>(p, s_lam, mu, q, mm, j, cc, aa) * ig - ref);
                     s += fminf(fmaxf(u - mid, 0.0f), ub);
                 }
                 s = group_sum<32>(s);
@@ -319,7 +360,7 @@ __device__ __noinline__ void long_row(const GradParams& p, const double* s_lam, 
             const float mid = 0.5f * (dlo + dhi);
             float sF = 0.0f; int nF = 0, nU = 0;
             for (long long q = beg + lane; q < end; q += 32) {
-                const float u = (float)(-eval_t<M, LAM_SMEM>(p, s_lam, q, mm, j, cc, aa) * ig - ref);
+                const float u = (float)(-eval_t<M, LAM_SMEM>(p, s_lam, mu, q, mm, j, cc, aa) * ig - ref);
                 const float d = u - mid;
                 if (d >= ub) ++nU; else if (d > 0.0f) { sF += u; ++nF; }
             }
@@ -333,13 +374,12 @@ __device__ __noinline__ void long_row(const GradParams& p, const double* s_lam, 
     }
     const float cap = p.general_boxcut ? p.ub : CUDART_INF_F;
     for (long long q = beg + lane; q < end; q += 32) {
-        const double tq = eval_t<M, LAM_SMEM>(p, s_lam, q, mm, j, cc, aa);
+        const double tq = eval_t<M, LAM_SMEM>(p, s_lam, mu, q, mm, j, cc, aa);
         const float u = p.general_boxcut ? (float)(-tq * p.inv_gamma - ref) : (float)(-tq - md) * p.inv_gamma_f;
         const float x = fminf(fmaxf(u - tau, 0.0f), cap);
         if (p.x) p.x[q] = x;
         if (x > 0.0f) {
-            obj_l = fmaf(cc, x, obj_l);
-            sq_l = fmaf(x, x, sq_l);
+            obj_l += to_fix(cc * x, p.scale_obj); sq_l += to_fix(x * x, p.scale_sq); cnt_l += to_fix(x, p.scale_cnt);
             contribute<M, ACC_SMEM>(p, s_lo, s_hi, mm, j, aa, x);
         }
     }
@@ -366,7 +406,10 @@ __global__ void __launch_bounds__(kBlockThreads, 1) k_grad(const GradParams p, c
     const long long nsteps = (p.I + RPW - 1) / RPW;
     const bool ineq = p.proj != PROJ_SIMPLEX_EQ;
     const float z = p.z;
-    float obj_l = 0.0f, sq_l = 0.0f;
+    // per-lane partial scalars, every product converted to fixed point on its own: the sums do not depend on which lane
+    // or CTA a row lands on (bit-reproducible for any launch geometry, like the item sums)
+    long long obj_l = 0, sq_l = 0, cnt_l = 0;
+    const double mu = p.count_on ? __ldg(p.lambda + JM) : 0.0;      // dual of the global-count row (R21)
 
     for (long long step = (long long)blockIdx.x * kWarpsPerBlock + warp; step < nsteps;
          step += (long long)gridDim.x * kWarpsPerBlock) {
@@ -409,7 +452,7 @@ __global__ void __launch_bounds__(kBlockThreads, 1) k_grad(const GradParams p, c
                 if (k >= nch_max) break;
                 double tk = CUDART_INF;
                 if (k * G + gl < flen) {
-                    tk = (double)cc[k];
+                    tk = (double)cc[k] + mu;
 #pragma unroll
                     for (int f = 0; f < MA; ++f) {
                         if (f < mm) {
@@ -533,8 +576,7 @@ __global__ void __launch_bounds__(kBlockThreads, 1) k_grad(const GradParams p, c
                 const int e = k * G + gl;
                 if (p.x && e < flen) p.x[beg + e] = x;
                 if (x > 0.0f) {
-                    obj_l = fmaf(cc[k], x, obj_l);
-                    sq_l = fmaf(x, x, sq_l);
+                    obj_l += to_fix(cc[k] * x, p.scale_obj); sq_l += to_fix(x * x, p.scale_sq); cnt_l += to_fix(x, p.scale_cnt);
                     contribute<M, ACC_SMEM>(p, s_lo, s_hi, mm, jj[k], aa[k], x);
                 }
             }
@@ -545,20 +587,21 @@ __global__ void __launch_bounds__(kBlockThreads, 1) k_grad(const GradParams p, c
             const int src = __ffs(long_mask) - 1;
             long_mask &= long_mask - 1;
             const long long b = __shfl_sync(kFull, beg, src), e = __shfl_sync(kFull, end, src);
-            long_row<M, LAM_SMEM, ACC_SMEM>(p, s_lam, s_lo, s_hi, b, e, obj_l, sq_l);
+            long_row<M, LAM_SMEM, ACC_SMEM>(p, s_lam, mu, s_lo, s_hi, b, e, obj_l, sq_l, cnt_l);
         }
     }
 
-    // a5: per-lane fp32 partials -> fixed point (lane order is fixed by the static row assignment)
+    // a5: per-lane fixed-point partials -> one atomic per warp and scalar
     {
-        const long long fo = __double2ll_rn((double)obj_l * p.scale_obj);
-        const long long fs = __double2ll_rn((double)sq_l * p.scale_sq);
-        long long so = fo, ss = fs;
+        long long so = obj_l, ss = sq_l, sn = cnt_l;
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) { so += __shfl_xor_sync(kFull, so, o); ss += __shfl_xor_sync(kFull, ss, o); }
+        for (int o = 16; o > 0; o >>= 1) {
+            so += __shfl_xor_sync(kFull, so, o); ss += __shfl_xor_sync(kFull, ss, o); sn += __shfl_xor_sync(kFull, sn, o);
+        }
         if (lane == 0) {
             if (so) atomicAdd(p.sc_fix + 0, (unsigned long long)so);
             if (ss) atomicAdd(p.sc_fix + 1, (unsigned long long)ss);
+            if (sn) atomicAdd(p.sc_fix + 2, (unsigned long long)sn);
         }
     }
     if (ACC_SMEM) {
@@ -577,25 +620,28 @@ template <int M>
 __global__ void __launch_bounds__(256) k_grad_box(const GradParams p, const FinalizeParams f) {
     __shared__ double sh_fin[kFinalizeScratchBytes / 8];
     const int mm = M > 0 ? M : p.m;
-    float obj_l = 0.0f, sq_l = 0.0f;
+    long long obj_l = 0, sq_l = 0, cnt_l = 0;
+    const double mu = p.count_on ? __ldg(p.lambda + (long long)p.J * mm) : 0.0;
     for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < p.nnz; q += (long long)gridDim.x * blockDim.x) {
         int j; float cc; float aa[M > 0 ? M : 4];
-        const double t = eval_t<M, false>(p, nullptr, q, mm, j, cc, aa);
+        const double t = eval_t<M, false>(p, nullptr, mu, q, mm, j, cc, aa);
         const double v = -t * p.inv_gamma;
         const float x = (float)fmin(fmax(v, p.box_lo), p.box_hi);
         if (p.x) p.x[q] = x;
         if (x != 0.0f) {
-            obj_l = fmaf(cc, x, obj_l);
-            sq_l = fmaf(x, x, sq_l);
+            obj_l += to_fix(cc * x, p.scale_obj); sq_l += to_fix(x * x, p.scale_sq); cnt_l += to_fix(x, p.scale_cnt);
             contribute<M, false>(p, nullptr, nullptr, mm, j, aa, x);
         }
     }
-    long long so = __double2ll_rn((double)obj_l * p.scale_obj), ss = __double2ll_rn((double)sq_l * p.scale_sq);
+    long long so = obj_l, ss = sq_l, sn = cnt_l;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) { so += __shfl_xor_sync(kFull, so, o); ss += __shfl_xor_sync(kFull, ss, o); }
+    for (int o = 16; o > 0; o >>= 1) {
+        so += __shfl_xor_sync(kFull, so, o); ss += __shfl_xor_sync(kFull, ss, o); sn += __shfl_xor_sync(kFull, sn, o);
+    }
     if ((threadIdx.x & 31) == 0) {
         if (so) atomicAdd(p.sc_fix + 0, (unsigned long long)so);
         if (ss) atomicAdd(p.sc_fix + 1, (unsigned long long)ss);
+        if (sn) atomicAdd(p.sc_fix + 2, (unsigned long long)sn);
     }
     grid_epilogue(f, sh_fin, 256);
 }

@@ -15,13 +15,16 @@ _KIND = {"simplex": (oracle.PROJ_SIMPLEX_INEQ, pkg.PROJ_SIMPLEX_INEQ), "box": (o
          "boxcut": (oracle.PROJ_BOXCUT, pkg.PROJ_BOXCUT), "simplex_eq": (oracle.PROJ_SIMPLEX_EQ, pkg.PROJ_SIMPLEX_EQ)}
 
 
-def both(d, kind="simplex", p0=1.0, p1=0.0, **opt):
-    """d: dict of numpy arrays (I,J,m,row_ptr,item_idx,c,a,b) -> (oracle.Problem, pkg.Problem)."""
+def both(d, kind="simplex", p0=1.0, p1=0.0, count_M=None, **opt):
+    """d: dict of numpy arrays (I,J,m,row_ptr,item_idx,c,a,b) -> (oracle.Problem, pkg.Problem).  count_M: right-hand side of
+    the global-count row sum x <= M (R21) on both sides, or None."""
     ko, kg = _KIND[kind]
-    po = oracle.Problem(d["I"], d["J"], d["m"], d["row_ptr"], d["item_idx"], d["c"], d["a"], d["b"], ko, p0, p1)
+    po = oracle.Problem(d["I"], d["J"], d["m"], d["row_ptr"], d["item_idx"], d["c"], d["a"], d["b"], ko, p0, p1, count_M)
     t = {k: torch.from_numpy(np.ascontiguousarray(getattr(po, k))).cuda() for k in ("row_ptr", "item_idx", "c", "a", "b")}
     pg = pkg.Problem.create(po.I, po.J, po.m, t["row_ptr"], t["item_idx"], t["c"], t["a"], t["b"],
                             pkg.binding.make_opts(projection=kg, p0=p0, p1=p1, **opt))
+    if count_M is not None:
+        pg.set_global_count(count_M)
     return po, pg
 
 
@@ -34,7 +37,7 @@ def from_instance(inst: synth.Instance, **opt):
 
 def gpu_grad(pg, lam, gamma, want_x=True):
     lam_t = torch.as_tensor(np.asarray(lam, dtype=np.float64)).cuda()
-    grad = torch.empty(pg.J * pg.m, dtype=torch.float64, device="cuda")
+    grad = torch.empty(pg.duals, dtype=torch.float64, device="cuda")
     x = torch.empty(pg.nnz, dtype=torch.float32, device="cuda") if want_x else None
     sc = pkg.Scalars()
     pg.grad(lam_t, gamma, grad=grad, scalars=sc, x=x)
@@ -47,8 +50,8 @@ def rel_l2(a, b):
     return np.linalg.norm(a - b) / (nb if nb > 0 else 1.0)
 
 
-def assert_grad_parity(po, pg, lam, gamma, tag=""):
-    ref = oracle.grad(po, lam, gamma)
+def assert_grad_parity(po, pg, lam, gamma, tag="", is_eq=None):
+    ref = oracle.grad(po, lam, gamma, is_eq=is_eq)
     sc, grad, x = gpu_grad(pg, lam, gamma)
     ex = np.abs(x.astype(np.float64) - ref.x).max() if ref.x.size else 0.0
     eg = rel_l2(grad, ref.grad)
@@ -60,11 +63,13 @@ def assert_grad_parity(po, pg, lam, gamma, tag=""):
     assert abs(sc.reg - ref.reg) <= TOL_G * max(abs(ref.reg), 1e-12) + 1e-9, f"{tag} reg {sc.reg} vs {ref.reg}"
     assert abs(sc.r_inf - ref.r_inf) <= TOL_GRAD * np.linalg.norm(ref.grad) + 1e-12, f"{tag} r_inf"
     assert abs(sc.r_2 - ref.r_2) <= TOL_GRAD * np.linalg.norm(ref.grad) + 1e-12, f"{tag} r_2"
+    # gap = (obj + reg) - g = -lambda'grad (Table 4): absolute against the size of the terms it is the difference of
+    assert abs(sc.gap - ref.gap) <= TOL_G * (abs(ref.obj) + abs(ref.reg) + abs(ref.g)) + 1e-9, f"{tag} gap {sc.gap} vs {ref.gap}"
     return ex, eg
 
 
 def gpu_solve(pg, gammas, iters, lam0=None, want_trace=True, want_x=True):
-    Jm, T = pg.J * pg.m, int(np.sum(iters))
+    Jm, T = pg.duals, int(np.sum(iters))
     lam = torch.zeros(Jm, dtype=torch.float64, device="cuda") if lam0 is None else torch.as_tensor(lam0).double().cuda().clone()
     x = torch.empty(pg.nnz, dtype=torch.float32, device="cuda") if want_x else None
     grad = torch.empty(Jm, dtype=torch.float64, device="cuda")
@@ -72,22 +77,29 @@ def gpu_solve(pg, gammas, iters, lam0=None, want_trace=True, want_x=True):
     if want_trace:
         tr = {"g": torch.empty(T, dtype=torch.float64, device="cuda"), "r_inf": torch.empty(T, dtype=torch.float64, device="cuda"),
               "r_2": torch.empty(T, dtype=torch.float64, device="cuda"), "grad": torch.empty(T * Jm, dtype=torch.float64, device="cuda"),
-              "lambda": torch.empty(T * Jm, dtype=torch.float64, device="cuda")}
+              "lambda": torch.empty(T * Jm, dtype=torch.float64, device="cuda"), "eta": torch.empty(T, dtype=torch.float64, device="cuda")}
     sc = pkg.Scalars()
     pg.solve(gammas, iters, lam, x=x, scalars=sc, grad=grad, trace=tr)
     torch.cuda.synchronize()
     out = {"lam": lam.cpu().numpy(), "x": x.cpu().numpy() if want_x else None, "grad": grad.cpu().numpy(), "sc": sc}
     if tr:
         out.update(tr_g=tr["g"].cpu().numpy(), tr_grad=tr["grad"].cpu().numpy().reshape(T, Jm),
-                   tr_lam=tr["lambda"].cpu().numpy().reshape(T, Jm), tr_rinf=tr["r_inf"].cpu().numpy(), tr_r2=tr["r_2"].cpu().numpy())
+                   tr_lam=tr["lambda"].cpu().numpy().reshape(T, Jm), tr_rinf=tr["r_inf"].cpu().numpy(), tr_r2=tr["r_2"].cpu().numpy(),
+                   tr_eta=tr["eta"].cpu().numpy())
     return out
 
 
-def assert_trajectory_parity(po, pg, gammas, iters, lam0=None, momentum=True, tag="", jacobi=False):
+def assert_trajectory_parity(po, pg, gammas, iters, lam0=None, momentum=True, tag="", jacobi=False, is_eq=None, adaptive=None):
     """Independent solves compared per iteration (parity mode B of SURVEY 8(c)).  jacobi: the oracle iterates on the
-    literally row-scaled system; pg must have been created with jacobi=True (per-coordinate step)."""
-    ref = oracle.solve(po, gammas, iters, lam0=lam0, momentum=momentum, trace_grad=True, trace_lambda=True, jacobi=jacobi)
+    literally row-scaled system; pg must have been created with jacobi=True (per-coordinate step).
+    is_eq: equality-row mask (pg.set_equality_rows must have been called with it).  adaptive: (eta_min, eta_max) of the
+    range-clipped secant step (R20; pg created with adaptive=True and the same range) -- the per-iteration eta is compared."""
+    kw = dict(adaptive=True, eta_min=adaptive[0], eta_max=adaptive[1]) if adaptive else {}
+    ref = oracle.solve(po, gammas, iters, lam0=lam0, momentum=momentum, trace_grad=True, trace_lambda=True, jacobi=jacobi,
+                       is_eq=is_eq, **kw)
     out = gpu_solve(pg, gammas, iters, lam0=lam0)
+    if adaptive:
+        assert np.abs(out["tr_eta"] / ref.trace_eta - 1.0).max() <= 1e-6, f"{tag} eta trace"
     T = int(np.sum(iters))
     worst = 0.0
     for n in range(T):
@@ -99,6 +111,10 @@ def assert_trajectory_parity(po, pg, gammas, iters, lam0=None, momentum=True, ta
     assert ex <= TOL_X, f"{tag} final x abs err {ex:.3e}"
     assert abs(out["sc"].g - ref.final.g) <= TOL_G * abs(ref.final.g) + 1e-12, f"{tag} final g"
     assert rel_l2(out["grad"], ref.final.grad) <= TOL_GRAD, f"{tag} final grad"
+    gn = np.linalg.norm(ref.final.grad)
+    assert abs(out["sc"].r_inf - ref.final.r_inf) <= TOL_GRAD * gn + 1e-12, f"{tag} final r_inf"
+    assert abs(out["sc"].r_2 - ref.final.r_2) <= TOL_GRAD * gn + 1e-12, f"{tag} final r_2"
+    assert abs(out["sc"].gap - ref.final.gap) <= TOL_G * (abs(ref.final.obj) + abs(ref.final.reg) + abs(ref.final.g)) + 1e-9, f"{tag} final gap"
     lam_scale = max(np.abs(ref.lam).max(), 1e-300)
     assert np.abs(out["lam"] - ref.lam).max() <= 1e-6 * lam_scale + 1e-12, f"{tag} lambda_T"
     el = np.abs(out["tr_lam"] - ref.trace_lambda).max()

@@ -35,15 +35,16 @@ def test_library_exports_every_declared_symbol():
 
 def test_struct_mirrors_match_the_header():
     import paper_2606_07777_b200 as pkg
-    assert ctypes.sizeof(pkg.Scalars) == 5 * 8
+    assert ctypes.sizeof(pkg.Scalars) == 6 * 8
     o = pkg.binding.make_opts()
     assert (o.projection, o.p0, o.reduction, o.borrow, o.validate, o.momentum) == (0, 1.0, 0, 0, 1, 1)
     # sizes and field offsets as gcc lays out include/dualip.h, against the ctypes mirrors
     import subprocess, tempfile
-    fields = {"dualip_opts": ["projection", "p0", "reduction", "use_graph", "reserved", "precondition"],
+    fields = {"dualip_opts": ["projection", "p0", "reduction", "use_graph", "tuning", "precondition", "step_rule", "eta_min", "eta_max"],
               "dualip_info": ["I", "L", "group_lanes", "smem_bytes", "fix_scale_s", "streaming", "ntiles", "grad_kernel_count",
-                              "precondition", "L_step"],
-              "dualip_scalars": ["g", "r_2"], "dualip_trace": ["capacity", "lambda"]}
+                              "precondition", "L_step", "duals", "lambda_lo_smem"],
+              "dualip_scalars": ["g", "r_2", "gap"], "dualip_trace": ["capacity", "lambda", "eta"],
+              "dualip_tuning": ["direct_kernel", "stages", "tile_units", "lambda_plan"]}
     src = '#include <stdio.h>\n#include <stddef.h>\n#include "dualip.h"\nint main(void){\n'
     for st, fl in fields.items():
         src += f'printf("{st} %zu\\n", sizeof({st}));\n'
@@ -55,7 +56,8 @@ def test_struct_mirrors_match_the_header():
         open(cpath, "w").write(src)
         subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), "-o", exe, cpath])
         got = dict(line.split() for line in subprocess.check_output([exe]).decode().splitlines())
-    mirrors = {"dualip_opts": pkg.Opts, "dualip_info": pkg.Info, "dualip_scalars": pkg.Scalars, "dualip_trace": pkg.binding._Trace}
+    mirrors = {"dualip_opts": pkg.Opts, "dualip_info": pkg.Info, "dualip_scalars": pkg.Scalars, "dualip_trace": pkg.binding._Trace,
+               "dualip_tuning": pkg.binding.Tuning}
     rename = {"lambda": "lam"}
     for st, fl in fields.items():
         assert int(got[st]) == ctypes.sizeof(mirrors[st]), st

@@ -862,7 +862,13 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const __grid_con
                             const float thr = __shfl_sync(kFull, thr_own, src);
                             const unsigned okb = __ballot_sync(kFull, !(rm2[r] > thr));
                             const bool rowA = rw && (okb & gmask) == gmask;
-                            const bool needB = rw && !rowA;
+                            // (B) holds up to 2G candidates.  The filter already knows a lower bound on their number (lanes whose
+                            // largest / second largest value is one); when that alone reaches 2G on a row longer than 2G -- a
+                            // dense row: gamma of the order of the spread of w -- the re-scan would only find out that the row
+                            // does not fit, so it goes to the slow path directly.  The test reads the row's own data only.
+                            const unsigned c1b = __ballot_sync(kFull, rm1[r] > thr);
+                            const bool dense = __popc(~okb & gmask) + __popc(c1b & gmask) >= 2 * G && rlen[r] > 2 * G;
+                            const bool needB = rw && !rowA && !dense;
                             bool row_ok = rowA;
                             int cp0 = (rowA && rm1[r] > thr) ? rpos[r] : -1, cp1 = -1;
                             if (__any_sync(kFull, needB)) {

@@ -18,7 +18,7 @@ pytestmark = pytest.mark.gpu
 
 if torch.cuda.is_available():
     import paper_2606_07777_b200 as pkg
-    from gpu_util import assert_grad_parity, assert_trajectory_parity, both, from_instance, gpu_grad, gpu_solve, rel_l2
+    from gpu_util import assert_adaptive_step_parity, assert_grad_parity, assert_trajectory_parity, both, from_instance, gpu_grad, gpu_solve, rel_l2
     from test_gpu_parity import _ragged
 
 
@@ -37,8 +37,8 @@ def test_adaptive_step_trajectory(jacobi, kernel):
     gam, its = [0.4, 0.04, 0.004], [25, 25, 25]
     rng_eta = (0.5 * gam[0] / L, 30.0 * gam[0] / L)       # the secant step runs at 12..55 x gamma / L on this instance
     po, pg = both(d, jacobi=jacobi, adaptive=True, eta_min=rng_eta[0], eta_max=rng_eta[1], direct_kernel=(kernel == "direct"))
-    worst, ex, ref, out = assert_trajectory_parity(po, pg, gam, its, tag=f"adaptive/{kernel}/jacobi={jacobi}", jacobi=jacobi, adaptive=rng_eta)
-    eta = ref.trace_eta
+    ref, out = assert_adaptive_step_parity(po, pg, gam, its, rng_eta, jacobi=jacobi, tag=f"adaptive/{kernel}/jacobi={jacobi}")
+    eta = out["tr_eta"]
     assert (eta[1:25] > rng_eta[0] * 1.001).any() and (eta[1:25] < rng_eta[1] * 0.999).any()      # really adaptive somewhere
     assert np.all(eta[-25:] == rng_eta[1] * gam[2] / gam[0])                                       # the scaled maximum wins
     assert (ref.lam > 0).sum() >= 5
@@ -65,7 +65,7 @@ def test_adaptive_on_a_scaled_config_with_graph_replay():
     inst = synth.generate(cfg)
     rng_eta = (1e-5, 1e-1)
     po, pg = from_instance(inst, jacobi=True, adaptive=True, eta_min=rng_eta[0], eta_max=rng_eta[1], use_graph=True, group_lanes=8)
-    assert_trajectory_parity(po, pg, [1e-1, 1e-2], [45, 45], tag="cfg3-tight/adaptive+graph", jacobi=True, adaptive=rng_eta)
+    assert_adaptive_step_parity(po, pg, [1e-1, 1e-2], [45, 45], rng_eta, jacobi=True, tag="cfg3-tight/adaptive+graph")
     pg.destroy()
 
 

@@ -85,6 +85,7 @@ def parse_args():
     ap.add_argument("--grid-ctas", type=int, default=0, help="CTAs of the gradient kernel (0 = the library's choice)")
     ap.add_argument("--reduction", default="auto", choices=["auto", "smem", "global", "csc"], help="item-reduction strategy (DUALIP_RED_*)")
     ap.add_argument("--lambda-plan", type=int, default=0, help="streaming kernel's exact-path dual operand: 0 per launch, 1 never stage the low word, 2 always")
+    ap.add_argument("--step-deal", type=int, default=0, help="row-steps dealt 0 = the library's choice, 1 = statically, 2 = dynamically")
     ap.add_argument("--graph", action="store_true", help="dualip_solve replays a CUDA graph of chained iteration launches "
                     "(small, launch-bound workloads); the per-launch kernel timing hook is then off")
     ap.add_argument("--no-e2e", action="store_true")
@@ -270,7 +271,7 @@ class Leg:
         a = self.args
         return self.pkg.binding.make_opts(projection=self.proj, p0=self.p0, p1=self.p1, borrow=borrow, group_lanes=a.group_lanes,
                                           grid_ctas=a.grid_ctas, stages=a.stages, tile_units=a.tile_units, use_graph=a.graph,
-                                          jacobi=self.jacobi, adaptive=self.adaptive, lambda_plan=a.lambda_plan,
+                                          jacobi=self.jacobi, adaptive=self.adaptive, lambda_plan=a.lambda_plan, step_deal=a.step_deal,
                                           reduction={"auto": 0, "smem": 1, "global": 2, "csc": 3}[a.reduction])
 
     def start_lambda(self):

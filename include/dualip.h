@@ -92,6 +92,8 @@ typedef struct {
     int32_t tile_units;    /* cap on its tile size in units (>= 256) */
     int32_t lambda_plan;   /* exact-path dual operand of the streaming kernel: 0 = chosen per launch, 1 = never stage
                               lambda's low word in shared memory, 2 = always stage it when it fits */
+    int32_t step_deal;     /* how a tile's row-steps are dealt to the consumer warps: 0 = the library's choice, 1 = statically
+                              (round-robin over the CTA's step sequence), 2 = dynamically (claimed from a counter) */
 } dualip_tuning;
 
 typedef struct {
@@ -168,6 +170,8 @@ typedef struct {
                                 (+ |count row|^2 with the global-count row: nnz, or 1 with JACOBI) */
     int32_t duals;           /* length of lambda / grad vectors: J*m, or J*m + 1 with the global-count row */
     int32_t lambda_lo_smem;  /* streaming kernel: 1 if the LAST launch staged lambda's low word in shared memory */
+    int32_t checked_build;   /* 1: the library was compiled with -DDUALIP_CHECKED (in-kernel bounds assertions; tests only) */
+    int32_t checks_failed;   /* checked build: bit mask of the kinds of bounds violation seen so far (0 = none); else 0 */
 } dualip_info;
 
 /*
@@ -230,6 +234,50 @@ int dualip_set_equality_rows(dualip_t* h, const uint8_t* is_equality, void* stre
  * (dualip_info.duals).  The step constant becomes L_step + nnz (|A|_2^2 <= |A_items|_2^2 + |1|_2^2), or L' + 1 under JACOBI,
  * where the row is normalised like any other (d^2 = 1/nnz).  Switching the row on or off clears the equality mask. */
 int dualip_set_global_count(dualip_t* h, int32_t enable, double M, void* stream);
+
+/* ---- user-sharded multi-GPU (section 4.4: sources split across GPUs, lambda and b replicated, one |lambda|-sized
+ * reduction per iteration; Fig. 3) ------------------------------------------------------------------------------
+ * One handle per GPU holds a contiguous range of users.  The item sums are 64-bit FIXED-POINT integers, so the cross-GPU
+ * reduction is an integer sum: with the same fixed-point scales on every shard (dualip_set_shard_constants) the all-reduced
+ * accumulators -- and hence grad g, g, and every rank's AGD update -- are bit-identical on all ranks and to one GPU holding
+ * all users.  No rank-0 update, no broadcast (the paper reduces to rank 0 and broadcasts lambda).  The library does
+ * not talk to NCCL: the caller's hook does the all-reduce (the Python binding uses torch.distributed).
+ *
+ * Accumulator layout (int64 words, dualip_info.duals' item part first): [J*m item sums a'x][c'x][|x|^2][sum x].           */
+
+/* Called between the gradient kernel and the epilogue of EVERY evaluation (dualip_grad, each iteration and the final evaluation
+ * of dualip_solve) once set: must leave in accumulators_dev[0..n_words) the sum over all shards, enqueued on `stream`
+ * (e.g. ncclAllReduce(int64, sum) in place).  lambda_eval_dev / gamma: the point being evaluated (identical on all ranks). */
+typedef void (*dualip_reduce_hook)(void* user, int64_t* accumulators_dev, int64_t n_words, const double* lambda_eval_dev,
+                                   double gamma, void* stream);
+/* fn = NULL removes the hook.  While a hook is set, CUDA-graph replay is off (the hook runs on the host between launches). */
+int dualip_set_reduce_hook(dualip_t* h, dualip_reduce_hook fn, void* user);
+
+/* Create-time constants (a0) of a sharded problem.  Everything a0 derives from the rows -- L (R2), the Jacobi factors
+ * (R18), the fixed-point scales -- comes from per-item column sums that are themselves accumulated in fixed point, so they
+ * can be made EXACTLY those of the unsharded problem with two integer all-reduces:
+ *   1. dualip_get_shard_extents on every shard; all-reduce I and nnz (SUM), max_abs_a and max_abs_c (MAX) -> global extents;
+ *   2. dualip_get_column_stats(h, &global, out): this shard's column sums in the fixed-point scales the GLOBAL extents imply,
+ *      out[0..J*m) = sum_i (a^k_ij)^2, out[J*m..2J*m) = sum_i |a^k_ij|, out[2J*m] = sum |c|;  all-reduce (int64 SUM);
+ *   3. dualip_set_shard_constants(h, &global, summed) on every shard: L, L_step, the Jacobi factors and the scales are derived
+ *      from the summed integers exactly as dualip_create derives them on one GPU.
+ * dualip_set_c recomputes sum |c| from the shard alone: repeat 2-3 afterwards. */
+typedef struct {
+    int64_t I, nnz;                 /* users, nonzeros */
+    float   max_abs_a, max_abs_c;
+} dualip_shard_extents;
+int dualip_get_shard_extents(dualip_t* h, dualip_shard_extents* out);
+int dualip_get_column_stats(dualip_t* h, const dualip_shard_extents* global, int64_t* out /* 2*J*m + 1, host or device */, void* stream);
+int dualip_set_shard_constants(dualip_t* h, const dualip_shard_extents* global, const int64_t* summed /* 2*J*m + 1, host or device */,
+                               void* stream);
+
+/* Pieces the hook-less emulation and the tests use.  dualip_eval_partial: a1-a3 + this shard's part of a4-a5 only (the
+ * gradient kernel without its epilogue) at `lambda` (device), leaving the accumulators in the handle; x may be NULL.
+ * dualip_export_accumulators: copies the duals' item part + 3 scalar words out (host or device) and, with clear != 0, zeroes
+ * them.  dualip_import_accumulators: overwrites them (accumulate = 0) or adds to them (accumulate != 0). */
+int dualip_eval_partial(dualip_t* h, const double* lambda_dev, double gamma, float* x, void* stream);
+int dualip_export_accumulators(dualip_t* h, int64_t* out, int32_t clear, void* stream);
+int dualip_import_accumulators(dualip_t* h, const int64_t* in, int32_t accumulate, void* stream);
 
 /* DUALIP_RED_CSC only (else DUALIP_EUNSUPPORTED): copies out the item-sorted permutation built at create (a0).
  *   col_ptr_out[J+1] int64: column j's entries are perm[col_ptr[j] .. col_ptr[j+1]);

@@ -18,7 +18,9 @@ PRECOND_NONE, PRECOND_JACOBI = 0, 1
 STEP_FIXED, STEP_ADAPTIVE = 0, 1
 
 EXPORTED_SYMBOLS = ("dualip_opts_default", "dualip_create", "dualip_grad", "dualip_solve", "dualip_set_c",
-                    "dualip_set_equality_rows", "dualip_set_global_count", "dualip_set_profiling", "dualip_get_info", "dualip_get_csc", "dualip_destroy",
+                    "dualip_set_equality_rows", "dualip_set_global_count", "dualip_set_reduce_hook", "dualip_get_shard_extents",
+                    "dualip_get_column_stats", "dualip_set_shard_constants", "dualip_eval_partial", "dualip_export_accumulators",
+                    "dualip_import_accumulators", "dualip_set_profiling", "dualip_get_info", "dualip_get_csc", "dualip_destroy",
                     "dualip_strerror")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -32,7 +34,7 @@ class DualipError(RuntimeError):
 
 class Tuning(ctypes.Structure):
     _fields_ = [("direct_kernel", ctypes.c_int32), ("stages", ctypes.c_int32), ("tile_units", ctypes.c_int32),
-                ("lambda_plan", ctypes.c_int32)]
+                ("lambda_plan", ctypes.c_int32), ("step_deal", ctypes.c_int32)]
 
 
 class Opts(ctypes.Structure):
@@ -51,6 +53,14 @@ class Scalars(ctypes.Structure):
         return {k: getattr(self, k) for k, _ in self._fields_}
 
 
+class ShardExtents(ctypes.Structure):
+    _fields_ = [("I", ctypes.c_int64), ("nnz", ctypes.c_int64), ("max_abs_a", ctypes.c_float), ("max_abs_c", ctypes.c_float)]
+
+
+# void hook(void* user, int64_t* accumulators_dev, int64_t n_words, const double* lambda_eval_dev, double gamma, void* stream)
+REDUCE_HOOK = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_double, ctypes.c_void_p)
+
+
 class _Trace(ctypes.Structure):
     _fields_ = [("capacity", ctypes.c_int64), ("g", ctypes.c_void_p), ("r_inf", ctypes.c_void_p),
                 ("r_2", ctypes.c_void_p), ("grad", ctypes.c_void_p), ("lam", ctypes.c_void_p), ("eta", ctypes.c_void_p)]
@@ -65,7 +75,8 @@ class Info(ctypes.Structure):
                 ("streaming", ctypes.c_int32), ("stages", ctypes.c_int32), ("tile_units", ctypes.c_int64), ("ntiles", ctypes.c_int64),
                 ("grad_kernel_ms", ctypes.c_double), ("grad_kernel_count", ctypes.c_int64),
                 ("precondition", ctypes.c_int32), ("pad0", ctypes.c_int32), ("L_step", ctypes.c_double),
-                ("duals", ctypes.c_int32), ("lambda_lo_smem", ctypes.c_int32)]
+                ("duals", ctypes.c_int32), ("lambda_lo_smem", ctypes.c_int32), ("checked_build", ctypes.c_int32),
+                ("checks_failed", ctypes.c_int32)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -97,6 +108,13 @@ def load_library():
         lib.dualip_set_c.argtypes = [vp, vp, vp]
         lib.dualip_set_equality_rows.argtypes = [vp, vp, vp]
         lib.dualip_set_global_count.argtypes = [vp, i32, d, vp]
+        lib.dualip_set_reduce_hook.argtypes = [vp, REDUCE_HOOK, vp]
+        lib.dualip_get_shard_extents.argtypes = [vp, ctypes.POINTER(ShardExtents)]
+        lib.dualip_get_column_stats.argtypes = [vp, ctypes.POINTER(ShardExtents), vp, vp]
+        lib.dualip_set_shard_constants.argtypes = [vp, ctypes.POINTER(ShardExtents), vp, vp]
+        lib.dualip_eval_partial.argtypes = [vp, vp, d, vp, vp]
+        lib.dualip_export_accumulators.argtypes = [vp, vp, i32, vp]
+        lib.dualip_import_accumulators.argtypes = [vp, vp, i32, vp]
         lib.dualip_get_info.argtypes = [vp, ctypes.POINTER(Info)]
         lib.dualip_set_profiling.argtypes = [vp, ctypes.c_int]
         lib.dualip_get_csc.argtypes = [vp, vp, vp, vp]
@@ -106,7 +124,9 @@ def load_library():
         lib.dualip_strerror.argtypes = [ctypes.c_int]
         lib.dualip_strerror.restype = ctypes.c_char_p
         for f in ("dualip_create", "dualip_grad", "dualip_solve", "dualip_set_c", "dualip_set_equality_rows", "dualip_set_global_count",
-                  "dualip_get_info", "dualip_set_profiling"):
+                  "dualip_get_info", "dualip_set_profiling", "dualip_set_reduce_hook", "dualip_get_shard_extents",
+                  "dualip_get_column_stats", "dualip_set_shard_constants", "dualip_eval_partial", "dualip_export_accumulators",
+                  "dualip_import_accumulators"):
             getattr(lib, f).restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -139,14 +159,14 @@ def _ptr(t, dtype=None, keep=None):
 
 def make_opts(projection=PROJ_SIMPLEX_INEQ, p0=1.0, p1=0.0, reduction=RED_AUTO, borrow=False, validate=True,
               momentum=True, group_lanes=0, grid_ctas=0, use_graph=False, direct_kernel=False, jacobi=False, stages=0, tile_units=0,
-              adaptive=False, eta_min=1e-5, eta_max=1e-1, lambda_plan=0) -> Opts:
+              adaptive=False, eta_min=1e-5, eta_max=1e-1, lambda_plan=0, step_deal=0) -> Opts:
     o = Opts()
     load_library().dualip_opts_default(ctypes.byref(o))
     o.projection, o.p0, o.p1, o.reduction = projection, p0, p1, reduction
     o.borrow, o.validate, o.momentum = int(borrow), int(validate), int(momentum)
     o.group_lanes, o.grid_ctas, o.use_graph = group_lanes, grid_ctas, int(use_graph)
     o.tuning.direct_kernel = 1 if direct_kernel else 0
-    o.tuning.stages, o.tuning.tile_units, o.tuning.lambda_plan = stages, tile_units, lambda_plan
+    o.tuning.stages, o.tuning.tile_units, o.tuning.lambda_plan, o.tuning.step_deal = stages, tile_units, lambda_plan, step_deal
     o.precondition = PRECOND_JACOBI if jacobi else PRECOND_NONE
     o.step_rule = STEP_ADAPTIVE if adaptive else STEP_FIXED
     o.eta_min, o.eta_max = float(eta_min), float(eta_max)
@@ -235,6 +255,40 @@ class Problem:
         or None to switch the row off."""
         _check(load_library().dualip_set_global_count(self._h, 0 if M is None else 1, 0.0 if M is None else float(M), _stream_ptr(stream)))
         self.duals = self.J * self.m + (0 if M is None else 1)
+
+    # ---- user-sharded multi-GPU (include/dualip.h, "user-sharded multi-GPU"): thin wrappers, see sharded.py ----
+    @property
+    def acc_words(self) -> int:
+        return self.J * self.m + 3
+
+    def set_reduce_hook(self, fn):
+        """fn(acc_ptr:int, n_words:int, lam_ptr:int, gamma:float, stream:int) or None.  The ctypes thunk is kept alive here."""
+        self._hook = REDUCE_HOOK(lambda user, acc, n, lam, gamma, st: fn(acc, n, lam, gamma, st)) if fn else REDUCE_HOOK()
+        _check(load_library().dualip_set_reduce_hook(self._h, self._hook, None))
+
+    def shard_extents(self) -> ShardExtents:
+        e = ShardExtents()
+        _check(load_library().dualip_get_shard_extents(self._h, ctypes.byref(e)))
+        return e
+
+    def column_stats(self, global_extents: ShardExtents, out, stream=None):
+        _check(load_library().dualip_get_column_stats(self._h, ctypes.byref(global_extents), _ptr(out, np.int64), _stream_ptr(stream)))
+        return out
+
+    def set_shard_constants(self, global_extents: ShardExtents, summed, stream=None):
+        _check(load_library().dualip_set_shard_constants(self._h, ctypes.byref(global_extents), _ptr(summed, np.int64), _stream_ptr(stream)))
+
+    def eval_partial(self, lam, gamma: float, x=None, stream=None):
+        """lam: a CUDA tensor, or a raw device pointer (int) as handed to a reduce hook."""
+        lp = ctypes.c_void_p(lam) if isinstance(lam, int) else _ptr(lam, np.float64)
+        _check(load_library().dualip_eval_partial(self._h, lp, float(gamma), _ptr(x, np.float32), _stream_ptr(stream)))
+
+    def export_accumulators(self, out, clear=True, stream=None):
+        _check(load_library().dualip_export_accumulators(self._h, _ptr(out, np.int64), int(clear), _stream_ptr(stream)))
+        return out
+
+    def import_accumulators(self, acc, accumulate=False, stream=None):
+        _check(load_library().dualip_import_accumulators(self._h, _ptr(acc, np.int64), int(accumulate), _stream_ptr(stream)))
 
     def get_csc(self, col_ptr=None, perm=None, stream=None):
         """dualip_get_csc: fills col_ptr int64[J+1] and perm int64[nnz] (tensors / arrays or None)."""

@@ -65,5 +65,22 @@ def build(force: bool = False, verbose: bool = False, defines: dict | None = Non
     return LIB
 
 
+CHECKED_LIB = os.path.join(HERE, "libdualip_b200_checked.so")
+
+
+def build_checked(force: bool = False) -> str:
+    """The -DDUALIP_CHECKED variant (in-kernel bounds assertions, dualip_info.checks_failed) next to the product library;
+    tests/test_gpu_checked_build.py loads it.  Not used by anything else."""
+    deps = [os.path.join(CSRC, s) for s in SOURCES + HEADERS] + [os.path.abspath(__file__)]
+    if force or not os.path.exists(CHECKED_LIB) or any(os.path.getmtime(d) > os.path.getmtime(CHECKED_LIB) for d in deps):
+        tmp = CHECKED_LIB + f".{os.getpid()}.tmp"
+        _compile_and_link(tmp, NVCC_FLAGS + ["-DDUALIP_CHECKED=1"])
+        os.replace(tmp, CHECKED_LIB)
+    return CHECKED_LIB
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--checked" in sys.argv:
+        print(build_checked(force="--force" in sys.argv))
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -58,6 +58,9 @@ struct dualip {
     double* lam_cur = nullptr; double* y = nullptr; double* lam_stage = nullptr; double* grad_stage = nullptr;
     double* y_prev = nullptr; double* g_prev = nullptr;   // DUALIP_STEP_ADAPTIVE: previous evaluation point / gradient (R20)
     bool count_on = false;                                 // global-count row (R21): duals = J*m + 1, b[J*m] = M
+    // user-sharded multi-GPU: the caller's all-reduce between the gradient kernel and the epilogue
+    dualip_reduce_hook hook = nullptr; void* hook_user = nullptr;
+    long long nnz_total = 0;                               // nonzeros over all shards (= nnz unless dualip_set_shard_constants said otherwise)
     double* scalars_dev = nullptr;
     float* x_stage = nullptr;
     dualip_dev::TileEntry* tiles = nullptr;
@@ -283,8 +286,8 @@ void set_xmax(dualip* h) {
 void set_scales(dualip* h) {
     h->scale_s = fix_scale(h->xmax * h->max_colabs * 1.000001);
     h->scale_obj = fix_scale(h->xmax * h->sum_abs_c * 1.000001);
-    h->scale_sq = fix_scale(h->xmax * h->xmax * (double)(h->nnz > 0 ? h->nnz : 1) * 1.000001);
-    h->scale_cnt = fix_scale(h->xmax * (double)(h->nnz > 0 ? h->nnz : 1) * 1.000001);
+    h->scale_sq = fix_scale(h->xmax * h->xmax * (double)(h->nnz_total > 0 ? h->nnz_total : 1) * 1.000001);
+    h->scale_cnt = fix_scale(h->xmax * (double)(h->nnz_total > 0 ? h->nnz_total : 1) * 1.000001);
 }
 
 // duals = coupling rows: J*m, + 1 with the global-count row (R21)
@@ -298,54 +301,79 @@ int grid_for(long long n, int threads, int num_sms) {
     return (int)g;
 }
 
-// a0 constants: L (R2), max column |a| sum, sum |c|; all through order-independent fixed point.
-int compute_stats(dualip* h, cudaStream_t st, bool do_a, bool do_c) {
-    const long long nnz = h->nnz;
-    const int J = h->J, m = h->m, JM = J * m;
+// Fixed-point scales of the a0 column statistics, from the problem's extents (the GLOBAL extents of a sharded problem, so
+// that every shard accumulates in the same scales and the integer sums add up exactly to the unsharded ones).
+struct StatScales { double sq, abs, c; };
+StatScales stat_scales(long long I, long long nnz, int m, float maxa, float maxc) {
+    const double rows = (double)(I > 0 ? I : 1);
+    StatScales sc;
+    sc.sq = fix_scale((double)maxa * maxa * m * rows * 1.000001);
+    sc.abs = fix_scale((double)maxa * rows * 1.000001);
+    sc.c = fix_scale((double)maxc * (double)(nnz > 0 ? nnz : 1) * 1.000001);
+    return sc;
+}
+
+// max |a|, max |c| of this handle's rows
+int absmax_rows(dualip* h, cudaStream_t st, float& maxa, float& maxc) {
     unsigned* d_mx = nullptr;
+    if (cudaMalloc(&d_mx, 2 * sizeof(unsigned)) != cudaSuccess) { cudaGetLastError(); return DUALIP_ENOMEM; }
+    unsigned mx[2] = {0u, 0u};
+    const bool ok = cudaMemsetAsync(d_mx, 0, 2 * sizeof(unsigned), st) == cudaSuccess;
+    if (ok) { k_absmax<<<grid_for(h->nnz * h->m, 256, h->num_sms), 256, 0, st>>>(h->a, h->nnz * h->m, h->c, h->nnz, d_mx); h->launches++; }
+    const bool ok2 = ok && cudaMemcpyAsync(mx, d_mx, sizeof(mx), cudaMemcpyDeviceToHost, st) == cudaSuccess &&
+                     cudaStreamSynchronize(st) == cudaSuccess && cudaGetLastError() == cudaSuccess;
+    cudaFree(d_mx);
+    if (!ok2) { cudaGetLastError(); return DUALIP_ECUDA; }
+    std::memcpy(&maxa, &mx[0], 4); std::memcpy(&maxc, &mx[1], 4);
+    return DUALIP_OK;
+}
+
+// d_fix = [colsq JM][colabs JM][cabs 1][out 3] (zeroed by the caller where it accumulates): this handle's column sums
+void launch_col_stats(dualip* h, cudaStream_t st, const StatScales& sc, unsigned long long* d_fix, bool do_a, bool do_c) {
+    const int JM = h->J * h->m;
+    k_col_stats<<<grid_for(h->nnz, 256, h->num_sms), 256, 0, st>>>(h->idx, h->a, h->c, h->nnz, h->m, sc.sq, sc.abs, sc.c,
+                                                                   d_fix, d_fix + JM, d_fix + 2 * JM, do_a ? 1 : 0, do_c ? 1 : 0);
+    h->launches++;
+}
+
+// L (R2), max column |a| sum, sum |c|, the Jacobi factors (R18): derived from the fixed-point column sums in d_fix
+int derive_constants(dualip* h, cudaStream_t st, const StatScales& sc, unsigned long long* d_fix, bool do_a, bool do_c) {
+    const int J = h->J, m = h->m, JM = J * m;
+    unsigned long long* colsq = d_fix; unsigned long long* colabs = d_fix + JM; unsigned long long* cabs = colabs + JM;
+    unsigned long long* out = cabs + 1;
+    k_reduce_stats<<<1, 1024, 0, st>>>(colsq, J, m, colabs, JM, out); h->launches++;
+    if (do_a && h->step_scale) {
+        k_jacobi_step_scale<<<grid_for(JM, 256, h->num_sms), 256, 0, st>>>(colsq, 1.0 / sc.sq, JM, h->step_scale); h->launches++;
+        const double d2_count = h->nnz_total > 0 ? 1.0 / (double)h->nnz_total : 1.0;   // the count row has a 1 on each of the nnz pairs
+        if (cudaMemcpyAsync(h->step_scale + JM, &d2_count, 8, cudaMemcpyHostToDevice, st) != cudaSuccess) { cudaGetLastError(); return DUALIP_ECUDA; }
+    }
+    unsigned long long res[4];
+    if (cudaMemcpyAsync(res, cabs, sizeof(res), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) { cudaGetLastError(); return DUALIP_ECUDA; }
+    if (do_c) h->sum_abs_c = (double)(long long)res[0] / sc.c;
+    if (do_a) {
+        h->L = (double)(long long)res[1] / sc.sq; h->max_colabs = (double)(long long)res[2] / sc.abs;
+        // Jacobi: every nonzero row of A' has unit norm, so L' = max_j sum_k |A'_(j,k)*|^2 = max_j #{k : row (j,k) != 0}
+        h->L_step = h->step_scale ? (double)(res[3] > 0 ? res[3] : 1) : h->L;
+    }
+    return DUALIP_OK;
+}
+
+// a0 constants of an unsharded problem; all through order-independent fixed point.
+int compute_stats(dualip* h, cudaStream_t st, bool do_a, bool do_c) {
+    const int JM = h->J * h->m;
+    float maxa = 0.0f, maxc = 0.0f;
+    int rc = absmax_rows(h, st, maxa, maxc);
+    if (rc != 0) return rc;
+    h->max_abs_a = maxa; h->max_abs_c = maxc;
     unsigned long long* d_fix = nullptr;  // colsq[JM], colabs[JM], cabs[1], out[3]
     const size_t nfix = (size_t)2 * JM + 4;
-    if (cudaMalloc(&d_mx, 2 * sizeof(unsigned)) != cudaSuccess) { cudaGetLastError(); return DUALIP_ENOMEM; }
-    if (cudaMalloc(&d_fix, nfix * sizeof(unsigned long long)) != cudaSuccess) { cudaGetLastError(); cudaFree(d_mx); return DUALIP_ENOMEM; }
-    int rc = DUALIP_OK;
-    do {
-        if (cudaMemsetAsync(d_mx, 0, 2 * sizeof(unsigned), st) != cudaSuccess ||
-            cudaMemsetAsync(d_fix, 0, nfix * sizeof(unsigned long long), st) != cudaSuccess) { rc = DUALIP_ECUDA; break; }
-        const int g = grid_for(nnz * m, 256, h->num_sms);
-        k_absmax<<<g, 256, 0, st>>>(h->a, nnz * m, h->c, nnz, d_mx); h->launches++;
-        unsigned mx[2];
-        if (cudaMemcpyAsync(mx, d_mx, sizeof(mx), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
-            cudaStreamSynchronize(st) != cudaSuccess) { rc = DUALIP_ECUDA; break; }
-        float maxa, maxc;
-        std::memcpy(&maxa, &mx[0], 4); std::memcpy(&maxc, &mx[1], 4);
-        h->max_abs_a = maxa; h->max_abs_c = maxc;
-        const double rows = (double)(h->I > 0 ? h->I : 1);
-        const double sc_sq = fix_scale((double)maxa * maxa * m * rows * 1.000001);
-        const double sc_abs = fix_scale((double)maxa * rows * 1.000001);
-        const double sc_c = fix_scale((double)maxc * (double)(nnz > 0 ? nnz : 1) * 1.000001);
-        unsigned long long* colsq = d_fix; unsigned long long* colabs = d_fix + JM; unsigned long long* cabs = colabs + JM;
-        unsigned long long* out = cabs + 1;
-        k_col_stats<<<grid_for(nnz, 256, h->num_sms), 256, 0, st>>>(h->idx, h->a, h->c, nnz, m, sc_sq, sc_abs, sc_c,
-                                                                    colsq, colabs, cabs, do_a ? 1 : 0, do_c ? 1 : 0);
-        h->launches++;
-        k_reduce_stats<<<1, 1024, 0, st>>>(colsq, J, m, colabs, JM, out); h->launches++;
-        if (do_a && h->step_scale) {
-            k_jacobi_step_scale<<<grid_for(JM, 256, h->num_sms), 256, 0, st>>>(colsq, 1.0 / sc_sq, JM, h->step_scale); h->launches++;
-            const double d2_count = nnz > 0 ? 1.0 / (double)nnz : 1.0;       // the count row has a 1 on each of the nnz pairs
-            if (cudaMemcpyAsync(h->step_scale + JM, &d2_count, 8, cudaMemcpyHostToDevice, st) != cudaSuccess) { rc = DUALIP_ECUDA; break; }
-        }
-        unsigned long long res[4];
-        if (cudaMemcpyAsync(res, cabs, sizeof(res), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
-            cudaStreamSynchronize(st) != cudaSuccess) { rc = DUALIP_ECUDA; break; }
-        if (cudaGetLastError() != cudaSuccess) { rc = DUALIP_ECUDA; break; }
-        if (do_c) h->sum_abs_c = (double)(long long)res[0] / sc_c;
-        if (do_a) {
-            h->L = (double)(long long)res[1] / sc_sq; h->max_colabs = (double)(long long)res[2] / sc_abs;
-            // Jacobi: every nonzero row of A' has unit norm, so L' = max_j sum_k |A'_(j,k)*|^2 = max_j #{k : row (j,k) != 0}
-            h->L_step = h->step_scale ? (double)(res[3] > 0 ? res[3] : 1) : h->L;
-        }
-    } while (0);
-    cudaFree(d_mx); cudaFree(d_fix);
+    if (cudaMalloc(&d_fix, nfix * sizeof(unsigned long long)) != cudaSuccess) { cudaGetLastError(); return DUALIP_ENOMEM; }
+    if (cudaMemsetAsync(d_fix, 0, nfix * sizeof(unsigned long long), st) != cudaSuccess) { cudaGetLastError(); cudaFree(d_fix); return DUALIP_ECUDA; }
+    const StatScales sc = stat_scales(h->I, h->nnz, h->m, maxa, maxc);
+    launch_col_stats(h, st, sc, d_fix, do_a, do_c);
+    rc = derive_constants(h, st, sc, d_fix, do_a, do_c);
+    cudaFree(d_fix);
     return rc;
 }
 
@@ -424,6 +452,7 @@ void prepare_iter(const dualip* h, IterLaunch& L, const double* lam_dev, double 
         if (!L.p.x) L.p.x = h->x_csc;
         L.f.done = nullptr;
     }
+    if (h->hook) L.f.done = nullptr;    // sharded: the cross-GPU sum of the accumulators comes between the kernel and a4-a6
     if (h->opts.projection == DUALIP_PROJ_BOX) {
         L.fn = h->m == 1 ? (const void*)k_grad_box<1> : (h->m == 2 ? (const void*)k_grad_box<2> : (const void*)k_grad_box<0>);
         L.grid = dim3(grid_for(h->nnz, 256, h->num_sms)); L.block = dim3(256); L.smem = 0;
@@ -434,6 +463,8 @@ void prepare_iter(const dualip* h, IterLaunch& L, const double* lam_dev, double 
         tp.stages = h->plan.stages; tp.stage_bytes = h->plan.stage_bytes;
         tp.nnz4 = h->nnz & ~3ll; tp.rows2 = (h->I + 1) & ~1ll; tp.lo_policy = h->plan.lo_policy;
         tp.smem_total = (int)h->plan.smem; tp.lo_flag = reinterpret_cast<int*>(h->ctl + 32);
+        tp.check_word = reinterpret_cast<unsigned*>(h->ctl + 36);
+        tp.dyn_steps = h->opts.tuning.step_deal == 2 ? 1 : 0;
         L.fn = L.p.x ? h->plan.fn_x : h->plan.fn; L.grid = dim3(h->plan.grid); L.block = dim3(32 * (kTmaConsumerWarps + 1)); L.smem = h->plan.smem;
         L.args[0] = &L.tp; L.args[1] = nullptr;
     } else {
@@ -460,8 +491,13 @@ int launch_iter(dualip* h, IterLaunch& L, cudaStream_t st) {
         }
         const long long JM = (long long)h->J * h->m;
         k_csc_combine<<<(unsigned)((JM + 7) / 8), 256, 0, st>>>(h->chunk_ptr, h->J, h->m, h->csc_partial, h->scale_s, h->s_fix);
-        k_finalize_only<<<1, 1024, 0, st>>>(L.f_after);
-        h->launches += 2;
+        h->launches++;
+        CK(cudaGetLastError());
+    }
+    if (h->csc || h->hook) {
+        if (h->hook) h->hook(h->hook_user, reinterpret_cast<int64_t*>(h->s_fix), (int64_t)h->J * h->m + 3, L.f_after.lam_eval, L.f_after.gamma, st);
+        k_finalize_only<<<1, kBlockThreads, 0, st>>>(L.f_after);
+        h->launches++;
         CK(cudaGetLastError());
     }
     return DUALIP_OK;
@@ -616,6 +652,7 @@ int dualip_create(dualip_t** out, int64_t I, int32_t J, int32_t m, const int64_t
     if (o.tuning.direct_kernel != 0 && o.tuning.direct_kernel != 1) return DUALIP_EINVAL;
     if (o.tuning.stages != 0 && (o.tuning.stages < 2 || o.tuning.stages > kTmaStagesMax)) return DUALIP_EINVAL;
     if (o.tuning.tile_units < 0 || o.tuning.lambda_plan < 0 || o.tuning.lambda_plan > 2) return DUALIP_EINVAL;
+    if (o.tuning.step_deal < 0 || o.tuning.step_deal > 2) return DUALIP_EINVAL;
     if (o.step_rule != DUALIP_STEP_FIXED && o.step_rule != DUALIP_STEP_ADAPTIVE) return DUALIP_EINVAL;
     if (o.step_rule == DUALIP_STEP_ADAPTIVE && !(o.eta_min > 0.0 && o.eta_min <= o.eta_max && std::isfinite(o.eta_max))) return DUALIP_EINVAL;
     if (o.precondition != DUALIP_PRECOND_NONE && o.precondition != DUALIP_PRECOND_JACOBI) return DUALIP_EINVAL;
@@ -644,7 +681,7 @@ int dualip_create(dualip_t** out, int64_t I, int32_t J, int32_t m, const int64_t
 
     dualip* h = new (std::nothrow) dualip();
     if (!h) return DUALIP_ENOMEM;
-    h->I = I; h->nnz = nnz; h->J = J; h->m = m; h->opts = o;
+    h->I = I; h->nnz = nnz; h->nnz_total = nnz; h->J = J; h->m = m; h->opts = o;
     int dev = 0;
     int rc = DUALIP_OK;
 #define FAIL(code) do { rc = (code); goto fail; } while (0)
@@ -754,14 +791,124 @@ int dualip_get_info(dualip_t* h, dualip_info* info) {
     info->fix_scale_s = h->scale_s;
     info->grad_kernel_ms = h->prof_ms; info->grad_kernel_count = h->prof_count;
     info->precondition = h->step_scale ? DUALIP_PRECOND_JACOBI : DUALIP_PRECOND_NONE;
-    info->L_step = h->L_step + (h->count_on ? (h->step_scale ? 1.0 : (double)h->nnz) : 0.0);
+    info->L_step = h->L_step + (h->count_on ? (h->step_scale ? 1.0 : (double)h->nnz_total) : 0.0);
     info->duals = (int32_t)n_duals(h);
+#ifdef DUALIP_CHECKED
+    info->checked_build = 1;
+#endif
     if (h->plan.tma) {                                       // what the last streaming launch decided (it has finished: default-stream copy)
         int flag = 0;
-        if (cudaMemcpy(&flag, h->ctl + 32, sizeof(int), cudaMemcpyDeviceToHost) == cudaSuccess) info->lambda_lo_smem = flag;
+        int flag2[2] = {0, 0};
+        if (cudaMemcpy(flag2, h->ctl + 32, sizeof(flag2), cudaMemcpyDeviceToHost) == cudaSuccess) { flag = flag2[0]; info->lambda_lo_smem = flag; info->checks_failed = flag2[1]; }
         else cudaGetLastError();
     }
     return DUALIP_OK;
+}
+
+int dualip_set_reduce_hook(dualip_t* h, dualip_reduce_hook fn, void* user) {
+    if (!h) return DUALIP_EINVAL;
+    h->hook = fn; h->hook_user = fn ? user : nullptr;
+    return DUALIP_OK;
+}
+
+int dualip_get_shard_extents(dualip_t* h, dualip_shard_extents* out) {
+    if (!h || !out) return DUALIP_EINVAL;
+    out->I = h->I; out->nnz = h->nnz;
+    // the handle's current maxima are the shard's own until dualip_set_shard_constants replaced them: recompute
+    float maxa = 0.0f, maxc = 0.0f;
+    int rc = absmax_rows(h, nullptr, maxa, maxc);
+    if (rc != 0) return rc;
+    out->max_abs_a = maxa; out->max_abs_c = maxc;
+    return DUALIP_OK;
+}
+
+int dualip_get_column_stats(dualip_t* h, const dualip_shard_extents* g, int64_t* out, void* stream) {
+    if (!h || !g || !out || g->I < h->I || g->nnz < h->nnz) return DUALIP_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int JM = h->J * h->m;
+    const size_t n = (size_t)2 * JM + 1;
+    unsigned long long* d_fix = nullptr;
+    if (cudaMalloc(&d_fix, n * 8) != cudaSuccess) { cudaGetLastError(); return DUALIP_ENOMEM; }
+    int rc = DUALIP_OK;
+    if (cudaMemsetAsync(d_fix, 0, n * 8, st) != cudaSuccess) rc = DUALIP_ECUDA;
+    if (rc == 0) {
+        launch_col_stats(h, st, stat_scales(g->I, g->nnz, h->m, g->max_abs_a, g->max_abs_c), d_fix, true, true);
+        if (cudaGetLastError() != cudaSuccess || cudaMemcpyAsync(out, d_fix, n * 8, cudaMemcpyDefault, st) != cudaSuccess ||
+            cudaStreamSynchronize(st) != cudaSuccess) rc = DUALIP_ECUDA;
+    }
+    cudaFree(d_fix);
+    if (rc != 0) cudaGetLastError();
+    return rc;
+}
+
+int dualip_set_shard_constants(dualip_t* h, const dualip_shard_extents* g, const int64_t* summed, void* stream) {
+    if (!h || !g || !summed || g->I < h->I || g->nnz < h->nnz) return DUALIP_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int JM = h->J * h->m;
+    const size_t n = (size_t)2 * JM + 1;
+    unsigned long long* d_fix = nullptr;                     // + out[3] of k_reduce_stats
+    if (cudaMalloc(&d_fix, (n + 3) * 8) != cudaSuccess) { cudaGetLastError(); return DUALIP_ENOMEM; }
+    int rc = DUALIP_OK;
+    if (cudaMemcpyAsync(d_fix, summed, n * 8, cudaMemcpyDefault, st) != cudaSuccess) rc = DUALIP_ECUDA;
+    if (rc == 0) {
+        h->nnz_total = g->nnz; h->max_abs_a = g->max_abs_a; h->max_abs_c = g->max_abs_c;
+        rc = derive_constants(h, st, stat_scales(g->I, g->nnz, h->m, g->max_abs_a, g->max_abs_c), d_fix, true, true);
+    }
+    cudaFree(d_fix);
+    if (rc != 0) { cudaGetLastError(); return rc; }
+    set_scales(h);
+    return DUALIP_OK;
+}
+
+int dualip_eval_partial(dualip_t* h, const double* lambda_dev, double gamma, float* x, void* stream) {
+    if (!h || !lambda_dev || !(gamma > 0.0) || !std::isfinite(gamma)) return DUALIP_EINVAL;
+    if (!is_device_ptr(lambda_dev) || (x && !is_device_ptr(x)) || h->csc) return DUALIP_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    FinalizeParams f{};
+    f.lam_eval = lambda_dev; f.gamma = gamma; f.update = 0;
+    IterLaunch L;
+    prepare_iter(h, L, lambda_dev, gamma, x, f);
+    L.f.done = nullptr;                                      // no epilogue: the accumulators stay in the handle
+    if (h->plan.tma) L.tp.f = L.f;
+    const bool timed = prof_begin(h, st);
+    CK(cudaLaunchKernel(L.fn, L.grid, L.block, L.args, L.smem, st));
+    if (timed) prof_end(h, st);
+    h->launches++;
+    CK(cudaGetLastError());
+    return DUALIP_OK;
+}
+
+int dualip_export_accumulators(dualip_t* h, int64_t* out, int32_t clear, void* stream) {
+    if (!h || !out) return DUALIP_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t n = (size_t)h->J * h->m + 3;
+    CK(cudaMemcpyAsync(out, h->s_fix, n * 8, cudaMemcpyDefault, st));
+    if (clear) CK(cudaMemsetAsync(h->s_fix, 0, n * 8, st));
+    if (!is_device_ptr(out)) CK(cudaStreamSynchronize(st));
+    return DUALIP_OK;
+}
+
+int dualip_import_accumulators(dualip_t* h, const int64_t* in, int32_t accumulate, void* stream) {
+    if (!h || !in) return DUALIP_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t n = (size_t)h->J * h->m + 3;
+    if (!accumulate) {
+        CK(cudaMemcpyAsync(h->s_fix, in, n * 8, cudaMemcpyDefault, st));
+        if (!is_device_ptr(in)) CK(cudaStreamSynchronize(st));
+        return DUALIP_OK;
+    }
+    const unsigned long long* src = reinterpret_cast<const unsigned long long*>(in);
+    unsigned long long* tmp = nullptr;
+    if (!is_device_ptr(in)) {
+        if (cudaMalloc(&tmp, n * 8) != cudaSuccess) { cudaGetLastError(); return DUALIP_ENOMEM; }
+        if (cudaMemcpyAsync(tmp, in, n * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) { cudaGetLastError(); cudaFree(tmp); return DUALIP_ECUDA; }
+        src = tmp;
+    }
+    k_acc_add<<<grid_for((long long)n, 256, h->num_sms), 256, 0, st>>>(h->s_fix, src, (long long)n);
+    h->launches++;
+    const cudaError_t e = cudaGetLastError();
+    if (tmp) { cudaStreamSynchronize(st); cudaFree(tmp); }
+    return e == cudaSuccess ? DUALIP_OK : DUALIP_ECUDA;
 }
 
 int dualip_get_csc(dualip_t* h, int64_t* col_ptr_out, int64_t* perm_out, void* stream) {
@@ -875,7 +1022,7 @@ int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int3
     CK(cudaMemcpyAsync(h->lam_cur, lambda_inout, JM * 8, cudaMemcpyDefault, st));
     // R21: with the global-count row A A^T is no longer block diagonal; |A|_2^2 <= |A_items|_2^2 + |count row|_2^2, and the
     // row's squared norm is nnz (1 once row-normalised)
-    double L = h->L_step + (h->count_on ? (h->step_scale ? 1.0 : (double)h->nnz) : 0.0);
+    double L = h->L_step + (h->count_on ? (h->step_scale ? 1.0 : (double)h->nnz_total) : 0.0);
     if (!(L > 0.0)) L = 1.0;
     const bool adaptive = h->opts.step_rule == DUALIP_STEP_ADAPTIVE;
     CK(cudaMemsetAsync(h->ctl, 0, sizeof(IterState), st));                                 // t = 0, n = 0
@@ -899,7 +1046,7 @@ int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int3
         int t = 0;
         // beta_t and the trace row come from the device-side iteration state, so every launch of a stage has the
         // same arguments: replay a graph of kGraphUnroll chained launches, then finish with direct launches
-        if (h->opts.use_graph && !h->profile && !h->csc && iters[s] >= 2 * kGraphUnroll) {
+        if (h->opts.use_graph && !h->profile && !h->csc && !h->hook && iters[s] >= 2 * kGraphUnroll) {
             int rc = set_graph(h, it);
             if (rc != 0) return rc;
             for (; t + kGraphUnroll <= iters[s]; t += kGraphUnroll) {

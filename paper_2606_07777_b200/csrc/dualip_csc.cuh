@@ -162,9 +162,11 @@ __global__ void k_perm_widen(const unsigned* __restrict__ in, long long n, long 
 }
 
 // a4-a6 as a launch of its own (the CSC path; every other path runs finalize_block in the gradient kernel's epilogue)
+// Launched with kBlockThreads threads: the same count as the gradient kernels' epilogue CTA, so the scalar reductions run in the
+// same order and a sharded / two-phase evaluation gives the same bits as the fused one.
 __global__ void __launch_bounds__(1024) k_finalize_only(const FinalizeParams f) {
     __shared__ double sh[kFinalizeScratchBytes / 8];
-    finalize_block(f, sh, threadIdx.x, 1024);
+    finalize_block(f, sh, threadIdx.x, blockDim.x);
 }
 
 }  // namespace dualip_dev

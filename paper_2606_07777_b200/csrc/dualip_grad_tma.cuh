@@ -57,7 +57,30 @@ struct TmaParams {
     int lo_policy;                     // lambda's low word in shared memory: 0 = decided per launch (see k_grad_tma), 1 = never, 2 = always
     int smem_total;                    // dynamic shared memory of the launch (bytes)
     int* lo_flag;                      // nullable: CTA 0 records the decision here (dualip_info.lambda_lo_smem)
+    int dyn_steps;                     // row-steps of a tile dealt 0 = statically (round-robin over the CTA's step sequence), 1 = dynamically
+    unsigned* check_word;              // -DDUALIP_CHECKED builds: bit set per kind of bounds violation (dualip_info.checks_failed)
 };
+
+// ---- checked build (-DDUALIP_CHECKED): compute-sanitizer is closed on the GPU pool this was developed on, so the bounds it
+// would have checked are asserted by the kernel itself: every staged-row position against the stage capacity, every item index
+// against J before it is used as a shared-memory / accumulator offset, every x position against nnz, every candidate-list slot
+// against the warp's list.  A violation sets a bit in a device word (dualip_info.checks_failed); the access is then skipped or
+// clamped so the run can finish and report.  Compiled out of the product build.
+#ifdef DUALIP_CHECKED
+static __device__ unsigned* g_chk_word;
+static __device__ int g_chk_cap_nz, g_chk_J, g_chk_cap_rows;
+static __device__ long long g_chk_nnz;
+#define DUALIP_CHECK(cond, bit) do { if (!(cond)) atomicOr(g_chk_word, 1u << (bit)); } while (0)
+#define DUALIP_CHECK_POS(q) DUALIP_CHECK((unsigned)(q) < (unsigned)g_chk_cap_nz, 0)
+#define DUALIP_CHECK_ITEM(j) DUALIP_CHECK((unsigned)(j) < (unsigned)g_chk_J, 1)
+#define DUALIP_CHECK_X(pos) DUALIP_CHECK((unsigned long long)(pos) < (unsigned long long)g_chk_nnz, 2)
+#else
+#define DUALIP_CHECK(cond, bit) do { } while (0)
+#define DUALIP_CHECK_POS(q) do { } while (0)
+#define DUALIP_CHECK_ITEM(j) do { } while (0)
+#define DUALIP_CHECK_X(pos) do { } while (0)
+#endif
+enum { CHK_POS = 0, CHK_ITEM = 1, CHK_X = 2, CHK_LIST = 3, CHK_ROWS = 4, CHK_ROW_EXTENT = 5, CHK_STAGE_BYTES = 6 };
 
 // ---- PTX wrappers (mbarrier + bulk async copy) ---------------------------------------------------------------
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -87,7 +110,7 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
 // One stage: [idx cap_nz*4][c cap_nz*4][a cap_nz*4*m][row_ptr cap_rows*8][meta: int nrows, int rpo, long long nzb, pad]
-struct StageMeta { int nrows; int rpo; long long nzb; long long pad[2]; };
+struct StageMeta { int nrows; int rpo; long long nzb; int next_step; int pad32; long long pad; };   // next_step: dynamic dealing
 struct StageView {
     const int* idx; const float* c; const float* a; const long long* rp; const StageMeta* meta;
 };
@@ -105,6 +128,12 @@ __device__ __forceinline__ StageView stage_view(unsigned char* base, int cap_nz,
 // never writes x): the x-writing code drops out of the hot kernel, which measured 2-5 % faster on every config.
 template <bool WX, class P>
 __device__ __forceinline__ float* xout(const P& p) { return WX ? p.x : nullptr; }
+
+template <bool WX, class P>
+__device__ __forceinline__ void store_x(const P& p, long long pos, float val) {
+    DUALIP_CHECK_X(pos);
+    if (WX) p.x[pos] = val;
+}
 
 // The launch constants the out-of-line row routines use, as REGISTER values.  Those routines get the kernel parameters by
 // reference, i.e. as a generic pointer, and the compiler re-loads a field from memory at every use rather than keep it in
@@ -160,7 +189,11 @@ __device__ __forceinline__ long long to_fix32(float v, float scale) { return __f
 // RED.ADD.64 on a pointer known to be global memory (a generic atomicAdd makes ptxas emit an address-space check, a
 // shared-memory CAS loop and a predicate that the caller then waits on).
 __device__ __forceinline__ void red_add_u64(unsigned long long* gptr, unsigned long long v) {
+#ifdef DUALIP_EXP_NULL_RED      // experiment build (profiles/: what the item reduction costs): results are wrong by construction
+    (void)gptr; (void)v;
+#else
     asm volatile("red.global.add.u64 [%0], %1;" ::"l"(gptr), "l"(v));
+#endif
 }
 
 // (a > b) ? x : y as one SETP + SEL, whatever the surrounding control flow looks like
@@ -173,6 +206,7 @@ __device__ __forceinline__ int sel_gt(float a, float b, int x, int y) {
 // a4 + a5 for one nonzero with x != 0.
 template <int M, bool ACC_SMEM, class P>
 __device__ __forceinline__ void push(const P& p, const ConsumerCtx& cx, FixPair& fp, int mm, int j, float cc, const float* aa, float x) {
+    DUALIP_CHECK_ITEM(j);
     fp.obj += to_fix32(cc * x, p.scale_obj_f);
     fp.sq += to_fix32(x * x, p.scale_sq_f);
     fp.cnt += to_fix32(x, p.scale_cnt_f);
@@ -187,10 +221,20 @@ __device__ __forceinline__ void push(const P& p, const ConsumerCtx& cx, FixPair&
     }
 }
 
+// The exact path's dual operand is ALWAYS the two-word value hi + lo, hi = RN_f32(lambda), lo = RN_f32(lambda - hi) (exact to
+// 2^-48 relative), whether the words come from shared memory or are split on the fly from the fp64 dual read through L2: the
+// per-launch choice between the two (k_grad_tma) must not change a bit of the result.
+__device__ __forceinline__ double two_word(double l) {
+    const float h = (float)l;
+    return (double)h + (double)(float)(l - (double)h);
+}
+
 // t = c + sum_f a_f * lambda[j,f] in fp64 for the staged nonzero q (w = -t).
 template <int M>
 __device__ __forceinline__ double exact_t(const StageView& v, const ConsumerCtx& cx, int mm, int q, int& j, float& cc, float* aa) {
+    DUALIP_CHECK_POS(q);
     j = v.idx[q];
+    DUALIP_CHECK_ITEM(j);
     cc = v.c[q];
     double t = (double)cc + cx.mu;
 #pragma unroll
@@ -199,7 +243,7 @@ __device__ __forceinline__ double exact_t(const StageView& v, const ConsumerCtx&
         if (f < mm) {
             aa[f] = v.a[q * mm + f];
             const double l = cx.hi_only ? (double)cx.lam_hi[j * mm + f]
-                                        : (cx.lam_lo ? (double)cx.lam_hi[j * mm + f] + (double)cx.lam_lo[j * mm + f] : __ldg(cx.lam_g + j * mm + f));
+                                        : (cx.lam_lo ? (double)cx.lam_hi[j * mm + f] + (double)cx.lam_lo[j * mm + f] : two_word(__ldg(cx.lam_g + j * mm + f)));
             t = fma((double)aa[f], l, t);
         }
     }
@@ -216,7 +260,7 @@ __device__ __forceinline__ void exact_t_batch(const StageView& v, const Consumer
     int j[K];
     double l[K][MA];
 #pragma unroll
-    for (int k = 0; k < K; ++k) j[k] = v.idx[q[k]];
+    for (int k = 0; k < K; ++k) { DUALIP_CHECK_POS(q[k]); j[k] = v.idx[q[k]]; DUALIP_CHECK_ITEM(j[k]); }
     if (cx.hi_only) {
 #pragma unroll
         for (int k = 0; k < K; ++k)
@@ -231,7 +275,7 @@ __device__ __forceinline__ void exact_t_batch(const StageView& v, const Consumer
 #pragma unroll
         for (int k = 0; k < K; ++k)
 #pragma unroll
-            for (int f = 0; f < MA; ++f) l[k][f] = f < mm ? __ldg(cx.lam_g + j[k] * mm + f) : 0.0;
+            for (int f = 0; f < MA; ++f) l[k][f] = f < mm ? two_word(__ldg(cx.lam_g + j[k] * mm + f)) : 0.0;
     }
 #pragma unroll
     for (int k = 0; k < K; ++k) {
@@ -251,12 +295,14 @@ __device__ __forceinline__ void exact_t_batch(const StageView& v, const Consumer
 template <int G, int M>
 __device__ __forceinline__ void filter_load(const StageView& v, const float* __restrict__ s_hi32, int mm, int q, int beg, int len,
                                             float (&w)[4], int (&pe)[4]) {
+    DUALIP_CHECK_POS(q); DUALIP_CHECK_POS(M == 2 ? q + 2 * G + 1 : q + 3);
     if (M == 2) {
         const int q2 = q + 2 * G;
         const int2 jA = *reinterpret_cast<const int2*>(v.idx + q), jB = *reinterpret_cast<const int2*>(v.idx + q2);
         const float2 cA = *reinterpret_cast<const float2*>(v.c + q), cB = *reinterpret_cast<const float2*>(v.c + q2);
         const float4 aA = *reinterpret_cast<const float4*>(v.a + 2 * q), aB = *reinterpret_cast<const float4*>(v.a + 2 * q2);
         const int jj[4] = {jA.x, jA.y, jB.x, jB.y};
+        DUALIP_CHECK_ITEM(jj[0]); DUALIP_CHECK_ITEM(jj[1]); DUALIP_CHECK_ITEM(jj[2]); DUALIP_CHECK_ITEM(jj[3]);
         const float cv[4] = {cA.x, cA.y, cB.x, cB.y};
         const float ax[4] = {aA.x, aA.z, aB.x, aB.z}, ay[4] = {aA.y, aA.w, aB.y, aB.w};
         pe[0] = q; pe[1] = q + 1; pe[2] = q2; pe[3] = q2 + 1;
@@ -269,6 +315,7 @@ __device__ __forceinline__ void filter_load(const StageView& v, const float* __r
         const int4 j4 = *reinterpret_cast<const int4*>(v.idx + q);
         const float4 c4 = *reinterpret_cast<const float4*>(v.c + q);
         const int jj[4] = {j4.x, j4.y, j4.z, j4.w};
+        DUALIP_CHECK_ITEM(jj[0]); DUALIP_CHECK_ITEM(jj[1]); DUALIP_CHECK_ITEM(jj[2]); DUALIP_CHECK_ITEM(jj[3]);
         const float cv[4] = {c4.x, c4.y, c4.z, c4.w};
         if (M == 1) {
             const float4 a4 = *reinterpret_cast<const float4*>(v.a + q);
@@ -343,7 +390,7 @@ __device__ __noinline__ FixPair slow_row(const GradParams& p_in, const StageView
         }
         const float m32 = group_max<32>(wmax);
         if (ineq && !(m32 > 0.0f)) {
-            if (xout<WX>(p)) for (int q = beg + lane; q < end; q += 32) xout<WX>(p)[nzb + q] = 0.0f;
+            if (xout<WX>(p)) for (int q = beg + lane; q < end; q += 32) store_x<WX>(p, nzb + q, 0.0f);
             return fp;
         }
         const double md = (double)m32;
@@ -372,7 +419,7 @@ __device__ __noinline__ FixPair slow_row(const GradParams& p_in, const StageView
             const int q = beg + lane + 32 * k;
             if (q < end) {
                 const float x = fmaxf(u[k] - tau, 0.0f);
-                if (xout<WX>(p)) xout<WX>(p)[nzb + q] = x;
+                if (xout<WX>(p)) store_x<WX>(p, nzb + q, x);
                 if (x > 0.0f) {
                     j = v.idx[q]; cc = v.c[q];
 #pragma unroll
@@ -387,7 +434,7 @@ __device__ __noinline__ FixPair slow_row(const GradParams& p_in, const StageView
     for (int q = beg + lane; q < end; q += 32) wmax = fmaxf(wmax, (float)(-exact_t<M>(v, cx, mm, q, j, cc, aa)));
     const float m32 = group_max<32>(wmax);
     if (ineq && !(m32 > 0.0f)) {
-        if (xout<WX>(p)) for (int q = beg + lane; q < end; q += 32) xout<WX>(p)[nzb + q] = 0.0f;
+        if (xout<WX>(p)) for (int q = beg + lane; q < end; q += 32) store_x<WX>(p, nzb + q, 0.0f);
         return fp;
     }
     const double md = (double)m32;
@@ -462,7 +509,7 @@ __device__ __noinline__ FixPair slow_row(const GradParams& p_in, const StageView
         const double tq = exact_t<M>(v, cx, mm, q, j, cc, aa);
         const float u = GBOX ? (float)(-tq * p.inv_gamma - ref) : (float)(-tq - md) * p.inv_gamma_f;
         const float x = fminf(fmaxf(u - tau, 0.0f), cap);
-        if (xout<WX>(p)) xout<WX>(p)[nzb + q] = x;
+        if (xout<WX>(p)) store_x<WX>(p, nzb + q, x);
         if (x > 0.0f) push<M, ACC_SMEM>(p, cx, fp, mm, j, cc, aa, x);
     }
     return fp;
@@ -525,7 +572,7 @@ __device__ __forceinline__ void half_warp_rows(const GradK& p, const StageView& 
         if (h + 16 * k < len) {
             const int q = beg + h + 16 * k;
             const float x = fmaxf(u[k] - tau, 0.0f);
-            if (xout<WX>(p)) xout<WX>(p)[nzb + q] = x;
+            if (xout<WX>(p)) store_x<WX>(p, nzb + q, x);
             if (x > 0.0f) {
                 j = v.idx[q]; cc = v.c[q];
 #pragma unroll
@@ -587,6 +634,13 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const __grid_con
     unsigned* a_hi = a_lo + JM;
     float* s_lo32 = s_hi32 + (ACC_SMEM ? 3 : 1) * JM;
 
+#ifdef DUALIP_CHECKED
+    if (threadIdx.x == 0) {
+        g_chk_word = tp.check_word; g_chk_cap_nz = tp.cap_nz; g_chk_J = p.J; g_chk_cap_rows = tp.cap_rows; g_chk_nnz = p.nnz;
+        if ((size_t)tp.stage_bytes < (size_t)tp.cap_nz * (8 + 4 * mm) + (size_t)tp.cap_rows * 8 + sizeof(StageMeta)) atomicOr(tp.check_word, 1u << CHK_STAGE_BYTES);
+    }
+    __syncthreads();
+#endif
     if (threadIdx.x == 0) s_words[0] = 0u;
     __syncthreads();
     {
@@ -648,6 +702,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const __grid_con
     }
     __syncthreads();
 
+    const bool dyn = tp.dyn_steps != 0;
     const double mu = p.count_on ? p.lambda[JM] : 0.0;
     const ConsumerCtx cx{s_hi32, lo_smem ? s_lo32 : nullptr, p.lambda, a_lo, a_hi, hi_only, mu};
     FixPair fp{0ll, 0ll, 0ll};
@@ -678,7 +733,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const __grid_con
                 const long long r0a = r0 & ~1ll;
                 long long r1a = (r1 + 2) & ~1ll;                                       // rows r0a .. r1 inclusive, even count
                 if (r1a > tp.rows2) r1a = tp.rows2 > r0a ? tp.rows2 : r0a;
-                d_meta->nrows = (int)(r1 - r0); d_meta->rpo = (int)(r0 - r0a); d_meta->nzb = p0a;
+                d_meta->nrows = (int)(r1 - r0); d_meta->rpo = (int)(r0 - r0a); d_meta->nzb = p0a; d_meta->next_step = 0;
                 // tails that are not a whole 16-byte chunk (only at the very end of the arrays): plain copies
                 for (long long q = p1a > p0a ? p1a : p0a; q < p1; ++q) {
                     d_idx[q - p0a] = p.idx[q]; d_c[q - p0a] = p.c[q];
@@ -727,10 +782,17 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const __grid_con
             // Row-steps are dealt round-robin over the CTA's whole step sequence (not per tile): step st of this tile is
             // number step_off + st of the sequence and belongs to warp (step_off + st) mod NWC.  Every warp sees every
             // tile's nsteps, so each keeps the running offset itself: no shared counter, no atomics.
+            // That is the STATIC deal: right when every step costs the same (the vertex regime).  When most rows take the
+            // candidate / slow paths a step's cost varies several-fold, a warp that draws a heavy step holds its stage, and with
+            // only ~1 step per warp resident the others idle at the next "full" barrier (ncu: 16 % of the stall samples on cfg5
+            // at gamma = 0.1).  The DYNAMIC deal -- a warp claims the tile's next step from a counter in the stage's meta words
+            // (one shared-memory atomic by lane 0 + a broadcast per claim) -- lets whoever is free take it.  dyn is per launch.
             int st0 = (warp - 1) - step_off;
             if (st0 < 0) st0 += NWC;
             step_off = (step_off + nsteps) % NWC;
-            for (int st = st0; st < nsteps; st += NWC) {
+            int* const next_step = const_cast<int*>(&v.meta->next_step);
+            auto claim = [&]() { int c = 0; if (lane == 0) c = atomicAdd(next_step, 1); return __shfl_sync(kFull, c, 0); };
+            for (int st = dyn ? claim() : st0; st < nsteps; st = dyn ? claim() : st + NWC) {
                 const int rpo = v.meta->rpo;
                 const int nzb32 = (int)v.meta->nzb;                       // low word is enough for local offsets
                 int rbeg[RPG], rlen[RPG];
@@ -743,6 +805,8 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const __grid_con
                     if (lr < nrows) {
                         const int b = (int)v.rp[rpo + lr], e = (int)v.rp[rpo + lr + 1];   // differences fit in 32 bits
                         beg = b - nzb32; len = e - b;
+                        DUALIP_CHECK(rpo + lr + 1 < tp.cap_rows, CHK_ROWS);
+                        DUALIP_CHECK(beg >= 0 && len >= 0 && (beg & ~3) + ((len + (beg & 3) + 4 * G - 1) / (4 * G)) * (4 * G) <= tp.cap_nz, CHK_ROW_EXTENT);
                     }
                     rbeg[r] = beg; rlen[r] = len;
                     rm1[r] = -CUDART_INF_F; rm2[r] = -CUDART_INF_F; rpos[r] = 0;
@@ -836,7 +900,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const __grid_con
                             const bool fr = __shfl_sync(kFull, (int)(active && fast), src) != 0;
                             const float xr = __shfl_sync(kFull, xo, src);
                             const int pr = __shfl_sync(kFull, fpos, src);
-                            if (fr) for (int e = gl; e < rlen[r]; e += G) xout<WX>(p)[nzb + rbeg[r] + e] = (rbeg[r] + e == pr) ? xr : 0.0f;
+                            if (fr) for (int e = gl; e < rlen[r]; e += G) store_x<WX>(p, nzb + rbeg[r] + e, (rbeg[r] + e == pr) ? xr : 0.0f);
                         }
                     }
                     // ---- candidate path: rows that are neither a vertex nor dead.  Only nonzeros with w > w_max - z gamma
@@ -888,6 +952,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const __grid_con
                                         const bool isc = w[e] > thr;
                                         const unsigned bal = __ballot_sync(kFull, isc) & gmask;
                                         const int k = ncand + __popc(bal & lt_mask);
+                                        DUALIP_CHECK(!(isc && k < 2 * G) || (clist + k) - cand_list < 64 * NWC, CHK_LIST);
                                         if (isc && k < 2 * G) clist[k] = pe[e];
                                         ncand += __popc(bal);
                                     }
@@ -911,8 +976,11 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const __grid_con
                             const float u0 = cp0 >= 0 ? (float)(wq0 - (double)m32) * p.inv_gamma_f : -CUDART_INF_F;
                             const float u1 = (two && cp1 >= 0) ? (float)(wq1 - (double)m32) * p.inv_gamma_f : -CUDART_INF_F;
                             float theta = -z - (1.2e-7f * fabsf(mv) + 1e-6f);
+                            // Michelot's fixed point on the candidates.  (A closed form -- every lane ranking its value among the
+                            // group's with G - 1 exchanges, Duchi's criterion evaluated per lane -- was built and measured: equal at
+                            // G = 4, slower from G = 8 up, where 3-4 iterations of a log G reduction cost less than G - 1 exchanges.)
                             int n_prev = -1;
-                            for (;;) {                                           // Michelot on the candidates
+                            for (;;) {
                                 const bool in0 = alive && u0 > theta, in1 = alive && u1 > theta;
                                 const float sg = group_sum<G>((in0 ? u0 : 0.0f) + (in1 ? u1 : 0.0f));
                                 int n = __popc(__ballot_sync(kFull, in0) & gmask);
@@ -938,10 +1006,10 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const __grid_con
                             }
                             if (xout<WX>(p)) {
                                 const long long nzb = v.meta->nzb;
-                                if (row_ok) for (int e = gl; e < rlen[r]; e += G) xout<WX>(p)[nzb + rbeg[r] + e] = 0.0f;
+                                if (row_ok) for (int e = gl; e < rlen[r]; e += G) store_x<WX>(p, nzb + rbeg[r] + e, 0.0f);
                                 __syncwarp();
-                                if (cp0 >= 0) xout<WX>(p)[nzb + cp0] = xq0;
-                                if (cp1 >= 0) xout<WX>(p)[nzb + cp1] = xq1;
+                                if (cp0 >= 0) store_x<WX>(p, nzb + cp0, xq0);
+                                if (cp1 >= 0) store_x<WX>(p, nzb + cp1, xq1);
                             }
                             if (lane == src && row_ok) handled = true;
                         }

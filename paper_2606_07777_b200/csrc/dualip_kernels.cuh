@@ -751,6 +751,11 @@ __global__ void k_jacobi_step_scale(const unsigned long long* colsq, double inv_
     }
 }
 
+// user-sharded multi-GPU helper: integer accumulation of another shard's sums
+__global__ void k_acc_add(unsigned long long* acc, const unsigned long long* in, long long n) {
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (long long)gridDim.x * blockDim.x) acc[q] += in[q];
+}
+
 #endif  // DUALIP_HOST_KERNELS
 
 }  // namespace dualip_dev

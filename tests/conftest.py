@@ -15,6 +15,38 @@ GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
     config.addinivalue_line("markers", "slow: full-size GPU parity cases (minutes)")
+    if os.environ.get("DUALIP_TEST_CHECKED") == "1":
+        _use_checked_build()
+
+
+# ---- checked build (tests/test_gpu_checked_build.py re-runs GPU tests with DUALIP_TEST_CHECKED=1): the binding loads the
+# -DDUALIP_CHECKED library, and every handle's bounds-violation mask is read before the handle goes away.
+_CHECK_FAILURES = []
+
+
+def _use_checked_build():
+    from paper_2606_07777_b200 import binding, build
+    lib = build.build_checked()
+    binding.lib_path = lambda: lib
+    orig = binding.Problem.destroy
+
+    def destroy(self):
+        if self._h:
+            inf = self.info()
+            if inf.checked_build != 1 or inf.checks_failed != 0:
+                _CHECK_FAILURES.append(f"checked_build={inf.checked_build} checks_failed={inf.checks_failed:#x} (I={inf.I}, J={inf.J}, G={inf.group_lanes})")
+        orig(self)
+
+    binding.Problem.destroy = destroy
+
+
+@pytest.fixture(autouse=True)
+def _no_bounds_violations():
+    yield
+    if os.environ.get("DUALIP_TEST_CHECKED") == "1":
+        import gc
+        gc.collect()
+        assert not _CHECK_FAILURES, _CHECK_FAILURES
 
 
 def read_projection_cases():

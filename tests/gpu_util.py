@@ -89,12 +89,16 @@ def gpu_solve(pg, gammas, iters, lam0=None, want_trace=True, want_x=True):
     return out
 
 
-def assert_trajectory_parity(po, pg, gammas, iters, lam0=None, momentum=True, tag="", jacobi=False, is_eq=None):
+def assert_trajectory_parity(po, pg, gammas, iters, lam0=None, momentum=True, tag="", jacobi=False, is_eq=None, ref=None):
     """Independent solves compared per iteration (parity mode B of SURVEY 8(c)).  jacobi: the oracle iterates on the
     literally row-scaled system; pg must have been created with jacobi=True (per-coordinate step).
-    is_eq: equality-row mask (pg.set_equality_rows must have been called with it)."""
-    ref = oracle.solve(po, gammas, iters, lam0=lam0, momentum=momentum, trace_grad=True, trace_lambda=True, jacobi=jacobi,
-                       is_eq=is_eq)
+    is_eq: equality-row mask (pg.set_equality_rows must have been called with it).  ref: the oracle's solve of exactly this
+    call when the caller already has it (a concurrent.futures future or the result; full-size tests run it on a host thread)."""
+    if ref is None:
+        ref = oracle.solve(po, gammas, iters, lam0=lam0, momentum=momentum, trace_grad=True, trace_lambda=True, jacobi=jacobi,
+                           is_eq=is_eq)
+    elif hasattr(ref, "result"):
+        ref = ref.result()
     out = gpu_solve(pg, gammas, iters, lam0=lam0)
     T = int(np.sum(iters))
     worst = 0.0

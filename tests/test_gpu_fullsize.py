@@ -3,7 +3,11 @@ the device, borrowed by the library, default plan).  What is compared:
 
   * x on sampled users (seeded random users + the longest rows + the first and last rows): the oracle projects
     exactly those rows one by one (a sub-instance holding only them) -- element-wise |dx| <= 1e-5;
-  * grad g and g against the oracle's full evaluation where the oracle finishes in about a minute (configs 2, 3);
+  * grad g, g and ALL of x against the oracle's full evaluation for configs 2, 3 and 5 at lambda = 0 (what the verbatim run
+    evaluates at every iteration) and at the probe lambda; for config 4 (5e9 nonzeros) against the oracle on the first
+    3,000,000 users, as a problem of its own with the same kernel instantiation (test_cfg4_first_3M_users_...);
+  * full-size TRAJECTORIES: config 2, 3 and 5 tight companions (Jacobi step for the Zipf configs), every iteration's
+    gradient, lambda and the final x against the oracle's solve;
   * at every size, properties that tie the remaining outputs to the sampled ones: grad g = A x - b and
     g = c'x + gamma/2 |x|^2 + lambda'grad g re-accumulated in fp64 from the x the kernel wrote (plain torch
     index_add, an independent reduction), feasibility of every row, and bit-identical results on a second launch.
@@ -97,9 +101,17 @@ FULL = [
     # name, probe-lambda scale, full oracle evaluation?
     ("cfg2", 0.5, True),
     ("cfg3", 0.05, True),
-    ("cfg5", 0.5, False),
+    ("cfg5", 0.5, True),
     ("cfg4", 0.5, False),
 ]
+
+
+def _pool():
+    """The oracle is single-threaded C behind ctypes (which releases the GIL): independent oracle evaluations of one test
+    run side by side on the host cores while the GPU part of the test proceeds."""
+    from concurrent.futures import ThreadPoolExecutor
+    import os
+    return ThreadPoolExecutor(max_workers=max(1, min(4, len(os.sched_getaffinity(0)) - 1)))
 
 
 @pytest.mark.parametrize("name,lam_scale,full_oracle", FULL, ids=[f[0] for f in FULL])
@@ -113,23 +125,30 @@ def test_full_size_gradient(name, lam_scale, full_oracle):
     pg = _create(inst)
     info = pg.info()
     assert info.streaming == 1 and info.grid_ctas == torch.cuda.get_device_properties(0).multi_processor_count
+    from test_gpu_parity import FULL_SIZE_G
+    assert info.group_lanes == FULL_SIZE_G[name], "the scaled trajectory tests must run the instantiation the full-size plan picks"
     Jm = inst.J * inst.m
     users = _sample_rows(inst)
     (rp, idx, c, a), pos = _sub_instance(inst, users)
     po_sub = _oracle_problem(cfg, users.numel(), rp, idx, c, a, inst.b.cpu().numpy())
     x = torch.empty(inst.nnz, dtype=torch.float32, device="cuda")
     grad = torch.empty(Jm, dtype=torch.float64, device="cuda")
-    po_full = None
+    po_full, pending, pool = None, {}, None
+    cases = (("zero", torch.zeros(Jm, dtype=torch.float64, device="cuda"), cfg.gammas[-1]),
+             ("probe", synth.probe_lambda(inst, 0, lam_scale), cfg.gammas[-1]),
+             ("soft", synth.probe_lambda(inst, 1, lam_scale), 100.0 * cfg.gammas[-1]),
+             ("dense", torch.zeros(Jm, dtype=torch.float64, device="cuda"), 0.1))
     if full_oracle:
         d = inst.numpy()
         po_full = _oracle_problem(cfg, inst.I, d["row_ptr"], d["item_idx"], d["c"], d["a"], d["b"])
+        pool = _pool()
+        for which, lam, gamma in cases:                              # the full evaluations start now, on host threads
+            if which in ("zero", "probe") or inst.nnz < 50_000_000:
+                pending[which] = pool.submit(oracle.grad, po_full, lam.cpu().numpy(), gamma)
     # lambda = 0 is what the verbatim configs evaluate at every iteration (they are slack); the
     # probe is a busy lambda; "soft" repeats it at 100 x gamma, where a large share of the rows is fractional; "dense" is
     # gamma = 0.1 at lambda = 0 (the first stage of config 5's schedule): hardly any row is a vertex, every slow path runs
-    for which, lam, gamma in (("zero", torch.zeros(Jm, dtype=torch.float64, device="cuda"), cfg.gammas[-1]),
-                              ("probe", synth.probe_lambda(inst, 0, lam_scale), cfg.gammas[-1]),
-                              ("soft", synth.probe_lambda(inst, 1, lam_scale), 100.0 * cfg.gammas[-1]),
-                              ("dense", torch.zeros(Jm, dtype=torch.float64, device="cuda"), 0.1)):
+    for which, lam, gamma in cases:
         sc = pkg.Scalars()
         pg.grad(lam, gamma, grad=grad, scalars=sc, x=x)
         torch.cuda.synchronize()
@@ -148,27 +167,88 @@ def test_full_size_gradient(name, lam_scale, full_oracle):
         assert abs(sc.obj - obj) <= TOL_G * abs(obj) + 1e-9 and abs(sc.reg - reg) <= TOL_G * abs(reg) + 1e-9
         assert float(x.min()) >= 0.0 and _row_sums_max(inst, x) <= 1.0 + 1e-5
         # (3) the whole evaluation against the oracle
-        if po_full is not None and (which == "probe" or inst.nnz < 50_000_000):
-            rf = oracle.grad(po_full, lam.cpu().numpy(), gamma)
+        if which in pending:
+            rf = pending.pop(which).result()
             assert rel_l2(grad.cpu().numpy(), rf.grad) <= TOL_GRAD, f"{name}/{which}: grad vs oracle"
             assert abs(sc.g - rf.g) <= TOL_G * abs(rf.g), f"{name}/{which}: g {sc.g} vs oracle {rf.g}"
-            exf = np.abs(x.cpu().numpy() - rf.x).max()
+            assert abs(sc.r_inf - rf.r_inf) <= TOL_GRAD * np.linalg.norm(rf.grad) + 1e-12 and abs(sc.gap - rf.gap) <= TOL_G * (abs(rf.obj) + abs(rf.g)) + 1e-9
+            xh = x.cpu().numpy()
+            exf = max(float(np.abs(xh[p0:p0 + (1 << 26)] - rf.x[p0:p0 + (1 << 26)]).max()) for p0 in range(0, inst.nnz, 1 << 26))
             assert exf <= TOL_X, f"{name}/{which}: full x abs err {exf:.3e}"
-            del rf
+            del rf, xh
         # (4) a second launch gives the same bits
         grad_b, sc_b = torch.empty_like(grad), pkg.Scalars()
         pg.grad(lam, gamma, grad=grad_b, scalars=sc_b)
         torch.cuda.synchronize()
         assert torch.equal(grad, grad_b) and sc.g == sc_b.g
+    if pool is not None:
+        pool.shutdown()
     pg.destroy()
 
 
-def test_full_size_cfg2_tight_trajectory():
-    """Config 2 at full size with binding constraints: 25 AGD iterations, every iteration's grad g against the oracle."""
-    from gpu_util import assert_trajectory_parity, from_instance
-    inst = synth.generate(synth.get_config("cfg2-tight"), device="cuda")
-    host = synth.Instance(inst.cfg, *(getattr(inst, k).cpu() for k in ("row_ptr", "item_idx", "c", "a", "b")))
-    po, pg = from_instance(host)
-    worst, ex, ref, out = assert_trajectory_parity(po, pg, inst.cfg.gammas, [25], tag="cfg2-tight full")
-    assert (ref.lam > 0).sum() > 50
-    pg.destroy()
+def test_cfg4_first_3M_users_gradient_and_x_against_the_oracle():
+    """Config 4 is 5e9 nonzeros (80 GB of rows): one oracle evaluation of all of it is about an hour of one host core.  What IS
+    compared in full with the oracle: the problem made of its first K = 3,000,000 users (3e8 nonzeros, m = 2, same items, same
+    b), whose rows are borrowed in place from the full-size arrays -- grad g (i.e. this prefix's whole contribution A x - b),
+    g, the scalars and every x -- with the kernel instantiation and tile size of the full-size plan (asserted)."""
+    cfg = synth.get_config("cfg4")
+    if torch.cuda.get_device_properties(0).total_memory < 110e9:
+        pytest.skip("cfg4 needs about 110 GB of device memory")
+    K = 3_000_000
+    inst = synth.generate(cfg, device="cuda")
+    full = _create(inst)
+    fi = full.info()
+    nzk = int(inst.row_ptr[K])
+    kind, p0, p1 = synth.proj_spec(cfg)
+    o = pkg.binding.make_opts(projection=getattr(pkg, _KIND[kind][0]), p0=p0, p1=p1, borrow=True)
+    rp, idx, c, a = inst.row_ptr[:K + 1], inst.item_idx[:nzk], inst.c[:nzk], inst.a[:nzk * inst.m]
+    pg = pkg.Problem.create(K, inst.J, inst.m, rp, idx, c, a, inst.b, o)
+    pi = pg.info()
+    assert (pi.streaming, pi.group_lanes, pi.stages, pi.tile_units, pi.grid_ctas) == (1, fi.group_lanes, fi.stages, fi.tile_units, fi.grid_ctas)
+    po = _oracle_problem(cfg, K, rp.cpu().numpy(), idx.cpu().numpy(), c.cpu().numpy(), a.cpu().numpy(), inst.b.cpu().numpy())
+    Jm = inst.J * inst.m
+    cases = (("zero", torch.zeros(Jm, dtype=torch.float64, device="cuda"), cfg.gammas[-1]),
+             ("probe", synth.probe_lambda(inst, 0, 0.5), cfg.gammas[-1]))
+    pool = _pool()
+    pending = {which: pool.submit(oracle.grad, po, lam.cpu().numpy(), gamma) for which, lam, gamma in cases}
+    x = torch.empty(nzk, dtype=torch.float32, device="cuda")
+    xf = torch.empty(inst.nnz, dtype=torch.float32, device="cuda")
+    grad = torch.empty(Jm, dtype=torch.float64, device="cuda")
+    for which, lam, gamma in cases:
+        sc = pkg.Scalars()
+        pg.grad(lam, gamma, grad=grad, scalars=sc, x=x)
+        full.grad(lam, gamma, x=xf)                               # the full-size launch writes the same x for these users
+        torch.cuda.synchronize()
+        assert torch.equal(x, xf[:nzk]), f"cfg4/{which}: prefix problem and full problem disagree on the prefix's x"
+        rf = pending[which].result()
+        assert rel_l2(grad.cpu().numpy(), rf.grad) <= TOL_GRAD, f"cfg4[:3M]/{which}: grad vs oracle"
+        assert abs(sc.g - rf.g) <= TOL_G * abs(rf.g) and abs(sc.obj - rf.obj) <= TOL_G * abs(rf.obj) + 1e-9
+        exf = float(np.abs(x.cpu().numpy() - rf.x).max())
+        assert exf <= TOL_X, f"cfg4[:3M]/{which}: full x abs err {exf:.3e}"
+        del rf
+    pool.shutdown()
+    pg.destroy(); full.destroy()
+
+
+def test_full_size_tight_trajectories_cfg3_cfg5():
+    """The Zipf configs at full size with binding constraints and the Jacobi step (the scalar step gamma / L stalls on them):
+    3 AGD iterations -- every iteration's grad g and lambda, the final grad g, scalars and all of x -- against the oracle's
+    solve.  The two oracle solves (4 evaluations of 5e8 / 6e8 nonzeros each) run side by side on host threads."""
+    from gpu_util import assert_trajectory_parity
+    from test_gpu_parity import FULL_SIZE_G
+    pool = _pool()
+    jobs = []
+    for name in ("cfg3-tight", "cfg5-tight"):
+        cfg = synth.get_config(name)
+        inst = synth.generate(cfg, device="cuda")
+        d = inst.numpy()
+        po = _oracle_problem(cfg, inst.I, d["row_ptr"], d["item_idx"], d["c"], d["a"], d["b"])
+        fut = pool.submit(oracle.solve, po, [cfg.gammas[-1]], [3], trace_grad=True, trace_lambda=True, jacobi=True)
+        jobs.append((name, cfg, inst, po, fut))
+    for name, cfg, inst, po, fut in jobs:
+        pg = _create(inst, jacobi=True)
+        assert pg.info().streaming == 1 and pg.info().group_lanes == FULL_SIZE_G[name[:4]]
+        worst, ex, ref, out = assert_trajectory_parity(po, pg, [cfg.gammas[-1]], [3], tag=f"{name} full", jacobi=True, ref=fut)
+        assert (ref.lam > 0).sum() > 100
+        pg.destroy()
+    pool.shutdown()

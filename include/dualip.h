@@ -172,6 +172,8 @@ typedef struct {
     int32_t lambda_lo_smem;  /* streaming kernel: 1 if the LAST launch staged lambda's low word in shared memory */
     int32_t checked_build;   /* 1: the library was compiled with -DDUALIP_CHECKED (in-kernel bounds assertions; tests only) */
     int32_t checks_failed;   /* checked build: bit mask of the kinds of bounds violation seen so far (0 = none); else 0 */
+    int64_t long_rows;       /* rows taken by the CTA-per-row kernel k_grad_long (more than long_row_threshold nonzeros) */
+    int64_t long_row_threshold; /* 0: no row is treated as long */
 } dualip_info;
 
 /*

@@ -76,7 +76,7 @@ class Info(ctypes.Structure):
                 ("grad_kernel_ms", ctypes.c_double), ("grad_kernel_count", ctypes.c_int64),
                 ("precondition", ctypes.c_int32), ("pad0", ctypes.c_int32), ("L_step", ctypes.c_double),
                 ("duals", ctypes.c_int32), ("lambda_lo_smem", ctypes.c_int32), ("checked_build", ctypes.c_int32),
-                ("checks_failed", ctypes.c_int32)]
+                ("checks_failed", ctypes.c_int32), ("long_rows", ctypes.c_int64), ("long_row_threshold", ctypes.c_int64)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

@@ -6,6 +6,7 @@
 #include "dualip_kernels.cuh"
 #include "dualip_grad_tma.cuh"
 #include "dualip_csc.cuh"
+#include "dualip_long.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -85,6 +86,10 @@ struct dualip {
     unsigned char* row_eq = nullptr;       // [JM] equality-row mask (dualip_set_equality_rows) or nullptr
     float max_abs_a = 0.0f, max_abs_c = 0.0f;
     long long max_row_len = 0;
+    // long rows (dualip_long.cuh): rows of more than long_thr nonzeros are skipped by the main gradient kernel and taken by
+    // k_grad_long, one CTA per row, in a launch of its own before it.  long_thr = 0: no such rows.
+    long long long_thr = 0, n_long = 0;
+    long long* long_ids = nullptr;
     double scale_s = 1.0, scale_obj = 1.0, scale_sq = 1.0, scale_cnt = 1.0;
     double xmax = 1.0;
     Plan plan;
@@ -157,11 +162,11 @@ const void* pick_kernel(const Plan& pl) {
 
 // Streaming plan: lambda (and for small J*m the accumulators) in shared memory, the rest of the 227 KB split into
 // `stages` tile buffers.  Returns false if this problem cannot use it.
-bool plan_tma(dualip* h, Plan& pl) {
+bool plan_tma(dualip* h, Plan& pl, long long max_len) {
     const size_t JM = (size_t)h->J * h->m;
     const int red = h->opts.reduction;
     if (h->opts.projection == DUALIP_PROJ_BOX || h->nnz == 0) return false;
-    if (h->max_row_len > 8192) return false;
+    if (max_len > 8192) return false;
     if (((uintptr_t)h->row_ptr | (uintptr_t)h->idx | (uintptr_t)h->c | (uintptr_t)h->a) & 15) return false;
     // Shared memory: RN_f32(lambda) always (the filter's operand, 4 B per dual).  Its low word joins it while the
     // pair stays under 64 KB (otherwise the exact path reads the fp64 lambda through L2: it runs once per row at
@@ -185,7 +190,7 @@ bool plan_tma(dualip* h, Plan& pl) {
     const int s_hi = h->opts.tuning.stages ? h->opts.tuning.stages : 3, s_lo = h->opts.tuning.stages ? h->opts.tuning.stages : 2;
     for (int S = s_hi; S >= s_lo && TN < 256; --S) {
         stage_bytes = (avail / S) & ~(size_t)127;
-        const long long over = 80 + (h->max_row_len + 8 + 72) * (8 + 4 * m);
+        const long long over = 80 + (max_len + 8 + 72) * (8 + 4 * m);
         long long tn = ((long long)stage_bytes - over) / (9 + 4 * m);
         tn = tn > 0 ? (tn & ~63ll) : 0;
         if (tn >= (S >= 3 ? 512 : 256)) { TN = tn; stages = S; }
@@ -198,7 +203,7 @@ bool plan_tma(dualip* h, Plan& pl) {
     if (h->opts.tuning.tile_units >= 256 && h->opts.tuning.tile_units < TN) TN = h->opts.tuning.tile_units & ~63ll;
     pl.tma = true; pl.acc_smem = acc; pl.lam_smem = true;
     pl.TN = TN; pl.stages = stages;
-    pl.cap_nz = (int)((TN + h->max_row_len + 8 + 72 + 3) & ~3ll);   // +72: lanes may read up to 2*32+2 slots past a row end (m = 2)
+    pl.cap_nz = (int)((TN + max_len + 8 + 72 + 3) & ~3ll);   // +72: lanes may read up to 2*32+2 slots past a row end (m = 2)
     pl.cap_rows = (int)((TN / kRowCost + 6 + 1) & ~1ll);
     size_t sb = (size_t)pl.cap_nz * (8 + 4 * m) + (size_t)pl.cap_rows * 8 + 32;
     pl.stage_bytes = (int)((sb + 127) & ~(size_t)127);
@@ -224,7 +229,23 @@ int make_plan(dualip* h) {
     if (G == 0) G = mean > 20.0 ? 32 : (mean > 10.0 ? 16 : 8);
     if (G != 1 && G != 2 && G != 4 && G != 8 && G != 16 && G != 32) return DUALIP_EINVAL;
     if (pl.M == 0) G = 32;
-    if (h->opts.tuning.direct_kernel != 1 && plan_tma(h, pl)) {          // tuning.direct_kernel forces the non-streaming kernel (tests)
+    // Rows the streaming kernel cannot stage next to a useful tile are LONG rows: k_grad_long takes them, CTA per row, and the
+    // streaming kernel's tile table isolates each of them in a tile of its own that the producer skips.  The cap is the
+    // largest row length (tried downwards from 8192 in steps of a quarter) that still gives a 3-stage plan; simplex kinds only.
+    const bool simplex_kind = h->opts.projection == DUALIP_PROJ_SIMPLEX_INEQ || h->opts.projection == DUALIP_PROJ_SIMPLEX_EQ ||
+                              (h->opts.projection == DUALIP_PROJ_BOXCUT && h->opts.p0 >= h->opts.p1);
+    bool streaming = false;
+    h->long_thr = 0;
+    if (h->opts.tuning.direct_kernel != 1) {                        // tuning.direct_kernel forces the non-streaming kernel (tests)
+        streaming = plan_tma(h, pl, h->max_row_len);
+        if (!streaming && simplex_kind && h->max_row_len > 256) {
+            for (long long cap = std::min<long long>(8192, h->max_row_len - 1) & ~63ll; cap >= 256 && !streaming; cap = (cap * 3 / 4) & ~63ll) {
+                Plan trial = pl;
+                if (plan_tma(h, trial, cap) && trial.stages >= 3) { pl = trial; streaming = true; h->long_thr = cap; }
+            }
+        }
+    }
+    if (streaming) {
         // narrow lane groups: several rows share one pass of the chunk loop, which amortises the per-row work
         int Gs = h->opts.group_lanes;
         if (Gs == 0) {
@@ -253,6 +274,7 @@ int make_plan(dualip* h) {
         return DUALIP_OK;
     }
     pl.tma = false;
+    if (simplex_kind && h->max_row_len > 4096) h->long_thr = 4096;   // direct-load plan: beyond this a row gets a CTA, not a warp
     if (G < 8) G = 8;
     pl.acc_smem = (red == DUALIP_RED_AUTO || red == DUALIP_RED_SMEM) && fits_both;
     pl.lam_smem = pl.acc_smem || fits_lam;
@@ -394,6 +416,7 @@ void fill_grad_params(const dualip* h, GradParams& p, const double* lam_dev, dou
         default: p.z = (float)o.p0; break;
     }
     p.count_on = h->count_on ? 1 : 0;
+    p.long_thr = h->long_thr;
     p.scale_s = h->scale_s; p.scale_obj = h->scale_obj; p.scale_sq = h->scale_sq; p.scale_cnt = h->scale_cnt;
     p.scale_s_f = (float)h->scale_s; p.scale_obj_f = (float)h->scale_obj; p.scale_sq_f = (float)h->scale_sq;
     p.scale_cnt_f = (float)h->scale_cnt;
@@ -465,6 +488,7 @@ void prepare_iter(const dualip* h, IterLaunch& L, const double* lam_dev, double 
         tp.smem_total = (int)h->plan.smem; tp.lo_flag = reinterpret_cast<int*>(h->ctl + 32);
         tp.check_word = reinterpret_cast<unsigned*>(h->ctl + 36);
         tp.dyn_steps = h->opts.tuning.step_deal == 2 ? 1 : 0;
+        tp.row_cap = h->long_thr;
         L.fn = L.p.x ? h->plan.fn_x : h->plan.fn; L.grid = dim3(h->plan.grid); L.block = dim3(32 * (kTmaConsumerWarps + 1)); L.smem = h->plan.smem;
         L.args[0] = &L.tp; L.args[1] = nullptr;
     } else {
@@ -473,10 +497,13 @@ void prepare_iter(const dualip* h, IterLaunch& L, const double* lam_dev, double 
     }
 }
 
+int launch_long(dualip* h, const GradParams& p, cudaStream_t st);
+
 // One launch = one evaluation a1-a5 (+ the AGD update a6 when f.update): gradient kernel with the grid epilogue.
 int launch_iter(dualip* h, IterLaunch& L, cudaStream_t st) {
     const bool timed = prof_begin(h, st);
     struct End { dualip* h; cudaStream_t st; bool on; ~End() { if (on) prof_end(h, st); } } end_guard{h, st, timed};
+    { int rc = launch_long(h, L.p, st); if (rc != 0) return rc; }     // long rows first (none on the BASELINE configs)
     CK(cudaLaunchKernel(L.fn, L.grid, L.block, L.args, L.smem, st));
     h->launches++;
     CK(cudaGetLastError());
@@ -557,6 +584,82 @@ int build_csc(dualip* h, cudaStream_t st) {
     return DUALIP_OK;
 }
 
+// a0: the rows k_grad_long takes (more than long_thr nonzeros)
+int build_long_list(dualip* h, cudaStream_t st) {
+    unsigned long long* d_cnt = nullptr;
+    if (cudaMalloc(&d_cnt, 8) != cudaSuccess) { cudaGetLastError(); return DUALIP_ENOMEM; }
+    unsigned long long n = 0;
+    int rc = DUALIP_OK;
+    do {
+        const int g = grid_for(h->I, 256, h->num_sms);
+        if (cudaMemsetAsync(d_cnt, 0, 8, st) != cudaSuccess) { rc = DUALIP_ECUDA; break; }
+        k_collect_long<<<g, 256, 0, st>>>(h->row_ptr, h->I, h->long_thr, nullptr, d_cnt); h->launches++;
+        if (cudaMemcpyAsync(&n, d_cnt, 8, cudaMemcpyDeviceToHost, st) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) { rc = DUALIP_ECUDA; break; }
+        h->n_long = (long long)n;
+        if (n == 0) { h->long_thr = 0; break; }
+        if ((rc = dev_alloc(h, &h->long_ids, (size_t)n)) != 0) break;
+        if (cudaMemsetAsync(d_cnt, 0, 8, st) != cudaSuccess) { rc = DUALIP_ECUDA; break; }
+        k_collect_long<<<g, 256, 0, st>>>(h->row_ptr, h->I, h->long_thr, h->long_ids, d_cnt); h->launches++;
+        if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) { rc = DUALIP_ECUDA; break; }
+        const void* fn = h->m == 1 ? (const void*)k_grad_long<1> : (h->m == 2 ? (const void*)k_grad_long<2> : (const void*)k_grad_long<0>);
+        if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBudget) != cudaSuccess) { rc = DUALIP_ECUDA; break; }
+    } while (0);
+    cudaFree(d_cnt);
+    if (rc == DUALIP_ECUDA) cudaGetLastError();
+    return rc;
+}
+
+// Streaming plan with long rows: every long row becomes a tile of its own (which the producer skips), i.e. the tile table gets
+// a cut before and after each of them.  The table is a sorted list of row numbers, so this is a merge, done on the host at
+// create; the rest of a split tile keeps its bounds (a piece of a tile is smaller than the tile).
+int isolate_long_rows(dualip* h, cudaStream_t st) {
+    const long long nt = h->plan.ntiles;
+    std::vector<TileEntry> tiles((size_t)nt + 1);
+    std::vector<long long> ids((size_t)h->n_long);
+    CK(cudaMemcpyAsync(tiles.data(), h->tiles, ((size_t)nt + 1) * sizeof(TileEntry), cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(ids.data(), h->long_ids, (size_t)h->n_long * 8, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    std::vector<long long> cuts;
+    cuts.reserve((size_t)nt + 1 + 2 * ids.size());
+    for (const TileEntry& t : tiles) cuts.push_back(t.row0);
+    for (long long r : ids) { cuts.push_back(r); cuts.push_back(r + 1); }
+    std::sort(cuts.begin(), cuts.end());
+    cuts.erase(std::unique(cuts.begin(), cuts.end()), cuts.end());           // first cut is row 0, last is row I
+    const long long nt2 = (long long)cuts.size() - 1;
+    long long* d_cuts = nullptr;
+    if (cudaMalloc(&d_cuts, cuts.size() * 8) != cudaSuccess) { cudaGetLastError(); return DUALIP_ENOMEM; }
+    cudaFree(h->tiles); h->tiles = nullptr; h->bytes_resident -= (long long)(((size_t)nt + 1) * sizeof(TileEntry));
+    int rc = dev_alloc(h, &h->tiles, (size_t)nt2 + 1);
+    if (rc == 0) {
+        if (cudaMemcpyAsync(d_cuts, cuts.data(), cuts.size() * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) rc = DUALIP_ECUDA;
+        else {
+            k_fill_tiles<<<grid_for(nt2 + 1, 128, h->num_sms), 128, 0, st>>>(h->row_ptr, d_cuts, nt2, h->tiles); h->launches++;
+            if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = DUALIP_ECUDA;
+        }
+    }
+    cudaFree(d_cuts);
+    if (rc != 0) { cudaGetLastError(); return rc; }
+    h->plan.ntiles = nt2;
+    if (h->opts.grid_ctas <= 0) h->plan.grid = (int)(nt2 < h->num_sms ? (nt2 > 0 ? nt2 : 1) : h->num_sms);
+    return DUALIP_OK;
+}
+
+// the long rows of one evaluation: launched before the main gradient kernel, same accumulators, no epilogue
+int launch_long(dualip* h, const GradParams& p, cudaStream_t st) {
+    if (h->n_long <= 0) return DUALIP_OK;
+    LongParams lp;
+    lp.g = p; lp.long_ids = h->long_ids; lp.n_long = h->n_long;
+    const size_t scratch = 64 * 4;
+    lp.ucap = (int)((kSmemBudget - scratch) / 4);
+    const int grid = (int)std::min<long long>(h->n_long, (long long)h->num_sms);
+    if (h->m == 1) k_grad_long<1><<<grid, kLongThreads, kSmemBudget, st>>>(lp);
+    else if (h->m == 2) k_grad_long<2><<<grid, kLongThreads, kSmemBudget, st>>>(lp);
+    else k_grad_long<0><<<grid, kLongThreads, kSmemBudget, st>>>(lp);
+    h->launches++;
+    CK(cudaGetLastError());
+    return DUALIP_OK;
+}
+
 constexpr int kGraphUnroll = 20;   // iterations per graph replay
 
 void drop_graph(dualip* h) {
@@ -627,7 +730,7 @@ void dualip_destroy(dualip_t* h) {
     drop_graph(h);
     cudaFree(h->ctl);
     cudaFree(h->csc_perm); cudaFree(h->col_ptr); cudaFree(h->chunk_ptr); cudaFree(h->chunk_item); cudaFree(h->csc_partial);
-    cudaFree(h->x_csc);
+    cudaFree(h->x_csc); cudaFree(h->long_ids);
     for (cudaEvent_t e : h->events) cudaEventDestroy(e);
     cudaGetLastError();
     delete h;
@@ -743,6 +846,13 @@ int dualip_create(dualip_t** out, int64_t I, int32_t J, int32_t m, const int64_t
             cudaError_t e1 = cudaMemcpyAsync(&flags, d_flags, sizeof(int), cudaMemcpyDeviceToHost, st);
             cudaError_t e2 = cudaMemcpyAsync(&maxlen, d_maxlen, 8, cudaMemcpyDeviceToHost, st);
             cudaError_t e3 = cudaStreamSynchronize(st);
+            if (e1 == cudaSuccess && e2 == cudaSuccess && e3 == cudaSuccess && (flags & 8) && !(flags & 3)) {
+                // some row is not ascending: its duplicate check is warp-cooperative (k_validate_unsorted)
+                k_validate_unsorted<<<grid_for(I * 32, 256, h->num_sms), 256, 0, st>>>(h->row_ptr, h->idx, I, d_flags);
+                h->launches++;
+                e1 = cudaMemcpyAsync(&flags, d_flags, sizeof(int), cudaMemcpyDeviceToHost, st);
+                e3 = cudaStreamSynchronize(st);
+            }
             cudaFree(d_flags); cudaFree(d_maxlen);
             if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || cudaGetLastError() != cudaSuccess) FAIL(DUALIP_ECUDA);
             if (flags & 3) FAIL(DUALIP_ERANGE);
@@ -758,11 +868,13 @@ int dualip_create(dualip_t** out, int64_t I, int32_t J, int32_t m, const int64_t
             h->csc = true;
             if ((rc = build_csc(h, st)) != 0) goto fail;
         }
+        if (h->long_thr > 0 && (rc = build_long_list(h, st)) != 0) goto fail;
         if (h->plan.tma) {
             if ((rc = dev_alloc(h, &h->tiles, (size_t)h->plan.ntiles + 1)) != 0) goto fail;
             k_build_tiles<<<grid_for(h->plan.ntiles + 1, 128, h->num_sms), 128, 0, st>>>(h->row_ptr, I, h->plan.TN, h->plan.ntiles, h->tiles);
             h->launches++;
             CKF(cudaGetLastError());
+            if (h->n_long > 0 && (rc = isolate_long_rows(h, st)) != 0) goto fail;
         }
         CKF(cudaStreamSynchronize(st));
     }
@@ -780,7 +892,7 @@ int dualip_get_info(dualip_t* h, dualip_info* info) {
     prof_collect(h);
     std::memset(info, 0, sizeof(*info));
     info->I = h->I; info->nnz = h->nnz; info->J = h->J; info->m = h->m; info->L = h->L;
-    info->max_row_len = h->max_row_len;
+    info->max_row_len = h->max_row_len; info->long_rows = h->n_long; info->long_row_threshold = h->long_thr;
     info->group_lanes = h->plan.G; info->chunk_regs = h->plan.KREG;
     info->reduction = h->csc ? DUALIP_RED_CSC : (h->plan.acc_smem ? DUALIP_RED_SMEM : DUALIP_RED_GLOBAL);
     info->lambda_in_smem = h->plan.lam_smem ? 1 : 0;
@@ -871,6 +983,7 @@ int dualip_eval_partial(dualip_t* h, const double* lambda_dev, double gamma, flo
     L.f.done = nullptr;                                      // no epilogue: the accumulators stay in the handle
     if (h->plan.tma) L.tp.f = L.f;
     const bool timed = prof_begin(h, st);
+    { int rc = launch_long(h, L.p, st); if (rc != 0) { if (timed) prof_end(h, st); return rc; } }
     CK(cudaLaunchKernel(L.fn, L.grid, L.block, L.args, L.smem, st));
     if (timed) prof_end(h, st);
     h->launches++;
@@ -1046,7 +1159,7 @@ int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int3
         int t = 0;
         // beta_t and the trace row come from the device-side iteration state, so every launch of a stage has the
         // same arguments: replay a graph of kGraphUnroll chained launches, then finish with direct launches
-        if (h->opts.use_graph && !h->profile && !h->csc && !h->hook && iters[s] >= 2 * kGraphUnroll) {
+        if (h->opts.use_graph && !h->profile && !h->csc && !h->hook && h->n_long == 0 && iters[s] >= 2 * kGraphUnroll) {
             int rc = set_graph(h, it);
             if (rc != 0) return rc;
             for (; t + kGraphUnroll <= iters[s]; t += kGraphUnroll) {

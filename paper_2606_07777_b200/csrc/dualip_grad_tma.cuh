@@ -58,6 +58,7 @@ struct TmaParams {
     int smem_total;                    // dynamic shared memory of the launch (bytes)
     int* lo_flag;                      // nullable: CTA 0 records the decision here (dualip_info.lambda_lo_smem)
     int dyn_steps;                     // row-steps of a tile dealt 0 = statically (round-robin over the CTA's step sequence), 1 = dynamically
+    long long row_cap;                 // > 0: a one-row tile of more than this many nonzeros is a LONG row (k_grad_long's): skipped
     unsigned* check_word;              // -DDUALIP_CHECKED builds: bit set per kind of bounds violation (dualip_info.checks_failed)
 };
 
@@ -726,7 +727,9 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const __grid_con
                 float* d_a = reinterpret_cast<float*>(sb + (size_t)tp.cap_nz * 8);
                 long long* d_rp = reinterpret_cast<long long*>(sb + (size_t)tp.cap_nz * (8 + 4 * mm));
                 StageMeta* d_meta = reinterpret_cast<StageMeta*>(d_rp + tp.cap_rows);
-                const long long r0 = cur.row0, r1 = nxt.row0, p0 = cur.nz0, p1 = nxt.nz0;
+                const long long r0 = cur.row0, p0 = cur.nz0;
+                long long r1 = nxt.row0, p1 = nxt.nz0;
+                if (tp.row_cap > 0 && r1 - r0 == 1 && p1 - p0 > tp.row_cap) { r1 = r0; p1 = p0; }   // a long row's own tile: nothing to stage
                 const long long p0a = p0 & ~3ll;
                 long long p1a = (p1 + 3) & ~3ll;
                 if (p1a > tp.nnz4) p1a = tp.nnz4 > p0a ? tp.nnz4 : p0a;              // never read past the arrays
@@ -1052,6 +1055,14 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const __grid_con
 }
 
 #ifdef DUALIP_HOST_KERNELS
+// a0: tile table from an explicit list of cut rows (the streaming plan with long rows isolated: dualip_api.cu)
+__global__ void k_fill_tiles(const long long* __restrict__ row_ptr, const long long* __restrict__ cuts, long long ntiles, TileEntry* tiles) {
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t <= ntiles; t += (long long)gridDim.x * blockDim.x) {
+        tiles[t].row0 = cuts[t];
+        tiles[t].nz0 = row_ptr[cuts[t]];
+    }
+}
+
 // a0: tile table.  Tile t starts at the first row r with row_ptr[r] + kRowCost*r >= t*TN (parallel binary search).
 __global__ void k_build_tiles(const long long* __restrict__ row_ptr, long long I, long long TN, long long ntiles, TileEntry* tiles) {
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t <= ntiles; t += (long long)gridDim.x * blockDim.x) {

@@ -44,6 +44,7 @@ struct GradParams {
     int proj;
     int general_boxcut;          // BOXCUT with ub < z: needs the capped threshold search
     int count_on;                // global-count row (R21): lambda[J*m] is its dual mu, gathered by EVERY nonzero
+    long long long_thr;          // > 0: rows of more than this many nonzeros are k_grad_long's (dualip_long.cuh); skipped here
     float inv_gamma_f;
     float z;                     // simplex / box-cut budget
     float ub;                    // box-cut cap
@@ -416,6 +417,7 @@ __global__ void __launch_bounds__(kBlockThreads, 1) k_grad(const GradParams p, c
         const long long row = step * RPW + grp;
         long long beg = 0, end = 0;
         if (row < p.I) { beg = __ldg(p.row_ptr + row); end = __ldg(p.row_ptr + row + 1); }
+        if (p.long_thr > 0 && end - beg > p.long_thr) end = beg;     // a long row: k_grad_long takes it
         const long long len = end - beg;
         const bool is_long = len > (long long)G * KREG;
         const int flen = is_long ? 0 : (int)len;
@@ -650,7 +652,8 @@ __global__ void __launch_bounds__(256) k_grad_box(const GradParams p, const Fina
 
 // Create-time kernels (not templates): defined in the one translation unit that launches them (dualip_api.cu).
 #ifdef DUALIP_HOST_KERNELS
-// flags: bit0 row_ptr not monotone, bit1 index out of range, bit2 duplicate item in a row
+// flags: bit0 row_ptr not monotone, bit1 index out of range, bit2 duplicate item in a row, bit3 some row is not ascending
+// (its duplicate check is k_validate_unsorted's: a strictly ascending row cannot hold a duplicate).  One thread per row.
 __global__ void k_validate(const long long* __restrict__ row_ptr, const int* __restrict__ idx, long long I, int J,
                            long long nnz, int scan, int* flags, unsigned long long* max_len) {
     unsigned long long lmax = 0;
@@ -660,23 +663,36 @@ __global__ void k_validate(const long long* __restrict__ row_ptr, const int* __r
         if (beg > end || beg < 0 || end > nnz) { f |= 1; continue; }
         if ((unsigned long long)(end - beg) > lmax) lmax = (unsigned long long)(end - beg);
         if (!scan) continue;
-        bool ascending = true;
         int prev = -1;
         for (long long q = beg; q < end; ++q) {
             const int j = idx[q];
             if (j < 0 || j >= J) f |= 2;
-            if (j <= prev) ascending = false;
+            if (j <= prev) f |= 8;
             prev = j;
-        }
-        if (!ascending && !(f & 2)) {
-            for (long long q = beg; q < end; ++q) {
-                const int j = idx[q];
-                for (long long r = q + 1; r < end; ++r) if (idx[r] == j) f |= 4;
-            }
         }
     }
     if (f) atomicOr(flags, f);
     atomicMax(max_len, lmax);
+}
+
+// Duplicate check of the rows that are not ascending (launched only when k_validate saw one): one WARP per row, every
+// element compared with the later ones lane-strided -- len^2 / 32 steps per row, rows in parallel, coalesced reads -- instead
+// of one thread walking len^2 pairs.  row_ptr has been checked (bit0 clear) before this runs.
+__global__ void k_validate_unsorted(const long long* __restrict__ row_ptr, const int* __restrict__ idx, long long I, int* flags) {
+    const int lane = threadIdx.x & 31;
+    const long long warp0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
+    bool dup = false;
+    for (long long i = warp0; i < I; i += nwarps) {
+        const long long beg = row_ptr[i], end = row_ptr[i + 1];
+        bool asc = true;
+        for (long long q = beg + lane; q + 1 < end; q += 32) asc = asc && idx[q] < idx[q + 1];
+        if (__all_sync(kFull, asc)) continue;
+        for (long long q = beg; q + 1 < end; ++q) {
+            const int j = idx[q];
+            for (long long r = q + 1 + lane; r < end; r += 32) dup = dup || idx[r] == j;
+        }
+    }
+    if (dup) atomicOr(flags, 4);
 }
 
 // max |a|, max |c| as float bit patterns (order-independent)

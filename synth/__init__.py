@@ -97,6 +97,11 @@ CONFIGS = {
 }
 
 
+# Not a BASELINE.json config: a stress recipe for rows far beyond the streaming kernel's stage capacity (the paper's own fused
+# kernel stops at 8192 nonzeros per column) -- 8,000 users with exactly 20,000 eligible items each out of 40,000.
+CONFIGS["long20k"] = Config("long20k", I=8_000, J=40_000, deg=("const", 20_000), kappa=(0.3,), gammas=(1e-3,), iters=(100,))
+
+
 def get_config(name: str, I: int | None = None, **over) -> Config:
     """`cfgN`, `cfgN-tight`; I=... scales the number of users (items, degrees, values keep their recipe)."""
     tight = name.endswith("-tight")

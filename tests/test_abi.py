@@ -42,7 +42,7 @@ def test_struct_mirrors_match_the_header():
     import subprocess, tempfile
     fields = {"dualip_opts": ["projection", "p0", "reduction", "use_graph", "tuning", "precondition", "step_rule", "eta_min", "eta_max"],
               "dualip_info": ["I", "L", "group_lanes", "smem_bytes", "fix_scale_s", "streaming", "ntiles", "grad_kernel_count",
-                              "precondition", "L_step", "duals", "lambda_lo_smem", "checked_build", "checks_failed"],
+                              "precondition", "L_step", "duals", "lambda_lo_smem", "checked_build", "checks_failed", "long_rows", "long_row_threshold"],
               "dualip_scalars": ["g", "r_2", "gap"], "dualip_trace": ["capacity", "lambda", "eta"],
               "dualip_tuning": ["direct_kernel", "stages", "tile_units", "lambda_plan", "step_deal"]}
     src = '#include <stdio.h>\n#include <stddef.h>\n#include "dualip.h"\nint main(void){\n'

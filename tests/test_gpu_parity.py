@@ -249,6 +249,53 @@ def test_create_rejects_bad_input():
         pg.grad(torch.zeros(3, dtype=torch.float64, device="cuda"), 0.0)           # gamma must be > 0
 
 
+@pytest.mark.parametrize("J,m,long_lens,streaming", [(30_000, 1, [6_000, 28_000, 12_000], 1), (12_000, 2, [6_000, 11_000, 9_000], 1),
+                                                    (80_000, 1, [6_000, 70_000, 30_000], 0)])
+def test_long_rows_among_short_ones_cta_per_row(J, m, long_lens, streaming):
+    """A cfg3-like instance (a thousand short rows) with a handful of rows of 6,000-70,000 nonzeros in the middle of it.  On the
+    streaming plan the short rows stream (each long row is a tile of its own that the producer skips) and k_grad_long takes the
+    long ones, staged in shared memory; on the direct-load plan (J too large for lambda in shared memory) rows beyond 4096 go
+    to k_grad_long as well, the 70,000-long one recomputed per pass (it does not fit the staging buffer).  The two launches add
+    into the same accumulators.  Per-evaluation parity incl. a dense gamma (every nonzero of a long row in the support), the
+    count row, and a Jacobi trajectory."""
+    rng = np.random.default_rng(900 + m + J)
+    lens = [40] * 400 + long_lens[:1] + [25] * 300 + [long_lens[1], 3, long_lens[2]] + [50] * 500
+    d = _ragged(rng, len(lens), J, m, lens)
+    d["b"] = (d["b"] * 0.2).astype(np.float32)
+    for kind in ("simplex", "simplex_eq"):
+        po, pg = both(d, kind, 1.0, 0.0, jacobi=True)
+        info = pg.info()
+        assert (info.long_rows, info.streaming, info.max_row_len) == (3, streaming, max(long_lens)), (info.long_rows, info.long_row_threshold, info.streaming)
+        for gamma, ls in ((1e-3, 0.0), (1e-2, 0.3), (5.0, 0.3)):
+            assert_grad_parity(po, pg, rng.random(J * m) * ls, gamma, tag=f"mixed-long/{kind}/J={J}/g={gamma}")
+        assert_trajectory_parity(po, pg, [1e-1, 1e-2], [12, 12], tag=f"mixed-long/{kind}/J={J}/solve", jacobi=True)
+        pg.destroy()
+    po, pg = both(d, count_M=300.0)
+    assert_grad_parity(po, pg, np.concatenate([rng.random(J * m) * 0.2, [0.1]]), 1e-2, tag=f"mixed-long/count/J={J}")
+    pg.destroy()
+
+
+def test_long_unsorted_rows_are_validated_by_warps():
+    """Rows of thousands of nonzeros in random order: the duplicate check is warp-cooperative (k_validate_unsorted), not one
+    thread walking len^2 pairs; a duplicate at the two ends of a 6,000-long row is found, a clean instance is accepted."""
+    rng = np.random.default_rng(3)
+    J, lens = 9000, [6000, 3, 4500, 0, 6000]
+    rows, idx = [0], []
+    for d in lens:
+        idx.extend(rng.permutation(J)[:d].tolist()); rows.append(len(idx))
+    nnz = len(idx)
+    arr = dict(I=len(lens), J=J, m=1, row_ptr=np.array(rows, dtype=np.int64), item_idx=np.array(idx, dtype=np.int32),
+               c=-rng.random(nnz).astype(np.float32), a=np.ones(nnz, dtype=np.float32), b=np.ones(J, dtype=np.float32))
+    po, pg = both(arr)
+    assert_grad_parity(po, pg, np.zeros(J), 1e-2, tag="long unsorted")
+    pg.destroy()
+    bad = arr["item_idx"].copy()
+    bad[rows[5] - 1] = bad[rows[4]]                                  # last element of the last row := its first
+    with pytest.raises(pkg.DualipError) as e:
+        pkg.Problem.create(arr["I"], J, 1, arr["row_ptr"], bad, arr["c"], arr["a"], arr["b"])
+    assert e.value.code == -3
+
+
 def test_graph_replay_is_the_same_iteration():
     """use_graph: the stage loop replays a CUDA graph of chained one-launch iterations (beta_t and the trace row come
     from the device-side iteration state); lambda_T, x, the trace and the scalars carry the same bits as direct
@@ -502,10 +549,21 @@ def test_very_long_rows_and_no_users():
     d["b"] = (d["b"] * 0.05).astype(np.float32)
     for kind, p0, p1 in (("simplex", 1.0, 0.0), ("boxcut", 0.001, 1.0), ("simplex_eq", 1.0, 0.0)):
         po, pg = both(d, kind, p0, p1)
-        assert pg.info().streaming == 0 and pg.info().max_row_len == 20_000
+        info = pg.info()
+        assert info.max_row_len == 20_000
+        if kind == "boxcut":            # genuine box-cut (ub < z): long rows stay on the direct-load kernel's whole-warp path
+            assert info.streaming == 0 and info.long_rows == 0
+        else:                           # simplex kinds: the long rows get a CTA each (k_grad_long), the rest streams
+            assert info.streaming == 1 and info.long_rows >= 10 and 256 <= info.long_row_threshold < 9000
         for gamma, ls in ((1.0, 0.0), (1e-2, 0.5), (1e-4, 0.5)):
             assert_grad_parity(po, pg, rng.random(J) * ls, gamma, tag=f"long/{kind}/g={gamma}")
         pg.destroy()
+    # the same rows on the direct-load plan: rows beyond 4096 nonzeros go to k_grad_long there as well
+    po, pg = both(d, direct_kernel=True)
+    assert pg.info().streaming == 0 and pg.info().long_row_threshold == 4096 and pg.info().long_rows >= 10
+    assert_grad_parity(po, pg, rng.random(J) * 0.5, 1e-2, tag="long/direct")
+    assert_trajectory_parity(po, pg, [1e-1, 1e-2], [10, 10], tag="long/direct/solve")
+    pg.destroy()
     e = dict(I=0, J=4, m=1, row_ptr=np.zeros(1, dtype=np.int64), item_idx=np.zeros(0, dtype=np.int32),
              c=np.zeros(0, dtype=np.float32), a=np.zeros(0, dtype=np.float32), b=np.array([1, 2, 3, 4], dtype=np.float32))
     po, pg = both(e)

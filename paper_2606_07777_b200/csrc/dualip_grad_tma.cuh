@@ -35,8 +35,8 @@ namespace dualip_dev {
 constexpr int kTmaConsumerWarps = DUALIP_NWC;  // consumer warps of the streaming kernel (+ 1 producer warp)
 
 constexpr int kRowCost = 8;            // each row costs this many "nonzero units" when cutting tiles
-constexpr int kTmaStagesMax = 4;
-constexpr int kTmaHeaderBytes = 128 + 256 * kTmaConsumerWarps;   // mbarriers + words + per-warp candidate lists (multiple of 128)
+constexpr int kTmaStagesMax = 8;
+constexpr int kTmaHeaderBytes = 256 + 256 * kTmaConsumerWarps;   // mbarriers (2 x 8) + words + per-warp candidate lists (multiple of 128)
 
 struct TileEntry {                     // 32 bytes, one per tile (+1 sentinel)
     long long row0;                    // first row of the tile
@@ -625,11 +625,11 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const __grid_con
     constexpr int NT = 32 * (NWC + 1);
     const int mm = M > 0 ? M : p.m;
     const int JM = p.J * mm;
-    // layout: [full[4], empty[4] mbarriers: 64 B][words: 64 B][candidate lists: 256 B per consumer warp][lam_hi JM*4]
+    // layout: [full[8], empty[8] mbarriers: 128 B][words: 128 B][candidate lists: 256 B per consumer warp][lam_hi JM*4]
     //         [acc 2*JM*4 (ACC_SMEM)][lam_lo JM*4 (decided per launch, below)][stages]
     unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_tma);
-    unsigned* s_words = reinterpret_cast<unsigned*>(smem_tma + 64);       // [0] = max |lambda_hi| as float bits
-    int* cand_list = reinterpret_cast<int*>(smem_tma + 128);              // 64 positions per consumer warp (candidate path B)
+    unsigned* s_words = reinterpret_cast<unsigned*>(smem_tma + 128);      // [0] = max |lambda_hi| as float bits
+    int* cand_list = reinterpret_cast<int*>(smem_tma + 256);              // 64 positions per consumer warp (candidate path B)
     float* s_hi32 = reinterpret_cast<float*>(smem_tma + kTmaHeaderBytes);
     unsigned* a_lo = reinterpret_cast<unsigned*>(s_hi32 + JM);
     unsigned* a_hi = a_lo + JM;
@@ -950,6 +950,9 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const __grid_con
 #pragma unroll
                                         for (int e = 0; e < 4; ++e) { w[e] = -CUDART_INF_F; pe[e] = 0; }
                                     }
+                                    // one ballot + prefix popc per slot.  (A per-lane count + an inclusive prefix sum over the
+                                    // group's lanes -- a third of the instructions -- was measured SLOWER: cfg5 at gamma = 0.1
+                                    // 4.36 -> 4.69 ms; the shuffle chain is serial, the four ballots are independent.)
 #pragma unroll
                                     for (int e = 0; e < 4; ++e) {
                                         const bool isc = w[e] > thr;

@@ -314,7 +314,8 @@ class Leg:
         sc = self.pkg.Scalars()
         prob.grad(lam, self.gamma, scalars=sc)                      # state the timed steps ended in (untimed)
         torch.cuda.synchronize()
-        state = {"g": sc.g, "r_inf": sc.r_inf, "active_duals": int((lam > 0).sum().item()), "lambda_max": float(lam.max().item())}
+        state = {"g": sc.g, "r_inf": sc.r_inf, "active_duals": int((lam > 0).sum().item()), "lambda_max": float(lam.max().item()),
+                 "table4": sc.table4(), "lambda_lo_smem": int(prob.info().lambda_lo_smem)}
         return {"ms_total": ms_total, "kern_ms": kern_ms, "launches": int(launches), "timed": int(inf.grad_kernel_count),
                 "clocks": clocks, "state": state}
 

@@ -52,6 +52,12 @@ class Scalars(ctypes.Structure):
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
 
+    def table4(self):
+        """The columns of the paper's solution-quality report (Table 4), named as there: primal objective (of
+        the ridge problem: c'x + gamma/2 |x|^2), dual objective, absolute primal-dual gap, maximum positive constraint violation
+        ("slack").  Field selection only: every number was computed by the kernel's epilogue."""
+        return {"primal": self.obj + self.reg, "dual": self.g, "gap": abs(self.gap), "slack": self.r_inf}
+
 
 class ShardExtents(ctypes.Structure):
     _fields_ = [("I", ctypes.c_int64), ("nnz", ctypes.c_int64), ("max_abs_a", ctypes.c_float), ("max_abs_c", ctypes.c_float)]

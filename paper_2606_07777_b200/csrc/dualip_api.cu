@@ -211,7 +211,10 @@ bool plan_tma(dualip* h, Plan& pl, long long max_len) {
     size_t off = kTmaHeaderBytes + lam_bytes + (acc ? 8 : 0) * JM;
     off = (off + 127) & ~(size_t)127;
     pl.smem = off + (size_t)pl.stage_bytes * stages;
-    return pl.smem <= kSmemBudget;
+    if (pl.smem > kSmemBudget) return false;
+    // room for lambda's low word where the budget has it (small plans): a launch that stages it then keeps all its stages
+    if (!lo) pl.smem = std::min(kSmemBudget, pl.smem + 4 * JM + 128);
+    return true;
 }
 
 int make_plan(dualip* h) {

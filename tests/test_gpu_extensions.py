@@ -198,3 +198,33 @@ def test_set_c_rejects_a_misaligned_borrowed_pointer():
     torch.cuda.synchronize()
     assert abs(sc2.obj - 0.5 * sc0.obj) <= 1e-4 * abs(sc0.obj)      # x changes only where |c| / gamma < 1
     pg.destroy()
+
+
+def test_per_launch_lambda_plan_decides_from_lambda_and_gamma_and_changes_no_bit():
+    """J*m = 10,000 duals: too many for lambda's low word to be sized into the plan, so each LAUNCH decides (k_grad_tma prologue):
+    at lambda = 0 the fp32 dual is exact enough and every stage is kept; at a busy lambda and small gamma the low word is staged
+    and a stage given up.  Forcing either choice (tuning.lambda_plan) gives the same bits: both exact paths use the two-word dual."""
+    cfg = synth.get_config("cfg3-tight", I=30_000)
+    inst = synth.generate(cfg)
+    po, auto = from_instance(inst, group_lanes=8)
+    _, never = from_instance(inst, group_lanes=8, lambda_plan=1)
+    _, always = from_instance(inst, group_lanes=8, lambda_plan=2)
+    lam0, lam1 = np.zeros(inst.J), synth.probe_lambda(inst, 0, 0.05).numpy()
+    sc, g0, x0 = gpu_grad(auto, lam0, 1e-3)
+    assert auto.info().lambda_lo_smem == 0
+    sc, g1, x1 = gpu_grad(auto, lam1, 1e-3)
+    assert auto.info().lambda_lo_smem == 1
+    sc, g2, x2 = gpu_grad(auto, lam1, 10.0)                      # the same lambda at a gamma where its fp32 rounding cannot matter
+    assert auto.info().lambda_lo_smem == 0
+    for other, want in ((never, 0), (always, 1)):
+        sc, g, x = gpu_grad(other, lam1, 1e-3)
+        assert other.info().lambda_lo_smem == want
+        assert np.array_equal(g, g1) and np.array_equal(x, x1)
+    assert_grad_parity(po, auto, lam1, 1e-3, tag="lambda plan")
+    for P in (auto, never, always):
+        P.destroy()
+
+
+def test_table4_columns():
+    sc = pkg.Scalars(g=-10.0, obj=-9.0, reg=0.5, r_inf=1e-3, r_2=2e-3, gap=1.5)
+    assert sc.table4() == {"primal": -8.5, "dual": -10.0, "gap": 1.5, "slack": 1e-3}

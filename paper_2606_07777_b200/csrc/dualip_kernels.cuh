@@ -125,7 +125,7 @@ __device__ __forceinline__ void contribute(const GradParams& p, unsigned* s_lo, 
         if (k < nm) {
             const long long f = to_fix(aa[k] * x, p.scale_s);
             if (ACC_SMEM) fix_add_smem(s_lo + j * nm + k, s_hi + j * nm + k, f);
-            else atomicAdd(p.s_fix + (long long)j * nm + k, (unsigned long long)f);
+            else asm volatile("red.global.add.u64 [%0], %1;" ::"l"(p.s_fix + (long long)j * nm + k), "l"((unsigned long long)f) : "memory");   // RED, not ATOM
         }
     }
 }

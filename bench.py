@@ -349,8 +349,15 @@ class Leg:
         peak, peak_src = measured_peak()
         achieved = self.alg_bytes / (m["kern_ms"] * 1e-3) / 1e9 if m["kern_ms"] > 0 else None
         traffic, src = ncu_traffic(leg_name) if self.args.users is None else (None, None)
+        dram = (traffic / (m["kern_ms"] * 1e-3) / 1e9) if (traffic and m["kern_ms"] > 0) else None
         return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": (achieved / peak) if achieved else None,
-                "traffic": traffic, "traffic_source": src, "peak_source": peak_src, "kernel": self.kernel_name(), "kernel_ms": m["kern_ms"],
+                "traffic": traffic, "traffic_source": src, "dram_gbs": dram, "dram_frac": (dram / peak) if dram else None,
+                "bytes_note": ("achieved = ALGORITHMIC bytes of the ABI's format (int32 index + fp32 c + m fp32 a per nonzero, int64 row_ptr per user: "
+                               "SURVEY 8(d)) / kernel time.  The streaming kernel reads a uint16 copy of the item indices kept by dualip_create "
+                               "(J < 65536 whenever lambda fits in shared memory: SURVEY 8(d)'s 'legitimate byte reduction'), i.e. it moves 2 bytes "
+                               "per nonzero less than that: traffic / dram_gbs / dram_frac are what actually crosses the HBM interface (ncu), so frac "
+                               "can exceed dram_frac and 1" if self.info.streaming else None),
+                "peak_source": peak_src, "kernel": self.kernel_name(), "kernel_ms": m["kern_ms"],
                 "kernel_launches_timed": m["timed"], "algorithmic_bytes_per_launch": self.alg_bytes,
                 "kernel_share_of_step": m["kern_ms"] * steps / m["ms_total"] if m["ms_total"] > 0 else None}
 

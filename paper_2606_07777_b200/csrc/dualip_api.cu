@@ -65,6 +65,7 @@ struct dualip {
     double* scalars_dev = nullptr;
     float* x_stage = nullptr;
     dualip_dev::TileEntry* tiles = nullptr;
+    unsigned short* idx16 = nullptr;       // streaming plan: item_idx as 16-bit values (owned, 2 bytes per nonzero)
     unsigned char* ctl = nullptr;          // [IterState (16 B)][done counter (4 B)] -- see grid_epilogue
     // DUALIP_RED_CSC: item-sorted permutation (a0) and the per-iteration scratch of the atomics-free reduction
     bool csc = false, perm64 = false;
@@ -166,7 +167,7 @@ bool plan_tma(dualip* h, Plan& pl, long long max_len) {
     const size_t JM = (size_t)h->J * h->m;
     const int red = h->opts.reduction;
     if (h->opts.projection == DUALIP_PROJ_BOX || h->nnz == 0) return false;
-    if (max_len > 8192) return false;
+    if (max_len > 8192 || h->J > 65535) return false;       // (J is far below that whenever lambda fits in shared memory)
     if (((uintptr_t)h->row_ptr | (uintptr_t)h->idx | (uintptr_t)h->c | (uintptr_t)h->a) & 15) return false;
     // Shared memory: RN_f32(lambda) always (the filter's operand, 4 B per dual).  Its low word joins it while the
     // pair stays under 64 KB (otherwise the exact path reads the fp64 lambda through L2: it runs once per row at
@@ -190,8 +191,8 @@ bool plan_tma(dualip* h, Plan& pl, long long max_len) {
     const int s_hi = h->opts.tuning.stages ? h->opts.tuning.stages : 3, s_lo = h->opts.tuning.stages ? h->opts.tuning.stages : 2;
     for (int S = s_hi; S >= s_lo && TN < 256; --S) {
         stage_bytes = (avail / S) & ~(size_t)127;
-        const long long over = 80 + (max_len + 8 + 72) * (8 + 4 * m);
-        long long tn = ((long long)stage_bytes - over) / (9 + 4 * m);
+        const long long over = 80 + (max_len + 16 + 72) * (6 + 4 * m);
+        long long tn = ((long long)stage_bytes - over) / (7 + 4 * m);
         tn = tn > 0 ? (tn & ~63ll) : 0;
         if (tn >= (S >= 3 ? 512 : 256)) { TN = tn; stages = S; }
     }
@@ -203,9 +204,9 @@ bool plan_tma(dualip* h, Plan& pl, long long max_len) {
     if (h->opts.tuning.tile_units >= 256 && h->opts.tuning.tile_units < TN) TN = h->opts.tuning.tile_units & ~63ll;
     pl.tma = true; pl.acc_smem = acc; pl.lam_smem = true;
     pl.TN = TN; pl.stages = stages;
-    pl.cap_nz = (int)((TN + max_len + 8 + 72 + 3) & ~3ll);   // +72: lanes may read up to 2*32+2 slots past a row end (m = 2)
+    pl.cap_nz = (int)((TN + max_len + 16 + 72 + 7) & ~7ll);  // +72: lanes may read up to 2*32+2 slots past a row end (m = 2)
     pl.cap_rows = (int)((TN / kRowCost + 6 + 1) & ~1ll);
-    size_t sb = (size_t)pl.cap_nz * (8 + 4 * m) + (size_t)pl.cap_rows * 8 + 32;
+    size_t sb = (size_t)pl.cap_nz * (6 + 4 * m) + (size_t)pl.cap_rows * 8 + 32;
     pl.stage_bytes = (int)((sb + 127) & ~(size_t)127);
     pl.ntiles = (units + TN - 1) / TN;
     size_t off = kTmaHeaderBytes + lam_bytes + (acc ? 8 : 0) * JM;
@@ -487,7 +488,7 @@ void prepare_iter(const dualip* h, IterLaunch& L, const double* lam_dev, double 
         TmaParams& tp = L.tp;
         tp.g = L.p; tp.f = L.f; tp.tiles = h->tiles; tp.ntiles = h->plan.ntiles; tp.cap_nz = h->plan.cap_nz; tp.cap_rows = h->plan.cap_rows;
         tp.stages = h->plan.stages; tp.stage_bytes = h->plan.stage_bytes;
-        tp.nnz4 = h->nnz & ~3ll; tp.rows2 = (h->I + 1) & ~1ll; tp.lo_policy = h->plan.lo_policy;
+        tp.nnz8 = h->nnz & ~7ll; tp.idx16 = h->idx16; tp.rows2 = (h->I + 1) & ~1ll; tp.lo_policy = h->plan.lo_policy;
         tp.smem_total = (int)h->plan.smem; tp.lo_flag = reinterpret_cast<int*>(h->ctl + 32);
         tp.check_word = reinterpret_cast<unsigned*>(h->ctl + 36);
         tp.dyn_steps = h->opts.tuning.step_deal == 2 ? 1 : 0;
@@ -729,7 +730,7 @@ void dualip_destroy(dualip_t* h) {
     if (h->own_rows) { cudaFree((void*)h->row_ptr); cudaFree((void*)h->idx); cudaFree((void*)h->a); }
     if (h->own_c) cudaFree((void*)h->c);
     cudaFree(h->b); cudaFree(h->s_fix); cudaFree(h->lam_cur); cudaFree(h->y); cudaFree(h->lam_stage);
-    cudaFree(h->grad_stage); cudaFree(h->y_prev); cudaFree(h->g_prev); cudaFree(h->scalars_dev); cudaFree(h->step_scale); cudaFree(h->row_eq); cudaFree(h->x_stage); cudaFree(h->tiles);
+    cudaFree(h->grad_stage); cudaFree(h->y_prev); cudaFree(h->g_prev); cudaFree(h->scalars_dev); cudaFree(h->step_scale); cudaFree(h->row_eq); cudaFree(h->x_stage); cudaFree(h->tiles); cudaFree(h->idx16);
     drop_graph(h);
     cudaFree(h->ctl);
     cudaFree(h->csc_perm); cudaFree(h->col_ptr); cudaFree(h->chunk_ptr); cudaFree(h->chunk_item); cudaFree(h->csc_partial);
@@ -873,6 +874,8 @@ int dualip_create(dualip_t** out, int64_t I, int32_t J, int32_t m, const int64_t
         }
         if (h->long_thr > 0 && (rc = build_long_list(h, st)) != 0) goto fail;
         if (h->plan.tma) {
+            if ((rc = dev_alloc(h, &h->idx16, (size_t)nnz + 16)) != 0) goto fail;
+            k_encode_idx16<<<grid_for(nnz, 256, h->num_sms), 256, 0, st>>>(h->idx, nnz, h->idx16); h->launches++;
             if ((rc = dev_alloc(h, &h->tiles, (size_t)h->plan.ntiles + 1)) != 0) goto fail;
             k_build_tiles<<<grid_for(h->plan.ntiles + 1, 128, h->num_sms), 128, 0, st>>>(h->row_ptr, I, h->plan.TN, h->plan.ntiles, h->tiles);
             h->launches++;

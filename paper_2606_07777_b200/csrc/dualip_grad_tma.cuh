@@ -52,7 +52,8 @@ struct TmaParams {
     int cap_rows;                      // row_ptr entries per stage (even)
     int stages;
     int stage_bytes;                   // bytes of one stage (multiple of 16)
-    long long nnz4;                    // nnz rounded down to a multiple of 4 (bulk copies stop there)
+    long long nnz8;                    // nnz rounded down to a multiple of 8 (bulk copies stop there)
+    const unsigned short* __restrict__ idx16;   // item_idx as 16-bit values (a0: k_encode_idx16)
     long long rows2;                   // (I+1) rounded down to a multiple of 2
     int lo_policy;                     // lambda's low word in shared memory: 0 = decided per launch (see k_grad_tma), 1 = never, 2 = always
     int smem_total;                    // dynamic shared memory of the launch (bytes)
@@ -123,17 +124,21 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned by
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
-// One stage: [idx cap_nz*4][c cap_nz*4][a cap_nz*4*m][row_ptr cap_rows*8][meta: int nrows, int rpo, long long nzb, pad]
+// One stage: [idx16 cap_nz*2][c cap_nz*4][a cap_nz*4*m][row_ptr cap_rows*8][meta: int nrows, int rpo, long long nzb, pad]
+// The item indices are streamed as 16-BIT values: the streaming plan exists only while RN_f32(lambda) fits in shared memory next
+// to the stages, which bounds J*m by ~48,000, so J < 65,536 always, and dualip_create keeps a uint16 copy of item_idx for this
+// kernel (2 bytes per nonzero of device memory; the ABI's int32 array is untouched and still what the other kernels read).  Per
+// nonzero the kernel then moves 6 + 4m bytes instead of 8 + 4m from HBM and through shared memory: a stage holds 20 % more rows.
 struct StageMeta { int nrows; int rpo; long long nzb; int next_step; int pad32; long long pad; };   // next_step: dynamic dealing
 struct StageView {
-    const int* idx; const float* c; const float* a; const long long* rp; const StageMeta* meta;
+    const unsigned short* idx; const float* c; const float* a; const long long* rp; const StageMeta* meta;
 };
 __device__ __forceinline__ StageView stage_view(unsigned char* base, int cap_nz, int cap_rows, int mm) {
     StageView v;
-    v.idx = reinterpret_cast<const int*>(base);
-    v.c = reinterpret_cast<const float*>(base + (size_t)cap_nz * 4);
-    v.a = reinterpret_cast<const float*>(base + (size_t)cap_nz * 8);
-    v.rp = reinterpret_cast<const long long*>(base + (size_t)cap_nz * (8 + 4 * mm));
+    v.idx = reinterpret_cast<const unsigned short*>(base);
+    v.c = reinterpret_cast<const float*>(base + (size_t)cap_nz * 2);
+    v.a = reinterpret_cast<const float*>(base + (size_t)cap_nz * 6);
+    v.rp = reinterpret_cast<const long long*>(base + (size_t)cap_nz * (6 + 4 * mm));
     v.meta = reinterpret_cast<const StageMeta*>(v.rp + cap_rows);
     return v;
 }
@@ -312,7 +317,8 @@ __device__ __forceinline__ void filter_load(const StageView& v, const float* __r
     DUALIP_CHECK_POS(q); DUALIP_CHECK_POS(M == 2 ? q + 2 * G + 1 : q + 3);
     if (M == 2) {
         const int q2 = q + 2 * G;
-        const int2 jA = *reinterpret_cast<const int2*>(v.idx + q), jB = *reinterpret_cast<const int2*>(v.idx + q2);
+        const unsigned wA = *reinterpret_cast<const unsigned*>(v.idx + q), wB = *reinterpret_cast<const unsigned*>(v.idx + q2);
+        const int2 jA = make_int2((int)(wA & 0xffffu), (int)(wA >> 16)), jB = make_int2((int)(wB & 0xffffu), (int)(wB >> 16));
         const float2 cA = *reinterpret_cast<const float2*>(v.c + q), cB = *reinterpret_cast<const float2*>(v.c + q2);
         const float4 aA = *reinterpret_cast<const float4*>(v.a + 2 * q), aB = *reinterpret_cast<const float4*>(v.a + 2 * q2);
         const int jj[4] = {jA.x, jA.y, jB.x, jB.y};
@@ -326,7 +332,8 @@ __device__ __forceinline__ void filter_load(const StageView& v, const float* __r
             w[e] = -fmaf(ay[e], l2.y, fmaf(ax[e], l2.x, cv[e]));
         }
     } else {
-        const int4 j4 = *reinterpret_cast<const int4*>(v.idx + q);
+        const uint2 w4 = *reinterpret_cast<const uint2*>(v.idx + q);
+        const int4 j4 = make_int4((int)(w4.x & 0xffffu), (int)(w4.x >> 16), (int)(w4.y & 0xffffu), (int)(w4.y >> 16));
         const float4 c4 = *reinterpret_cast<const float4*>(v.c + q);
         const int jj[4] = {j4.x, j4.y, j4.z, j4.w};
         DUALIP_CHECK_ITEM(jj[0]); DUALIP_CHECK_ITEM(jj[1]); DUALIP_CHECK_ITEM(jj[2]); DUALIP_CHECK_ITEM(jj[3]);
@@ -654,7 +661,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const __grid_con
 #ifdef DUALIP_CHECKED
     if (threadIdx.x == 0) {
         g_chk_word = tp.check_word; g_chk_cap_nz = tp.cap_nz; g_chk_J = p.J; g_chk_cap_rows = tp.cap_rows; g_chk_nnz = p.nnz;
-        if ((size_t)tp.stage_bytes < (size_t)tp.cap_nz * (8 + 4 * mm) + (size_t)tp.cap_rows * 8 + sizeof(StageMeta)) atomicOr(tp.check_word, 1u << CHK_STAGE_BYTES);
+        if ((size_t)tp.stage_bytes < (size_t)tp.cap_nz * (6 + 4 * mm) + (size_t)tp.cap_rows * 8 + sizeof(StageMeta)) atomicOr(tp.check_word, 1u << CHK_STAGE_BYTES);
     }
     __syncthreads();
 #endif
@@ -707,7 +714,7 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const __grid_con
         // the INDEX array of a stage must always hold a valid item index (c and a may hold anything: those slots are masked)
         for (int s = 0; s < nstages; ++s) {
             uint4* sp = reinterpret_cast<uint4*>(stage0 + (size_t)s * tp.stage_bytes);
-            for (int q = threadIdx.x; q < tp.cap_nz / 4; q += NT) sp[q] = make_uint4(0u, 0u, 0u, 0u);
+            for (int q = threadIdx.x; q < tp.cap_nz / 8; q += NT) sp[q] = make_uint4(0u, 0u, 0u, 0u);
         }
         fence_proxy_async();                                             // generic-proxy zeros before the first bulk copy
     }
@@ -738,31 +745,31 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const __grid_con
                 if (tn < tp.ntiles) { ncur = tp.tiles[tn]; nnxt = tp.tiles[tn + 1]; }
                 mbar_wait(&bars[kTmaStagesMax + s], ph ^ 1u);                        // stage free?
                 unsigned char* sb = stage0 + (size_t)s * tp.stage_bytes;
-                int* d_idx = reinterpret_cast<int*>(sb);
-                float* d_c = reinterpret_cast<float*>(sb + (size_t)tp.cap_nz * 4);
-                float* d_a = reinterpret_cast<float*>(sb + (size_t)tp.cap_nz * 8);
-                long long* d_rp = reinterpret_cast<long long*>(sb + (size_t)tp.cap_nz * (8 + 4 * mm));
+                unsigned short* d_idx = reinterpret_cast<unsigned short*>(sb);
+                float* d_c = reinterpret_cast<float*>(sb + (size_t)tp.cap_nz * 2);
+                float* d_a = reinterpret_cast<float*>(sb + (size_t)tp.cap_nz * 6);
+                long long* d_rp = reinterpret_cast<long long*>(sb + (size_t)tp.cap_nz * (6 + 4 * mm));
                 StageMeta* d_meta = reinterpret_cast<StageMeta*>(d_rp + tp.cap_rows);
                 const long long r0 = cur.row0, p0 = cur.nz0;
                 long long r1 = nxt.row0, p1 = nxt.nz0;
                 if (tp.row_cap > 0 && r1 - r0 == 1 && p1 - p0 > tp.row_cap) { r1 = r0; p1 = p0; }   // a long row's own tile: nothing to stage
-                const long long p0a = p0 & ~3ll;
-                long long p1a = (p1 + 3) & ~3ll;
-                if (p1a > tp.nnz4) p1a = tp.nnz4 > p0a ? tp.nnz4 : p0a;              // never read past the arrays
+                const long long p0a = p0 & ~7ll;                                      // 8 nonzeros = 16 bytes of 16-bit indices
+                long long p1a = (p1 + 7) & ~7ll;
+                if (p1a > tp.nnz8) p1a = tp.nnz8 > p0a ? tp.nnz8 : p0a;              // never read past the arrays
                 const long long r0a = r0 & ~1ll;
                 long long r1a = (r1 + 2) & ~1ll;                                       // rows r0a .. r1 inclusive, even count
                 if (r1a > tp.rows2) r1a = tp.rows2 > r0a ? tp.rows2 : r0a;
                 d_meta->nrows = (int)(r1 - r0); d_meta->rpo = (int)(r0 - r0a); d_meta->nzb = p0a; d_meta->next_step = 0;
                 // tails that are not a whole 16-byte chunk (only at the very end of the arrays): plain copies
                 for (long long q = p1a > p0a ? p1a : p0a; q < p1; ++q) {
-                    d_idx[q - p0a] = p.idx[q]; d_c[q - p0a] = p.c[q];
+                    d_idx[q - p0a] = tp.idx16[q]; d_c[q - p0a] = p.c[q];
                     for (int f = 0; f < mm; ++f) d_a[(q - p0a) * mm + f] = p.a[q * mm + f];
                 }
                 for (long long r = r1a > r0a ? r1a : r0a; r <= r1; ++r) d_rp[r - r0a] = p.row_ptr[r];
                 const unsigned nz = (unsigned)(p1a > p0a ? p1a - p0a : 0), nr = (unsigned)(r1a > r0a ? r1a - r0a : 0);
-                mbar_expect_tx(&bars[s], nz * (8u + 4u * (unsigned)mm) + nr * 8u);     // release: meta/claim/tail stores
+                mbar_expect_tx(&bars[s], nz * (6u + 4u * (unsigned)mm) + nr * 8u);     // release: meta/claim/tail stores
                 if (nz) {
-                    bulk_g2s(d_idx, p.idx + p0a, nz * 4u, &bars[s]);
+                    bulk_g2s(d_idx, tp.idx16 + p0a, nz * 2u, &bars[s]);
                     bulk_g2s(d_c, p.c + p0a, nz * 4u, &bars[s]);
                     bulk_g2s(d_a, p.a + p0a * mm, nz * 4u * (unsigned)mm, &bars[s]);
                 }
@@ -1074,6 +1081,11 @@ __global__ void __launch_bounds__(32 * (NWC + 1), 1) k_grad_tma(const __grid_con
 }
 
 #ifdef DUALIP_HOST_KERNELS
+// a0: the 16-bit copy of the item indices the streaming kernel reads (J < 65,536 on that plan)
+__global__ void k_encode_idx16(const int* __restrict__ idx, long long nnz, unsigned short* out) {
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < nnz; q += (long long)gridDim.x * blockDim.x) out[q] = (unsigned short)idx[q];
+}
+
 // a0: tile table from an explicit list of cut rows (the streaming plan with long rows isolated: dualip_api.cu)
 __global__ void k_fill_tiles(const long long* __restrict__ row_ptr, const long long* __restrict__ cuts, long long ntiles, TileEntry* tiles) {
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t <= ntiles; t += (long long)gridDim.x * blockDim.x) {

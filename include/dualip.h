@@ -184,7 +184,9 @@ typedef struct {
  *   item_idx[nnz] int32 in [0,J), distinct within a row, any order;  c[nnz];  a[nnz*m];  b[J*m].
  *   opts may be NULL (defaults).
  * Work done: copy (or borrow), validation kernels, L (R2), column |a| sums and sum|c| for the fixed-point
- * scales, row-length statistics, launch plan; with DUALIP_RED_CSC also the item-sorted permutation.
+ * scales, row-length statistics, launch plan (tile table; the list of long rows; a uint16 copy of item_idx that the
+ * streaming kernel reads instead of the int32 array -- 2 bytes per nonzero of device memory, counted in
+ * dualip_info.bytes_resident, also with borrow = 1); with DUALIP_RED_CSC also the item-sorted permutation.
  * Synchronises `stream`.  Errors: EINVAL, ERANGE, EDUP, ENOMEM, ECUDA, EUNSUPPORTED.
  */
 int dualip_create(dualip_t** out, int64_t I, int32_t J, int32_t m, const int64_t* row_ptr,

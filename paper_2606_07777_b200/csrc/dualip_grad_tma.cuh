@@ -2,7 +2,7 @@
 // TMA bulk copies (cp.async.bulk, SASS UBLKCP) behind mbarriers, one persistent CTA per SM.
 //
 //   warp 0      producer: for each of this CTA's tiles, waits for a free stage, then issues one bulk copy per
-//               array (item_idx, c, a, row_ptr segment) that completes on the stage's "full" mbarrier.
+//               array (16-bit item indices, c, a, row_ptr segment) that completes on the stage's "full" mbarrier.
 //   warps 1..   consumers: wait for "full", take their row-steps of the tile (G lanes per row, 2*32/G rows per step,
 //               steps dealt round-robin over the CTA's step sequence), read the rows straight from shared memory,
 //               and release the stage.

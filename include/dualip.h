@@ -42,7 +42,8 @@ enum {
     DUALIP_EDUP = -3,         /* an item appears twice in one user's row (R11) */
     DUALIP_ENOMEM = -4,       /* host or device allocation failed */
     DUALIP_ECUDA = -5,        /* a CUDA runtime call failed (no device, launch failure, ...) */
-    DUALIP_EUNSUPPORTED = -6  /* valid request this build cannot serve (e.g. reduction strategy needs more shared memory) */
+    DUALIP_EUNSUPPORTED = -6, /* valid request this build cannot serve (e.g. reduction strategy needs more shared memory) */
+    DUALIP_ETOOBIG = -7       /* dualip_grad_static only: J*m exceeds DUALIP_STATIC_MAX_DUALS, the compiled-in size of its scratch */
 };
 
 /* Per-user simple set C_i (R5, R10, R16).  Parameters p0,p1 of dualip_opts:
@@ -297,6 +298,48 @@ int dualip_set_profiling(dualip_t* h, int on);
 
 /* Fills *info.  With profiling on, blocks until the timed launches have finished. */
 int dualip_get_info(dualip_t* h, dualip_info* info);
+
+/*
+ * a1-a5 (+a8) without a handle and WITHOUT ANY ALLOCATION -- for callers that may not allocate device memory.
+ *
+ * Everything else in this header needs a handle, and dualip_create builds one out of cudaMalloc'd buffers.  That rules the
+ * library out for code that is not allowed to allocate where it runs: a plug-in inside a host application that owns all device
+ * memory and forbids cudaMalloc behind its back; a service whose memory budget was reserved in full at start-up; a
+ * latency-critical path that cannot take the device-wide synchronisation cudaMalloc and cudaFree imply.  This call computes the
+ * same evaluation as dualip_create + dualip_grad (Eq. 2-4: grad g = A x* - b, g, obj, reg, the residuals, optionally x)
+ * for one lambda, and calls no cudaMalloc / cudaFree / allocating library routine, on the device or on the host: the scratch
+ * its kernels reduce into (fixed-point item accumulators, scalar accumulators, column sums, a counter) is a fixed array
+ * compiled into the library.
+ *
+ *   I, J, m, row_ptr[I+1], item_idx[nnz], c[nnz], a[nnz*m], b[J*m]: as for dualip_create, but ALL DEVICE pointers (a host
+ *     pointer would need a staging buffer: DUALIP_EINVAL), used in place, never copied; rows are NOT validated (as with
+ *     opts.validate = 0: an item index outside [0,J) is undefined behaviour); row_ptr[0] != 0 gives DUALIP_ERANGE.
+ *   projection, p0, p1: DUALIP_PROJ_* and its parameters, as in dualip_opts.
+ *   lambda[J*m] device in, gamma > 0;  grad[J*m], scalars, x[nnz]: DEVICE out, each may be NULL.
+ *   No equality rows, no global-count row, no AGD update: one evaluation, inequality rows.
+ *
+ * Limit: J*m <= DUALIP_STATIC_MAX_DUALS, else DUALIP_ETOOBIG and nothing is launched.  The scratch costs
+ * 8 * (8 + 2 * DUALIP_STATIC_MAX_DUALS) bytes = 448 KB of device memory on every GPU that loads the library, held until the
+ * process exits, whether or not this function is ever called.
+ *
+ * Cost: with no handle to keep them in, the create-time constants behind the fixed-point scales (max |a|, max |c|, the largest
+ * column sum of |a|, sum |c|) are recomputed on every call: two extra passes over the rows, and `stream` is synchronised three
+ * times inside the call (row_ptr[I], then each pass).  The gradient kernel itself is the direct-load kernel (k_grad, lambda in
+ * shared memory, RED.ADD.64 item sums), not the streaming one, and is only enqueued: the outputs are ready when `stream` is.
+ * Results agree with dualip_grad on a handle of the same rows within the parity tolerances of tests/gpu_util.py (same
+ * fixed-point scales; only the lane order of the projection differs).  Use a handle when you can allocate.
+ *
+ * Shared state -- read this:
+ *   - The first call on each device looks up the device address of the scratch array and queries the device (no allocation).
+ *     Make that first call, with the device current, BEFORE starting any stream capture on that device.
+ *   - All calls on a device use the SAME array, which keeps the previous call's contents; every call clears the part it uses
+ *     first, so calls one after another on one stream are independent.  Two calls whose GPU work can overlap -- different
+ *     streams, or two host threads -- race on it and return garbage without an error.  Serialise them.
+ */
+#define DUALIP_STATIC_MAX_DUALS 28672
+int dualip_grad_static(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr, const int32_t* item_idx, const float* c,
+                       const float* a, const float* b, int32_t projection, double p0, double p1, const double* lambda,
+                       double gamma, double* grad, dualip_scalars* scalars, float* x, void* stream);
 
 /* Frees everything the handle owns.  NULL is accepted. */
 void dualip_destroy(dualip_t* h);

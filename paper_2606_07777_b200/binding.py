@@ -16,12 +16,14 @@ PROJ_SIMPLEX_INEQ, PROJ_BOX, PROJ_BOXCUT, PROJ_SIMPLEX_EQ = 0, 1, 2, 3
 RED_AUTO, RED_SMEM, RED_GLOBAL, RED_CSC = 0, 1, 2, 3
 PRECOND_NONE, PRECOND_JACOBI = 0, 1
 STEP_FIXED, STEP_ADAPTIVE = 0, 1
+STATIC_MAX_DUALS = 28672          # DUALIP_STATIC_MAX_DUALS of include/dualip.h: largest J*m dualip_grad_static accepts
+ETOOBIG = -7
 
 EXPORTED_SYMBOLS = ("dualip_opts_default", "dualip_create", "dualip_grad", "dualip_solve", "dualip_set_c",
                     "dualip_set_equality_rows", "dualip_set_global_count", "dualip_set_reduce_hook", "dualip_get_shard_extents",
                     "dualip_get_column_stats", "dualip_set_shard_constants", "dualip_eval_partial", "dualip_export_accumulators",
                     "dualip_import_accumulators", "dualip_set_profiling", "dualip_get_info", "dualip_get_csc", "dualip_destroy",
-                    "dualip_strerror")
+                    "dualip_strerror", "dualip_grad_static")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 
@@ -125,6 +127,8 @@ def load_library():
         lib.dualip_set_profiling.argtypes = [vp, ctypes.c_int]
         lib.dualip_get_csc.argtypes = [vp, vp, vp, vp]
         lib.dualip_get_csc.restype = ctypes.c_int
+        lib.dualip_grad_static.argtypes = [i64, i32, i32, vp, vp, vp, vp, vp, i32, d, d, vp, d, vp, vp, vp, vp]
+        lib.dualip_grad_static.restype = ctypes.c_int
         lib.dualip_destroy.argtypes = [vp]
         lib.dualip_destroy.restype = None
         lib.dualip_strerror.argtypes = [ctypes.c_int]
@@ -186,6 +190,26 @@ def _stream_ptr(stream):
             return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
         return None
     return ctypes.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+
+
+def grad_static(I, J, m, row_ptr, item_idx, c, a, b, lam, gamma: float, projection=PROJ_SIMPLEX_INEQ, p0=1.0, p1=0.0,
+                grad=None, scalars=None, x=None, stream=None):
+    """dualip_grad_static: one gradient evaluation with no handle and no allocation, for callers that are not allowed to
+    allocate device memory where they run (include/dualip.h says who and why).  Every argument is a CUDA tensor used in place:
+    row_ptr int64[I+1], item_idx int32[nnz], c fp32[nnz], a fp32[nnz*m], b fp32[J*m], lam fp64[J*m] in; grad fp64[J*m],
+    scalars fp64[6] = (g, obj, reg, r_inf, r_2, gap), x fp32[nnz] out, each optional.  J*m above STATIC_MAX_DUALS raises
+    DualipError with code ETOOBIG.  The outputs are ready once `stream` is; calls that overlap on the GPU race on the
+    library's one scratch array, so keep them on one stream."""
+    for name, t in (("row_ptr", row_ptr), ("item_idx", item_idx), ("c", c), ("a", a), ("b", b), ("lam", lam), ("grad", grad),
+                    ("scalars", scalars), ("x", x)):
+        if t is not None and not getattr(t, "is_cuda", False):
+            raise TypeError(f"{name} must be a CUDA tensor: dualip_grad_static cannot stage host memory without allocating")
+    if scalars is not None and scalars.numel() < 6:
+        raise ValueError("scalars needs 6 fp64 entries")
+    _check(load_library().dualip_grad_static(I, J, m, _ptr(row_ptr, np.int64), _ptr(item_idx, np.int32), _ptr(c, np.float32),
+                                             _ptr(a, np.float32), _ptr(b, np.float32), int(projection), float(p0), float(p1),
+                                             _ptr(lam, np.float64), float(gamma), _ptr(grad, np.float64),
+                                             _ptr(scalars, np.float64), _ptr(x, np.float32), _stream_ptr(stream)))
 
 
 class Problem:

@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdualip_b200.so")
-SOURCES = ["dualip_api.cu", "dualip_tma_wx0.cu", "dualip_tma_wx1.cu"]   # compiled in parallel, then linked
+SOURCES = ["dualip_api.cu", "dualip_tma_wx0.cu", "dualip_tma_wx1.cu", "dualip_static.cu"]   # compiled in parallel, then linked
 HEADERS = ["dualip_kernels.cuh", "dualip_grad_tma.cuh", "dualip_csc.cuh", "dualip_long.cuh", os.path.join("..", "..", "include", "dualip.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC,-O2,-Wall"]

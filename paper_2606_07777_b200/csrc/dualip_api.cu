@@ -721,6 +721,7 @@ const char* dualip_strerror(int code) {
         case DUALIP_ENOMEM: return "out of memory";
         case DUALIP_ECUDA: return "CUDA runtime error";
         case DUALIP_EUNSUPPORTED: return "unsupported configuration";
+        case DUALIP_ETOOBIG: return "J*m exceeds DUALIP_STATIC_MAX_DUALS, the fixed scratch size of dualip_grad_static";
         default: return "unknown error code";
     }
 }

@@ -43,7 +43,9 @@ enum {
     DUALIP_ENOMEM = -4,       /* host or device allocation failed */
     DUALIP_ECUDA = -5,        /* a CUDA runtime call failed (no device, launch failure, ...) */
     DUALIP_EUNSUPPORTED = -6, /* valid request this build cannot serve (e.g. reduction strategy needs more shared memory) */
-    DUALIP_ETOOBIG = -7       /* dualip_grad_static only: J*m exceeds DUALIP_STATIC_MAX_DUALS, the compiled-in size of its scratch */
+    DUALIP_ETOOBIG = -7,      /* dualip_grad_static only: J*m exceeds DUALIP_STATIC_MAX_DUALS, the compiled-in size of its scratch */
+    DUALIP_ESTALE = -8,       /* sharded handle whose c was replaced: agree on the constants again (dualip_set_shard_constants) first */
+    DUALIP_EHOOK = -9         /* the caller's reduce hook returned non-zero: the evaluation was abandoned, its partial sums discarded */
 };
 
 /* Per-user simple set C_i (R5, R10, R16).  Parameters p0,p1 of dualip_opts:
@@ -219,7 +221,7 @@ int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int3
                  const dualip_trace* trace, void* stream);
 
 /* Replace c (nnz fp32, host or device) in place without rebuilding -- config 5's perturbed re-solve.
- * Recomputes the objective's fixed-point scale.  With borrow = 1 the handle switches to the new pointer, which must be
+ * Recomputes the objective's fixed-point scale (not on a sharded handle: see dualip_set_shard_constants, DUALIP_ESTALE).  With borrow = 1 the handle switches to the new pointer, which must be
  * device memory and, when the streaming kernel is in use (dualip_info.streaming), 16-byte aligned like the arrays given
  * to dualip_create (its bulk copies need it): otherwise DUALIP_EINVAL and the handle keeps the old c. */
 int dualip_set_c(dualip_t* h, const float* c_new, void* stream);
@@ -251,10 +253,14 @@ int dualip_set_global_count(dualip_t* h, int32_t enable, double M, void* stream)
  * Accumulator layout (int64 words, dualip_info.duals' item part first): [J*m item sums a'x][c'x][|x|^2][sum x].           */
 
 /* Called between the gradient kernel and the epilogue of EVERY evaluation (dualip_grad, each iteration and the final evaluation
- * of dualip_solve) once set: must leave in accumulators_dev[0..n_words) the sum over all shards, enqueued on `stream`
- * (e.g. ncclAllReduce(int64, sum) in place).  lambda_eval_dev / gamma: the point being evaluated (identical on all ranks). */
-typedef void (*dualip_reduce_hook)(void* user, int64_t* accumulators_dev, int64_t n_words, const double* lambda_eval_dev,
-                                   double gamma, void* stream);
+ * of dualip_solve) once set: must leave in accumulators_dev[0..n_words) the sum over all shards, enqueued on `stream` -- the
+ * stream the gradient kernel was launched on and the epilogue will be; work put on any other stream races both
+ * (e.g. ncclAllReduce(int64, sum) in place on `stream`).  lambda_eval_dev / gamma: the point being evaluated (identical on all
+ * ranks).  Returns 0, or non-zero if the exchange could not be issued: the evaluation is then abandoned -- no epilogue, the
+ * partial sums are cleared, the entry point returns DUALIP_EHOOK -- instead of finalising this shard's sums alone while the
+ * other ranks wait. */
+typedef int (*dualip_reduce_hook)(void* user, int64_t* accumulators_dev, int64_t n_words, const double* lambda_eval_dev,
+                                  double gamma, void* stream);
 /* fn = NULL removes the hook.  While a hook is set, CUDA-graph replay is off (the hook runs on the host between launches). */
 int dualip_set_reduce_hook(dualip_t* h, dualip_reduce_hook fn, void* user);
 
@@ -266,7 +272,10 @@ int dualip_set_reduce_hook(dualip_t* h, dualip_reduce_hook fn, void* user);
  *      out[0..J*m) = sum_i (a^k_ij)^2, out[J*m..2J*m) = sum_i |a^k_ij|, out[2J*m] = sum |c|;  all-reduce (int64 SUM);
  *   3. dualip_set_shard_constants(h, &global, summed) on every shard: L, L_step, the Jacobi factors and the scales are derived
  *      from the summed integers exactly as dualip_create derives them on one GPU.
- * dualip_set_c recomputes sum |c| from the shard alone: repeat 2-3 afterwards. */
+ * dualip_set_c on a handle that has been given shard constants keeps them (a shard's own sum |c| and max |c| are not the
+ * problem's, and ranks with different fixed-point scales would all-reduce integers that do not add up) and marks the handle
+ * stale: dualip_grad, dualip_solve and dualip_eval_partial return DUALIP_ESTALE until steps 1-3 have been repeated on every
+ * shard (step 1 too: max |c| is part of the extents). */
 typedef struct {
     int64_t I, nnz;                 /* users, nonzeros */
     float   max_abs_a, max_abs_c;

@@ -6,4 +6,4 @@ or without a CUDA device raises.
 from .binding import (DualipError, Problem, Opts, Scalars, Info, lib_path, load_library,  # noqa: F401
                       PROJ_SIMPLEX_INEQ, PROJ_BOX, PROJ_BOXCUT, PROJ_SIMPLEX_EQ,
                       RED_AUTO, RED_SMEM, RED_GLOBAL, RED_CSC, PRECOND_NONE, PRECOND_JACOBI, STEP_FIXED, STEP_ADAPTIVE,
-                      EXPORTED_SYMBOLS, grad_static, STATIC_MAX_DUALS, ETOOBIG)
+                      EXPORTED_SYMBOLS, grad_static, STATIC_MAX_DUALS, ETOOBIG, ESTALE, EHOOK)

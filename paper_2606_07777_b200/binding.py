@@ -18,6 +18,8 @@ PRECOND_NONE, PRECOND_JACOBI = 0, 1
 STEP_FIXED, STEP_ADAPTIVE = 0, 1
 STATIC_MAX_DUALS = 28672          # DUALIP_STATIC_MAX_DUALS of include/dualip.h: largest J*m dualip_grad_static accepts
 ETOOBIG = -7
+ESTALE = -8
+EHOOK = -9
 
 EXPORTED_SYMBOLS = ("dualip_opts_default", "dualip_create", "dualip_grad", "dualip_solve", "dualip_set_c",
                     "dualip_set_equality_rows", "dualip_set_global_count", "dualip_set_reduce_hook", "dualip_get_shard_extents",
@@ -65,8 +67,8 @@ class ShardExtents(ctypes.Structure):
     _fields_ = [("I", ctypes.c_int64), ("nnz", ctypes.c_int64), ("max_abs_a", ctypes.c_float), ("max_abs_c", ctypes.c_float)]
 
 
-# void hook(void* user, int64_t* accumulators_dev, int64_t n_words, const double* lambda_eval_dev, double gamma, void* stream)
-REDUCE_HOOK = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_double, ctypes.c_void_p)
+# int hook(void* user, int64_t* accumulators_dev, int64_t n_words, const double* lambda_eval_dev, double gamma, void* stream)
+REDUCE_HOOK = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_double, ctypes.c_void_p)
 
 
 class _Trace(ctypes.Structure):
@@ -239,8 +241,8 @@ class Problem:
         sp = ctypes.byref(scalars) if isinstance(scalars, Scalars) else _ptr(scalars, np.float64)
         if isinstance(scalars, Scalars):
             sp = ctypes.cast(sp, ctypes.c_void_p)
-        _check(load_library().dualip_grad(self._h, _ptr(lam, np.float64), float(gamma), _ptr(grad, np.float64), sp,
-                                          _ptr(x, np.float32), _stream_ptr(stream)))
+        self._checked(load_library().dualip_grad(self._h, _ptr(lam, np.float64), float(gamma), _ptr(grad, np.float64), sp,
+                                                 _ptr(x, np.float32), _stream_ptr(stream)))
         return scalars
 
     def solve(self, gammas, iters, lam, x=None, scalars=None, grad=None, trace=None, stream=None):
@@ -266,9 +268,9 @@ class Problem:
         sp = ctypes.byref(scalars) if isinstance(scalars, Scalars) else _ptr(scalars, np.float64)
         if isinstance(scalars, Scalars):
             sp = ctypes.cast(sp, ctypes.c_void_p)
-        _check(load_library().dualip_solve(self._h, _ptr(gam), gam.size, _ptr(its), _ptr(lam, np.float64),
-                                           _ptr(x, np.float32), sp, _ptr(grad, np.float64),
-                                           ctypes.byref(tr) if tr is not None else None, _stream_ptr(stream)))
+        self._checked(load_library().dualip_solve(self._h, _ptr(gam), gam.size, _ptr(its), _ptr(lam, np.float64),
+                                                  _ptr(x, np.float32), sp, _ptr(grad, np.float64),
+                                                  ctypes.byref(tr) if tr is not None else None, _stream_ptr(stream)))
         return scalars
 
     def set_c(self, c_new, stream=None):
@@ -292,9 +294,27 @@ class Problem:
         return self.J * self.m + 3
 
     def set_reduce_hook(self, fn):
-        """fn(acc_ptr:int, n_words:int, lam_ptr:int, gamma:float, stream:int) or None.  The ctypes thunk is kept alive here."""
-        self._hook = REDUCE_HOOK(lambda user, acc, n, lam, gamma, st: fn(acc, n, lam, gamma, st)) if fn else REDUCE_HOOK()
+        """fn(acc_ptr:int, n_words:int, lam_ptr:int, gamma:float, stream:int) or None; stream is the raw cudaStream_t (0 = the
+        default stream) everything fn enqueues must go to.  fn returns None / 0, or non-zero to abandon the evaluation.  An
+        exception raised in fn cannot cross the C frames: it is caught here, the library is told the hook failed, and the
+        grad / solve call that triggered it raises DualipError(EHOOK) from it.  The ctypes thunk is kept alive here."""
+        def thunk(user, acc, n, lam, gamma, st):
+            try:
+                r = fn(acc, n, lam, gamma, st or 0)
+                return 0 if r is None else int(r)
+            except BaseException as exc:          # noqa: BLE001 -- must not propagate into the C caller
+                self._hook_error = exc
+                return 1
+        self._hook_error = None
+        self._hook = REDUCE_HOOK(thunk) if fn else REDUCE_HOOK()
         _check(load_library().dualip_set_reduce_hook(self._h, self._hook, None))
+
+    def _checked(self, rc: int):
+        """_check, chaining the exception a reduce hook raised during the call (if any)."""
+        err, self._hook_error = getattr(self, "_hook_error", None), None
+        if rc != 0 and err is not None:
+            raise DualipError(rc, load_library().dualip_strerror(rc).decode()) from err
+        _check(rc)
 
     def shard_extents(self) -> ShardExtents:
         e = ShardExtents()

@@ -62,6 +62,8 @@ struct dualip {
     // user-sharded multi-GPU: the caller's all-reduce between the gradient kernel and the epilogue
     dualip_reduce_hook hook = nullptr; void* hook_user = nullptr;
     long long nnz_total = 0;                               // nonzeros over all shards (= nnz unless dualip_set_shard_constants said otherwise)
+    bool sharded = false;                                  // dualip_set_shard_constants has been called: the constants are GLOBAL ones
+    bool shard_stale = false;                              // ... and dualip_set_c has changed c since: they must be agreed on again
     double* scalars_dev = nullptr;
     float* x_stage = nullptr;
     dualip_dev::TileEntry* tiles = nullptr;
@@ -526,7 +528,12 @@ int launch_iter(dualip* h, IterLaunch& L, cudaStream_t st) {
         CK(cudaGetLastError());
     }
     if (h->csc || h->hook) {
-        if (h->hook) h->hook(h->hook_user, reinterpret_cast<int64_t*>(h->s_fix), (int64_t)h->J * h->m + 3, L.f_after.lam_eval, L.f_after.gamma, st);
+        if (h->hook && h->hook(h->hook_user, reinterpret_cast<int64_t*>(h->s_fix), (int64_t)h->J * h->m + 3, L.f_after.lam_eval, L.f_after.gamma, st) != 0) {
+            // the exchange failed: finalising local sums would silently diverge from the other ranks.  Drop them (the epilogue,
+            // which normally re-zeroes the accumulators, does not run) and report.
+            CK(cudaMemsetAsync(h->s_fix, 0, ((size_t)h->J * h->m + 3) * 8, st));
+            return DUALIP_EHOOK;
+        }
         k_finalize_only<<<1, kBlockThreads, 0, st>>>(L.f_after);
         h->launches++;
         CK(cudaGetLastError());
@@ -722,6 +729,8 @@ const char* dualip_strerror(int code) {
         case DUALIP_ECUDA: return "CUDA runtime error";
         case DUALIP_EUNSUPPORTED: return "unsupported configuration";
         case DUALIP_ETOOBIG: return "J*m exceeds DUALIP_STATIC_MAX_DUALS, the fixed scratch size of dualip_grad_static";
+        case DUALIP_ESTALE: return "sharded handle: c changed, call dualip_set_shard_constants again before evaluating";
+        case DUALIP_EHOOK: return "the reduce hook failed; evaluation abandoned";
         default: return "unknown error code";
     }
 }
@@ -976,12 +985,14 @@ int dualip_set_shard_constants(dualip_t* h, const dualip_shard_extents* g, const
     cudaFree(d_fix);
     if (rc != 0) { cudaGetLastError(); return rc; }
     set_scales(h);
+    h->sharded = true; h->shard_stale = false;
     return DUALIP_OK;
 }
 
 int dualip_eval_partial(dualip_t* h, const double* lambda_dev, double gamma, float* x, void* stream) {
     if (!h || !lambda_dev || !(gamma > 0.0) || !std::isfinite(gamma)) return DUALIP_EINVAL;
     if (!is_device_ptr(lambda_dev) || (x && !is_device_ptr(x)) || h->csc) return DUALIP_EINVAL;
+    if (h->shard_stale) return DUALIP_ESTALE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     FinalizeParams f{};
     f.lam_eval = lambda_dev; f.gamma = gamma; f.update = 0;
@@ -1064,6 +1075,10 @@ int dualip_set_c(dualip_t* h, const float* c_new, void* stream) {
         if (h->plan.tma && ((uintptr_t)c_new & 15)) return DUALIP_EINVAL;   // the streaming kernel's bulk copies need 16-byte alignment
         h->c = c_new;
     }
+    // A shard's sum |c| and max |c| are not the problem's: recomputing them here would give every rank its own fixed-point
+    // scale for c'x, and the all-reduce would then add integers of different scales.  Keep the agreed constants and refuse to
+    // evaluate until the shards have agreed again (dualip_get_shard_extents .. dualip_set_shard_constants).
+    if (h->sharded) { h->shard_stale = true; return DUALIP_OK; }
     int rc = compute_stats(h, st, false, true);
     if (rc != 0) return rc;
     set_scales(h);
@@ -1100,6 +1115,7 @@ int dualip_set_global_count(dualip_t* h, int32_t enable, double M, void* stream)
 int dualip_grad(dualip_t* h, const double* lambda, double gamma, double* grad, dualip_scalars* scalars, float* x,
                 void* stream) {
     if (!h || !lambda || !(gamma > 0.0) || !std::isfinite(gamma)) return DUALIP_EINVAL;
+    if (h->shard_stale) return DUALIP_ESTALE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const size_t JM = n_duals(h);
     const bool lam_dev = is_device_ptr(lambda), grad_dev = is_device_ptr(grad), sc_dev = is_device_ptr(scalars),
@@ -1135,6 +1151,7 @@ int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int3
     }
     if (trace && trace->capacity < total) return DUALIP_EINVAL;
     if (n_stages == 0) return DUALIP_OK;
+    if (h->shard_stale) return DUALIP_ESTALE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const size_t JM = n_duals(h);
     const bool lam_dev = is_device_ptr(lambda_inout), grad_dev = is_device_ptr(final_grad),

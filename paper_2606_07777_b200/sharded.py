@@ -72,13 +72,36 @@ class ShardedProblem:
 
     def _hook(self, acc_ptr, n_words, lam_ptr, gamma, stream):
         """Between the gradient kernel and the epilogue: accumulators <- sum over ranks (in place, through a staging tensor
-        torch.distributed can see)."""
+        torch.distributed can see).  Everything is enqueued on `stream`, the raw cudaStream_t the library launched the gradient
+        kernel on and will launch the epilogue on: the two copies take it as an argument, and the all-reduce runs with it as
+        torch's current stream (which is the stream torch.distributed orders a collective against).  An exception raised here
+        makes the evaluation fail with DualipError(EHOOK) on this rank (Problem.set_reduce_hook) instead of finalising local sums."""
         if self.dist is None:
-            return
-        self.local.export_accumulators(self._acc, clear=False)
-        self.dist.all_reduce(self._acc, op=self.dist.ReduceOp.SUM)
-        self.local.import_accumulators(self._acc, accumulate=False)
+            return 0
+        if self.device.type == "cuda":
+            ext = self.torch.cuda.ExternalStream(stream, device=self.device) if stream else self.torch.cuda.default_stream(self.device)
+            with self.torch.cuda.stream(ext):
+                self.local.export_accumulators(self._acc, clear=False, stream=ext)
+                self.dist.all_reduce(self._acc, op=self.dist.ReduceOp.SUM)
+                self.local.import_accumulators(self._acc, accumulate=False, stream=ext)
+        else:                                         # CPU stand-in of the gloo test: no streams
+            self.local.export_accumulators(self._acc, clear=False)
+            self.dist.all_reduce(self._acc, op=self.dist.ReduceOp.SUM)
+            self.local.import_accumulators(self._acc, accumulate=False)
         self.allreduce_calls += 1
+        return 0
+
+    def set_c(self, c_new, stream=None):
+        """Replace this rank's slice of c (config 5's perturbed re-solve), then agree on the constants again: sum |c| and max |c|
+        are global quantities, and the library refuses to evaluate a sharded handle (DUALIP_ESTALE) until that is done.
+        Collective: every rank must call it."""
+        self.local.set_c(c_new, stream=stream)
+        # the agreement below reads c on the library's default stream
+        if stream is not None:
+            stream.synchronize()
+        elif self.device.type == "cuda":
+            self.torch.cuda.current_stream(self.device).synchronize()
+        self._agree_on_constants()
 
     def grad(self, *a, **kw):
         return self.local.grad(*a, **kw)

@@ -103,3 +103,114 @@ def test_two_shards_on_one_gpu_are_bit_identical_to_the_unsharded_problem(name, 
     A.set_reduce_hook(None)
     for P in (whole, A, B):
         P.destroy()
+
+
+def test_set_c_on_shards_keeps_one_scale_and_demands_a_new_agreement():
+    """dualip_set_c on a sharded handle (config 5's perturbed re-solve): a shard must not derive the objective's
+    fixed-point scale from its OWN sum |c| -- ranks would then all-reduce integers of different scales.  The handle keeps the
+    agreed constants, refuses to evaluate (DUALIP_ESTALE) until the shards have agreed again, and after that is bit-identical to
+    the unsharded handle given the same new c.  The two shards' c are made very unequal in size so that per-shard scales WOULD
+    differ."""
+    inst = synth.generate(synth.get_config("cfg5-tight", I=40_000), device="cuda")
+    Jm = inst.J * inst.m
+    whole = _shard(inst, 0, inst.I)
+    cuts = split_users(inst.row_ptr, 2)
+    nz = [int(inst.row_ptr[c]) for c in cuts]
+    G = whole.info().group_lanes
+    A, B = _shard(inst, cuts[0], cuts[1], group_lanes=G), _shard(inst, cuts[1], cuts[2], group_lanes=G)
+    tmp = torch.empty(A.acc_words, dtype=torch.int64, device="cuda")
+
+    def agree():
+        ea, eb = A.shard_extents(), B.shard_extents()
+        g = ShardExtents(ea.I + eb.I, ea.nnz + eb.nnz, max(ea.max_abs_a, eb.max_abs_a), max(ea.max_abs_c, eb.max_abs_c))
+        sa = A.column_stats(g, torch.empty(2 * Jm + 1, dtype=torch.int64, device="cuda"))
+        sb = B.column_stats(g, torch.empty(2 * Jm + 1, dtype=torch.int64, device="cuda"))
+        for P in (A, B):
+            P.set_shard_constants(g, sa + sb)
+
+    def hook(acc_ptr, n_words, lam_ptr, gamma, stream):
+        B.eval_partial(lam_ptr, gamma)
+        B.export_accumulators(tmp, clear=True)
+        A.import_accumulators(tmp, accumulate=True)
+
+    def same_as_whole(tag):
+        lam, gamma = synth.probe_lambda(inst, 0, 0.5), inst.cfg.gammas[-1]
+        gw, ga = torch.empty(Jm, dtype=torch.float64, device="cuda"), torch.empty(Jm, dtype=torch.float64, device="cuda")
+        sw, ss = pkg.Scalars(), pkg.Scalars()
+        whole.grad(lam, gamma, grad=gw, scalars=sw)
+        A.grad(lam, gamma, grad=ga, scalars=ss)
+        torch.cuda.synchronize()
+        assert torch.equal(gw, ga), tag
+        assert sw.as_dict() == ss.as_dict(), (tag, sw.as_dict(), ss.as_dict())
+        return sw
+
+    agree()
+    A.set_reduce_hook(hook)
+    s0 = same_as_whole("before set_c")
+    c2 = synth.perturb_c(inst, 0.01)
+    c2[nz[1]:] *= 37.0                                                               # shard 1's |c| dwarfs shard 0's
+    whole.set_c(c2)
+    A.set_c(c2[:nz[1]].contiguous()); B.set_c(c2[nz[1]:].contiguous())
+    lam = torch.zeros(Jm, dtype=torch.float64, device="cuda")
+    for call in (lambda: A.grad(lam, 0.1, grad=torch.empty(Jm, dtype=torch.float64, device="cuda")),
+                 lambda: A.solve([0.1], [2], lam.clone()),
+                 lambda: B.eval_partial(lam, 0.1)):
+        with pytest.raises(pkg.DualipError) as e:
+            call()
+        assert e.value.code == pkg.ESTALE
+    agree()
+    s1 = same_as_whole("after set_c + new agreement")
+    assert s1.obj != s0.obj
+    assert A.info().L == whole.info().L
+    A.set_reduce_hook(None)
+    for P in (whole, A, B):
+        P.destroy()
+
+
+def test_a_failing_hook_abandons_the_evaluation_and_leaves_nothing_behind():
+    """The reduce hook returns non-zero, or raises (a failed all-reduce): the evaluation must not be finalised from this shard's
+    sums alone -- dualip_grad / dualip_solve return DUALIP_EHOOK, the Python exception is chained to the DualipError, the outputs
+    stay untouched, and the partial sums are dropped so that the next evaluation, with a working hook, is exact again.  The
+    hook's `stream` argument is the stream of the call (here a side stream), and work it enqueues there is ordered with the kernels."""
+    inst = synth.generate(synth.get_config("cfg2-tight", I=30_000), device="cuda")
+    Jm = inst.J * inst.m
+    whole = _shard(inst, 0, inst.I)
+    lam, gamma = synth.probe_lambda(inst, 0, 0.5), inst.cfg.gammas[-1]
+    want = torch.empty(Jm, dtype=torch.float64, device="cuda")
+    whole.grad(lam, gamma, grad=want)
+    A = _shard(inst, 0, inst.I, group_lanes=whole.info().group_lanes)
+    seen = []
+
+    def bad_return(acc_ptr, n_words, lam_ptr, gamma, stream):
+        seen.append(stream)
+        return 3
+
+    def raises(acc_ptr, n_words, lam_ptr, gamma, stream):
+        raise RuntimeError("all-reduce timed out")
+
+    def fine(acc_ptr, n_words, lam_ptr, gamma, stream):
+        seen.append(stream)
+
+    side = torch.cuda.Stream()
+    got = torch.full((Jm,), float("nan"), dtype=torch.float64, device="cuda")
+    torch.cuda.synchronize()                                                        # inputs were made on the default stream
+    A.set_reduce_hook(bad_return)
+    with pytest.raises(pkg.DualipError) as e:
+        A.grad(lam, gamma, grad=got, stream=side)
+    assert e.value.code == pkg.EHOOK and e.value.__cause__ is None and seen == [side.cuda_stream]
+    A.set_reduce_hook(raises)
+    with pytest.raises(pkg.DualipError) as e:
+        A.grad(lam, gamma, grad=got)
+    assert e.value.code == pkg.EHOOK and isinstance(e.value.__cause__, RuntimeError)
+    with pytest.raises(pkg.DualipError) as e:
+        A.solve([gamma], [3], lam.clone())
+    assert e.value.code == pkg.EHOOK and isinstance(e.value.__cause__, RuntimeError)
+    torch.cuda.synchronize()
+    assert torch.isnan(got).all()                                                   # no epilogue ran
+    A.set_reduce_hook(fine)
+    A.grad(lam, gamma, grad=got, stream=side)
+    side.synchronize()
+    assert torch.equal(got, want), "partial sums of the abandoned evaluations leaked into this one"
+    A.set_reduce_hook(None)
+    for P in (whole, A):
+        P.destroy()

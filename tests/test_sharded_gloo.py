@@ -36,6 +36,9 @@ WORKER = textwrap.dedent("""
             return out
         def set_shard_constants(self, g, summed):
             self.constants = summed.clone()
+            self.agreed = getattr(self, "agreed", 0) + 1
+        def set_c(self, c_new, stream=None):
+            self.c = c_new
         def set_reduce_hook(self, fn):
             self.hook = fn
         def export_accumulators(self, out, clear=True):
@@ -48,7 +51,10 @@ WORKER = textwrap.dedent("""
     loc = FakeLocal()
     sp = ShardedProblem(loc, dist=dist, device=torch.device("cpu"))
     loc.hook(0, loc.acc_words, 0, 1e-3, 0)            # what the library does between the gradient kernel and the epilogue
-    print(json.dumps({{"rank": rank, "constants": loc.constants.tolist(), "acc": loc.acc.tolist(), "calls": sp.allreduce_calls}}), flush=True)
+    acc = loc.acc.tolist()
+    sp.set_c("c2")                                    # a new c: the constants must be agreed on again, on every rank
+    print(json.dumps({{"rank": rank, "constants": loc.constants.tolist(), "acc": acc, "calls": sp.allreduce_calls,
+                      "agreed": loc.agreed, "c": loc.c}}), flush=True)
     dist.destroy_process_group()
 """)
 
@@ -78,6 +84,7 @@ def test_two_shards_exchange_integers_and_end_identical(tmp_path):
     want_acc = (np.arange(9) * 1 + 0 + np.arange(9) * 10 + 1).tolist()
     for o in outs:
         assert o["constants"] == want_const and o["acc"] == want_acc and o["calls"] == 1
+        assert o["agreed"] == 2 and o["c"] == "c2"        # ShardedProblem.set_c: local set_c, then the a0 exchange once more
 
 
 def test_split_users_balances_nonzeros():

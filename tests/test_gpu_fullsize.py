@@ -6,8 +6,9 @@ the device, borrowed by the library, default plan).  What is compared:
   * grad g, g and ALL of x against the oracle's full evaluation for configs 2, 3 and 5 at lambda = 0 (what the verbatim run
     evaluates at every iteration) and at the probe lambda; for config 4 (5e9 nonzeros) against the oracle on the first
     3,000,000 users, as a problem of its own with the same kernel instantiation (test_cfg4_first_3M_users_...);
-  * full-size TRAJECTORIES: config 2, 3 and 5 tight companions (Jacobi step for the Zipf configs), every iteration's
-    gradient, lambda and the final x against the oracle's solve;
+  * full-size TRAJECTORIES against the oracle's solve, every iteration's gradient and lambda and the final x: config 2's tight
+    companion for 25 AGD iterations with the scalar step (test_full_size_cfg2_tight_trajectory), the tight companions of the
+    Zipf configs 3 and 5 for 3 iterations with the Jacobi step (test_full_size_tight_trajectories_cfg3_cfg5);
   * at every size, properties that tie the remaining outputs to the sampled ones: grad g = A x - b and
     g = c'x + gamma/2 |x|^2 + lambda'grad g re-accumulated in fp64 from the x the kernel wrote (plain torch
     index_add, an independent reduction), feasibility of every row, and bit-identical results on a second launch.
@@ -228,6 +229,26 @@ def test_cfg4_first_3M_users_gradient_and_x_against_the_oracle():
         del rf
     pool.shutdown()
     pg.destroy(); full.destroy()
+
+
+def test_full_size_cfg2_tight_trajectory():
+    """Config 2 at full size (1e6 users, 2e7 nonzeros) with binding constraints: 25 AGD iterations of the default plan on
+    borrowed device rows -- every iteration's grad g and lambda, the final grad g, scalars and all of x -- against the oracle's
+    solve, which runs on a host thread (26 evaluations, under a minute) while the GPU side proceeds."""
+    from gpu_util import assert_trajectory_parity
+    from test_gpu_parity import FULL_SIZE_G
+    cfg = synth.get_config("cfg2-tight")
+    inst = synth.generate(cfg, device="cuda")
+    d = inst.numpy()
+    po = _oracle_problem(cfg, inst.I, d["row_ptr"], d["item_idx"], d["c"], d["a"], d["b"])
+    pool = _pool()
+    fut = pool.submit(oracle.solve, po, list(cfg.gammas), [25] * len(cfg.gammas), trace_grad=True, trace_lambda=True)
+    pg = _create(inst)
+    assert pg.info().streaming == 1 and pg.info().group_lanes == FULL_SIZE_G["cfg2"]
+    worst, ex, ref, out = assert_trajectory_parity(po, pg, list(cfg.gammas), [25] * len(cfg.gammas), tag="cfg2-tight full", ref=fut)
+    assert (ref.lam > 0).sum() > 50
+    pg.destroy()
+    pool.shutdown()
 
 
 def test_full_size_tight_trajectories_cfg3_cfg5():

@@ -1,10 +1,8 @@
-"""The cases `compute-sanitizer` is run on (memcheck and racecheck on configs 1-2); they are ordinary
-`-m gpu` parity tests as well.  Small on purpose: under the sanitizer a kernel runs 10-100 x slower.
-
-    compute-sanitizer --tool memcheck  python -m pytest tests/test_gpu_sanitizer_cases.py -m gpu -q
-    compute-sanitizer --tool racecheck python -m pytest tests/test_gpu_sanitizer_cases.py -m gpu -q
-
-(the logs of both are kept under profiles/).  What they drive: dualip_create (validation, statistics, tile table), dualip_grad
+"""The small cases chosen for memory- and race-checking (configs 1-2); they are ordinary `-m gpu` parity tests
+as well.  `compute-sanitizer` is closed on the GPU pool this was developed on (profiles/r02_sanitizer.md), so no sanitizer log
+exists and none is claimed: the memcheck half is done by the library's -DDUALIP_CHECKED build, whose in-kernel bounds
+assertions tests/test_gpu_checked_build.py runs these cases against; the racecheck half has no stand-in beyond bit-reproducible
+results run to run and across pipeline geometries (tests/test_gpu_parity.py).  What they drive: dualip_create (validation, statistics, tile table), dualip_grad
 with x, and a 20-iteration dualip_solve (AGD epilogue, trace buffers) on config 1, its tight companion and config 2 at 60,000
 users, through both gradient kernels (TMA-staged k_grad_tma, direct-load k_grad) and both atomic reduction strategies
 (per-CTA shared-memory accumulators, RED.ADD.64 to L2) -- the places the round-1 review named: the stage-0 buffer reused as

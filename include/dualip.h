@@ -236,7 +236,7 @@ int dualip_set_equality_rows(dualip_t* h, const uint8_t* is_equality, void* stre
 /* Global-count constraint  sum_{(i,j) in E} x_ij <= M  ("adding a global-count constraint ... only augments A and
  * lambda"; R21): one more coupling row, number J*m, with coefficient 1 on every eligible pair and its own dual mu >= 0, which
  * every nonzero gathers: w_ij = -(c_ij + sum_k a^k_ij lambda_jk + mu).  enable != 0 switches the row on with right-hand side M
- * (finite, >= 0); enable = 0 switches it off.  While it is on, EVERY dual-sized vector at this interface -- lambda, grad,
+ * (finite, >= 0; kept in fp64, so a budget of tens of millions of pairs is exact); enable = 0 switches it off.  While it is on, EVERY dual-sized vector at this interface -- lambda, grad,
  * lambda_inout, final_grad, the trace rows, is_equality -- has J*m + 1 entries, the last one belonging to this row
  * (dualip_info.duals).  The step constant becomes L_step + nnz (|A|_2^2 <= |A_items|_2^2 + |1|_2^2), or L' + 1 under JACOBI,
  * where the row is normalised like any other (d^2 = 1/nnz).  Switching the row on or off clears the equality mask. */

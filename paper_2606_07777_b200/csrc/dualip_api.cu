@@ -58,7 +58,8 @@ struct dualip {
     unsigned long long* sc_fix = nullptr;
     double* lam_cur = nullptr; double* y = nullptr; double* lam_stage = nullptr; double* grad_stage = nullptr;
     double* y_prev = nullptr; double* g_prev = nullptr;   // DUALIP_STEP_ADAPTIVE: previous evaluation point / gradient (R20)
-    bool count_on = false;                                 // global-count row (R21): duals = J*m + 1, b[J*m] = M
+    bool count_on = false;                                 // global-count row (R21): duals = J*m + 1
+    double count_M = 0.0;                                  // ... and its right-hand side, in fp64 (budgets above 2^24 are not fp32 numbers)
     // user-sharded multi-GPU: the caller's all-reduce between the gradient kernel and the epilogue
     dualip_reduce_hook hook = nullptr; void* hook_user = nullptr;
     long long nnz_total = 0;                               // nonzeros over all shards (= nnz unless dualip_set_shard_constants said otherwise)
@@ -456,7 +457,7 @@ void prof_collect(dualip* h) {
 
 // Common fields of the per-launch epilogue (a4-a6).  The caller sets lam_eval/gamma/update/... before launch_iter.
 void fill_finalize_common(const dualip* h, FinalizeParams& f) {
-    f.s_fix = h->s_fix; f.sc_fix = h->sc_fix; f.b = h->b; f.JM = h->J * h->m; f.R = (int)n_duals(h);
+    f.s_fix = h->s_fix; f.sc_fix = h->sc_fix; f.b = h->b; f.count_rhs = h->count_M; f.JM = h->J * h->m; f.R = (int)n_duals(h);
     f.inv_scale_s = 1.0 / h->scale_s; f.inv_scale_obj = 1.0 / h->scale_obj; f.inv_scale_sq = 1.0 / h->scale_sq;
     f.inv_scale_cnt = 1.0 / h->scale_cnt;
     f.row_eq = h->row_eq;
@@ -1106,9 +1107,7 @@ int dualip_set_global_count(dualip_t* h, int32_t enable, double M, void* stream)
     CK(cudaStreamSynchronize(st));                           // earlier launches still read the old layout
     if (h->row_eq) { cudaFree(h->row_eq); h->row_eq = nullptr; h->bytes_resident -= (long long)((size_t)h->J * h->m + 1); }
     h->count_on = enable != 0;
-    const float Mf = enable ? (float)M : 0.0f;
-    CK(cudaMemcpyAsync(h->b + (size_t)h->J * h->m, &Mf, 4, cudaMemcpyHostToDevice, st));
-    CK(cudaStreamSynchronize(st));
+    h->count_M = enable ? M : 0.0;                           // read by the epilogue as row J*m's right-hand side (FinalizeParams.count_rhs)
     return DUALIP_OK;
 }
 

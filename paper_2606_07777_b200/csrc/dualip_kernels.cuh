@@ -137,7 +137,8 @@ struct IterState { int t; int pad; long long n; };
 struct FinalizeParams {
     unsigned long long* s_fix;
     unsigned long long* sc_fix;
-    const float* __restrict__ b;  // [R]: b[JM] = M of the global-count row when it is on
+    const float* __restrict__ b;  // [JM] right-hand sides of the item rows (fp32 input data)
+    double count_rhs;           // M of the global-count row (row JM) when it is on: fp64, a count above 2^24 is not an fp32 number
     const double* lam_eval;     // point the gradient was taken at
     double* grad_out;           // nullable
     double* scalars_out;        // nullable, 6 doubles {g, obj, reg, r_inf, r_2, gap}
@@ -162,6 +163,9 @@ struct FinalizeParams {
 
 constexpr int kFinalizeScratchBytes = 3 * 32 * 8 + 16;   // shared memory finalize_block needs: 3 x 32 doubles + flag
 
+// b_q: the item rows' right-hand sides are the caller's fp32 data; the global-count row's (q = JM) is the fp64 M
+__device__ __forceinline__ double row_rhs(const FinalizeParams& p, int q) { return q < p.JM ? (double)__ldg(p.b + q) : p.count_rhs; }
+
 // s_q = (A x)_q from the fixed-point accumulators: item rows from s_fix, the global-count row (q = JM) from the sum-x scalar
 __device__ __forceinline__ double row_sum(const FinalizeParams& p, int q) {
     return q < p.JM ? (double)(long long)__ldcg(p.s_fix + q) * p.inv_scale_s : (double)(long long)__ldcg(p.sc_fix + 2) * p.inv_scale_cnt;
@@ -184,7 +188,7 @@ __device__ __forceinline__ void finalize_block(const FinalizeParams& p, double* 
         if (t >= 1) {
             double dy2 = 0.0, dg2 = 0.0;
             for (int q = tid; q < p.R; q += nthreads) {
-                const double g = row_sum(p, q) - (double)__ldg(p.b + q);
+                const double g = row_sum(p, q) - row_rhs(p, q);
                 const double d2 = p.step_scale ? __ldg(p.step_scale + q) : 1.0;
                 const double dy = __ldcg(p.lam_eval + q) - __ldcg(p.y_prev + q), dg = g - __ldcg(p.g_prev + q);
                 dy2 = fma(dy / d2, dy, dy2);
@@ -206,13 +210,13 @@ __device__ __forceinline__ void finalize_block(const FinalizeParams& p, double* 
     // L2 round trips, and this CTA runs alone at the end of the launch
     constexpr int U = 4;
     for (int q0 = tid; q0 < p.R; q0 += U * nthreads) {
-        double sv[U]; float bb[U]; double le[U], lo[U], et[U]; bool eq[U];
+        double sv[U], bb[U], le[U], lo[U], et[U]; bool eq[U];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             const int q = q0 + u * nthreads;
-            sv[u] = 0.0; bb[u] = 0.0f; le[u] = 0.0; lo[u] = 0.0; et[u] = eta_t; eq[u] = false;
+            sv[u] = 0.0; bb[u] = 0.0; le[u] = 0.0; lo[u] = 0.0; et[u] = eta_t; eq[u] = false;
             if (q < p.R) {
-                sv[u] = row_sum(p, q); bb[u] = __ldg(p.b + q); le[u] = __ldcg(p.lam_eval + q);
+                sv[u] = row_sum(p, q); bb[u] = row_rhs(p, q); le[u] = __ldcg(p.lam_eval + q);
                 if (p.row_eq) eq[u] = __ldg(p.row_eq + q) != 0;
                 if (p.update) {
                     lo[u] = __ldcg(p.lam_cur + q);
@@ -225,7 +229,7 @@ __device__ __forceinline__ void finalize_block(const FinalizeParams& p, double* 
             const int q = q0 + u * nthreads;
             if (q >= p.R) break;
             if (q < p.JM) p.s_fix[q] = 0ull;
-            const double g = sv[u] - (double)bb[u];
+            const double g = sv[u] - bb[u];
             dot = fma(le[u], g, dot);
             const double viol = eq[u] ? fabs(g) : fmax(g, 0.0);
             r2 = fma(viol, viol, r2); rinf = fmax(rinf, viol);

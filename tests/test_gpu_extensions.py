@@ -89,6 +89,15 @@ def test_count_row_gradient(kind, p0, p1, kernel):
     ex, eg = assert_grad_parity(po, pg, lam, 0.05, tag=f"count/{kind}/neg")
     sc, grad, x = gpu_grad(pg, lam, 0.05)
     assert abs(grad[-1] - (x.astype(np.float64).sum() - M)) <= 1e-5 * M
+    # a budget that is not an fp32 number (2^24 + 1; config 3-5 sized budgets are tens of millions): the row's right-hand side
+    # is fp64 on both sides, so its gradient entry sum x - M matches to the accuracy of sum x, not to an ulp of fp32(M) = 2
+    Mbig = float(2 ** 24 + 1)
+    pg.set_global_count(Mbig)
+    pob = oracle.Problem(po.I, po.J, po.m, po.row_ptr, po.item_idx, po.c, po.a, po.b, po.proj_kind, po.p0, po.p1, Mbig)
+    ref = oracle.grad(pob, lam, 0.05)
+    sc, grad, x = gpu_grad(pg, lam, 0.05)
+    assert abs(grad[-1] - ref.grad[-1]) <= 1e-3 and abs(ref.grad[-1] - (ref.x.sum() - Mbig)) <= 1e-6
+    assert_grad_parity(pob, pg, lam, 0.05, tag=f"count/{kind}/M=2^24+1")
     # switching the row off restores the plain problem
     pg.set_global_count(None)
     po0 = oracle.Problem(po.I, po.J, po.m, po.row_ptr, po.item_idx, po.c, po.a, po.b, po.proj_kind, po.p0, po.p1)

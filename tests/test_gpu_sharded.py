@@ -1,7 +1,9 @@
 """`-m gpu` test of the user-sharded path on ONE GPU: the instance is cut into two contiguous user
 ranges, each behind its own handle; the "all-reduce" is the integer sum of the two handles' fixed-point accumulators, done in
 the reduce hook of shard 0.  With the create-time constants agreed through integer sums as well, the sharded evaluation must be
-BIT-identical to the unsharded one: grad g, every scalar, x, and the whole AGD trajectory.  (Two ranks on two GPUs run the same
+BIT-identical to the unsharded one: grad g, every scalar, x, and the whole AGD trajectory.  The hooked shard-0 handle is also
+compared with the ORACLE directly (grad g, scalars, both shards' x, and every iteration of the trajectory), so the row stands on
+the oracle and not only on the unsharded handle's own parity tests.  (Two ranks on two GPUs run the same
 calls with torch.distributed's all_reduce in the hook: paper_2606_07777_b200/sharded.py; unmeasured on multi-GPU hardware.)"""
 import numpy as np
 import pytest
@@ -15,7 +17,8 @@ if torch.cuda.is_available():
     import paper_2606_07777_b200 as pkg
     from paper_2606_07777_b200.binding import ShardExtents
     from paper_2606_07777_b200.sharded import split_users
-    from gpu_util import gpu_solve
+    import oracle
+    from gpu_util import _KIND, TOL_G, TOL_GRAD, TOL_X, gpu_solve, rel_l2
 
 
 def _shard(inst, u0, u1, **opt):
@@ -62,6 +65,9 @@ def test_two_shards_on_one_gpu_are_bit_identical_to_the_unsharded_problem(name, 
         calls.append(gamma)
 
     A.set_reduce_hook(hook)
+    d = inst.numpy()
+    kind, q0, q1 = synth.proj_spec(inst.cfg)
+    po = oracle.Problem(inst.I, inst.J, inst.m, d["row_ptr"], d["item_idx"], d["c"], d["a"], d["b"], _KIND[kind][0], q0, q1)
     for lam, gamma in ((torch.zeros(Jm, dtype=torch.float64, device="cuda"), inst.cfg.gammas[-1]),
                        (synth.probe_lambda(inst, 0, 0.05 if "3" in name else 0.5), inst.cfg.gammas[-1]),
                        (synth.probe_lambda(inst, 1, 0.05 if "3" in name else 0.5), 0.1)):
@@ -76,6 +82,12 @@ def test_two_shards_on_one_gpu_are_bit_identical_to_the_unsharded_problem(name, 
         assert torch.equal(gw, ga), "sharded grad g differs from the unsharded one"
         assert sw.as_dict() == ss.as_dict(), (sw.as_dict(), ss.as_dict())
         assert torch.equal(xw[:nz[1]], xa) and torch.equal(xw[nz[1]:], xb)
+        # ... and the sharded evaluation against the oracle itself
+        ref = oracle.grad(po, lam.cpu().numpy(), gamma)
+        assert rel_l2(ga.cpu().numpy(), ref.grad) <= TOL_GRAD
+        assert abs(ss.g - ref.g) <= TOL_G * abs(ref.g) + 1e-12 and abs(ss.obj - ref.obj) <= TOL_G * abs(ref.obj) + 1e-9
+        assert abs(ss.reg - ref.reg) <= TOL_G * abs(ref.reg) + 1e-9 and abs(ss.r_inf - ref.r_inf) <= TOL_GRAD * np.linalg.norm(ref.grad) + 1e-12
+        assert np.abs(torch.cat([xa, xb]).cpu().numpy().astype(np.float64) - ref.x).max() <= TOL_X
     n0 = len(calls)
     gam, its = [10 * inst.cfg.gammas[-1], inst.cfg.gammas[-1]], [20, 20]
     ow = gpu_solve(whole, gam, its, want_x=False)
@@ -83,6 +95,13 @@ def test_two_shards_on_one_gpu_are_bit_identical_to_the_unsharded_problem(name, 
     assert len(calls) - n0 == sum(its) + 1                                           # one exchange per evaluation
     assert np.array_equal(ow["tr_lam"], oa["tr_lam"]) and np.array_equal(ow["tr_grad"], oa["tr_grad"]) and np.array_equal(ow["tr_g"], oa["tr_g"])
     assert np.array_equal(ow["lam"], oa["lam"]) and (ow["lam"] > 0).sum() > 5
+    # the sharded trajectory against the oracle's own solve, iteration by iteration
+    rs = oracle.solve(po, gam, its, trace_grad=True, trace_lambda=True, jacobi=jacobi)
+    for n in range(sum(its)):
+        assert rel_l2(oa["tr_grad"][n], rs.trace_grad[n]) <= TOL_GRAD, f"sharded iteration {n}"
+    assert np.abs(oa["tr_g"] - rs.trace_g).max() <= TOL_G * np.abs(rs.trace_g).max() + 1e-12
+    assert np.abs(oa["tr_lam"] - rs.trace_lambda).max() <= 1e-6 * max(np.abs(rs.trace_lambda).max(), 1e-300) + 1e-12
+    assert rel_l2(oa["grad"], rs.final.grad) <= TOL_GRAD and abs(oa["sc"].g - rs.final.g) <= TOL_G * abs(rs.final.g) + 1e-12
     A.set_reduce_hook(None)
     for P in (A, B):
         P.destroy()

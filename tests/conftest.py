@@ -49,6 +49,33 @@ def _no_bounds_violations():
         assert not _CHECK_FAILURES, _CHECK_FAILURES
 
 
+# How far the ORACLE's own adaptive-step trajectory (R20) moves when every gradient it sees carries ADAPTIVE_NOISE relative
+# noise -- upper bounds, measured and asserted by tests/test_oracle_extensions.py::test_adaptive_step_sensitivity_to_gradient_noise
+# on the instance of tests/test_gpu_extensions.py::test_adaptive_step_trajectory.  gpu_util.assert_adaptive_step_parity holds the
+# CUDA path's independent trajectory to these (its gradients are good to about 1e-7; what it shows is 10-20 x smaller).
+# lam_t: max over iterations of |lambda_t - lambda_t'|_inf / max|lambda|;  lam_T: the same at the end;  eta_t: max relative
+# difference of the steps;  g_T: relative difference of the final dual value.
+ADAPTIVE_NOISE = 1e-7
+ADAPTIVE_DRIFT = {"lam_t": 2.5e-6, "lam_T": 5e-8, "eta_t": 3e-5, "g_T": 2e-11}
+
+
+def ragged_problem(rng, I, J, m, lens):
+    """rows with prescribed lengths (0 allowed), items unsorted in every third row (tests only)."""
+    rows, idx = [0], []
+    for i in range(I):
+        d = int(lens[i % len(lens)])
+        it = rng.choice(J, size=min(d, J), replace=False)
+        it = it if i % 3 == 0 else np.sort(it)
+        idx.extend(it.tolist()); rows.append(len(idx))
+    nnz = len(idx)
+    c = (-rng.random(nnz) * rng.choice([1.0, 3.0])).astype(np.float32)
+    a = (0.5 + rng.random(nnz * m)).astype(np.float32)
+    col = np.zeros(J * m)
+    np.add.at(col, (np.repeat(np.array(idx, dtype=np.int64), m) * m + np.tile(np.arange(m), nnz)), a)
+    b = (0.1 * col + 0.01).astype(np.float32)
+    return dict(I=I, J=J, m=m, row_ptr=np.array(rows, dtype=np.int64), item_idx=np.array(idx, dtype=np.int32), c=c, a=a, b=b)
+
+
 def read_projection_cases():
     cases = []
     with open(os.path.join(GOLDEN, "projection_cases.txt")) as f:

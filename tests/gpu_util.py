@@ -6,6 +6,7 @@ import torch
 import oracle
 import paper_2606_07777_b200 as pkg
 import synth
+from conftest import ADAPTIVE_DRIFT
 
 TOL_X = 1e-5        # x: element-wise absolute
 TOL_GRAD = 1e-5     # grad g: relative L2, per evaluation / per iteration
@@ -130,10 +131,15 @@ def assert_adaptive_step_parity(po, pg, gammas, iters, eta_range, jacobi=False, 
       (A) same-lambda parity of every iteration: the oracle's grad g(y_t) against the traced gradient (1e-5);
       (B) the rule: eta_t recomputed in fp64 from the traced (y, grad) pairs by R20's definition (norms in the iterated system:
           y / d and d grad under Jacobi scaling, d from the oracle), and lambda_{t+1} = max(0, y_t + eta_t d^2 grad_t), to 1e-9;
-      (C) the two independent trajectories still end close: final dual value 1e-4 relative, lambda_T within 1 % of its scale."""
+      (C) the two INDEPENDENT trajectories (this one and the oracle's own solve) stay as close as the oracle's trajectory stays
+          to itself when its gradients carry 1e-7 relative noise -- conftest.ADAPTIVE_DRIFT, measured on the oracle alone by
+          tests/test_oracle_extensions.py::test_adaptive_step_sensitivity_to_gradient_noise: every lambda_t within 2.5e-6 of
+          the scale of lambda, lambda_T within 5e-8, every eta_t within 3e-5 relative; the final dual value within 1e-9
+          relative (its drift part is 2e-11; the rest is the accuracy of one evaluation of g).  The CUDA path shows 1.8e-7 /
+          1.5e-8 / 1.2e-6 / 1.3e-10 on the test instances ("Adaptive step and parity")."""
     emin, emax = eta_range
     out = gpu_solve(pg, gammas, iters)
-    ref = oracle.solve(po, gammas, iters, momentum=momentum, jacobi=jacobi, adaptive=True, eta_min=emin, eta_max=emax)
+    ref = oracle.solve(po, gammas, iters, momentum=momentum, jacobi=jacobi, adaptive=True, eta_min=emin, eta_max=emax, trace_lambda=True, trace_grad=True)
     R = pg.duals
     d = np.ones(R)
     if jacobi:
@@ -172,6 +178,12 @@ def assert_adaptive_step_parity(po, pg, gammas, iters, eta_range, jacobi=False, 
             y = lam_new + beta * (lam_new - lam_prev)
             lam_prev = lam_new
             n += 1
-    assert abs(out["sc"].g - ref.final.g) <= 1e-4 * abs(ref.final.g), f"{tag} final g {out['sc'].g} vs {ref.final.g}"
-    assert np.abs(out["lam"] - ref.lam).max() <= 1e-2 * max(np.abs(ref.lam).max(), 1e-300), f"{tag} lambda_T"
+    lam_scale = max(np.abs(ref.trace_lambda).max(), 1e-300)
+    seen = {"lam_t": np.abs(out["tr_lam"] - ref.trace_lambda).max() / lam_scale, "lam_T": np.abs(out["lam"] - ref.lam).max() / lam_scale,
+            "g_T": abs(out["sc"].g - ref.final.g) / abs(ref.final.g), "eta_t": np.abs(out["tr_eta"] / ref.trace_eta - 1.0).max(),
+            "grad_t": max(rel_l2(out["tr_grad"][k], ref.trace_grad[k]) for k in range(n))}
+    print(f"{tag} adaptive drift CUDA vs oracle: " + " ".join(f"{k}={v:.3e}" for k, v in seen.items()))
+    for k in ("lam_t", "lam_T", "eta_t"):
+        assert seen[k] <= ADAPTIVE_DRIFT[k], f"{tag} {k}: {seen[k]:.3e} exceeds the oracle's own drift under 1e-7 gradient noise ({ADAPTIVE_DRIFT[k]:g})"
+    assert seen["g_T"] <= 1e-9, f"{tag} final g {out['sc'].g} vs {ref.final.g}"
     return ref, out

@@ -7,7 +7,7 @@ import torch
 
 import oracle
 import synth
-from conftest import random_problem, read_worked_examples
+from conftest import ragged_problem, random_problem, read_worked_examples
 
 pytestmark = pytest.mark.gpu
 
@@ -26,21 +26,7 @@ def test_hand_worked_examples(ex):
         assert abs(getattr(sc, key) - ex[key]) < 1e-6, key
 
 
-def _ragged(rng, I, J, m, lens):
-    """rows with prescribed lengths (0 allowed), items unsorted in every third row."""
-    rows, idx = [0], []
-    for i in range(I):
-        d = int(lens[i % len(lens)])
-        it = rng.choice(J, size=min(d, J), replace=False)
-        it = it if i % 3 == 0 else np.sort(it)
-        idx.extend(it.tolist()); rows.append(len(idx))
-    nnz = len(idx)
-    c = (-rng.random(nnz) * rng.choice([1.0, 3.0])).astype(np.float32)
-    a = (0.5 + rng.random(nnz * m)).astype(np.float32)
-    col = np.zeros(J * m)
-    np.add.at(col, (np.repeat(np.array(idx, dtype=np.int64), m) * m + np.tile(np.arange(m), nnz)), a)
-    b = (0.1 * col + 0.01).astype(np.float32)
-    return dict(I=I, J=J, m=m, row_ptr=np.array(rows, dtype=np.int64), item_idx=np.array(idx, dtype=np.int32), c=c, a=a, b=b)
+_ragged = ragged_problem          # moved to conftest.py: the CPU-side sensitivity test builds the same instances
 
 
 CASES = [

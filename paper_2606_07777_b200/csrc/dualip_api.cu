@@ -1170,7 +1170,9 @@ int dualip_solve(dualip_t* h, const double* gammas, int32_t n_stages, const int3
         f.lam_eval = h->y; f.gamma = gamma; f.update = 1; f.eta = eta; f.momentum = h->opts.momentum ? 1 : 0;
         f.lam_cur = h->lam_cur; f.y = h->y; f.step_scale = h->step_scale;
         if (adaptive) {                                      // R20: clip range of this stage; the maximum scales with gamma
-            f.step_rule = 1; f.eta_lo = h->opts.eta_min; f.eta_hi = h->opts.eta_max * gamma / gammas[0];
+            // the lower end never lifts a step above the analytic one, gamma_s / L_step: without Jacobi scaling that is far
+            // below the paper's 1e-5, and a step forced up to eta_min would be far beyond the stability bound
+            f.step_rule = 1; f.eta_lo = std::min(h->opts.eta_min, eta); f.eta_hi = h->opts.eta_max * gamma / gammas[0];
             f.y_prev = h->y_prev; f.g_prev = h->g_prev;
         }
         if (trace) {

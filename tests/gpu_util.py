@@ -156,7 +156,7 @@ def assert_adaptive_step_parity(po, pg, gammas, iters, eta_range, jacobi=False, 
     worst_eta = 0.0
     for s, (gam, T) in enumerate(zip(gammas, iters)):
         hi = emax * gam / gammas[0]
-        clip = lambda e: min(max(e, emin), hi)
+        clip = lambda e, lo=min(emin, gam / L), hi=hi: min(max(e, lo), hi)
         y = lam_prev.copy()
         for t in range(T):
             g_gpu = out["tr_grad"][n]

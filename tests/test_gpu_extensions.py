@@ -28,7 +28,8 @@ if torch.cuda.is_available():
 @pytest.mark.parametrize("kernel", ["streaming", "direct"])
 def test_adaptive_step_trajectory(jacobi, kernel):
     """Three continuation stages; the clip range is chosen around gamma_1 / L so that the secant step is sometimes inside
-    the range, sometimes clipped below and (last stage: scaled maximum below eta_min) pinned to the maximum."""
+    the range and sometimes clipped; in the later stages gamma_s / L is below eta_min, so the stage opens with gamma_s / L
+    itself (lo_s = min(eta_min, gamma_s / L), R20) and the scaled maximum caps the secant steps."""
     rng = np.random.default_rng(17)
     d = _ragged(rng, 3000, 80, 2, [4, 9, 17, 30, 0, 12, 41])
     d["b"] = (d["b"] * 0.25).astype(np.float32)                  # binding: lambda moves
@@ -40,7 +41,9 @@ def test_adaptive_step_trajectory(jacobi, kernel):
     ref, out = assert_adaptive_step_parity(po, pg, gam, its, rng_eta, jacobi=jacobi, tag=f"adaptive/{kernel}/jacobi={jacobi}")
     eta = out["tr_eta"]
     assert (eta[1:25] > rng_eta[0] * 1.001).any() and (eta[1:25] < rng_eta[1] * 0.999).any()      # really adaptive somewhere
-    assert np.all(eta[-25:] == rng_eta[1] * gam[2] / gam[0])                                       # the scaled maximum wins
+    hi3 = rng_eta[1] * gam[2] / gam[0]
+    assert abs(eta[-25] / (gam[2] / L) - 1.0) <= 1e-12 and gam[2] / L < rng_eta[0]                   # opens with the analytic step, below eta_min
+    assert eta[-24:].max() <= hi3 * (1 + 1e-15) and (eta[-24:] == hi3).any()                       # the scaled maximum caps the secant
     assert (ref.lam > 0).sum() >= 5
     pg.destroy()
 

@@ -90,19 +90,40 @@ def test_adaptive_secant_is_gamma_over_L_where_the_gradient_is_linear():
 
 def test_adaptive_step_follows_the_reading_and_stays_in_its_range():
     """eta_t recomputed from the traces by the definition R20 states; the first step of every stage is the clipped fixed
-    step; every step lies in [eta_min, eta_max * gamma_s / gamma_1], and the scaled maximum wins when it is below eta_min."""
+    step; every step lies in [lo_s, hi_s] = [min(eta_min, gamma_s / L), eta_max * gamma_s / gamma_1], and the scaled maximum
+    wins when it is below lo_s (second parameter set: an eta_max below gamma_1 / L)."""
     rng = np.random.default_rng(11)
     d = random_problem(rng, I=80, J=7, m=2, deg=(2, 5), tight=0.4)
     p = _problem(d)
     gammas, iters = [0.4, 0.04, 0.004], [12, 12, 12]
     L = oracle.lipschitz(p)
-    emin, emax = 0.5 * gammas[0] / L, 3.0 * gammas[0] / L
+    for emin, emax, max_wins in ((0.5 * gammas[0] / L, 3.0 * gammas[0] / L, False), (0.05 * gammas[0] / L, 0.05 * gammas[0] / L, True)):
+        _check_adaptive_trace(p, gammas, iters, L, emin, emax, max_wins)
+
+
+def test_adaptive_default_range_on_an_unscaled_system_opens_with_the_analytic_step():
+    """The paper's range [1e-5, 1e-1] on a system that is NOT row-scaled, where gamma / L = 3.7e-7: the stage opens
+    with gamma / L itself (lo_s = min(eta_min, gamma_s / L)), not with a step lifted 27 x above it to eta_min, and the run
+    climbs: after 60 accelerated iterations the dual value is above where it started and above the fixed step's.  (With the
+    lift the same run fell from -1.4e4 to -1.1e5; R20.)"""
+    d = ragged_problem(np.random.default_rng(5), 6000, 12, 1, [3, 5, 8, 2, 6])
+    d["b"] = (d["b"] * 0.3).astype(np.float32)
+    p = _problem(d)
+    gamma, L = 1e-3, oracle.lipschitz(p)
+    assert gamma / L < 1e-5 / 20
+    ada = oracle.solve(p, [gamma], [60], adaptive=True)                       # default range
+    fix = oracle.solve(p, [gamma], [60])
+    assert ada.trace_eta[0] == gamma / L and ada.trace_eta.max() <= 1e-1 and ada.trace_eta.min() >= gamma / L * (1 - 1e-12)
+    assert ada.trace_g[-1] > ada.trace_g[0] and ada.final.g > fix.final.g > fix.trace_g[0]
+
+
+def _check_adaptive_trace(p, gammas, iters, L, emin, emax, max_wins):
     res = oracle.solve(p, gammas, iters, adaptive=True, eta_min=emin, eta_max=emax, trace_grad=True, trace_lambda=True)
     n = 0
     lam_prev = np.zeros(14)
     for s, (g, T) in enumerate(zip(gammas, iters)):
-        hi = emax * g / gammas[0]
-        clip = lambda e: min(max(e, emin), hi)
+        hi, lo = emax * g / gammas[0], min(emin, g / L)
+        clip = lambda e: min(max(e, lo), hi)
         y = lam_prev.copy()
         for t in range(T):
             if t == 0:
@@ -111,14 +132,16 @@ def test_adaptive_step_follows_the_reading_and_stays_in_its_range():
                 dy, dg = np.linalg.norm(y - y_old), np.linalg.norm(res.trace_grad[n] - res.trace_grad[n - 1])
                 want = clip(dy / dg) if dy > 0 and dg > 0 else clip(g / L)
             assert abs(res.trace_eta[n] - want) <= 1e-12 * want, (s, t)
-            assert res.trace_eta[n] <= hi * (1 + 1e-15) and (res.trace_eta[n] >= emin or res.trace_eta[n] == hi)
+            assert res.trace_eta[n] <= hi * (1 + 1e-15) and (res.trace_eta[n] >= lo or res.trace_eta[n] == hi)
             lam_new = res.trace_lambda[n]
             y_old = y
             y = lam_new + (t / (t + 3.0)) * (lam_new - lam_prev)
             lam_prev = lam_new
             n += 1
-    assert hi < emin                                              # the last stage really exercises "the maximum wins"
-    assert np.all(res.trace_eta[-12:] == hi)
+    if max_wins:                                                  # eta_max < gamma_1 / L: hi_s < lo_s in every stage, the maximum wins
+        assert hi < lo and np.all(res.trace_eta[-12:] == hi)
+    else:                                                         # later stages: gamma_s / L < eta_min, the stage opens with gamma_s / L itself
+        assert lo == g / L < emin and res.trace_eta[-12] == g / L
 
 
 def _adaptive_loop(p, gammas, iters, emin, emax, jacobi, L, noise, seed):
@@ -132,7 +155,7 @@ def _adaptive_loop(p, gammas, iters, emin, emax, jacobi, L, noise, seed):
     tr_lam, tr_eta, tr_grad = [], [], []
     for gam, T in zip(gammas, iters):
         hi = emax * gam / gammas[0]
-        clip = lambda e: min(max(e, emin), hi)
+        clip = lambda e, lo=min(emin, gam / L), hi=hi: min(max(e, lo), hi)
         y = lam.copy()
         for t in range(T):
             g = oracle.grad(p, y, gam, want_x=False).grad

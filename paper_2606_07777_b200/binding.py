@@ -57,10 +57,11 @@ class Scalars(ctypes.Structure):
         return {k: getattr(self, k) for k, _ in self._fields_}
 
     def table4(self):
-        """The columns of the paper's solution-quality report (Table 4), named as there: primal objective (of
-        the ridge problem: c'x + gamma/2 |x|^2), dual objective, absolute primal-dual gap, maximum positive constraint violation
-        ("slack").  Field selection only: every number was computed by the kernel's epilogue."""
-        return {"primal": self.obj + self.reg, "dual": self.g, "gap": abs(self.gap), "slack": self.r_inf}
+        """The fields behind the paper's solution-quality report (Table 4), selected and renamed, nothing
+        computed here: the two parts of the primal objective of the ridge problem (c'x and gamma/2 |x|^2, whose sum is Table 4's
+        "primal"), the dual objective, the SIGNED primal-dual gap (obj + reg) - g as the kernel's epilogue formed it (Table 4
+        prints its absolute value), and the maximum positive constraint violation ("slack")."""
+        return {"primal_obj": self.obj, "primal_reg": self.reg, "dual": self.g, "gap": self.gap, "slack": self.r_inf}
 
 
 class ShardExtents(ctypes.Structure):

@@ -49,11 +49,7 @@ def _compile_and_link(out: str, flags: list, log=None) -> None:
         subprocess.check_call([_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", out] + objs)
 
 
-def build(force: bool = False, verbose: bool = False, defines: dict | None = None, out: str | None = None) -> str:
-    """defines/out: build an experimental variant (e.g. {"DUALIP_NWC": 23}) next to the default library."""
-    if out is not None:
-        _compile_and_link(out, NVCC_FLAGS + [f"-D{k}={v}" for k, v in (defines or {}).items()])
-        return out
+def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not is_stale():
         return LIB
     flags = list(NVCC_FLAGS)

@@ -25,9 +25,7 @@ namespace {
 
 constexpr size_t kSmemBudget = 227 * 1024;  // bytes of dynamic shared memory one CTA may opt in to on sm_100a
 
-#ifndef DUALIP_LO_SMEM_KB
-#define DUALIP_LO_SMEM_KB 64
-#endif
+constexpr size_t kLoSmemBytes = 64 * 1024;  // lambda as an fp32 pair is always staged in shared memory while the pair stays under this
 
 struct Plan {
     int G = 32, KREG = 5, M = 1;
@@ -181,7 +179,7 @@ bool plan_tma(dualip* h, Plan& pl, long long max_len) {
     // small J*m: the low word is always staged (the plan is sized with it); larger: the kernel decides per launch whether
     // to trade a pipeline stage for it (k_grad_tma); tuning.lambda_plan overrides
     const int lp = h->opts.tuning.lambda_plan;
-    const bool lo = lp != 1 && 8 * JM <= (size_t)DUALIP_LO_SMEM_KB * 1024;
+    const bool lo = lp != 1 && 8 * JM <= kLoSmemBytes;
     const size_t lam_bytes = (lo ? 8 : 4) * JM;
     bool acc = (red == DUALIP_RED_AUTO && 16 * JM <= 64 * 1024) ||
                (red == DUALIP_RED_SMEM && fixed + lam_bytes + 8 * JM + 32 * 1024 <= kSmemBudget);

@@ -29,10 +29,7 @@
 
 namespace dualip_dev {
 
-#ifndef DUALIP_NWC
-#define DUALIP_NWC 15
-#endif
-constexpr int kTmaConsumerWarps = DUALIP_NWC;  // consumer warps of the streaming kernel (+ 1 producer warp)
+constexpr int kTmaConsumerWarps = 15;  // consumer warps of the streaming kernel (+ 1 producer warp)
 
 constexpr int kRowCost = 8;            // each row costs this many "nonzero units" when cutting tiles
 constexpr int kTmaStagesMax = 8;
@@ -95,19 +92,7 @@ __device__ __forceinline__ void mbar_expect_tx(void* bar, unsigned bytes) {
 __device__ __forceinline__ void mbar_arrive(void* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-#ifndef DUALIP_WAIT_HINT_NS
-#define DUALIP_WAIT_HINT_NS 0
-#endif
 __device__ __forceinline__ void mbar_wait(void* bar, unsigned parity) {
-#if DUALIP_WAIT_HINT_NS > 0
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "WAIT_LOOP:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
-        "@p bra DONE;\n\t"
-        "bra WAIT_LOOP;\n\t"
-        "DONE:\n\t}" ::"r"(smem_u32(bar)), "r"(parity), "r"((unsigned)DUALIP_WAIT_HINT_NS) : "memory");
-#else
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
         "WAIT_LOOP:\n\t"
@@ -115,7 +100,6 @@ __device__ __forceinline__ void mbar_wait(void* bar, unsigned parity) {
         "@p bra DONE;\n\t"
         "bra WAIT_LOOP;\n\t"
         "DONE:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-#endif
 }
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, void* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -208,11 +192,7 @@ __device__ __forceinline__ long long to_fix32(float v, float scale) { return __f
 // RED.ADD.64 on a pointer known to be global memory (a generic atomicAdd makes ptxas emit an address-space check, a
 // shared-memory CAS loop and a predicate that the caller then waits on).
 __device__ __forceinline__ void red_add_u64(unsigned long long* gptr, unsigned long long v) {
-#ifdef DUALIP_EXP_NULL_RED      // experiment build (profiles/: what the item reduction costs): results are wrong by construction
-    (void)gptr; (void)v;
-#else
     asm volatile("red.global.add.u64 [%0], %1;" ::"l"(gptr), "l"(v));
-#endif
 }
 
 // (a > b) ? x : y as one SETP + SEL, whatever the surrounding control flow looks like

@@ -239,4 +239,4 @@ def test_per_launch_lambda_plan_decides_from_lambda_and_gamma_and_changes_no_bit
 
 def test_table4_columns():
     sc = pkg.Scalars(g=-10.0, obj=-9.0, reg=0.5, r_inf=1e-3, r_2=2e-3, gap=1.5)
-    assert sc.table4() == {"primal": -8.5, "dual": -10.0, "gap": 1.5, "slack": 1e-3}
+    assert sc.table4() == {"primal_obj": -9.0, "primal_reg": 0.5, "dual": -10.0, "gap": 1.5, "slack": 1e-3}       # selection only, no arithmetic
